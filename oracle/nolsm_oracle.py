@@ -1,0 +1,297 @@
+"""FP64 CPU oracle for the NOLSM hot path (arXiv 2104.08245).  TEST INFRASTRUCTURE ONLY.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference leg may import
+this module.  It shares no code with the CUDA path (paper_2104_08245_b200/) and never imports it;
+the only thing both sides see are the seeded inputs from nolsm_inputs/.
+
+What it computes (PAPER.md = /root/reference/PAPER.md):
+  * submatrix construction T_j, application of the matrix function, write-back of the own columns
+    (PAPER.md:140-146 steps i-iii; NOLSM with one merged index set for H and S);
+  * T_j(D) = 1/2 (I - sign(T_j(S)^-1 T_j(H) - mu I)) T_j(S)^-1   (Eq. 12), evaluated
+    by its plain definition: the Newton-Schulz iterations of Eq. 9-10 / Eq. 15-17 converge to exactly
+    sign(A) and S^-1, so the oracle solves H v = lambda S v (LAPACK) and forms sign and D from the
+    eigenvectors;
+  * the chemical potential mu such that 2 tr(DS) = N_electrons by bisection.
+The literal iterations (Eq. 9-10, Eq. 15-17) are also written out step by step
+(`newton_schulz_sign`, `newton_schulz_inverse`) for fixed-iteration comparisons and residual traces.
+
+Readings of the paper taken here are listed in DESIGN.md ("Readings").
+Pins: tests/test_oracle_*.py (-m "not gpu").  Unpinned: the paper's fixed iteration count
+(PAPER.md:217 never states it) -- "parity unpinned" for that number only; the oracle does not use it.
+"""
+import numpy as np
+import scipy.linalg as sla
+
+BS = 6  # basis functions per molecule (uniform block size)
+
+
+# --------------------------------------------------------------------------------------------
+# a0: neighbour lists / index sets  (Fig. 2 b,c PAPER.md:172,190; merged pattern PAPER.md:158)
+# --------------------------------------------------------------------------------------------
+def min_image(d, box):
+    """Per-axis minimum image on integers: d>L/2 -> d-L ; d<-L/2 -> d+L (box even)."""
+    d = np.asarray(d, dtype=np.int64)
+    box = np.asarray(box, dtype=np.int64)
+    half = box // 2
+    d = np.where(d > half, d - box, d)
+    d = np.where(d < -half, d + box, d)
+    return d
+
+
+def neighbours_of(pos_q, box_q, rc_q, j):
+    """Ascending ids i with |c_i - c_j|_min-image <= r_c (closed ball, self included).
+    Exact: int64 squared distances on the 2^-16 A grid."""
+    p = np.asarray(pos_q, dtype=np.int64)
+    d = min_image(p - p[j], box_q)
+    d2 = (d * d).sum(axis=1)
+    return np.nonzero(d2 <= np.int64(rc_q) * np.int64(rc_q))[0].astype(np.int32)
+
+
+def neighbour_list(pos_q, box_q, rc_q):
+    """CSR (row_ptr int32 [N+1], col_idx int32) of all neighbour lists, brute force O(N^2)."""
+    n = np.asarray(pos_q).shape[0]
+    lists = [neighbours_of(pos_q, box_q, rc_q, j) for j in range(n)]
+    row_ptr = np.zeros(n + 1, dtype=np.int32)
+    row_ptr[1:] = np.cumsum([len(l) for l in lists])
+    col_idx = np.concatenate(lists).astype(np.int32) if n else np.zeros(0, np.int32)
+    return row_ptr, col_idx
+
+
+def index_set(nbrs):
+    """Row/column indices of the submatrix of molecule j: {6 i + o : i in N_j, o = 0..5}, in the
+    order of N_j (ascending) times orbital."""
+    nbrs = np.asarray(nbrs, dtype=np.int64)
+    return (nbrs[:, None] * BS + np.arange(BS)[None, :]).reshape(-1)
+
+
+# --------------------------------------------------------------------------------------------
+# a1: submatrix construction T_j(.)  (step (i); NOLSM PAPER.md:158)
+# --------------------------------------------------------------------------------------------
+def dense_submatrix(row_ptr, col_idx, val, nbrs):
+    """T_j(M) = M[idx, idx] for the block-sparse matrix M (block k of row i = block (i, col_idx[k])),
+    zero where a pair of neighbours of j is not itself stored.  FP64 copy of the FP32 values."""
+    nbrs = np.asarray(nbrs, dtype=np.int64)
+    m = nbrs.shape[0]
+    out = np.zeros((m * BS, m * BS), dtype=np.float64)
+    for a in range(m):
+        i = nbrs[a]
+        lo, hi = int(row_ptr[i]), int(row_ptr[i + 1])
+        cols = col_idx[lo:hi]
+        pos = np.searchsorted(cols, nbrs)
+        ok = (pos < cols.shape[0])
+        ok[ok] = cols[pos[ok]] == nbrs[ok]
+        for b in np.nonzero(ok)[0]:
+            out[a * BS:(a + 1) * BS, b * BS:(b + 1) * BS] = val[lo + pos[b]]
+    return out
+
+
+# --------------------------------------------------------------------------------------------
+# a2-a5: the matrix function by its definition  (Eq. 6 / Eq. 12)
+# --------------------------------------------------------------------------------------------
+def generalized_eig(h_sub, s_sub):
+    """H v = lambda S v, V^T S V = I (LAPACK dsygvd). Raises LinAlgError if S is not SPD."""
+    lam, v = sla.eigh(h_sub, s_sub, driver="gvd")
+    return lam, v
+
+
+def sign_from_eig(lam, v, s_sub, mu):
+    """sign(S^-1 H - mu I) = V diag(sign(lambda - mu)) V^T S  (S^-1 H = V Lambda V^-1, V^-1 = V^T S)."""
+    return (v * np.sign(lam - mu)[None, :]) @ (v.T @ s_sub)
+
+
+def density_from_eig(lam, v, mu):
+    """T_j(D) = 1/2 (I - sign(S^-1H - mu I)) S^-1 = V_occ V_occ^T, occ = {k: lambda_k < mu}."""
+    occ = lam < mu
+    vo = v[:, occ]
+    return vo @ vo.T
+
+
+def own_position(nbrs, j):
+    """Position a of molecule j inside its own neighbour list; own columns are 6a..6a+5."""
+    a = int(np.searchsorted(nbrs, j))
+    assert nbrs[a] == j
+    return a
+
+
+def mulliken_weights(v, s_sub, own):
+    """w_k = sum_{c in own} V[c,k] (S V)[c,k]; population q(mu) = 2 sum_{k occ} w_k."""
+    sv = s_sub @ v
+    return (v[own, :] * sv[own, :]).sum(axis=0)
+
+
+# --------------------------------------------------------------------------------------------
+# The iterations the paper uses, step by step (fixed-iteration comparisons, residual traces)
+# --------------------------------------------------------------------------------------------
+def newton_schulz_sign(a, n_iter, scale=None, history=False):
+    """Eq. 9-10: X0 = A/scale, X_{k+1} = 1/2 X_k (3I - X_k^2).
+    Returns X_{n_iter} (and r_k = ||X_k^2 - I||_F / sqrt(n) for k = 0..n_iter-1 if history)."""
+    a = np.asarray(a, dtype=np.float64)
+    n = a.shape[0]
+    eye = np.eye(n)
+    x = a / (1.0 if scale is None else scale)
+    res = []
+    for _ in range(n_iter):
+        x2 = x @ x
+        res.append(np.linalg.norm(x2 - eye, "fro") / np.sqrt(n))
+        x = 0.5 * x @ (3.0 * eye - x2)
+    return (x, np.array(res)) if history else x
+
+
+def newton_schulz_inverse(s, n_iter, scale=None, history=False):
+    """Eq. 15-17: Y0 = S/scale, Z0 = I, V_k = Z_k Y_k,
+    Y_{k+1} = 1/2 Y_k (3I - V_k), Z_{k+1} = 1/2 (3I - V_k) Z_k; Z -> Y0^{-1/2}; S^-1 = Z^2/scale.
+    Returns (S^-1, Z, Y) after n_iter steps (and ||V_k - I||_F/sqrt(n) if history)."""
+    s = np.asarray(s, dtype=np.float64)
+    n = s.shape[0]
+    eye = np.eye(n)
+    c = 1.0 if scale is None else scale
+    y = s / c
+    z = eye.copy()
+    res = []
+    for _ in range(n_iter):
+        v = z @ y
+        res.append(np.linalg.norm(v - eye, "fro") / np.sqrt(n))
+        t = 3.0 * eye - v
+        y = 0.5 * y @ t
+        z = 0.5 * t @ z
+    sinv = (z @ z) / c
+    return (sinv, z, y, np.array(res)) if history else (sinv, z, y)
+
+
+# --------------------------------------------------------------------------------------------
+# Whole path for one molecule and for a system
+# --------------------------------------------------------------------------------------------
+class SubmatrixSolution:
+    """Eigen-decomposition of one submatrix; everything mu-dependent is derived from it."""
+
+    def __init__(self, j, nbrs, h_sub, s_sub):
+        self.j = int(j)
+        self.nbrs = np.asarray(nbrs, dtype=np.int32)
+        self.h_sub, self.s_sub = h_sub, s_sub
+        self.lam, self.v = generalized_eig(h_sub, s_sub)
+        a = own_position(self.nbrs, j)
+        self.own = np.arange(a * BS, (a + 1) * BS)
+        self.w = mulliken_weights(self.v, s_sub, self.own)
+
+    @property
+    def n(self):
+        return self.h_sub.shape[0]
+
+    def sign(self, mu):
+        return sign_from_eig(self.lam, self.v, self.s_sub, mu)
+
+    def density(self, mu):
+        return density_from_eig(self.lam, self.v, mu)
+
+    def density_columns(self, mu):
+        """Own columns of T_j(D): [n_j, 6]; rows 6a..6a+5 are block D(N_j[a], j)  (step iii)."""
+        occ = self.lam < mu
+        return self.v[:, occ] @ self.v[self.own][:, occ].T
+
+    def population(self, mu):
+        """q_j(mu) = 2 sum_{c in own} (D S)[c,c] restricted to the submatrix = 2 sum_{k occ} w_k."""
+        return 2.0 * float(self.w[self.lam < mu].sum())
+
+    def homo_lumo(self, n_occ):
+        return float(self.lam[n_occ - 1]), float(self.lam[n_occ])
+
+
+def solve_molecule(row_ptr, col_idx, h_val, s_val, j, nbrs=None):
+    if nbrs is None:
+        nbrs = col_idx[row_ptr[j]:row_ptr[j + 1]]
+    h_sub = dense_submatrix(row_ptr, col_idx, h_val, nbrs)
+    s_sub = dense_submatrix(row_ptr, col_idx, s_val, nbrs)
+    return SubmatrixSolution(j, nbrs, h_sub, s_sub)
+
+
+def electron_count(solutions, mu):
+    """N(mu) = 2 tr(DS) over stored blocks = sum_j q_j(mu)."""
+    return float(sum(s.population(mu) for s in solutions))
+
+
+def electron_count_blocks(row_ptr, col_idx, d_val, s_val):
+    """N = 2 sum over stored blocks <D(i,j), S(i,j)>_F with D column-owned: block k of row j of
+    d_val holds D(col_idx[k], j); S(i,j) is looked up in row i of the S store."""
+    total = 0.0
+    n = row_ptr.shape[0] - 1
+    for j in range(n):
+        for k in range(row_ptr[j], row_ptr[j + 1]):
+            i = col_idx[k]
+            lo, hi = row_ptr[i], row_ptr[i + 1]
+            p = lo + int(np.searchsorted(col_idx[lo:hi], j))
+            if p < hi and col_idx[p] == j:
+                total += float((d_val[k].astype(np.float64) * s_val[p].astype(np.float64)).sum())
+    return 2.0 * total
+
+
+def bisect_mu(solutions, n_electrons, mu_lo, mu_hi, tol_per_mol=1e-3, max_steps=60):
+    """Midpoint bisection on N(mu) - N_e: N(mu) > N_e -> mu_hi = mu, else mu_lo = mu;
+    stop when |N(mu) - N_e| <= tol_per_mol * n_molecules.  Returns (mu, N(mu), steps, trace)."""
+    n_mol = len(solutions)
+    trace = []
+    mu = 0.5 * (mu_lo + mu_hi)
+    ne = electron_count(solutions, mu)
+    for step in range(1, max_steps + 1):
+        mu = 0.5 * (mu_lo + mu_hi)
+        ne = electron_count(solutions, mu)
+        trace.append((mu, ne))
+        if abs(ne - n_electrons) <= tol_per_mol * n_mol:
+            return mu, ne, step, trace
+        if ne > n_electrons:
+            mu_hi = mu
+        else:
+            mu_lo = mu
+    return mu, ne, max_steps, trace
+
+
+def density_blocks(solutions, row_ptr, mu, dtype=np.float64):
+    """Column-owned D store: block k of row j = D(col_idx[k], j) = rows of molecule col_idx[k] in the
+    own columns of submatrix j.  Requires solutions[j].nbrs == col_idx[row_ptr[j]:row_ptr[j+1]]."""
+    nnzb = int(row_ptr[-1])
+    out = np.zeros((nnzb, BS, BS), dtype=dtype)
+    for s in solutions:
+        cols = s.density_columns(mu)
+        lo = int(row_ptr[s.j])
+        out[lo:lo + s.nbrs.shape[0]] = cols.reshape(-1, BS, BS)
+    return out
+
+
+def mu_plateau(solutions, n_occ_per_sub_fn):
+    """[max_j HOMO_j, min_j LUMO_j] given the number of occupied states of each submatrix."""
+    homo = max(s.homo_lumo(n_occ_per_sub_fn(s))[0] for s in solutions)
+    lumo = min(s.homo_lumo(n_occ_per_sub_fn(s))[1] for s in solutions)
+    return homo, lumo
+
+
+def solve_system(system, mu=None, mu_lo=-3.0, mu_hi=0.0, tol_per_mol=1e-3, molecules=None):
+    """Whole path on a nolsm_inputs.WaterSystem.  If `molecules` is given only those are solved
+    (sampled oracle for large configs; bisection then needs `mu`)."""
+    rp, ci = system.row_ptr, system.col_idx
+    mols = range(system.n_mol) if molecules is None else molecules
+    sols = [solve_molecule(rp, ci, system.h_val, system.s_val, int(j)) for j in mols]
+    out = {"solutions": sols}
+    if mu is None:
+        assert molecules is None, "bisection needs every molecule"
+        mu, ne, steps, trace = bisect_mu(sols, system.n_electrons, mu_lo, mu_hi, tol_per_mol)
+        out.update(steps=steps, trace=trace)
+    else:
+        ne = electron_count(sols, mu)
+    out.update(mu=mu, n_electrons=ne)
+    if molecules is None:
+        out["d_val"] = density_blocks(sols, rp, mu)
+    return out
+
+
+# --------------------------------------------------------------------------------------------
+# Dense microbench (BASELINE.json:configs[4]): sign known by construction
+# --------------------------------------------------------------------------------------------
+def sign_by_construction(q, lam):
+    """sign(Q diag(lam) Q^T) = Q diag(sign(lam)) Q^T."""
+    return (q * np.sign(lam)[None, :]) @ q.T
+
+
+def sign_residual(x):
+    """||X^2 - I||_F / sqrt(n) in FP64 on a returned iterate (acceptance test, reading 10)."""
+    x = np.asarray(x, dtype=np.float64)
+    n = x.shape[0]
+    return float(np.linalg.norm(x @ x - np.eye(n), "fro") / np.sqrt(n))

@@ -1,0 +1,302 @@
+"""Pins for the FP64 oracle against things other than itself: closed forms, textbook/library
+routines, invariants, brute force on tiny inputs, and the full-matrix limit of the submatrix method
+(the submatrix of a column whose pattern is full IS the matrix)."""
+import os
+from fractions import Fraction
+
+import numpy as np
+import pytest
+import scipy.linalg as sla
+import scipy.sparse as sp
+
+import nolsm_inputs as gi
+from nolsm_inputs.water import to_dense
+import oracle.nolsm_oracle as orc
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+# ------------------------------------------------------------------ a0 neighbour lists
+def _bruteforce_python(pos, box, rc):
+    n = len(pos)
+    out = []
+    for j in range(n):
+        row = []
+        for i in range(n):
+            d2 = 0
+            for ax in range(3):
+                d = int(pos[i][ax]) - int(pos[j][ax])
+                L = int(box[ax])
+                if d > L // 2:
+                    d -= L
+                elif d < -(L // 2):
+                    d += L
+                d2 += d * d
+            if d2 <= rc * rc:
+                row.append(i)
+        out.append(row)
+    return out
+
+
+def test_neighbours_match_pure_python_bruteforce(tiny_system):
+    s = tiny_system
+    ref = _bruteforce_python(s.pos_q.tolist(), s.box_q.tolist(), s.rc_q)
+    rp, ci = orc.neighbour_list(s.pos_q, s.box_q, s.rc_q)
+    for j in range(s.n_mol):
+        assert ci[rp[j]:rp[j + 1]].tolist() == ref[j]
+    # and the generator's stored pattern is that same list (H and S share it; PAPER.md:158 merge = identity)
+    assert np.array_equal(rp, s.row_ptr) and np.array_equal(ci, s.col_idx)
+
+
+def test_neighbours_symmetric_self_included_and_full_at_large_cutoff(tiny_system):
+    s = tiny_system
+    rp, ci = orc.neighbour_list(s.pos_q, s.box_q, s.rc_q)
+    pairs = {(j, int(i)) for j in range(s.n_mol) for i in ci[rp[j]:rp[j + 1]]}
+    assert all((i, j) in pairs for (j, i) in pairs)
+    assert all((j, j) in pairs for j in range(s.n_mol))
+    # r_c >= L*sqrt(3)/2 (half the box diagonal) -> every molecule is everyone's neighbour
+    rc_full = int(np.ceil(np.sqrt(3.0) / 2.0 * s.box_q[0])) + 1
+    rp2, ci2 = orc.neighbour_list(s.pos_q, s.box_q, rc_full)
+    assert np.array_equal(np.diff(rp2), np.full(s.n_mol, s.n_mol))
+    assert np.array_equal(ci2.reshape(s.n_mol, s.n_mol), np.tile(np.arange(s.n_mol), (s.n_mol, 1)))
+
+
+def test_neighbour_counts_match_continuum_estimate():
+    # 4/3 pi r^3 rho molecules in a ball: 8 A -> 71.6 ; lattice + jitter gives ~80 (SURVEY table)
+    s = gi.make_water_system(512, 8.0)
+    m = np.diff(s.row_ptr)
+    assert 70 <= m.mean() <= 90 and m.min() >= 60 and m.max() <= 100
+
+
+def test_index_set_order():
+    idx = orc.index_set(np.array([2, 5, 7]))
+    assert idx.tolist() == [12, 13, 14, 15, 16, 17, 30, 31, 32, 33, 34, 35, 42, 43, 44, 45, 46, 47]
+
+
+# ------------------------------------------------------------------ a1 submatrix construction
+def test_dense_submatrix_equals_sparse_slicing(tiny_system):
+    s = tiny_system
+    n = s.n_mol * 6
+    for val in (s.h_val, s.s_val):
+        m = sp.bsr_matrix((val.astype(np.float64), s.col_idx, s.row_ptr), shape=(n, n)).tocsr()
+        for j in (0, 7, 31):
+            nb = s.col_idx[s.row_ptr[j]:s.row_ptr[j + 1]]
+            idx = orc.index_set(nb)
+            ref = m[idx][:, idx].toarray()
+            got = orc.dense_submatrix(s.row_ptr, s.col_idx, val, nb)
+            assert np.array_equal(ref, got)
+            # not every neighbour pair of j is itself a stored pair -> genuine zeros appear
+    nb = s.col_idx[s.row_ptr[0]:s.row_ptr[1]]
+    sub = orc.dense_submatrix(s.row_ptr, s.col_idx, s.s_val, nb)
+    assert (sub == 0).mean() > 0.05
+
+
+# ------------------------------------------------------------------ Eq. 9-10 Newton-Schulz
+def test_newton_schulz_scalar_closed_form():
+    rows = [l.split() for l in open(os.path.join(GOLD, "ns_scalar_sequence.txt")) if not l.startswith("#")]
+    exact = {int(k): Fraction(int(a), int(b)) for k, a, b in rows}
+    # independent re-derivation of the golden rationals
+    x = Fraction(1, 2)
+    for k in range(4):
+        assert x == exact[k]
+        x = Fraction(1, 2) * x * (3 - x * x)
+    # the oracle's matrix iteration on diag(0.5, -0.5) must reproduce them (sign is odd)
+    for k in range(4):
+        xk = orc.newton_schulz_sign(np.diag([0.5, -0.5]), k)
+        assert abs(xk[0, 0] - float(exact[k])) < 1e-15 and abs(xk[1, 1] + float(exact[k])) < 1e-15
+        assert xk[0, 1] == 0 and xk[1, 0] == 0
+    # decimals quoted in SURVEY.md 8(c): 0.6875, 0.868774414062, 0.975299630819
+    assert abs(float(exact[2]) - 0.868774414062) < 1e-12 and abs(float(exact[3]) - 0.975299630819) < 1e-12
+    # from x0 = 0.05 ten iterations are needed to reach |x^2-1| < 1e-2
+    x, k = 0.05, 0
+    while abs(x * x - 1) >= 1e-2:
+        x, k = 0.5 * x * (3 - x * x), k + 1
+    assert k == 10
+    _, res = orc.newton_schulz_sign(np.array([[0.05]]), 12, history=True)
+    assert (res[:10] >= 1e-2).all() and res[10] < 1e-2
+
+
+def test_newton_schulz_sign_converges_to_construction_and_quadratically():
+    a, q, lam = gi.make_gapped_symmetric(48, seed=3)
+    a = (q * lam) @ q.T
+    exact = orc.sign_by_construction(q, lam)
+    x, res = orc.newton_schulz_sign(a, 14, scale=np.abs(lam).max(), history=True)
+    assert np.abs(x - exact).max() < 1e-12
+    tail = res[(res < 1e-1) & (res > 1e-7)]
+    # per eigenvalue e = x^2-1 maps to e' = 3/4 e^2 + O(e^3); with r = rms(e): 3/4 r^2 <= r' <= 3/4 sqrt(n) r^2
+    for r0, r1 in zip(res[:-1], res[1:]):
+        if 1e-6 < r0 < 3e-2:
+            assert 0.74 * r0 * r0 < r1 < 0.77 * np.sqrt(48) * r0 * r0
+    assert len(tail) >= 1
+    # every iterate commutes with A
+    x5 = orc.newton_schulz_sign(a, 5, scale=np.abs(lam).max())
+    assert np.abs(x5 @ a - a @ x5).max() < 1e-13
+
+
+def test_sign_by_construction_matches_library_signm():
+    a, q, lam = gi.make_gapped_symmetric(24, seed=5)
+    a64 = (q * lam) @ q.T
+    ref = sla.signm(a64)
+    assert np.abs(orc.sign_by_construction(q, lam) - ref).max() < 1e-10
+
+
+# ------------------------------------------------------------------ Eq. 15-17 inverse
+def test_newton_schulz_inverse_limits(tiny_system):
+    s = tiny_system
+    nb = s.col_idx[s.row_ptr[3]:s.row_ptr[4]]
+    ssub = orc.dense_submatrix(s.row_ptr, s.col_idx, s.s_val, nb)
+    c = np.abs(ssub).sum(axis=1).max()           # >= lambda_max
+    sinv, z, y, res = orc.newton_schulz_inverse(ssub, 30, scale=c, history=True)
+    assert np.abs(sinv - np.linalg.inv(ssub)).max() < 1e-12
+    assert np.abs(y - sla.sqrtm(ssub / c)).max() < 1e-12          # Y -> Y0^{1/2}
+    assert np.abs(z @ z @ (ssub / c) - np.eye(len(ssub))).max() < 1e-12   # Z -> Y0^{-1/2}
+    assert np.abs(y @ z - np.eye(len(ssub))).max() < 1e-12
+    # invariant Y_k = Y0 Z_k at every k
+    for k in (1, 3):
+        _, zk, yk = orc.newton_schulz_inverse(ssub, k, scale=c)
+        assert np.abs(yk - (ssub / c) @ zk).max() < 1e-14
+    assert res[0] > res[5] > res[-1]
+    # 1x1: S = 4 -> inverse 1/4 whatever the (valid) scale
+    sinv1, _, _ = orc.newton_schulz_inverse(np.array([[4.0]]), 40, scale=5.0)
+    assert abs(sinv1[0, 0] - 0.25) < 1e-14
+
+
+# ------------------------------------------------------------------ Eq. 6 / 12 by eigenvectors
+def test_sign_and_density_identities(tiny_solution):
+    sol = tiny_solution["solutions"][5]
+    mu = -0.85
+    n = sol.n
+    sg = sol.sign(mu)
+    a = np.linalg.solve(sol.s_sub, sol.h_sub) - mu * np.eye(n)
+    assert np.abs(sg @ sg - np.eye(n)).max() < 1e-11                       # sign^2 = I
+    assert np.abs(sg @ a - a @ sg).max() < 1e-11                           # commutes with A
+    d = sol.density(mu)
+    assert np.abs(sg - (np.eye(n) - 2 * d @ sol.s_sub)).max() < 1e-11      # sign = I - 2 D S
+    assert np.abs(d - 0.5 * (np.eye(n) - sg) @ np.linalg.inv(sol.s_sub)).max() < 1e-11   # Eq. 12 literally
+    assert np.abs(d @ sol.s_sub @ d - d).max() < 1e-12                     # D S D = D
+    assert np.abs(d - d.T).max() < 1e-14
+    nocc = int((sol.lam < mu).sum())
+    assert abs(np.trace(d @ sol.s_sub) - nocc) < 1e-10                     # tr(DS) = # occupied, an integer
+    ev = np.sort(np.linalg.eigvals(sg).real)
+    assert np.abs(ev[:nocc] + 1).max() < 1e-9 and np.abs(ev[nocc:] - 1).max() < 1e-9
+    # the literal Newton-Schulz iteration (Eq. 9-10) reaches the same sign
+    x = orc.newton_schulz_sign(a, 40, scale=1.05 * np.abs(np.linalg.eigvals(a)).max())
+    assert np.abs(x - sg).max() < 1e-9
+    # own columns / populations are consistent with the full D
+    assert np.abs(sol.density_columns(mu) - d[:, sol.own]).max() < 1e-14
+    q = 2 * (d @ sol.s_sub)[sol.own, sol.own].sum()
+    assert abs(q - sol.population(mu)) < 1e-11
+    assert abs(q - 8.0) < 0.05
+
+
+def test_orthogonal_case_reduces_to_textbook_eigh():
+    rng = np.random.default_rng(0)
+    h = rng.standard_normal((20, 20))
+    h = h + h.T
+    lam, v = orc.generalized_eig(h, np.eye(20))
+    w, u = np.linalg.eigh(h)
+    assert np.abs(lam - w).max() < 1e-12
+    mu = 0.1
+    p_ref = u[:, w < mu] @ u[:, w < mu].T
+    assert np.abs(orc.density_from_eig(lam, v, mu) - p_ref).max() < 1e-12
+    assert np.abs(orc.sign_from_eig(lam, v, np.eye(20), mu) - sla.signm(h - mu * np.eye(20))).max() < 1e-9
+
+
+# ------------------------------------------------------------------ whole method, limit case
+def test_full_cutoff_limit_equals_full_matrix_diagonalisation():
+    """With r_c >= half the box diagonal every submatrix is the whole matrix, so the submatrix
+    method must reproduce the full-matrix projector (north_star pin)."""
+    s = gi.make_water_system(32, 9.0)
+    assert (np.diff(s.row_ptr) == 32).all()
+    H, S = to_dense(s, "H"), to_dense(s, "S")
+    lam, v = sla.eigh(H, S)
+    nocc = 4 * s.n_mol
+    mu = 0.5 * (lam[nocc - 1] + lam[nocc])
+    d_full = v[:, :nocc] @ v[:, :nocc].T
+    out = orc.solve_system(s, mu=mu)
+    assert abs(out["n_electrons"] - 8 * s.n_mol) < 1e-9                    # tr(DS) = 4N exactly
+    d_val = out["d_val"]
+    for j in range(s.n_mol):
+        for k in range(s.row_ptr[j], s.row_ptr[j + 1]):
+            i = s.col_idx[k]
+            assert np.abs(d_val[k] - d_full[6 * i:6 * i + 6, 6 * j:6 * j + 6]).max() < 1e-11
+    assert np.abs(d_full @ S @ d_full - d_full).max() < 1e-12
+    # block contraction equals the trace
+    assert abs(orc.electron_count_blocks(s.row_ptr, s.col_idx, d_val, s.s_val) - 8 * s.n_mol) < 1e-9
+
+
+def test_submatrix_result_close_to_full_matrix_at_finite_cutoff(tiny_system, tiny_solution):
+    """At 6 A the submatrix D differs from the full-matrix D by a few 1e-3 (nearsightedness)."""
+    s = tiny_system
+    H, S = to_dense(s, "H"), to_dense(s, "S")
+    lam, v = sla.eigh(H, S)
+    nocc = 4 * s.n_mol
+    d_full = v[:, :nocc] @ v[:, :nocc].T
+    d_val = tiny_solution["d_val"]
+    err = 0.0
+    for j in range(s.n_mol):
+        for k in range(s.row_ptr[j], s.row_ptr[j + 1]):
+            i = s.col_idx[k]
+            err = max(err, np.abs(d_val[k] - d_full[6 * i:6 * i + 6, 6 * j:6 * j + 6]).max())
+    assert 1e-5 < err < 2e-2
+
+
+# ------------------------------------------------------------------ a7 electron count and mu
+def test_electron_count_staircase_and_bisection(tiny_system, tiny_solution):
+    s, sols = tiny_system, tiny_solution["solutions"]
+    assert orc.electron_count(sols, -1e9) == 0.0
+    assert abs(orc.electron_count(sols, 1e9) - 12 * s.n_mol) < 1e-9       # all 6 orbitals x 2
+    homo, lumo = orc.mu_plateau(sols, lambda x: 4 * len(x.nbrs))
+    assert homo < lumo
+    mus = np.linspace(homo + 1e-6, lumo - 1e-6, 7)
+    ne = [orc.electron_count(sols, m) for m in mus]
+    assert max(ne) - min(ne) < 1e-12                                       # constant on the gap plateau
+    assert abs(ne[0] - 8 * s.n_mol) < 2e-3 * s.n_mol                      # plateau is N_e only approximately
+    grid = np.linspace(-2.5, -0.3, 400)
+    vals = np.array([orc.electron_count(sols, m) for m in grid])
+    assert (np.diff(vals) > -1e-3).all()                                   # monotone up to Mulliken wiggles
+    mu, n_e, steps, trace = bisect_mu = orc.bisect_mu(sols, s.n_electrons, -3.0, 0.0)
+    assert [t[0] for t in trace] == [-1.5, -0.75] and steps == 2
+    assert homo < mu < lumo and abs(n_e - s.n_electrons) <= 1e-3 * s.n_mol
+    # block contraction on the stored D equals the sum of populations
+    nb = orc.electron_count_blocks(s.row_ptr, s.col_idx, tiny_solution["d_val"], s.s_val)
+    assert abs(nb - tiny_solution["n_electrons"]) < 1e-9
+    # per-molecule populations close to 8
+    q = np.array([x.population(mu) for x in sols])
+    assert np.abs(q - 8).max() < 0.03
+
+
+def test_density_blocks_layout(tiny_system, tiny_solution):
+    """Block k of row j of D is D(col_idx[k], j): rows of the neighbour, own columns of j."""
+    s = tiny_system
+    sol = tiny_solution["solutions"][9]
+    mu = tiny_solution["mu"]
+    d = sol.density(mu)
+    a = 4
+    k = s.row_ptr[9] + a
+    assert np.abs(tiny_solution["d_val"][k] - d[6 * a:6 * a + 6][:, sol.own]).max() < 1e-14
+
+
+# ------------------------------------------------------------------ generator sanity (inputs)
+def test_generator_properties(tiny_system):
+    s = tiny_system
+    S, H = to_dense(s, "S"), to_dense(s, "H")
+    assert np.array_equal(S, S.T) and np.array_equal(H, H.T)
+    w = np.linalg.eigvalsh(S)
+    assert w[0] > 0.3 and w[-1] < 2.5                                     # SPD without any shift
+    lam = sla.eigh(H, S, eigvals_only=True)
+    nocc = 4 * s.n_mol
+    assert lam[nocc] - lam[nocc - 1] > 0.2                                 # gap at 4 occupied per molecule
+    assert (s.box_q % 2 == 0).all() and s.pos_q.min() >= 0 and (s.pos_q < s.box_q).all()
+    s2 = gi.make_water_system(32, 6.0)
+    assert np.array_equal(s2.pos_q, s.pos_q) and np.array_equal(s2.h_val, s.h_val)   # seeded
+    s3 = gi.make_water_system(32, 6.0, seed=1)
+    assert not np.array_equal(s3.pos_q, s.pos_q)
+
+
+def test_microbench_matrix_properties():
+    a, q, lam = gi.make_gapped_symmetric(64, seed=11)
+    assert np.abs(q.T @ q - np.eye(64)).max() < 1e-12
+    assert 0.05 <= np.abs(lam).min() and np.abs(lam).max() <= 1.0 and (lam > 0).any() and (lam < 0).any()
+    assert np.abs(np.linalg.eigvalsh(a.astype(np.float64)) - np.sort(lam)).max() < 1e-6
+    assert gi.microbench_batch(256) == 512 and gi.microbench_batch(1024) == 8 and gi.microbench_batch(4096) == 1
