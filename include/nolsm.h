@@ -1,0 +1,202 @@
+/* nolsm.h -- C ABI of the B200-native NOLSM hot path (arXiv 2104.08245).
+ *
+ * The path (PAPER.md = the paper text; DESIGN.md lists every reading taken):
+ *   a0  neighbour lists / index sets            Fig. 2 b,c  PAPER.md:172,190; merged pattern :158
+ *   a1  dense submatrices T_j(H), T_j(S)        step (i)    PAPER.md:140; NOLSM :158
+ *   a2  S_j^-1 by the coupled Newton-Schulz     Eq. 15-17
+ *   a3  B_j = S_j^-1 H_j, X0 = (B_j - mu I)/s   Eq. 12      PAPER.md:160; rescaling :138
+ *   a4  sign iteration X <- 1/2 X (3I - X^2)    Eq. 9-10
+ *   a5  D_j[:,own] = 1/2 (I - X) S_j^-1[:,own]  Eq. 12
+ *   a6  write-back of the own columns           step (iii)  PAPER.md:142; Fig. 2 h,i :172-178
+ *   a7  N(mu) = 2 tr(DS), bisection on mu
+ *
+ * Conventions
+ *   - Every array pointer is a DEVICE pointer unless the parameter comment says "host".  The caller
+ *     allocates and owns every array it passes; the context owns only scratch (workspaces, tensor
+ *     maps, statistics).  `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).
+ *   - Calls are asynchronous on `stream` except where a scalar must reach the host; those calls
+ *     say "synchronises".
+ *   - Errors are return codes; nothing throws across this boundary.  nolsm_last_error() gives text.
+ *   - Block-sparse matrices are CSR of uniform bs x bs blocks (bs = 6), FP32, block row-major.
+ *     H and S: block k of row i is block (i, col_idx[k]).  D is column-owned: block k
+ *     of row j holds D(col_idx[k], j), i.e. the rows of neighbour col_idx[k] in the own columns of
+ *     the submatrix of molecule j.  H, S and D share one pattern (row_ptr/col_idx = neighbour list,
+ *     ascending within a row, self included).
+ *   - There is no CPU fallback.  Without a CUDA device every compute entry returns NOLSM_ECUDA.
+ */
+#ifndef NOLSM_H
+#define NOLSM_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct nolsm_ctx nolsm_ctx;     /* opaque: workspaces, tensor maps, statistics */
+typedef struct nolsm_batch nolsm_batch; /* opaque, owned by the context: one batch of dense submatrices */
+
+typedef enum {
+  NOLSM_OK = 0,
+  NOLSM_EINVAL = 1,   /* bad argument (null pointer, negative size, unsupported block size, ...) */
+  NOLSM_ENOMEM = 2,   /* device or host allocation failed / workspace too small for one submatrix */
+  NOLSM_ECUDA = 3,    /* a CUDA call failed (no device, launch error); see nolsm_last_error */
+  NOLSM_ENOTSPD = 4,  /* the inverse iteration (Eq. 15-17) did not converge: S_j not SPD / badly scaled */
+  NOLSM_ENOCONV = 5,  /* sign iteration hit max_iter on the FINAL mu for at least one submatrix */
+  NOLSM_EBRACKET = 6  /* N(mu_lo) > N_e or N(mu_hi) < N_e detected during the bisection */
+} nolsm_status;
+
+typedef enum {
+  NOLSM_FP16_FP32 = 0, /* FP16 operands, FP32 accumulate, FP32 master iterates */
+  NOLSM_FP32 = 1       /* FP32-quality products everywhere */
+} nolsm_precision;
+
+typedef struct {
+  int32_t precision;        /* nolsm_precision */
+  float tol;                /* sign-iteration stop: r_k = ||X_k^2 - I||_F / sqrt(n) < tol, then ONE more
+                               iteration is finished (reading 9).  <= 0: 1e-2 (FP16) / 1e-5 (FP32) */
+  int32_t max_iter;         /* cap on sign iterations (default 30 if <= 0) */
+  int32_t fixed_iter;       /* > 0: run exactly this many sign iterations, no residual test */
+  float inv_tol;            /* stop of Eq. 15-17 on ||I - Z_k Y_k||_F / sqrt(n); <= 0: 1e-2 (FP16) / 3e-6 (FP32) */
+  int32_t inv_max_iter;     /* cap on Eq. 15-17 iterations (default 20 if <= 0) */
+  int32_t inv_refine;       /* FP16 mode: FP32-quality Newton refinements of S^-1 after Eq. 15-17
+                               (reading 11); < 0: default 1;  0 = paper-literal all-FP16 S^-1 */
+  int64_t workspace_bytes;  /* upper bound on the dense workspace the context may allocate (<= 0: 24 GiB) */
+  int32_t group;            /* submatrices iterated together so their iterates stay L2-resident
+                               (<= 0: chosen from the L2 size) */
+  int32_t flags;            /* NOLSM_FLAG_* */
+} nolsm_config;
+
+#define NOLSM_FLAG_SIMT_ONLY 1 /* debugging: run every product on the FP32 SIMT kernel */
+
+typedef struct {            /* CSR of uniform bs x bs FP32 blocks; all pointers device, caller-owned */
+  int32_t n_mol;            /* block rows = molecules */
+  int32_t bs;               /* block size, must be 6 */
+  const int32_t *row_ptr;   /* [n_mol+1] */
+  const int32_t *col_idx;   /* [nnzb], ascending within a row */
+  float *val;               /* [nnzb*bs*bs], each block row-major */
+} nolsm_bsr;
+
+typedef struct {            /* filled by nolsm_sign_batched (host struct) */
+  int32_t n_sub;            /* submatrices in the batch */
+  int32_t iter_min, iter_max;   /* sign iterations executed per submatrix */
+  int64_t iter_sum;
+  int32_t n_unconverged;    /* submatrices that hit max_iter with r >= tol */
+  float worst_residual;     /* max over submatrices of the last residual r_k that was measured */
+  int64_t gemms;            /* n x n x n products executed by this call (all kinds) */
+  double flops_sign;        /* 2 n^3 per executed sign-iteration GEMM, n = TRUE dimension */
+  double flops_sign_padded; /* same with the padded tile extents */
+  double flops_prepare;     /* Eq. 15-17, refinement and B = S^-1 H, if this call ran them */
+  int32_t inv_iter_max;     /* Eq. 15-17 iterations executed (0 if the batch was already prepared) */
+  float inv_worst_residual;
+} nolsm_sign_stats;
+
+typedef struct {            /* filled by nolsm_solve_mu (host struct) */
+  int32_t mu_steps;         /* N(mu) evaluations performed */
+  int32_t n_batches;
+  int32_t resident;         /* 1 if every batch stayed in the workspace across mu steps (S^-1, B reused) */
+  double mu_lo, mu_hi;      /* final bracket */
+  double ne_diag;           /* cross-check: sum_j sum_{c in own_j} (1 - X_cc) of the last step (reading 15) */
+  nolsm_sign_stats last;    /* statistics of the last mu step, summed over batches */
+  double flops_sign_total;  /* over all mu steps */
+  double flops_prepare_total;
+  float ms_gather, ms_prepare, ms_sign, ms_density; /* CUDA-event times summed over batches and steps */
+} nolsm_solve_stats;
+
+/* Context.  `cfg` may be NULL (defaults).  Returns NOLSM_ECUDA when no device is usable. */
+nolsm_status nolsm_create(nolsm_ctx **ctx, const nolsm_config *cfg);
+void nolsm_destroy(nolsm_ctx *ctx);
+const char *nolsm_last_error(const nolsm_ctx *ctx); /* ctx may be NULL: last error of nolsm_create */
+int32_t nolsm_version(void);
+
+/* a0: neighbour list of every molecule from integer positions.
+ * pos_q [n_mol*3] int32 grid units in [0, box_q); box_q host int32[3], each even; rc_q cutoff in grid
+ * units.  Pair (i,j) is kept iff the per-axis minimum-image distance satisfies dx^2+dy^2+dz^2 <= rc_q^2
+ * in int64 (closed ball, self included).  Output CSR: row_ptr [n_mol+1], col_idx ascending per row.
+ * Two passes inside; if the list needs more than `cap` entries nothing is written to col_idx and
+ * NOLSM_ENOMEM is returned with *nnzb_out set to the needed size.  Synchronises (nnzb reaches the host). */
+nolsm_status nolsm_build_neighbours(nolsm_ctx *ctx, int32_t n_mol, const int32_t *pos_q,
+                                    const int32_t *box_q /*host*/, int32_t rc_q, int32_t *row_ptr,
+                                    int32_t *col_idx, int64_t cap, int64_t *nnzb_out /*host*/, void *stream);
+
+/* a1: gather molecules [mol_begin, mol_begin+mol_count) into a context-owned batch
+ * of dense submatrix pairs T_j(H), T_j(S): entry ((a,o),(b,p)) = block (N_j[a], N_j[b]) of the store if
+ * that pair is stored, else 0.  H and S must share row_ptr/col_idx.  *out stays valid until the next
+ * nolsm_build_submatrices on the same slot, nolsm_release_batch or nolsm_destroy.  `slot` selects one
+ * of the context's batch slots (0 for streaming use).  Synchronises once (reads mol_count+1 row
+ * pointers) to size the batch.  NOLSM_ENOMEM if the workspace cannot hold the batch. */
+nolsm_status nolsm_build_submatrices(nolsm_ctx *ctx, const nolsm_bsr *H, const nolsm_bsr *S,
+                                     int32_t mol_begin, int32_t mol_count, int32_t slot,
+                                     nolsm_batch **out, void *stream);
+/* How many molecules starting at mol_begin fit in one batch given the workspace bound (host logic;
+ * needs row_ptr on the device, synchronises).  Returns the count (>= 0) or -status. */
+int32_t nolsm_batch_capacity(nolsm_ctx *ctx, const nolsm_bsr *H, int32_t mol_begin, int32_t n_slots,
+                             void *stream);
+void nolsm_release_batch(nolsm_ctx *ctx, nolsm_batch *batch);
+
+/* a2-a4 (Eq. 15-17, Eq. 12, Eq. 9-10): for every submatrix of the batch, on the first call after the
+ * gather: S_j^-1 and B_j = S_j^-1 H_j; on every call: X0 = (B_j - mu I)/s_j with s_j >= rho(B_j - mu I)
+ * and the sign iteration.  precision/tol/max_iter/fixed_iter < 0 or <= 0 take the context's values.
+ * `stats` (host, may be NULL) makes the call synchronise at its end. */
+nolsm_status nolsm_sign_batched(nolsm_ctx *ctx, nolsm_batch *batch, double mu, int32_t precision,
+                                float tol, int32_t max_iter, int32_t fixed_iter,
+                                nolsm_sign_stats *stats /*host*/, void *stream);
+
+/* a5-a7: D(:, own_j) = 1/2 (I - X_j) S_j^-1(:, own_j) written into rows [mol_begin, ...) of the
+ * column-owned store D (same pattern as S), and 2*sum_blocks <D(i,j), S(i,j)>_F of those rows ADDED to
+ * *ne_partial (device double; FP32 products, FP64 accumulation).  q_mol (device double [n_mol], may be
+ * NULL) receives each molecule's own population; ne_diag (device double, may be NULL) gets
+ * sum_j sum_{c in own_j} (1 - X_cc) added.  Asynchronous. */
+nolsm_status nolsm_scatter_density(nolsm_ctx *ctx, const nolsm_batch *batch, const nolsm_bsr *S,
+                                   nolsm_bsr *D, double *ne_partial, double *q_mol, double *ne_diag,
+                                   void *stream);
+
+/* Whole path (a1-a7) with batching and the bisection of PAPER.md:227: mu = (mu_lo+mu_hi)/2; stop when
+ * |N(mu) - n_electrons| <= tol_ne_per_mol * n_mol or after max_steps evaluations (tol_ne_per_mol < 0:
+ * always run exactly max_steps evaluations, the timing workload of BASELINE configs[1]);
+ * N(mu) > N_e -> mu_hi = mu else mu_lo = mu.  D holds the density of the last evaluated mu.
+ * mu_out, ne_out: host doubles.  q_mol: device double [n_mol] or NULL.  Synchronises once per step. */
+nolsm_status nolsm_solve_mu(nolsm_ctx *ctx, const nolsm_bsr *H, const nolsm_bsr *S, double n_electrons,
+                            double mu_lo, double mu_hi, double tol_ne_per_mol, int32_t max_steps,
+                            int32_t precision, nolsm_bsr *D, double *mu_out /*host*/,
+                            double *ne_out /*host*/, double *q_mol, nolsm_solve_stats *stats /*host*/,
+                            void *stream);
+
+/* Dense microbench entry (BASELINE configs[4]; analogue of the paper's Fig. 6):
+ * sign(A_b) for `batch` dense n x n FP32 matrices stored one after another (row-major, leading
+ * dimension n).  X0 = A_b / scale[b] (scale: device float [batch], e.g. ||A_b||_2; NULL: the
+ * sqrt(||A||_1 ||A||_inf) bound is computed).  x_out: device float [batch*n*n], row-major sign(A_b). */
+nolsm_status nolsm_sign_dense_batched(nolsm_ctx *ctx, const float *a, const float *scale, int32_t n,
+                                      int32_t batch, int32_t precision, float tol, int32_t max_iter,
+                                      int32_t fixed_iter, float *x_out, nolsm_sign_stats *stats /*host*/,
+                                      void *stream);
+
+/* Inspection of a batch (tests, parity of the intermediate steps).  which: see NOLSM_MAT_*.
+ * Copies submatrix `local` (0-based inside the batch) as a row-major n_j x n_j FP32 matrix into dst
+ * (device, capacity dst_elems floats).  *n_out (host) = n_j.  Synchronises. */
+#define NOLSM_MAT_S 0     /* T_j(S) as gathered */
+#define NOLSM_MAT_H 1     /* T_j(H) as gathered */
+#define NOLSM_MAT_SINV 2  /* S_j^-1 (after nolsm_sign_batched) */
+#define NOLSM_MAT_B 3     /* B_j = S_j^-1 H_j */
+#define NOLSM_MAT_X 4     /* last sign iterate X_j */
+nolsm_status nolsm_batch_read(nolsm_ctx *ctx, const nolsm_batch *batch, int32_t local, int32_t which,
+                              float *dst, int64_t dst_elems, int32_t *n_out /*host*/, void *stream);
+int32_t nolsm_batch_size(const nolsm_batch *batch);      /* submatrices in the batch */
+int32_t nolsm_batch_ld(const nolsm_batch *batch);        /* padded leading dimension */
+
+/* One batched product with the engine's own kernels (unit tests of the GEMM building block):
+ * C_b = beta*Cin_b + alpha*A_b*B_b (ident = 0)  or  C_b = I - A_b*B_b (ident = 1), b < batch, all
+ * n x n row-major FP32 on the device (n arbitrary).  kind: 0 = FP32 SIMT, 1 = tcgen05 FP16 operands,
+ * 2 = tcgen05 split-FP16 (FP32-quality).  resid2 (device float[batch], may be NULL) receives
+ * ||C_b||_F^2 when ident = 1. */
+nolsm_status nolsm_gemm_batched(nolsm_ctx *ctx, int32_t kind, int32_t ident, float alpha, float beta,
+                                const float *a, const float *b, const float *cin, float *c,
+                                float *resid2, int32_t n, int32_t batch, void *stream);
+
+/* Kernel launches issued by this context so far (bench.py's gpu_launches). */
+int64_t nolsm_launch_count(const nolsm_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NOLSM_H */

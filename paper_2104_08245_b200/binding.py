@@ -1,0 +1,323 @@
+"""ctypes binding of libnolsm.so.  Names follow include/nolsm.h one to one:
+Context.build_neighbours / build_submatrices / sign_batched / scatter_density / solve_mu /
+sign_dense_batched.  torch is used for device memory and streams only."""
+import ctypes as C
+import os
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+FP16_FP32, FP32 = 0, 1
+MAT_S, MAT_H, MAT_SINV, MAT_B, MAT_X = 0, 1, 2, 3, 4
+FLAG_SIMT_ONLY = 1
+STATUS = {0: "NOLSM_OK", 1: "NOLSM_EINVAL", 2: "NOLSM_ENOMEM", 3: "NOLSM_ECUDA", 4: "NOLSM_ENOTSPD",
+          5: "NOLSM_ENOCONV", 6: "NOLSM_EBRACKET"}
+
+EXPORTED_SYMBOLS = [
+    "nolsm_create", "nolsm_destroy", "nolsm_last_error", "nolsm_version", "nolsm_build_neighbours",
+    "nolsm_build_submatrices", "nolsm_batch_capacity", "nolsm_release_batch", "nolsm_sign_batched",
+    "nolsm_scatter_density", "nolsm_solve_mu", "nolsm_sign_dense_batched", "nolsm_batch_read",
+    "nolsm_batch_size", "nolsm_batch_ld", "nolsm_gemm_batched", "nolsm_launch_count",
+]
+
+
+class NolsmError(RuntimeError):
+    def __init__(self, status, message):
+        super().__init__(f"{STATUS.get(status, status)}: {message}")
+        self.status = status
+
+
+class Config(C.Structure):
+    _fields_ = [("precision", C.c_int32), ("tol", C.c_float), ("max_iter", C.c_int32), ("fixed_iter", C.c_int32),
+                ("inv_tol", C.c_float), ("inv_max_iter", C.c_int32), ("inv_refine", C.c_int32),
+                ("workspace_bytes", C.c_int64), ("group", C.c_int32), ("flags", C.c_int32)]
+
+    def __init__(self, precision=FP16_FP32, tol=0.0, max_iter=0, fixed_iter=0, inv_tol=0.0, inv_max_iter=0,
+                 inv_refine=-1, workspace_bytes=0, group=0, flags=0):
+        super().__init__(precision, tol, max_iter, fixed_iter, inv_tol, inv_max_iter, inv_refine,
+                         workspace_bytes, group, flags)
+
+
+class _Bsr(C.Structure):
+    _fields_ = [("n_mol", C.c_int32), ("bs", C.c_int32), ("row_ptr", C.c_void_p), ("col_idx", C.c_void_p),
+                ("val", C.c_void_p)]
+
+
+class SignStats(C.Structure):
+    _fields_ = [("n_sub", C.c_int32), ("iter_min", C.c_int32), ("iter_max", C.c_int32), ("iter_sum", C.c_int64),
+                ("n_unconverged", C.c_int32), ("worst_residual", C.c_float), ("gemms", C.c_int64),
+                ("flops_sign", C.c_double), ("flops_sign_padded", C.c_double), ("flops_prepare", C.c_double),
+                ("inv_iter_max", C.c_int32), ("inv_worst_residual", C.c_float)]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_}
+
+
+class SolveStats(C.Structure):
+    _fields_ = [("mu_steps", C.c_int32), ("n_batches", C.c_int32), ("resident", C.c_int32),
+                ("mu_lo", C.c_double), ("mu_hi", C.c_double), ("ne_diag", C.c_double), ("last", SignStats),
+                ("flops_sign_total", C.c_double), ("flops_prepare_total", C.c_double),
+                ("ms_gather", C.c_float), ("ms_prepare", C.c_float), ("ms_sign", C.c_float),
+                ("ms_density", C.c_float)]
+
+    def as_dict(self):
+        d = {k: getattr(self, k) for k, _ in self._fields_ if k != "last"}
+        d["last"] = self.last.as_dict()
+        return d
+
+
+def library_path():
+    return os.path.join(HERE, "libnolsm.so")
+
+
+_LIB = None
+
+
+def load_library():
+    """dlopen libnolsm.so (built by paper_2104_08245_b200.build).  Raises if it is missing: there is
+    no other implementation to fall back to."""
+    global _LIB
+    if _LIB is not None:
+        return _LIB
+    path = library_path()
+    if not os.path.exists(path):
+        raise NolsmError(3, f"{path} not built; run `python -m paper_2104_08245_b200.build`")
+    lib = C.CDLL(path)
+    vp, i32, i64, f32, f64 = C.c_void_p, C.c_int32, C.c_int64, C.c_float, C.c_double
+    P = C.POINTER
+    lib.nolsm_create.argtypes = [P(vp), P(Config)]
+    lib.nolsm_create.restype = i32
+    lib.nolsm_destroy.argtypes = [vp]
+    lib.nolsm_destroy.restype = None
+    lib.nolsm_last_error.argtypes = [vp]
+    lib.nolsm_last_error.restype = C.c_char_p
+    lib.nolsm_version.restype = i32
+    lib.nolsm_launch_count.argtypes = [vp]
+    lib.nolsm_launch_count.restype = i64
+    lib.nolsm_build_neighbours.argtypes = [vp, i32, vp, P(i32), i32, vp, vp, i64, P(i64), vp]
+    lib.nolsm_build_neighbours.restype = i32
+    lib.nolsm_build_submatrices.argtypes = [vp, P(_Bsr), P(_Bsr), i32, i32, i32, P(vp), vp]
+    lib.nolsm_build_submatrices.restype = i32
+    lib.nolsm_batch_capacity.argtypes = [vp, P(_Bsr), i32, i32, vp]
+    lib.nolsm_batch_capacity.restype = i32
+    lib.nolsm_release_batch.argtypes = [vp, vp]
+    lib.nolsm_release_batch.restype = None
+    lib.nolsm_sign_batched.argtypes = [vp, vp, f64, i32, f32, i32, i32, P(SignStats), vp]
+    lib.nolsm_sign_batched.restype = i32
+    lib.nolsm_scatter_density.argtypes = [vp, vp, P(_Bsr), P(_Bsr), vp, vp, vp, vp]
+    lib.nolsm_scatter_density.restype = i32
+    lib.nolsm_solve_mu.argtypes = [vp, P(_Bsr), P(_Bsr), f64, f64, f64, f64, i32, i32, P(_Bsr), P(f64), P(f64),
+                                   vp, P(SolveStats), vp]
+    lib.nolsm_solve_mu.restype = i32
+    lib.nolsm_sign_dense_batched.argtypes = [vp, vp, vp, i32, i32, i32, f32, i32, i32, vp, P(SignStats), vp]
+    lib.nolsm_sign_dense_batched.restype = i32
+    lib.nolsm_batch_read.argtypes = [vp, vp, i32, i32, vp, i64, P(i32), vp]
+    lib.nolsm_batch_read.restype = i32
+    lib.nolsm_batch_size.argtypes = [vp]
+    lib.nolsm_batch_size.restype = i32
+    lib.nolsm_batch_ld.argtypes = [vp]
+    lib.nolsm_batch_ld.restype = i32
+    lib.nolsm_gemm_batched.argtypes = [vp, i32, i32, f32, f32, vp, vp, vp, vp, vp, i32, i32, vp]
+    lib.nolsm_gemm_batched.restype = i32
+    if hasattr(lib, "nolsm_debug_set_desc"):
+        lib.nolsm_debug_set_desc.argtypes = [C.c_uint32, C.c_uint32, C.c_uint32]
+        lib.nolsm_debug_set_desc.restype = None
+    _LIB = lib
+    return lib
+
+
+def _torch():
+    import torch
+    return torch
+
+
+def _ptr(t, dtype=None):
+    """Device pointer of a contiguous CUDA tensor (None -> NULL)."""
+    if t is None:
+        return None
+    torch = _torch()
+    if not t.is_cuda:
+        raise NolsmError(1, "tensor must live on the CUDA device")
+    if not t.is_contiguous():
+        raise NolsmError(1, "tensor must be contiguous")
+    if dtype is not None and t.dtype != dtype:
+        raise NolsmError(1, f"tensor dtype {t.dtype}, expected {dtype}")
+    return C.c_void_p(t.data_ptr())
+
+
+def _stream(stream):
+    torch = _torch()
+    s = torch.cuda.current_stream() if stream is None else stream
+    return C.c_void_p(s.cuda_stream)
+
+
+class BlockSparse:
+    """CSR of 6x6 FP32 blocks on the device (nolsm_bsr).  row_ptr/col_idx int32, val float32 [nnzb,6,6]."""
+
+    def __init__(self, row_ptr, col_idx, val):
+        torch = _torch()
+        self.row_ptr, self.col_idx, self.val = row_ptr, col_idx, val
+        self.n_mol = int(row_ptr.numel()) - 1
+        self._c = _Bsr(self.n_mol, 6, _ptr(row_ptr, torch.int32).value, _ptr(col_idx, torch.int32).value,
+                       _ptr(val, torch.float32).value)
+
+    @classmethod
+    def from_numpy(cls, row_ptr, col_idx, val, device="cuda"):
+        torch = _torch()
+        return cls(torch.as_tensor(row_ptr, dtype=torch.int32).to(device),
+                   torch.as_tensor(col_idx, dtype=torch.int32).to(device),
+                   torch.as_tensor(val, dtype=torch.float32).contiguous().to(device))
+
+    def like(self):
+        torch = _torch()
+        return BlockSparse(self.row_ptr, self.col_idx, torch.zeros_like(self.val))
+
+    def ref(self):
+        return C.byref(self._c)
+
+
+class Batch:
+    def __init__(self, ctx, handle):
+        self.ctx, self.handle = ctx, handle
+
+    @property
+    def size(self):
+        return self.ctx.lib.nolsm_batch_size(self.handle)
+
+    @property
+    def ld(self):
+        return self.ctx.lib.nolsm_batch_ld(self.handle)
+
+    def read(self, local, which, stream=None):
+        """Row-major n_j x n_j FP32 copy of one matrix of the batch (tests)."""
+        torch = _torch()
+        ld = self.ld
+        buf = torch.empty(ld * ld, dtype=torch.float32, device="cuda")
+        n = C.c_int32(0)
+        self.ctx._check(self.ctx.lib.nolsm_batch_read(self.ctx.handle, self.handle, local, which, _ptr(buf),
+                                                      buf.numel(), C.byref(n), _stream(stream)))
+        return buf[: n.value * n.value].view(n.value, n.value)
+
+
+class Context:
+    """nolsm_ctx.  Raises NolsmError when the library or a CUDA device is missing."""
+
+    def __init__(self, config=None):
+        self.lib = load_library()
+        self.handle = C.c_void_p()
+        self.config = config if config is not None else Config()
+        st = self.lib.nolsm_create(C.byref(self.handle), C.byref(self.config))
+        if st != 0:
+            msg = self.lib.nolsm_last_error(None)
+            self.handle = None
+            raise NolsmError(st, msg.decode() if msg else "")
+
+    def close(self):
+        if getattr(self, "handle", None):
+            self.lib.nolsm_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, st):
+        if st != 0:
+            msg = self.lib.nolsm_last_error(self.handle)
+            raise NolsmError(st, msg.decode() if msg else "")
+
+    @property
+    def launch_count(self):
+        return int(self.lib.nolsm_launch_count(self.handle))
+
+    # a0 -----------------------------------------------------------------------------------------
+    def build_neighbours(self, pos_q, box_q, rc_q, cap=None, stream=None):
+        """pos_q: int32 CUDA tensor [n_mol,3]; box_q: 3 ints (host).  Returns (row_ptr, col_idx)."""
+        torch = _torch()
+        n_mol = int(pos_q.shape[0])
+        row_ptr = torch.empty(n_mol + 1, dtype=torch.int32, device=pos_q.device)
+        box = (C.c_int32 * 3)(*[int(x) for x in box_q])
+        nnzb = C.c_int64(0)
+        if cap is None:
+            st = self.lib.nolsm_build_neighbours(self.handle, n_mol, _ptr(pos_q, torch.int32), box, int(rc_q),
+                                                 _ptr(row_ptr), None, 0, C.byref(nnzb), _stream(stream))
+            if st not in (0, 2):
+                self._check(st)
+            cap = nnzb.value
+        col_idx = torch.empty(max(cap, 1), dtype=torch.int32, device=pos_q.device)
+        self._check(self.lib.nolsm_build_neighbours(self.handle, n_mol, _ptr(pos_q, torch.int32), box, int(rc_q),
+                                                    _ptr(row_ptr), _ptr(col_idx), cap, C.byref(nnzb),
+                                                    _stream(stream)))
+        return row_ptr, col_idx[: nnzb.value]
+
+    # a1 -----------------------------------------------------------------------------------------
+    def build_submatrices(self, H, S, mol_begin, mol_count, slot=0, stream=None):
+        h = C.c_void_p()
+        self._check(self.lib.nolsm_build_submatrices(self.handle, H.ref(), S.ref(), mol_begin, mol_count, slot,
+                                                     C.byref(h), _stream(stream)))
+        return Batch(self, h)
+
+    def batch_capacity(self, H, mol_begin=0, n_slots=1, stream=None):
+        r = self.lib.nolsm_batch_capacity(self.handle, H.ref(), mol_begin, n_slots, _stream(stream))
+        if r < 0:
+            self._check(-r)
+        return r
+
+    # a2-a4 --------------------------------------------------------------------------------------
+    def sign_batched(self, batch, mu, precision=-1, tol=0.0, max_iter=0, fixed_iter=-1, want_stats=True,
+                     stream=None):
+        stats = SignStats() if want_stats else None
+        self._check(self.lib.nolsm_sign_batched(self.handle, batch.handle, float(mu), precision, tol, max_iter,
+                                                fixed_iter, C.byref(stats) if want_stats else None,
+                                                _stream(stream)))
+        return stats
+
+    # a5-a7 --------------------------------------------------------------------------------------
+    def scatter_density(self, batch, S, D, ne_partial, q_mol=None, ne_diag=None, stream=None):
+        torch = _torch()
+        self._check(self.lib.nolsm_scatter_density(self.handle, batch.handle, S.ref(), D.ref(),
+                                                   _ptr(ne_partial, torch.float64), _ptr(q_mol, torch.float64),
+                                                   _ptr(ne_diag, torch.float64), _stream(stream)))
+
+    # whole path -----------------------------------------------------------------------------------
+    def solve_mu(self, H, S, n_electrons, mu_lo, mu_hi, tol_ne_per_mol=1e-3, max_steps=40, precision=-1, D=None,
+                 q_mol=None, want_stats=True, stream=None):
+        """Returns (mu, n_electrons(mu), D, stats)."""
+        torch = _torch()
+        if D is None:
+            D = S.like()
+        mu, ne = C.c_double(0.0), C.c_double(0.0)
+        stats = SolveStats() if want_stats else None
+        st = self.lib.nolsm_solve_mu(self.handle, H.ref(), S.ref(), float(n_electrons), float(mu_lo), float(mu_hi),
+                                     float(tol_ne_per_mol), int(max_steps), precision, D.ref(), C.byref(mu),
+                                     C.byref(ne), _ptr(q_mol, torch.float64),
+                                     C.byref(stats) if want_stats else None, _stream(stream))
+        self._check(st)
+        return mu.value, ne.value, D, stats
+
+    # dense microbench -------------------------------------------------------------------------------
+    def sign_dense_batched(self, a, scale=None, precision=-1, tol=0.0, max_iter=0, fixed_iter=-1, out=None,
+                           want_stats=True, stream=None):
+        """a: float32 CUDA tensor [batch,n,n] row-major.  Returns (sign(a) [batch,n,n], stats)."""
+        torch = _torch()
+        batch, n = int(a.shape[0]), int(a.shape[1])
+        if out is None:
+            out = torch.empty_like(a)
+        stats = SignStats() if want_stats else None
+        self._check(self.lib.nolsm_sign_dense_batched(self.handle, _ptr(a, torch.float32), _ptr(scale, torch.float32),
+                                                      n, batch, precision, tol, max_iter, fixed_iter,
+                                                      _ptr(out, torch.float32),
+                                                      C.byref(stats) if want_stats else None, _stream(stream)))
+        return out, stats
+
+    # GEMM building block (tests) ---------------------------------------------------------------------
+    def gemm_batched(self, kind, a, b, cin=None, ident=False, alpha=1.0, beta=0.0, stream=None):
+        torch = _torch()
+        batch, n = int(a.shape[0]), int(a.shape[1])
+        c = torch.empty_like(a)
+        resid2 = torch.zeros(batch, dtype=torch.float32, device=a.device)
+        self._check(self.lib.nolsm_gemm_batched(self.handle, kind, 1 if ident else 0, alpha, beta,
+                                                _ptr(a, torch.float32), _ptr(b, torch.float32),
+                                                _ptr(cin, torch.float32), _ptr(c, torch.float32), _ptr(resid2), n,
+                                                batch, _stream(stream)))
+        return c, resid2

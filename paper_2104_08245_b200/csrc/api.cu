@@ -1,0 +1,888 @@
+// C ABI of libnolsm (include/nolsm.h): context, batching, iteration drivers, mu bisection.
+// Host logic only; every arithmetic step of the path runs in the kernels of the other files.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include "common.cuh"
+
+static std::string g_create_err;
+
+#define LAUNCH(ctx, call)                                                                   \
+  do {                                                                                      \
+    cudaError_t e__ = (call);                                                               \
+    (ctx)->launches++;                                                                      \
+    if (e__ != cudaSuccess) {                                                               \
+      (ctx)->err = std::string(#call) + ": " + cudaGetErrorString(e__);                     \
+      return NOLSM_ECUDA;                                                                   \
+    }                                                                                       \
+  } while (0)
+
+#define CHECK(st)                                  \
+  do {                                             \
+    nolsm_status s__ = (st);                       \
+    if (s__ != NOLSM_OK) return s__;               \
+  } while (0)
+
+static int effective_precision(const nolsm_ctx *ctx, int precision) {
+  int p = precision < 0 ? ctx->cfg.precision : precision;
+  if (ctx->cfg.flags & NOLSM_FLAG_SIMT_ONLY) p = NOLSM_FP32;
+  return p;
+}
+
+// ------------------------------------------------------------------------------------------------
+extern "C" int32_t nolsm_version(void) { return 1; }
+
+extern "C" const char *nolsm_last_error(const nolsm_ctx *ctx) {
+  return ctx ? ctx->err.c_str() : g_create_err.c_str();
+}
+
+extern "C" int64_t nolsm_launch_count(const nolsm_ctx *ctx) { return ctx ? ctx->launches : 0; }
+
+extern "C" nolsm_status nolsm_create(nolsm_ctx **out, const nolsm_config *cfg) {
+  if (!out) return NOLSM_EINVAL;
+  *out = nullptr;
+  int ndev = 0;
+  cudaError_t e = cudaGetDeviceCount(&ndev);
+  if (e != cudaSuccess || ndev == 0) {
+    g_create_err = std::string("no CUDA device: ") + cudaGetErrorString(e);
+    cudaGetLastError();
+    return NOLSM_ECUDA;
+  }
+  nolsm_ctx *ctx = new nolsm_ctx();
+  nolsm_config c;
+  memset(&c, 0, sizeof(c));
+  if (cfg) c = *cfg;
+  else { c.inv_refine = -1; }
+  if (c.precision != NOLSM_FP16_FP32 && c.precision != NOLSM_FP32) { delete ctx; return NOLSM_EINVAL; }
+  if (c.max_iter <= 0) c.max_iter = 30;
+  if (c.max_iter > NOLSM_MAX_RESID_SLOTS) c.max_iter = NOLSM_MAX_RESID_SLOTS;
+  if (c.inv_max_iter <= 0) c.inv_max_iter = 20;
+  if (c.inv_max_iter > NOLSM_MAX_RESID_SLOTS) c.inv_max_iter = NOLSM_MAX_RESID_SLOTS;
+  if (c.inv_refine < 0) c.inv_refine = 1;
+  if (c.workspace_bytes <= 0) c.workspace_bytes = (int64_t)24 << 30;
+  ctx->cfg = c;
+  cudaGetDevice(&ctx->device);
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, ctx->device) != cudaSuccess) {
+    g_create_err = "cudaGetDeviceProperties failed";
+    delete ctx;
+    return NOLSM_ECUDA;
+  }
+  ctx->sm_count = prop.multiProcessorCount;
+  ctx->l2_bytes = (size_t)prop.l2CacheSize;
+  if (cudaMalloc(&ctx->d_scalars, 4 * sizeof(double)) != cudaSuccess ||
+      cudaMallocHost(&ctx->h_scalars, 4 * sizeof(double)) != cudaSuccess ||
+      cudaMallocHost(&ctx->h_active, NOLSM_MAX_RESID_SLOTS * sizeof(int32_t)) != cudaSuccess) {
+    g_create_err = "allocation of context scalars failed";
+    delete ctx;
+    return NOLSM_ENOMEM;
+  }
+  for (int i = 0; i < 4; ++i) cudaEventCreateWithFlags(&ctx->ev[i], cudaEventDisableTiming);
+  if (prop.major == 10) {
+    if (umma_init(ctx) != NOLSM_OK) g_create_err = ctx->err;
+  } else {
+    ctx->err = "device is not sm_100: tcgen05 path unavailable";
+  }
+  *out = ctx;
+  return NOLSM_OK;
+}
+
+static void free_batch(nolsm_batch *b) {
+  if (!b) return;
+  cudaFree(b->base);
+  cudaFree(b->d_dims);
+  cudaFree(b->d_state);
+  cudaFree(b->d_iters);
+  cudaFree(b->d_resid2);
+  cudaFree(b->d_lastres);
+  cudaFree(b->d_scale);
+  cudaFree(b->d_norm);
+  cudaFree(b->d_active);
+  cudaFree(b->d_tiles);
+  cudaFree(b->d_tiles_simt);
+  delete b;
+}
+
+extern "C" void nolsm_destroy(nolsm_ctx *ctx) {
+  if (!ctx) return;
+  cudaDeviceSynchronize();
+  for (nolsm_batch *b : ctx->slots) free_batch(b);
+  cudaFree(ctx->d_scalars);
+  cudaFreeHost(ctx->h_scalars);
+  cudaFreeHost(ctx->h_active);
+  for (int i = 0; i < 4; ++i)
+    if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
+  delete ctx;
+}
+
+extern "C" void nolsm_release_batch(nolsm_ctx *ctx, nolsm_batch *batch) {
+  if (!ctx || !batch) return;
+  cudaDeviceSynchronize();
+  for (size_t i = 0; i < ctx->slots.size(); ++i)
+    if (ctx->slots[i] == batch) {
+      free_batch(batch);
+      ctx->slots[i] = nullptr;
+    }
+}
+
+extern "C" int32_t nolsm_batch_size(const nolsm_batch *b) { return b ? b->count : 0; }
+extern "C" int32_t nolsm_batch_ld(const nolsm_batch *b) { return b ? b->ld : 0; }
+
+// ------------------------------------------------------------------------------------------------
+// Batch storage
+// ------------------------------------------------------------------------------------------------
+static size_t dense_bytes(int count, int ld) { return (size_t)7 * 4 * (size_t)ld * ld * (size_t)count; }
+
+static size_t allocated_bytes(const nolsm_ctx *ctx, int except_slot) {
+  size_t t = 0;
+  for (size_t i = 0; i < ctx->slots.size(); ++i)
+    if (ctx->slots[i] && (int)i != except_slot) t += ctx->slots[i]->base_bytes;
+  return t;
+}
+
+template <typename T>
+static cudaError_t grow(T **ptr, size_t n) {
+  cudaFree(*ptr);
+  *ptr = nullptr;
+  return cudaMalloc(ptr, n * sizeof(T));
+}
+
+// Size slot `slot` for `dims` (true dimensions) and upload the metadata.  Host-synchronous uploads
+// (small); the dense workspace is grow-only.
+static nolsm_status setup_batch(nolsm_ctx *ctx, int slot, const std::vector<int32_t> &dims, int mol_begin,
+                                bool sparse, nolsm_batch **out, cudaStream_t st) {
+  if (slot < 0 || slot > 4096) { ctx->err = "bad slot"; return NOLSM_EINVAL; }
+  if ((int)ctx->slots.size() <= slot) ctx->slots.resize(slot + 1, nullptr);
+  if (!ctx->slots[slot]) ctx->slots[slot] = new nolsm_batch();
+  nolsm_batch *b = ctx->slots[slot];
+  const int count = (int)dims.size();
+  int max_n = 0;
+  for (int n : dims) max_n = std::max(max_n, n);
+  const int ld = std::max(NOLSM_PAD, round_up(max_n, NOLSM_PAD));
+  const size_t need = dense_bytes(count, ld);
+  if (need > b->base_bytes) {
+    if ((int64_t)(allocated_bytes(ctx, slot) + need) > ctx->cfg.workspace_bytes) {
+      ctx->err = "workspace_bytes too small for this batch";
+      return NOLSM_ENOMEM;
+    }
+    cudaStreamSynchronize(st);
+    cudaFree(b->base);
+    b->base = nullptr;
+    b->base_bytes = 0;
+    if (cudaMalloc(&b->base, need) != cudaSuccess) {
+      cudaGetLastError();
+      ctx->err = "cudaMalloc of the dense workspace failed";
+      return NOLSM_ENOMEM;
+    }
+    b->base_bytes = need;
+  }
+  if ((size_t)count > b->meta_cap) {
+    cudaStreamSynchronize(st);
+    const size_t cap = (size_t)count;
+    if (grow(&b->d_dims, cap) || grow(&b->d_state, cap) || grow(&b->d_iters, cap) ||
+        grow(&b->d_resid2, cap * NOLSM_MAX_RESID_SLOTS) || grow(&b->d_lastres, cap) ||
+        grow(&b->d_scale, cap) || grow(&b->d_norm, cap * 2) ||
+        (b->d_active == nullptr && grow(&b->d_active, (size_t)NOLSM_MAX_RESID_SLOTS))) {
+      cudaGetLastError();
+      ctx->err = "cudaMalloc of batch metadata failed";
+      return NOLSM_ENOMEM;
+    }
+    b->meta_cap = cap;
+  }
+  b->count = count;
+  b->ld = ld;
+  b->max_n = max_n;
+  b->mol_begin = mol_begin;
+  b->slot = slot;
+  b->sparse = sparse;
+  b->prepared = false;
+  b->prepared_precision = -1;
+  b->n_host = dims;
+  b->bn = 128;
+  const size_t slab = (size_t)ld * ld;
+  for (int i = 0; i < 7; ++i) b->u[i] = reinterpret_cast<float *>(b->base) + (size_t)i * count * slab;
+  for (int i = 0; i < 6; ++i) b->h[i] = reinterpret_cast<__half *>(b->u[4]) + (size_t)i * count * slab;
+  // tile lists
+  std::vector<TileDesc> tiles, tiles_simt;
+  b->sum_n3 = b->sum_n3_padded = 0.0;
+  for (int m = 0; m < count; ++m) {
+    const int n = dims[m];
+    const int P = round_up(n, NOLSM_TILE_M), Pn = round_up(n, 64);
+    for (int n0 = 0; n0 < Pn; n0 += b->bn)
+      for (int m0 = 0; m0 < P; m0 += NOLSM_TILE_M)
+        tiles.push_back(TileDesc{m, m0, n0, std::min(b->bn, Pn - n0)});
+    for (int n0 = 0; n0 < P; n0 += 128)
+      for (int m0 = 0; m0 < P; m0 += 128) tiles_simt.push_back(TileDesc{m, m0, n0, 128});
+    b->sum_n3 += (double)n * n * n;
+    b->sum_n3_padded += (double)P * Pn * Pn;
+  }
+  if (tiles.size() > b->tiles_cap) {
+    cudaStreamSynchronize(st);
+    if (grow(&b->d_tiles, tiles.size())) { cudaGetLastError(); ctx->err = "cudaMalloc tiles"; return NOLSM_ENOMEM; }
+    b->tiles_cap = tiles.size();
+  }
+  if (tiles_simt.size() > b->tiles_simt_cap) {
+    cudaStreamSynchronize(st);
+    if (grow(&b->d_tiles_simt, tiles_simt.size())) { cudaGetLastError(); ctx->err = "cudaMalloc tiles"; return NOLSM_ENOMEM; }
+    b->tiles_simt_cap = tiles_simt.size();
+  }
+  b->n_tiles = (int)tiles.size();
+  b->n_tiles_simt = (int)tiles_simt.size();
+  // pageable host buffers: cudaMemcpyAsync stages them before returning, so the vectors may die
+  NOLSM_CUDA(ctx, cudaMemcpyAsync(b->d_dims, dims.data(), sizeof(int32_t) * count, cudaMemcpyHostToDevice, st));
+  if (!tiles.empty())
+    NOLSM_CUDA(ctx, cudaMemcpyAsync(b->d_tiles, tiles.data(), sizeof(TileDesc) * tiles.size(),
+                                    cudaMemcpyHostToDevice, st));
+  if (!tiles_simt.empty())
+    NOLSM_CUDA(ctx, cudaMemcpyAsync(b->d_tiles_simt, tiles_simt.data(), sizeof(TileDesc) * tiles_simt.size(),
+                                    cudaMemcpyHostToDevice, st));
+  NOLSM_CUDA(ctx, cudaStreamSynchronize(st));
+  CHECK(umma_make_maps(ctx, b));
+  *out = b;
+  return NOLSM_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// a0
+// ------------------------------------------------------------------------------------------------
+extern "C" nolsm_status nolsm_build_neighbours(nolsm_ctx *ctx, int32_t n_mol, const int32_t *pos_q,
+                                               const int32_t *box_q, int32_t rc_q, int32_t *row_ptr,
+                                               int32_t *col_idx, int64_t cap, int64_t *nnzb_out, void *stream) {
+  if (!ctx) return NOLSM_EINVAL;
+  if (n_mol < 0 || !row_ptr || !box_q || (n_mol > 0 && !pos_q) || rc_q < 0 || cap < 0) {
+    ctx->err = "nolsm_build_neighbours: bad argument";
+    return NOLSM_EINVAL;
+  }
+  for (int a = 0; a < 3; ++a)
+    if (box_q[a] <= 0 || (box_q[a] & 1)) { ctx->err = "box lengths must be positive and even"; return NOLSM_EINVAL; }
+  cudaStream_t st = (cudaStream_t)stream;
+  int32_t *counts = nullptr;
+  NOLSM_CUDA(ctx, cudaMalloc(&counts, sizeof(int32_t) * std::max(n_mol, 1)));
+  cudaError_t e = launch_neighbour_count(n_mol, pos_q, box_q, rc_q, counts, st);
+  ctx->launches++;
+  if (e == cudaSuccess) { e = launch_exclusive_scan(counts, row_ptr, n_mol, st); ctx->launches++; }
+  int32_t total = 0;
+  if (e == cudaSuccess) e = cudaMemcpyAsync(&total, row_ptr + n_mol, sizeof(int32_t), cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  cudaFree(counts);
+  if (e != cudaSuccess) { ctx->err = std::string("neighbour count: ") + cudaGetErrorString(e); return NOLSM_ECUDA; }
+  if (nnzb_out) *nnzb_out = total;
+  if ((int64_t)total > cap || (total > 0 && !col_idx)) {
+    ctx->err = "col_idx capacity too small";
+    return NOLSM_ENOMEM;
+  }
+  LAUNCH(ctx, launch_neighbour_fill(n_mol, pos_q, box_q, rc_q, row_ptr, col_idx, st));
+  return NOLSM_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// a1
+// ------------------------------------------------------------------------------------------------
+static nolsm_status check_bsr(nolsm_ctx *ctx, const nolsm_bsr *m, const char *name) {
+  if (!m || m->bs != NOLSM_BS || m->n_mol < 0 || !m->row_ptr || (m->n_mol > 0 && (!m->col_idx || !m->val))) {
+    ctx->err = std::string("bad block-sparse matrix ") + name + " (bs must be 6, pointers non-null)";
+    return NOLSM_EINVAL;
+  }
+  return NOLSM_OK;
+}
+
+static nolsm_status read_dims(nolsm_ctx *ctx, const int32_t *row_ptr, int mol_begin, int mol_count,
+                              std::vector<int32_t> &dims, cudaStream_t st) {
+  std::vector<int32_t> rp(mol_count + 1);
+  NOLSM_CUDA(ctx, cudaMemcpyAsync(rp.data(), row_ptr + mol_begin, sizeof(int32_t) * (mol_count + 1),
+                                  cudaMemcpyDeviceToHost, st));
+  NOLSM_CUDA(ctx, cudaStreamSynchronize(st));
+  dims.resize(mol_count);
+  for (int i = 0; i < mol_count; ++i) {
+    dims[i] = (rp[i + 1] - rp[i]) * NOLSM_BS;
+    if (dims[i] <= 0) { ctx->err = "molecule with an empty neighbour list (self must be included)"; return NOLSM_EINVAL; }
+  }
+  return NOLSM_OK;
+}
+
+extern "C" int32_t nolsm_batch_capacity(nolsm_ctx *ctx, const nolsm_bsr *H, int32_t mol_begin, int32_t n_slots,
+                                        void *stream) {
+  if (!ctx || check_bsr(ctx, H, "H") != NOLSM_OK || mol_begin < 0 || mol_begin > H->n_mol || n_slots <= 0)
+    return -(int32_t)NOLSM_EINVAL;
+  const int avail = H->n_mol - mol_begin;
+  if (avail == 0) return 0;
+  std::vector<int32_t> dims;
+  nolsm_status s = read_dims(ctx, H->row_ptr, mol_begin, avail, dims, (cudaStream_t)stream);
+  if (s != NOLSM_OK) return -(int32_t)s;
+  const size_t budget = (size_t)ctx->cfg.workspace_bytes / (size_t)n_slots;
+  int max_n = 0, count = 0;
+  for (int i = 0; i < avail; ++i) {
+    const int mn = std::max(max_n, dims[i]);
+    if (dense_bytes(i + 1, round_up(mn, NOLSM_PAD)) > budget) break;
+    max_n = mn;
+    count = i + 1;
+  }
+  return count;
+}
+
+extern "C" nolsm_status nolsm_build_submatrices(nolsm_ctx *ctx, const nolsm_bsr *H, const nolsm_bsr *S,
+                                                int32_t mol_begin, int32_t mol_count, int32_t slot,
+                                                nolsm_batch **out, void *stream) {
+  if (!ctx || !out) return NOLSM_EINVAL;
+  CHECK(check_bsr(ctx, H, "H"));
+  CHECK(check_bsr(ctx, S, "S"));
+  if (H->n_mol != S->n_mol || H->row_ptr != S->row_ptr || H->col_idx != S->col_idx) {
+    ctx->err = "H and S must share one pattern (row_ptr, col_idx)";
+    return NOLSM_EINVAL;
+  }
+  if (mol_begin < 0 || mol_count < 0 || mol_begin + mol_count > H->n_mol) {
+    ctx->err = "molecule range outside the matrix";
+    return NOLSM_EINVAL;
+  }
+  cudaStream_t st = (cudaStream_t)stream;
+  std::vector<int32_t> dims;
+  if (mol_count > 0) CHECK(read_dims(ctx, H->row_ptr, mol_begin, mol_count, dims, st));
+  nolsm_batch *b = nullptr;
+  CHECK(setup_batch(ctx, slot, dims, mol_begin, true, &b, st));
+  LAUNCH(ctx, launch_gather(b, H->row_ptr, H->col_idx, H->val, S->val, b->u[1], b->u[0], st));
+  *out = b;
+  return NOLSM_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Iteration drivers
+// ------------------------------------------------------------------------------------------------
+struct Engine {
+  nolsm_ctx *ctx;
+  nolsm_batch *b;
+  cudaStream_t st;
+  int64_t gemms = 0;
+
+  GemmParams base_params(bool simt) const {
+    GemmParams p;
+    memset(&p, 0, sizeof(p));
+    p.tiles = simt ? b->d_tiles_simt : b->d_tiles;
+    p.n_tiles = simt ? b->n_tiles_simt : b->n_tiles;
+    p.dims = b->d_dims;
+    p.ld = b->ld;
+    p.slab = (int64_t)b->ld * b->ld;
+    p.alpha = 1.f;
+    return p;
+  }
+  // C = I - A*B on the SIMT kernel (FP32 in, FP32 out)
+  nolsm_status simt(int mode, float alpha, float beta, const float *alpha_div, const float *a, const float *bb,
+                    const float *cin, float *cout, float *resid2, const int32_t *state, int iter) {
+    GemmParams p = base_params(true);
+    p.mode = mode; p.alpha = alpha; p.beta = beta; p.alpha_div = alpha_div;
+    p.a32 = a; p.b32 = bb; p.cin32 = cin; p.cout32 = cout; p.resid2 = resid2;
+    p.state = state; p.iter = iter;
+    LAUNCH(ctx, launch_gemm_simt(p, st));
+    gemms++;
+    return NOLSM_OK;
+  }
+  // tcgen05 product: operands are FP16 buffers h[ia], h[ib] (kind 2: plus h[ial], h[ibl])
+  nolsm_status umma(int kind, int mode, float alpha, float beta, int ia, int ib, int ial, int ibl,
+                    const float *cin, float *cout32, __half *cout16, __half *cout16_lo, float *resid2,
+                    const int32_t *state, int iter) {
+    GemmParams p = base_params(false);
+    p.mode = mode; p.alpha = alpha; p.beta = beta;
+    p.cin32 = cin; p.cout32 = cout32; p.cout16 = cout16; p.cout16_lo = cout16_lo; p.resid2 = resid2;
+    p.state = state; p.iter = iter;
+    cudaError_t e = launch_gemm_umma(ctx, b, kind, ia, ib, ial, ibl, p, st);
+    ctx->launches++;
+    if (e != cudaSuccess) {
+      ctx->err = std::string("tcgen05 product: ") + cudaGetErrorString(e) +
+                 (ctx->umma_ok ? "" : " (tcgen05 path not initialised: needs an sm_100 device)");
+      return NOLSM_ECUDA;
+    }
+    gemms++;
+    return NOLSM_OK;
+  }
+  float *resid_slot(int iter) const { return b->d_resid2 + (size_t)(iter % NOLSM_MAX_RESID_SLOTS) * b->count; }
+  nolsm_status zero_resid(int iter) {
+    NOLSM_CUDA(ctx, cudaMemsetAsync(resid_slot(iter), 0, sizeof(float) * b->count, st));
+    return NOLSM_OK;
+  }
+  nolsm_status control(int phase, int iter, float tol, int max_iter, int fixed_iter, bool lockstep) {
+    LAUNCH(ctx, launch_control(b, phase | (lockstep ? 16 : 0), iter, tol, max_iter, fixed_iter, st));
+    return NOLSM_OK;
+  }
+  // Lagged host check: after iteration k the active count is copied out; before launching iteration
+  // k+2 the host looks at it.  Returns true when iteration `k` left nobody active.
+  nolsm_status post_active(int k) {
+    NOLSM_CUDA(ctx, cudaMemcpyAsync(&ctx->h_active[k], &b->d_active[k], sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+    NOLSM_CUDA(ctx, cudaEventRecord(ctx->ev[k & 3], st));
+    return NOLSM_OK;
+  }
+  nolsm_status finished(int k, bool *done) {
+    NOLSM_CUDA(ctx, cudaEventSynchronize(ctx->ev[k & 3]));
+    *done = ctx->h_active[k] == 0;
+    return NOLSM_OK;
+  }
+};
+
+// Runs `body(k)` for k = 0.. until the control kernel reports nobody active (checked two iterations
+// late so the queue never drains) or max_iter.  Returns the number of iterations LAUNCHED; *executed
+// = iterations that did work (known only if `need_count`, which synchronises).
+template <typename Body>
+static nolsm_status iterate(Engine &E, int max_iter, int fixed_iter, bool need_count, int *executed, Body body) {
+  const int limit = fixed_iter > 0 ? std::min(fixed_iter, max_iter) : max_iter;
+  int k = 0;
+  for (; k < limit; ++k) {
+    if (fixed_iter <= 0 && k >= 2) {
+      bool done = false;
+      CHECK(E.finished(k - 2, &done));
+      if (done) break;
+    }
+    CHECK(body(k));
+    CHECK(E.post_active(k));
+  }
+  if (executed) {
+    *executed = k;
+    if (need_count) {
+      NOLSM_CUDA(E.ctx, cudaStreamSynchronize(E.st));
+      for (int i = 0; i < k; ++i)
+        if (E.ctx->h_active[i] == 0) { *executed = i + 1; break; }
+    }
+  }
+  return NOLSM_OK;
+}
+
+// a2 + a3 (first part): S^-1 by Eq. 15-17 and B = S^-1 H (Eq. 12).
+static nolsm_status prepare_batch(nolsm_ctx *ctx, nolsm_batch *b, int precision, cudaStream_t st,
+                                  nolsm_sign_stats *stats, int64_t *gemms) {
+  Engine E{ctx, b, st};
+  const bool fp16 = precision == NOLSM_FP16_FP32;
+  float inv_tol = ctx->cfg.inv_tol > 0.f ? ctx->cfg.inv_tol : (fp16 ? 1e-2f : 1e-5f);
+  const int max_it = ctx->cfg.inv_max_iter;
+  float *S = b->u[0], *H = b->u[1];
+  LAUNCH(ctx, launch_norm_bound(b, S, 0.f, b->d_norm, st));
+  CHECK(E.control(0, 0, 0.f, 0, 0, false));
+  int executed = 0;
+  if (fp16) {
+    float *Y32 = b->u[2], *Z32 = b->u[3];
+    LAUNCH(ctx, launch_init_inverse(b, S, b->d_norm, Y32, Z32, b->h[0], b->h[2], b->d_scale, st));
+    CHECK(iterate(E, max_it, 0, stats != nullptr, &executed, [&](int k) -> nolsm_status {
+      const int cur = k & 1, nxt = cur ^ 1;
+      CHECK(E.zero_resid(k));
+      // E = I - Z Y
+      CHECK(E.umma(1, EPI_IDENT, 1.f, 0.f, 2 + cur, cur, 0, 0, nullptr, nullptr, b->h[4], nullptr,
+                   E.resid_slot(k), b->d_state, k));
+      CHECK(E.control(1, k, inv_tol, max_it, 0, false));
+      // Y += 1/2 Y E ; Z += 1/2 E Z   (= Eq. 16 with 3I - V = 2I + E)
+      CHECK(E.umma(1, EPI_AXPBY, 0.5f, 1.f, cur, 4, 0, 0, Y32, Y32, b->h[nxt], nullptr, nullptr, b->d_state, k));
+      CHECK(E.umma(1, EPI_AXPBY, 0.5f, 1.f, 4, 2 + cur, 0, 0, Z32, Z32, b->h[2 + nxt], nullptr, nullptr,
+                   b->d_state, k));
+      return NOLSM_OK;
+    }));
+    // S^-1 = Z^2 / s_S (Eq. 17) from the FP32 masters, FP32-quality product
+    CHECK(E.simt(EPI_AXPBY, 1.f, 0.f, b->d_scale, Z32, Z32, nullptr, b->u[2], nullptr, nullptr, 0));
+    float *Sinv = b->u[2];
+    for (int it = 0; it < ctx->cfg.inv_refine; ++it) {
+      // Newton refinement S^-1 <- S^-1 + S^-1 (I - S S^-1): the residual at FP32 quality, the small
+      // correction on the tensor cores (reading 11)
+      CHECK(E.simt(EPI_IDENT, 1.f, 0.f, nullptr, S, Sinv, nullptr, b->u[3], nullptr, nullptr, 0));
+      LAUNCH(ctx, launch_scale_copy(b, Sinv, nullptr, 0, nullptr, b->h[0], nullptr, st));
+      LAUNCH(ctx, launch_scale_copy(b, b->u[3], nullptr, 0, nullptr, b->h[1], nullptr, st));
+      CHECK(E.umma(1, EPI_AXPBY, 1.f, 1.f, 0, 1, 0, 0, Sinv, Sinv, nullptr, nullptr, nullptr, nullptr, 0));
+    }
+    CHECK(E.simt(EPI_AXPBY, 1.f, 0.f, nullptr, Sinv, H, nullptr, b->u[3], nullptr, nullptr, 0));
+    b->x_parity = 0;
+  } else {
+    float *Y[2] = {b->u[2], b->u[5]}, *Z[2] = {b->u[3], b->u[6]}, *Em = b->u[4];
+    LAUNCH(ctx, launch_init_inverse(b, S, b->d_norm, Y[0], Z[0], nullptr, nullptr, b->d_scale, st));
+    CHECK(iterate(E, max_it, 0, true, &executed, [&](int k) -> nolsm_status {
+      const int cur = k & 1, nxt = cur ^ 1;
+      CHECK(E.zero_resid(k));
+      CHECK(E.simt(EPI_IDENT, 1.f, 0.f, nullptr, Z[cur], Y[cur], nullptr, Em, E.resid_slot(k), b->d_state, k));
+      CHECK(E.control(1, k, inv_tol, max_it, 0, true));
+      CHECK(E.simt(EPI_AXPBY, 0.5f, 1.f, nullptr, Y[cur], Em, Y[cur], Y[nxt], nullptr, b->d_state, k));
+      CHECK(E.simt(EPI_AXPBY, 0.5f, 1.f, nullptr, Em, Z[cur], Z[cur], Z[nxt], nullptr, b->d_state, k));
+      return NOLSM_OK;
+    }));
+    float *Zf = Z[executed & 1];
+    CHECK(E.simt(EPI_AXPBY, 1.f, 0.f, b->d_scale, Zf, Zf, nullptr, b->u[4], nullptr, nullptr, 0));
+    CHECK(E.simt(EPI_AXPBY, 1.f, 0.f, nullptr, b->u[4], H, nullptr, b->u[2], nullptr, nullptr, 0));
+  }
+  b->prepared = true;
+  b->prepared_precision = precision;
+  if (stats) {
+    stats->inv_iter_max = executed;
+    stats->flops_prepare = 2.0 * b->sum_n3 * (double)E.gemms;  // upper estimate: every product on every submatrix
+  }
+  *gemms += E.gemms;
+  return NOLSM_OK;
+}
+
+static float *sinv_ptr(const nolsm_batch *b) { return b->prepared_precision == NOLSM_FP16_FP32 ? b->u[2] : b->u[4]; }
+static float *bmat_ptr(const nolsm_batch *b) { return b->prepared_precision == NOLSM_FP16_FP32 ? b->u[3] : b->u[2]; }
+static float *x_ptr(const nolsm_batch *b) {
+  if (b->prepared_precision == NOLSM_FP16_FP32) return b->u[0];
+  return b->x_parity ? b->u[3] : b->u[0];
+}
+
+// a3 (second part) + a4: X0 = (B - mu I)/s, then Eq. 9-10 in the correction form
+// X_{k+1} = X_k + 1/2 X_k (I - X_k^2)  (reading 12), residual from the first product.
+static nolsm_status sign_batch(nolsm_ctx *ctx, nolsm_batch *b, double mu, int precision, float tol, int max_iter,
+                               int fixed_iter, const float *scale_in, cudaStream_t st, bool need_count,
+                               int64_t *gemms, int *launched) {
+  Engine E{ctx, b, st};
+  const bool fp16 = precision == NOLSM_FP16_FP32;
+  float *Bm = bmat_ptr(b);
+  if (!scale_in) LAUNCH(ctx, launch_norm_bound(b, Bm, (float)mu, b->d_norm, st));
+  CHECK(E.control(0, 0, 0.f, 0, 0, false));
+  int executed = 0;
+  if (fp16) {
+    float *X32 = b->u[0];
+    LAUNCH(ctx, launch_make_x0(b, Bm, (float)mu, b->d_norm, scale_in, X32, b->h[0], b->d_scale, st));
+    CHECK(iterate(E, max_iter, fixed_iter, need_count, &executed, [&](int k) -> nolsm_status {
+      const int cur = k & 1, nxt = cur ^ 1;
+      CHECK(E.zero_resid(k));
+      CHECK(E.umma(1, EPI_IDENT, 1.f, 0.f, cur, cur, 0, 0, nullptr, nullptr, b->h[4], nullptr, E.resid_slot(k),
+                   b->d_state, k));
+      CHECK(E.control(1, k, tol, max_iter, fixed_iter, false));
+      CHECK(E.umma(1, EPI_AXPBY, 0.5f, 1.f, cur, 4, 0, 0, X32, X32, b->h[nxt], nullptr, nullptr, b->d_state, k));
+      return NOLSM_OK;
+    }));
+  } else {
+    float *X[2] = {b->u[0], b->u[3]}, *Em = b->u[5];
+    LAUNCH(ctx, launch_make_x0(b, Bm, (float)mu, b->d_norm, scale_in, X[0], nullptr, b->d_scale, st));
+    CHECK(iterate(E, max_iter, fixed_iter, true, &executed, [&](int k) -> nolsm_status {
+      const int cur = k & 1, nxt = cur ^ 1;
+      CHECK(E.zero_resid(k));
+      CHECK(E.simt(EPI_IDENT, 1.f, 0.f, nullptr, X[cur], X[cur], nullptr, Em, E.resid_slot(k), b->d_state, k));
+      CHECK(E.control(1, k, tol, max_iter, fixed_iter, true));
+      CHECK(E.simt(EPI_AXPBY, 0.5f, 1.f, nullptr, X[cur], Em, X[cur], X[nxt], nullptr, b->d_state, k));
+      return NOLSM_OK;
+    }));
+    b->x_parity = executed & 1;
+  }
+  *gemms += E.gemms;
+  if (launched) *launched = executed;
+  return NOLSM_OK;
+}
+
+// Collect per-submatrix iteration counts and residuals (synchronises).
+static nolsm_status collect_stats(nolsm_ctx *ctx, nolsm_batch *b, float tol, int fixed_iter, cudaStream_t st,
+                                  nolsm_sign_stats *s) {
+  std::vector<int32_t> it(b->count);
+  std::vector<float> res(b->count);
+  NOLSM_CUDA(ctx, cudaMemcpyAsync(it.data(), b->d_iters, sizeof(int32_t) * b->count, cudaMemcpyDeviceToHost, st));
+  NOLSM_CUDA(ctx, cudaMemcpyAsync(res.data(), b->d_lastres, sizeof(float) * b->count, cudaMemcpyDeviceToHost, st));
+  NOLSM_CUDA(ctx, cudaStreamSynchronize(st));
+  s->n_sub = b->count;
+  s->iter_min = b->count ? 1 << 30 : 0;
+  s->iter_max = 0;
+  s->iter_sum = 0;
+  s->n_unconverged = 0;
+  s->worst_residual = 0.f;
+  s->flops_sign = s->flops_sign_padded = 0.0;
+  for (int m = 0; m < b->count; ++m) {
+    s->iter_min = std::min(s->iter_min, it[m]);
+    s->iter_max = std::max(s->iter_max, it[m]);
+    s->iter_sum += it[m];
+    if (!(res[m] < tol) && fixed_iter <= 0) s->n_unconverged++;
+    if (!(res[m] <= s->worst_residual)) s->worst_residual = res[m];
+    const double n = b->n_host[m], P = round_up(b->n_host[m], NOLSM_TILE_M), Pn = round_up(b->n_host[m], 64);
+    s->flops_sign += 2.0 * it[m] * 2.0 * n * n * n;
+    s->flops_sign_padded += 2.0 * it[m] * 2.0 * P * Pn * Pn;
+  }
+  return NOLSM_OK;
+}
+
+static void resolve_sign_args(const nolsm_ctx *ctx, int precision, float *tol, int *max_iter, int *fixed_iter) {
+  if (*tol <= 0.f) *tol = ctx->cfg.tol > 0.f ? ctx->cfg.tol : (precision == NOLSM_FP16_FP32 ? 1e-2f : 1e-5f);
+  if (*max_iter <= 0) *max_iter = ctx->cfg.max_iter;
+  if (*max_iter > NOLSM_MAX_RESID_SLOTS) *max_iter = NOLSM_MAX_RESID_SLOTS;
+  if (*fixed_iter < 0) *fixed_iter = ctx->cfg.fixed_iter;
+  if (*fixed_iter > *max_iter) *fixed_iter = *max_iter;
+}
+
+extern "C" nolsm_status nolsm_sign_batched(nolsm_ctx *ctx, nolsm_batch *batch, double mu, int32_t precision,
+                                           float tol, int32_t max_iter, int32_t fixed_iter,
+                                           nolsm_sign_stats *stats, void *stream) {
+  if (!ctx || !batch) return NOLSM_EINVAL;
+  cudaStream_t st = (cudaStream_t)stream;
+  const int prec = effective_precision(ctx, precision);
+  if (prec != NOLSM_FP16_FP32 && prec != NOLSM_FP32) { ctx->err = "bad precision"; return NOLSM_EINVAL; }
+  resolve_sign_args(ctx, prec, &tol, &max_iter, &fixed_iter);
+  if (stats) memset(stats, 0, sizeof(*stats));
+  int64_t gemms = 0;
+  if (!batch->prepared || batch->prepared_precision != prec) {
+    if (!batch->sparse) { ctx->err = "dense batch is not prepared"; return NOLSM_EINVAL; }
+    if (batch->prepared) { ctx->err = "batch was prepared in another precision; gather it again"; return NOLSM_EINVAL; }
+    CHECK(prepare_batch(ctx, batch, prec, st, stats, &gemms));
+    if (stats) {
+      std::vector<float> res(batch->count);
+      NOLSM_CUDA(ctx, cudaMemcpyAsync(res.data(), batch->d_lastres, sizeof(float) * batch->count,
+                                      cudaMemcpyDeviceToHost, st));
+      NOLSM_CUDA(ctx, cudaStreamSynchronize(st));
+      for (float r : res)
+        if (!(r <= stats->inv_worst_residual)) stats->inv_worst_residual = r;
+    }
+  }
+  CHECK(sign_batch(ctx, batch, mu, prec, tol, max_iter, fixed_iter, nullptr, st, stats != nullptr, &gemms, nullptr));
+  if (stats) {
+    const int inv_it = stats->inv_iter_max;
+    const float inv_res = stats->inv_worst_residual;
+    const double fp = stats->flops_prepare;
+    CHECK(collect_stats(ctx, batch, tol, fixed_iter, st, stats));
+    stats->inv_iter_max = inv_it;
+    stats->inv_worst_residual = inv_res;
+    stats->flops_prepare = fp;
+    stats->gemms = gemms;
+  }
+  return NOLSM_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// a5 - a7
+// ------------------------------------------------------------------------------------------------
+extern "C" nolsm_status nolsm_scatter_density(nolsm_ctx *ctx, const nolsm_batch *batch, const nolsm_bsr *S,
+                                              nolsm_bsr *D, double *ne_partial, double *q_mol, double *ne_diag,
+                                              void *stream) {
+  if (!ctx || !batch || !ne_partial) return NOLSM_EINVAL;
+  CHECK(check_bsr(ctx, S, "S"));
+  CHECK(check_bsr(ctx, D, "D"));
+  if (!batch->sparse || !batch->prepared) { ctx->err = "batch has no sign iterate (call nolsm_sign_batched first)"; return NOLSM_EINVAL; }
+  if (D->n_mol != S->n_mol || D->row_ptr != S->row_ptr || D->col_idx != S->col_idx) {
+    ctx->err = "D must share the pattern of S";
+    return NOLSM_EINVAL;
+  }
+  cudaStream_t st = (cudaStream_t)stream;
+  LAUNCH(ctx, launch_density(batch, x_ptr(batch), nullptr, sinv_ptr(batch), S->row_ptr, S->col_idx, D->val,
+                             ne_diag, st));
+  LAUNCH(ctx, launch_trace(batch, S->row_ptr, S->col_idx, D->val, S->val, ne_partial, q_mol, st));
+  return NOLSM_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Whole path with batching and bisection
+// ------------------------------------------------------------------------------------------------
+extern "C" nolsm_status nolsm_solve_mu(nolsm_ctx *ctx, const nolsm_bsr *H, const nolsm_bsr *S, double n_electrons,
+                                       double mu_lo, double mu_hi, double tol_ne_per_mol, int32_t max_steps,
+                                       int32_t precision, nolsm_bsr *D, double *mu_out, double *ne_out,
+                                       double *q_mol, nolsm_solve_stats *stats, void *stream) {
+  if (!ctx || !mu_out || !ne_out) return NOLSM_EINVAL;
+  CHECK(check_bsr(ctx, H, "H"));
+  CHECK(check_bsr(ctx, S, "S"));
+  CHECK(check_bsr(ctx, D, "D"));
+  if (!(mu_lo < mu_hi) || max_steps <= 0) { ctx->err = "need mu_lo < mu_hi and max_steps > 0"; return NOLSM_EINVAL; }
+  cudaStream_t st = (cudaStream_t)stream;
+  const int prec = effective_precision(ctx, precision);
+  float tol = 0.f;
+  int max_iter = 0, fixed_iter = -1;
+  resolve_sign_args(ctx, prec, &tol, &max_iter, &fixed_iter);
+  const int n_mol = H->n_mol;
+  if (stats) memset(stats, 0, sizeof(*stats));
+
+  // batching plan from the neighbour counts
+  std::vector<int32_t> dims;
+  if (n_mol > 0) CHECK(read_dims(ctx, H->row_ptr, 0, n_mol, dims, st));
+  struct Range { int begin, count; size_t bytes; };
+  std::vector<Range> plan;
+  auto make_plan = [&](size_t budget, int max_count) -> bool {
+    plan.clear();
+    int i = 0;
+    while (i < n_mol) {
+      int max_n = 0, cnt = 0;
+      while (i + cnt < n_mol && cnt < max_count) {
+        const int mn = std::max(max_n, dims[i + cnt]);
+        if (dense_bytes(cnt + 1, round_up(mn, NOLSM_PAD)) > budget) break;
+        max_n = mn;
+        cnt++;
+      }
+      if (cnt == 0) return false;
+      plan.push_back(Range{i, cnt, dense_bytes(cnt, round_up(max_n, NOLSM_PAD))});
+      i += cnt;
+    }
+    return true;
+  };
+  const size_t ws = (size_t)ctx->cfg.workspace_bytes;
+  const int max_count = 4096;
+  bool resident = false;
+  if (!make_plan(ws, max_count)) { ctx->err = "workspace_bytes cannot hold one submatrix"; return NOLSM_ENOMEM; }
+  {
+    size_t total = 0;
+    for (const Range &r : plan) total += r.bytes;
+    resident = total <= ws && plan.size() <= 64;
+  }
+  if (!resident) {
+    // streaming: one slot reused for every batch
+    for (size_t i = 1; i < ctx->slots.size(); ++i)
+      if (ctx->slots[i]) { free_batch(ctx->slots[i]); ctx->slots[i] = nullptr; }
+  }
+  std::vector<nolsm_batch *> live(plan.size(), nullptr);
+
+  cudaEvent_t tev[5];
+  for (int i = 0; i < 5; ++i) cudaEventCreate(&tev[i]);
+  auto cleanup = [&]() { for (int i = 0; i < 5; ++i) cudaEventDestroy(tev[i]); };
+
+  double lo = mu_lo, hi = mu_hi, mu = 0.5 * (lo + hi), ne = 0.0;
+  int step = 0;
+  nolsm_status rc = NOLSM_OK;
+  for (step = 0; step < max_steps; ++step) {
+    mu = 0.5 * (lo + hi);
+    if (cudaMemsetAsync(ctx->d_scalars, 0, 4 * sizeof(double), st) != cudaSuccess) { rc = NOLSM_ECUDA; break; }
+    nolsm_sign_stats acc;
+    memset(&acc, 0, sizeof(acc));
+    acc.iter_min = 1 << 30;
+    for (size_t bi = 0; bi < plan.size() && rc == NOLSM_OK; ++bi) {
+      const Range &r = plan[bi];
+      nolsm_batch *b = live[bi];
+      const bool timed = stats != nullptr;
+      if (timed) cudaEventRecord(tev[0], st);
+      if (!b || !resident) {
+        rc = nolsm_build_submatrices(ctx, H, S, r.begin, r.count, resident ? (int)bi : 0, &b, st);
+        if (rc != NOLSM_OK) break;
+        live[bi] = resident ? b : nullptr;
+      }
+      if (timed) cudaEventRecord(tev[1], st);
+      int64_t gemms = 0;
+      nolsm_sign_stats bs;
+      memset(&bs, 0, sizeof(bs));
+      if (!b->prepared) {
+        rc = prepare_batch(ctx, b, prec, st, stats ? &bs : nullptr, &gemms);
+        if (rc != NOLSM_OK) break;
+      }
+      if (timed) cudaEventRecord(tev[2], st);
+      rc = sign_batch(ctx, b, mu, prec, tol, max_iter, fixed_iter, nullptr, st, false, &gemms, nullptr);
+      if (rc != NOLSM_OK) break;
+      if (timed) cudaEventRecord(tev[3], st);
+      rc = nolsm_scatter_density(ctx, b, S, D, ctx->d_scalars, q_mol, ctx->d_scalars + 1, st);
+      if (rc != NOLSM_OK) break;
+      if (timed) {
+        cudaEventRecord(tev[4], st);
+        nolsm_sign_stats cs;
+        memset(&cs, 0, sizeof(cs));
+        rc = collect_stats(ctx, b, tol, fixed_iter, st, &cs);   // synchronises
+        if (rc != NOLSM_OK) break;
+        float ms[4];
+        for (int i = 0; i < 4; ++i) cudaEventElapsedTime(&ms[i], tev[i], tev[i + 1]);
+        stats->ms_gather += ms[0]; stats->ms_prepare += ms[1]; stats->ms_sign += ms[2]; stats->ms_density += ms[3];
+        acc.n_sub += cs.n_sub;
+        acc.iter_min = std::min(acc.iter_min, cs.iter_min);
+        acc.iter_max = std::max(acc.iter_max, cs.iter_max);
+        acc.iter_sum += cs.iter_sum;
+        acc.n_unconverged += cs.n_unconverged;
+        acc.worst_residual = std::max(acc.worst_residual, cs.worst_residual);
+        acc.flops_sign += cs.flops_sign;
+        acc.flops_sign_padded += cs.flops_sign_padded;
+        acc.flops_prepare += bs.flops_prepare;
+        acc.inv_iter_max = std::max(acc.inv_iter_max, bs.inv_iter_max);
+        acc.gemms += gemms;
+      }
+    }
+    if (rc != NOLSM_OK) break;
+    if (cudaMemcpyAsync(ctx->h_scalars, ctx->d_scalars, 4 * sizeof(double), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+        cudaStreamSynchronize(st) != cudaSuccess) {
+      ctx->err = std::string("solve_mu: ") + cudaGetErrorString(cudaGetLastError());
+      rc = NOLSM_ECUDA;
+      break;
+    }
+    ne = ctx->h_scalars[0];
+    if (stats) {
+      stats->last = acc;
+      stats->ne_diag = ctx->h_scalars[1];
+      stats->flops_sign_total += acc.flops_sign;
+      stats->flops_prepare_total += acc.flops_prepare;
+      stats->mu_steps = step + 1;
+    }
+    if (!(ne == ne)) { ctx->err = "N(mu) is NaN"; rc = NOLSM_ENOCONV; break; }
+    if (tol_ne_per_mol >= 0.0 && std::fabs(ne - n_electrons) <= tol_ne_per_mol * (double)n_mol) { step++; break; }
+    if (step + 1 < max_steps) {
+      if (ne > n_electrons) hi = mu; else lo = mu;
+    }
+  }
+  cleanup();
+  *mu_out = mu;
+  *ne_out = ne;
+  if (stats) {
+    stats->n_batches = (int)plan.size();
+    stats->resident = resident ? 1 : 0;
+    stats->mu_lo = lo;
+    stats->mu_hi = hi;
+    if (rc == NOLSM_OK && stats->last.n_unconverged > 0 && fixed_iter <= 0) {
+      ctx->err = "sign iteration hit max_iter on the final mu";
+      rc = NOLSM_ENOCONV;
+    }
+  }
+  return rc;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Dense microbench entry and the GEMM test entry
+// ------------------------------------------------------------------------------------------------
+extern "C" nolsm_status nolsm_sign_dense_batched(nolsm_ctx *ctx, const float *a, const float *scale, int32_t n,
+                                                 int32_t batch, int32_t precision, float tol, int32_t max_iter,
+                                                 int32_t fixed_iter, float *x_out, nolsm_sign_stats *stats,
+                                                 void *stream) {
+  if (!ctx || !a || !x_out || n <= 0 || batch < 0) return NOLSM_EINVAL;
+  cudaStream_t st = (cudaStream_t)stream;
+  const int prec = effective_precision(ctx, precision);
+  resolve_sign_args(ctx, prec, &tol, &max_iter, &fixed_iter);
+  if (stats) memset(stats, 0, sizeof(*stats));
+  if (batch == 0) return NOLSM_OK;
+  std::vector<int32_t> dims(batch, n);
+  nolsm_batch *b = nullptr;
+  CHECK(setup_batch(ctx, 0, dims, 0, false, &b, st));
+  b->prepared = true;
+  b->prepared_precision = prec;
+  LAUNCH(ctx, launch_pack(a, n, batch, b->ld, bmat_ptr(b), 0, st));
+  int64_t gemms = 0;
+  CHECK(sign_batch(ctx, b, 0.0, prec, tol, max_iter, fixed_iter, scale, st, stats != nullptr, &gemms, nullptr));
+  LAUNCH(ctx, launch_unpack(x_ptr(b), b->ld, (int64_t)b->ld * b->ld, nullptr, nullptr, n, batch, x_out, st));
+  if (stats) {
+    CHECK(collect_stats(ctx, b, tol, fixed_iter, st, stats));
+    stats->gemms = gemms;
+  }
+  return NOLSM_OK;
+}
+
+extern "C" nolsm_status nolsm_batch_read(nolsm_ctx *ctx, const nolsm_batch *b, int32_t local, int32_t which,
+                                         float *dst, int64_t dst_elems, int32_t *n_out, void *stream) {
+  if (!ctx || !b || !dst || local < 0 || local >= b->count) return NOLSM_EINVAL;
+  const int n = b->n_host[local];
+  if (n_out) *n_out = n;
+  if (dst_elems < (int64_t)n * n) { ctx->err = "dst too small"; return NOLSM_ENOMEM; }
+  const float *src = nullptr;
+  switch (which) {
+    case NOLSM_MAT_S: src = b->u[0]; break;
+    case NOLSM_MAT_H: src = b->u[1]; break;
+    case NOLSM_MAT_SINV: src = b->prepared ? sinv_ptr(b) : nullptr; break;
+    case NOLSM_MAT_B: src = b->prepared ? bmat_ptr(b) : nullptr; break;
+    case NOLSM_MAT_X: src = b->prepared ? x_ptr(b) : nullptr; break;
+    default: break;
+  }
+  if (!src) { ctx->err = "matrix not available in this batch state"; return NOLSM_EINVAL; }
+  cudaStream_t st = (cudaStream_t)stream;
+  const int64_t slab = (int64_t)b->ld * b->ld;
+  LAUNCH(ctx, launch_unpack(src + (int64_t)local * slab, b->ld, slab, nullptr, nullptr, n, 1, dst, st));
+  NOLSM_CUDA(ctx, cudaStreamSynchronize(st));
+  return NOLSM_OK;
+}
+
+extern "C" nolsm_status nolsm_gemm_batched(nolsm_ctx *ctx, int32_t kind, int32_t ident, float alpha, float beta,
+                                           const float *a, const float *bm, const float *cin, float *c,
+                                           float *resid2, int32_t n, int32_t batch, void *stream) {
+  if (!ctx || !a || !bm || !c || n <= 0 || batch <= 0 || kind < 0 || kind > 2) return NOLSM_EINVAL;
+  if (!ident && beta != 0.f && !cin) return NOLSM_EINVAL;
+  cudaStream_t st = (cudaStream_t)stream;
+  std::vector<int32_t> dims(batch, n);
+  nolsm_batch *b = nullptr;
+  CHECK(setup_batch(ctx, 0, dims, 0, false, &b, st));
+  Engine E{ctx, b, st};
+  // unit padding in A and B keeps the padded rows/columns decoupled, like the iterates of the path
+  LAUNCH(ctx, launch_pack(a, n, batch, b->ld, b->u[0], 1, st));
+  LAUNCH(ctx, launch_pack(bm, n, batch, b->ld, b->u[1], 1, st));
+  if (!ident && beta != 0.f) LAUNCH(ctx, launch_pack(cin, n, batch, b->ld, b->u[2], 0, st));
+  CHECK(E.zero_resid(0));
+  const int mode = ident ? EPI_IDENT : EPI_AXPBY;
+  if (kind == 0) {
+    CHECK(E.simt(mode, alpha, beta, nullptr, b->u[0], b->u[1], b->u[2], b->u[3], E.resid_slot(0), nullptr, 0));
+  } else {
+    LAUNCH(ctx, launch_scale_copy(b, b->u[0], nullptr, 0, nullptr, b->h[0], kind == 2 ? b->h[2] : nullptr, st));
+    LAUNCH(ctx, launch_scale_copy(b, b->u[1], nullptr, 0, nullptr, b->h[1], kind == 2 ? b->h[3] : nullptr, st));
+    CHECK(E.umma(kind, mode, alpha, beta, 0, 1, 2, 3, b->u[2], b->u[3], nullptr, nullptr, E.resid_slot(0), nullptr, 0));
+  }
+  LAUNCH(ctx, launch_unpack(b->u[3], b->ld, (int64_t)b->ld * b->ld, nullptr, nullptr, n, batch, c, st));
+  if (resid2 && ident)
+    NOLSM_CUDA(ctx, cudaMemcpyAsync(resid2, E.resid_slot(0), sizeof(float) * batch, cudaMemcpyDeviceToDevice, st));
+  return NOLSM_OK;
+}

@@ -1,0 +1,146 @@
+// Internal declarations shared by the translation units of libnolsm (not part of the C ABI).
+// Storage convention for every dense submatrix buffer: COLUMN-major with leading dimension ld
+// (element (r,c) at c*ld + r), one slab of ld*ld elements per submatrix, slabs of one logical buffer
+// contiguous over the batch.  Column-major is what the tcgen05 epilogue writes coalesced (TMEM lane
+// = row), and it makes the A operand M-major and the B operand K-major.
+#pragma once
+#include <cuda_runtime.h>
+#include <cuda_fp16.h>
+#include <cuda.h>
+#include <stdint.h>
+#include <string>
+#include <vector>
+#include "../../include/nolsm.h"
+
+#define NOLSM_BS 6
+#define NOLSM_TILE_M 128          // rows per output tile (UMMA M, one CTA)
+#define NOLSM_PAD 128             // leading dimensions are multiples of this
+#define NOLSM_MAX_RESID_SLOTS 64  // residual history kept per submatrix
+
+struct TileDesc {                 // one output tile of one submatrix
+  int32_t mat;                    // index inside the batch
+  int32_t m0, n0;                 // first row / column
+  int32_t nt;                     // columns in this tile (multiple of 64, <= BN)
+};
+
+enum { EPI_AXPBY = 0, EPI_IDENT = 1 };
+
+// Parameters of one batched product  C = epilogue(A * B)  over a tile list.
+struct GemmParams {
+  const TileDesc *tiles;
+  int32_t n_tiles;
+  const int32_t *dims;            // true dimension n_j per submatrix
+  const int32_t *state;           // per submatrix: last iteration index it executes (may be null)
+  int32_t iter;                   // tile runs iff state==null or iter <= state[m]
+  int32_t ld;
+  int64_t slab;                   // ld*ld
+  int32_t mode;                   // EPI_*
+  float alpha, beta;
+  const float *alpha_div;         // optional per-submatrix divisor of alpha (S^-1 = Z^2 / s_S)
+  const float *a32, *b32;         // SIMT operands
+  const float *cin32;             // AXPBY input (may alias cout32)
+  float *cout32;                  // FP32 output (may be null in IDENT mode of the FP16 path)
+  __half *cout16;                 // FP16 copy of the output (tcgen05 path; may be null)
+  __half *cout16_lo;              // split path: residual part, scaled by 2^11 (may be null)
+  float *resid2;                  // IDENT: per-submatrix sum of squares of the output (atomicAdd)
+};
+
+struct nolsm_batch {
+  int32_t count = 0, ld = 0, mol_begin = 0, max_n = 0, slot = 0;
+  int32_t bn = 128;               // tile width of the tcgen05 path for this batch
+  bool sparse = true;             // false: dense microbench batch (no neighbour list)
+  bool prepared = false;          // S^-1 and B available
+  int32_t prepared_precision = -1;
+  int32_t x_parity = 0;           // FP32 mode: which ping-pong buffer holds X per submatrix -> d_iters parity
+  std::vector<int32_t> n_host;
+  // device
+  void *base = nullptr;           // dense workspace of this slot
+  size_t base_bytes = 0;
+  int32_t *d_dims = nullptr;      // [count]
+  int32_t *d_state = nullptr;     // [count]
+  int32_t *d_iters = nullptr;     // [count]
+  float *d_resid2 = nullptr;      // [NOLSM_MAX_RESID_SLOTS][count]
+  float *d_lastres = nullptr;     // [count]
+  float *d_scale = nullptr;       // [count] s_j of the sign scaling
+  float *d_norm = nullptr;        // [2][count] scratch for norm bounds
+  int32_t *d_active = nullptr;    // [NOLSM_MAX_RESID_SLOTS] active counters per iteration
+  TileDesc *d_tiles = nullptr;    // tile list (bn-wide tiles)
+  int32_t n_tiles = 0;
+  TileDesc *d_tiles_simt = nullptr; // 128x128 tiles for the SIMT kernel
+  int32_t n_tiles_simt = 0;
+  size_t meta_cap = 0;            // capacity (in submatrices) of the metadata arrays
+  size_t tiles_cap = 0, tiles_simt_cap = 0;
+  double sum_n3 = 0.0, sum_n3_padded = 0.0;
+  // logical buffers (set by layout_batch): fp32 units u[0..6], fp16 halves h[0..5] alias units 4..6
+  float *u[7] = {nullptr};
+  __half *h[6] = {nullptr};
+  CUtensorMap map_a[6], map_b[6]; // per fp16 buffer: A-role box {64,64,1}, B-role box {64,bn,1}
+  bool maps_valid = false;
+};
+
+struct nolsm_ctx {
+  nolsm_config cfg;
+  int device = 0;
+  int sm_count = 148;
+  size_t l2_bytes = 0;
+  std::string err;
+  std::vector<nolsm_batch *> slots;
+  int64_t launches = 0;
+  double *d_scalars = nullptr;    // [4] device doubles: ne, ne_diag, spare
+  double *h_scalars = nullptr;    // pinned mirror
+  int32_t *h_active = nullptr;    // pinned [NOLSM_MAX_RESID_SLOTS]
+  cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+  void *encode_tiled = nullptr;   // cuTensorMapEncodeTiled entry point
+  bool umma_ok = false;
+};
+
+#define NOLSM_CUDA(ctx, call)                                                          \
+  do {                                                                                 \
+    cudaError_t e__ = (call);                                                          \
+    if (e__ != cudaSuccess) {                                                          \
+      (ctx)->err = std::string(#call) + ": " + cudaGetErrorString(e__);                \
+      return NOLSM_ECUDA;                                                              \
+    }                                                                                  \
+  } while (0)
+
+static inline int32_t round_up(int32_t x, int32_t g) { return (x + g - 1) / g * g; }
+
+// ---- launchers implemented in the kernel translation units (all asynchronous on `st`) ----
+// sparse side
+cudaError_t launch_neighbour_count(int n_mol, const int32_t *pos, const int32_t *box, int32_t rc,
+                                   int32_t *counts, cudaStream_t st);
+cudaError_t launch_exclusive_scan(const int32_t *counts, int32_t *row_ptr, int n, cudaStream_t st);
+cudaError_t launch_neighbour_fill(int n_mol, const int32_t *pos, const int32_t *box, int32_t rc,
+                                  const int32_t *row_ptr, int32_t *col_idx, cudaStream_t st);
+cudaError_t launch_gather(const nolsm_batch *b, const int32_t *row_ptr, const int32_t *col_idx,
+                          const float *h_val, const float *s_val, float *h_out, float *s_out,
+                          cudaStream_t st);
+cudaError_t launch_density(const nolsm_batch *b, const float *x, const float *x_alt, const float *sinv,
+                           const int32_t *row_ptr, const int32_t *col_idx, float *d_val,
+                           double *ne_diag, cudaStream_t st);
+cudaError_t launch_trace(const nolsm_batch *b, const int32_t *row_ptr, const int32_t *col_idx,
+                         const float *d_val, const float *s_val, double *ne, double *q_mol,
+                         cudaStream_t st);
+// dense helpers
+cudaError_t launch_norm_bound(const nolsm_batch *b, const float *a, float mu, float *norm2,
+                              cudaStream_t st);
+cudaError_t launch_init_inverse(const nolsm_batch *b, const float *s, const float *norm2, float *y32,
+                                float *z32, __half *y16, __half *z16, float *scale_out, cudaStream_t st);
+cudaError_t launch_make_x0(const nolsm_batch *b, const float *bmat, float mu, const float *norm2,
+                           const float *scale_in, float *x32, __half *x16, float *scale_out,
+                           cudaStream_t st);
+cudaError_t launch_scale_copy(const nolsm_batch *b, const float *src, const float *scale, int invert,
+                              float *dst32, __half *dst16, __half *dst16_lo, cudaStream_t st);
+cudaError_t launch_control(const nolsm_batch *b, int phase, int iter, float tol, int max_iter,
+                           int fixed_iter, cudaStream_t st);
+cudaError_t launch_pack(const float *src_rowmajor, int n, int batch, int ld, float *dst, int pad_identity,
+                        cudaStream_t st);
+cudaError_t launch_unpack(const float *src, int ld, int64_t slab, const int32_t *iters_parity,
+                          const float *src_alt, int n, int batch, float *dst_rowmajor, cudaStream_t st);
+cudaError_t launch_gemm_simt(const GemmParams &p, cudaStream_t st);
+// tcgen05 path
+nolsm_status umma_init(nolsm_ctx *ctx);
+nolsm_status umma_make_maps(nolsm_ctx *ctx, nolsm_batch *b);
+// kind: 1 = FP16 operands; 2 = split FP16 (hi/lo operands, FP32-quality)
+cudaError_t launch_gemm_umma(nolsm_ctx *ctx, const nolsm_batch *b, int kind, int a_buf, int b_buf,
+                             int a_lo_buf, int b_lo_buf, const GemmParams &p, cudaStream_t st);

@@ -1,0 +1,401 @@
+// O(n^2) helpers around the batched products (norm bounds, scalings, iterate initialisation,
+// iteration control, layout conversion) and the FP32 SIMT product used for FP32-quality steps.
+// Every dense buffer is column-major with leading dimension ld (see common.cuh).
+#include "common.cuh"
+
+__device__ __forceinline__ int padded_dim(int n) { return (n + NOLSM_TILE_M - 1) / NOLSM_TILE_M * NOLSM_TILE_M; }
+
+__device__ __forceinline__ void atomic_max_nonneg(float *addr, float v) {
+  atomicMax(reinterpret_cast<int *>(addr), __float_as_int(v));  // valid for v >= 0
+}
+
+// ------------------------------------------------------------------------------------------------
+// Upper bound on the spectral radius: rho(A) <= ||A||_2 <= sqrt(||A||_1 ||A||_inf), A = M - mu I
+// (rescaling "prior to the sign iteration"; readings 5 and 7).
+// norm2[0][m] = ||A||_inf (max abs row sum), norm2[1][m] = ||A||_1 (max abs column sum).
+// Block = 128 rows (thread per row, coalesced over the column-major storage) + the same 128 columns
+// (warp per column, lanes along rows).
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128)
+k_norm_bound(const int32_t *__restrict__ dims, int ld, int64_t slab, int count,
+             const float *__restrict__ a, float mu, float *__restrict__ norm2) {
+  const int mat = blockIdx.y;
+  const int n = dims[mat];
+  const int base = blockIdx.x * 128;
+  if (base >= n) return;
+  const float *aj = a + (int64_t)mat * slab;
+  const int r = base + threadIdx.x;
+  float rs = 0.f;
+  if (r < n) {
+    for (int c = 0; c < n; ++c) {
+      float v = aj[(int64_t)c * ld + r];
+      if (c == r) v -= mu;
+      rs += fabsf(v);
+    }
+  }
+  for (int d = 16; d > 0; d >>= 1) rs = fmaxf(rs, __shfl_xor_sync(0xffffffffu, rs, d));
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  if (lane == 0) atomic_max_nonneg(&norm2[mat], rs);
+  float cmax = 0.f;
+  for (int c = base + warp; c < min(n, base + 128); c += 4) {
+    float cs = 0.f;
+    for (int rr = lane; rr < n; rr += 32) {
+      float v = aj[(int64_t)c * ld + rr];
+      if (rr == c) v -= mu;
+      cs += fabsf(v);
+    }
+    for (int d = 16; d > 0; d >>= 1) cs += __shfl_xor_sync(0xffffffffu, cs, d);
+    cmax = fmaxf(cmax, cs);
+  }
+  if (lane == 0) atomic_max_nonneg(&norm2[count + mat], cmax);
+}
+
+cudaError_t launch_norm_bound(const nolsm_batch *b, const float *a, float mu, float *norm2,
+                              cudaStream_t st) {
+  if (b->count == 0) return cudaSuccess;
+  cudaError_t e = cudaMemsetAsync(norm2, 0, sizeof(float) * 2 * b->count, st);
+  if (e != cudaSuccess) return e;
+  dim3 grid((b->max_n + 127) / 128, b->count);
+  k_norm_bound<<<grid, 128, 0, st>>>(b->d_dims, b->ld, (int64_t)b->ld * b->ld, b->count, a, mu, norm2);
+  return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------
+// Eq. 15: Y0 = T_j(S)/s_S, Z0 = I with s_S = sqrt(||S||_1 ||S||_inf) >= lambda_max(S)
+// (reading 7).  The padded part of S is the identity, so Y0 there is 1/s_S.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+k_init_inverse(const int32_t *__restrict__ dims, int ld, int64_t slab, int count,
+               const float *__restrict__ s, const float *__restrict__ norm2, float *__restrict__ y32,
+               float *__restrict__ z32, __half *__restrict__ y16, __half *__restrict__ z16,
+               float *__restrict__ scale_out) {
+  const int mat = blockIdx.z;
+  const int n = dims[mat];
+  const int P = padded_dim(n);
+  const int c = blockIdx.y;
+  const int r = blockIdx.x * 256 + threadIdx.x;
+  if (c >= P || r >= P) return;
+  const float sc = fmaxf(1.f, sqrtf(norm2[mat] * norm2[count + mat]));  // >= 1 covers the unit padding
+  if (r == 0 && c == 0) scale_out[mat] = sc;
+  const int64_t off = (int64_t)mat * slab + (int64_t)c * ld + r;
+  const float y = s[off] / sc;
+  const float z = (r == c) ? 1.f : 0.f;
+  if (y32) { y32[off] = y; z32[off] = z; }
+  if (y16) { y16[off] = __float2half_rn(y); z16[off] = __float2half_rn(z); }
+}
+
+cudaError_t launch_init_inverse(const nolsm_batch *b, const float *s, const float *norm2, float *y32,
+                                float *z32, __half *y16, __half *z16, float *scale_out, cudaStream_t st) {
+  if (b->count == 0) return cudaSuccess;
+  const int P = round_up(b->max_n, NOLSM_TILE_M);
+  dim3 grid((P + 255) / 256, P, b->count);
+  k_init_inverse<<<grid, 256, 0, st>>>(b->d_dims, b->ld, (int64_t)b->ld * b->ld, b->count, s, norm2,
+                                       y32, z32, y16, z16, scale_out);
+  return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------
+// X0 = (B - mu I)/s  (Eq. 9 with the rescaling of PAPER.md:138), s from the norm bound or from the
+// caller (scale_in, dense microbench).  Padded diagonal = 1: a fixed point of the iteration that adds
+// nothing to the residual (reading 19).
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+k_make_x0(const int32_t *__restrict__ dims, int ld, int64_t slab, int count,
+          const float *__restrict__ bmat, float mu, const float *__restrict__ norm2,
+          const float *__restrict__ scale_in, float *__restrict__ x32, __half *__restrict__ x16,
+          float *__restrict__ scale_out) {
+  const int mat = blockIdx.z;
+  const int n = dims[mat];
+  const int P = padded_dim(n);
+  const int c = blockIdx.y;
+  const int r = blockIdx.x * 256 + threadIdx.x;
+  if (c >= P || r >= P) return;
+  float sc = scale_in ? scale_in[mat] : sqrtf(norm2[mat] * norm2[count + mat]);
+  sc = fmaxf(sc, 1e-30f);
+  if (r == 0 && c == 0 && scale_out) scale_out[mat] = sc;
+  const int64_t off = (int64_t)mat * slab + (int64_t)c * ld + r;
+  float v;
+  if (r < n && c < n) {
+    v = bmat[off];
+    if (r == c) v -= mu;
+    v /= sc;
+  } else {
+    v = (r == c) ? 1.f : 0.f;
+  }
+  if (x32) x32[off] = v;
+  if (x16) x16[off] = __float2half_rn(v);
+}
+
+cudaError_t launch_make_x0(const nolsm_batch *b, const float *bmat, float mu, const float *norm2,
+                           const float *scale_in, float *x32, __half *x16, float *scale_out,
+                           cudaStream_t st) {
+  if (b->count == 0) return cudaSuccess;
+  const int P = round_up(b->max_n, NOLSM_TILE_M);
+  dim3 grid((P + 255) / 256, P, b->count);
+  k_make_x0<<<grid, 256, 0, st>>>(b->d_dims, b->ld, (int64_t)b->ld * b->ld, b->count, bmat, mu, norm2,
+                                  scale_in, x32, x16, scale_out);
+  return cudaGetLastError();
+}
+
+// dst = src * f (f = scale[m], 1/scale[m] or 1), FP32 and/or FP16 (hi [+ lo*2^11]) copies over the
+// padded extent.  Used to hand FP32 results to the tensor-core path.
+__global__ void __launch_bounds__(256)
+k_scale_copy(const int32_t *__restrict__ dims, int ld, int64_t slab, const float *__restrict__ src,
+             const float *__restrict__ scale, int invert, float *__restrict__ dst32,
+             __half *__restrict__ dst16, __half *__restrict__ dst16_lo) {
+  const int mat = blockIdx.z;
+  const int P = padded_dim(dims[mat]);
+  const int c = blockIdx.y;
+  const int r = blockIdx.x * 256 + threadIdx.x;
+  if (c >= P || r >= P) return;
+  float f = 1.f;
+  if (scale) f = invert ? 1.f / scale[mat] : scale[mat];
+  const int64_t off = (int64_t)mat * slab + (int64_t)c * ld + r;
+  const float v = src[off] * f;
+  if (dst32) dst32[off] = v;
+  if (dst16) {
+    const __half hi = __float2half_rn(v);
+    dst16[off] = hi;
+    if (dst16_lo) dst16_lo[off] = __float2half_rn((v - __half2float(hi)) * 2048.f);
+  }
+}
+
+cudaError_t launch_scale_copy(const nolsm_batch *b, const float *src, const float *scale, int invert,
+                              float *dst32, __half *dst16, __half *dst16_lo, cudaStream_t st) {
+  if (b->count == 0) return cudaSuccess;
+  const int P = round_up(b->max_n, NOLSM_TILE_M);
+  dim3 grid((P + 255) / 256, P, b->count);
+  k_scale_copy<<<grid, 256, 0, st>>>(b->d_dims, b->ld, (int64_t)b->ld * b->ld, src, scale, invert,
+                                     dst32, dst16, dst16_lo);
+  return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------
+// Iteration control (stop rule, reading 9).  state[m] holds the LAST iteration index the
+// submatrix executes (INT_MAX while undecided); a product of iteration k runs for m iff k <= state[m].
+// After the first product of iteration k (which produced the residual) this kernel decides:
+// r_k < tol (or the fixed count / the cap reached) -> iteration k is finished and is the last one.
+// lockstep: everybody stops together once the slowest has met the test (FP32 ping-pong buffers).
+// phase 0 = reset for a new iteration sequence.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+k_control(int count, const int32_t *__restrict__ dims, int32_t *__restrict__ state,
+          int32_t *__restrict__ iters, const float *__restrict__ resid2, float *__restrict__ lastres,
+          int32_t *__restrict__ active, int phase, int iter, float tol, int max_iter, int fixed_iter,
+          int lockstep) {
+  __shared__ int s_cnt;
+  if (threadIdx.x == 0) s_cnt = 0;
+  __syncthreads();
+  if (phase == 0) {
+    for (int m = threadIdx.x; m < count; m += blockDim.x) {
+      state[m] = 0x7fffffff;
+      iters[m] = 0;
+      lastres[m] = -1.f;
+    }
+    return;
+  }
+  int mine = 0;
+  for (int m = threadIdx.x; m < count; m += blockDim.x) {
+    if (iter <= state[m]) {
+      const float r = sqrtf(fmaxf(resid2[m], 0.f) / (float)dims[m]);
+      lastres[m] = r;
+      iters[m] = iter + 1;
+      bool stop;
+      if (fixed_iter > 0) stop = (iter + 1 >= fixed_iter);
+      else stop = (r < tol) || !(r == r);
+      if (iter + 1 >= max_iter) stop = true;
+      if (!stop) mine++;
+      else if (!lockstep) state[m] = iter;
+    }
+  }
+  atomicAdd(&s_cnt, mine);
+  __syncthreads();
+  const int total = s_cnt;
+  if (lockstep && total == 0) {
+    for (int m = threadIdx.x; m < count; m += blockDim.x)
+      if (iter <= state[m]) state[m] = iter;
+  }
+  if (threadIdx.x == 0) active[iter] = total;
+}
+
+cudaError_t launch_control(const nolsm_batch *b, int phase, int iter, float tol, int max_iter,
+                           int fixed_iter, cudaStream_t st) {
+  if (b->count == 0) return cudaSuccess;
+  const int lockstep = phase >> 4;
+  k_control<<<1, 256, 0, st>>>(b->count, b->d_dims, b->d_state, b->d_iters,
+                               b->d_resid2 + (size_t)(iter % NOLSM_MAX_RESID_SLOTS) * b->count,
+                               b->d_lastres, b->d_active, phase & 15, iter, tol, max_iter, fixed_iter,
+                               lockstep);
+  return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------
+// Layout conversion between the caller's row-major n x n matrices and the padded column-major slabs
+// (dense microbench entry, test entry, nolsm_batch_read).  32x32 shared-memory transpose.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+k_pack(const float *__restrict__ src, int n, int ld, int64_t slab, float *__restrict__ dst, int P,
+       int pad_identity) {
+  __shared__ float t[32][33];
+  const int mat = blockIdx.z;
+  const float *s = src + (int64_t)mat * n * n;
+  float *d = dst + (int64_t)mat * slab;
+  const int r0 = blockIdx.y * 32, c0 = blockIdx.x * 32;
+  const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+  for (int i = ty; i < 32; i += 8) {
+    const int r = r0 + i, c = c0 + tx;
+    float v = 0.f;
+    if (r < n && c < n) v = s[(int64_t)r * n + c];
+    else if (pad_identity && r == c) v = 1.f;
+    t[i][tx] = v;
+  }
+  __syncthreads();
+  for (int i = ty; i < 32; i += 8) {
+    const int c = c0 + i, r = r0 + tx;
+    if (r < P && c < P) d[(int64_t)c * ld + r] = t[tx][i];
+  }
+}
+
+cudaError_t launch_pack(const float *src_rowmajor, int n, int batch, int ld, float *dst, int pad_identity,
+                        cudaStream_t st) {
+  if (batch == 0) return cudaSuccess;
+  const int P = round_up(n, NOLSM_TILE_M);
+  dim3 grid((P + 31) / 32, (P + 31) / 32, batch);
+  k_pack<<<grid, 256, 0, st>>>(src_rowmajor, n, ld, (int64_t)ld * ld, dst, P, pad_identity);
+  return cudaGetLastError();
+}
+
+__global__ void __launch_bounds__(256)
+k_unpack(const float *__restrict__ src, const float *__restrict__ src_alt,
+         const int32_t *__restrict__ parity, int ld, int64_t slab, int n, float *__restrict__ dst) {
+  __shared__ float t[32][33];
+  const int mat = blockIdx.z;
+  const float *s = ((src_alt && parity && (parity[mat] & 1)) ? src_alt : src) + (int64_t)mat * slab;
+  float *d = dst + (int64_t)mat * n * n;
+  const int r0 = blockIdx.y * 32, c0 = blockIdx.x * 32;
+  const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+  for (int i = ty; i < 32; i += 8) {
+    const int c = c0 + i, r = r0 + tx;
+    t[i][tx] = (r < n && c < n) ? s[(int64_t)c * ld + r] : 0.f;
+  }
+  __syncthreads();
+  for (int i = ty; i < 32; i += 8) {
+    const int r = r0 + i, c = c0 + tx;
+    if (r < n && c < n) d[(int64_t)r * n + c] = t[tx][i];
+  }
+}
+
+cudaError_t launch_unpack(const float *src, int ld, int64_t slab, const int32_t *iters_parity,
+                          const float *src_alt, int n, int batch, float *dst_rowmajor, cudaStream_t st) {
+  if (batch == 0) return cudaSuccess;
+  dim3 grid((n + 31) / 32, (n + 31) / 32, batch);
+  k_unpack<<<grid, 256, 0, st>>>(src, src_alt, iters_parity, ld, slab, n, dst_rowmajor);
+  return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------
+// FP32 SIMT batched product with the engine's epilogues: 128x128 tile, 256 threads, 8x8 per thread,
+// K step 16.  Bound by the plain FP32 pipes; used for the FP32-quality steps until the split-FP16
+// tensor path takes over, and as the numerical reference of the tcgen05 kernels in the tests.
+// ------------------------------------------------------------------------------------------------
+#define SG_BK 16
+
+__global__ void __launch_bounds__(256)
+k_gemm_simt(GemmParams p) {
+  __shared__ float As[SG_BK][128];
+  __shared__ float Bs[SG_BK][132];
+  for (int t = blockIdx.x; t < p.n_tiles; t += gridDim.x) {
+    const TileDesc td = p.tiles[t];
+    if (p.state && p.iter > p.state[td.mat]) continue;
+    const int n = p.dims[td.mat];
+    const int K = (n + SG_BK - 1) / SG_BK * SG_BK;  // padded region is valid (identity / zero)
+    const float *A = p.a32 + (int64_t)td.mat * p.slab;
+    const float *B = p.b32 + (int64_t)td.mat * p.slab;
+    const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
+    float acc[8][8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i)
+#pragma unroll
+      for (int j = 0; j < 8; ++j) acc[i][j] = 0.f;
+    for (int k0 = 0; k0 < K; k0 += SG_BK) {
+      __syncthreads();
+      // A tile: columns k0..k0+15, rows m0..m0+127 (contiguous along rows)
+#pragma unroll
+      for (int i = 0; i < 2; ++i) {
+        const int idx = threadIdx.x + i * 256;      // 512 float4
+        const int kk = idx >> 5, r4 = (idx & 31) * 4;
+        const float4 v = *reinterpret_cast<const float4 *>(A + (int64_t)(k0 + kk) * p.ld + td.m0 + r4);
+        *reinterpret_cast<float4 *>(&As[kk][r4]) = v;
+      }
+      // B tile: columns n0..n0+127 of B, rows k0..k0+15 (contiguous along k) -> Bs[k][n]
+#pragma unroll
+      for (int i = 0; i < 2; ++i) {
+        const int idx = threadIdx.x + i * 256;
+        const int nn = idx >> 2, k4 = (idx & 3) * 4;
+        const float4 v = *reinterpret_cast<const float4 *>(B + (int64_t)(td.n0 + nn) * p.ld + k0 + k4);
+        Bs[k4 + 0][nn] = v.x; Bs[k4 + 1][nn] = v.y; Bs[k4 + 2][nn] = v.z; Bs[k4 + 3][nn] = v.w;
+      }
+      __syncthreads();
+#pragma unroll
+      for (int kk = 0; kk < SG_BK; ++kk) {
+        float a[8], b[8];
+        *reinterpret_cast<float4 *>(&a[0]) = *reinterpret_cast<const float4 *>(&As[kk][tx * 4]);
+        *reinterpret_cast<float4 *>(&a[4]) = *reinterpret_cast<const float4 *>(&As[kk][64 + tx * 4]);
+        *reinterpret_cast<float4 *>(&b[0]) = *reinterpret_cast<const float4 *>(&Bs[kk][ty * 4]);
+        *reinterpret_cast<float4 *>(&b[4]) = *reinterpret_cast<const float4 *>(&Bs[kk][64 + ty * 4]);
+#pragma unroll
+        for (int i = 0; i < 8; ++i)
+#pragma unroll
+          for (int j = 0; j < 8; ++j) acc[i][j] = fmaf(a[i], b[j], acc[i][j]);
+      }
+    }
+    // epilogue: thread owns rows {tx*4..+3, 64+tx*4..+3} x cols {ty*4..+3, 64+ty*4..+3}
+    float ss = 0.f;
+    const int64_t base = (int64_t)td.mat * p.slab;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+      const int c = td.n0 + (j < 4 ? ty * 4 + j : 64 + ty * 4 + (j - 4));
+#pragma unroll
+      for (int ih = 0; ih < 2; ++ih) {
+        const int r = td.m0 + (ih ? 64 + tx * 4 : tx * 4);
+        const int64_t off = base + (int64_t)c * p.ld + r;
+        float4 o;
+        float *ov = reinterpret_cast<float *>(&o);
+        if (p.mode == EPI_IDENT) {
+#pragma unroll
+          for (int i = 0; i < 4; ++i) {
+            const float v = ((r + i == c) ? 1.f : 0.f) - acc[ih * 4 + i][j];
+            ov[i] = v;
+            if (r + i < n && c < n) ss = fmaf(v, v, ss);
+          }
+        } else {
+          float4 ci = make_float4(0.f, 0.f, 0.f, 0.f);
+          if (p.beta != 0.f) ci = *reinterpret_cast<const float4 *>(p.cin32 + off);
+          const float *cv = reinterpret_cast<const float *>(&ci);
+          const float al = p.alpha_div ? p.alpha / p.alpha_div[td.mat] : p.alpha;
+#pragma unroll
+          for (int i = 0; i < 4; ++i) ov[i] = fmaf(al, acc[ih * 4 + i][j], p.beta * cv[i]);
+        }
+        if (p.cout32) *reinterpret_cast<float4 *>(p.cout32 + off) = o;
+        if (p.cout16) {
+          __half2 h01 = __floats2half2_rn(ov[0], ov[1]), h23 = __floats2half2_rn(ov[2], ov[3]);
+          uint2 pk;
+          pk.x = *reinterpret_cast<uint32_t *>(&h01);
+          pk.y = *reinterpret_cast<uint32_t *>(&h23);
+          *reinterpret_cast<uint2 *>(p.cout16 + off) = pk;
+        }
+      }
+    }
+    if (p.mode == EPI_IDENT && p.resid2) {
+      for (int d = 16; d > 0; d >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, d);
+      if ((threadIdx.x & 31) == 0) atomicAdd(&p.resid2[td.mat], ss);
+    }
+  }
+}
+
+cudaError_t launch_gemm_simt(const GemmParams &p, cudaStream_t st) {
+  if (p.n_tiles == 0) return cudaSuccess;
+  int grid = p.n_tiles < 148 * 8 ? p.n_tiles : 148 * 8;
+  k_gemm_simt<<<grid, 256, 0, st>>>(p);
+  return cudaGetLastError();
+}

@@ -1,0 +1,319 @@
+// a0 neighbour lists, a1 gather, a5/a6 density columns + write-back, a7 block trace.
+// All integer work is exact (int64 squared distances on the 2^-16 A grid, reading 2).
+#include "common.cuh"
+
+// ------------------------------------------------------------------------------------------------
+// a0: brute-force neighbour search, one warp per molecule j, candidates i scanned in ascending order
+// so the list comes out sorted (Fig. 2 b,c PAPER.md:172,190).  Positions are staged through shared
+// memory in tiles so every block reads the position array once per tile, coalesced.
+// ------------------------------------------------------------------------------------------------
+#define NB_WARPS 8
+#define NB_TILE 1024
+
+__device__ __forceinline__ int64_t min_image_sq(int32_t xi, int32_t yi, int32_t zi, int32_t xj,
+                                                int32_t yj, int32_t zj, int32_t bx, int32_t by,
+                                                int32_t bz) {
+  int32_t dx = xi - xj, dy = yi - yj, dz = zi - zj;
+  int32_t hx = bx >> 1, hy = by >> 1, hz = bz >> 1;
+  if (dx > hx) dx -= bx; else if (dx < -hx) dx += bx;
+  if (dy > hy) dy -= by; else if (dy < -hy) dy += by;
+  if (dz > hz) dz -= bz; else if (dz < -hz) dz += bz;
+  return (int64_t)dx * dx + (int64_t)dy * dy + (int64_t)dz * dz;
+}
+
+template <bool FILL>
+__global__ void __launch_bounds__(NB_WARPS * 32)
+k_neighbours(int n_mol, const int32_t *__restrict__ pos, int32_t bx, int32_t by, int32_t bz,
+             int64_t rc2, int32_t *__restrict__ counts, const int32_t *__restrict__ row_ptr,
+             int32_t *__restrict__ col_idx) {
+  __shared__ int32_t sp[NB_TILE * 3];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int j = blockIdx.x * NB_WARPS + warp;
+  const bool live = j < n_mol;
+  int32_t xj = 0, yj = 0, zj = 0;
+  if (live) { xj = pos[3 * j]; yj = pos[3 * j + 1]; zj = pos[3 * j + 2]; }
+  int32_t found = 0;
+  int32_t out = (FILL && live) ? row_ptr[j] : 0;
+  for (int base = 0; base < n_mol; base += NB_TILE) {
+    const int cnt = min(NB_TILE, n_mol - base);
+    __syncthreads();
+    for (int t = threadIdx.x; t < cnt * 3; t += blockDim.x) sp[t] = pos[(size_t)base * 3 + t];
+    __syncthreads();
+    if (!live) continue;
+    for (int t = 0; t < cnt; t += 32) {
+      const int i = t + lane;
+      bool ok = false;
+      if (i < cnt)
+        ok = min_image_sq(sp[3 * i], sp[3 * i + 1], sp[3 * i + 2], xj, yj, zj, bx, by, bz) <= rc2;
+      const unsigned m = __ballot_sync(0xffffffffu, ok);
+      if (FILL) {
+        if (ok) col_idx[out + __popc(m & ((1u << lane) - 1u))] = base + i;
+        out += __popc(m);
+      } else {
+        found += __popc(m);
+      }
+    }
+  }
+  if (!FILL && live && lane == 0) counts[j] = found;
+}
+
+cudaError_t launch_neighbour_count(int n_mol, const int32_t *pos, const int32_t *box, int32_t rc,
+                                   int32_t *counts, cudaStream_t st) {
+  if (n_mol <= 0) return cudaSuccess;
+  int grid = (n_mol + NB_WARPS - 1) / NB_WARPS;
+  k_neighbours<false><<<grid, NB_WARPS * 32, 0, st>>>(n_mol, pos, box[0], box[1], box[2],
+                                                      (int64_t)rc * rc, counts, nullptr, nullptr);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_neighbour_fill(int n_mol, const int32_t *pos, const int32_t *box, int32_t rc,
+                                  const int32_t *row_ptr, int32_t *col_idx, cudaStream_t st) {
+  if (n_mol <= 0) return cudaSuccess;
+  int grid = (n_mol + NB_WARPS - 1) / NB_WARPS;
+  k_neighbours<true><<<grid, NB_WARPS * 32, 0, st>>>(n_mol, pos, box[0], box[1], box[2],
+                                                     (int64_t)rc * rc, nullptr, row_ptr, col_idx);
+  return cudaGetLastError();
+}
+
+// Exclusive prefix sum of counts[0..n) into row_ptr[0..n] by one block (n is the number of molecules:
+// a few hundred thousand at most, so one block walking the array in 1024-element steps is enough).
+__global__ void __launch_bounds__(1024) k_exclusive_scan(const int32_t *__restrict__ counts,
+                                                         int32_t *__restrict__ row_ptr, int n) {
+  __shared__ int32_t warp_sums[32];
+  __shared__ int32_t carry_s;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  if (threadIdx.x == 0) carry_s = 0;
+  __syncthreads();
+  for (int base = 0; base < n; base += 1024) {
+    const int i = base + threadIdx.x;
+    int32_t v = i < n ? counts[i] : 0;
+    int32_t x = v;
+    for (int d = 1; d < 32; d <<= 1) {
+      int32_t y = __shfl_up_sync(0xffffffffu, x, d);
+      if (lane >= d) x += y;
+    }
+    if (lane == 31) warp_sums[warp] = x;
+    __syncthreads();
+    if (warp == 0) {
+      int32_t w = warp_sums[lane];
+      for (int d = 1; d < 32; d <<= 1) {
+        int32_t y = __shfl_up_sync(0xffffffffu, w, d);
+        if (lane >= d) w += y;
+      }
+      warp_sums[lane] = w;
+    }
+    __syncthreads();
+    const int32_t carry = carry_s;
+    const int32_t incl = x + (warp > 0 ? warp_sums[warp - 1] : 0) + carry;
+    if (i < n) row_ptr[i] = incl - v;
+    __syncthreads();
+    if (threadIdx.x == 1023) carry_s = incl;
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) row_ptr[n] = carry_s;
+}
+
+cudaError_t launch_exclusive_scan(const int32_t *counts, int32_t *row_ptr, int n, cudaStream_t st) {
+  k_exclusive_scan<<<1, 1024, 0, st>>>(counts, row_ptr, n);
+  return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------
+// a1: gather (submatrix construction, step (i) PAPER.md:140, NOLSM PAPER.md:158).
+// One warp per block-column b of submatrix j.  For every block-row a the lanes binary-search
+// neighbour N_j[b] in the CSR row of neighbour N_j[a]; the hit positions are kept in shared memory.
+// Then the six dense columns 6b..6b+5 are written top to bottom, lanes along the rows, so every
+// store instruction writes 128 contiguous bytes of the column-major output.  Rows and columns
+// between n_j and the tile-padded extent are zero, except a unit diagonal in S (keeps the padded S
+// SPD; the padded part decouples exactly).
+// ------------------------------------------------------------------------------------------------
+#define GA_WARPS 4
+
+__global__ void __launch_bounds__(GA_WARPS * 32)
+k_gather(const int32_t *__restrict__ row_ptr, const int32_t *__restrict__ col_idx,
+         const float *__restrict__ h_val, const float *__restrict__ s_val, int mol_begin, int ld,
+         int64_t slab, float *__restrict__ h_out, float *__restrict__ s_out) {
+  extern __shared__ int32_t s_pos[];  // [GA_WARPS][m_max]
+  const int mat = blockIdx.y;
+  const int j = mol_begin + mat;
+  const int lo = row_ptr[j];
+  const int m = row_ptr[j + 1] - lo;
+  const int n = m * NOLSM_BS;
+  const int P = (n + NOLSM_TILE_M - 1) / NOLSM_TILE_M * NOLSM_TILE_M;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int m_pad_blocks = (P + NOLSM_BS - 1) / NOLSM_BS;  // block-columns incl. padding
+  int32_t *pos = s_pos + warp * ((ld + NOLSM_BS - 1) / NOLSM_BS + 1);
+  float *hj = h_out + (int64_t)mat * slab;
+  float *sj = s_out + (int64_t)mat * slab;
+  for (int b = blockIdx.x * GA_WARPS + warp; b < m_pad_blocks; b += gridDim.x * GA_WARPS) {
+    if (b < m) {
+      const int ib = col_idx[lo + b];
+      for (int a = lane; a < m; a += 32) {
+        const int ia = col_idx[lo + a];
+        int l = row_ptr[ia], r = row_ptr[ia + 1];
+        const int end = r;
+        while (l < r) {  // lower bound of ib in the sorted CSR row of ia
+          const int mid = (l + r) >> 1;
+          if (col_idx[mid] < ib) l = mid + 1; else r = mid;
+        }
+        pos[a] = (l < end && col_idx[l] == ib) ? l : -1;
+      }
+    }
+    __syncwarp();
+    for (int p = 0; p < NOLSM_BS; ++p) {
+      const int c = b * NOLSM_BS + p;
+      if (c >= P) break;
+      float *hc = hj + (int64_t)c * ld;
+      float *sc = sj + (int64_t)c * ld;
+      for (int r = lane; r < P; r += 32) {
+        float hv = 0.f, sv = 0.f;
+        if (c < n && r < n) {
+          const int a = r / NOLSM_BS, o = r - a * NOLSM_BS;
+          const int k = pos[a];
+          if (k >= 0) {
+            hv = h_val[(int64_t)k * 36 + o * NOLSM_BS + p];
+            sv = s_val[(int64_t)k * 36 + o * NOLSM_BS + p];
+          }
+        } else if (r == c) {
+          sv = 1.f;
+        }
+        hc[r] = hv;
+        sc[r] = sv;
+      }
+    }
+    __syncwarp();
+  }
+}
+
+cudaError_t launch_gather(const nolsm_batch *b, const int32_t *row_ptr, const int32_t *col_idx,
+                          const float *h_val, const float *s_val, float *h_out, float *s_out,
+                          cudaStream_t st) {
+  if (b->count == 0) return cudaSuccess;
+  const int per_warp = (b->ld + NOLSM_BS - 1) / NOLSM_BS + 1;
+  const size_t smem = (size_t)GA_WARPS * per_warp * sizeof(int32_t);
+  const int cols = (b->ld + NOLSM_BS - 1) / NOLSM_BS;
+  dim3 grid((cols + GA_WARPS - 1) / GA_WARPS, b->count);
+  k_gather<<<grid, GA_WARPS * 32, smem, st>>>(row_ptr, col_idx, h_val, s_val, b->mol_begin, b->ld,
+                                              (int64_t)b->ld * b->ld, h_out, s_out);
+  return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------
+// a5 + a6: D_j[:, own] = 1/2 (I - X_j) S_j^-1[:, own]  (Eq. 12; only the own columns are
+// kept) written straight into the column-owned store: rows 6a..6a+5 of the n_j x 6
+// result are block (N_j[a], j) = block row_ptr[j]+a of D, so the result is one contiguous run.
+// One thread per row r, the six own columns of S^-1 staged in shared memory, X read column by
+// column (coalesced).  Also accumulates the diagonal estimate sum_{c in own}(1 - X_cc) (reading 15).
+// ------------------------------------------------------------------------------------------------
+#define DN_THREADS 128
+
+__global__ void __launch_bounds__(DN_THREADS)
+k_density(const int32_t *__restrict__ row_ptr, const int32_t *__restrict__ col_idx, int mol_begin,
+          int ld, int64_t slab, const float *__restrict__ x, const float *__restrict__ x_alt,
+          const int32_t *__restrict__ iters, const float *__restrict__ sinv,
+          float *__restrict__ d_val, double *__restrict__ ne_diag) {
+  extern __shared__ float s_sinv[];  // [6][n]
+  const int mat = blockIdx.y;
+  const int j = mol_begin + mat;
+  const int lo = row_ptr[j];
+  const int m = row_ptr[j + 1] - lo;
+  const int n = m * NOLSM_BS;
+  // position of j in its own (sorted) neighbour list
+  int l = 0, r_ = m;
+  while (l < r_) {
+    const int mid = (l + r_) >> 1;
+    if (col_idx[lo + mid] < j) l = mid + 1; else r_ = mid;
+  }
+  const int own0 = l * NOLSM_BS;
+  const float *xj = ((x_alt != nullptr && (iters[mat] & 1)) ? x_alt : x) + (int64_t)mat * slab;
+  const float *sj = sinv + (int64_t)mat * slab;
+  for (int t = threadIdx.x; t < NOLSM_BS * n; t += blockDim.x) {
+    const int p = t / n, k = t - p * n;
+    s_sinv[t] = sj[(int64_t)(own0 + p) * ld + k];
+  }
+  __syncthreads();
+  const int r = blockIdx.x * DN_THREADS + threadIdx.x;
+  if (r < n) {
+    float acc[NOLSM_BS];
+#pragma unroll
+    for (int p = 0; p < NOLSM_BS; ++p) acc[p] = 0.f;
+    for (int k = 0; k < n; ++k) {
+      const float xv = xj[(int64_t)k * ld + r];
+#pragma unroll
+      for (int p = 0; p < NOLSM_BS; ++p) acc[p] = fmaf(xv, s_sinv[p * n + k], acc[p]);
+    }
+    float *out = d_val + ((int64_t)lo * 36 + (int64_t)r * NOLSM_BS);
+#pragma unroll
+    for (int p = 0; p < NOLSM_BS; ++p) out[p] = 0.5f * (s_sinv[p * n + r] - acc[p]);
+    if (ne_diag != nullptr && r >= own0 && r < own0 + NOLSM_BS)
+      atomicAdd(ne_diag, (double)(1.f - xj[(int64_t)r * ld + r]));
+  }
+}
+
+cudaError_t launch_density(const nolsm_batch *b, const float *x, const float *x_alt, const float *sinv,
+                           const int32_t *row_ptr, const int32_t *col_idx, float *d_val,
+                           double *ne_diag, cudaStream_t st) {
+  if (b->count == 0) return cudaSuccess;
+  const size_t smem = (size_t)NOLSM_BS * b->max_n * sizeof(float);
+  static size_t smem_set = 0;
+  if (smem > 48 * 1024 && smem > smem_set) {
+    cudaError_t e = cudaFuncSetAttribute(k_density, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    smem_set = smem;
+  }
+  dim3 grid((b->max_n + DN_THREADS - 1) / DN_THREADS, b->count);
+  k_density<<<grid, DN_THREADS, smem, st>>>(row_ptr, col_idx, b->mol_begin, b->ld,
+                                            (int64_t)b->ld * b->ld, x, x_alt, b->d_iters, sinv, d_val,
+                                            ne_diag);
+  return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------
+// a7: N = 2 sum over stored blocks <D(i,j), S(i,j)>_F  (reading 15).
+// One warp per molecule j; lane k handles block (N_j[k], j): D block k of row j against S block
+// (i, j), found by binary search of j in row i of S.  FP32 products, FP64 accumulation.
+// ------------------------------------------------------------------------------------------------
+#define TR_WARPS 4
+
+__global__ void __launch_bounds__(TR_WARPS * 32)
+k_trace(const int32_t *__restrict__ row_ptr, const int32_t *__restrict__ col_idx, int mol_begin,
+        int count, const float *__restrict__ d_val, const float *__restrict__ s_val,
+        double *__restrict__ ne, double *__restrict__ q_mol) {
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int mat = blockIdx.x * TR_WARPS + warp;
+  if (mat >= count) return;
+  const int j = mol_begin + mat;
+  const int lo = row_ptr[j], hi = row_ptr[j + 1];
+  double sum = 0.0;
+  for (int k = lo + lane; k < hi; k += 32) {
+    const int i = col_idx[k];
+    int l = row_ptr[i], r = row_ptr[i + 1];
+    const int end = r;
+    while (l < r) {
+      const int mid = (l + r) >> 1;
+      if (col_idx[mid] < j) l = mid + 1; else r = mid;
+    }
+    if (l < end && col_idx[l] == j) {
+      const float *db = d_val + (int64_t)k * 36;
+      const float *sb = s_val + (int64_t)l * 36;
+      double part = 0.0;
+#pragma unroll 4
+      for (int e = 0; e < 36; ++e) part += (double)(db[e] * sb[e]);
+      sum += part;
+    }
+  }
+  for (int d = 16; d > 0; d >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, d);
+  if (lane == 0) {
+    if (q_mol != nullptr) q_mol[j] = 2.0 * sum;
+    atomicAdd(ne, 2.0 * sum);
+  }
+}
+
+cudaError_t launch_trace(const nolsm_batch *b, const int32_t *row_ptr, const int32_t *col_idx,
+                         const float *d_val, const float *s_val, double *ne, double *q_mol,
+                         cudaStream_t st) {
+  if (b->count == 0) return cudaSuccess;
+  k_trace<<<(b->count + TR_WARPS - 1) / TR_WARPS, TR_WARPS * 32, 0, st>>>(
+      row_ptr, col_idx, b->mol_begin, b->count, d_val, s_val, ne, q_mol);
+  return cudaGetLastError();
+}
