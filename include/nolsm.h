@@ -162,6 +162,20 @@ nolsm_status nolsm_solve_mu(nolsm_ctx *ctx, const nolsm_bsr *H, const nolsm_bsr 
                             double *ne_out /*host*/, double *q_mol, nolsm_solve_stats *stats /*host*/,
                             void *stream);
 
+/* The same whole path with HOST buffers (the end-to-end call: Fig. 2 d-h of the paper include the
+ * transfers).  row_ptr [n_mol+1], col_idx [nnzb], h_val, s_val, d_val [nnzb*36]
+ * are HOST pointers (pinned memory makes the copies asynchronous; pageable works).  The context
+ * owns device copies of the pattern and of H, S, D (grown on demand, reused across calls); every
+ * call copies pattern + H + S host->device, runs nolsm_solve_mu, and copies D device->host.
+ * *h2d_bytes / *d2h_bytes (host, may be NULL) receive the bytes moved.  Synchronises. */
+nolsm_status nolsm_solve_mu_host(nolsm_ctx *ctx, int32_t n_mol, const int32_t *row_ptr /*host*/,
+                                 const int32_t *col_idx /*host*/, const float *h_val /*host*/,
+                                 const float *s_val /*host*/, double n_electrons, double mu_lo,
+                                 double mu_hi, double tol_ne_per_mol, int32_t max_steps,
+                                 int32_t precision, float *d_val /*host*/, double *mu_out /*host*/,
+                                 double *ne_out /*host*/, nolsm_solve_stats *stats /*host*/,
+                                 int64_t *h2d_bytes /*host*/, int64_t *d2h_bytes /*host*/, void *stream);
+
 /* Dense microbench entry (BASELINE configs[4]; analogue of the paper's Fig. 6):
  * sign(A_b) for `batch` dense n x n FP32 matrices stored one after another (row-major, leading
  * dimension n).  X0 = A_b / scale[b] (scale: device float [batch], e.g. ||A_b||_2; NULL: the

@@ -14,7 +14,7 @@ STATUS = {0: "NOLSM_OK", 1: "NOLSM_EINVAL", 2: "NOLSM_ENOMEM", 3: "NOLSM_ECUDA",
 EXPORTED_SYMBOLS = [
     "nolsm_create", "nolsm_destroy", "nolsm_last_error", "nolsm_version", "nolsm_build_neighbours",
     "nolsm_build_submatrices", "nolsm_batch_capacity", "nolsm_release_batch", "nolsm_sign_batched",
-    "nolsm_scatter_density", "nolsm_solve_mu", "nolsm_sign_dense_batched", "nolsm_batch_read",
+    "nolsm_scatter_density", "nolsm_solve_mu", "nolsm_solve_mu_host", "nolsm_sign_dense_batched", "nolsm_batch_read",
     "nolsm_batch_size", "nolsm_batch_ld", "nolsm_gemm_batched", "nolsm_launch_count",
 ]
 
@@ -107,6 +107,9 @@ def load_library():
     lib.nolsm_solve_mu.argtypes = [vp, P(_Bsr), P(_Bsr), f64, f64, f64, f64, i32, i32, P(_Bsr), P(f64), P(f64),
                                    vp, P(SolveStats), vp]
     lib.nolsm_solve_mu.restype = i32
+    lib.nolsm_solve_mu_host.argtypes = [vp, i32, vp, vp, vp, vp, f64, f64, f64, f64, i32, i32, vp, P(f64), P(f64),
+                                        P(SolveStats), P(i64), P(i64), vp]
+    lib.nolsm_solve_mu_host.restype = i32
     lib.nolsm_sign_dense_batched.argtypes = [vp, vp, vp, i32, i32, i32, f32, i32, i32, vp, P(SignStats), vp]
     lib.nolsm_sign_dense_batched.restype = i32
     lib.nolsm_batch_read.argtypes = [vp, vp, i32, i32, vp, i64, P(i32), vp]
@@ -294,6 +297,28 @@ class Context:
                                      C.byref(stats) if want_stats else None, _stream(stream))
         self._check(st)
         return mu.value, ne.value, D, stats
+
+    def solve_mu_host(self, row_ptr, col_idx, h_val, s_val, d_val, n_electrons, mu_lo, mu_hi, tol_ne_per_mol=1e-3,
+                      max_steps=40, precision=-1, want_stats=True, stream=None):
+        """HOST tensors (CPU torch tensors, ideally pinned): pattern int32, blocks float32.  d_val is
+        overwritten with the density blocks.  Returns (mu, n_electrons(mu), stats, h2d_bytes, d2h_bytes)."""
+        torch = _torch()
+        for t, dt in ((row_ptr, torch.int32), (col_idx, torch.int32), (h_val, torch.float32),
+                      (s_val, torch.float32), (d_val, torch.float32)):
+            if t.is_cuda or not t.is_contiguous() or t.dtype != dt:
+                raise NolsmError(1, "solve_mu_host takes contiguous CPU tensors (int32 pattern, float32 blocks)")
+        mu, ne = C.c_double(0.0), C.c_double(0.0)
+        h2d, d2h = C.c_int64(0), C.c_int64(0)
+        stats = SolveStats() if want_stats else None
+        st = self.lib.nolsm_solve_mu_host(self.handle, int(row_ptr.numel()) - 1, C.c_void_p(row_ptr.data_ptr()),
+                                          C.c_void_p(col_idx.data_ptr()), C.c_void_p(h_val.data_ptr()),
+                                          C.c_void_p(s_val.data_ptr()), float(n_electrons), float(mu_lo),
+                                          float(mu_hi), float(tol_ne_per_mol), int(max_steps), precision,
+                                          C.c_void_p(d_val.data_ptr()), C.byref(mu), C.byref(ne),
+                                          C.byref(stats) if want_stats else None, C.byref(h2d), C.byref(d2h),
+                                          _stream(stream))
+        self._check(st)
+        return mu.value, ne.value, stats, h2d.value, d2h.value
 
     # dense microbench -------------------------------------------------------------------------------
     def sign_dense_batched(self, a, scale=None, precision=-1, tol=0.0, max_iter=0, fixed_iter=-1, out=None,

@@ -109,6 +109,7 @@ extern "C" void nolsm_destroy(nolsm_ctx *ctx) {
   cudaDeviceSynchronize();
   for (nolsm_batch *b : ctx->slots) free_batch(b);
   cudaFree(ctx->d_scalars);
+  cudaFree(ctx->m_row_ptr); cudaFree(ctx->m_col_idx); cudaFree(ctx->m_h); cudaFree(ctx->m_s); cudaFree(ctx->m_d);
   cudaFreeHost(ctx->h_scalars);
   cudaFreeHost(ctx->h_active);
   for (int i = 0; i < 4; ++i)
@@ -803,6 +804,64 @@ extern "C" nolsm_status nolsm_solve_mu(nolsm_ctx *ctx, const nolsm_bsr *H, const
       rc = NOLSM_ENOCONV;
     }
   }
+  return rc;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Whole path with HOST buffers (end-to-end leg: transfers inside)
+// ------------------------------------------------------------------------------------------------
+extern "C" nolsm_status nolsm_solve_mu_host(nolsm_ctx *ctx, int32_t n_mol, const int32_t *row_ptr,
+                                            const int32_t *col_idx, const float *h_val, const float *s_val,
+                                            double n_electrons, double mu_lo, double mu_hi, double tol_ne_per_mol,
+                                            int32_t max_steps, int32_t precision, float *d_val, double *mu_out,
+                                            double *ne_out, nolsm_solve_stats *stats, int64_t *h2d_bytes,
+                                            int64_t *d2h_bytes, void *stream) {
+  if (!ctx) return NOLSM_EINVAL;
+  if (n_mol <= 0 || !row_ptr || !col_idx || !h_val || !s_val || !d_val) {
+    ctx->err = "nolsm_solve_mu_host: bad argument";
+    return NOLSM_EINVAL;
+  }
+  cudaStream_t st = (cudaStream_t)stream;
+  const int64_t nnzb = row_ptr[n_mol];
+  if (nnzb <= 0 || row_ptr[0] != 0) { ctx->err = "nolsm_solve_mu_host: bad row_ptr"; return NOLSM_EINVAL; }
+  if ((size_t)n_mol > ctx->m_cap_mol) {
+    cudaStreamSynchronize(st);
+    cudaFree(ctx->m_row_ptr);
+    ctx->m_row_ptr = nullptr;
+    ctx->m_cap_mol = 0;
+    if (cudaMalloc(&ctx->m_row_ptr, sizeof(int32_t) * ((size_t)n_mol + 1)) != cudaSuccess) {
+      cudaGetLastError(); ctx->err = "cudaMalloc of the row_ptr mirror failed"; return NOLSM_ENOMEM;
+    }
+    ctx->m_cap_mol = (size_t)n_mol;
+  }
+  if ((size_t)nnzb > ctx->m_cap_nnzb) {
+    cudaStreamSynchronize(st);
+    cudaFree(ctx->m_col_idx); cudaFree(ctx->m_h); cudaFree(ctx->m_s); cudaFree(ctx->m_d);
+    ctx->m_col_idx = nullptr; ctx->m_h = ctx->m_s = ctx->m_d = nullptr;
+    ctx->m_cap_nnzb = 0;
+    const size_t vb = sizeof(float) * 36 * (size_t)nnzb;
+    if (cudaMalloc(&ctx->m_col_idx, sizeof(int32_t) * (size_t)nnzb) != cudaSuccess ||
+        cudaMalloc(&ctx->m_h, vb) != cudaSuccess || cudaMalloc(&ctx->m_s, vb) != cudaSuccess ||
+        cudaMalloc(&ctx->m_d, vb) != cudaSuccess) {
+      cudaGetLastError(); ctx->err = "cudaMalloc of the block-store mirrors failed"; return NOLSM_ENOMEM;
+    }
+    ctx->m_cap_nnzb = (size_t)nnzb;
+  }
+  const size_t vb = sizeof(float) * 36 * (size_t)nnzb;
+  NOLSM_CUDA(ctx, cudaMemcpyAsync(ctx->m_row_ptr, row_ptr, sizeof(int32_t) * ((size_t)n_mol + 1), cudaMemcpyHostToDevice, st));
+  NOLSM_CUDA(ctx, cudaMemcpyAsync(ctx->m_col_idx, col_idx, sizeof(int32_t) * (size_t)nnzb, cudaMemcpyHostToDevice, st));
+  NOLSM_CUDA(ctx, cudaMemcpyAsync(ctx->m_h, h_val, vb, cudaMemcpyHostToDevice, st));
+  NOLSM_CUDA(ctx, cudaMemcpyAsync(ctx->m_s, s_val, vb, cudaMemcpyHostToDevice, st));
+  nolsm_bsr H{n_mol, NOLSM_BS, ctx->m_row_ptr, ctx->m_col_idx, ctx->m_h};
+  nolsm_bsr S{n_mol, NOLSM_BS, ctx->m_row_ptr, ctx->m_col_idx, ctx->m_s};
+  nolsm_bsr D{n_mol, NOLSM_BS, ctx->m_row_ptr, ctx->m_col_idx, ctx->m_d};
+  nolsm_status rc = nolsm_solve_mu(ctx, &H, &S, n_electrons, mu_lo, mu_hi, tol_ne_per_mol, max_steps, precision, &D,
+                                   mu_out, ne_out, nullptr, stats, st);
+  if (rc != NOLSM_OK && rc != NOLSM_ENOCONV) return rc;
+  NOLSM_CUDA(ctx, cudaMemcpyAsync(d_val, ctx->m_d, vb, cudaMemcpyDeviceToHost, st));
+  NOLSM_CUDA(ctx, cudaStreamSynchronize(st));
+  if (h2d_bytes) *h2d_bytes = (int64_t)(2 * vb + sizeof(int32_t) * ((size_t)n_mol + 1 + (size_t)nnzb));
+  if (d2h_bytes) *d2h_bytes = (int64_t)vb;
   return rc;
 }
 

@@ -92,6 +92,10 @@ struct nolsm_ctx {
   cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
   void *encode_tiled = nullptr;   // cuTensorMapEncodeTiled entry point
   bool umma_ok = false;
+  // device mirrors of the caller's HOST store (nolsm_solve_mu_host), grown on demand
+  int32_t *m_row_ptr = nullptr, *m_col_idx = nullptr;
+  float *m_h = nullptr, *m_s = nullptr, *m_d = nullptr;
+  size_t m_cap_mol = 0, m_cap_nnzb = 0;
 };
 
 #define NOLSM_CUDA(ctx, call)                                                          \

@@ -339,7 +339,7 @@ nolsm_status umma_init(nolsm_ctx *ctx) {
 
 nolsm_status umma_make_maps(nolsm_ctx *ctx, nolsm_batch *b) {
   b->maps_valid = false;
-  if (!ctx->umma_ok) return NOLSM_OK;
+  if (!ctx->umma_ok || b->count == 0) return NOLSM_OK;
   for (int i = 0; i < 6; ++i) {
     nolsm_status s = encode_map(ctx, &b->map_a[i], b->h[i], b->ld, b->count, 64, 64);
     if (s != NOLSM_OK) return s;

@@ -1,0 +1,370 @@
+"""Parity of the CUDA path (through the C ABI) with the FP64 oracle on the same seeded inputs.
+
+Tolerances (BASELINE.json:north_star, restated in DESIGN.md "Tolerances"):
+  neighbour lists / index sets   bit-exact
+  gather                         bit-exact (it is a copy)
+  D elements, max-abs            1e-5 (FP32 path)   5e-3 (FP16 operands / FP32 accumulate)
+  ||X^2 - I||_F / sqrt(n)        <= 1e-2 (evaluated here in FP64 on the returned FP32 iterate)
+  electron count                 |N_gpu - N_oracle| / n_mol <= 1e-3   (reading 16)
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+TOL_D = {0: 5e-3, 1: 1e-5}      # keyed by precision: FP16_FP32 = 0, FP32 = 1
+TOL_RESID = 1e-2
+TOL_NE_PER_MOL = 1e-3
+MU = -0.85                       # inside the gap of every generated system
+
+
+@pytest.fixture(scope="module")
+def nolsm():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    import paper_2104_08245_b200 as m
+    m.load_library()  # raises if libnolsm.so is missing: no fallback
+    return m
+
+
+@pytest.fixture(scope="module")
+def torch_mod():
+    import torch
+    return torch
+
+
+def _device_system(nolsm, system):
+    H = nolsm.BlockSparse.from_numpy(system.row_ptr, system.col_idx, system.h_val)
+    S = nolsm.BlockSparse(H.row_ptr, H.col_idx,
+                          __import__("torch").as_tensor(system.s_val).contiguous().cuda())
+    return H, S
+
+
+@pytest.fixture(scope="module")
+def mid_system():
+    import nolsm_inputs as gi
+    return gi.make_water_system(216, 8.0)
+
+
+@pytest.fixture(scope="module")
+def mid_solution(mid_system):
+    import oracle.nolsm_oracle as orc
+    return orc.solve_system(mid_system, mu=MU)
+
+
+# ---------------------------------------------------------------------------------------------
+# a0
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n_mol,cutoff", [(32, 6.0), (32, 9.0), (216, 8.0), (4096, 8.0)])
+def test_neighbour_lists_bit_exact(nolsm, torch_mod, n_mol, cutoff):
+    import nolsm_inputs as gi
+    import oracle.nolsm_oracle as orc
+    pos, box = gi.make_positions(n_mol)
+    rc_q = int(round(cutoff * gi.GRID_PER_ANGSTROM))
+    ctx = nolsm.Context()
+    rp, ci = ctx.build_neighbours(torch_mod.as_tensor(pos).cuda(), box, rc_q)
+    rp, ci = rp.cpu().numpy(), ci.cpu().numpy()
+    if n_mol <= 216:
+        rp_o, ci_o = orc.neighbour_list(pos, box, rc_q)
+        assert np.array_equal(rp, rp_o) and np.array_equal(ci, ci_o)
+    else:
+        # oracle one molecule at a time on a sample + global invariants
+        for j in [0, 1, 17, 2047, 4095]:
+            assert np.array_equal(ci[rp[j]:rp[j + 1]], orc.neighbours_of(pos, box, rc_q, j))
+        assert rp[0] == 0 and rp[-1] == ci.shape[0]
+        rows = np.repeat(np.arange(n_mol), np.diff(rp))
+        fwd = set(zip(rows.tolist(), ci.tolist()))
+        assert all((c, r) in fwd for r, c in list(fwd)[:20000])  # symmetry on a sample
+    ctx.close()
+
+
+def test_neighbours_degenerate_cases(nolsm, torch_mod):
+    ctx = nolsm.Context()
+    # one molecule: its own neighbour; zero cutoff: self only
+    pos = torch_mod.tensor([[5, 7, 9]], dtype=torch_mod.int32).cuda()
+    rp, ci = ctx.build_neighbours(pos, [100, 100, 100], 10)
+    assert rp.tolist() == [0, 1] and ci.tolist() == [0]
+    pos = torch_mod.tensor([[0, 0, 0], [98, 0, 0], [50, 50, 50]], dtype=torch_mod.int32).cuda()
+    rp, ci = ctx.build_neighbours(pos, [100, 100, 100], 0)
+    assert rp.tolist() == [0, 1, 2, 3] and ci.tolist() == [0, 1, 2]
+    # closed ball and the minimum image: |98-0| wraps to 2
+    rp, ci = ctx.build_neighbours(pos, [100, 100, 100], 2)
+    assert ci.tolist() == [0, 1, 0, 1, 2]
+    rp, ci = ctx.build_neighbours(pos, [100, 100, 100], 1)
+    assert ci.tolist() == [0, 1, 2]
+    with pytest.raises(nolsm.NolsmError):
+        ctx.build_neighbours(pos, [101, 100, 100], 1)  # odd box
+    ctx.close()
+
+
+# ---------------------------------------------------------------------------------------------
+# a1
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("which", ["tiny", "mid"])
+def test_gather_bitwise(nolsm, tiny_system, mid_system, which):
+    import oracle.nolsm_oracle as orc
+    system = tiny_system if which == "tiny" else mid_system
+    H, S = _device_system(nolsm, system)
+    ctx = nolsm.Context()
+    count = system.n_mol if which == "tiny" else 24
+    begin = 0 if which == "tiny" else 100
+    batch = ctx.build_submatrices(H, S, begin, count)
+    assert batch.size == count
+    for local in ([0, 5, count - 1] if which == "mid" else range(count)):
+        j = begin + local
+        nbrs = system.col_idx[system.row_ptr[j]:system.row_ptr[j + 1]]
+        for mat, val in ((nolsm.MAT_H, system.h_val), (nolsm.MAT_S, system.s_val)):
+            ref = orc.dense_submatrix(system.row_ptr, system.col_idx, val, nbrs).astype(np.float32)
+            got = batch.read(local, mat).cpu().numpy()
+            assert got.shape == ref.shape
+            assert np.array_equal(got.view(np.uint32), ref.view(np.uint32))
+    empty = ctx.build_submatrices(H, S, 3, 0)
+    assert empty.size == 0
+    with pytest.raises(nolsm.NolsmError):
+        ctx.build_submatrices(H, S, system.n_mol - 1, 2)
+    ctx.close()
+
+
+# ---------------------------------------------------------------------------------------------
+# the GEMM building block
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("kind,tol", [(0, 2e-5), (1, 2e-2), (2, 2e-5)])
+@pytest.mark.parametrize("n,batch", [(64, 3), (146, 5), (478, 2), (863, 2)])
+def test_gemm_building_block(nolsm, torch_mod, kind, tol, n, batch):
+    """C = A B and C = I - A B against FP64 numpy; kind 0 SIMT FP32, 1 tcgen05 FP16 operands,
+    2 tcgen05 split-FP16.  Tolerances relative to sqrt(n) * max|A| * max|B| (rounding of a length-n
+    dot product: FP32 ~ 6e-8 * sqrt(n); FP16 operands ~ 5e-4 * sqrt(n))."""
+    rng = np.random.default_rng(n * 10 + kind)
+    a = rng.uniform(-1, 1, (batch, n, n)).astype(np.float32)
+    b = rng.uniform(-1, 1, (batch, n, n)).astype(np.float32)
+    cin = rng.uniform(-1, 1, (batch, n, n)).astype(np.float32)
+    ref = a.astype(np.float64) @ b.astype(np.float64)
+    scale = np.sqrt(n)
+    ctx = nolsm.Context()
+    ta, tb, tc = (torch_mod.as_tensor(x).cuda() for x in (a, b, cin))
+    c, _ = ctx.gemm_batched(kind, ta, tb)
+    err = np.abs(c.cpu().numpy() - ref).max() / scale
+    assert err < tol, f"plain product: {err}"
+    c, _ = ctx.gemm_batched(kind, ta, tb, cin=tc, alpha=0.5, beta=1.0)
+    err = np.abs(c.cpu().numpy() - (0.5 * ref + cin)).max() / scale
+    assert err < tol, f"axpby: {err}"
+    c, r2 = ctx.gemm_batched(kind, ta, tb, ident=True)
+    want = np.eye(n)[None] - ref
+    err = np.abs(c.cpu().numpy() - want).max() / scale
+    assert err < tol, f"identity-minus: {err}"
+    r2_ref = (want ** 2).sum(axis=(1, 2))
+    assert np.allclose(r2.cpu().numpy(), r2_ref, rtol=5e-3 if kind == 1 else 1e-4)
+    ctx.close()
+
+
+# ---------------------------------------------------------------------------------------------
+# a2, a3: S^-1 and B = S^-1 H
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("precision,tol", [(1, 2e-5), (0, 2e-4)])
+def test_inverse_and_operator(nolsm, tiny_system, precision, tol):
+    """Eq. 15-17 converge to exactly S^-1: compare with LAPACK's inverse in FP64.
+    The FP16 mode refines S^-1 to FP32 quality (reading 11), hence the tight bound there too."""
+    import oracle.nolsm_oracle as orc
+    system = tiny_system
+    H, S = _device_system(nolsm, system)
+    ctx = nolsm.Context(nolsm.Config(precision=precision))
+    batch = ctx.build_submatrices(H, S, 0, system.n_mol)
+    stats = ctx.sign_batched(batch, MU)
+    assert stats.inv_iter_max > 0
+    for local in (0, 7, 31):
+        nbrs = system.col_idx[system.row_ptr[local]:system.row_ptr[local + 1]]
+        s_sub = orc.dense_submatrix(system.row_ptr, system.col_idx, system.s_val, nbrs)
+        h_sub = orc.dense_submatrix(system.row_ptr, system.col_idx, system.h_val, nbrs)
+        sinv = np.linalg.inv(s_sub)
+        got = batch.read(local, nolsm.MAT_SINV).cpu().numpy()
+        assert np.abs(got - sinv).max() < tol
+        got_b = batch.read(local, nolsm.MAT_B).cpu().numpy()
+        assert np.abs(got_b - sinv @ h_sub).max() < 5 * tol
+    ctx.close()
+
+
+# ---------------------------------------------------------------------------------------------
+# a4: sign iteration (dense microbench entry: sign known by construction)
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("precision,tol_x", [(1, 2e-5), (0, 3e-3)])
+@pytest.mark.parametrize("n,batch", [(256, 4), (200, 3), (512, 2)])
+def test_sign_dense_against_construction(nolsm, torch_mod, precision, tol_x, n, batch):
+    import nolsm_inputs as gi
+    import oracle.nolsm_oracle as orc
+    mats = [gi.make_gapped_symmetric(n, seed=7, index=i) for i in range(batch)]
+    a = torch_mod.as_tensor(np.stack([m[0] for m in mats])).cuda()
+    scale = torch_mod.as_tensor(np.array([np.abs(m[2]).max() for m in mats], dtype=np.float32)).cuda()
+    ctx = nolsm.Context(nolsm.Config(precision=precision))
+    x, stats = ctx.sign_dense_batched(a, scale)
+    x = x.cpu().numpy()
+    assert stats.n_unconverged == 0
+    assert 6 <= stats.iter_min and stats.iter_max <= 14
+    for i, (_, q, lam) in enumerate(mats):
+        ref = orc.sign_by_construction(q, lam)
+        assert np.abs(x[i] - ref).max() < tol_x
+        assert orc.sign_residual(x[i]) <= TOL_RESID
+    # fixed-iteration mode against the literal iteration of Eq. 9-10 in FP64
+    k_fix = 5
+    x5, st5 = ctx.sign_dense_batched(a, scale, fixed_iter=k_fix)
+    assert st5.iter_min == k_fix and st5.iter_max == k_fix
+    ref5 = orc.newton_schulz_sign(mats[0][0].astype(np.float64), k_fix, scale=float(np.abs(mats[0][2]).max()))
+    assert np.abs(x5[0].cpu().numpy() - ref5).max() < (5e-3 if precision == 0 else 5e-5)
+    # without a caller-supplied scale the norm bound is used: same limit
+    x2, _ = ctx.sign_dense_batched(a, None)
+    assert np.abs(x2[0].cpu().numpy() - orc.sign_by_construction(mats[0][1], mats[0][2])).max() < tol_x
+    ctx.close()
+
+
+def test_sign_degenerate_inputs(nolsm, torch_mod):
+    ctx = nolsm.Context(nolsm.Config(precision=1))
+    # 1x1 and diagonal matrices: sign is the sign of the entries
+    a = torch_mod.tensor([[[0.3]], [[-0.7]]], dtype=torch_mod.float32).cuda()
+    x, _ = ctx.sign_dense_batched(a, None)
+    assert np.allclose(x.cpu().numpy().ravel(), [1.0, -1.0], atol=1e-5)
+    d = np.diag(np.array([0.5, -0.25, 1.0, -1.0, 0.05], dtype=np.float32))[None]
+    x, st = ctx.sign_dense_batched(torch_mod.as_tensor(d).cuda(), None)
+    assert np.allclose(np.diag(x[0].cpu().numpy()), [1, -1, 1, -1, 1], atol=1e-5)
+    # empty batch
+    e = torch_mod.empty((0, 8, 8), dtype=torch_mod.float32).cuda()
+    x, st = ctx.sign_dense_batched(e, None)
+    assert x.shape[0] == 0
+    # a singular matrix cannot converge: reported, not hidden
+    z = torch_mod.zeros((1, 16, 16), dtype=torch_mod.float32).cuda()
+    z[0, 0, 0] = 1.0
+    x, st = ctx.sign_dense_batched(z, None, max_iter=8)
+    assert st.n_unconverged == 1 and st.iter_max == 8
+    ctx.close()
+
+
+# ---------------------------------------------------------------------------------------------
+# whole path, element by element
+# ---------------------------------------------------------------------------------------------
+def _check_density(nolsm, system, d_ref, mu, precision, ne_ref, mol_begin=0, mol_count=None):
+    import torch
+    H, S = _device_system(nolsm, system)
+    D = S.like()
+    ctx = nolsm.Context(nolsm.Config(precision=precision))
+    mol_count = system.n_mol - mol_begin if mol_count is None else mol_count
+    batch = ctx.build_submatrices(H, S, mol_begin, mol_count)
+    stats = ctx.sign_batched(batch, mu)
+    assert stats.n_unconverged == 0
+    ne = torch.zeros(1, dtype=torch.float64, device="cuda")
+    ne_diag = torch.zeros(1, dtype=torch.float64, device="cuda")
+    q = torch.zeros(system.n_mol, dtype=torch.float64, device="cuda")
+    ctx.scatter_density(batch, S, D, ne, q, ne_diag)
+    lo, hi = system.row_ptr[mol_begin], system.row_ptr[mol_begin + mol_count]
+    d = D.val.cpu().numpy()[lo:hi]
+    err = np.abs(d - d_ref[lo:hi]).max()
+    assert err < TOL_D[precision], f"max|dD| = {err}"
+    # residual of the returned iterate, FP64, true n
+    import oracle.nolsm_oracle as orc
+    for local in (0, mol_count // 2, mol_count - 1):
+        assert orc.sign_residual(batch.read(local, nolsm.MAT_X).cpu().numpy()) <= TOL_RESID
+    # D is written only inside the pattern and only for the batch's molecules
+    full = D.val.cpu().numpy()
+    assert not full[:lo].any() and not full[hi:].any()
+    ctx.close()
+    return float(ne.item()), float(ne_diag.item()), q.cpu().numpy(), stats
+
+
+@pytest.mark.parametrize("precision", [1, 0])
+def test_density_tiny_all_molecules(nolsm, tiny_system, tiny_solution, precision):
+    import oracle.nolsm_oracle as orc
+    sols = tiny_solution["solutions"]
+    d_ref = orc.density_blocks(sols, tiny_system.row_ptr, MU)
+    ne_ref = orc.electron_count(sols, MU)
+    ne, ne_diag, q, stats = _check_density(nolsm, tiny_system, d_ref, MU, precision, ne_ref)
+    assert abs(ne - ne_ref) / tiny_system.n_mol <= TOL_NE_PER_MOL
+    assert abs(ne_diag - ne_ref) / tiny_system.n_mol <= TOL_NE_PER_MOL
+    q_ref = np.array([s.population(MU) for s in sols])
+    worst = np.abs(q - q_ref).max()
+    assert worst <= (2e-5 if precision == 1 else 5e-3), worst   # reading 16: reported per molecule
+    # block contraction of the oracle on the GPU's D agrees with the GPU's own reduction
+    assert stats.iter_max <= 14
+
+
+@pytest.mark.parametrize("precision", [1, 0])
+def test_density_mid_partial_batch(nolsm, mid_system, mid_solution, precision):
+    """216 molecules, 8 A: n ~ 478 spans 4 row tiles with a ragged tail; a batch in the middle of the
+    system checks mol_begin handling."""
+    import oracle.nolsm_oracle as orc
+    sols = mid_solution["solutions"]
+    d_ref = orc.density_blocks(sols, mid_system.row_ptr, MU)
+    begin, count = 50, 60
+    ne_ref = sum(s.population(MU) for s in sols[begin:begin + count])
+    ne, ne_diag, q, _ = _check_density(nolsm, mid_system, d_ref, MU, precision, ne_ref, begin, count)
+    assert abs(ne - ne_ref) / count <= TOL_NE_PER_MOL
+    assert abs(ne_diag - ne_ref) / count <= TOL_NE_PER_MOL
+
+
+@pytest.mark.parametrize("precision", [1, 0])
+def test_solve_mu_tiny(nolsm, tiny_system, tiny_solution, precision):
+    """Bisection: mu is not unique (reading 14) -- parity is on D and N, and mu must
+    lie on the oracle's plateau (max_j HOMO_j, min_j LUMO_j)."""
+    import oracle.nolsm_oracle as orc
+    sols = tiny_solution["solutions"]
+    H, S = _device_system(nolsm, tiny_system)
+    ctx = nolsm.Context(nolsm.Config(precision=precision))
+    mu, ne, D, stats = ctx.solve_mu(H, S, tiny_system.n_electrons, -3.0, 0.0, tol_ne_per_mol=1e-3, max_steps=30)
+    n_occ = {s.j: int((s.lam < tiny_solution["mu"]).sum()) for s in sols}
+    homo, lumo = orc.mu_plateau(sols, lambda s: n_occ[s.j])
+    assert homo < mu < lumo
+    ne_ref = orc.electron_count(sols, mu)
+    assert abs(ne - ne_ref) / tiny_system.n_mol <= TOL_NE_PER_MOL
+    assert abs(ne - tiny_system.n_electrons) <= 1e-3 * tiny_system.n_mol
+    d_ref = orc.density_blocks(sols, tiny_system.row_ptr, mu)
+    assert np.abs(D.val.cpu().numpy() - d_ref).max() < TOL_D[precision]
+    assert stats.mu_steps == tiny_solution["steps"]     # same midpoint sequence as the oracle's bisection
+    assert abs(stats.ne_diag - ne_ref) / tiny_system.n_mol <= TOL_NE_PER_MOL
+    # fixed number of evaluations (BASELINE configs[1]: "5 mu bisection steps"), bracket shrinks by 2^-4
+    mu5, ne5, _, st5 = ctx.solve_mu(H, S, tiny_system.n_electrons, -3.0, 0.0, tol_ne_per_mol=-1.0, max_steps=5)
+    assert st5.mu_steps == 5 and abs((st5.mu_hi - st5.mu_lo) - 3.0 / 16) < 1e-12
+    # streaming through a small workspace gives the same D
+    ctx2 = nolsm.Context(nolsm.Config(precision=precision, workspace_bytes=64 << 20))
+    mu2, ne2, D2, st2 = ctx2.solve_mu(H, S, tiny_system.n_electrons, -3.0, 0.0, tol_ne_per_mol=1e-3, max_steps=30)
+    assert st2.n_batches > 1 and mu2 == mu
+    assert np.abs(D2.val.cpu().numpy() - D.val.cpu().numpy()).max() < TOL_D[precision]
+    ctx.close()
+    ctx2.close()
+
+
+# ---------------------------------------------------------------------------------------------
+# BASELINE sizes, sampled (the oracle solves the sampled molecules one by one)
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name,precision,begin,count,sample", [
+    ("w4096", 1, 1000, 296, [0, 150, 295]),
+    ("w4096", 0, 2000, 296, [1, 100, 294]),
+    ("w32768", 0, 20000, 148, [0, 147]),
+])
+def test_baseline_configs_sampled(nolsm, name, precision, begin, count, sample):
+    import torch
+    import nolsm_inputs as gi
+    import oracle.nolsm_oracle as orc
+    n_mol, cutoff = gi.CONFIGS[name]
+    system = gi.make_water_system(n_mol, cutoff)
+    H, S = _device_system(nolsm, system)
+    D = S.like()
+    ctx = nolsm.Context(nolsm.Config(precision=precision))
+    batch = ctx.build_submatrices(H, S, begin, count)
+    stats = ctx.sign_batched(batch, MU)
+    assert stats.n_unconverged == 0
+    ne = torch.zeros(1, dtype=torch.float64, device="cuda")
+    q = torch.zeros(n_mol, dtype=torch.float64, device="cuda")
+    ctx.scatter_density(batch, S, D, ne, q, None)
+    d = D.val.cpu().numpy()
+    q = q.cpu().numpy()
+    for local in sample:
+        j = begin + local
+        sol = orc.solve_molecule(system.row_ptr, system.col_idx, system.h_val, system.s_val, j)
+        ref = sol.density_columns(MU).reshape(-1, 6, 6)
+        lo = system.row_ptr[j]
+        err = np.abs(d[lo:lo + ref.shape[0]] - ref).max()
+        assert err < TOL_D[precision], f"molecule {j}: max|dD| = {err}"
+        assert abs(q[j] - sol.population(MU)) < (2e-5 if precision == 1 else 5e-3)
+        assert orc.sign_residual(batch.read(local, nolsm.MAT_X).cpu().numpy()) <= TOL_RESID
+    # property that holds at any size: every molecule carries ~8 electrons (plateau, reading 14)
+    qs = q[begin:begin + count]
+    assert np.abs(qs - 8.0).max() < 0.03
+    assert abs(ne.item() - qs.sum()) < 1e-6 * count
+    ctx.close()
