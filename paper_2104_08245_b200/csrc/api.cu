@@ -872,7 +872,9 @@ extern "C" nolsm_status nolsm_sign_dense_batched(nolsm_ctx *ctx, const float *a,
                                                  int32_t batch, int32_t precision, float tol, int32_t max_iter,
                                                  int32_t fixed_iter, float *x_out, nolsm_sign_stats *stats,
                                                  void *stream) {
-  if (!ctx || !a || !x_out || n <= 0 || batch < 0) return NOLSM_EINVAL;
+  if (!ctx || n <= 0 || batch < 0) return NOLSM_EINVAL;
+  if (batch == 0) { if (stats) memset(stats, 0, sizeof(*stats)); return NOLSM_OK; }
+  if (!a || !x_out) { ctx->err = "nolsm_sign_dense_batched: null matrix pointer"; return NOLSM_EINVAL; }
   cudaStream_t st = (cudaStream_t)stream;
   const int prec = effective_precision(ctx, precision);
   resolve_sign_args(ctx, prec, &tol, &max_iter, &fixed_iter);

@@ -321,7 +321,7 @@ def test_solve_mu_tiny(nolsm, tiny_system, tiny_solution, precision):
     mu5, ne5, _, st5 = ctx.solve_mu(H, S, tiny_system.n_electrons, -3.0, 0.0, tol_ne_per_mol=-1.0, max_steps=5)
     assert st5.mu_steps == 5 and abs((st5.mu_hi - st5.mu_lo) - 3.0 / 16) < 1e-12
     # streaming through a small workspace gives the same D
-    ctx2 = nolsm.Context(nolsm.Config(precision=precision, workspace_bytes=64 << 20))
+    ctx2 = nolsm.Context(nolsm.Config(precision=precision, workspace_bytes=16 << 20))
     mu2, ne2, D2, st2 = ctx2.solve_mu(H, S, tiny_system.n_electrons, -3.0, 0.0, tol_ne_per_mol=1e-3, max_steps=30)
     assert st2.n_batches > 1 and mu2 == mu
     assert np.abs(D2.val.cpu().numpy() - D.val.cpu().numpy()).max() < TOL_D[precision]
