@@ -99,8 +99,11 @@ static void free_batch(nolsm_batch *b) {
   cudaFree(b->d_scale);
   cudaFree(b->d_norm);
   cudaFree(b->d_active);
-  cudaFree(b->d_tiles);
   cudaFree(b->d_tiles_simt);
+  cudaFree(b->d_ready);
+  cudaFree(b->d_tiles_done);
+  cudaFree(b->d_group_active);
+  cudaFree(b->d_maps);
   delete b;
 }
 
@@ -133,7 +136,12 @@ extern "C" int32_t nolsm_batch_ld(const nolsm_batch *b) { return b ? b->ld : 0; 
 // ------------------------------------------------------------------------------------------------
 // Batch storage
 // ------------------------------------------------------------------------------------------------
-static size_t dense_bytes(int count, int ld) { return (size_t)7 * 4 * (size_t)ld * ld * (size_t)count; }
+// FP32 units per submatrix: S/X, H, Y/S^-1, Z/B and the FP16 operand buffers (two per unit):
+// 6 of them in FP16 mode, 10 in FP32 mode (split hi/lo operands).
+static int units_for(int precision) { return precision == NOLSM_FP16_FP32 ? 7 : 9; }
+static size_t dense_bytes(int count, int ld, int units) {
+  return (size_t)units * 4 * (size_t)ld * ld * (size_t)count;
+}
 
 static size_t allocated_bytes(const nolsm_ctx *ctx, int except_slot) {
   size_t t = 0;
@@ -152,7 +160,7 @@ static cudaError_t grow(T **ptr, size_t n) {
 // Size slot `slot` for `dims` (true dimensions) and upload the metadata.  Host-synchronous uploads
 // (small); the dense workspace is grow-only.
 static nolsm_status setup_batch(nolsm_ctx *ctx, int slot, const std::vector<int32_t> &dims, int mol_begin,
-                                bool sparse, nolsm_batch **out, cudaStream_t st) {
+                                bool sparse, int units, nolsm_batch **out, cudaStream_t st) {
   if (slot < 0 || slot > 4096) { ctx->err = "bad slot"; return NOLSM_EINVAL; }
   if ((int)ctx->slots.size() <= slot) ctx->slots.resize(slot + 1, nullptr);
   if (!ctx->slots[slot]) ctx->slots[slot] = new nolsm_batch();
@@ -161,7 +169,7 @@ static nolsm_status setup_batch(nolsm_ctx *ctx, int slot, const std::vector<int3
   int max_n = 0;
   for (int n : dims) max_n = std::max(max_n, n);
   const int ld = std::max(NOLSM_PAD, round_up(max_n, NOLSM_PAD));
-  const size_t need = dense_bytes(count, ld);
+  const size_t need = dense_bytes(count, ld, units);
   if (need > b->base_bytes) {
     if ((int64_t)(allocated_bytes(ctx, slot) + need) > ctx->cfg.workspace_bytes) {
       ctx->err = "workspace_bytes too small for this batch";
@@ -183,7 +191,8 @@ static nolsm_status setup_batch(nolsm_ctx *ctx, int slot, const std::vector<int3
     const size_t cap = (size_t)count;
     if (grow(&b->d_dims, cap) || grow(&b->d_state, cap) || grow(&b->d_iters, cap) ||
         grow(&b->d_resid2, cap * NOLSM_MAX_RESID_SLOTS) || grow(&b->d_lastres, cap) ||
-        grow(&b->d_scale, cap) || grow(&b->d_norm, cap * 2) ||
+        grow(&b->d_scale, cap) || grow(&b->d_norm, cap * 2) || grow(&b->d_ready, cap) ||
+        grow(&b->d_tiles_done, cap) || grow(&b->d_group_active, cap) ||
         (b->d_active == nullptr && grow(&b->d_active, (size_t)NOLSM_MAX_RESID_SLOTS))) {
       cudaGetLastError();
       ctx->err = "cudaMalloc of batch metadata failed";
@@ -200,41 +209,32 @@ static nolsm_status setup_batch(nolsm_ctx *ctx, int slot, const std::vector<int3
   b->prepared = false;
   b->prepared_precision = -1;
   b->n_host = dims;
-  b->bn = 128;
+  b->n_unit = units;
+  b->n_half = 2 * (units - 4);
   const size_t slab = (size_t)ld * ld;
-  for (int i = 0; i < 7; ++i) b->u[i] = reinterpret_cast<float *>(b->base) + (size_t)i * count * slab;
-  for (int i = 0; i < 6; ++i) b->h[i] = reinterpret_cast<__half *>(b->u[4]) + (size_t)i * count * slab;
-  // tile lists
-  std::vector<TileDesc> tiles, tiles_simt;
+  for (int i = 0; i < units; ++i) b->u[i] = reinterpret_cast<float *>(b->base) + (size_t)i * count * slab;
+  for (int i = 0; i < b->n_half; ++i) b->h[i] = reinterpret_cast<__half *>(b->u[4]) + (size_t)i * count * slab;
+  // tile list of the SIMT kernel (debug path); the tcgen05 engine enumerates its tiles arithmetically
+  std::vector<TileDesc> tiles_simt;
   b->sum_n3 = b->sum_n3_padded = 0.0;
+  const bool simt = (ctx->cfg.flags & NOLSM_FLAG_SIMT_ONLY) != 0 || !ctx->umma_ok || !sparse;
   for (int m = 0; m < count; ++m) {
     const int n = dims[m];
-    const int P = round_up(n, NOLSM_TILE_M), Pn = round_up(n, 64);
-    for (int n0 = 0; n0 < Pn; n0 += b->bn)
-      for (int m0 = 0; m0 < P; m0 += NOLSM_TILE_M)
-        tiles.push_back(TileDesc{m, m0, n0, std::min(b->bn, Pn - n0)});
-    for (int n0 = 0; n0 < P; n0 += 128)
-      for (int m0 = 0; m0 < P; m0 += 128) tiles_simt.push_back(TileDesc{m, m0, n0, 128});
+    const int P = round_up(n, NOLSM_TILE_M), Pn = round_up(n, 16);
+    if (simt)
+      for (int n0 = 0; n0 < P; n0 += 128)
+        for (int m0 = 0; m0 < P; m0 += 128) tiles_simt.push_back(TileDesc{m, m0, n0, 128});
     b->sum_n3 += (double)n * n * n;
     b->sum_n3_padded += (double)P * Pn * Pn;
-  }
-  if (tiles.size() > b->tiles_cap) {
-    cudaStreamSynchronize(st);
-    if (grow(&b->d_tiles, tiles.size())) { cudaGetLastError(); ctx->err = "cudaMalloc tiles"; return NOLSM_ENOMEM; }
-    b->tiles_cap = tiles.size();
   }
   if (tiles_simt.size() > b->tiles_simt_cap) {
     cudaStreamSynchronize(st);
     if (grow(&b->d_tiles_simt, tiles_simt.size())) { cudaGetLastError(); ctx->err = "cudaMalloc tiles"; return NOLSM_ENOMEM; }
     b->tiles_simt_cap = tiles_simt.size();
   }
-  b->n_tiles = (int)tiles.size();
   b->n_tiles_simt = (int)tiles_simt.size();
   // pageable host buffers: cudaMemcpyAsync stages them before returning, so the vectors may die
   NOLSM_CUDA(ctx, cudaMemcpyAsync(b->d_dims, dims.data(), sizeof(int32_t) * count, cudaMemcpyHostToDevice, st));
-  if (!tiles.empty())
-    NOLSM_CUDA(ctx, cudaMemcpyAsync(b->d_tiles, tiles.data(), sizeof(TileDesc) * tiles.size(),
-                                    cudaMemcpyHostToDevice, st));
   if (!tiles_simt.empty())
     NOLSM_CUDA(ctx, cudaMemcpyAsync(b->d_tiles_simt, tiles_simt.data(), sizeof(TileDesc) * tiles_simt.size(),
                                     cudaMemcpyHostToDevice, st));
@@ -312,19 +312,20 @@ extern "C" int32_t nolsm_batch_capacity(nolsm_ctx *ctx, const nolsm_bsr *H, int3
   nolsm_status s = read_dims(ctx, H->row_ptr, mol_begin, avail, dims, (cudaStream_t)stream);
   if (s != NOLSM_OK) return -(int32_t)s;
   const size_t budget = (size_t)ctx->cfg.workspace_bytes / (size_t)n_slots;
+  const int units = units_for(effective_precision(ctx, -1));
   int max_n = 0, count = 0;
   for (int i = 0; i < avail; ++i) {
     const int mn = std::max(max_n, dims[i]);
-    if (dense_bytes(i + 1, round_up(mn, NOLSM_PAD)) > budget) break;
+    if (dense_bytes(i + 1, round_up(mn, NOLSM_PAD), units) > budget) break;
     max_n = mn;
     count = i + 1;
   }
   return count;
 }
 
-extern "C" nolsm_status nolsm_build_submatrices(nolsm_ctx *ctx, const nolsm_bsr *H, const nolsm_bsr *S,
-                                                int32_t mol_begin, int32_t mol_count, int32_t slot,
-                                                nolsm_batch **out, void *stream) {
+static nolsm_status build_submatrices_impl(nolsm_ctx *ctx, const nolsm_bsr *H, const nolsm_bsr *S,
+                                           int32_t mol_begin, int32_t mol_count, int32_t slot, int units,
+                                           nolsm_batch **out, void *stream) {
   if (!ctx || !out) return NOLSM_EINVAL;
   CHECK(check_bsr(ctx, H, "H"));
   CHECK(check_bsr(ctx, S, "S"));
@@ -340,58 +341,235 @@ extern "C" nolsm_status nolsm_build_submatrices(nolsm_ctx *ctx, const nolsm_bsr 
   std::vector<int32_t> dims;
   if (mol_count > 0) CHECK(read_dims(ctx, H->row_ptr, mol_begin, mol_count, dims, st));
   nolsm_batch *b = nullptr;
-  CHECK(setup_batch(ctx, slot, dims, mol_begin, true, &b, st));
+  CHECK(setup_batch(ctx, slot, dims, mol_begin, true, units, &b, st));
   LAUNCH(ctx, launch_gather(b, H->row_ptr, H->col_idx, H->val, S->val, b->u[1], b->u[0], st));
   *out = b;
   return NOLSM_OK;
 }
 
+extern "C" nolsm_status nolsm_build_submatrices(nolsm_ctx *ctx, const nolsm_bsr *H, const nolsm_bsr *S,
+                                                int32_t mol_begin, int32_t mol_count, int32_t slot,
+                                                nolsm_batch **out, void *stream) {
+  if (!ctx) return NOLSM_EINVAL;
+  return build_submatrices_impl(ctx, H, S, mol_begin, mol_count, slot, units_for(effective_precision(ctx, -1)), out,
+                                stream);
+}
+
 // ------------------------------------------------------------------------------------------------
 // Iteration drivers
 // ------------------------------------------------------------------------------------------------
+static bool use_simt(const nolsm_ctx *ctx) { return (ctx->cfg.flags & NOLSM_FLAG_SIMT_ONLY) != 0; }
+
+static int group_size(const nolsm_ctx *ctx, const nolsm_batch *b, int bytes_per_elem) {
+  if (ctx->cfg.group > 0) return ctx->cfg.group;
+  // iterates of one group must stay in L2 over a whole iteration, yet a
+  // group must hold a few waves of tiles so that dependent products are far apart in the schedule
+  const double per = (double)bytes_per_elem * b->ld * b->ld;
+  int g = (int)(0.75 * (double)ctx->l2_bytes / per);
+  const int tiles = std::max(1, ((b->max_n + 127) / 128) * ((b->max_n + 255) / 256));
+  const int g_min = (3 * ctx->sm_count + tiles - 1) / tiles;
+  g = std::max(g, g_min);
+  return std::max(1, std::min(g, 1024));
+}
+
+static ChainOp make_op(int mode, float alpha, float beta) {
+  ChainOp o;
+  memset(&o, 0, sizeof(o));
+  for (int p = 0; p < 2; ++p) o.a[p] = o.b[p] = o.a_lo[p] = o.b_lo[p] = o.out16[p] = o.out16_lo[p] = -1;
+  o.cin32 = o.cout32 = -1;
+  o.mode = mode;
+  o.alpha = alpha;
+  o.beta = beta;
+  return o;
+}
+static void set2(int32_t (&d)[2], int even, int odd) { d[0] = even; d[1] = odd; }
+
+static nolsm_status run_chain(nolsm_ctx *ctx, nolsm_batch *b, const ChainProgram &pg, const float *alpha_div,
+                              bool touch_stats, cudaStream_t st) {
+  cudaError_t e = launch_chain(ctx, b, pg, alpha_div, touch_stats, st);
+  ctx->launches += 2;   // reset kernel + chain kernel
+  if (e != cudaSuccess) {
+    ctx->err = std::string("tcgen05 chain: ") + cudaGetErrorString(e) +
+               (ctx->umma_ok ? "" : " (tcgen05 path not initialised: needs an sm_100 device)");
+    cudaGetLastError();
+    return NOLSM_ECUDA;
+  }
+  return NOLSM_OK;
+}
+
+static ChainProgram one_shot(int group) {
+  ChainProgram pg;
+  memset(&pg, 0, sizeof(pg));
+  pg.max_iter = 1;
+  pg.fixed_iter = 1;
+  pg.group = group;
+  return pg;
+}
+
+// a2 + a3 (first part) on the tensor cores: S^-1 by Eq. 15-17 in the correction
+// form  E = I - Z Y,  Y += 1/2 Y E,  Z += 1/2 E Z  (= Eq. 16 with 3I - V = 2I + E), then
+// S^-1 = Z^2 / s_S (Eq. 17), optional Newton refinements (reading 11) and B = S^-1 H
+// (Eq. 12).  FP16 mode: the iteration runs on plain FP16 operands, everything after it
+// on split (hi + lo) operands; FP32 mode: every product on split operands.
+static nolsm_status prepare_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, int precision, cudaStream_t st,
+                                        nolsm_sign_stats *stats, int64_t *gemms) {
+  const bool fp16 = precision == NOLSM_FP16_FP32;
+  const float inv_tol = ctx->cfg.inv_tol > 0.f ? ctx->cfg.inv_tol : (fp16 ? 1e-2f : 1e-5f);
+  const int refine = ctx->cfg.inv_refine >= 0 ? ctx->cfg.inv_refine : (fp16 ? 1 : 0);
+  float *S = b->u[0], *H = b->u[1];
+  LAUNCH(ctx, launch_norm_bound(b, S, 0.f, b->d_norm, st));
+  ChainProgram pg;
+  memset(&pg, 0, sizeof(pg));
+  pg.n_ops = 3;
+  pg.max_iter = ctx->cfg.inv_max_iter;
+  pg.fixed_iter = 0;
+  pg.tol = inv_tol;
+  if (fp16) {
+    // Y16: h0/h1 (ping-pong), Z16: h2/h3, E16: h4; masters Y32 = u2, Z32 = u3
+    LAUNCH(ctx, launch_init_inverse(b, S, b->d_norm, b->u[2], b->u[3], b->h[0], b->h[2], nullptr, nullptr,
+                                    b->d_scale, st));
+    pg.group = group_size(ctx, b, 18);
+    ChainOp &e = pg.ops[0] = make_op(EPI_IDENT, 1.f, 0.f);
+    set2(e.a, 2, 3); set2(e.b, 0, 1); set2(e.out16, 4, 4); e.resid = 1;
+    ChainOp &y = pg.ops[1] = make_op(EPI_AXPBY, 0.5f, 1.f);
+    set2(y.a, 0, 1); set2(y.b, 4, 4); y.cin32 = y.cout32 = 2; set2(y.out16, 1, 0);
+    ChainOp &z = pg.ops[2] = make_op(EPI_AXPBY, 0.5f, 1.f);
+    set2(z.a, 4, 4); set2(z.b, 2, 3); z.cin32 = z.cout32 = 3; set2(z.out16, 3, 2);
+  } else {
+    // split operands: Y (h0,h1)/(h2,h3), Z (h4,h5)/(h6,h7), E (h8,h9)
+    LAUNCH(ctx, launch_init_inverse(b, S, b->d_norm, b->u[2], b->u[3], b->h[0], b->h[4], b->h[1], b->h[5],
+                                    b->d_scale, st));
+    pg.group = group_size(ctx, b, 28);
+    ChainOp &e = pg.ops[0] = make_op(EPI_IDENT, 1.f, 0.f);
+    set2(e.a, 4, 6); set2(e.a_lo, 5, 7); set2(e.b, 0, 2); set2(e.b_lo, 1, 3);
+    set2(e.out16, 8, 8); set2(e.out16_lo, 9, 9); e.resid = 1;
+    ChainOp &y = pg.ops[1] = make_op(EPI_AXPBY, 0.5f, 1.f);
+    set2(y.a, 0, 2); set2(y.a_lo, 1, 3); set2(y.b, 8, 8); set2(y.b_lo, 9, 9);
+    y.cin32 = y.cout32 = 2; set2(y.out16, 2, 0); set2(y.out16_lo, 3, 1);
+    ChainOp &z = pg.ops[2] = make_op(EPI_AXPBY, 0.5f, 1.f);
+    set2(z.a, 8, 8); set2(z.a_lo, 9, 9); set2(z.b, 4, 6); set2(z.b_lo, 5, 7);
+    z.cin32 = z.cout32 = 3; set2(z.out16, 6, 4); set2(z.out16_lo, 7, 5);
+  }
+  CHECK(run_chain(ctx, b, pg, nullptr, true, st));
+  int64_t inv_gemm_sum = 0;
+  if (stats) {   // iterations and residuals of Eq. 15-17, before the sign iteration reuses the arrays
+    std::vector<int32_t> it(b->count);
+    std::vector<float> res(b->count);
+    NOLSM_CUDA(ctx, cudaMemcpyAsync(it.data(), b->d_iters, sizeof(int32_t) * b->count, cudaMemcpyDeviceToHost, st));
+    NOLSM_CUDA(ctx, cudaMemcpyAsync(res.data(), b->d_lastres, sizeof(float) * b->count, cudaMemcpyDeviceToHost, st));
+    NOLSM_CUDA(ctx, cudaStreamSynchronize(st));
+    double fl = 0.0;
+    for (int m = 0; m < b->count; ++m) {
+      stats->inv_iter_max = std::max(stats->inv_iter_max, it[m]);
+      if (!(res[m] <= stats->inv_worst_residual)) stats->inv_worst_residual = res[m];
+      const double n = b->n_host[m];
+      const int products = 3 * it[m] + 2 + 2 * refine;
+      inv_gemm_sum += products;
+      fl += 2.0 * n * n * n * products;
+    }
+    stats->flops_prepare = fl;
+  }
+  const int g1 = group_size(ctx, b, 16);
+  // S^-1 = Z^2 / s_S from the FP32 master: split Z -> (h0,h1); result -> u2 and split (h2,h3)
+  LAUNCH(ctx, launch_scale_copy(b, b->u[3], nullptr, 0, nullptr, b->h[0], b->h[1], st));
+  {
+    ChainProgram p1 = one_shot(g1);
+    p1.n_ops = 1;
+    ChainOp &o = p1.ops[0] = make_op(EPI_AXPBY, 1.f, 0.f);
+    set2(o.a, 0, 0); set2(o.a_lo, 1, 1); set2(o.b, 0, 0); set2(o.b_lo, 1, 1);
+    o.use_div = 1; o.cout32 = 2; set2(o.out16, 2, 2); set2(o.out16_lo, 3, 3);
+    CHECK(run_chain(ctx, b, p1, b->d_scale, false, st));
+  }
+  if (refine > 0) LAUNCH(ctx, launch_scale_copy(b, S, nullptr, 0, nullptr, b->h[0], b->h[1], st));
+  for (int it = 0; it < refine; ++it) {
+    // Newton refinement S^-1 <- S^-1 + S^-1 (I - S S^-1): the residual on split operands, the small
+    // correction on plain FP16 operands (reading 11)
+    ChainProgram p2 = one_shot(g1);
+    p2.n_ops = 2;
+    ChainOp &r = p2.ops[0] = make_op(EPI_IDENT, 1.f, 0.f);
+    set2(r.a, 0, 0); set2(r.a_lo, 1, 1); set2(r.b, 2, 2); set2(r.b_lo, 3, 3); set2(r.out16, 4, 4);
+    ChainOp &c = p2.ops[1] = make_op(EPI_AXPBY, 1.f, 1.f);
+    set2(c.a, 2, 2); set2(c.b, 4, 4); c.cin32 = c.cout32 = 2;
+    CHECK(run_chain(ctx, b, p2, nullptr, false, st));
+    LAUNCH(ctx, launch_scale_copy(b, b->u[2], nullptr, 0, nullptr, b->h[2], b->h[3], st));
+  }
+  // B = S^-1 H on split operands: H -> (h0,h1); result -> u3
+  LAUNCH(ctx, launch_scale_copy(b, H, nullptr, 0, nullptr, b->h[0], b->h[1], st));
+  {
+    ChainProgram p4 = one_shot(g1);
+    p4.n_ops = 1;
+    ChainOp &o = p4.ops[0] = make_op(EPI_AXPBY, 1.f, 0.f);
+    set2(o.a, 2, 2); set2(o.a_lo, 3, 3); set2(o.b, 0, 0); set2(o.b_lo, 1, 1); o.cout32 = 3;
+    CHECK(run_chain(ctx, b, p4, nullptr, false, st));
+  }
+  b->engine_simt = false;
+  b->prepared = true;
+  b->prepared_precision = precision;
+  *gemms += inv_gemm_sum;
+  return NOLSM_OK;
+}
+
+// a3 (second part) + a4 on the tensor cores: X0 = (B - mu I)/s, then Eq. 9-10 in the correction form
+// E = I - X_k^2,  X_{k+1} = X_k + 1/2 X_k E  (reading 12); the residual of the stop rule
+// (reading 9) comes out of the first product's epilogue.  One kernel launch for all iterations.
+static nolsm_status sign_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, double mu, int precision, float tol,
+                                     int max_iter, int fixed_iter, const float *scale_in, cudaStream_t st) {
+  const bool fp16 = precision == NOLSM_FP16_FP32;
+  float *Bm = b->u[3], *X32 = b->u[0];
+  if (!scale_in) LAUNCH(ctx, launch_norm_bound(b, Bm, (float)mu, b->d_norm, st));
+  ChainProgram pg;
+  memset(&pg, 0, sizeof(pg));
+  pg.n_ops = 2;
+  pg.max_iter = max_iter;
+  pg.fixed_iter = fixed_iter > 0 ? fixed_iter : 0;
+  pg.tol = tol;
+  ChainOp &e = pg.ops[0] = make_op(EPI_IDENT, 1.f, 0.f);
+  ChainOp &x = pg.ops[1] = make_op(EPI_AXPBY, 0.5f, 1.f);
+  e.resid = 1;
+  x.cin32 = x.cout32 = 0;
+  if (fp16) {
+    // X16: h0/h1 (ping-pong), E16: h4
+    LAUNCH(ctx, launch_make_x0(b, Bm, (float)mu, b->d_norm, scale_in, X32, b->h[0], nullptr, b->d_scale, st));
+    pg.group = group_size(ctx, b, 10);
+    set2(e.a, 0, 1); set2(e.b, 0, 1); set2(e.out16, 4, 4);
+    set2(x.a, 0, 1); set2(x.b, 4, 4); set2(x.out16, 1, 0);
+  } else {
+    // split operands: X (h0,h1)/(h2,h3), E (h4,h5)
+    LAUNCH(ctx, launch_make_x0(b, Bm, (float)mu, b->d_norm, scale_in, X32, b->h[0], b->h[1], b->d_scale, st));
+    pg.group = group_size(ctx, b, 16);
+    set2(e.a, 0, 2); set2(e.a_lo, 1, 3); set2(e.b, 0, 2); set2(e.b_lo, 1, 3);
+    set2(e.out16, 4, 4); set2(e.out16_lo, 5, 5);
+    set2(x.a, 0, 2); set2(x.a_lo, 1, 3); set2(x.b, 4, 4); set2(x.b_lo, 5, 5);
+    set2(x.out16, 2, 0); set2(x.out16_lo, 3, 1);
+  }
+  return run_chain(ctx, b, pg, nullptr, true, st);
+}
+
+// ---- debugging path: every product on the FP32 SIMT kernel (NOLSM_FLAG_SIMT_ONLY) ----
 struct Engine {
   nolsm_ctx *ctx;
   nolsm_batch *b;
   cudaStream_t st;
   int64_t gemms = 0;
 
-  GemmParams base_params(bool simt) const {
+  GemmParams base_params() const {
     GemmParams p;
     memset(&p, 0, sizeof(p));
-    p.tiles = simt ? b->d_tiles_simt : b->d_tiles;
-    p.n_tiles = simt ? b->n_tiles_simt : b->n_tiles;
+    p.tiles = b->d_tiles_simt;
+    p.n_tiles = b->n_tiles_simt;
     p.dims = b->d_dims;
     p.ld = b->ld;
     p.slab = (int64_t)b->ld * b->ld;
     p.alpha = 1.f;
     return p;
   }
-  // C = I - A*B on the SIMT kernel (FP32 in, FP32 out)
   nolsm_status simt(int mode, float alpha, float beta, const float *alpha_div, const float *a, const float *bb,
                     const float *cin, float *cout, float *resid2, const int32_t *state, int iter) {
-    GemmParams p = base_params(true);
+    GemmParams p = base_params();
     p.mode = mode; p.alpha = alpha; p.beta = beta; p.alpha_div = alpha_div;
     p.a32 = a; p.b32 = bb; p.cin32 = cin; p.cout32 = cout; p.resid2 = resid2;
     p.state = state; p.iter = iter;
     LAUNCH(ctx, launch_gemm_simt(p, st));
-    gemms++;
-    return NOLSM_OK;
-  }
-  // tcgen05 product: operands are FP16 buffers h[ia], h[ib] (kind 2: plus h[ial], h[ibl])
-  nolsm_status umma(int kind, int mode, float alpha, float beta, int ia, int ib, int ial, int ibl,
-                    const float *cin, float *cout32, __half *cout16, __half *cout16_lo, float *resid2,
-                    const int32_t *state, int iter) {
-    GemmParams p = base_params(false);
-    p.mode = mode; p.alpha = alpha; p.beta = beta;
-    p.cin32 = cin; p.cout32 = cout32; p.cout16 = cout16; p.cout16_lo = cout16_lo; p.resid2 = resid2;
-    p.state = state; p.iter = iter;
-    cudaError_t e = launch_gemm_umma(ctx, b, kind, ia, ib, ial, ibl, p, st);
-    ctx->launches++;
-    if (e != cudaSuccess) {
-      ctx->err = std::string("tcgen05 product: ") + cudaGetErrorString(e) +
-                 (ctx->umma_ok ? "" : " (tcgen05 path not initialised: needs an sm_100 device)");
-      return NOLSM_ECUDA;
-    }
     gemms++;
     return NOLSM_OK;
   }
@@ -405,7 +583,7 @@ struct Engine {
     return NOLSM_OK;
   }
   // Lagged host check: after iteration k the active count is copied out; before launching iteration
-  // k+2 the host looks at it.  Returns true when iteration `k` left nobody active.
+  // k+2 the host looks at it.
   nolsm_status post_active(int k) {
     NOLSM_CUDA(ctx, cudaMemcpyAsync(&ctx->h_active[k], &b->d_active[k], sizeof(int32_t), cudaMemcpyDeviceToHost, st));
     NOLSM_CUDA(ctx, cudaEventRecord(ctx->ev[k & 3], st));
@@ -418,11 +596,8 @@ struct Engine {
   }
 };
 
-// Runs `body(k)` for k = 0.. until the control kernel reports nobody active (checked two iterations
-// late so the queue never drains) or max_iter.  Returns the number of iterations LAUNCHED; *executed
-// = iterations that did work (known only if `need_count`, which synchronises).
 template <typename Body>
-static nolsm_status iterate(Engine &E, int max_iter, int fixed_iter, bool need_count, int *executed, Body body) {
+static nolsm_status iterate(Engine &E, int max_iter, int fixed_iter, int *executed, Body body) {
   const int limit = fixed_iter > 0 ? std::min(fixed_iter, max_iter) : max_iter;
   int k = 0;
   for (; k < limit; ++k) {
@@ -434,130 +609,88 @@ static nolsm_status iterate(Engine &E, int max_iter, int fixed_iter, bool need_c
     CHECK(body(k));
     CHECK(E.post_active(k));
   }
-  if (executed) {
-    *executed = k;
-    if (need_count) {
-      NOLSM_CUDA(E.ctx, cudaStreamSynchronize(E.st));
-      for (int i = 0; i < k; ++i)
-        if (E.ctx->h_active[i] == 0) { *executed = i + 1; break; }
-    }
-  }
+  NOLSM_CUDA(E.ctx, cudaStreamSynchronize(E.st));
+  *executed = k;
+  for (int i = 0; i < k; ++i)
+    if (E.ctx->h_active[i] == 0) { *executed = i + 1; break; }
   return NOLSM_OK;
 }
 
-// a2 + a3 (first part): S^-1 by Eq. 15-17 and B = S^-1 H (Eq. 12).
-static nolsm_status prepare_batch(nolsm_ctx *ctx, nolsm_batch *b, int precision, cudaStream_t st,
-                                  nolsm_sign_stats *stats, int64_t *gemms) {
+static nolsm_status prepare_batch_simt(nolsm_ctx *ctx, nolsm_batch *b, cudaStream_t st, nolsm_sign_stats *stats,
+                                       int64_t *gemms) {
   Engine E{ctx, b, st};
-  const bool fp16 = precision == NOLSM_FP16_FP32;
-  float inv_tol = ctx->cfg.inv_tol > 0.f ? ctx->cfg.inv_tol : (fp16 ? 1e-2f : 1e-5f);
+  const float inv_tol = ctx->cfg.inv_tol > 0.f ? ctx->cfg.inv_tol : 1e-5f;
   const int max_it = ctx->cfg.inv_max_iter;
   float *S = b->u[0], *H = b->u[1];
   LAUNCH(ctx, launch_norm_bound(b, S, 0.f, b->d_norm, st));
   CHECK(E.control(0, 0, 0.f, 0, 0, false));
   int executed = 0;
-  if (fp16) {
-    float *Y32 = b->u[2], *Z32 = b->u[3];
-    LAUNCH(ctx, launch_init_inverse(b, S, b->d_norm, Y32, Z32, b->h[0], b->h[2], b->d_scale, st));
-    CHECK(iterate(E, max_it, 0, stats != nullptr, &executed, [&](int k) -> nolsm_status {
-      const int cur = k & 1, nxt = cur ^ 1;
-      CHECK(E.zero_resid(k));
-      // E = I - Z Y
-      CHECK(E.umma(1, EPI_IDENT, 1.f, 0.f, 2 + cur, cur, 0, 0, nullptr, nullptr, b->h[4], nullptr,
-                   E.resid_slot(k), b->d_state, k));
-      CHECK(E.control(1, k, inv_tol, max_it, 0, false));
-      // Y += 1/2 Y E ; Z += 1/2 E Z   (= Eq. 16 with 3I - V = 2I + E)
-      CHECK(E.umma(1, EPI_AXPBY, 0.5f, 1.f, cur, 4, 0, 0, Y32, Y32, b->h[nxt], nullptr, nullptr, b->d_state, k));
-      CHECK(E.umma(1, EPI_AXPBY, 0.5f, 1.f, 4, 2 + cur, 0, 0, Z32, Z32, b->h[2 + nxt], nullptr, nullptr,
-                   b->d_state, k));
-      return NOLSM_OK;
-    }));
-    // S^-1 = Z^2 / s_S (Eq. 17) from the FP32 masters, FP32-quality product
-    CHECK(E.simt(EPI_AXPBY, 1.f, 0.f, b->d_scale, Z32, Z32, nullptr, b->u[2], nullptr, nullptr, 0));
-    float *Sinv = b->u[2];
-    for (int it = 0; it < ctx->cfg.inv_refine; ++it) {
-      // Newton refinement S^-1 <- S^-1 + S^-1 (I - S S^-1): the residual at FP32 quality, the small
-      // correction on the tensor cores (reading 11)
-      CHECK(E.simt(EPI_IDENT, 1.f, 0.f, nullptr, S, Sinv, nullptr, b->u[3], nullptr, nullptr, 0));
-      LAUNCH(ctx, launch_scale_copy(b, Sinv, nullptr, 0, nullptr, b->h[0], nullptr, st));
-      LAUNCH(ctx, launch_scale_copy(b, b->u[3], nullptr, 0, nullptr, b->h[1], nullptr, st));
-      CHECK(E.umma(1, EPI_AXPBY, 1.f, 1.f, 0, 1, 0, 0, Sinv, Sinv, nullptr, nullptr, nullptr, nullptr, 0));
-    }
-    CHECK(E.simt(EPI_AXPBY, 1.f, 0.f, nullptr, Sinv, H, nullptr, b->u[3], nullptr, nullptr, 0));
-    b->x_parity = 0;
-  } else {
-    float *Y[2] = {b->u[2], b->u[5]}, *Z[2] = {b->u[3], b->u[6]}, *Em = b->u[4];
-    LAUNCH(ctx, launch_init_inverse(b, S, b->d_norm, Y[0], Z[0], nullptr, nullptr, b->d_scale, st));
-    CHECK(iterate(E, max_it, 0, true, &executed, [&](int k) -> nolsm_status {
-      const int cur = k & 1, nxt = cur ^ 1;
-      CHECK(E.zero_resid(k));
-      CHECK(E.simt(EPI_IDENT, 1.f, 0.f, nullptr, Z[cur], Y[cur], nullptr, Em, E.resid_slot(k), b->d_state, k));
-      CHECK(E.control(1, k, inv_tol, max_it, 0, true));
-      CHECK(E.simt(EPI_AXPBY, 0.5f, 1.f, nullptr, Y[cur], Em, Y[cur], Y[nxt], nullptr, b->d_state, k));
-      CHECK(E.simt(EPI_AXPBY, 0.5f, 1.f, nullptr, Em, Z[cur], Z[cur], Z[nxt], nullptr, b->d_state, k));
-      return NOLSM_OK;
-    }));
-    float *Zf = Z[executed & 1];
-    CHECK(E.simt(EPI_AXPBY, 1.f, 0.f, b->d_scale, Zf, Zf, nullptr, b->u[4], nullptr, nullptr, 0));
-    CHECK(E.simt(EPI_AXPBY, 1.f, 0.f, nullptr, b->u[4], H, nullptr, b->u[2], nullptr, nullptr, 0));
-  }
+  float *Y[2] = {b->u[2], b->u[5]}, *Z[2] = {b->u[3], b->u[6]}, *Em = b->u[4];
+  LAUNCH(ctx, launch_init_inverse(b, S, b->d_norm, Y[0], Z[0], nullptr, nullptr, nullptr, nullptr, b->d_scale, st));
+  CHECK(iterate(E, max_it, 0, &executed, [&](int k) -> nolsm_status {
+    const int cur = k & 1, nxt = cur ^ 1;
+    CHECK(E.zero_resid(k));
+    CHECK(E.simt(EPI_IDENT, 1.f, 0.f, nullptr, Z[cur], Y[cur], nullptr, Em, E.resid_slot(k), b->d_state, k));
+    CHECK(E.control(1, k, inv_tol, max_it, 0, true));
+    CHECK(E.simt(EPI_AXPBY, 0.5f, 1.f, nullptr, Y[cur], Em, Y[cur], Y[nxt], nullptr, b->d_state, k));
+    CHECK(E.simt(EPI_AXPBY, 0.5f, 1.f, nullptr, Em, Z[cur], Z[cur], Z[nxt], nullptr, b->d_state, k));
+    return NOLSM_OK;
+  }));
+  float *Zf = Z[executed & 1];
+  CHECK(E.simt(EPI_AXPBY, 1.f, 0.f, b->d_scale, Zf, Zf, nullptr, b->u[4], nullptr, nullptr, 0));
+  CHECK(E.simt(EPI_AXPBY, 1.f, 0.f, nullptr, b->u[4], H, nullptr, b->u[2], nullptr, nullptr, 0));
+  b->engine_simt = true;
   b->prepared = true;
-  b->prepared_precision = precision;
+  b->prepared_precision = NOLSM_FP32;
   if (stats) {
     stats->inv_iter_max = executed;
-    stats->flops_prepare = 2.0 * b->sum_n3 * (double)E.gemms;  // upper estimate: every product on every submatrix
+    stats->flops_prepare = 2.0 * b->sum_n3 * (double)E.gemms;
+    std::vector<float> res(b->count);
+    NOLSM_CUDA(ctx, cudaMemcpyAsync(res.data(), b->d_lastres, sizeof(float) * b->count, cudaMemcpyDeviceToHost, st));
+    NOLSM_CUDA(ctx, cudaStreamSynchronize(st));
+    for (float r : res)
+      if (!(r <= stats->inv_worst_residual)) stats->inv_worst_residual = r;
   }
-  *gemms += E.gemms;
+  *gemms += E.gemms * b->count;
   return NOLSM_OK;
 }
 
-static float *sinv_ptr(const nolsm_batch *b) { return b->prepared_precision == NOLSM_FP16_FP32 ? b->u[2] : b->u[4]; }
-static float *bmat_ptr(const nolsm_batch *b) { return b->prepared_precision == NOLSM_FP16_FP32 ? b->u[3] : b->u[2]; }
-static float *x_ptr(const nolsm_batch *b) {
-  if (b->prepared_precision == NOLSM_FP16_FP32) return b->u[0];
-  return b->x_parity ? b->u[3] : b->u[0];
-}
-
-// a3 (second part) + a4: X0 = (B - mu I)/s, then Eq. 9-10 in the correction form
-// X_{k+1} = X_k + 1/2 X_k (I - X_k^2)  (reading 12), residual from the first product.
-static nolsm_status sign_batch(nolsm_ctx *ctx, nolsm_batch *b, double mu, int precision, float tol, int max_iter,
-                               int fixed_iter, const float *scale_in, cudaStream_t st, bool need_count,
-                               int64_t *gemms, int *launched) {
+static nolsm_status sign_batch_simt(nolsm_ctx *ctx, nolsm_batch *b, double mu, float tol, int max_iter,
+                                    int fixed_iter, const float *scale_in, cudaStream_t st) {
   Engine E{ctx, b, st};
-  const bool fp16 = precision == NOLSM_FP16_FP32;
-  float *Bm = bmat_ptr(b);
+  float *Bm = b->u[2];
   if (!scale_in) LAUNCH(ctx, launch_norm_bound(b, Bm, (float)mu, b->d_norm, st));
   CHECK(E.control(0, 0, 0.f, 0, 0, false));
   int executed = 0;
-  if (fp16) {
-    float *X32 = b->u[0];
-    LAUNCH(ctx, launch_make_x0(b, Bm, (float)mu, b->d_norm, scale_in, X32, b->h[0], b->d_scale, st));
-    CHECK(iterate(E, max_iter, fixed_iter, need_count, &executed, [&](int k) -> nolsm_status {
-      const int cur = k & 1, nxt = cur ^ 1;
-      CHECK(E.zero_resid(k));
-      CHECK(E.umma(1, EPI_IDENT, 1.f, 0.f, cur, cur, 0, 0, nullptr, nullptr, b->h[4], nullptr, E.resid_slot(k),
-                   b->d_state, k));
-      CHECK(E.control(1, k, tol, max_iter, fixed_iter, false));
-      CHECK(E.umma(1, EPI_AXPBY, 0.5f, 1.f, cur, 4, 0, 0, X32, X32, b->h[nxt], nullptr, nullptr, b->d_state, k));
-      return NOLSM_OK;
-    }));
-  } else {
-    float *X[2] = {b->u[0], b->u[3]}, *Em = b->u[5];
-    LAUNCH(ctx, launch_make_x0(b, Bm, (float)mu, b->d_norm, scale_in, X[0], nullptr, b->d_scale, st));
-    CHECK(iterate(E, max_iter, fixed_iter, true, &executed, [&](int k) -> nolsm_status {
-      const int cur = k & 1, nxt = cur ^ 1;
-      CHECK(E.zero_resid(k));
-      CHECK(E.simt(EPI_IDENT, 1.f, 0.f, nullptr, X[cur], X[cur], nullptr, Em, E.resid_slot(k), b->d_state, k));
-      CHECK(E.control(1, k, tol, max_iter, fixed_iter, true));
-      CHECK(E.simt(EPI_AXPBY, 0.5f, 1.f, nullptr, X[cur], Em, X[cur], X[nxt], nullptr, b->d_state, k));
-      return NOLSM_OK;
-    }));
-    b->x_parity = executed & 1;
-  }
-  *gemms += E.gemms;
-  if (launched) *launched = executed;
+  float *X[2] = {b->u[0], b->u[3]}, *Em = b->u[5];
+  LAUNCH(ctx, launch_make_x0(b, Bm, (float)mu, b->d_norm, scale_in, X[0], nullptr, nullptr, b->d_scale, st));
+  CHECK(iterate(E, max_iter, fixed_iter, &executed, [&](int k) -> nolsm_status {
+    const int cur = k & 1, nxt = cur ^ 1;
+    CHECK(E.zero_resid(k));
+    CHECK(E.simt(EPI_IDENT, 1.f, 0.f, nullptr, X[cur], X[cur], nullptr, Em, E.resid_slot(k), b->d_state, k));
+    CHECK(E.control(1, k, tol, max_iter, fixed_iter, true));
+    CHECK(E.simt(EPI_AXPBY, 0.5f, 1.f, nullptr, X[cur], Em, X[cur], X[nxt], nullptr, b->d_state, k));
+    return NOLSM_OK;
+  }));
+  b->x_parity = executed & 1;
   return NOLSM_OK;
 }
+
+static nolsm_status prepare_batch(nolsm_ctx *ctx, nolsm_batch *b, int precision, cudaStream_t st,
+                                  nolsm_sign_stats *stats, int64_t *gemms) {
+  if (use_simt(ctx)) return prepare_batch_simt(ctx, b, st, stats, gemms);
+  return prepare_batch_chain(ctx, b, precision, st, stats, gemms);
+}
+
+static nolsm_status sign_batch(nolsm_ctx *ctx, nolsm_batch *b, double mu, int precision, float tol, int max_iter,
+                               int fixed_iter, const float *scale_in, cudaStream_t st) {
+  if (b->engine_simt) return sign_batch_simt(ctx, b, mu, tol, max_iter, fixed_iter, scale_in, st);
+  return sign_batch_chain(ctx, b, mu, precision, tol, max_iter, fixed_iter, scale_in, st);
+}
+
+static float *sinv_ptr(const nolsm_batch *b) { return b->engine_simt ? b->u[4] : b->u[2]; }
+static float *bmat_ptr(const nolsm_batch *b) { return b->engine_simt ? b->u[2] : b->u[3]; }
+static float *x_ptr(const nolsm_batch *b) { return (b->engine_simt && b->x_parity) ? b->u[3] : b->u[0]; }
 
 // Collect per-submatrix iteration counts and residuals (synchronises).
 static nolsm_status collect_stats(nolsm_ctx *ctx, nolsm_batch *b, float tol, int fixed_iter, cudaStream_t st,
@@ -605,20 +738,16 @@ extern "C" nolsm_status nolsm_sign_batched(nolsm_ctx *ctx, nolsm_batch *batch, d
   resolve_sign_args(ctx, prec, &tol, &max_iter, &fixed_iter);
   if (stats) memset(stats, 0, sizeof(*stats));
   int64_t gemms = 0;
+  if (batch->n_unit < units_for(prec)) {
+    ctx->err = "batch was built for another precision (create the context with the precision you run)";
+    return NOLSM_EINVAL;
+  }
   if (!batch->prepared || batch->prepared_precision != prec) {
     if (!batch->sparse) { ctx->err = "dense batch is not prepared"; return NOLSM_EINVAL; }
     if (batch->prepared) { ctx->err = "batch was prepared in another precision; gather it again"; return NOLSM_EINVAL; }
     CHECK(prepare_batch(ctx, batch, prec, st, stats, &gemms));
-    if (stats) {
-      std::vector<float> res(batch->count);
-      NOLSM_CUDA(ctx, cudaMemcpyAsync(res.data(), batch->d_lastres, sizeof(float) * batch->count,
-                                      cudaMemcpyDeviceToHost, st));
-      NOLSM_CUDA(ctx, cudaStreamSynchronize(st));
-      for (float r : res)
-        if (!(r <= stats->inv_worst_residual)) stats->inv_worst_residual = r;
-    }
   }
-  CHECK(sign_batch(ctx, batch, mu, prec, tol, max_iter, fixed_iter, nullptr, st, stats != nullptr, &gemms, nullptr));
+  CHECK(sign_batch(ctx, batch, mu, prec, tol, max_iter, fixed_iter, nullptr, st));
   if (stats) {
     const int inv_it = stats->inv_iter_max;
     const float inv_res = stats->inv_worst_residual;
@@ -627,7 +756,7 @@ extern "C" nolsm_status nolsm_sign_batched(nolsm_ctx *ctx, nolsm_batch *batch, d
     stats->inv_iter_max = inv_it;
     stats->inv_worst_residual = inv_res;
     stats->flops_prepare = fp;
-    stats->gemms = gemms;
+    stats->gemms = gemms + 2 * stats->iter_sum;
   }
   return NOLSM_OK;
 }
@@ -678,6 +807,7 @@ extern "C" nolsm_status nolsm_solve_mu(nolsm_ctx *ctx, const nolsm_bsr *H, const
   if (n_mol > 0) CHECK(read_dims(ctx, H->row_ptr, 0, n_mol, dims, st));
   struct Range { int begin, count; size_t bytes; };
   std::vector<Range> plan;
+  const int units = units_for(prec);
   auto make_plan = [&](size_t budget, int max_count) -> bool {
     plan.clear();
     int i = 0;
@@ -685,12 +815,12 @@ extern "C" nolsm_status nolsm_solve_mu(nolsm_ctx *ctx, const nolsm_bsr *H, const
       int max_n = 0, cnt = 0;
       while (i + cnt < n_mol && cnt < max_count) {
         const int mn = std::max(max_n, dims[i + cnt]);
-        if (dense_bytes(cnt + 1, round_up(mn, NOLSM_PAD)) > budget) break;
+        if (dense_bytes(cnt + 1, round_up(mn, NOLSM_PAD), units) > budget) break;
         max_n = mn;
         cnt++;
       }
       if (cnt == 0) return false;
-      plan.push_back(Range{i, cnt, dense_bytes(cnt, round_up(max_n, NOLSM_PAD))});
+      plan.push_back(Range{i, cnt, dense_bytes(cnt, round_up(max_n, NOLSM_PAD), units)});
       i += cnt;
     }
     return true;
@@ -730,7 +860,7 @@ extern "C" nolsm_status nolsm_solve_mu(nolsm_ctx *ctx, const nolsm_bsr *H, const
       const bool timed = stats != nullptr;
       if (timed) cudaEventRecord(tev[0], st);
       if (!b || !resident) {
-        rc = nolsm_build_submatrices(ctx, H, S, r.begin, r.count, resident ? (int)bi : 0, &b, st);
+        rc = build_submatrices_impl(ctx, H, S, r.begin, r.count, resident ? (int)bi : 0, units, &b, st);
         if (rc != NOLSM_OK) break;
         live[bi] = resident ? b : nullptr;
       }
@@ -743,7 +873,7 @@ extern "C" nolsm_status nolsm_solve_mu(nolsm_ctx *ctx, const nolsm_bsr *H, const
         if (rc != NOLSM_OK) break;
       }
       if (timed) cudaEventRecord(tev[2], st);
-      rc = sign_batch(ctx, b, mu, prec, tol, max_iter, fixed_iter, nullptr, st, false, &gemms, nullptr);
+      rc = sign_batch(ctx, b, mu, prec, tol, max_iter, fixed_iter, nullptr, st);
       if (rc != NOLSM_OK) break;
       if (timed) cudaEventRecord(tev[3], st);
       rc = nolsm_scatter_density(ctx, b, S, D, ctx->d_scalars, q_mol, ctx->d_scalars + 1, st);
@@ -767,7 +897,7 @@ extern "C" nolsm_status nolsm_solve_mu(nolsm_ctx *ctx, const nolsm_bsr *H, const
         acc.flops_sign_padded += cs.flops_sign_padded;
         acc.flops_prepare += bs.flops_prepare;
         acc.inv_iter_max = std::max(acc.inv_iter_max, bs.inv_iter_max);
-        acc.gemms += gemms;
+        acc.gemms += gemms + 2 * cs.iter_sum;
       }
     }
     if (rc != NOLSM_OK) break;
@@ -882,16 +1012,16 @@ extern "C" nolsm_status nolsm_sign_dense_batched(nolsm_ctx *ctx, const float *a,
   if (batch == 0) return NOLSM_OK;
   std::vector<int32_t> dims(batch, n);
   nolsm_batch *b = nullptr;
-  CHECK(setup_batch(ctx, 0, dims, 0, false, &b, st));
+  CHECK(setup_batch(ctx, 0, dims, 0, false, units_for(prec), &b, st));
   b->prepared = true;
   b->prepared_precision = prec;
+  b->engine_simt = use_simt(ctx);
   LAUNCH(ctx, launch_pack(a, n, batch, b->ld, bmat_ptr(b), 0, st));
-  int64_t gemms = 0;
-  CHECK(sign_batch(ctx, b, 0.0, prec, tol, max_iter, fixed_iter, scale, st, stats != nullptr, &gemms, nullptr));
+  CHECK(sign_batch(ctx, b, 0.0, prec, tol, max_iter, fixed_iter, scale, st));
   LAUNCH(ctx, launch_unpack(x_ptr(b), b->ld, (int64_t)b->ld * b->ld, nullptr, nullptr, n, batch, x_out, st));
   if (stats) {
     CHECK(collect_stats(ctx, b, tol, fixed_iter, st, stats));
-    stats->gemms = gemms;
+    stats->gemms = 2 * stats->iter_sum;
   }
   return NOLSM_OK;
 }
@@ -927,23 +1057,32 @@ extern "C" nolsm_status nolsm_gemm_batched(nolsm_ctx *ctx, int32_t kind, int32_t
   cudaStream_t st = (cudaStream_t)stream;
   std::vector<int32_t> dims(batch, n);
   nolsm_batch *b = nullptr;
-  CHECK(setup_batch(ctx, 0, dims, 0, false, &b, st));
-  Engine E{ctx, b, st};
+  CHECK(setup_batch(ctx, 0, dims, 0, false, 7, &b, st));
   // unit padding in A and B keeps the padded rows/columns decoupled, like the iterates of the path
   LAUNCH(ctx, launch_pack(a, n, batch, b->ld, b->u[0], 1, st));
   LAUNCH(ctx, launch_pack(bm, n, batch, b->ld, b->u[1], 1, st));
   if (!ident && beta != 0.f) LAUNCH(ctx, launch_pack(cin, n, batch, b->ld, b->u[2], 0, st));
-  CHECK(E.zero_resid(0));
   const int mode = ident ? EPI_IDENT : EPI_AXPBY;
+  float *resid_src = b->d_resid2;
   if (kind == 0) {
+    Engine E{ctx, b, st};
+    CHECK(E.zero_resid(0));
     CHECK(E.simt(mode, alpha, beta, nullptr, b->u[0], b->u[1], b->u[2], b->u[3], E.resid_slot(0), nullptr, 0));
   } else {
-    LAUNCH(ctx, launch_scale_copy(b, b->u[0], nullptr, 0, nullptr, b->h[0], kind == 2 ? b->h[2] : nullptr, st));
-    LAUNCH(ctx, launch_scale_copy(b, b->u[1], nullptr, 0, nullptr, b->h[1], kind == 2 ? b->h[3] : nullptr, st));
-    CHECK(E.umma(kind, mode, alpha, beta, 0, 1, 2, 3, b->u[2], b->u[3], nullptr, nullptr, E.resid_slot(0), nullptr, 0));
+    LAUNCH(ctx, launch_scale_copy(b, b->u[0], nullptr, 0, nullptr, b->h[0], kind == 2 ? b->h[1] : nullptr, st));
+    LAUNCH(ctx, launch_scale_copy(b, b->u[1], nullptr, 0, nullptr, b->h[2], kind == 2 ? b->h[3] : nullptr, st));
+    ChainProgram pg = one_shot(group_size(ctx, b, 16));
+    pg.n_ops = 1;
+    ChainOp &o = pg.ops[0] = make_op(mode, alpha, beta);
+    set2(o.a, 0, 0); set2(o.b, 2, 2);
+    if (kind == 2) { set2(o.a_lo, 1, 1); set2(o.b_lo, 3, 3); }
+    if (!ident && beta != 0.f) o.cin32 = 2;
+    o.cout32 = 3;
+    o.resid = ident ? 1 : 0;
+    CHECK(run_chain(ctx, b, pg, nullptr, true, st));
   }
   LAUNCH(ctx, launch_unpack(b->u[3], b->ld, (int64_t)b->ld * b->ld, nullptr, nullptr, n, batch, c, st));
   if (resid2 && ident)
-    NOLSM_CUDA(ctx, cudaMemcpyAsync(resid2, E.resid_slot(0), sizeof(float) * batch, cudaMemcpyDeviceToDevice, st));
+    NOLSM_CUDA(ctx, cudaMemcpyAsync(resid2, resid_src, sizeof(float) * batch, cudaMemcpyDeviceToDevice, st));
   return NOLSM_OK;
 }

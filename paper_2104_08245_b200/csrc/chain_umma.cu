@@ -1,0 +1,579 @@
+// The batched matrix-iteration engine: ONE persistent, cooperative kernel runs a whole chain of
+// dependent n x n x n products (every iteration of Eq. 9-10, or of Eq. 15-17
+// PAPER.md:203-215) for every submatrix of a batch on the 5th-generation tensor cores
+// (tcgen05 + TMEM + TMA), sm_100a only.
+//
+// Why one kernel: the two products of a sign iteration are strictly dependent and one product of an
+// n ~ 860 submatrix is < 1 us of the whole GPU, so kernel boundaries would cost more than the work, and
+// a batch-wide launch per product streams every iterate through HBM (18 n^2 bytes per 4 n^3 FLOP,
+// DESIGN.md "Roofline").  Here the submatrices are walked in GROUPS small enough that the iterates of
+// a group stay in the 126 MB L2 for all of its iterations (the B200 analogue of the paper's "caching
+// strategy for the matrices during the iterations"), and the products inside a group
+// are ordered  iteration -> op -> submatrix -> tile  so that by the time a CTA reaches a tile of op
+// s of a submatrix, op s-1 of that submatrix finished several waves ago.  The dependency itself is
+// enforced by a per-submatrix counter in global memory (ready[m] = ops completed, acquire/release at
+// GPU scope), not by a grid barrier; every tile only ever waits for tiles that come earlier in the
+// common order, and all CTAs are co-resident (cooperative launch), so the schedule cannot deadlock.
+//
+// Layout facts:
+//   * all matrices are column-major, so the A operand (M x K) is M-major and the B operand (K x N) is
+//     K-major in shared memory; one TMA tensor map per FP16 buffer with box {64 storage rows,
+//     64 storage columns} serves both roles (A: 2 boxes per 128-row tile and K block; B: one box per
+//     64 tile columns), 128-byte swizzle.
+//   * accumulator: 128 TMEM lanes = tile rows, one 32-bit column per tile column; two accumulator
+//     stages so the epilogue of tile i overlaps the MMAs of tile i+1.
+//   * the FP32 master iterate (reading 12) is read in the epilogue through per-warp TMA
+//     prefetches ({32 rows, 32 columns} FP32 boxes) and written back with coalesced stores.
+//
+// Warp roles (192 threads): warp 0 = scheduler + TMA producer, warp 1 = MMA issuer (+ TMEM
+// allocation), warps 2..5 = epilogue (TMEM lane quadrant = warp_id % 4).
+#include "common.cuh"
+
+namespace {
+
+constexpr int kThreads = 192;
+constexpr int kBK = 64;                  // K elements per pipeline stage (= one 128-byte swizzle row)
+constexpr int kMaxStages = 8;
+constexpr int kTmemCols = 512;
+constexpr int kBoxBytes = 64 * 128;      // one {64 x 64} FP16 box
+constexpr int kATileBytes = 2 * kBoxBytes;
+constexpr int kRing = 4;                 // tile-command ring depth
+constexpr int kEpiBytes = 4 * 2 * 4096;  // per epilogue warp: two {32 x 32} FP32 boxes
+constexpr int kSmemLimit = 232448 - 2048;  // 227 KB minus the static part (barriers, commands)
+constexpr int32_t kDone = 0x7fffffff;
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) {
+  return static_cast<uint32_t>(__cvta_generic_to_shared(p));
+}
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
+               : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
+  asm volatile(
+      "{\n\t"
+      ".reg .pred p;\n\t"
+      "WAIT_LOOP:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+      "@p bra WAIT_DONE;\n\t"
+      "bra WAIT_LOOP;\n\t"
+      "WAIT_DONE:\n\t"
+      "}\n" ::"r"(smem_u32(bar)),
+      "r"(parity)
+      : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(void *dst, const CUtensorMap *map, uint64_t *bar, int c0,
+                                            int c1, int c2) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, "
+      "%4, %5}], [%2];" ::"r"(smem_u32(dst)),
+      "l"(reinterpret_cast<uint64_t>(map)), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2)
+      : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_commit(uint64_t *bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(
+                   smem_u32(bar))
+               : "memory");
+}
+__device__ __forceinline__ void tc_mma_f16(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc,
+                                           uint32_t accumulate) {
+  asm volatile(
+      "{\n\t"
+      ".reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t"
+      "}\n" ::"r"(tmem_d),
+      "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+__device__ __forceinline__ void tc_ld32(uint32_t taddr, uint32_t (&v)[32]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, %17, %18, %19, %20, %21, "
+      "%22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+      : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+        "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]),
+        "=r"(v[15]), "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]),
+        "=r"(v[22]), "=r"(v[23]), "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]),
+        "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+      : "r"(taddr));
+}
+__device__ __forceinline__ void tc_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ int32_t ld_acquire(const int32_t *p) {
+  int32_t v;
+  asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_release(int32_t *p, int32_t v) {
+  asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+
+// Shared-memory matrix descriptor (tcgen05): start address, leading / stride byte offsets (all >> 4),
+// descriptor version 1, 128-byte swizzle.
+__device__ __forceinline__ uint64_t make_smem_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
+  uint64_t d = 0;
+  d |= (uint64_t)((saddr & 0x3FFFF) >> 4);
+  d |= (uint64_t)((lbo_bytes >> 4) & 0x3FFF) << 16;
+  d |= (uint64_t)((sbo_bytes >> 4) & 0x3FFF) << 32;
+  d |= (uint64_t)1 << 46;   // version
+  d |= (uint64_t)2 << 61;   // SWIZZLE_128B
+  return d;
+}
+
+struct TileCmd {              // scheduler -> MMA issuer and epilogue warps
+  int32_t mat, m0, n0, nt;    // submatrix, first row / column, tile columns (multiple of 16, <= bn)
+  int32_t kblocks, ktail;     // K blocks of 64; K=16 steps in the last one (1..4)
+  int32_t op, iter;           // op < 0: no more tiles
+};
+
+struct ChainArgs {
+  ChainProgram prog;
+  const CUtensorMap *maps;    // [n_half] FP16 maps, then [n_unit] FP32 maps
+  __half *hbuf[NOLSM_MAX_HALF];
+  float *ubuf[NOLSM_MAX_UNIT];
+  int32_t n_half;
+  int32_t count, ld;
+  int64_t slab;
+  int32_t bn, b_bytes, stages, stage_bytes;
+  int32_t mt, ntl;            // uniform tile grid per submatrix: mt row tiles x ntl column tiles
+  const int32_t *dims;
+  const float *alpha_div;
+  int32_t *ready, *tiles_done, *state, *iters, *group_active;
+  float *resid2, *lastres;
+};
+
+__global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
+  extern __shared__ __align__(1024) uint8_t smem_raw[];
+  __shared__ uint64_t full_bar[kMaxStages], empty_bar[kMaxStages], tfull_bar[2], tempty_bar[2];
+  __shared__ uint64_t cmd_full[kRing], cmd_empty[kRing], cin_bar[4][2];
+  __shared__ TileCmd cmds[kRing];
+  __shared__ uint32_t tmem_base_s;
+
+  const ChainProgram &pg = args.prog;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+  uint8_t *epi_smem = smem + (size_t)args.stages * args.stage_bytes;
+  // stage layout: [A hi 16K][B hi b_bytes][A lo 16K][B lo b_bytes]
+  const int off_b = kATileBytes, off_a_lo = kATileBytes + args.b_bytes, off_b_lo = 2 * kATileBytes + args.b_bytes;
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < args.stages; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], 1); }
+    for (int a = 0; a < 2; ++a) { mbar_init(&tfull_bar[a], 1); mbar_init(&tempty_bar[a], 4); }
+    for (int r = 0; r < kRing; ++r) { mbar_init(&cmd_full[r], 1); mbar_init(&cmd_empty[r], 5); }
+    for (int w = 0; w < 4; ++w) { mbar_init(&cin_bar[w][0], 1); mbar_init(&cin_bar[w][1], 1); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  if (warp == 1) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_base_s)),
+                 "r"(kTmemCols)
+                 : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = tmem_base_s;
+
+  if (warp == 0) {
+    // ===================== scheduler + TMA producer =====================
+    if (lane == 0) {
+      int stage = 0, slot = 0;
+      uint32_t phase = 0, ring_phase = 0;
+      const int T = args.mt * args.ntl;
+      const int limit = pg.fixed_iter > 0 ? min(pg.fixed_iter, pg.max_iter) : pg.max_iter;
+      const int n_groups = (args.count + pg.group - 1) / pg.group;
+      for (int g = 0; g < n_groups; ++g) {
+        const int gbase = g * pg.group;
+        const int gs = min(pg.group, args.count - gbase);
+        const int per_seg = gs * T;
+        const int64_t total = (int64_t)limit * pg.n_ops * per_seg;
+        int k_checked = 0;
+        for (int64_t L = blockIdx.x; L < total; L += gridDim.x) {
+          const int seg = (int)(L / per_seg), rem = (int)(L % per_seg);
+          const int k = seg / pg.n_ops, op = seg % pg.n_ops;
+          if (k != k_checked) {   // whole group converged: go to the next group
+            if (ld_acquire(&args.group_active[g]) == 0) break;
+            k_checked = k;
+          }
+          const int ml = rem / T, t = rem % T;
+          const int m = gbase + ml;
+          const int n = args.dims[m];
+          const int n16 = (n + 15) & ~15;
+          const int m0 = (t % args.mt) * NOLSM_TILE_M, n0 = (t / args.mt) * args.bn;
+          if (m0 >= n || n0 >= n16) continue;          // tile outside this submatrix
+          const int need = k * pg.n_ops + op;          // ops of this submatrix that must be complete
+          if (need > 0) {
+            int32_t r = ld_acquire(&args.ready[m]);
+            while (r < need) { __nanosleep(64); r = ld_acquire(&args.ready[m]); }
+            if (r == kDone) continue;                  // submatrix finished at an earlier iteration
+            fence_proxy_async();                       // other CTAs' generic-proxy writes -> our TMA reads
+          }
+          const ChainOp &o = pg.ops[op];
+          const int par = k & 1;
+          const int nt = min(args.bn, n16 - n0);
+          const int kblocks = (n16 + kBK - 1) / kBK;
+          // command to the other roles
+          mbar_wait(&cmd_empty[slot], ring_phase ^ 1u);
+          cmds[slot] = TileCmd{m, m0, n0, nt, kblocks, (n16 - (kblocks - 1) * kBK) / 16, op, k};
+          mbar_arrive(&cmd_full[slot]);
+          if (++slot == kRing) { slot = 0; ring_phase ^= 1u; }
+          // operand loads
+          const bool split = o.a_lo[par] >= 0;
+          const int nbox = (nt + 63) >> 6;
+          const uint32_t bytes = (uint32_t)(kATileBytes + nbox * kBoxBytes) * (split ? 2u : 1u);
+          const CUtensorMap *ma = &args.maps[o.a[par]], *mb = &args.maps[o.b[par]];
+          const CUtensorMap *mal = split ? &args.maps[o.a_lo[par]] : nullptr;
+          const CUtensorMap *mbl = split ? &args.maps[o.b_lo[par]] : nullptr;
+          for (int kb = 0; kb < kblocks; ++kb) {
+            mbar_wait(&empty_bar[stage], phase ^ 1u);
+            uint8_t *st = smem + (size_t)stage * args.stage_bytes;
+            mbar_expect_tx(&full_bar[stage], bytes);
+            const int k0 = kb * kBK;
+            tma_load_3d(st, ma, &full_bar[stage], m0, k0, m);
+            tma_load_3d(st + kBoxBytes, ma, &full_bar[stage], m0 + 64, k0, m);
+            for (int j = 0; j < nbox; ++j)
+              tma_load_3d(st + off_b + j * kBoxBytes, mb, &full_bar[stage], k0, n0 + 64 * j, m);
+            if (split) {
+              tma_load_3d(st + off_a_lo, mal, &full_bar[stage], m0, k0, m);
+              tma_load_3d(st + off_a_lo + kBoxBytes, mal, &full_bar[stage], m0 + 64, k0, m);
+              for (int j = 0; j < nbox; ++j)
+                tma_load_3d(st + off_b_lo + j * kBoxBytes, mbl, &full_bar[stage], k0, n0 + 64 * j, m);
+            }
+            if (++stage == args.stages) { stage = 0; phase ^= 1u; }
+          }
+        }
+      }
+      mbar_wait(&cmd_empty[slot], ring_phase ^ 1u);
+      cmds[slot] = TileCmd{0, 0, 0, 0, 0, 0, -1, 0};
+      mbar_arrive(&cmd_full[slot]);
+    }
+  } else if (warp == 1) {
+    // ===================== MMA issuer =====================
+    if (lane == 0) {
+      int stage = 0, slot = 0, acc = 0;
+      uint32_t phase = 0, ring_phase = 0, acc_phase = 0;
+      for (;;) {
+        mbar_wait(&cmd_full[slot], ring_phase);
+        const TileCmd c = cmds[slot];
+        mbar_arrive(&cmd_empty[slot]);
+        if (++slot == kRing) { slot = 0; ring_phase ^= 1u; }
+        if (c.op < 0) break;
+        const bool split = pg.ops[c.op].a_lo[c.iter & 1] >= 0;
+        // instruction descriptor: D=F32, A=B=F16, A M-major, B K-major, N = nt, M = 128
+        const uint32_t idesc = (1u << 4) | (1u << 15) | ((uint32_t)(c.nt >> 3) << 17) | ((128u >> 4) << 24);
+        mbar_wait(&tempty_bar[acc], acc_phase ^ 1u);
+        tc_fence_after();
+        const uint32_t d_main = tmem_base + (uint32_t)(acc * 256);
+        const uint32_t d_corr = d_main + 128;
+        for (int kb = 0; kb < c.kblocks; ++kb) {
+          mbar_wait(&full_bar[stage], phase);
+          tc_fence_after();
+          const uint32_t sa = smem_u32(smem + (size_t)stage * args.stage_bytes);
+          const int steps = kb == c.kblocks - 1 ? c.ktail : kBK / 16;
+          for (int k4 = 0; k4 < steps; ++k4) {
+            // A (M-major): 16 K-rows of 128 B per MMA -> +2048 B; B (K-major): 16 K elements -> +32 B
+            const uint64_t ad = make_smem_desc(sa + k4 * 2048, kBoxBytes, 1024);
+            const uint64_t bd = make_smem_desc(sa + off_b + k4 * 32, 16, 1024);
+            const uint32_t accum = (kb | k4) ? 1u : 0u;
+            tc_mma_f16(d_main, ad, bd, idesc, accum);
+            if (split) {
+              const uint64_t adl = make_smem_desc(sa + off_a_lo + k4 * 2048, kBoxBytes, 1024);
+              const uint64_t bdl = make_smem_desc(sa + off_b_lo + k4 * 32, 16, 1024);
+              tc_mma_f16(d_corr, ad, bdl, idesc, accum);
+              tc_mma_f16(d_corr, adl, bd, idesc, 1u);
+            }
+          }
+          tc_commit(&empty_bar[stage]);
+          if (++stage == args.stages) { stage = 0; phase ^= 1u; }
+        }
+        tc_commit(&tfull_bar[acc]);
+        if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
+      }
+    }
+  } else {
+    // ===================== epilogue =====================
+    const int q = warp & 3;          // TMEM lane quadrant this warp may access
+    int slot = 0, acc = 0;
+    uint32_t ring_phase = 0, acc_phase = 0, cin_phase[2] = {0u, 0u};
+    float *cin_s = reinterpret_cast<float *>(epi_smem + (size_t)q * 8192);
+    const int limit = pg.fixed_iter > 0 ? min(pg.fixed_iter, pg.max_iter) : pg.max_iter;
+    for (;;) {
+      mbar_wait(&cmd_full[slot], ring_phase);
+      const TileCmd c = cmds[slot];
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&cmd_empty[slot]);
+      if (++slot == kRing) { slot = 0; ring_phase ^= 1u; }
+      if (c.op < 0) break;
+      const ChainOp &o = pg.ops[c.op];
+      const int par = c.iter & 1;
+      const int n = args.dims[c.mat];
+      const int r = c.m0 + q * 32 + lane;
+      const int64_t base = (int64_t)c.mat * args.slab + r;
+      const bool split = o.a_lo[par] >= 0;
+      const bool ident = o.mode == EPI_IDENT;
+      const bool has_cin = !ident && o.cin32 >= 0 && o.beta != 0.f;
+      const float alpha = o.use_div ? o.alpha / args.alpha_div[c.mat] : o.alpha;
+      float *cout32 = o.cout32 >= 0 ? args.ubuf[o.cout32] : nullptr;
+      __half *out16 = o.out16[par] >= 0 ? args.hbuf[o.out16[par]] : nullptr;
+      __half *out16_lo = o.out16_lo[par] >= 0 ? args.hbuf[o.out16_lo[par]] : nullptr;
+      const int nchunks = (c.nt + 31) >> 5;
+      const CUtensorMap *mc = has_cin ? &args.maps[args.n_half + o.cin32] : nullptr;
+      if (has_cin && lane == 0) {   // prefetch the first two FP32 chunks of this warp's 32 rows
+        fence_proxy_async();
+        for (int ci = 0; ci < min(2, nchunks); ++ci) {
+          mbar_expect_tx(&cin_bar[q][ci], 4096u);
+          tma_load_3d(cin_s + ci * 1024, mc, &cin_bar[q][ci], c.m0 + q * 32, c.n0 + ci * 32, c.mat);
+        }
+      }
+      mbar_wait(&tfull_bar[acc], acc_phase);
+      tc_fence_after();
+      const uint32_t t_main = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(acc * 256);
+      float ss = 0.f;
+      for (int ci = 0; ci < nchunks; ++ci) {
+        const int c0 = ci * 32;
+        uint32_t v[32];
+        tc_ld32(t_main + c0, v);
+        tc_ld_wait();
+        if (split) {
+          uint32_t w[32];
+          tc_ld32(t_main + 128 + c0, w);
+          tc_ld_wait();
+#pragma unroll
+          for (int j = 0; j < 32; ++j)
+            v[j] = __float_as_uint(fmaf(__uint_as_float(w[j]), 1.f / 2048.f, __uint_as_float(v[j])));
+        }
+        if (has_cin) {
+          const int bi = ci & 1;
+          mbar_wait(&cin_bar[q][bi], cin_phase[bi]);
+          cin_phase[bi] ^= 1u;
+          const float *cs = cin_s + bi * 1024 + lane;
+#pragma unroll
+          for (int j = 0; j < 32; ++j)
+            v[j] = __float_as_uint(fmaf(o.beta, cs[j * 32], alpha * __uint_as_float(v[j])));
+          __syncwarp();
+          if (lane == 0 && ci + 2 < nchunks) {
+            mbar_expect_tx(&cin_bar[q][bi], 4096u);
+            tma_load_3d(cin_s + bi * 1024, mc, &cin_bar[q][bi], c.m0 + q * 32, c.n0 + c0 + 64, c.mat);
+          }
+        } else if (ident) {
+#pragma unroll
+          for (int j = 0; j < 32; ++j) {
+            const int cc = c.n0 + c0 + j;
+            const float e = ((r == cc) ? 1.f : 0.f) - __uint_as_float(v[j]);
+            if (r < n && cc < n && c0 + j < c.nt) ss = fmaf(e, e, ss);
+            v[j] = __float_as_uint(e);
+          }
+        } else {
+#pragma unroll
+          for (int j = 0; j < 32; ++j) v[j] = __float_as_uint(alpha * __uint_as_float(v[j]));
+        }
+#pragma unroll
+        for (int j = 0; j < 32; ++j) {
+          if (c0 + j < c.nt) {
+            const int64_t off = base + (int64_t)(c.n0 + c0 + j) * args.ld;
+            const float val = __uint_as_float(v[j]);
+            if (cout32) cout32[off] = val;
+            if (out16) {
+              const __half hi = __float2half_rn(val);
+              out16[off] = hi;
+              if (out16_lo) out16_lo[off] = __float2half_rn((val - __half2float(hi)) * 2048.f);
+            }
+          }
+        }
+      }
+      tc_fence_before();
+      fence_proxy_async();     // our generic-proxy stores -> later TMA reads (any CTA)
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&tempty_bar[acc]);
+      if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
+      if (o.resid) {
+        for (int d = 16; d > 0; d >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, d);
+        if (lane == 0) atomicAdd(&args.resid2[(size_t)(c.iter % NOLSM_MAX_RESID_SLOTS) * args.count + c.mat], ss);
+      }
+      if (lane == 0) {
+        // completion: 4 warp arrivals per tile; the last arrival of the op publishes it
+        const int n16 = (n + 15) & ~15;
+        const int tiles_m = ((n + NOLSM_TILE_M - 1) / NOLSM_TILE_M) * ((n16 + args.bn - 1) / args.bn);
+        const int need = c.iter * pg.n_ops + c.op;
+        __threadfence();
+        const int32_t old = atomicAdd(&args.tiles_done[c.mat], 1);
+        if (old + 1 == (need + 1) * tiles_m * 4) {
+          __threadfence();
+          const int k = c.iter;
+          if (o.resid) {
+            const float r2 = *reinterpret_cast<volatile float *>(
+                &args.resid2[(size_t)(k % NOLSM_MAX_RESID_SLOTS) * args.count + c.mat]);
+            const float res = sqrtf(fmaxf(r2, 0.f) / (float)n);
+            args.lastres[c.mat] = res;
+            args.iters[c.mat] = k + 1;
+            bool stop = pg.fixed_iter > 0 ? (k + 1 >= pg.fixed_iter) : ((res < pg.tol) || !(res == res));
+            if (k + 1 >= pg.max_iter) stop = true;
+            if (stop) *reinterpret_cast<volatile int32_t *>(&args.state[c.mat]) = k;
+          }
+          const int32_t stv = *reinterpret_cast<volatile int32_t *>(&args.state[c.mat]);
+          if (c.op == pg.n_ops - 1 && (stv == k || k + 1 >= limit)) {
+            st_release(&args.ready[c.mat], kDone);
+            __threadfence();
+            atomicSub(&args.group_active[c.mat / pg.group], 1);
+          } else {
+            st_release(&args.ready[c.mat], need + 1);
+          }
+        }
+      }
+    }
+  }
+
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) {
+    tc_fence_after();
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(kTmemCols) : "memory");
+  }
+}
+
+// Reset of the per-launch control state.
+__global__ void __launch_bounds__(256)
+k_chain_reset(int count, int group, int32_t *ready, int32_t *tiles_done, int32_t *state, int32_t *group_active,
+              float *resid2, int resid_elems, int32_t *iters, float *lastres, int touch_stats) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int stride = gridDim.x * blockDim.x;
+  for (int m = i; m < count; m += stride) {
+    ready[m] = 0;
+    tiles_done[m] = 0;
+    state[m] = 0x7fffffff;
+    if (touch_stats) { iters[m] = 0; lastres[m] = -1.f; }
+  }
+  const int n_groups = (count + group - 1) / group;
+  for (int g = i; g < n_groups; g += stride) group_active[g] = min(group, count - g * group);
+  for (int e = i; e < resid_elems; e += stride) resid2[e] = 0.f;
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *,
+                                  CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
+                                  CUtensorMapFloatOOBfill);
+
+// stored matrix: dim0 = row index (contiguous), dim1 = column index, dim2 = submatrix
+nolsm_status encode_map(nolsm_ctx *ctx, CUtensorMap *map, void *ptr, bool half, int ld, int count) {
+  const size_t es = half ? sizeof(__half) : sizeof(float);
+  cuuint64_t dims[3] = {(cuuint64_t)ld, (cuuint64_t)ld, (cuuint64_t)count};
+  cuuint64_t strides[2] = {(cuuint64_t)ld * es, (cuuint64_t)ld * ld * es};
+  cuuint32_t box[3] = {half ? 64u : 32u, half ? 64u : 32u, 1};
+  cuuint32_t estr[3] = {1, 1, 1};
+  CUresult r = reinterpret_cast<EncodeTiledFn>(ctx->encode_tiled)(
+      map, half ? CU_TENSOR_MAP_DATA_TYPE_FLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, ptr, dims, strides, box,
+      estr, CU_TENSOR_MAP_INTERLEAVE_NONE, half ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE,
+      CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) {
+    ctx->err = "cuTensorMapEncodeTiled failed with CUresult " + std::to_string((int)r);
+    return NOLSM_ECUDA;
+  }
+  return NOLSM_OK;
+}
+
+}  // namespace
+
+nolsm_status umma_init(nolsm_ctx *ctx) {
+  ctx->umma_ok = false;
+  cudaDriverEntryPointQueryResult qres;
+  void *fn = nullptr;
+  cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
+  if (e != cudaSuccess || fn == nullptr || qres != cudaDriverEntryPointSuccess) {
+    ctx->err = "cuTensorMapEncodeTiled entry point not available";
+    cudaGetLastError();
+    return NOLSM_ECUDA;
+  }
+  ctx->encode_tiled = fn;
+  e = cudaFuncSetAttribute(k_chain, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit);
+  if (e != cudaSuccess) {
+    ctx->err = std::string("cudaFuncSetAttribute(k_chain): ") + cudaGetErrorString(e);
+    cudaGetLastError();
+    return NOLSM_ECUDA;
+  }
+  int coop = 0;
+  cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, ctx->device);
+  if (!coop) {
+    ctx->err = "device does not support cooperative launches";
+    return NOLSM_ECUDA;
+  }
+  ctx->umma_ok = true;
+  return NOLSM_OK;
+}
+
+nolsm_status umma_make_maps(nolsm_ctx *ctx, nolsm_batch *b) {
+  b->maps_valid = false;
+  if (!ctx->umma_ok || b->count == 0) return NOLSM_OK;
+  std::vector<CUtensorMap> maps(b->n_half + b->n_unit);
+  for (int i = 0; i < b->n_half; ++i) {
+    nolsm_status s = encode_map(ctx, &maps[i], b->h[i], true, b->ld, b->count);
+    if (s != NOLSM_OK) return s;
+  }
+  for (int i = 0; i < b->n_unit; ++i) {
+    nolsm_status s = encode_map(ctx, &maps[b->n_half + i], b->u[i], false, b->ld, b->count);
+    if (s != NOLSM_OK) return s;
+  }
+  if (!b->d_maps) {
+    if (cudaMalloc(&b->d_maps, sizeof(CUtensorMap) * (NOLSM_MAX_HALF + NOLSM_MAX_UNIT)) != cudaSuccess) {
+      cudaGetLastError();
+      ctx->err = "cudaMalloc of the tensor maps failed";
+      return NOLSM_ENOMEM;
+    }
+  }
+  NOLSM_CUDA(ctx, cudaMemcpy(b->d_maps, maps.data(), sizeof(CUtensorMap) * maps.size(), cudaMemcpyHostToDevice));
+  b->maps_valid = true;
+  return NOLSM_OK;
+}
+
+// Runs `prog` over every submatrix of the batch.  touch_stats: reset and fill iters / lastres.
+cudaError_t launch_chain(nolsm_ctx *ctx, const nolsm_batch *b, const ChainProgram &prog, const float *alpha_div,
+                         bool touch_stats, cudaStream_t st) {
+  if (b->count == 0) return cudaSuccess;
+  if (!ctx->umma_ok || !b->maps_valid) return cudaErrorNotSupported;
+  ChainArgs a;
+  memset(&a, 0, sizeof(a));
+  a.prog = prog;
+  bool split = false;
+  for (int i = 0; i < prog.n_ops; ++i) split |= prog.ops[i].a_lo[0] >= 0 || prog.ops[i].a_lo[1] >= 0;
+  const int n16max = (b->max_n + 15) & ~15;
+  a.bn = std::min(split ? 128 : 256, n16max);
+  a.b_bytes = ((a.bn + 63) / 64) * kBoxBytes;
+  a.stage_bytes = (kATileBytes + a.b_bytes) * (split ? 2 : 1);
+  a.stages = std::min(kMaxStages, (kSmemLimit - 1024 - kEpiBytes) / a.stage_bytes);
+  a.mt = (b->max_n + NOLSM_TILE_M - 1) / NOLSM_TILE_M;
+  a.ntl = (n16max + a.bn - 1) / a.bn;
+  a.maps = b->d_maps;
+  a.n_half = b->n_half;
+  for (int i = 0; i < b->n_half; ++i) a.hbuf[i] = b->h[i];
+  for (int i = 0; i < b->n_unit; ++i) a.ubuf[i] = b->u[i];
+  a.count = b->count;
+  a.ld = b->ld;
+  a.slab = (int64_t)b->ld * b->ld;
+  a.dims = b->d_dims;
+  a.alpha_div = alpha_div;
+  a.ready = b->d_ready;
+  a.tiles_done = b->d_tiles_done;
+  a.state = b->d_state;
+  a.iters = b->d_iters;
+  a.group_active = b->d_group_active;
+  a.resid2 = b->d_resid2;
+  a.lastres = b->d_lastres;
+  if (a.prog.group <= 0) a.prog.group = 1;
+  const int slots = std::min(prog.max_iter, NOLSM_MAX_RESID_SLOTS);
+  k_chain_reset<<<64, 256, 0, st>>>(b->count, a.prog.group, a.ready, a.tiles_done, a.state, a.group_active,
+                                    a.resid2, slots * b->count, a.iters, a.lastres, touch_stats ? 1 : 0);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  const int smem_bytes = a.stages * a.stage_bytes + kEpiBytes + 1024;
+  void *params[] = {&a};
+  return cudaLaunchCooperativeKernel(reinterpret_cast<void *>(k_chain), dim3(ctx->sm_count), dim3(kThreads), params,
+                                     (size_t)smem_bytes, st);
+}

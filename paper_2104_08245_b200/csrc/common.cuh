@@ -16,6 +16,8 @@
 #define NOLSM_TILE_M 128          // rows per output tile (UMMA M, one CTA)
 #define NOLSM_PAD 128             // leading dimensions are multiples of this
 #define NOLSM_MAX_RESID_SLOTS 64  // residual history kept per submatrix
+#define NOLSM_MAX_HALF 10         // FP16 operand buffers of a batch (6 in FP16 mode, 10 in FP32 mode)
+#define NOLSM_MAX_UNIT 9          // FP32 buffers of a batch (the FP16 buffers alias units 4..)
 
 struct TileDesc {                 // one output tile of one submatrix
   int32_t mat;                    // index inside the batch
@@ -45,9 +47,30 @@ struct GemmParams {
   float *resid2;                  // IDENT: per-submatrix sum of squares of the output (atomicAdd)
 };
 
+// One product of a chain (chain_umma.cu).  Buffer indices refer to the batch's FP16 buffers h[] and
+// FP32 units u[]; entries indexed by the iteration parity implement the ping-pong of the iterates.
+struct ChainOp {
+  int32_t a[2], b[2];             // FP16 operands (hi parts), by iteration parity
+  int32_t a_lo[2], b_lo[2];       // lo parts of split operands (FP32-quality product), -1: plain FP16
+  int32_t out16[2], out16_lo[2];  // FP16 copy of the result (hi [, lo * 2^11]), -1: none
+  int32_t cin32, cout32;          // FP32 units read (AXPBY, beta != 0) / written, -1: none
+  int32_t mode;                   // EPI_IDENT: I - A B     EPI_AXPBY: beta * Cin + alpha * A B
+  int32_t resid;                  // 1: ||result||_F^2 over the true n x n part drives the stop rule
+  int32_t use_div;                // alpha /= alpha_div[submatrix]
+  float alpha, beta;
+};
+
+struct ChainProgram {
+  ChainOp ops[3];
+  int32_t n_ops;                  // products per iteration, strictly ordered per submatrix
+  int32_t max_iter, fixed_iter;   // fixed_iter > 0: exactly that many iterations, no residual test
+  float tol;                      // stop rule of DESIGN.md reading 9 on the residual of the `resid` op
+  int32_t group;                  // submatrices iterated together (L2 residency)
+};
+
 struct nolsm_batch {
   int32_t count = 0, ld = 0, mol_begin = 0, max_n = 0, slot = 0;
-  int32_t bn = 128;               // tile width of the tcgen05 path for this batch
+  bool engine_simt = false;       // prepared by the FP32 SIMT debugging path (different buffer roles)
   bool sparse = true;             // false: dense microbench batch (no neighbour list)
   bool prepared = false;          // S^-1 and B available
   int32_t prepared_precision = -1;
@@ -64,17 +87,19 @@ struct nolsm_batch {
   float *d_scale = nullptr;       // [count] s_j of the sign scaling
   float *d_norm = nullptr;        // [2][count] scratch for norm bounds
   int32_t *d_active = nullptr;    // [NOLSM_MAX_RESID_SLOTS] active counters per iteration
-  TileDesc *d_tiles = nullptr;    // tile list (bn-wide tiles)
-  int32_t n_tiles = 0;
   TileDesc *d_tiles_simt = nullptr; // 128x128 tiles for the SIMT kernel
   int32_t n_tiles_simt = 0;
   size_t meta_cap = 0;            // capacity (in submatrices) of the metadata arrays
-  size_t tiles_cap = 0, tiles_simt_cap = 0;
+  size_t tiles_simt_cap = 0;
   double sum_n3 = 0.0, sum_n3_padded = 0.0;
   // logical buffers (set by layout_batch): fp32 units u[0..6], fp16 halves h[0..5] alias units 4..6
-  float *u[7] = {nullptr};
-  __half *h[6] = {nullptr};
-  CUtensorMap map_a[6], map_b[6]; // per fp16 buffer: A-role box {64,64,1}, B-role box {64,bn,1}
+  float *u[NOLSM_MAX_UNIT] = {nullptr};
+  __half *h[NOLSM_MAX_HALF] = {nullptr};
+  int32_t n_half = 6, n_unit = 7; // buffers laid out in this batch (precision dependent)
+  int32_t *d_ready = nullptr;     // [count] chain engine: ops completed per submatrix
+  int32_t *d_tiles_done = nullptr;// [count] chain engine: epilogue-warp arrivals per submatrix
+  int32_t *d_group_active = nullptr; // [count] chain engine: unfinished submatrices per group
+  CUtensorMap *d_maps = nullptr;  // device array: n_half FP16 maps {64,64,1}, then n_unit FP32 maps {32,32,1}
   bool maps_valid = false;
 };
 
@@ -129,9 +154,10 @@ cudaError_t launch_trace(const nolsm_batch *b, const int32_t *row_ptr, const int
 cudaError_t launch_norm_bound(const nolsm_batch *b, const float *a, float mu, float *norm2,
                               cudaStream_t st);
 cudaError_t launch_init_inverse(const nolsm_batch *b, const float *s, const float *norm2, float *y32,
-                                float *z32, __half *y16, __half *z16, float *scale_out, cudaStream_t st);
+                                float *z32, __half *y16, __half *z16, __half *y16_lo, __half *z16_lo,
+                                float *scale_out, cudaStream_t st);
 cudaError_t launch_make_x0(const nolsm_batch *b, const float *bmat, float mu, const float *norm2,
-                           const float *scale_in, float *x32, __half *x16, float *scale_out,
+                           const float *scale_in, float *x32, __half *x16, __half *x16_lo, float *scale_out,
                            cudaStream_t st);
 cudaError_t launch_scale_copy(const nolsm_batch *b, const float *src, const float *scale, int invert,
                               float *dst32, __half *dst16, __half *dst16_lo, cudaStream_t st);
@@ -145,6 +171,5 @@ cudaError_t launch_gemm_simt(const GemmParams &p, cudaStream_t st);
 // tcgen05 path
 nolsm_status umma_init(nolsm_ctx *ctx);
 nolsm_status umma_make_maps(nolsm_ctx *ctx, nolsm_batch *b);
-// kind: 1 = FP16 operands; 2 = split FP16 (hi/lo operands, FP32-quality)
-cudaError_t launch_gemm_umma(nolsm_ctx *ctx, const nolsm_batch *b, int kind, int a_buf, int b_buf,
-                             int a_lo_buf, int b_lo_buf, const GemmParams &p, cudaStream_t st);
+cudaError_t launch_chain(nolsm_ctx *ctx, const nolsm_batch *b, const ChainProgram &prog, const float *alpha_div,
+                         bool touch_stats, cudaStream_t st);

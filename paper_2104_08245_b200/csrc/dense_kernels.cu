@@ -68,7 +68,7 @@ __global__ void __launch_bounds__(256)
 k_init_inverse(const int32_t *__restrict__ dims, int ld, int64_t slab, int count,
                const float *__restrict__ s, const float *__restrict__ norm2, float *__restrict__ y32,
                float *__restrict__ z32, __half *__restrict__ y16, __half *__restrict__ z16,
-               float *__restrict__ scale_out) {
+               __half *__restrict__ y16_lo, __half *__restrict__ z16_lo, float *__restrict__ scale_out) {
   const int mat = blockIdx.z;
   const int n = dims[mat];
   const int P = padded_dim(n);
@@ -81,16 +81,25 @@ k_init_inverse(const int32_t *__restrict__ dims, int ld, int64_t slab, int count
   const float y = s[off] / sc;
   const float z = (r == c) ? 1.f : 0.f;
   if (y32) { y32[off] = y; z32[off] = z; }
-  if (y16) { y16[off] = __float2half_rn(y); z16[off] = __float2half_rn(z); }
+  if (y16) {
+    const __half yh = __float2half_rn(y);
+    y16[off] = yh;
+    z16[off] = __float2half_rn(z);
+    if (y16_lo) {   // split operands of the FP32-quality products: value = hi + lo / 2^11
+      y16_lo[off] = __float2half_rn((y - __half2float(yh)) * 2048.f);
+      z16_lo[off] = __float2half_rn(0.f);
+    }
+  }
 }
 
 cudaError_t launch_init_inverse(const nolsm_batch *b, const float *s, const float *norm2, float *y32,
-                                float *z32, __half *y16, __half *z16, float *scale_out, cudaStream_t st) {
+                                float *z32, __half *y16, __half *z16, __half *y16_lo, __half *z16_lo,
+                                float *scale_out, cudaStream_t st) {
   if (b->count == 0) return cudaSuccess;
   const int P = round_up(b->max_n, NOLSM_TILE_M);
   dim3 grid((P + 255) / 256, P, b->count);
   k_init_inverse<<<grid, 256, 0, st>>>(b->d_dims, b->ld, (int64_t)b->ld * b->ld, b->count, s, norm2,
-                                       y32, z32, y16, z16, scale_out);
+                                       y32, z32, y16, z16, y16_lo, z16_lo, scale_out);
   return cudaGetLastError();
 }
 
@@ -103,7 +112,7 @@ __global__ void __launch_bounds__(256)
 k_make_x0(const int32_t *__restrict__ dims, int ld, int64_t slab, int count,
           const float *__restrict__ bmat, float mu, const float *__restrict__ norm2,
           const float *__restrict__ scale_in, float *__restrict__ x32, __half *__restrict__ x16,
-          float *__restrict__ scale_out) {
+          __half *__restrict__ x16_lo, float *__restrict__ scale_out) {
   const int mat = blockIdx.z;
   const int n = dims[mat];
   const int P = padded_dim(n);
@@ -123,17 +132,21 @@ k_make_x0(const int32_t *__restrict__ dims, int ld, int64_t slab, int count,
     v = (r == c) ? 1.f : 0.f;
   }
   if (x32) x32[off] = v;
-  if (x16) x16[off] = __float2half_rn(v);
+  if (x16) {
+    const __half hi = __float2half_rn(v);
+    x16[off] = hi;
+    if (x16_lo) x16_lo[off] = __float2half_rn((v - __half2float(hi)) * 2048.f);
+  }
 }
 
 cudaError_t launch_make_x0(const nolsm_batch *b, const float *bmat, float mu, const float *norm2,
-                           const float *scale_in, float *x32, __half *x16, float *scale_out,
+                           const float *scale_in, float *x32, __half *x16, __half *x16_lo, float *scale_out,
                            cudaStream_t st) {
   if (b->count == 0) return cudaSuccess;
   const int P = round_up(b->max_n, NOLSM_TILE_M);
   dim3 grid((P + 255) / 256, P, b->count);
   k_make_x0<<<grid, 256, 0, st>>>(b->d_dims, b->ld, (int64_t)b->ld * b->ld, b->count, bmat, mu, norm2,
-                                  scale_in, x32, x16, scale_out);
+                                  scale_in, x32, x16, x16_lo, scale_out);
   return cudaGetLastError();
 }
 
