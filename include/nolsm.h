@@ -89,6 +89,7 @@ typedef struct {            /* filled by nolsm_sign_batched (host struct) */
   double flops_prepare;     /* Eq. 15-17, refinement and B = S^-1 H, if this call ran them */
   int32_t inv_iter_max;     /* Eq. 15-17 iterations executed (0 if the batch was already prepared) */
   float inv_worst_residual;
+  float ms_chain;           /* CUDA-event time of the sign-iteration kernel alone (all iterations of the batch) */
 } nolsm_sign_stats;
 
 typedef struct {            /* filled by nolsm_solve_mu (host struct) */
@@ -101,6 +102,8 @@ typedef struct {            /* filled by nolsm_solve_mu (host struct) */
   double flops_sign_total;  /* over all mu steps */
   double flops_prepare_total;
   float ms_gather, ms_prepare, ms_sign, ms_density; /* CUDA-event times summed over batches and steps */
+  float ms_chain;           /* of ms_sign: the sign-iteration kernel alone (without norm bound and X0) */
+  int32_t chain_launches;   /* launches of that kernel behind ms_chain */
 } nolsm_solve_stats;
 
 /* Context.  `cfg` may be NULL (defaults).  Returns NOLSM_ECUDA when no device is usable. */

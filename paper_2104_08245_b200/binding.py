@@ -45,7 +45,7 @@ class SignStats(C.Structure):
     _fields_ = [("n_sub", C.c_int32), ("iter_min", C.c_int32), ("iter_max", C.c_int32), ("iter_sum", C.c_int64),
                 ("n_unconverged", C.c_int32), ("worst_residual", C.c_float), ("gemms", C.c_int64),
                 ("flops_sign", C.c_double), ("flops_sign_padded", C.c_double), ("flops_prepare", C.c_double),
-                ("inv_iter_max", C.c_int32), ("inv_worst_residual", C.c_float)]
+                ("inv_iter_max", C.c_int32), ("inv_worst_residual", C.c_float), ("ms_chain", C.c_float)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
@@ -56,7 +56,7 @@ class SolveStats(C.Structure):
                 ("mu_lo", C.c_double), ("mu_hi", C.c_double), ("ne_diag", C.c_double), ("last", SignStats),
                 ("flops_sign_total", C.c_double), ("flops_prepare_total", C.c_double),
                 ("ms_gather", C.c_float), ("ms_prepare", C.c_float), ("ms_sign", C.c_float),
-                ("ms_density", C.c_float)]
+                ("ms_density", C.c_float), ("ms_chain", C.c_float), ("chain_launches", C.c_int32)]
 
     def as_dict(self):
         d = {k: getattr(self, k) for k, _ in self._fields_ if k != "last"}

@@ -79,6 +79,7 @@ extern "C" nolsm_status nolsm_create(nolsm_ctx **out, const nolsm_config *cfg) {
     return NOLSM_ENOMEM;
   }
   for (int i = 0; i < 4; ++i) cudaEventCreateWithFlags(&ctx->ev[i], cudaEventDisableTiming);
+  for (int i = 0; i < 2; ++i) cudaEventCreate(&ctx->tev[i]);
   if (prop.major == 10) {
     if (umma_init(ctx) != NOLSM_OK) g_create_err = ctx->err;
   } else {
@@ -117,6 +118,8 @@ extern "C" void nolsm_destroy(nolsm_ctx *ctx) {
   cudaFreeHost(ctx->h_active);
   for (int i = 0; i < 4; ++i)
     if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
+  for (int i = 0; i < 2; ++i)
+    if (ctx->tev[i]) cudaEventDestroy(ctx->tev[i]);
   delete ctx;
 }
 
@@ -513,7 +516,8 @@ static nolsm_status prepare_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, int prec
 // E = I - X_k^2,  X_{k+1} = X_k + 1/2 X_k E  (reading 12); the residual of the stop rule
 // (reading 9) comes out of the first product's epilogue.  One kernel launch for all iterations.
 static nolsm_status sign_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, double mu, int precision, float tol,
-                                     int max_iter, int fixed_iter, const float *scale_in, cudaStream_t st) {
+                                     int max_iter, int fixed_iter, const float *scale_in, cudaStream_t st,
+                                     bool timed) {
   const bool fp16 = precision == NOLSM_FP16_FP32;
   float *Bm = b->u[3], *X32 = b->u[0];
   if (!scale_in) LAUNCH(ctx, launch_norm_bound(b, Bm, (float)mu, b->d_norm, st));
@@ -542,7 +546,10 @@ static nolsm_status sign_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, double mu, 
     set2(x.a, 0, 2); set2(x.a_lo, 1, 3); set2(x.b, 4, 4); set2(x.b_lo, 5, 5);
     set2(x.out16, 2, 0); set2(x.out16_lo, 3, 1);
   }
-  return run_chain(ctx, b, pg, nullptr, true, st);
+  if (timed) NOLSM_CUDA(ctx, cudaEventRecord(ctx->tev[0], st));
+  CHECK(run_chain(ctx, b, pg, nullptr, true, st));
+  if (timed) NOLSM_CUDA(ctx, cudaEventRecord(ctx->tev[1], st));
+  return NOLSM_OK;
 }
 
 // ---- debugging path: every product on the FP32 SIMT kernel (NOLSM_FLAG_SIMT_ONLY) ----
@@ -682,10 +689,18 @@ static nolsm_status prepare_batch(nolsm_ctx *ctx, nolsm_batch *b, int precision,
   return prepare_batch_chain(ctx, b, precision, st, stats, gemms);
 }
 
+// timed: records ctx->tev[0..1] around the chain kernel; read with chain_ms() after a synchronise
 static nolsm_status sign_batch(nolsm_ctx *ctx, nolsm_batch *b, double mu, int precision, float tol, int max_iter,
-                               int fixed_iter, const float *scale_in, cudaStream_t st) {
+                               int fixed_iter, const float *scale_in, cudaStream_t st, bool timed) {
   if (b->engine_simt) return sign_batch_simt(ctx, b, mu, tol, max_iter, fixed_iter, scale_in, st);
-  return sign_batch_chain(ctx, b, mu, precision, tol, max_iter, fixed_iter, scale_in, st);
+  return sign_batch_chain(ctx, b, mu, precision, tol, max_iter, fixed_iter, scale_in, st, timed);
+}
+
+static float chain_ms(nolsm_ctx *ctx, const nolsm_batch *b) {
+  float ms = 0.f;
+  if (b->engine_simt || b->count == 0) return 0.f;
+  if (cudaEventElapsedTime(&ms, ctx->tev[0], ctx->tev[1]) != cudaSuccess) { cudaGetLastError(); return 0.f; }
+  return ms;
 }
 
 static float *sinv_ptr(const nolsm_batch *b) { return b->engine_simt ? b->u[4] : b->u[2]; }
@@ -747,7 +762,7 @@ extern "C" nolsm_status nolsm_sign_batched(nolsm_ctx *ctx, nolsm_batch *batch, d
     if (batch->prepared) { ctx->err = "batch was prepared in another precision; gather it again"; return NOLSM_EINVAL; }
     CHECK(prepare_batch(ctx, batch, prec, st, stats, &gemms));
   }
-  CHECK(sign_batch(ctx, batch, mu, prec, tol, max_iter, fixed_iter, nullptr, st));
+  CHECK(sign_batch(ctx, batch, mu, prec, tol, max_iter, fixed_iter, nullptr, st, stats != nullptr));
   if (stats) {
     const int inv_it = stats->inv_iter_max;
     const float inv_res = stats->inv_worst_residual;
@@ -757,6 +772,7 @@ extern "C" nolsm_status nolsm_sign_batched(nolsm_ctx *ctx, nolsm_batch *batch, d
     stats->inv_worst_residual = inv_res;
     stats->flops_prepare = fp;
     stats->gemms = gemms + 2 * stats->iter_sum;
+    stats->ms_chain = chain_ms(ctx, batch);
   }
   return NOLSM_OK;
 }
@@ -873,7 +889,7 @@ extern "C" nolsm_status nolsm_solve_mu(nolsm_ctx *ctx, const nolsm_bsr *H, const
         if (rc != NOLSM_OK) break;
       }
       if (timed) cudaEventRecord(tev[2], st);
-      rc = sign_batch(ctx, b, mu, prec, tol, max_iter, fixed_iter, nullptr, st);
+      rc = sign_batch(ctx, b, mu, prec, tol, max_iter, fixed_iter, nullptr, st, timed);
       if (rc != NOLSM_OK) break;
       if (timed) cudaEventRecord(tev[3], st);
       rc = nolsm_scatter_density(ctx, b, S, D, ctx->d_scalars, q_mol, ctx->d_scalars + 1, st);
@@ -887,6 +903,8 @@ extern "C" nolsm_status nolsm_solve_mu(nolsm_ctx *ctx, const nolsm_bsr *H, const
         float ms[4];
         for (int i = 0; i < 4; ++i) cudaEventElapsedTime(&ms[i], tev[i], tev[i + 1]);
         stats->ms_gather += ms[0]; stats->ms_prepare += ms[1]; stats->ms_sign += ms[2]; stats->ms_density += ms[3];
+        stats->ms_chain += chain_ms(ctx, b);
+        stats->chain_launches += b->engine_simt ? 0 : 1;
         acc.n_sub += cs.n_sub;
         acc.iter_min = std::min(acc.iter_min, cs.iter_min);
         acc.iter_max = std::max(acc.iter_max, cs.iter_max);
@@ -1017,11 +1035,12 @@ extern "C" nolsm_status nolsm_sign_dense_batched(nolsm_ctx *ctx, const float *a,
   b->prepared_precision = prec;
   b->engine_simt = use_simt(ctx);
   LAUNCH(ctx, launch_pack(a, n, batch, b->ld, bmat_ptr(b), 0, st));
-  CHECK(sign_batch(ctx, b, 0.0, prec, tol, max_iter, fixed_iter, scale, st));
+  CHECK(sign_batch(ctx, b, 0.0, prec, tol, max_iter, fixed_iter, scale, st, stats != nullptr));
   LAUNCH(ctx, launch_unpack(x_ptr(b), b->ld, (int64_t)b->ld * b->ld, nullptr, nullptr, n, batch, x_out, st));
   if (stats) {
     CHECK(collect_stats(ctx, b, tol, fixed_iter, st, stats));
     stats->gemms = 2 * stats->iter_sum;
+    stats->ms_chain = chain_ms(ctx, b);
   }
   return NOLSM_OK;
 }

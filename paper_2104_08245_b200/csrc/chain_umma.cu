@@ -129,6 +129,28 @@ __device__ __forceinline__ uint64_t make_smem_desc(uint32_t saddr, uint32_t lbo_
   return d;
 }
 
+// Stores `cnt` (16 or 32) consecutive tile columns of one row held in v[]: FP32 master and / or FP16
+// operand copies (hi [, lo * 2^11]).  Column stride = ld elements; lanes hold consecutive rows, so
+// every store instruction of a warp writes one contiguous 128-byte (FP32) or 64-byte (FP16) segment.
+template <bool H32, bool H16, bool HLO>
+__device__ __forceinline__ void store_cols(const uint32_t (&v)[32], float *p32, __half *p16, __half *p16l, int ld,
+                                           bool full) {
+#pragma unroll
+  for (int half = 0; half < 2; ++half) {
+    if (half == 1 && !full) break;
+#pragma unroll
+    for (int jj = 0; jj < 16; ++jj) {
+      const float val = __uint_as_float(v[half * 16 + jj]);
+      if (H32) { *p32 = val; p32 += ld; }
+      if (H16) {
+        const __half hi = __float2half_rn(val);
+        *p16 = hi; p16 += ld;
+        if (HLO) { *p16l = __float2half_rn((val - __half2float(hi)) * 2048.f); p16l += ld; }
+      }
+    }
+  }
+}
+
 struct TileCmd {              // scheduler -> MMA issuer and epilogue warps
   int32_t mat, m0, n0, nt;    // submatrix, first row / column, tile columns (multiple of 16, <= bn)
   int32_t kblocks, ktail;     // K blocks of 64; K=16 steps in the last one (1..4)
@@ -334,15 +356,21 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
           tma_load_3d(cin_s + ci * 1024, mc, &cin_bar[q][ci], c.m0 + q * 32, c.n0 + ci * 32, c.mat);
         }
       }
+      const int64_t tile_off = base + (int64_t)c.n0 * args.ld;   // element (r, n0)
+      float *p32 = cout32 ? cout32 + tile_off : nullptr;
+      __half *p16 = out16 ? out16 + tile_off : nullptr;
+      __half *p16l = out16_lo ? out16_lo + tile_off : nullptr;
+      const int store_kind = (p32 ? 1 : 0) | (p16 ? 2 : 0) | (p16l ? 4 : 0);
+      const int64_t chunk_stride = (int64_t)32 * args.ld;
       mbar_wait(&tfull_bar[acc], acc_phase);
       tc_fence_after();
       const uint32_t t_main = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(acc * 256);
       float ss = 0.f;
       for (int ci = 0; ci < nchunks; ++ci) {
         const int c0 = ci * 32;
+        const bool full = c.nt - c0 >= 32;
         uint32_t v[32];
         tc_ld32(t_main + c0, v);
-        tc_ld_wait();
         if (split) {
           uint32_t w[32];
           tc_ld32(t_main + 128 + c0, w);
@@ -350,6 +378,8 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
 #pragma unroll
           for (int j = 0; j < 32; ++j)
             v[j] = __float_as_uint(fmaf(__uint_as_float(w[j]), 1.f / 2048.f, __uint_as_float(v[j])));
+        } else {
+          tc_ld_wait();
         }
         if (has_cin) {
           const int bi = ci & 1;
@@ -365,30 +395,30 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
             tma_load_3d(cin_s + bi * 1024, mc, &cin_bar[q][bi], c.m0 + q * 32, c.n0 + c0 + 64, c.mat);
           }
         } else if (ident) {
+          // valid columns of this chunk inside the true n x n part (residual of the stop rule)
+          const int nvalid = (r < n) ? min(full ? 32 : 16, n - (c.n0 + c0)) : 0;
+          const int dj = r - (c.n0 + c0);     // chunk column that holds the diagonal element of row r
 #pragma unroll
           for (int j = 0; j < 32; ++j) {
-            const int cc = c.n0 + c0 + j;
-            const float e = ((r == cc) ? 1.f : 0.f) - __uint_as_float(v[j]);
-            if (r < n && cc < n && c0 + j < c.nt) ss = fmaf(e, e, ss);
+            const float e = ((j == dj) ? 1.f : 0.f) - __uint_as_float(v[j]);
+            if (j < nvalid) ss = fmaf(e, e, ss);
             v[j] = __float_as_uint(e);
           }
         } else {
 #pragma unroll
           for (int j = 0; j < 32; ++j) v[j] = __float_as_uint(alpha * __uint_as_float(v[j]));
         }
-#pragma unroll
-        for (int j = 0; j < 32; ++j) {
-          if (c0 + j < c.nt) {
-            const int64_t off = base + (int64_t)(c.n0 + c0 + j) * args.ld;
-            const float val = __uint_as_float(v[j]);
-            if (cout32) cout32[off] = val;
-            if (out16) {
-              const __half hi = __float2half_rn(val);
-              out16[off] = hi;
-              if (out16_lo) out16_lo[off] = __float2half_rn((val - __half2float(hi)) * 2048.f);
-            }
-          }
+        switch (store_kind) {
+          case 1: store_cols<true, false, false>(v, p32, p16, p16l, args.ld, full); break;
+          case 2: store_cols<false, true, false>(v, p32, p16, p16l, args.ld, full); break;
+          case 3: store_cols<true, true, false>(v, p32, p16, p16l, args.ld, full); break;
+          case 6: store_cols<false, true, true>(v, p32, p16, p16l, args.ld, full); break;
+          case 7: store_cols<true, true, true>(v, p32, p16, p16l, args.ld, full); break;
+          default: break;
         }
+        if (p32) p32 += chunk_stride;
+        if (p16) p16 += chunk_stride;
+        if (p16l) p16l += chunk_stride;
       }
       tc_fence_before();
       fence_proxy_async();     // our generic-proxy stores -> later TMA reads (any CTA)

@@ -115,6 +115,7 @@ struct nolsm_ctx {
   double *h_scalars = nullptr;    // pinned mirror
   int32_t *h_active = nullptr;    // pinned [NOLSM_MAX_RESID_SLOTS]
   cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+  cudaEvent_t tev[2] = {nullptr, nullptr};   // timing of the sign-iteration chain kernel
   void *encode_tiled = nullptr;   // cuTensorMapEncodeTiled entry point
   bool umma_ok = false;
   // device mirrors of the caller's HOST store (nolsm_solve_mu_host), grown on demand
