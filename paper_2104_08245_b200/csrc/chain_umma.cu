@@ -22,23 +22,24 @@
 //     64 tile columns), 128-byte swizzle.
 //   * accumulator: 128 TMEM lanes = tile rows, one 32-bit column per tile column; two accumulator
 //     stages so the epilogue of tile i overlaps the MMAs of tile i+1.
-//   * the FP32 master iterate (reading 12) is read in the epilogue through per-warp TMA
-//     prefetches ({32 rows, 32 columns} FP32 boxes) and written back with coalesced stores.
+//   * the FP32 master iterate (reading 12) is read in the epilogue with L2-only loads
+//     (ld.global.cg: other SMs wrote it) issued one chunk ahead, and written back with coalesced stores.
 //
-// Warp roles (192 threads): warp 0 = scheduler + TMA producer, warp 1 = MMA issuer (+ TMEM
-// allocation), warps 2..5 = epilogue (TMEM lane quadrant = warp_id % 4).
+// Warp roles (320 threads): warp 0 = scheduler + TMA producer, warp 1 = MMA issuer (+ TMEM
+// allocation), warps 2..9 = epilogue (TMEM lane quadrant = warp_id % 4; the two warps of a quadrant
+// take alternate 32-column chunks of the tile).
 #include "common.cuh"
 
 namespace {
 
-constexpr int kThreads = 192;
+constexpr int kThreads = 320;
+constexpr int kEpiWarps = 8;
 constexpr int kBK = 64;                  // K elements per pipeline stage (= one 128-byte swizzle row)
 constexpr int kMaxStages = 8;
 constexpr int kTmemCols = 512;
 constexpr int kBoxBytes = 64 * 128;      // one {64 x 64} FP16 box
 constexpr int kATileBytes = 2 * kBoxBytes;
 constexpr int kRing = 4;                 // tile-command ring depth
-constexpr int kEpiBytes = 4 * 2 * 4096;  // per epilogue warp: two {32 x 32} FP32 boxes
 constexpr int kSmemLimit = 232448 - 2048;  // 227 KB minus the static part (barriers, commands)
 constexpr int32_t kDone = 0x7fffffff;
 
@@ -176,22 +177,20 @@ struct ChainArgs {
 __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   __shared__ uint64_t full_bar[kMaxStages], empty_bar[kMaxStages], tfull_bar[2], tempty_bar[2];
-  __shared__ uint64_t cmd_full[kRing], cmd_empty[kRing], cin_bar[4][2];
+  __shared__ uint64_t cmd_full[kRing], cmd_empty[kRing];
   __shared__ TileCmd cmds[kRing];
   __shared__ uint32_t tmem_base_s;
 
   const ChainProgram &pg = args.prog;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
-  uint8_t *epi_smem = smem + (size_t)args.stages * args.stage_bytes;
   // stage layout: [A hi 16K][B hi b_bytes][A lo 16K][B lo b_bytes]
   const int off_b = kATileBytes, off_a_lo = kATileBytes + args.b_bytes, off_b_lo = 2 * kATileBytes + args.b_bytes;
 
   if (threadIdx.x == 0) {
     for (int s = 0; s < args.stages; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], 1); }
-    for (int a = 0; a < 2; ++a) { mbar_init(&tfull_bar[a], 1); mbar_init(&tempty_bar[a], 4); }
-    for (int r = 0; r < kRing; ++r) { mbar_init(&cmd_full[r], 1); mbar_init(&cmd_empty[r], 5); }
-    for (int w = 0; w < 4; ++w) { mbar_init(&cin_bar[w][0], 1); mbar_init(&cin_bar[w][1], 1); }
+    for (int a = 0; a < 2; ++a) { mbar_init(&tfull_bar[a], 1); mbar_init(&tempty_bar[a], kEpiWarps); }
+    for (int r = 0; r < kRing; ++r) { mbar_init(&cmd_full[r], 1); mbar_init(&cmd_empty[r], 1 + kEpiWarps); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == 1) {
@@ -324,9 +323,9 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
   } else {
     // ===================== epilogue =====================
     const int q = warp & 3;          // TMEM lane quadrant this warp may access
+    const int chunk_first = (warp - 2) >> 2;   // this warp's chunks: chunk_first, chunk_first + 2, ...
     int slot = 0, acc = 0;
-    uint32_t ring_phase = 0, acc_phase = 0, cin_phase[2] = {0u, 0u};
-    float *cin_s = reinterpret_cast<float *>(epi_smem + (size_t)q * 8192);
+    uint32_t ring_phase = 0, acc_phase = 0;
     const int limit = pg.fixed_iter > 0 ? min(pg.fixed_iter, pg.max_iter) : pg.max_iter;
     for (;;) {
       mbar_wait(&cmd_full[slot], ring_phase);
@@ -348,25 +347,28 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
       __half *out16 = o.out16[par] >= 0 ? args.hbuf[o.out16[par]] : nullptr;
       __half *out16_lo = o.out16_lo[par] >= 0 ? args.hbuf[o.out16_lo[par]] : nullptr;
       const int nchunks = (c.nt + 31) >> 5;
-      const CUtensorMap *mc = has_cin ? &args.maps[args.n_half + o.cin32] : nullptr;
-      if (has_cin && lane == 0) {   // prefetch the first two FP32 chunks of this warp's 32 rows
-        fence_proxy_async();
-        for (int ci = 0; ci < min(2, nchunks); ++ci) {
-          mbar_expect_tx(&cin_bar[q][ci], 4096u);
-          tma_load_3d(cin_s + ci * 1024, mc, &cin_bar[q][ci], c.m0 + q * 32, c.n0 + ci * 32, c.mat);
-        }
-      }
       const int64_t tile_off = base + (int64_t)c.n0 * args.ld;   // element (r, n0)
       float *p32 = cout32 ? cout32 + tile_off : nullptr;
       __half *p16 = out16 ? out16 + tile_off : nullptr;
       __half *p16l = out16_lo ? out16_lo + tile_off : nullptr;
       const int store_kind = (p32 ? 1 : 0) | (p16 ? 2 : 0) | (p16l ? 4 : 0);
       const int64_t chunk_stride = (int64_t)32 * args.ld;
+      if (p32) p32 += chunk_first * chunk_stride;
+      if (p16) p16 += chunk_first * chunk_stride;
+      if (p16l) p16l += chunk_first * chunk_stride;
+      // FP32 master of this row, one chunk ahead (columns beyond the tile stay inside the slab)
+      const float *cinp = has_cin ? args.ubuf[o.cin32] + tile_off + chunk_first * chunk_stride : nullptr;
+      float cpre[32];
+      if (has_cin && chunk_first < nchunks) {
+        const float *pc = cinp;
+#pragma unroll
+        for (int j = 0; j < 32; ++j) { cpre[j] = __ldcg(pc); pc += args.ld; }
+      }
       mbar_wait(&tfull_bar[acc], acc_phase);
       tc_fence_after();
       const uint32_t t_main = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(acc * 256);
       float ss = 0.f;
-      for (int ci = 0; ci < nchunks; ++ci) {
+      for (int ci = chunk_first; ci < nchunks; ci += 2) {
         const int c0 = ci * 32;
         const bool full = c.nt - c0 >= 32;
         uint32_t v[32];
@@ -382,17 +384,14 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
           tc_ld_wait();
         }
         if (has_cin) {
-          const int bi = ci & 1;
-          mbar_wait(&cin_bar[q][bi], cin_phase[bi]);
-          cin_phase[bi] ^= 1u;
-          const float *cs = cin_s + bi * 1024 + lane;
 #pragma unroll
           for (int j = 0; j < 32; ++j)
-            v[j] = __float_as_uint(fmaf(o.beta, cs[j * 32], alpha * __uint_as_float(v[j])));
-          __syncwarp();
-          if (lane == 0 && ci + 2 < nchunks) {
-            mbar_expect_tx(&cin_bar[q][bi], 4096u);
-            tma_load_3d(cin_s + bi * 1024, mc, &cin_bar[q][bi], c.m0 + q * 32, c.n0 + c0 + 64, c.mat);
+            v[j] = __float_as_uint(fmaf(o.beta, cpre[j], alpha * __uint_as_float(v[j])));
+          if (ci + 2 < nchunks) {
+            cinp += 2 * chunk_stride;
+            const float *pc = cinp;
+#pragma unroll
+            for (int j = 0; j < 32; ++j) { cpre[j] = __ldcg(pc); pc += args.ld; }
           }
         } else if (ident) {
           // valid columns of this chunk inside the true n x n part (residual of the stop rule)
@@ -416,9 +415,9 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
           case 7: store_cols<true, true, true>(v, p32, p16, p16l, args.ld, full); break;
           default: break;
         }
-        if (p32) p32 += chunk_stride;
-        if (p16) p16 += chunk_stride;
-        if (p16l) p16l += chunk_stride;
+        if (p32) p32 += 2 * chunk_stride;
+        if (p16) p16 += 2 * chunk_stride;
+        if (p16l) p16l += 2 * chunk_stride;
       }
       tc_fence_before();
       fence_proxy_async();     // our generic-proxy stores -> later TMA reads (any CTA)
@@ -430,13 +429,13 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
         if (lane == 0) atomicAdd(&args.resid2[(size_t)(c.iter % NOLSM_MAX_RESID_SLOTS) * args.count + c.mat], ss);
       }
       if (lane == 0) {
-        // completion: 4 warp arrivals per tile; the last arrival of the op publishes it
+        // completion: one arrival per epilogue warp and tile; the last arrival of the op publishes it
         const int n16 = (n + 15) & ~15;
         const int tiles_m = ((n + NOLSM_TILE_M - 1) / NOLSM_TILE_M) * ((n16 + args.bn - 1) / args.bn);
         const int need = c.iter * pg.n_ops + c.op;
         __threadfence();
         const int32_t old = atomicAdd(&args.tiles_done[c.mat], 1);
-        if (old + 1 == (need + 1) * tiles_m * 4) {
+        if (old + 1 == (need + 1) * tiles_m * kEpiWarps) {
           __threadfence();
           const int k = c.iter;
           if (o.resid) {
@@ -577,7 +576,7 @@ cudaError_t launch_chain(nolsm_ctx *ctx, const nolsm_batch *b, const ChainProgra
   a.bn = std::min(split ? 128 : 256, n16max);
   a.b_bytes = ((a.bn + 63) / 64) * kBoxBytes;
   a.stage_bytes = (kATileBytes + a.b_bytes) * (split ? 2 : 1);
-  a.stages = std::min(kMaxStages, (kSmemLimit - 1024 - kEpiBytes) / a.stage_bytes);
+  a.stages = std::min(kMaxStages, (kSmemLimit - 1024) / a.stage_bytes);
   a.mt = (b->max_n + NOLSM_TILE_M - 1) / NOLSM_TILE_M;
   a.ntl = (n16max + a.bn - 1) / a.bn;
   a.maps = b->d_maps;
@@ -602,7 +601,7 @@ cudaError_t launch_chain(nolsm_ctx *ctx, const nolsm_batch *b, const ChainProgra
                                     a.resid2, slots * b->count, a.iters, a.lastres, touch_stats ? 1 : 0);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
-  const int smem_bytes = a.stages * a.stage_bytes + kEpiBytes + 1024;
+  const int smem_bytes = a.stages * a.stage_bytes + 1024;
   void *params[] = {&a};
   return cudaLaunchCooperativeKernel(reinterpret_cast<void *>(k_chain), dim3(ctx->sm_count), dim3(kThreads), params,
                                      (size_t)smem_bytes, st);
