@@ -32,6 +32,9 @@ WORKLOADS = {          # name -> (precision, description)
     "w262144": (0, "configs[3]: 262144 molecules, 12 A, FP16/FP32, streamed"),
 }
 DATASHEET_FP16_TFLOPS = 2250.0
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE sign-iteration launch of k_chain, from the
+# `ncu --set full` capture named in profiles/ (None where no capture of that workload exists)
+NCU_TRAFFIC = {}
 METRIC = "molecules/s per NOLSM step (sign-iteration TFLOP/s in roofline.achieved)"
 
 
@@ -217,13 +220,13 @@ def run_native(args, system, rank, world, local_rank):
     l0 = ctx.launch_count
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     agg = {"ms_gather": 0.0, "ms_prepare": 0.0, "ms_sign": 0.0, "ms_density": 0.0, "flops_sign": 0.0,
-           "flops_sign_padded": 0.0, "flops_prepare": 0.0}
+           "flops_sign_padded": 0.0, "flops_prepare": 0.0, "ms_chain": 0.0, "chain_launches": 0}
     ev0.record()
     last = None
     for _ in range(args.steps):
         mu, ne, D, st = step()
         last = (mu, ne, st)
-        for k in ("ms_gather", "ms_prepare", "ms_sign", "ms_density"):
+        for k in ("ms_gather", "ms_prepare", "ms_sign", "ms_density", "ms_chain", "chain_launches"):
             agg[k] += getattr(st, k)
         agg["flops_sign"] += st.flops_sign_total
         agg["flops_sign_padded"] += st.last.flops_sign_padded
@@ -271,11 +274,15 @@ def run_native(args, system, rank, world, local_rank):
     if rank != 0:
         return None
     peaks = measured_peaks()
-    sign_tflops = agg["flops_sign"] / max(agg["ms_sign"], 1e-9) * 1e-9
+    # dominant kernel: k_chain running the sign iteration (Eq. 9-10) of one batch, all iterations in
+    # one launch; timed with CUDA events on the library's stream around every such launch
+    ms_kernel = agg["ms_chain"] if agg["ms_chain"] > 0 else agg["ms_sign"]
+    sign_tflops = agg["flops_sign"] / max(ms_kernel, 1e-9) * 1e-9
+    n_launch = max(int(agg["chain_launches"]), 1)
     out = {
         "metric": METRIC, "value": value, "unit": "molecules/s", "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": None, "dtype": "f16 operands / f32 accumulate" if precision == 0 else "f32",
+        "vs_baseline": None, "dtype": "f16 operands / f32 accumulate" if precision == 0 else "f32 (split f16 operands)",
         "data": "synthetic",
         "config": {"workload": args.workload, "description": WORKLOADS[args.workload][1], "n_mol": system.n_mol,
                    "cutoff_A": system.cutoff, "mu": MU, "seed": system.seed, "nnz_blocks": system.nnzb,
@@ -284,13 +291,20 @@ def run_native(args, system, rank, world, local_rank):
                    "l2": "inputs larger than L2 (block stores 3 x %.0f MB, dense workspace %.0f GiB)" %
                          (system.nnzb * 144 / 1e6, args.workspace_gib)},
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
-        "roofline": {"bound": "tensor", "kernel": "k_gemm_umma (tcgen05 batched product of the sign iteration)",
+        "roofline": {"bound": "tensor",
+                     "kernel": "k_chain, sign-iteration launches (all iterations of Eq. 9-10 for one batch per launch)",
                      "achieved": sign_tflops, "peak": peaks["tflops_sustained"], "unit": "TFLOP/s",
-                     "frac": sign_tflops / peaks["tflops_sustained"], "traffic": None,
-                     "peak_source": peaks["source"] + " bf16_tflops_sustained (kernel timed inside a long step)",
+                     "frac": sign_tflops / peaks["tflops_sustained"], "traffic": NCU_TRAFFIC.get(args.workload),
+                     "peak_source": peaks["source"] + " bf16_tflops_sustained (kernel timed inside a long step); "
+                                    "FP32 mode issues 3 FP16 MMAs per product, so its bound is peak / 3"
+                                    if precision == 1 else
+                                    peaks["source"] + " bf16_tflops_sustained (kernel timed inside a long step)",
                      "frac_of_datasheet_fp16": sign_tflops / DATASHEET_FP16_TFLOPS,
                      "flops": "2 n^3 per executed sign-iteration GEMM, true n (PAPER.md:246)",
-                     "achieved_padded": agg["flops_sign_padded"] / max(agg["ms_sign"], 1e-9) * 1e-9},
+                     "flops_per_launch": agg["flops_sign"] / n_launch, "launches": n_launch,
+                     "avg_launch_ms": ms_kernel / n_launch,
+                     "achieved_padded": agg["flops_sign_padded"] / max(ms_kernel, 1e-9) * 1e-9,
+                     "achieved_whole_sign_stage": agg["flops_sign"] / max(agg["ms_sign"], 1e-9) * 1e-9},
         "cpu_baseline": cpu,
         "detail": {"sign_tflops": sign_tflops, "ms_gather": agg["ms_gather"] / args.steps,
                    "ms_prepare": agg["ms_prepare"] / args.steps, "ms_sign": agg["ms_sign"] / args.steps,

@@ -25,14 +25,15 @@
 //   * the FP32 master iterate (reading 12) is read in the epilogue with L2-only loads
 //     (ld.global.cg: other SMs wrote it) issued one chunk ahead, and written back with coalesced stores.
 //
-// Warp roles (320 threads): warp 0 = scheduler + TMA producer, warp 1 = MMA issuer (+ TMEM
-// allocation), warps 2..9 = epilogue (TMEM lane quadrant = warp_id % 4; the two warps of a quadrant
-// take alternate 32-column chunks of the tile).
+// Warp roles (352 threads): warp 0 = scheduler (resolves the next tiles and their dependencies, up to
+// kRing tiles ahead), warp 1 = MMA issuer (+ TMEM allocation), warp 2 = TMA producer, warps 3..10 =
+// epilogue (TMEM lane quadrant = warp_id % 4; the two warps of a quadrant take alternate 32-column
+// chunks of the tile).
 #include "common.cuh"
 
 namespace {
 
-constexpr int kThreads = 320;
+constexpr int kThreads = 352;
 constexpr int kEpiWarps = 8;
 constexpr int kBK = 64;                  // K elements per pipeline stage (= one 128-byte swizzle row)
 constexpr int kMaxStages = 8;
@@ -190,7 +191,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
   if (threadIdx.x == 0) {
     for (int s = 0; s < args.stages; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], 1); }
     for (int a = 0; a < 2; ++a) { mbar_init(&tfull_bar[a], 1); mbar_init(&tempty_bar[a], kEpiWarps); }
-    for (int r = 0; r < kRing; ++r) { mbar_init(&cmd_full[r], 1); mbar_init(&cmd_empty[r], 1 + kEpiWarps); }
+    for (int r = 0; r < kRing; ++r) { mbar_init(&cmd_full[r], 1); mbar_init(&cmd_empty[r], 2 + kEpiWarps); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == 1) {
@@ -205,10 +206,10 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
   const uint32_t tmem_base = tmem_base_s;
 
   if (warp == 0) {
-    // ===================== scheduler + TMA producer =====================
+    // ===================== scheduler =====================
     if (lane == 0) {
-      int stage = 0, slot = 0;
-      uint32_t phase = 0, ring_phase = 0;
+      int slot = 0;
+      uint32_t ring_phase = 0;
       const int T = args.mt * args.ntl;
       const int limit = pg.fixed_iter > 0 ? min(pg.fixed_iter, pg.max_iter) : pg.max_iter;
       const int n_groups = (args.count + pg.group - 1) / pg.group;
@@ -236,10 +237,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
             int32_t r = ld_acquire(&args.ready[m]);
             while (r < need) { __nanosleep(64); r = ld_acquire(&args.ready[m]); }
             if (r == kDone) continue;                  // submatrix finished at an earlier iteration
-            fence_proxy_async();                       // other CTAs' generic-proxy writes -> our TMA reads
           }
-          const ChainOp &o = pg.ops[op];
-          const int par = k & 1;
           const int nt = min(args.bn, n16 - n0);
           const int kblocks = (n16 + kBK - 1) / kBK;
           // command to the other roles
@@ -247,35 +245,51 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
           cmds[slot] = TileCmd{m, m0, n0, nt, kblocks, (n16 - (kblocks - 1) * kBK) / 16, op, k};
           mbar_arrive(&cmd_full[slot]);
           if (++slot == kRing) { slot = 0; ring_phase ^= 1u; }
-          // operand loads
-          const bool split = o.a_lo[par] >= 0;
-          const int nbox = (nt + 63) >> 6;
-          const uint32_t bytes = (uint32_t)(kATileBytes + nbox * kBoxBytes) * (split ? 2u : 1u);
-          const CUtensorMap *ma = &args.maps[o.a[par]], *mb = &args.maps[o.b[par]];
-          const CUtensorMap *mal = split ? &args.maps[o.a_lo[par]] : nullptr;
-          const CUtensorMap *mbl = split ? &args.maps[o.b_lo[par]] : nullptr;
-          for (int kb = 0; kb < kblocks; ++kb) {
-            mbar_wait(&empty_bar[stage], phase ^ 1u);
-            uint8_t *st = smem + (size_t)stage * args.stage_bytes;
-            mbar_expect_tx(&full_bar[stage], bytes);
-            const int k0 = kb * kBK;
-            tma_load_3d(st, ma, &full_bar[stage], m0, k0, m);
-            tma_load_3d(st + kBoxBytes, ma, &full_bar[stage], m0 + 64, k0, m);
-            for (int j = 0; j < nbox; ++j)
-              tma_load_3d(st + off_b + j * kBoxBytes, mb, &full_bar[stage], k0, n0 + 64 * j, m);
-            if (split) {
-              tma_load_3d(st + off_a_lo, mal, &full_bar[stage], m0, k0, m);
-              tma_load_3d(st + off_a_lo + kBoxBytes, mal, &full_bar[stage], m0 + 64, k0, m);
-              for (int j = 0; j < nbox; ++j)
-                tma_load_3d(st + off_b_lo + j * kBoxBytes, mbl, &full_bar[stage], k0, n0 + 64 * j, m);
-            }
-            if (++stage == args.stages) { stage = 0; phase ^= 1u; }
-          }
         }
       }
       mbar_wait(&cmd_empty[slot], ring_phase ^ 1u);
       cmds[slot] = TileCmd{0, 0, 0, 0, 0, 0, -1, 0};
       mbar_arrive(&cmd_full[slot]);
+    }
+  } else if (warp == 2) {
+    // ===================== TMA producer =====================
+    if (lane == 0) {
+      int stage = 0, slot = 0;
+      uint32_t phase = 0, ring_phase = 0;
+      for (;;) {
+        mbar_wait(&cmd_full[slot], ring_phase);
+        const TileCmd c = cmds[slot];
+        mbar_arrive(&cmd_empty[slot]);
+        if (++slot == kRing) { slot = 0; ring_phase ^= 1u; }
+        if (c.op < 0) break;
+        fence_proxy_async();   // other CTAs' generic-proxy writes (ordered by the scheduler's acquire) -> TMA reads
+        const ChainOp &o = pg.ops[c.op];
+        const int par = c.iter & 1;
+        const int m = c.mat, m0 = c.m0, n0 = c.n0;
+        const bool split = o.a_lo[par] >= 0;
+        const int nbox = (c.nt + 63) >> 6;
+        const uint32_t bytes = (uint32_t)(kATileBytes + nbox * kBoxBytes) * (split ? 2u : 1u);
+        const CUtensorMap *ma = &args.maps[o.a[par]], *mb = &args.maps[o.b[par]];
+        const CUtensorMap *mal = split ? &args.maps[o.a_lo[par]] : nullptr;
+        const CUtensorMap *mbl = split ? &args.maps[o.b_lo[par]] : nullptr;
+        for (int kb = 0; kb < c.kblocks; ++kb) {
+          mbar_wait(&empty_bar[stage], phase ^ 1u);
+          uint8_t *st = smem + (size_t)stage * args.stage_bytes;
+          mbar_expect_tx(&full_bar[stage], bytes);
+          const int k0 = kb * kBK;
+          tma_load_3d(st, ma, &full_bar[stage], m0, k0, m);
+          tma_load_3d(st + kBoxBytes, ma, &full_bar[stage], m0 + 64, k0, m);
+          for (int j = 0; j < nbox; ++j)
+            tma_load_3d(st + off_b + j * kBoxBytes, mb, &full_bar[stage], k0, n0 + 64 * j, m);
+          if (split) {
+            tma_load_3d(st + off_a_lo, mal, &full_bar[stage], m0, k0, m);
+            tma_load_3d(st + off_a_lo + kBoxBytes, mal, &full_bar[stage], m0 + 64, k0, m);
+            for (int j = 0; j < nbox; ++j)
+              tma_load_3d(st + off_b_lo + j * kBoxBytes, mbl, &full_bar[stage], k0, n0 + 64 * j, m);
+          }
+          if (++stage == args.stages) { stage = 0; phase ^= 1u; }
+        }
+      }
     }
   } else if (warp == 1) {
     // ===================== MMA issuer =====================
@@ -323,7 +337,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
   } else {
     // ===================== epilogue =====================
     const int q = warp & 3;          // TMEM lane quadrant this warp may access
-    const int chunk_first = (warp - 2) >> 2;   // this warp's chunks: chunk_first, chunk_first + 2, ...
+    const int chunk_first = (warp - 3) >> 2;   // this warp's chunks: chunk_first, chunk_first + 2, ...
     int slot = 0, acc = 0;
     uint32_t ring_phase = 0, acc_phase = 0;
     const int limit = pg.fixed_iter > 0 ? min(pg.fixed_iter, pg.max_iter) : pg.max_iter;

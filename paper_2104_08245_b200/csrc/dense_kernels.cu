@@ -61,34 +61,74 @@ cudaError_t launch_norm_bound(const nolsm_batch *b, const float *a, float mu, fl
 }
 
 // ------------------------------------------------------------------------------------------------
+// Element-wise passes over the padded P x P part of every submatrix.  One thread = four consecutive
+// rows of one column (16-byte FP32 accesses, 8-byte FP16 stores; ld is a multiple of 128, so every
+// access is aligned); blockIdx.y = submatrix.
+// ------------------------------------------------------------------------------------------------
+struct Elem4 { int r, c, n; int64_t off; };
+
+__device__ __forceinline__ bool elem4(const int32_t *__restrict__ dims, int ld, int64_t slab, Elem4 &e) {
+  const int mat = blockIdx.y;
+  e.n = dims[mat];
+  const int P = padded_dim(e.n);
+  const int q = P >> 2;
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= q * P) return false;
+  e.c = i / q;
+  e.r = (i - e.c * q) << 2;
+  e.off = (int64_t)mat * slab + (int64_t)e.c * ld + e.r;
+  return true;
+}
+
+__device__ __forceinline__ void store_half4(__half *dst, const float (&v)[4]) {
+  const __half2 a = __floats2half2_rn(v[0], v[1]), b = __floats2half2_rn(v[2], v[3]);
+  uint2 pk;
+  pk.x = *reinterpret_cast<const uint32_t *>(&a);
+  pk.y = *reinterpret_cast<const uint32_t *>(&b);
+  *reinterpret_cast<uint2 *>(dst) = pk;
+}
+
+// hi = fp16(v), lo = fp16((v - hi) * 2^11): the split operands of the FP32-quality products
+__device__ __forceinline__ void store_split4(__half *hi, __half *lo, const float (&v)[4]) {
+  float h[4], l[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    h[i] = __half2float(__float2half_rn(v[i]));
+    l[i] = (v[i] - h[i]) * 2048.f;
+  }
+  store_half4(hi, h);
+  if (lo) store_half4(lo, l);
+}
+
+static dim3 elem4_grid(const nolsm_batch *b) {
+  const int P = round_up(b->max_n, NOLSM_TILE_M);
+  return dim3((unsigned)(((int64_t)(P >> 2) * P + 255) / 256), (unsigned)b->count);
+}
+
 // Eq. 15: Y0 = T_j(S)/s_S, Z0 = I with s_S = sqrt(||S||_1 ||S||_inf) >= lambda_max(S)
 // (reading 7).  The padded part of S is the identity, so Y0 there is 1/s_S.
-// ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
 k_init_inverse(const int32_t *__restrict__ dims, int ld, int64_t slab, int count,
                const float *__restrict__ s, const float *__restrict__ norm2, float *__restrict__ y32,
                float *__restrict__ z32, __half *__restrict__ y16, __half *__restrict__ z16,
                __half *__restrict__ y16_lo, __half *__restrict__ z16_lo, float *__restrict__ scale_out) {
-  const int mat = blockIdx.z;
-  const int n = dims[mat];
-  const int P = padded_dim(n);
-  const int c = blockIdx.y;
-  const int r = blockIdx.x * 256 + threadIdx.x;
-  if (c >= P || r >= P) return;
+  Elem4 e;
+  if (!elem4(dims, ld, slab, e)) return;
+  const int mat = blockIdx.y;
   const float sc = fmaxf(1.f, sqrtf(norm2[mat] * norm2[count + mat]));  // >= 1 covers the unit padding
-  if (r == 0 && c == 0) scale_out[mat] = sc;
-  const int64_t off = (int64_t)mat * slab + (int64_t)c * ld + r;
-  const float y = s[off] / sc;
-  const float z = (r == c) ? 1.f : 0.f;
-  if (y32) { y32[off] = y; z32[off] = z; }
+  if (e.r == 0 && e.c == 0) scale_out[mat] = sc;
+  const float4 sv = *reinterpret_cast<const float4 *>(s + e.off);
+  const float y[4] = {sv.x / sc, sv.y / sc, sv.z / sc, sv.w / sc};
+  float z[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) z[i] = (e.r + i == e.c) ? 1.f : 0.f;
+  if (y32) {
+    *reinterpret_cast<float4 *>(y32 + e.off) = make_float4(y[0], y[1], y[2], y[3]);
+    *reinterpret_cast<float4 *>(z32 + e.off) = make_float4(z[0], z[1], z[2], z[3]);
+  }
   if (y16) {
-    const __half yh = __float2half_rn(y);
-    y16[off] = yh;
-    z16[off] = __float2half_rn(z);
-    if (y16_lo) {   // split operands of the FP32-quality products: value = hi + lo / 2^11
-      y16_lo[off] = __float2half_rn((y - __half2float(yh)) * 2048.f);
-      z16_lo[off] = __float2half_rn(0.f);
-    }
+    store_split4(y16 + e.off, y16_lo ? y16_lo + e.off : nullptr, y);
+    store_split4(z16 + e.off, z16_lo ? z16_lo + e.off : nullptr, z);
   }
 }
 
@@ -96,90 +136,68 @@ cudaError_t launch_init_inverse(const nolsm_batch *b, const float *s, const floa
                                 float *z32, __half *y16, __half *z16, __half *y16_lo, __half *z16_lo,
                                 float *scale_out, cudaStream_t st) {
   if (b->count == 0) return cudaSuccess;
-  const int P = round_up(b->max_n, NOLSM_TILE_M);
-  dim3 grid((P + 255) / 256, P, b->count);
-  k_init_inverse<<<grid, 256, 0, st>>>(b->d_dims, b->ld, (int64_t)b->ld * b->ld, b->count, s, norm2,
-                                       y32, z32, y16, z16, y16_lo, z16_lo, scale_out);
+  k_init_inverse<<<elem4_grid(b), 256, 0, st>>>(b->d_dims, b->ld, (int64_t)b->ld * b->ld, b->count, s, norm2,
+                                                y32, z32, y16, z16, y16_lo, z16_lo, scale_out);
   return cudaGetLastError();
 }
 
-// ------------------------------------------------------------------------------------------------
 // X0 = (B - mu I)/s  (Eq. 9 with the rescaling of PAPER.md:138), s from the norm bound or from the
 // caller (scale_in, dense microbench).  Padded diagonal = 1: a fixed point of the iteration that adds
 // nothing to the residual (reading 19).
-// ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
 k_make_x0(const int32_t *__restrict__ dims, int ld, int64_t slab, int count,
           const float *__restrict__ bmat, float mu, const float *__restrict__ norm2,
           const float *__restrict__ scale_in, float *__restrict__ x32, __half *__restrict__ x16,
           __half *__restrict__ x16_lo, float *__restrict__ scale_out) {
-  const int mat = blockIdx.z;
-  const int n = dims[mat];
-  const int P = padded_dim(n);
-  const int c = blockIdx.y;
-  const int r = blockIdx.x * 256 + threadIdx.x;
-  if (c >= P || r >= P) return;
+  Elem4 e;
+  if (!elem4(dims, ld, slab, e)) return;
+  const int mat = blockIdx.y;
   float sc = scale_in ? scale_in[mat] : sqrtf(norm2[mat] * norm2[count + mat]);
   sc = fmaxf(sc, 1e-30f);
-  if (r == 0 && c == 0 && scale_out) scale_out[mat] = sc;
-  const int64_t off = (int64_t)mat * slab + (int64_t)c * ld + r;
-  float v;
-  if (r < n && c < n) {
-    v = bmat[off];
-    if (r == c) v -= mu;
-    v /= sc;
-  } else {
-    v = (r == c) ? 1.f : 0.f;
+  if (e.r == 0 && e.c == 0 && scale_out) scale_out[mat] = sc;
+  const float4 bv = *reinterpret_cast<const float4 *>(bmat + e.off);
+  const float in[4] = {bv.x, bv.y, bv.z, bv.w};
+  float v[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const int r = e.r + i;
+    if (r < e.n && e.c < e.n) v[i] = (in[i] - (r == e.c ? mu : 0.f)) / sc;
+    else v[i] = (r == e.c) ? 1.f : 0.f;
   }
-  if (x32) x32[off] = v;
-  if (x16) {
-    const __half hi = __float2half_rn(v);
-    x16[off] = hi;
-    if (x16_lo) x16_lo[off] = __float2half_rn((v - __half2float(hi)) * 2048.f);
-  }
+  if (x32) *reinterpret_cast<float4 *>(x32 + e.off) = make_float4(v[0], v[1], v[2], v[3]);
+  if (x16) store_split4(x16 + e.off, x16_lo ? x16_lo + e.off : nullptr, v);
 }
 
 cudaError_t launch_make_x0(const nolsm_batch *b, const float *bmat, float mu, const float *norm2,
                            const float *scale_in, float *x32, __half *x16, __half *x16_lo, float *scale_out,
                            cudaStream_t st) {
   if (b->count == 0) return cudaSuccess;
-  const int P = round_up(b->max_n, NOLSM_TILE_M);
-  dim3 grid((P + 255) / 256, P, b->count);
-  k_make_x0<<<grid, 256, 0, st>>>(b->d_dims, b->ld, (int64_t)b->ld * b->ld, b->count, bmat, mu, norm2,
-                                  scale_in, x32, x16, x16_lo, scale_out);
+  k_make_x0<<<elem4_grid(b), 256, 0, st>>>(b->d_dims, b->ld, (int64_t)b->ld * b->ld, b->count, bmat, mu, norm2,
+                                           scale_in, x32, x16, x16_lo, scale_out);
   return cudaGetLastError();
 }
 
 // dst = src * f (f = scale[m], 1/scale[m] or 1), FP32 and/or FP16 (hi [+ lo*2^11]) copies over the
-// padded extent.  Used to hand FP32 results to the tensor-core path.
+// padded extent.  Hands FP32 results to the tensor-core path.
 __global__ void __launch_bounds__(256)
 k_scale_copy(const int32_t *__restrict__ dims, int ld, int64_t slab, const float *__restrict__ src,
              const float *__restrict__ scale, int invert, float *__restrict__ dst32,
              __half *__restrict__ dst16, __half *__restrict__ dst16_lo) {
-  const int mat = blockIdx.z;
-  const int P = padded_dim(dims[mat]);
-  const int c = blockIdx.y;
-  const int r = blockIdx.x * 256 + threadIdx.x;
-  if (c >= P || r >= P) return;
+  Elem4 e;
+  if (!elem4(dims, ld, slab, e)) return;
   float f = 1.f;
-  if (scale) f = invert ? 1.f / scale[mat] : scale[mat];
-  const int64_t off = (int64_t)mat * slab + (int64_t)c * ld + r;
-  const float v = src[off] * f;
-  if (dst32) dst32[off] = v;
-  if (dst16) {
-    const __half hi = __float2half_rn(v);
-    dst16[off] = hi;
-    if (dst16_lo) dst16_lo[off] = __float2half_rn((v - __half2float(hi)) * 2048.f);
-  }
+  if (scale) f = invert ? 1.f / scale[blockIdx.y] : scale[blockIdx.y];
+  const float4 sv = *reinterpret_cast<const float4 *>(src + e.off);
+  const float v[4] = {sv.x * f, sv.y * f, sv.z * f, sv.w * f};
+  if (dst32) *reinterpret_cast<float4 *>(dst32 + e.off) = make_float4(v[0], v[1], v[2], v[3]);
+  if (dst16) store_split4(dst16 + e.off, dst16_lo ? dst16_lo + e.off : nullptr, v);
 }
 
 cudaError_t launch_scale_copy(const nolsm_batch *b, const float *src, const float *scale, int invert,
                               float *dst32, __half *dst16, __half *dst16_lo, cudaStream_t st) {
   if (b->count == 0) return cudaSuccess;
-  const int P = round_up(b->max_n, NOLSM_TILE_M);
-  dim3 grid((P + 255) / 256, P, b->count);
-  k_scale_copy<<<grid, 256, 0, st>>>(b->d_dims, b->ld, (int64_t)b->ld * b->ld, src, scale, invert,
-                                     dst32, dst16, dst16_lo);
+  k_scale_copy<<<elem4_grid(b), 256, 0, st>>>(b->d_dims, b->ld, (int64_t)b->ld * b->ld, src, scale, invert,
+                                              dst32, dst16, dst16_lo);
   return cudaGetLastError();
 }
 
