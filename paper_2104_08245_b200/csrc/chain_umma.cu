@@ -153,6 +153,15 @@ __device__ __forceinline__ void store_cols(const uint32_t (&v)[32], float *p32, 
   }
 }
 
+#ifdef NOLSM_TRACE
+__device__ long long g_trace[4][4096][2];
+#define TRACE(role, ti, j) do { if (blockIdx.x == 0 && (ti) < 4096) g_trace[role][ti][j] = clock64(); } while (0)
+#define TRACEV(role, ti, j, v) do { if (blockIdx.x == 0 && (ti) < 4096) g_trace[role][ti][j] = (v); } while (0)
+#else
+#define TRACE(role, ti, j)
+#define TRACEV(role, ti, j, v)
+#endif
+
 struct TileCmd {              // scheduler -> MMA issuer and epilogue warps
   int32_t mat, m0, n0, nt;    // submatrix, first row / column, tile columns (multiple of 16, <= bn)
   int32_t kblocks, ktail;     // K blocks of 64; K=16 steps in the last one (1..4)
@@ -254,6 +263,9 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
   } else if (warp == 2) {
     // ===================== TMA producer =====================
     if (lane == 0) {
+#ifdef NOLSM_TRACE
+      int tti = 0;
+#endif
       int stage = 0, slot = 0;
       uint32_t phase = 0, ring_phase = 0;
       for (;;) {
@@ -262,6 +274,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
         mbar_arrive(&cmd_empty[slot]);
         if (++slot == kRing) { slot = 0; ring_phase ^= 1u; }
         if (c.op < 0) break;
+        TRACE(2, tti, 0);
         fence_proxy_async();   // other CTAs' generic-proxy writes (ordered by the scheduler's acquire) -> TMA reads
         const ChainOp &o = pg.ops[c.op];
         const int par = c.iter & 1;
@@ -289,11 +302,18 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
           }
           if (++stage == args.stages) { stage = 0; phase ^= 1u; }
         }
+        TRACE(2, tti, 1);
+#ifdef NOLSM_TRACE
+        ++tti;
+#endif
       }
     }
   } else if (warp == 1) {
     // ===================== MMA issuer =====================
     if (lane == 0) {
+#ifdef NOLSM_TRACE
+      int mti = 0;
+#endif
       int stage = 0, slot = 0, acc = 0;
       uint32_t phase = 0, ring_phase = 0, acc_phase = 0;
       for (;;) {
@@ -305,8 +325,13 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
         const bool split = pg.ops[c.op].a_lo[c.iter & 1] >= 0;
         // instruction descriptor: D=F32, A=B=F16, A M-major, B K-major, N = nt, M = 128
         const uint32_t idesc = (1u << 4) | (1u << 15) | ((uint32_t)(c.nt >> 3) << 17) | ((128u >> 4) << 24);
+        TRACE(0, mti, 0);
         mbar_wait(&tempty_bar[acc], acc_phase ^ 1u);
         tc_fence_after();
+        TRACE(0, mti, 1);
+#ifdef NOLSM_TRACE
+        ++mti;
+#endif
         const uint32_t d_main = tmem_base + (uint32_t)(acc * 256);
         const uint32_t d_corr = d_main + 128;
         for (int kb = 0; kb < c.kblocks; ++kb) {
@@ -337,6 +362,9 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
   } else {
     // ===================== epilogue =====================
     const int q = warp & 3;          // TMEM lane quadrant this warp may access
+#ifdef NOLSM_TRACE
+    int eti = 0;
+#endif
     const int chunk_first = (warp - 3) >> 2;   // this warp's chunks: chunk_first, chunk_first + 2, ...
     int slot = 0, acc = 0;
     uint32_t ring_phase = 0, acc_phase = 0;
@@ -378,8 +406,10 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
 #pragma unroll
         for (int j = 0; j < 32; ++j) { cpre[j] = __ldcg(pc); pc += args.ld; }
       }
+      if (warp == 3 && lane == 0) { TRACE(1, eti, 0); }
       mbar_wait(&tfull_bar[acc], acc_phase);
       tc_fence_after();
+      if (warp == 3 && lane == 0) { TRACE(1, eti, 1); TRACEV(3, eti, 0, (long long)c.op); }
       const uint32_t t_main = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(acc * 256);
       float ss = 0.f;
       for (int ci = chunk_first; ci < nchunks; ci += 2) {
@@ -472,6 +502,10 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
           }
         }
       }
+      if (warp == 3 && lane == 0) { TRACE(3, eti, 1); }
+#ifdef NOLSM_TRACE
+      ++eti;
+#endif
     }
   }
 
@@ -524,6 +558,13 @@ nolsm_status encode_map(nolsm_ctx *ctx, CUtensorMap *map, void *ptr, bool half, 
 }
 
 }  // namespace
+
+#ifdef NOLSM_TRACE
+extern "C" void nolsm_debug_trace(long long *host_out) {
+  cudaDeviceSynchronize();
+  cudaMemcpyFromSymbol(host_out, g_trace, sizeof(g_trace));
+}
+#endif
 
 nolsm_status umma_init(nolsm_ctx *ctx) {
   ctx->umma_ok = false;
