@@ -34,7 +34,7 @@ WORKLOADS = {          # name -> (precision, description)
 DATASHEET_FP16_TFLOPS = 2250.0
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE sign-iteration launch of k_chain, from the
 # `ncu --set full` capture named in profiles/ (None where no capture of that workload exists)
-NCU_TRAFFIC = {}
+NCU_TRAFFIC = {"w32768": 80.07e9}   # profiles/r1_k_chain_sign_w32768.md
 METRIC = "molecules/s per NOLSM step (sign-iteration TFLOP/s in roofline.achieved)"
 
 
@@ -143,6 +143,25 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------------------------
+# N > 1: independent replicas -- the only cross-rank step is the max of the times
+# ------------------------------------------------------------------------------------------------
+def max_over_ranks(ms, device="cpu"):
+    """Max over the ranks of a per-rank time (all-reduce MAX; identity without a process group)."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()):
+        return float(ms)
+    t = torch.tensor([float(ms)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_value(world, n_mol, ms_step):
+    """Whole-job molecules/s: every rank processes its own replica of n_mol molecules per step."""
+    return world * n_mol / (ms_step * 1e-3)
+
+
+# ------------------------------------------------------------------------------------------------
 # the two arms
 # ------------------------------------------------------------------------------------------------
 def run_reference(args, system, rank):
@@ -235,14 +254,10 @@ def run_native(args, system, rank, world, local_rank):
     barrier()
     clocks = sampler.stop()
     launches = ctx.launch_count - l0
-    ms = ev0.elapsed_time(ev1)
-    if dist is not None:
-        t = torch.tensor([ms], device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(ev0.elapsed_time(ev1), dev)
     mu, ne, st = last
     ms_step = ms / args.steps
-    value = world * system.n_mol / (ms_step * 1e-3)
+    value = job_value(world, system.n_mol, ms_step)
 
     # end to end through the host-buffer entry (transfers inside the timed region)
     e2e = None
@@ -261,12 +276,8 @@ def run_native(args, system, rank, world, local_rank):
                                                      mu_lo, mu_hi, -1.0, 1)
         e1.record()
         barrier()
-        ms_e = max(e0.elapsed_time(e1), 1e3 * (time.perf_counter() - t0)) / reps
-        if dist is not None:
-            t = torch.tensor([ms_e], device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms_e = float(t.item())
-        e2e = {"value": world * system.n_mol / (ms_e * 1e-3), "unit": "molecules/s", "h2d_bytes_per_step": h2d,
+        ms_e = max_over_ranks(max(e0.elapsed_time(e1), 1e3 * (time.perf_counter() - t0)) / reps, dev)
+        e2e = {"value": job_value(world, system.n_mol, ms_e), "unit": "molecules/s", "h2d_bytes_per_step": h2d,
                "d2h_bytes_per_step": d2h, "ms_per_step": ms_e, "n_electrons": ne_h,
                "note": "nolsm_solve_mu_host: pattern+H+S pinned host->device, D device->host, per step"}
     if dist is not None:
