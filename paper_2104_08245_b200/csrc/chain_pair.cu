@@ -1,0 +1,570 @@
+// Pair-CTA variant of the matrix-iteration engine (see chain_umma.cu for the scheduling, the
+// dependency protocol and the epilogues, which are identical): two CTAs of a cluster (one TPC)
+// compute ONE 256 x N tile with tcgen05.mma.cta_group::2.  Each CTA stages its own 128 rows of the A
+// operand and only HALF of the B operand's columns, so the operand bytes an SM must take in per
+// 64-deep K block drop from 48 KB (128 x 256 tile, cta_group::1) to 32 KB.  That delivery rate, not the
+// tensor pipe, bounds the single-CTA kernel (profiles/r1_k_chain_sign_w32768.md).
+//
+// Protocol differences to chain_umma.cu:
+//   * the scheduler runs in the leader CTA (cluster rank 0) only and writes every tile command into
+//     both CTAs' rings (st.shared::cluster + remote mbarrier arrive), so the two CTAs can never
+//     disagree on the tile sequence;
+//   * `full` (operands landed) and `tmem empty` barriers live in the leader: both CTAs' TMA loads
+//     signal the leader's `full` barrier (cp.async.bulk.tensor ... cta_group::2), the peer's epilogue
+//     warps arrive remotely on `tmem empty`;
+//   * the leader's single MMA thread issues for both CTAs and releases smem stages / publishes the
+//     accumulator in both CTAs with tcgen05.commit ... multicast::cluster.
+#include "common.cuh"
+
+namespace pair {
+
+constexpr int kThreads = 352;
+constexpr int kEpiWarps = 8;
+constexpr int kBK = 64;
+constexpr int kMaxStages = 8;
+constexpr int kTmemCols = 512;
+constexpr int kBoxBytes = 64 * 128;
+constexpr int kATileBytes = 2 * kBoxBytes;     // this CTA's 128 rows x 64 K
+constexpr int kRing = 4;
+constexpr int kSmemLimit = 232448 - 2048;
+constexpr int32_t kDone = 0x7fffffff;
+constexpr int kTileM = 256;                    // rows of a pair tile
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) {
+  return static_cast<uint32_t>(__cvta_generic_to_shared(p));
+}
+// shared::cluster address of the same variable in CTA `rank` of the cluster
+__device__ __forceinline__ uint32_t mapa(uint32_t saddr, uint32_t rank) {
+  uint32_t r;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(saddr), "r"(rank));
+  return r;
+}
+__device__ __forceinline__ uint32_t cluster_rank() {
+  uint32_t r;
+  asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+  return r;
+}
+__device__ __forceinline__ void cluster_sync() {
+  asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
+               : "memory");
+}
+// arrive on a barrier given by its shared::cluster address (own or peer CTA), release at cluster scope
+__device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr) {
+  asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+}
+// wait with acquire at cluster scope (the arrivals may come from the peer CTA)
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
+  asm volatile(
+      "{\n\t"
+      ".reg .pred p;\n\t"
+      "PWAIT_LOOP:\n\t"
+      "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%0], %1;\n\t"
+      "@p bra PWAIT_DONE;\n\t"
+      "bra PWAIT_LOOP;\n\t"
+      "PWAIT_DONE:\n\t"
+      "}\n" ::"r"(smem_u32(bar)),
+      "r"(parity)
+      : "memory");
+}
+// TMA load into THIS CTA's shared memory that signals the barrier at shared::cluster address `bar`
+__device__ __forceinline__ void tma_load_3d(void *dst, const CUtensorMap *map, uint32_t bar, int c0, int c1,
+                                            int c2) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.cta_group::2.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, "
+      "{%3, %4, %5}], [%2];" ::"r"(smem_u32(dst)),
+      "l"(reinterpret_cast<uint64_t>(map)), "r"(bar), "r"(c0), "r"(c1), "r"(c2)
+      : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+// arrives on the barrier at the same offset in BOTH CTAs once all prior MMAs of this thread are done
+__device__ __forceinline__ void tc_commit_both(uint64_t *bar) {
+  asm volatile(
+      "tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(
+          smem_u32(bar)),
+      "h"((uint16_t)3)
+      : "memory");
+}
+__device__ __forceinline__ void tc_mma2_f16(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc,
+                                            uint32_t accumulate) {
+  asm volatile(
+      "{\n\t"
+      ".reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n\t"
+      "}\n" ::"r"(tmem_d),
+      "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+__device__ __forceinline__ void tc_ld32(uint32_t taddr, uint32_t (&v)[32]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, %17, %18, %19, %20, %21, "
+      "%22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+      : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+        "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]),
+        "=r"(v[15]), "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]),
+        "=r"(v[22]), "=r"(v[23]), "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]),
+        "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+      : "r"(taddr));
+}
+__device__ __forceinline__ void tc_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ int32_t ld_acquire(const int32_t *p) {
+  int32_t v;
+  asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_release(int32_t *p, int32_t v) {
+  asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+__device__ __forceinline__ uint64_t make_smem_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
+  uint64_t d = 0;
+  d |= (uint64_t)((saddr & 0x3FFFF) >> 4);
+  d |= (uint64_t)((lbo_bytes >> 4) & 0x3FFF) << 16;
+  d |= (uint64_t)((sbo_bytes >> 4) & 0x3FFF) << 32;
+  d |= (uint64_t)1 << 46;   // version
+  d |= (uint64_t)2 << 61;   // SWIZZLE_128B
+  return d;
+}
+
+template <bool H32, bool H16, bool HLO>
+__device__ __forceinline__ void store_cols(const uint32_t (&v)[32], float *p32, __half *p16, __half *p16l, int ld,
+                                           bool full) {
+#pragma unroll
+  for (int half = 0; half < 2; ++half) {
+    if (half == 1 && !full) break;
+#pragma unroll
+    for (int jj = 0; jj < 16; ++jj) {
+      const float val = __uint_as_float(v[half * 16 + jj]);
+      if (H32) { *p32 = val; p32 += ld; }
+      if (H16) {
+        const __half hi = __float2half_rn(val);
+        *p16 = hi; p16 += ld;
+        if (HLO) { *p16l = __float2half_rn((val - __half2float(hi)) * 2048.f); p16l += ld; }
+      }
+    }
+  }
+}
+
+struct TileCmd {              // scheduler -> TMA producers, MMA issuer and epilogue warps of both CTAs
+  int32_t mat, m0, n0, nt;    // submatrix, first row of the PAIR tile / first column, tile columns (mult. of 32)
+  int32_t kblocks, ktail;     // K blocks of 64; K=16 steps in the last one (1..4)
+  int32_t op, iter;           // op < 0: no more tiles
+};
+
+struct PairArgs {
+  ChainProgram prog;
+  const CUtensorMap *maps;
+  __half *hbuf[NOLSM_MAX_HALF];
+  float *ubuf[NOLSM_MAX_UNIT];
+  int32_t count, ld;
+  int64_t slab;
+  int32_t bn, b_bytes, stages, stage_bytes;   // b_bytes: this CTA's half of the B tile
+  int32_t mt, ntl;            // uniform tile grid per submatrix: mt pair-row tiles x ntl column tiles
+  const int32_t *dims;
+  const float *alpha_div;
+  int32_t *ready, *tiles_done, *state, *iters, *group_active;
+  float *resid2, *lastres;
+};
+
+__global__ void __launch_bounds__(kThreads, 1) k_chain_pair(const PairArgs args) {
+  extern __shared__ __align__(1024) uint8_t smem_raw[];
+  __shared__ uint64_t full_bar[kMaxStages], empty_bar[kMaxStages], tfull_bar[2], tempty_bar[2];
+  __shared__ uint64_t cmd_full[kRing], cmd_empty[kRing];
+  __shared__ __align__(16) TileCmd cmds[kRing];
+  __shared__ uint32_t tmem_base_s;
+
+  const ChainProgram &pg = args.prog;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint32_t rank = cluster_rank();
+  const bool leader = rank == 0;
+  uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+  // stage layout: [A hi 16K][B hi b_bytes][A lo 16K][B lo b_bytes]
+  const int off_b = kATileBytes, off_a_lo = kATileBytes + args.b_bytes, off_b_lo = 2 * kATileBytes + args.b_bytes;
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < args.stages; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], 1); }
+    for (int a = 0; a < 2; ++a) { mbar_init(&tfull_bar[a], 1); mbar_init(&tempty_bar[a], 2 * kEpiWarps); }
+    // command ring: filled by the leader's scheduler in both CTAs; freed (leader's barrier) by the
+    // leader's MMA issuer + both TMA producers + both CTAs' epilogue warps
+    for (int r = 0; r < kRing; ++r) { mbar_init(&cmd_full[r], 1); mbar_init(&cmd_empty[r], 3 + 2 * kEpiWarps); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  if (warp == 1) {
+    asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_base_s)),
+                 "r"(kTmemCols)
+                 : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+  }
+  tc_fence_before();
+  __syncthreads();
+  cluster_sync();          // barriers of both CTAs initialised before any remote arrive / multicast commit
+  tc_fence_after();
+  const uint32_t tmem_base = tmem_base_s;
+
+  if (warp == 0) {
+    // ===================== scheduler (leader CTA only) =====================
+    if (leader && lane == 0) {
+      int slot = 0;
+      uint32_t ring_phase = 0;
+      const int T = args.mt * args.ntl;
+      const int limit = pg.fixed_iter > 0 ? min(pg.fixed_iter, pg.max_iter) : pg.max_iter;
+      const int n_groups = (args.count + pg.group - 1) / pg.group;
+      const int n_clusters = gridDim.x >> 1, cluster_id = blockIdx.x >> 1;
+      auto push = [&](const TileCmd &cmd) {
+        mbar_wait(&cmd_empty[slot], ring_phase ^ 1u);
+        cmds[slot] = cmd;
+        const uint32_t remote = mapa(smem_u32(&cmds[slot]), 1);
+        asm volatile("st.shared::cluster.v4.s32 [%0], {%1, %2, %3, %4};" ::"r"(remote), "r"(cmd.mat), "r"(cmd.m0),
+                     "r"(cmd.n0), "r"(cmd.nt)
+                     : "memory");
+        asm volatile("st.shared::cluster.v4.s32 [%0], {%1, %2, %3, %4};" ::"r"(remote + 16), "r"(cmd.kblocks),
+                     "r"(cmd.ktail), "r"(cmd.op), "r"(cmd.iter)
+                     : "memory");
+        mbar_arrive_cluster(mapa(smem_u32(&cmd_full[slot]), 0));
+        mbar_arrive_cluster(mapa(smem_u32(&cmd_full[slot]), 1));
+        if (++slot == kRing) { slot = 0; ring_phase ^= 1u; }
+      };
+      for (int g = 0; g < n_groups; ++g) {
+        const int gbase = g * pg.group;
+        const int gs = min(pg.group, args.count - gbase);
+        const int per_seg = gs * T;
+        const int64_t total = (int64_t)limit * pg.n_ops * per_seg;
+        int k_checked = 0;
+        for (int64_t L = cluster_id; L < total; L += n_clusters) {
+          const int seg = (int)(L / per_seg), rem = (int)(L % per_seg);
+          const int k = seg / pg.n_ops, op = seg % pg.n_ops;
+          if (k != k_checked) {   // whole group converged: go to the next group
+            if (ld_acquire(&args.group_active[g]) == 0) break;
+            k_checked = k;
+          }
+          const int ml = rem / T, t = rem % T;
+          const int m = gbase + ml;
+          const int n = args.dims[m];
+          const int n16 = (n + 15) & ~15, n32 = (n + 31) & ~31;
+          const int m0 = (t % args.mt) * kTileM, n0 = (t / args.mt) * args.bn;
+          if (m0 >= n || n0 >= n32) continue;          // tile outside this submatrix
+          const int need = k * pg.n_ops + op;          // ops of this submatrix that must be complete
+          if (need > 0) {
+            int32_t r = ld_acquire(&args.ready[m]);
+            while (r < need) { __nanosleep(64); r = ld_acquire(&args.ready[m]); }
+            if (r == kDone) continue;                  // submatrix finished at an earlier iteration
+          }
+          const int kblocks = (n16 + kBK - 1) / kBK;
+          push(TileCmd{m, m0, n0, min(args.bn, n32 - n0), kblocks, (n16 - (kblocks - 1) * kBK) / 16, op, k});
+        }
+      }
+      push(TileCmd{0, 0, 0, 0, 0, 0, -1, 0});
+    }
+  } else if (warp == 2) {
+    // ===================== TMA producer (both CTAs) =====================
+    if (lane == 0) {
+      int stage = 0, slot = 0;
+      uint32_t phase = 0, ring_phase = 0;
+      for (;;) {
+        mbar_wait(&cmd_full[slot], ring_phase);
+        const TileCmd c = cmds[slot];
+        mbar_arrive_cluster(mapa(smem_u32(&cmd_empty[slot]), 0));
+        if (++slot == kRing) { slot = 0; ring_phase ^= 1u; }
+        if (c.op < 0) break;
+        fence_proxy_async();   // other CTAs' generic-proxy writes (ordered by the scheduler's acquire) -> TMA reads
+        const ChainOp &o = pg.ops[c.op];
+        const int par = c.iter & 1;
+        const int m = c.mat;
+        const int m0 = c.m0 + 128 * (int)rank;               // this CTA's rows of the pair tile
+        const int half_n = c.nt >> 1;
+        const int n0 = c.n0 + half_n * (int)rank;            // this CTA's half of the B columns
+        const bool split = o.a_lo[par] >= 0;
+        const int nbox = (half_n + 63) >> 6;
+        const uint32_t bytes = 2u * (uint32_t)(kATileBytes + nbox * kBoxBytes) * (split ? 2u : 1u);  // both CTAs
+        const CUtensorMap *ma = &args.maps[o.a[par]], *mb = &args.maps[o.b[par]];
+        const CUtensorMap *mal = split ? &args.maps[o.a_lo[par]] : nullptr;
+        const CUtensorMap *mbl = split ? &args.maps[o.b_lo[par]] : nullptr;
+        for (int kb = 0; kb < c.kblocks; ++kb) {
+          mbar_wait(&empty_bar[stage], phase ^ 1u);
+          uint8_t *st = smem + (size_t)stage * args.stage_bytes;
+          if (leader) mbar_expect_tx(&full_bar[stage], bytes);
+          const uint32_t fb = mapa(smem_u32(&full_bar[stage]), 0);
+          const int k0 = kb * kBK;
+          tma_load_3d(st, ma, fb, m0, k0, m);
+          tma_load_3d(st + kBoxBytes, ma, fb, m0 + 64, k0, m);
+          for (int j = 0; j < nbox; ++j) tma_load_3d(st + off_b + j * kBoxBytes, mb, fb, k0, n0 + 64 * j, m);
+          if (split) {
+            tma_load_3d(st + off_a_lo, mal, fb, m0, k0, m);
+            tma_load_3d(st + off_a_lo + kBoxBytes, mal, fb, m0 + 64, k0, m);
+            for (int j = 0; j < nbox; ++j)
+              tma_load_3d(st + off_b_lo + j * kBoxBytes, mbl, fb, k0, n0 + 64 * j, m);
+          }
+          if (++stage == args.stages) { stage = 0; phase ^= 1u; }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ===================== MMA issuer (leader CTA only, for both CTAs) =====================
+    if (leader && lane == 0) {
+      int stage = 0, slot = 0, acc = 0;
+      uint32_t phase = 0, ring_phase = 0, acc_phase = 0;
+      for (;;) {
+        mbar_wait(&cmd_full[slot], ring_phase);
+        const TileCmd c = cmds[slot];
+        mbar_arrive_cluster(mapa(smem_u32(&cmd_empty[slot]), 0));
+        if (++slot == kRing) { slot = 0; ring_phase ^= 1u; }
+        if (c.op < 0) break;
+        const bool split = pg.ops[c.op].a_lo[c.iter & 1] >= 0;
+        // instruction descriptor: D=F32, A=B=F16, A M-major, B K-major, N = nt, M = 256 (128 per CTA)
+        const uint32_t idesc = (1u << 4) | (1u << 15) | ((uint32_t)(c.nt >> 3) << 17) | ((256u >> 4) << 24);
+        mbar_wait(&tempty_bar[acc], acc_phase ^ 1u);
+        tc_fence_after();
+        const uint32_t d_main = tmem_base + (uint32_t)(acc * 256);
+        const uint32_t d_corr = d_main + 128;
+        for (int kb = 0; kb < c.kblocks; ++kb) {
+          mbar_wait(&full_bar[stage], phase);
+          tc_fence_after();
+          const uint32_t sa = smem_u32(smem + (size_t)stage * args.stage_bytes);
+          const int steps = kb == c.kblocks - 1 ? c.ktail : kBK / 16;
+          for (int k4 = 0; k4 < steps; ++k4) {
+            const uint64_t ad = make_smem_desc(sa + k4 * 2048, kBoxBytes, 1024);
+            const uint64_t bd = make_smem_desc(sa + off_b + k4 * 32, 16, 1024);
+            const uint32_t accum = (kb | k4) ? 1u : 0u;
+            tc_mma2_f16(d_main, ad, bd, idesc, accum);
+            if (split) {
+              const uint64_t adl = make_smem_desc(sa + off_a_lo + k4 * 2048, kBoxBytes, 1024);
+              const uint64_t bdl = make_smem_desc(sa + off_b_lo + k4 * 32, 16, 1024);
+              tc_mma2_f16(d_corr, ad, bdl, idesc, accum);
+              tc_mma2_f16(d_corr, adl, bd, idesc, 1u);
+            }
+          }
+          tc_commit_both(&empty_bar[stage]);
+          if (++stage == args.stages) { stage = 0; phase ^= 1u; }
+        }
+        tc_commit_both(&tfull_bar[acc]);
+        if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
+      }
+    }
+  } else {
+    // ===================== epilogue (both CTAs: each drains its own 128 TMEM lanes) =====================
+    const int q = warp & 3;
+    const int chunk_first = (warp - 3) >> 2;
+    int slot = 0, acc = 0;
+    uint32_t ring_phase = 0, acc_phase = 0;
+    const int limit = pg.fixed_iter > 0 ? min(pg.fixed_iter, pg.max_iter) : pg.max_iter;
+    for (;;) {
+      mbar_wait(&cmd_full[slot], ring_phase);
+      const TileCmd c = cmds[slot];
+      __syncwarp();
+      if (lane == 0) mbar_arrive_cluster(mapa(smem_u32(&cmd_empty[slot]), 0));
+      if (++slot == kRing) { slot = 0; ring_phase ^= 1u; }
+      if (c.op < 0) break;
+      const ChainOp &o = pg.ops[c.op];
+      const int par = c.iter & 1;
+      const int n = args.dims[c.mat];
+      const int r = c.m0 + 128 * (int)rank + q * 32 + lane;
+      const bool rows_in = c.m0 + 128 * (int)rank < args.ld;    // the peer's half of the last pair tile may lie
+                                                                // beyond the leading dimension: nothing to store
+      const int64_t base = (int64_t)c.mat * args.slab + r;
+      const bool split = o.a_lo[par] >= 0;
+      const bool ident = o.mode == EPI_IDENT;
+      const bool has_cin = !ident && o.cin32 >= 0 && o.beta != 0.f && rows_in;
+      const float alpha = o.use_div ? o.alpha / args.alpha_div[c.mat] : o.alpha;
+      float *cout32 = (o.cout32 >= 0 && rows_in) ? args.ubuf[o.cout32] : nullptr;
+      __half *out16 = (o.out16[par] >= 0 && rows_in) ? args.hbuf[o.out16[par]] : nullptr;
+      __half *out16_lo = (o.out16_lo[par] >= 0 && rows_in) ? args.hbuf[o.out16_lo[par]] : nullptr;
+      const int nchunks = (c.nt + 31) >> 5;
+      const int64_t tile_off = base + (int64_t)c.n0 * args.ld;   // element (r, n0)
+      float *p32 = cout32 ? cout32 + tile_off : nullptr;
+      __half *p16 = out16 ? out16 + tile_off : nullptr;
+      __half *p16l = out16_lo ? out16_lo + tile_off : nullptr;
+      const int store_kind = (p32 ? 1 : 0) | (p16 ? 2 : 0) | (p16l ? 4 : 0);
+      const int64_t chunk_stride = (int64_t)32 * args.ld;
+      if (p32) p32 += chunk_first * chunk_stride;
+      if (p16) p16 += chunk_first * chunk_stride;
+      if (p16l) p16l += chunk_first * chunk_stride;
+      const float *cinp = has_cin ? args.ubuf[o.cin32] + tile_off + chunk_first * chunk_stride : nullptr;
+      float cpre[32];
+      if (has_cin && chunk_first < nchunks) {
+        const float *pc = cinp;
+#pragma unroll
+        for (int j = 0; j < 32; ++j) { cpre[j] = __ldcg(pc); pc += args.ld; }
+      }
+      mbar_wait(&tfull_bar[acc], acc_phase);
+      tc_fence_after();
+      const uint32_t t_main = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(acc * 256);
+      float ss = 0.f;
+      for (int ci = chunk_first; ci < nchunks && rows_in; ci += 2) {
+        const int c0 = ci * 32;
+        uint32_t v[32];
+        tc_ld32(t_main + c0, v);
+        if (split) {
+          uint32_t w[32];
+          tc_ld32(t_main + 128 + c0, w);
+          tc_ld_wait();
+#pragma unroll
+          for (int j = 0; j < 32; ++j)
+            v[j] = __float_as_uint(fmaf(__uint_as_float(w[j]), 1.f / 2048.f, __uint_as_float(v[j])));
+        } else {
+          tc_ld_wait();
+        }
+        if (has_cin) {
+#pragma unroll
+          for (int j = 0; j < 32; ++j)
+            v[j] = __float_as_uint(fmaf(o.beta, cpre[j], alpha * __uint_as_float(v[j])));
+          if (ci + 2 < nchunks) {
+            cinp += 2 * chunk_stride;
+            const float *pc = cinp;
+#pragma unroll
+            for (int j = 0; j < 32; ++j) { cpre[j] = __ldcg(pc); pc += args.ld; }
+          }
+        } else if (ident) {
+          const int nvalid = (r < n) ? min(32, n - (c.n0 + c0)) : 0;
+          const int dj = r - (c.n0 + c0);
+#pragma unroll
+          for (int j = 0; j < 32; ++j) {
+            const float e = ((j == dj) ? 1.f : 0.f) - __uint_as_float(v[j]);
+            if (j < nvalid) ss = fmaf(e, e, ss);
+            v[j] = __float_as_uint(e);
+          }
+        } else {
+#pragma unroll
+          for (int j = 0; j < 32; ++j) v[j] = __float_as_uint(alpha * __uint_as_float(v[j]));
+        }
+        switch (store_kind) {   // tiles are multiples of 32 columns wide here: always full chunks
+          case 1: store_cols<true, false, false>(v, p32, p16, p16l, args.ld, true); break;
+          case 2: store_cols<false, true, false>(v, p32, p16, p16l, args.ld, true); break;
+          case 3: store_cols<true, true, false>(v, p32, p16, p16l, args.ld, true); break;
+          case 6: store_cols<false, true, true>(v, p32, p16, p16l, args.ld, true); break;
+          case 7: store_cols<true, true, true>(v, p32, p16, p16l, args.ld, true); break;
+          default: break;
+        }
+        if (p32) p32 += 2 * chunk_stride;
+        if (p16) p16 += 2 * chunk_stride;
+        if (p16l) p16l += 2 * chunk_stride;
+      }
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive_cluster(mapa(smem_u32(&tempty_bar[acc]), 0));
+      if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
+      fence_proxy_async();     // our generic-proxy stores -> later TMA reads (any CTA)
+      __syncwarp();
+      if (o.resid) {
+        for (int d = 16; d > 0; d >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, d);
+        if (lane == 0) atomicAdd(&args.resid2[(size_t)(c.iter % NOLSM_MAX_RESID_SLOTS) * args.count + c.mat], ss);
+      }
+      if (lane == 0) {
+        // completion: one arrival per epilogue warp of either CTA; the last arrival of the op publishes it
+        const int n32 = (n + 31) & ~31;
+        const int tiles_m = ((n + kTileM - 1) / kTileM) * ((n32 + args.bn - 1) / args.bn);
+        const int need = c.iter * pg.n_ops + c.op;
+        __threadfence();
+        const int32_t old = atomicAdd(&args.tiles_done[c.mat], 1);
+        if (old + 1 == (need + 1) * tiles_m * 2 * kEpiWarps) {
+          __threadfence();
+          const int k = c.iter;
+          if (o.resid) {
+            const float r2 = *reinterpret_cast<volatile float *>(
+                &args.resid2[(size_t)(k % NOLSM_MAX_RESID_SLOTS) * args.count + c.mat]);
+            const float res = sqrtf(fmaxf(r2, 0.f) / (float)n);
+            args.lastres[c.mat] = res;
+            args.iters[c.mat] = k + 1;
+            bool stop = pg.fixed_iter > 0 ? (k + 1 >= pg.fixed_iter) : ((res < pg.tol) || !(res == res));
+            if (k + 1 >= pg.max_iter) stop = true;
+            if (stop) *reinterpret_cast<volatile int32_t *>(&args.state[c.mat]) = k;
+          }
+          const int32_t stv = *reinterpret_cast<volatile int32_t *>(&args.state[c.mat]);
+          if (c.op == pg.n_ops - 1 && (stv == k || k + 1 >= limit)) {
+            st_release(&args.ready[c.mat], kDone);
+            __threadfence();
+            atomicSub(&args.group_active[c.mat / pg.group], 1);
+          } else {
+            st_release(&args.ready[c.mat], need + 1);
+          }
+        }
+      }
+    }
+  }
+
+  tc_fence_before();
+  __syncthreads();
+  cluster_sync();            // nobody leaves while the peer may still signal our barriers or read our smem
+  if (warp == 1) {
+    tc_fence_after();
+    asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(kTmemCols) : "memory");
+  }
+}
+
+}  // namespace pair
+
+nolsm_status pair_init(nolsm_ctx *ctx) {
+  ctx->pair_ok = false;
+  cudaError_t e = cudaFuncSetAttribute(pair::k_chain_pair, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                       pair::kSmemLimit);
+  if (e != cudaSuccess) { cudaGetLastError(); return NOLSM_ECUDA; }
+  // all pairs must be co-resident: the CTAs wait on one another through global flags
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)(ctx->sm_count & ~1));
+  cfg.blockDim = dim3(pair::kThreads);
+  cfg.dynamicSmemBytes = pair::kSmemLimit;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeClusterDimension;
+  at[0].val.clusterDim.x = 2; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = 1;
+  int max_clusters = 0;
+  e = cudaOccupancyMaxActiveClusters(&max_clusters, pair::k_chain_pair, &cfg);
+  if (e != cudaSuccess || max_clusters < 1) { cudaGetLastError(); return NOLSM_ECUDA; }
+  ctx->pair_clusters = std::min(max_clusters, ctx->sm_count / 2);
+  ctx->pair_ok = true;
+  return NOLSM_OK;
+}
+
+// Same contract as the single-CTA launch in chain_umma.cu; the control state has been reset by the caller.
+cudaError_t launch_chain_pair(nolsm_ctx *ctx, const nolsm_batch *b, const ChainProgram &prog, const float *alpha_div,
+                              cudaStream_t st) {
+  using namespace pair;
+  PairArgs a;
+  memset(&a, 0, sizeof(a));
+  a.prog = prog;
+  bool split = false;
+  for (int i = 0; i < prog.n_ops; ++i) split |= prog.ops[i].a_lo[0] >= 0 || prog.ops[i].a_lo[1] >= 0;
+  const int n32max = (b->max_n + 31) & ~31;
+  a.bn = std::min(split ? 128 : 256, n32max);
+  a.b_bytes = (((a.bn >> 1) + 63) / 64) * kBoxBytes;
+  a.stage_bytes = (kATileBytes + a.b_bytes) * (split ? 2 : 1);
+  a.stages = std::min(kMaxStages, (kSmemLimit - 1024) / a.stage_bytes);
+  a.mt = (b->max_n + kTileM - 1) / kTileM;
+  a.ntl = (n32max + a.bn - 1) / a.bn;
+  a.maps = b->d_maps;
+  for (int i = 0; i < b->n_half; ++i) a.hbuf[i] = b->h[i];
+  for (int i = 0; i < b->n_unit; ++i) a.ubuf[i] = b->u[i];
+  a.count = b->count;
+  a.ld = b->ld;
+  a.slab = (int64_t)b->ld * b->ld;
+  a.dims = b->d_dims;
+  a.alpha_div = alpha_div;
+  a.ready = b->d_ready;
+  a.tiles_done = b->d_tiles_done;
+  a.state = b->d_state;
+  a.iters = b->d_iters;
+  a.group_active = b->d_group_active;
+  a.resid2 = b->d_resid2;
+  a.lastres = b->d_lastres;
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)(2 * ctx->pair_clusters));
+  cfg.blockDim = dim3(kThreads);
+  cfg.dynamicSmemBytes = (size_t)(a.stages * a.stage_bytes + 1024);
+  cfg.stream = st;
+  cudaLaunchAttribute at[2];
+  at[0].id = cudaLaunchAttributeClusterDimension;
+  at[0].val.clusterDim.x = 2; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+  at[1].id = cudaLaunchAttributeCooperative;
+  at[1].val.cooperative = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = 2;
+  return cudaLaunchKernelEx(&cfg, k_chain_pair, a);
+}

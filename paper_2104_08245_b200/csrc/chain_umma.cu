@@ -590,6 +590,7 @@ nolsm_status umma_init(nolsm_ctx *ctx) {
     return NOLSM_ECUDA;
   }
   ctx->umma_ok = true;
+  pair_init(ctx);   // optional: the single-CTA engine is the fallback
   return NOLSM_OK;
 }
 
@@ -656,6 +657,7 @@ cudaError_t launch_chain(nolsm_ctx *ctx, const nolsm_batch *b, const ChainProgra
                                     a.resid2, slots * b->count, a.iters, a.lastres, touch_stats ? 1 : 0);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
+  if (ctx->pair_ok && (ctx->cfg.flags & NOLSM_FLAG_PAIR)) return launch_chain_pair(ctx, b, a.prog, alpha_div, st);
   const int smem_bytes = a.stages * a.stage_bytes + 1024;
   void *params[] = {&a};
   return cudaLaunchCooperativeKernel(reinterpret_cast<void *>(k_chain), dim3(ctx->sm_count), dim3(kThreads), params,
