@@ -104,6 +104,7 @@ static void free_batch(nolsm_batch *b) {
   cudaFree(b->d_ready);
   cudaFree(b->d_tiles_done);
   cudaFree(b->d_group_active);
+  cudaFree(b->d_tile_counter);
   cudaFree(b->d_maps);
   delete b;
 }
@@ -195,7 +196,7 @@ static nolsm_status setup_batch(nolsm_ctx *ctx, int slot, const std::vector<int3
     if (grow(&b->d_dims, cap) || grow(&b->d_state, cap) || grow(&b->d_iters, cap) ||
         grow(&b->d_resid2, cap * NOLSM_MAX_RESID_SLOTS) || grow(&b->d_lastres, cap) ||
         grow(&b->d_scale, cap) || grow(&b->d_norm, cap * 2) || grow(&b->d_ready, cap) ||
-        grow(&b->d_tiles_done, cap) || grow(&b->d_group_active, cap) ||
+        grow(&b->d_tiles_done, cap) || grow(&b->d_group_active, cap) || grow(&b->d_tile_counter, (size_t)1) ||
         (b->d_active == nullptr && grow(&b->d_active, (size_t)NOLSM_MAX_RESID_SLOTS))) {
       cudaGetLastError();
       ctx->err = "cudaMalloc of batch metadata failed";

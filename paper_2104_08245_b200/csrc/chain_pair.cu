@@ -15,8 +15,12 @@
 //   * the leader's single MMA thread issues for both CTAs and releases smem stages / publishes the
 //     accumulator in both CTAs with tcgen05.commit ... multicast::cluster.
 #include "common.cuh"
+#include "chain_epilogue.cuh"
 
 namespace pair {
+
+using chainep::TileCmd;
+typedef chainep::ChainArgs PairArgs;
 
 constexpr int kThreads = 352;
 constexpr int kEpiWarps = 8;
@@ -25,7 +29,7 @@ constexpr int kMaxStages = 8;
 constexpr int kTmemCols = 512;
 constexpr int kBoxBytes = 64 * 128;
 constexpr int kATileBytes = 2 * kBoxBytes;     // this CTA's 128 rows x 64 K
-constexpr int kRing = 4;
+constexpr int kRing = 2;
 constexpr int kSmemLimit = 232448 - 2048;
 constexpr int32_t kDone = 0x7fffffff;
 constexpr int kTileM = 256;                    // rows of a pair tile
@@ -153,26 +157,15 @@ __device__ __forceinline__ void store_cols(const uint32_t (&v)[32], float *p32, 
   }
 }
 
-struct TileCmd {              // scheduler -> TMA producers, MMA issuer and epilogue warps of both CTAs
-  int32_t mat, m0, n0, nt;    // submatrix, first row of the PAIR tile / first column, tile columns (mult. of 32)
-  int32_t kblocks, ktail;     // K blocks of 64; K=16 steps in the last one (1..4)
-  int32_t op, iter;           // op < 0: no more tiles
-};
-
-struct PairArgs {
-  ChainProgram prog;
-  const CUtensorMap *maps;
-  __half *hbuf[NOLSM_MAX_HALF];
-  float *ubuf[NOLSM_MAX_UNIT];
-  int32_t count, ld;
-  int64_t slab;
-  int32_t bn, b_bytes, stages, stage_bytes;   // b_bytes: this CTA's half of the B tile
-  int32_t mt, ntl;            // uniform tile grid per submatrix: mt pair-row tiles x ntl column tiles
-  const int32_t *dims;
-  const float *alpha_div;
-  int32_t *ready, *tiles_done, *state, *iters, *group_active;
-  float *resid2, *lastres;
-};
+#ifdef NOLSM_TRACE
+__device__ long long g_ptrace[4][4096][2];
+__device__ long long g_pwait[4096][4];
+#define PTRACE(role, ti, j) do { if (blockIdx.x == 0 && (ti) < 4096) g_ptrace[role][ti][j] = clock64(); } while (0)
+#define PTRACEV(role, ti, j, v) do { if (blockIdx.x == 0 && (ti) < 4096) g_ptrace[role][ti][j] = (v); } while (0)
+#else
+#define PTRACE(role, ti, j)
+#define PTRACEV(role, ti, j, v)
+#endif
 
 __global__ void __launch_bounds__(kThreads, 1) k_chain_pair(const PairArgs args) {
   extern __shared__ __align__(1024) uint8_t smem_raw[];
@@ -232,32 +225,43 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain_pair(const PairArgs args)
         mbar_arrive_cluster(mapa(smem_u32(&cmd_full[slot]), 1));
         if (++slot == kRing) { slot = 0; ring_phase ^= 1u; }
       };
-      for (int g = 0; g < n_groups; ++g) {
+      // Dynamic, in-order tile claims: a tile only depends on tiles with a smaller index, all of which
+      // have been claimed by running CTAs, so the schedule cannot deadlock and balances itself.
+      const int64_t per_group = (int64_t)limit * pg.n_ops * pg.group * T;   // index space of one (full) group
+      int g_checked = -1, k_checked = 0;
+      for (;;) {
+        const int64_t L = (int64_t)atomicAdd(args.tile_counter, 1ull);
+        const int g = (int)(L / per_group);
+        if (g >= n_groups) break;
+        const int64_t Lg = L - (int64_t)g * per_group;
         const int gbase = g * pg.group;
         const int gs = min(pg.group, args.count - gbase);
         const int per_seg = gs * T;
-        const int64_t total = (int64_t)limit * pg.n_ops * per_seg;
-        int k_checked = 0;
-        for (int64_t L = cluster_id; L < total; L += n_clusters) {
-          const int seg = (int)(L / per_seg), rem = (int)(L % per_seg);
-          const int k = seg / pg.n_ops, op = seg % pg.n_ops;
-          if (k != k_checked) {   // whole group converged: go to the next group
-            if (ld_acquire(&args.group_active[g]) == 0) break;
-            k_checked = k;
+        if (Lg >= (int64_t)limit * pg.n_ops * per_seg) continue;   // index padding of the last group
+        const int seg = (int)(Lg / per_seg), rem = (int)(Lg % per_seg);
+        const int k = seg / pg.n_ops, op = seg % pg.n_ops;
+        if (g != g_checked) { g_checked = g; k_checked = 0; }
+        if (k != k_checked) {   // whole group converged: move the claim counter past it
+          if (ld_acquire(&args.group_active[g]) == 0) {
+            atomicMax(args.tile_counter, (unsigned long long)((int64_t)(g + 1) * per_group));
+            continue;
           }
-          const int ml = rem / T, t = rem % T;
-          const int m = gbase + ml;
-          const int n = args.dims[m];
-          const int n16 = (n + 15) & ~15, n32 = (n + 31) & ~31;
-          const int m0 = (t % args.mt) * kTileM, n0 = (t / args.mt) * args.bn;
-          if (m0 >= n || n0 >= n32) continue;          // tile outside this submatrix
-          const int need = k * pg.n_ops + op;          // ops of this submatrix that must be complete
-          if (need > 0) {
-            int32_t r = ld_acquire(&args.ready[m]);
-            while (r < need) { __nanosleep(64); r = ld_acquire(&args.ready[m]); }
-            if (r == kDone) continue;                  // submatrix finished at an earlier iteration
-          }
-          const int kblocks = (n16 + kBK - 1) / kBK;
+          k_checked = k;
+        }
+        const int ml = rem / T, t = rem % T;
+        const int m = gbase + ml;
+        const int n = args.dims[m];
+        const int n16 = (n + 15) & ~15, n32 = (n + 31) & ~31;
+        const int m0 = (t % args.mt) * kTileM, n0 = (t / args.mt) * args.bn;
+        if (m0 >= n || n0 >= n32) continue;          // tile outside this submatrix
+        const int need = k * pg.n_ops + op;          // ops of this submatrix that must be complete
+        if (need > 0) {
+          int32_t r = ld_acquire(&args.ready[m]);
+          while (r < need) { __nanosleep(64); r = ld_acquire(&args.ready[m]); }
+          if (r == kDone) continue;                  // submatrix finished at an earlier iteration
+        }
+        const int kblocks = (n16 + kBK - 1) / kBK;
+        {
           push(TileCmd{m, m0, n0, min(args.bn, n32 - n0), kblocks, (n16 - (kblocks - 1) * kBK) / 16, op, k});
         }
       }
@@ -266,6 +270,9 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain_pair(const PairArgs args)
   } else if (warp == 2) {
     // ===================== TMA producer (both CTAs) =====================
     if (lane == 0) {
+#ifdef NOLSM_TRACE
+      int tti = 0;
+#endif
       int stage = 0, slot = 0;
       uint32_t phase = 0, ring_phase = 0;
       for (;;) {
@@ -274,6 +281,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain_pair(const PairArgs args)
         mbar_arrive_cluster(mapa(smem_u32(&cmd_empty[slot]), 0));
         if (++slot == kRing) { slot = 0; ring_phase ^= 1u; }
         if (c.op < 0) break;
+        PTRACE(2, tti, 0);
         fence_proxy_async();   // other CTAs' generic-proxy writes (ordered by the scheduler's acquire) -> TMA reads
         const ChainOp &o = pg.ops[c.op];
         const int par = c.iter & 1;
@@ -304,11 +312,18 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain_pair(const PairArgs args)
           }
           if (++stage == args.stages) { stage = 0; phase ^= 1u; }
         }
+        PTRACE(2, tti, 1);
+#ifdef NOLSM_TRACE
+        ++tti;
+#endif
       }
     }
   } else if (warp == 1) {
     // ===================== MMA issuer (leader CTA only, for both CTAs) =====================
     if (leader && lane == 0) {
+#ifdef NOLSM_TRACE
+      int mti = 0;
+#endif
       int stage = 0, slot = 0, acc = 0;
       uint32_t phase = 0, ring_phase = 0, acc_phase = 0;
       for (;;) {
@@ -320,12 +335,27 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain_pair(const PairArgs args)
         const bool split = pg.ops[c.op].a_lo[c.iter & 1] >= 0;
         // instruction descriptor: D=F32, A=B=F16, A M-major, B K-major, N = nt, M = 256 (128 per CTA)
         const uint32_t idesc = (1u << 4) | (1u << 15) | ((uint32_t)(c.nt >> 3) << 17) | ((256u >> 4) << 24);
+        PTRACE(0, mti, 0);
         mbar_wait(&tempty_bar[acc], acc_phase ^ 1u);
         tc_fence_after();
+        PTRACE(0, mti, 1);
+#ifdef NOLSM_TRACE
+        ++mti;
+#endif
         const uint32_t d_main = tmem_base + (uint32_t)(acc * 256);
         const uint32_t d_corr = d_main + 128;
+#ifdef NOLSM_TRACE
+        long long wsum = 0, t_first = 0, t_begin = clock64();
+#endif
         for (int kb = 0; kb < c.kblocks; ++kb) {
+#ifdef NOLSM_TRACE
+          long long w0 = clock64();
+#endif
           mbar_wait(&full_bar[stage], phase);
+#ifdef NOLSM_TRACE
+          wsum += clock64() - w0;
+          if (kb == 0) t_first = clock64() - w0;
+#endif
           tc_fence_after();
           const uint32_t sa = smem_u32(smem + (size_t)stage * args.stage_bytes);
           const int steps = kb == c.kblocks - 1 ? c.ktail : kBK / 16;
@@ -345,6 +375,9 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain_pair(const PairArgs args)
           if (++stage == args.stages) { stage = 0; phase ^= 1u; }
         }
         tc_commit_both(&tfull_bar[acc]);
+#ifdef NOLSM_TRACE
+        if (blockIdx.x == 0 && mti - 1 < 4096) { g_pwait[mti - 1][0] = wsum; g_pwait[mti - 1][1] = t_first; g_pwait[mti - 1][2] = clock64() - t_begin; }
+#endif
         if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
       }
     }
@@ -352,9 +385,11 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain_pair(const PairArgs args)
     // ===================== epilogue (both CTAs: each drains its own 128 TMEM lanes) =====================
     const int q = warp & 3;
     const int chunk_first = (warp - 3) >> 2;
-    int slot = 0, acc = 0;
+#ifdef NOLSM_TRACE
+    int eti = 0;
+#endif
+    int slot = 0, acc = 0, tile_seq = 0;
     uint32_t ring_phase = 0, acc_phase = 0;
-    const int limit = pg.fixed_iter > 0 ? min(pg.fixed_iter, pg.max_iter) : pg.max_iter;
     for (;;) {
       mbar_wait(&cmd_full[slot], ring_phase);
       const TileCmd c = cmds[slot];
@@ -362,130 +397,32 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain_pair(const PairArgs args)
       if (lane == 0) mbar_arrive_cluster(mapa(smem_u32(&cmd_empty[slot]), 0));
       if (++slot == kRing) { slot = 0; ring_phase ^= 1u; }
       if (c.op < 0) break;
-      const ChainOp &o = pg.ops[c.op];
-      const int par = c.iter & 1;
-      const int n = args.dims[c.mat];
-      const int r = c.m0 + 128 * (int)rank + q * 32 + lane;
-      const bool rows_in = c.m0 + 128 * (int)rank < args.ld;    // the peer's half of the last pair tile may lie
-                                                                // beyond the leading dimension: nothing to store
-      const int64_t base = (int64_t)c.mat * args.slab + r;
-      const bool split = o.a_lo[par] >= 0;
-      const bool ident = o.mode == EPI_IDENT;
-      const bool has_cin = !ident && o.cin32 >= 0 && o.beta != 0.f && rows_in;
-      const float alpha = o.use_div ? o.alpha / args.alpha_div[c.mat] : o.alpha;
-      float *cout32 = (o.cout32 >= 0 && rows_in) ? args.ubuf[o.cout32] : nullptr;
-      __half *out16 = (o.out16[par] >= 0 && rows_in) ? args.hbuf[o.out16[par]] : nullptr;
-      __half *out16_lo = (o.out16_lo[par] >= 0 && rows_in) ? args.hbuf[o.out16_lo[par]] : nullptr;
-      const int nchunks = (c.nt + 31) >> 5;
-      const int64_t tile_off = base + (int64_t)c.n0 * args.ld;   // element (r, n0)
-      float *p32 = cout32 ? cout32 + tile_off : nullptr;
-      __half *p16 = out16 ? out16 + tile_off : nullptr;
-      __half *p16l = out16_lo ? out16_lo + tile_off : nullptr;
-      const int store_kind = (p32 ? 1 : 0) | (p16 ? 2 : 0) | (p16l ? 4 : 0);
-      const int64_t chunk_stride = (int64_t)32 * args.ld;
-      if (p32) p32 += chunk_first * chunk_stride;
-      if (p16) p16 += chunk_first * chunk_stride;
-      if (p16l) p16l += chunk_first * chunk_stride;
-      const float *cinp = has_cin ? args.ubuf[o.cin32] + tile_off + chunk_first * chunk_stride : nullptr;
-      float cpre[32];
-      if (has_cin && chunk_first < nchunks) {
-        const float *pc = cinp;
-#pragma unroll
-        for (int j = 0; j < 32; ++j) { cpre[j] = __ldcg(pc); pc += args.ld; }
-      }
+      // the peer's half of the last pair tile may lie beyond the leading dimension: nothing to load or store
+      const bool rows_in = c.m0 + 128 * (int)rank < args.ld;
+      chainep::EpiTile t;
+      chainep::epi_begin(args, c, c.m0 + 128 * (int)rank + q * 32, rows_in, lane, chunk_first, t);
+      if (warp == 3 && lane == 0) { PTRACE(1, eti, 0); }
       mbar_wait(&tfull_bar[acc], acc_phase);
       tc_fence_after();
+      if (warp == 3 && lane == 0) { PTRACE(1, eti, 1); PTRACEV(3, eti, 0, ((long long)c.mat << 40) | ((long long)c.iter << 32) | ((long long)c.op << 24) | ((long long)(c.m0 / 256) << 8) | (long long)(c.n0 / 64)); }
       const uint32_t t_main = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(acc * 256);
-      float ss = 0.f;
-      for (int ci = chunk_first; ci < nchunks && rows_in; ci += 2) {
-        const int c0 = ci * 32;
-        uint32_t v[32];
-        tc_ld32(t_main + c0, v);
-        if (split) {
-          uint32_t w[32];
-          tc_ld32(t_main + 128 + c0, w);
-          tc_ld_wait();
-#pragma unroll
-          for (int j = 0; j < 32; ++j)
-            v[j] = __float_as_uint(fmaf(__uint_as_float(w[j]), 1.f / 2048.f, __uint_as_float(v[j])));
-        } else {
-          tc_ld_wait();
-        }
-        if (has_cin) {
-#pragma unroll
-          for (int j = 0; j < 32; ++j)
-            v[j] = __float_as_uint(fmaf(o.beta, cpre[j], alpha * __uint_as_float(v[j])));
-          if (ci + 2 < nchunks) {
-            cinp += 2 * chunk_stride;
-            const float *pc = cinp;
-#pragma unroll
-            for (int j = 0; j < 32; ++j) { cpre[j] = __ldcg(pc); pc += args.ld; }
-          }
-        } else if (ident) {
-          const int nvalid = (r < n) ? min(32, n - (c.n0 + c0)) : 0;
-          const int dj = r - (c.n0 + c0);
-#pragma unroll
-          for (int j = 0; j < 32; ++j) {
-            const float e = ((j == dj) ? 1.f : 0.f) - __uint_as_float(v[j]);
-            if (j < nvalid) ss = fmaf(e, e, ss);
-            v[j] = __float_as_uint(e);
-          }
-        } else {
-#pragma unroll
-          for (int j = 0; j < 32; ++j) v[j] = __float_as_uint(alpha * __uint_as_float(v[j]));
-        }
-        switch (store_kind) {   // tiles are multiples of 32 columns wide here: always full chunks
-          case 1: store_cols<true, false, false>(v, p32, p16, p16l, args.ld, true); break;
-          case 2: store_cols<false, true, false>(v, p32, p16, p16l, args.ld, true); break;
-          case 3: store_cols<true, true, false>(v, p32, p16, p16l, args.ld, true); break;
-          case 6: store_cols<false, true, true>(v, p32, p16, p16l, args.ld, true); break;
-          case 7: store_cols<true, true, true>(v, p32, p16, p16l, args.ld, true); break;
-          default: break;
-        }
-        if (p32) p32 += 2 * chunk_stride;
-        if (p16) p16 += 2 * chunk_stride;
-        if (p16l) p16l += 2 * chunk_stride;
-      }
+      float ss = chainep::epi_chunks(args, c, t, t_main, lane);
       tc_fence_before();
       __syncwarp();
       if (lane == 0) mbar_arrive_cluster(mapa(smem_u32(&tempty_bar[acc]), 0));
       if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
-      fence_proxy_async();     // our generic-proxy stores -> later TMA reads (any CTA)
-      __syncwarp();
-      if (o.resid) {
+      if (t.o->resid) {
         for (int d = 16; d > 0; d >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, d);
         if (lane == 0) atomicAdd(&args.resid2[(size_t)(c.iter % NOLSM_MAX_RESID_SLOTS) * args.count + c.mat], ss);
       }
-      if (lane == 0) {
-        // completion: one arrival per epilogue warp of either CTA; the last arrival of the op publishes it
-        const int n32 = (n + 31) & ~31;
-        const int tiles_m = ((n + kTileM - 1) / kTileM) * ((n32 + args.bn - 1) / args.bn);
-        const int need = c.iter * pg.n_ops + c.op;
-        __threadfence();
-        const int32_t old = atomicAdd(&args.tiles_done[c.mat], 1);
-        if (old + 1 == (need + 1) * tiles_m * 2 * kEpiWarps) {
-          __threadfence();
-          const int k = c.iter;
-          if (o.resid) {
-            const float r2 = *reinterpret_cast<volatile float *>(
-                &args.resid2[(size_t)(k % NOLSM_MAX_RESID_SLOTS) * args.count + c.mat]);
-            const float res = sqrtf(fmaxf(r2, 0.f) / (float)n);
-            args.lastres[c.mat] = res;
-            args.iters[c.mat] = k + 1;
-            bool stop = pg.fixed_iter > 0 ? (k + 1 >= pg.fixed_iter) : ((res < pg.tol) || !(res == res));
-            if (k + 1 >= pg.max_iter) stop = true;
-            if (stop) *reinterpret_cast<volatile int32_t *>(&args.state[c.mat]) = k;
-          }
-          const int32_t stv = *reinterpret_cast<volatile int32_t *>(&args.state[c.mat]);
-          if (c.op == pg.n_ops - 1 && (stv == k || k + 1 >= limit)) {
-            st_release(&args.ready[c.mat], kDone);
-            __threadfence();
-            atomicSub(&args.group_active[c.mat / pg.group], 1);
-          } else {
-            st_release(&args.ready[c.mat], need + 1);
-          }
-        }
-      }
+      // all epilogue warps of this CTA have issued their stores: one thread publishes the CTA's half
+      asm volatile("bar.sync 1, %0;" ::"n"(kEpiWarps * 32) : "memory");
+      if (warp - 3 == (tile_seq & (kEpiWarps - 1)) && lane == 0) chainep::epi_complete<kTileM, 32, 2>(args, c);
+      ++tile_seq;
+      if (warp == 3 && lane == 0) { PTRACE(3, eti, 1); }
+#ifdef NOLSM_TRACE
+      ++eti;
+#endif
     }
   }
 
@@ -499,6 +436,14 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain_pair(const PairArgs args)
 }
 
 }  // namespace pair
+
+#ifdef NOLSM_TRACE
+extern "C" void nolsm_debug_ptrace(long long *host_out) {
+  cudaDeviceSynchronize();
+  cudaMemcpyFromSymbol(host_out, pair::g_ptrace, sizeof(pair::g_ptrace));
+}
+extern "C" void nolsm_debug_pwait(long long *host_out) { cudaMemcpyFromSymbol(host_out, pair::g_pwait, sizeof(pair::g_pwait)); }
+#endif
 
 nolsm_status pair_init(nolsm_ctx *ctx) {
   ctx->pair_ok = false;
@@ -540,6 +485,8 @@ cudaError_t launch_chain_pair(nolsm_ctx *ctx, const nolsm_batch *b, const ChainP
   a.mt = (b->max_n + kTileM - 1) / kTileM;
   a.ntl = (n32max + a.bn - 1) / a.bn;
   a.maps = b->d_maps;
+  a.n_half = b->n_half;
+  a.n_unit = b->n_unit;
   for (int i = 0; i < b->n_half; ++i) a.hbuf[i] = b->h[i];
   for (int i = 0; i < b->n_unit; ++i) a.ubuf[i] = b->u[i];
   a.count = b->count;
@@ -552,6 +499,7 @@ cudaError_t launch_chain_pair(nolsm_ctx *ctx, const nolsm_batch *b, const ChainP
   a.state = b->d_state;
   a.iters = b->d_iters;
   a.group_active = b->d_group_active;
+  a.tile_counter = b->d_tile_counter;
   a.resid2 = b->d_resid2;
   a.lastres = b->d_lastres;
   cudaLaunchConfig_t cfg = {};

@@ -30,6 +30,7 @@
 // epilogue (TMEM lane quadrant = warp_id % 4; the two warps of a quadrant take alternate 32-column
 // chunks of the tile).
 #include "common.cuh"
+#include "chain_epilogue.cuh"
 
 namespace {
 
@@ -40,7 +41,7 @@ constexpr int kMaxStages = 8;
 constexpr int kTmemCols = 512;
 constexpr int kBoxBytes = 64 * 128;      // one {64 x 64} FP16 box
 constexpr int kATileBytes = 2 * kBoxBytes;
-constexpr int kRing = 4;                 // tile-command ring depth
+constexpr int kRing = 2;                 // tile-command ring depth (how far the scheduler claims ahead)
 constexpr int kSmemLimit = 232448 - 2048;  // 227 KB minus the static part (barriers, commands)
 constexpr int32_t kDone = 0x7fffffff;
 
@@ -69,6 +70,19 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
       "}\n" ::"r"(smem_u32(bar)),
       "r"(parity)
       : "memory");
+}
+__device__ __forceinline__ bool mbar_test(uint64_t *bar, uint32_t parity) {
+  uint32_t ok;
+  asm volatile(
+      "{\n\t"
+      ".reg .pred p;\n\t"
+      "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+      "selp.b32 %0, 1, 0, p;\n\t"
+      "}\n"
+      : "=r"(ok)
+      : "r"(smem_u32(bar)), "r"(parity)
+      : "memory");
+  return ok != 0;
 }
 __device__ __forceinline__ void tma_load_3d(void *dst, const CUtensorMap *map, uint64_t *bar, int c0,
                                             int c1, int c2) {
@@ -157,32 +171,17 @@ __device__ __forceinline__ void store_cols(const uint32_t (&v)[32], float *p32, 
 __device__ long long g_trace[4][4096][2];
 #define TRACE(role, ti, j) do { if (blockIdx.x == 0 && (ti) < 4096) g_trace[role][ti][j] = clock64(); } while (0)
 #define TRACEV(role, ti, j, v) do { if (blockIdx.x == 0 && (ti) < 4096) g_trace[role][ti][j] = (v); } while (0)
+__device__ long long g_trace2[4096][8];
+__device__ long long g_wait[4096][4];
+#define TRACE2(ti, j) do { if (blockIdx.x == 0 && warp == 3 && lane == 0 && (ti) < 4096) g_trace2[ti][j] = clock64(); } while (0)
 #else
+#define TRACE2(ti, j)
 #define TRACE(role, ti, j)
 #define TRACEV(role, ti, j, v)
 #endif
 
-struct TileCmd {              // scheduler -> MMA issuer and epilogue warps
-  int32_t mat, m0, n0, nt;    // submatrix, first row / column, tile columns (multiple of 16, <= bn)
-  int32_t kblocks, ktail;     // K blocks of 64; K=16 steps in the last one (1..4)
-  int32_t op, iter;           // op < 0: no more tiles
-};
-
-struct ChainArgs {
-  ChainProgram prog;
-  const CUtensorMap *maps;    // [n_half] FP16 maps, then [n_unit] FP32 maps
-  __half *hbuf[NOLSM_MAX_HALF];
-  float *ubuf[NOLSM_MAX_UNIT];
-  int32_t n_half;
-  int32_t count, ld;
-  int64_t slab;
-  int32_t bn, b_bytes, stages, stage_bytes;
-  int32_t mt, ntl;            // uniform tile grid per submatrix: mt row tiles x ntl column tiles
-  const int32_t *dims;
-  const float *alpha_div;
-  int32_t *ready, *tiles_done, *state, *iters, *group_active;
-  float *resid2, *lastres;
-};
+using chainep::TileCmd;
+using chainep::ChainArgs;
 
 __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
   extern __shared__ __align__(1024) uint8_t smem_raw[];
@@ -222,36 +221,45 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
       const int T = args.mt * args.ntl;
       const int limit = pg.fixed_iter > 0 ? min(pg.fixed_iter, pg.max_iter) : pg.max_iter;
       const int n_groups = (args.count + pg.group - 1) / pg.group;
-      for (int g = 0; g < n_groups; ++g) {
+      // Dynamic, in-order tile claims: a tile only depends on tiles with a smaller index, all of which
+      // have been claimed by running CTAs, so the schedule cannot deadlock and balances itself.
+      const int64_t per_group = (int64_t)limit * pg.n_ops * pg.group * T;   // index space of one (full) group
+      int g_checked = -1, k_checked = 0;
+      for (;;) {
+        const int64_t L = (int64_t)atomicAdd(args.tile_counter, 1ull);
+        const int g = (int)(L / per_group);
+        if (g >= n_groups) break;
+        const int64_t Lg = L - (int64_t)g * per_group;
         const int gbase = g * pg.group;
         const int gs = min(pg.group, args.count - gbase);
         const int per_seg = gs * T;
-        const int64_t total = (int64_t)limit * pg.n_ops * per_seg;
-        int k_checked = 0;
-        for (int64_t L = blockIdx.x; L < total; L += gridDim.x) {
-          const int seg = (int)(L / per_seg), rem = (int)(L % per_seg);
-          const int k = seg / pg.n_ops, op = seg % pg.n_ops;
-          if (k != k_checked) {   // whole group converged: go to the next group
-            if (ld_acquire(&args.group_active[g]) == 0) break;
-            k_checked = k;
+        if (Lg >= (int64_t)limit * pg.n_ops * per_seg) continue;   // index padding of the last group
+        const int seg = (int)(Lg / per_seg), rem = (int)(Lg % per_seg);
+        const int k = seg / pg.n_ops, op = seg % pg.n_ops;
+        if (g != g_checked) { g_checked = g; k_checked = 0; }
+        if (k != k_checked) {   // whole group converged: move the claim counter past it
+          if (ld_acquire(&args.group_active[g]) == 0) {
+            atomicMax(args.tile_counter, (unsigned long long)((int64_t)(g + 1) * per_group));
+            continue;
           }
-          const int ml = rem / T, t = rem % T;
-          const int m = gbase + ml;
-          const int n = args.dims[m];
-          const int n16 = (n + 15) & ~15;
-          const int m0 = (t % args.mt) * NOLSM_TILE_M, n0 = (t / args.mt) * args.bn;
-          if (m0 >= n || n0 >= n16) continue;          // tile outside this submatrix
-          const int need = k * pg.n_ops + op;          // ops of this submatrix that must be complete
-          if (need > 0) {
-            int32_t r = ld_acquire(&args.ready[m]);
-            while (r < need) { __nanosleep(64); r = ld_acquire(&args.ready[m]); }
-            if (r == kDone) continue;                  // submatrix finished at an earlier iteration
-          }
-          const int nt = min(args.bn, n16 - n0);
-          const int kblocks = (n16 + kBK - 1) / kBK;
-          // command to the other roles
+          k_checked = k;
+        }
+        const int ml = rem / T, t = rem % T;
+        const int m = gbase + ml;
+        const int n = args.dims[m];
+        const int n16 = (n + 15) & ~15;
+        const int m0 = (t % args.mt) * NOLSM_TILE_M, n0 = (t / args.mt) * args.bn;
+        if (m0 >= n || n0 >= n16) continue;          // tile outside this submatrix
+        const int need = k * pg.n_ops + op;          // ops of this submatrix that must be complete
+        if (need > 0) {
+          int32_t r = ld_acquire(&args.ready[m]);
+          while (r < need) { __nanosleep(64); r = ld_acquire(&args.ready[m]); }
+          if (r == kDone) continue;                  // submatrix finished at an earlier iteration
+        }
+        const int kblocks = (n16 + kBK - 1) / kBK;
+        {
           mbar_wait(&cmd_empty[slot], ring_phase ^ 1u);
-          cmds[slot] = TileCmd{m, m0, n0, nt, kblocks, (n16 - (kblocks - 1) * kBK) / 16, op, k};
+          cmds[slot] = TileCmd{m, m0, n0, min(args.bn, n16 - n0), kblocks, (n16 - (kblocks - 1) * kBK) / 16, op, k};
           mbar_arrive(&cmd_full[slot]);
           if (++slot == kRing) { slot = 0; ring_phase ^= 1u; }
         }
@@ -334,8 +342,17 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
 #endif
         const uint32_t d_main = tmem_base + (uint32_t)(acc * 256);
         const uint32_t d_corr = d_main + 128;
+#ifdef NOLSM_TRACE
+        long long wsum = 0, t_begin = clock64();
+#endif
         for (int kb = 0; kb < c.kblocks; ++kb) {
+#ifdef NOLSM_TRACE
+          long long w0 = clock64();
+#endif
           mbar_wait(&full_bar[stage], phase);
+#ifdef NOLSM_TRACE
+          wsum += clock64() - w0;
+#endif
           tc_fence_after();
           const uint32_t sa = smem_u32(smem + (size_t)stage * args.stage_bytes);
           const int steps = kb == c.kblocks - 1 ? c.ktail : kBK / 16;
@@ -356,6 +373,9 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
           if (++stage == args.stages) { stage = 0; phase ^= 1u; }
         }
         tc_commit(&tfull_bar[acc]);
+#ifdef NOLSM_TRACE
+        if (blockIdx.x == 0 && mti - 1 < 4096) { g_wait[mti - 1][0] = wsum; g_wait[mti - 1][2] = clock64() - t_begin; }
+#endif
         if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
       }
     }
@@ -366,9 +386,8 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
     int eti = 0;
 #endif
     const int chunk_first = (warp - 3) >> 2;   // this warp's chunks: chunk_first, chunk_first + 2, ...
-    int slot = 0, acc = 0;
+    int slot = 0, acc = 0, tile_seq = 0;
     uint32_t ring_phase = 0, acc_phase = 0;
-    const int limit = pg.fixed_iter > 0 ? min(pg.fixed_iter, pg.max_iter) : pg.max_iter;
     for (;;) {
       mbar_wait(&cmd_full[slot], ring_phase);
       const TileCmd c = cmds[slot];
@@ -376,132 +395,33 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
       if (lane == 0) mbar_arrive(&cmd_empty[slot]);
       if (++slot == kRing) { slot = 0; ring_phase ^= 1u; }
       if (c.op < 0) break;
-      const ChainOp &o = pg.ops[c.op];
-      const int par = c.iter & 1;
-      const int n = args.dims[c.mat];
-      const int r = c.m0 + q * 32 + lane;
-      const int64_t base = (int64_t)c.mat * args.slab + r;
-      const bool split = o.a_lo[par] >= 0;
-      const bool ident = o.mode == EPI_IDENT;
-      const bool has_cin = !ident && o.cin32 >= 0 && o.beta != 0.f;
-      const float alpha = o.use_div ? o.alpha / args.alpha_div[c.mat] : o.alpha;
-      float *cout32 = o.cout32 >= 0 ? args.ubuf[o.cout32] : nullptr;
-      __half *out16 = o.out16[par] >= 0 ? args.hbuf[o.out16[par]] : nullptr;
-      __half *out16_lo = o.out16_lo[par] >= 0 ? args.hbuf[o.out16_lo[par]] : nullptr;
-      const int nchunks = (c.nt + 31) >> 5;
-      const int64_t tile_off = base + (int64_t)c.n0 * args.ld;   // element (r, n0)
-      float *p32 = cout32 ? cout32 + tile_off : nullptr;
-      __half *p16 = out16 ? out16 + tile_off : nullptr;
-      __half *p16l = out16_lo ? out16_lo + tile_off : nullptr;
-      const int store_kind = (p32 ? 1 : 0) | (p16 ? 2 : 0) | (p16l ? 4 : 0);
-      const int64_t chunk_stride = (int64_t)32 * args.ld;
-      if (p32) p32 += chunk_first * chunk_stride;
-      if (p16) p16 += chunk_first * chunk_stride;
-      if (p16l) p16l += chunk_first * chunk_stride;
-      // FP32 master of this row, one chunk ahead (columns beyond the tile stay inside the slab)
-      const float *cinp = has_cin ? args.ubuf[o.cin32] + tile_off + chunk_first * chunk_stride : nullptr;
-      float cpre[32];
-      if (has_cin && chunk_first < nchunks) {
-        const float *pc = cinp;
-#pragma unroll
-        for (int j = 0; j < 32; ++j) { cpre[j] = __ldcg(pc); pc += args.ld; }
-      }
+      chainep::EpiTile t;
+      chainep::epi_begin(args, c, c.m0 + q * 32, true, lane, chunk_first, t);
       if (warp == 3 && lane == 0) { TRACE(1, eti, 0); }
       mbar_wait(&tfull_bar[acc], acc_phase);
       tc_fence_after();
       if (warp == 3 && lane == 0) { TRACE(1, eti, 1); TRACEV(3, eti, 0, (long long)c.op); }
       const uint32_t t_main = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(acc * 256);
-      float ss = 0.f;
-      for (int ci = chunk_first; ci < nchunks; ci += 2) {
-        const int c0 = ci * 32;
-        const bool full = c.nt - c0 >= 32;
-        uint32_t v[32];
-        tc_ld32(t_main + c0, v);
-        if (split) {
-          uint32_t w[32];
-          tc_ld32(t_main + 128 + c0, w);
-          tc_ld_wait();
-#pragma unroll
-          for (int j = 0; j < 32; ++j)
-            v[j] = __float_as_uint(fmaf(__uint_as_float(w[j]), 1.f / 2048.f, __uint_as_float(v[j])));
-        } else {
-          tc_ld_wait();
-        }
-        if (has_cin) {
-#pragma unroll
-          for (int j = 0; j < 32; ++j)
-            v[j] = __float_as_uint(fmaf(o.beta, cpre[j], alpha * __uint_as_float(v[j])));
-          if (ci + 2 < nchunks) {
-            cinp += 2 * chunk_stride;
-            const float *pc = cinp;
-#pragma unroll
-            for (int j = 0; j < 32; ++j) { cpre[j] = __ldcg(pc); pc += args.ld; }
-          }
-        } else if (ident) {
-          // valid columns of this chunk inside the true n x n part (residual of the stop rule)
-          const int nvalid = (r < n) ? min(full ? 32 : 16, n - (c.n0 + c0)) : 0;
-          const int dj = r - (c.n0 + c0);     // chunk column that holds the diagonal element of row r
-#pragma unroll
-          for (int j = 0; j < 32; ++j) {
-            const float e = ((j == dj) ? 1.f : 0.f) - __uint_as_float(v[j]);
-            if (j < nvalid) ss = fmaf(e, e, ss);
-            v[j] = __float_as_uint(e);
-          }
-        } else {
-#pragma unroll
-          for (int j = 0; j < 32; ++j) v[j] = __float_as_uint(alpha * __uint_as_float(v[j]));
-        }
-        switch (store_kind) {
-          case 1: store_cols<true, false, false>(v, p32, p16, p16l, args.ld, full); break;
-          case 2: store_cols<false, true, false>(v, p32, p16, p16l, args.ld, full); break;
-          case 3: store_cols<true, true, false>(v, p32, p16, p16l, args.ld, full); break;
-          case 6: store_cols<false, true, true>(v, p32, p16, p16l, args.ld, full); break;
-          case 7: store_cols<true, true, true>(v, p32, p16, p16l, args.ld, full); break;
-          default: break;
-        }
-        if (p32) p32 += 2 * chunk_stride;
-        if (p16) p16 += 2 * chunk_stride;
-        if (p16l) p16l += 2 * chunk_stride;
-      }
+#ifdef NOLSM_TRACE
+      float ss = chainep::epi_chunks(args, c, t, t_main, lane,
+                                     (blockIdx.x == 0 && warp == 3 && eti < 4096) ? g_trace2[eti] : nullptr);
+#else
+      float ss = chainep::epi_chunks(args, c, t, t_main, lane);
+#endif
       tc_fence_before();
-      fence_proxy_async();     // our generic-proxy stores -> later TMA reads (any CTA)
       __syncwarp();
       if (lane == 0) mbar_arrive(&tempty_bar[acc]);
       if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
-      if (o.resid) {
+      if (t.o->resid) {
         for (int d = 16; d > 0; d >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, d);
         if (lane == 0) atomicAdd(&args.resid2[(size_t)(c.iter % NOLSM_MAX_RESID_SLOTS) * args.count + c.mat], ss);
       }
-      if (lane == 0) {
-        // completion: one arrival per epilogue warp and tile; the last arrival of the op publishes it
-        const int n16 = (n + 15) & ~15;
-        const int tiles_m = ((n + NOLSM_TILE_M - 1) / NOLSM_TILE_M) * ((n16 + args.bn - 1) / args.bn);
-        const int need = c.iter * pg.n_ops + c.op;
-        __threadfence();
-        const int32_t old = atomicAdd(&args.tiles_done[c.mat], 1);
-        if (old + 1 == (need + 1) * tiles_m * kEpiWarps) {
-          __threadfence();
-          const int k = c.iter;
-          if (o.resid) {
-            const float r2 = *reinterpret_cast<volatile float *>(
-                &args.resid2[(size_t)(k % NOLSM_MAX_RESID_SLOTS) * args.count + c.mat]);
-            const float res = sqrtf(fmaxf(r2, 0.f) / (float)n);
-            args.lastres[c.mat] = res;
-            args.iters[c.mat] = k + 1;
-            bool stop = pg.fixed_iter > 0 ? (k + 1 >= pg.fixed_iter) : ((res < pg.tol) || !(res == res));
-            if (k + 1 >= pg.max_iter) stop = true;
-            if (stop) *reinterpret_cast<volatile int32_t *>(&args.state[c.mat]) = k;
-          }
-          const int32_t stv = *reinterpret_cast<volatile int32_t *>(&args.state[c.mat]);
-          if (c.op == pg.n_ops - 1 && (stv == k || k + 1 >= limit)) {
-            st_release(&args.ready[c.mat], kDone);
-            __threadfence();
-            atomicSub(&args.group_active[c.mat / pg.group], 1);
-          } else {
-            st_release(&args.ready[c.mat], need + 1);
-          }
-        }
-      }
+      TRACE2(eti, 5);
+      // all epilogue warps have issued their stores and residual atomics: one thread publishes the tile
+      asm volatile("bar.sync 1, %0;" ::"n"(kEpiWarps * 32) : "memory");
+      if (warp - 3 == (tile_seq & (kEpiWarps - 1)) && lane == 0)
+        chainep::epi_complete<NOLSM_TILE_M, 16, 1>(args, c);
+      ++tile_seq;
       if (warp == 3 && lane == 0) { TRACE(3, eti, 1); }
 #ifdef NOLSM_TRACE
       ++eti;
@@ -520,8 +440,10 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
 // Reset of the per-launch control state.
 __global__ void __launch_bounds__(256)
 k_chain_reset(int count, int group, int32_t *ready, int32_t *tiles_done, int32_t *state, int32_t *group_active,
-              float *resid2, int resid_elems, int32_t *iters, float *lastres, int touch_stats) {
+              unsigned long long *tile_counter, float *resid2, int resid_elems, int32_t *iters, float *lastres,
+              int touch_stats) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i == 0) *tile_counter = 0ull;
   const int stride = gridDim.x * blockDim.x;
   for (int m = i; m < count; m += stride) {
     ready[m] = 0;
@@ -540,15 +462,17 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t
                                   CUtensorMapFloatOOBfill);
 
 // stored matrix: dim0 = row index (contiguous), dim1 = column index, dim2 = submatrix
-nolsm_status encode_map(nolsm_ctx *ctx, CUtensorMap *map, void *ptr, bool half, int ld, int count) {
+// operand: FP16 {64,64} box with 128-byte swizzle (TMA loads of the MMA operands); otherwise a plain
+// {32,32} box (FP32 units; FP16 store maps of the epilogue)
+nolsm_status encode_map(nolsm_ctx *ctx, CUtensorMap *map, void *ptr, bool half, bool operand, int ld, int count) {
   const size_t es = half ? sizeof(__half) : sizeof(float);
   cuuint64_t dims[3] = {(cuuint64_t)ld, (cuuint64_t)ld, (cuuint64_t)count};
   cuuint64_t strides[2] = {(cuuint64_t)ld * es, (cuuint64_t)ld * ld * es};
-  cuuint32_t box[3] = {half ? 64u : 32u, half ? 64u : 32u, 1};
+  cuuint32_t box[3] = {operand ? 64u : 32u, operand ? 64u : 32u, 1};
   cuuint32_t estr[3] = {1, 1, 1};
   CUresult r = reinterpret_cast<EncodeTiledFn>(ctx->encode_tiled)(
       map, half ? CU_TENSOR_MAP_DATA_TYPE_FLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, ptr, dims, strides, box,
-      estr, CU_TENSOR_MAP_INTERLEAVE_NONE, half ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE,
+      estr, CU_TENSOR_MAP_INTERLEAVE_NONE, operand ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE,
       CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) {
     ctx->err = "cuTensorMapEncodeTiled failed with CUresult " + std::to_string((int)r);
@@ -564,6 +488,8 @@ extern "C" void nolsm_debug_trace(long long *host_out) {
   cudaDeviceSynchronize();
   cudaMemcpyFromSymbol(host_out, g_trace, sizeof(g_trace));
 }
+extern "C" void nolsm_debug_pwait1(long long *host_out) { cudaMemcpyFromSymbol(host_out, g_wait, sizeof(g_wait)); }
+extern "C" void nolsm_debug_trace2(long long *host_out) { cudaMemcpyFromSymbol(host_out, g_trace2, sizeof(g_trace2)); }
 #endif
 
 nolsm_status umma_init(nolsm_ctx *ctx) {
@@ -597,17 +523,19 @@ nolsm_status umma_init(nolsm_ctx *ctx) {
 nolsm_status umma_make_maps(nolsm_ctx *ctx, nolsm_batch *b) {
   b->maps_valid = false;
   if (!ctx->umma_ok || b->count == 0) return NOLSM_OK;
-  std::vector<CUtensorMap> maps(b->n_half + b->n_unit);
+  std::vector<CUtensorMap> maps(2 * b->n_half + b->n_unit);
   for (int i = 0; i < b->n_half; ++i) {
-    nolsm_status s = encode_map(ctx, &maps[i], b->h[i], true, b->ld, b->count);
+    nolsm_status s = encode_map(ctx, &maps[i], b->h[i], true, true, b->ld, b->count);
+    if (s != NOLSM_OK) return s;
+    s = encode_map(ctx, &maps[b->n_half + b->n_unit + i], b->h[i], true, false, b->ld, b->count);
     if (s != NOLSM_OK) return s;
   }
   for (int i = 0; i < b->n_unit; ++i) {
-    nolsm_status s = encode_map(ctx, &maps[b->n_half + i], b->u[i], false, b->ld, b->count);
+    nolsm_status s = encode_map(ctx, &maps[b->n_half + i], b->u[i], false, false, b->ld, b->count);
     if (s != NOLSM_OK) return s;
   }
   if (!b->d_maps) {
-    if (cudaMalloc(&b->d_maps, sizeof(CUtensorMap) * (NOLSM_MAX_HALF + NOLSM_MAX_UNIT)) != cudaSuccess) {
+    if (cudaMalloc(&b->d_maps, sizeof(CUtensorMap) * (2 * NOLSM_MAX_HALF + NOLSM_MAX_UNIT)) != cudaSuccess) {
       cudaGetLastError();
       ctx->err = "cudaMalloc of the tensor maps failed";
       return NOLSM_ENOMEM;
@@ -637,6 +565,7 @@ cudaError_t launch_chain(nolsm_ctx *ctx, const nolsm_batch *b, const ChainProgra
   a.ntl = (n16max + a.bn - 1) / a.bn;
   a.maps = b->d_maps;
   a.n_half = b->n_half;
+  a.n_unit = b->n_unit;
   for (int i = 0; i < b->n_half; ++i) a.hbuf[i] = b->h[i];
   for (int i = 0; i < b->n_unit; ++i) a.ubuf[i] = b->u[i];
   a.count = b->count;
@@ -649,12 +578,13 @@ cudaError_t launch_chain(nolsm_ctx *ctx, const nolsm_batch *b, const ChainProgra
   a.state = b->d_state;
   a.iters = b->d_iters;
   a.group_active = b->d_group_active;
+  a.tile_counter = b->d_tile_counter;
   a.resid2 = b->d_resid2;
   a.lastres = b->d_lastres;
   if (a.prog.group <= 0) a.prog.group = 1;
   const int slots = std::min(prog.max_iter, NOLSM_MAX_RESID_SLOTS);
   k_chain_reset<<<64, 256, 0, st>>>(b->count, a.prog.group, a.ready, a.tiles_done, a.state, a.group_active,
-                                    a.resid2, slots * b->count, a.iters, a.lastres, touch_stats ? 1 : 0);
+                                    a.tile_counter, a.resid2, slots * b->count, a.iters, a.lastres, touch_stats ? 1 : 0);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
   if (ctx->pair_ok && (ctx->cfg.flags & NOLSM_FLAG_PAIR)) return launch_chain_pair(ctx, b, a.prog, alpha_div, st);

@@ -99,6 +99,7 @@ struct nolsm_batch {
   int32_t *d_ready = nullptr;     // [count] chain engine: ops completed per submatrix
   int32_t *d_tiles_done = nullptr;// [count] chain engine: epilogue-warp arrivals per submatrix
   int32_t *d_group_active = nullptr; // [count] chain engine: unfinished submatrices per group
+  unsigned long long *d_tile_counter = nullptr;   // chain engine: next tile index to claim
   CUtensorMap *d_maps = nullptr;  // device array: n_half FP16 maps {64,64,1}, then n_unit FP32 maps {32,32,1}
   bool maps_valid = false;
 };
