@@ -68,6 +68,7 @@ typedef struct {
 } nolsm_config;
 
 #define NOLSM_FLAG_SIMT_ONLY 1 /* debugging: run every product on the FP32 SIMT kernel */
+#define NOLSM_FLAG_MCAST 4     /* run them on CTA pairs that share the B operand by TMA multicast (cta_group::1) */
 #define NOLSM_FLAG_PAIR 2      /* run the matrix iterations on CTA pairs (tcgen05 cta_group::2, 256-row tiles) */
 
 typedef struct {            /* CSR of uniform bs x bs FP32 blocks; all pointers device, caller-owned */

@@ -15,6 +15,21 @@
 #pragma once
 #include "common.cuh"
 
+// store flavours (experiments: -DNOLSM_ST=1 streaming .cs, 2 write-through .wt, 3 .cg)
+#if NOLSM_ST == 1
+#define ST32(p, v) __stcs((p), (v))
+#define ST16(p, v) __stcs(reinterpret_cast<unsigned short *>(p), __half_as_ushort(v))
+#elif NOLSM_ST == 2
+#define ST32(p, v) __stwt((p), (v))
+#define ST16(p, v) __stwt(reinterpret_cast<unsigned short *>(p), __half_as_ushort(v))
+#elif NOLSM_ST == 3
+#define ST32(p, v) __stcg((p), (v))
+#define ST16(p, v) __stcg(reinterpret_cast<unsigned short *>(p), __half_as_ushort(v))
+#else
+#define ST32(p, v) (*(p) = (v))
+#define ST16(p, v) (*(p) = (v))
+#endif
+
 namespace chainep {
 
 constexpr int32_t kDone = 0x7fffffff;
@@ -216,10 +231,10 @@ __device__ __forceinline__ float epi_chunks(const ChainArgs &args, const TileCmd
     if (t.p32) {   // FP32 result: one 128-byte segment per column and warp
       float *q = t.p32;
 #pragma unroll
-      for (int j = 0; j < 16; ++j) { *q = __uint_as_float(v[j]); q += args.ld; }
+      for (int j = 0; j < 16; ++j) { ST32(q, __uint_as_float(v[j])); q += args.ld; }
       if (cnt == 32) {
 #pragma unroll
-        for (int j = 16; j < 32; ++j) { *q = __uint_as_float(v[j]); q += args.ld; }
+        for (int j = 16; j < 32; ++j) { ST32(q, __uint_as_float(v[j])); q += args.ld; }
       }
       t.p32 += 2 * chunk_stride;
     }
@@ -231,7 +246,7 @@ __device__ __forceinline__ float epi_chunks(const ChainArgs &args, const TileCmd
         if (j == 16 && cnt < 32) break;
         const float val = __uint_as_float(v[j]);
         const __half hi = __float2half_rn(val);
-        *q = hi; q += args.ld;
+        ST16(q, hi); q += args.ld;
         if (ql) { *ql = __float2half_rn((val - __half2float(hi)) * 2048.f); ql += args.ld; }
       }
       t.p16 += 2 * chunk_stride;

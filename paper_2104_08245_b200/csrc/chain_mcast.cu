@@ -1,0 +1,534 @@
+// Cluster-multicast variant of the matrix-iteration engine (scheduling, dependency protocol and
+// epilogues as in chain_umma.cu / chain_epilogue.cuh): the two CTAs of a cluster compute two
+// vertically adjacent 128 x N tiles of the same submatrix, each with its own tcgen05.mma.cta_group::1
+// issuer and accumulator, and SHARE the B operand: each CTA fetches half of the B tile's 64-column
+// boxes and multicasts them into both CTAs' shared memory.  L2 reads per SM and 64-deep K block drop
+// from 48 KB to 32 KB; the engine is bound by L2 throughput (profiles/r1_k_chain_sign_w32768.md).
+//
+// Protocol: the leader's scheduler writes every tile command into both CTAs' rings; every CTA has
+// its own `full` barrier (expects its A tile plus the whole B tile, half of which arrives from the
+// peer); a stage is free when BOTH CTAs' MMAs have consumed it (tcgen05.commit multicast to both
+// `empty` barriers, count 2).  A CTA whose 128 rows lie entirely in the padding ("phantom": odd number
+// of row tiles) still fetches and multicasts its share of B but issues no MMA and stores nothing.
+#include "common.cuh"
+#include "chain_epilogue.cuh"
+
+namespace mcast {
+
+using chainep::TileCmd;
+typedef chainep::ChainArgs PairArgs;
+
+constexpr int kThreads = 352;
+constexpr int kEpiWarps = 8;
+constexpr int kBK = 64;
+constexpr int kMaxStages = 8;
+constexpr int kTmemCols = 512;
+constexpr int kBoxBytes = 64 * 128;
+constexpr int kATileBytes = 2 * kBoxBytes;     // this CTA's 128 rows x 64 K
+constexpr int kRing = 2;
+constexpr int kSmemLimit = 232448 - 2048;
+constexpr int32_t kDone = 0x7fffffff;
+constexpr int kTileM = 256;                    // rows of a pair tile
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) {
+  return static_cast<uint32_t>(__cvta_generic_to_shared(p));
+}
+// shared::cluster address of the same variable in CTA `rank` of the cluster
+__device__ __forceinline__ uint32_t mapa(uint32_t saddr, uint32_t rank) {
+  uint32_t r;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(saddr), "r"(rank));
+  return r;
+}
+__device__ __forceinline__ uint32_t cluster_rank() {
+  uint32_t r;
+  asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+  return r;
+}
+__device__ __forceinline__ void cluster_sync() {
+  asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
+               : "memory");
+}
+// arrive on a barrier given by its shared::cluster address (own or peer CTA), release at cluster scope
+__device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr) {
+  asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+}
+// wait with acquire at cluster scope (the arrivals may come from the peer CTA)
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
+  asm volatile(
+      "{\n\t"
+      ".reg .pred p;\n\t"
+      "MWAIT_LOOP:\n\t"
+      "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%0], %1;\n\t"
+      "@p bra MWAIT_DONE;\n\t"
+      "bra MWAIT_LOOP;\n\t"
+      "MWAIT_DONE:\n\t"
+      "}\n" ::"r"(smem_u32(bar)),
+      "r"(parity)
+      : "memory");
+}
+// TMA load into this CTA's shared memory, signalling this CTA's barrier
+__device__ __forceinline__ void tma_load_3d(void *dst, const CUtensorMap *map, uint64_t *bar, int c0, int c1,
+                                            int c2) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, "
+      "%4, %5}], [%2];" ::"r"(smem_u32(dst)),
+      "l"(reinterpret_cast<uint64_t>(map)), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2)
+      : "memory");
+}
+// TMA load delivered to the same shared-memory offset of BOTH CTAs, signalling the barrier at the same
+// offset in each of them
+__device__ __forceinline__ void tma_load_3d_both(void *dst, const CUtensorMap *map, uint64_t *bar, int c0, int c1,
+                                                 int c2) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.multicast::cluster [%0], "
+      "[%1, {%3, %4, %5}], [%2], %6;" ::"r"(smem_u32(dst)),
+      "l"(reinterpret_cast<uint64_t>(map)), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "h"((uint16_t)3)
+      : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+// arrives on the barrier at the same offset in BOTH CTAs once all prior MMAs of this thread are done
+__device__ __forceinline__ void tc_commit_both(uint64_t *bar) {
+  asm volatile(
+      "tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(
+          smem_u32(bar)),
+      "h"((uint16_t)3)
+      : "memory");
+}
+__device__ __forceinline__ void tc_commit(uint64_t *bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar))
+               : "memory");
+}
+__device__ __forceinline__ void tc_mma2_f16(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc,
+                                            uint32_t accumulate) {
+  asm volatile(
+      "{\n\t"
+      ".reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t"
+      "}\n" ::"r"(tmem_d),
+      "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+__device__ __forceinline__ void tc_ld32(uint32_t taddr, uint32_t (&v)[32]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, %17, %18, %19, %20, %21, "
+      "%22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+      : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+        "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]),
+        "=r"(v[15]), "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]),
+        "=r"(v[22]), "=r"(v[23]), "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]),
+        "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+      : "r"(taddr));
+}
+__device__ __forceinline__ void tc_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ int32_t ld_acquire(const int32_t *p) {
+  int32_t v;
+  asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_release(int32_t *p, int32_t v) {
+  asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+__device__ __forceinline__ uint64_t make_smem_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
+  uint64_t d = 0;
+  d |= (uint64_t)((saddr & 0x3FFFF) >> 4);
+  d |= (uint64_t)((lbo_bytes >> 4) & 0x3FFF) << 16;
+  d |= (uint64_t)((sbo_bytes >> 4) & 0x3FFF) << 32;
+  d |= (uint64_t)1 << 46;   // version
+  d |= (uint64_t)2 << 61;   // SWIZZLE_128B
+  return d;
+}
+
+template <bool H32, bool H16, bool HLO>
+__device__ __forceinline__ void store_cols(const uint32_t (&v)[32], float *p32, __half *p16, __half *p16l, int ld,
+                                           bool full) {
+#pragma unroll
+  for (int half = 0; half < 2; ++half) {
+    if (half == 1 && !full) break;
+#pragma unroll
+    for (int jj = 0; jj < 16; ++jj) {
+      const float val = __uint_as_float(v[half * 16 + jj]);
+      if (H32) { *p32 = val; p32 += ld; }
+      if (H16) {
+        const __half hi = __float2half_rn(val);
+        *p16 = hi; p16 += ld;
+        if (HLO) { *p16l = __float2half_rn((val - __half2float(hi)) * 2048.f); p16l += ld; }
+      }
+    }
+  }
+}
+
+#ifdef NOLSM_TRACE
+__device__ long long g_mtrace[4][4096][2];
+__device__ long long g_mwait[4096][4];
+#define PTRACE(role, ti, j) do { if (blockIdx.x == 0 && (ti) < 4096) g_mtrace[role][ti][j] = clock64(); } while (0)
+#define PTRACEV(role, ti, j, v) do { if (blockIdx.x == 0 && (ti) < 4096) g_mtrace[role][ti][j] = (v); } while (0)
+#else
+#define PTRACE(role, ti, j)
+#define PTRACEV(role, ti, j, v)
+#endif
+
+__global__ void __launch_bounds__(kThreads, 1) k_chain_mcast(const PairArgs args) {
+  extern __shared__ __align__(1024) uint8_t smem_raw[];
+  __shared__ uint64_t full_bar[kMaxStages], empty_bar[kMaxStages], tfull_bar[2], tempty_bar[2];
+  __shared__ uint64_t cmd_full[kRing], cmd_empty[kRing];
+  __shared__ __align__(16) TileCmd cmds[kRing];
+  __shared__ uint32_t tmem_base_s;
+
+  const ChainProgram &pg = args.prog;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint32_t rank = cluster_rank();
+  const bool leader = rank == 0;
+  uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+  // stage layout: [A hi 16K][B hi b_bytes][A lo 16K][B lo b_bytes]
+  const int off_b = kATileBytes, off_a_lo = kATileBytes + args.b_bytes, off_b_lo = 2 * kATileBytes + args.b_bytes;
+
+  if (threadIdx.x == 0) {
+    // a stage is free when BOTH CTAs' MMA issuers have committed it (the peer multicasts into our smem)
+    for (int s = 0; s < args.stages; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], 2); }
+    for (int a = 0; a < 2; ++a) { mbar_init(&tfull_bar[a], 1); mbar_init(&tempty_bar[a], kEpiWarps); }
+    // command ring: filled by the leader's scheduler in both CTAs; freed (leader's barrier) by the
+    // MMA issuer + TMA producer + epilogue warps of both CTAs
+    for (int r = 0; r < kRing; ++r) { mbar_init(&cmd_full[r], 1); mbar_init(&cmd_empty[r], 2 * (2 + kEpiWarps)); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  if (warp == 1) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_base_s)),
+                 "r"(kTmemCols)
+                 : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  tc_fence_before();
+  __syncthreads();
+  cluster_sync();          // barriers of both CTAs initialised before any remote arrive / multicast commit
+  tc_fence_after();
+  const uint32_t tmem_base = tmem_base_s;
+
+  if (warp == 0) {
+    // ===================== scheduler (leader CTA only) =====================
+    if (leader && lane == 0) {
+      int slot = 0;
+      uint32_t ring_phase = 0;
+      const int T = args.mt * args.ntl;
+      const int limit = pg.fixed_iter > 0 ? min(pg.fixed_iter, pg.max_iter) : pg.max_iter;
+      const int n_groups = (args.count + pg.group - 1) / pg.group;
+      const int n_clusters = gridDim.x >> 1, cluster_id = blockIdx.x >> 1;
+      auto push = [&](const TileCmd &cmd) {
+        mbar_wait(&cmd_empty[slot], ring_phase ^ 1u);
+        cmds[slot] = cmd;
+        const uint32_t remote = mapa(smem_u32(&cmds[slot]), 1);
+        asm volatile("st.shared::cluster.v4.s32 [%0], {%1, %2, %3, %4};" ::"r"(remote), "r"(cmd.mat), "r"(cmd.m0),
+                     "r"(cmd.n0), "r"(cmd.nt)
+                     : "memory");
+        asm volatile("st.shared::cluster.v4.s32 [%0], {%1, %2, %3, %4};" ::"r"(remote + 16), "r"(cmd.kblocks),
+                     "r"(cmd.ktail), "r"(cmd.op), "r"(cmd.iter)
+                     : "memory");
+        mbar_arrive_cluster(mapa(smem_u32(&cmd_full[slot]), 0));
+        mbar_arrive_cluster(mapa(smem_u32(&cmd_full[slot]), 1));
+        if (++slot == kRing) { slot = 0; ring_phase ^= 1u; }
+      };
+      // Dynamic, in-order tile claims: a tile only depends on tiles with a smaller index, all of which
+      // have been claimed by running CTAs, so the schedule cannot deadlock and balances itself.
+      const int64_t per_group = (int64_t)limit * pg.n_ops * pg.group * T;   // index space of one (full) group
+      int g_checked = -1, k_checked = 0;
+      for (;;) {
+        const int64_t L = (int64_t)atomicAdd(args.tile_counter, 1ull);
+        const int g = (int)(L / per_group);
+        if (g >= n_groups) break;
+        const int64_t Lg = L - (int64_t)g * per_group;
+        const int gbase = g * pg.group;
+        const int gs = min(pg.group, args.count - gbase);
+        const int per_seg = gs * T;
+        if (Lg >= (int64_t)limit * pg.n_ops * per_seg) continue;   // index padding of the last group
+        const int seg = (int)(Lg / per_seg), rem = (int)(Lg % per_seg);
+        const int k = seg / pg.n_ops, op = seg % pg.n_ops;
+        if (g != g_checked) { g_checked = g; k_checked = 0; }
+        if (k != k_checked) {   // whole group converged: move the claim counter past it
+          if (ld_acquire(&args.group_active[g]) == 0) {
+            atomicMax(args.tile_counter, (unsigned long long)((int64_t)(g + 1) * per_group));
+            continue;
+          }
+          k_checked = k;
+        }
+        const int ml = rem / T, t = rem % T;
+        const int m = gbase + ml;
+        const int n = args.dims[m];
+        const int n16 = (n + 15) & ~15;
+        const int m0 = (t % args.mt) * kTileM, n0 = (t / args.mt) * args.bn;
+        if (m0 >= n || n0 >= n16) continue;          // tile outside this submatrix
+        const int need = k * pg.n_ops + op;          // ops of this submatrix that must be complete
+        if (need > 0) {
+          int32_t r = ld_acquire(&args.ready[m]);
+          while (r < need) { __nanosleep(64); r = ld_acquire(&args.ready[m]); }
+          if (r == kDone) continue;                  // submatrix finished at an earlier iteration
+        }
+        const int kblocks = (n16 + kBK - 1) / kBK;
+        {
+          push(TileCmd{m, m0, n0, min(args.bn, n16 - n0), kblocks, (n16 - (kblocks - 1) * kBK) / 16, op, k});
+        }
+      }
+      push(TileCmd{0, 0, 0, 0, 0, 0, -1, 0});
+    }
+  } else if (warp == 2) {
+    // ===================== TMA producer (both CTAs) =====================
+    if (lane == 0) {
+#ifdef NOLSM_TRACE
+      int tti = 0;
+#endif
+      int stage = 0, slot = 0;
+      uint32_t phase = 0, ring_phase = 0;
+      for (;;) {
+        mbar_wait(&cmd_full[slot], ring_phase);
+        const TileCmd c = cmds[slot];
+        mbar_arrive_cluster(mapa(smem_u32(&cmd_empty[slot]), 0));
+        if (++slot == kRing) { slot = 0; ring_phase ^= 1u; }
+        if (c.op < 0) break;
+        PTRACE(2, tti, 0);
+        fence_proxy_async();   // other CTAs' generic-proxy writes (ordered by the scheduler's acquire) -> TMA reads
+        const ChainOp &o = pg.ops[c.op];
+        const int par = c.iter & 1;
+        const int m = c.mat;
+        const int m0 = c.m0 + 128 * (int)rank;               // this CTA's tile of the vertical pair
+        const int n0 = c.n0;
+        const bool phantom = m0 >= args.dims[m];              // rows entirely in the padding: only serve B
+        const bool split = o.a_lo[par] >= 0;
+        const int nbox = (c.nt + 63) >> 6;                    // 64-column boxes of the shared B tile
+        const uint32_t bytes = (uint32_t)((phantom ? 0 : kATileBytes) + nbox * kBoxBytes) * (split ? 2u : 1u);
+        const CUtensorMap *ma = &args.maps[o.a[par]], *mb = &args.maps[o.b[par]];
+        const CUtensorMap *mal = split ? &args.maps[o.a_lo[par]] : nullptr;
+        const CUtensorMap *mbl = split ? &args.maps[o.b_lo[par]] : nullptr;
+        for (int kb = 0; kb < c.kblocks; ++kb) {
+          mbar_wait(&empty_bar[stage], phase ^ 1u);            // both CTAs have consumed this stage
+          uint8_t *st = smem + (size_t)stage * args.stage_bytes;
+          mbar_expect_tx(&full_bar[stage], bytes);
+          const int k0 = kb * kBK;
+          if (!phantom) {
+            tma_load_3d(st, ma, &full_bar[stage], m0, k0, m);
+            tma_load_3d(st + kBoxBytes, ma, &full_bar[stage], m0 + 64, k0, m);
+          }
+          for (int j = (int)rank; j < nbox; j += 2)             // our share of B, delivered to both CTAs
+            tma_load_3d_both(st + off_b + j * kBoxBytes, mb, &full_bar[stage], k0, n0 + 64 * j, m);
+          if (split) {
+            if (!phantom) {
+              tma_load_3d(st + off_a_lo, mal, &full_bar[stage], m0, k0, m);
+              tma_load_3d(st + off_a_lo + kBoxBytes, mal, &full_bar[stage], m0 + 64, k0, m);
+            }
+            for (int j = (int)rank; j < nbox; j += 2)
+              tma_load_3d_both(st + off_b_lo + j * kBoxBytes, mbl, &full_bar[stage], k0, n0 + 64 * j, m);
+          }
+          if (++stage == args.stages) { stage = 0; phase ^= 1u; }
+        }
+        PTRACE(2, tti, 1);
+#ifdef NOLSM_TRACE
+        ++tti;
+#endif
+      }
+    }
+  } else if (warp == 1) {
+    // ===================== MMA issuer (each CTA for its own tile) =====================
+    if (lane == 0) {
+#ifdef NOLSM_TRACE
+      int mti = 0;
+#endif
+      int stage = 0, slot = 0, acc = 0;
+      uint32_t phase = 0, ring_phase = 0, acc_phase = 0;
+      for (;;) {
+        mbar_wait(&cmd_full[slot], ring_phase);
+        const TileCmd c = cmds[slot];
+        mbar_arrive_cluster(mapa(smem_u32(&cmd_empty[slot]), 0));
+        if (++slot == kRing) { slot = 0; ring_phase ^= 1u; }
+        if (c.op < 0) break;
+        const bool split = pg.ops[c.op].a_lo[c.iter & 1] >= 0;
+        const bool phantom = c.m0 + 128 * (int)rank >= args.dims[c.mat];
+        // instruction descriptor: D=F32, A=B=F16, A M-major, B K-major, N = nt, M = 128
+        const uint32_t idesc = (1u << 4) | (1u << 15) | ((uint32_t)(c.nt >> 3) << 17) | ((128u >> 4) << 24);
+        PTRACE(0, mti, 0);
+        mbar_wait(&tempty_bar[acc], acc_phase ^ 1u);
+        tc_fence_after();
+        PTRACE(0, mti, 1);
+#ifdef NOLSM_TRACE
+        ++mti;
+#endif
+        const uint32_t d_main = tmem_base + (uint32_t)(acc * 256);
+        const uint32_t d_corr = d_main + 128;
+#ifdef NOLSM_TRACE
+        long long wsum = 0, t_first = 0, t_begin = clock64();
+#endif
+        for (int kb = 0; kb < c.kblocks; ++kb) {
+#ifdef NOLSM_TRACE
+          long long w0 = clock64();
+#endif
+          mbar_wait(&full_bar[stage], phase);
+#ifdef NOLSM_TRACE
+          wsum += clock64() - w0;
+          if (kb == 0) t_first = clock64() - w0;
+#endif
+          tc_fence_after();
+          const uint32_t sa = smem_u32(smem + (size_t)stage * args.stage_bytes);
+          const int steps = phantom ? 0 : (kb == c.kblocks - 1 ? c.ktail : kBK / 16);
+          for (int k4 = 0; k4 < steps; ++k4) {
+            const uint64_t ad = make_smem_desc(sa + k4 * 2048, kBoxBytes, 1024);
+            const uint64_t bd = make_smem_desc(sa + off_b + k4 * 32, 16, 1024);
+            const uint32_t accum = (kb | k4) ? 1u : 0u;
+            tc_mma2_f16(d_main, ad, bd, idesc, accum);
+            if (split) {
+              const uint64_t adl = make_smem_desc(sa + off_a_lo + k4 * 2048, kBoxBytes, 1024);
+              const uint64_t bdl = make_smem_desc(sa + off_b_lo + k4 * 32, 16, 1024);
+              tc_mma2_f16(d_corr, ad, bdl, idesc, accum);
+              tc_mma2_f16(d_corr, adl, bd, idesc, 1u);
+            }
+          }
+          tc_commit_both(&empty_bar[stage]);
+          if (++stage == args.stages) { stage = 0; phase ^= 1u; }
+        }
+        tc_commit(&tfull_bar[acc]);
+#ifdef NOLSM_TRACE
+        if (blockIdx.x == 0 && mti - 1 < 4096) { g_mwait[mti - 1][0] = wsum; g_mwait[mti - 1][1] = t_first; g_mwait[mti - 1][2] = clock64() - t_begin; }
+#endif
+        if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
+      }
+    }
+  } else {
+    // ===================== epilogue (both CTAs: each drains its own 128 TMEM lanes) =====================
+    const int q = warp & 3;
+    const int chunk_first = (warp - 3) >> 2;
+#ifdef NOLSM_TRACE
+    int eti = 0;
+#endif
+    int slot = 0, acc = 0, tile_seq = 0;
+    uint32_t ring_phase = 0, acc_phase = 0;
+    for (;;) {
+      mbar_wait(&cmd_full[slot], ring_phase);
+      const TileCmd c = cmds[slot];
+      __syncwarp();
+      if (lane == 0) mbar_arrive_cluster(mapa(smem_u32(&cmd_empty[slot]), 0));
+      if (++slot == kRing) { slot = 0; ring_phase ^= 1u; }
+      if (c.op < 0) break;
+      // phantom tile (rows entirely in the padding): nothing to load or store
+      const bool rows_in = c.m0 + 128 * (int)rank < args.dims[c.mat];
+      chainep::EpiTile t;
+      chainep::epi_begin(args, c, c.m0 + 128 * (int)rank + q * 32, rows_in, lane, chunk_first, t);
+      if (warp == 3 && lane == 0) { PTRACE(1, eti, 0); }
+      mbar_wait(&tfull_bar[acc], acc_phase);
+      tc_fence_after();
+      if (warp == 3 && lane == 0) { PTRACE(1, eti, 1); PTRACEV(3, eti, 0, ((long long)c.mat << 40) | ((long long)c.iter << 32) | ((long long)c.op << 24) | ((long long)(c.m0 / 256) << 8) | (long long)(c.n0 / 64)); }
+      const uint32_t t_main = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(acc * 256);
+      float ss = chainep::epi_chunks(args, c, t, t_main, lane);
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive_cluster(mapa(smem_u32(&tempty_bar[acc]), rank));
+      if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
+      if (t.o->resid) {
+        for (int d = 16; d > 0; d >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, d);
+        if (lane == 0) atomicAdd(&args.resid2[(size_t)(c.iter % NOLSM_MAX_RESID_SLOTS) * args.count + c.mat], ss);
+      }
+      // all epilogue warps of this CTA have issued their stores: one thread publishes the CTA's half
+      asm volatile("bar.sync 1, %0;" ::"n"(kEpiWarps * 32) : "memory");
+      if (warp - 3 == (tile_seq & (kEpiWarps - 1)) && lane == 0) chainep::epi_complete<kTileM, 16, 2>(args, c);
+      ++tile_seq;
+      if (warp == 3 && lane == 0) { PTRACE(3, eti, 1); }
+#ifdef NOLSM_TRACE
+      ++eti;
+#endif
+    }
+  }
+
+  tc_fence_before();
+  __syncthreads();
+  cluster_sync();            // nobody leaves while the peer may still signal our barriers or read our smem
+  if (warp == 1) {
+    tc_fence_after();
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(kTmemCols) : "memory");
+  }
+}
+
+}  // namespace mcast
+
+#ifdef NOLSM_TRACE
+extern "C" void nolsm_debug_mtrace(long long *host_out) {
+  cudaDeviceSynchronize();
+  cudaMemcpyFromSymbol(host_out, mcast::g_mtrace, sizeof(mcast::g_mtrace));
+}
+extern "C" void nolsm_debug_mwait(long long *host_out) { cudaMemcpyFromSymbol(host_out, mcast::g_mwait, sizeof(mcast::g_mwait)); }
+#endif
+
+nolsm_status mcast_init(nolsm_ctx *ctx) {
+  ctx->mcast_ok = false;
+  cudaError_t e = cudaFuncSetAttribute(mcast::k_chain_mcast, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                       mcast::kSmemLimit);
+  if (e != cudaSuccess) { cudaGetLastError(); return NOLSM_ECUDA; }
+  // all pairs must be co-resident: the CTAs wait on one another through global flags
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)(ctx->sm_count & ~1));
+  cfg.blockDim = dim3(mcast::kThreads);
+  cfg.dynamicSmemBytes = mcast::kSmemLimit;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeClusterDimension;
+  at[0].val.clusterDim.x = 2; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = 1;
+  int max_clusters = 0;
+  e = cudaOccupancyMaxActiveClusters(&max_clusters, mcast::k_chain_mcast, &cfg);
+  if (e != cudaSuccess || max_clusters < 1) { cudaGetLastError(); return NOLSM_ECUDA; }
+  ctx->mcast_clusters = std::min(max_clusters, ctx->sm_count / 2);
+  ctx->mcast_ok = true;
+  return NOLSM_OK;
+}
+
+// Same contract as the single-CTA launch in chain_umma.cu; the control state has been reset by the caller.
+cudaError_t launch_chain_mcast(nolsm_ctx *ctx, const nolsm_batch *b, const ChainProgram &prog, const float *alpha_div,
+                              cudaStream_t st) {
+  using namespace mcast;
+  PairArgs a;
+  memset(&a, 0, sizeof(a));
+  a.prog = prog;
+  bool split = false;
+  for (int i = 0; i < prog.n_ops; ++i) split |= prog.ops[i].a_lo[0] >= 0 || prog.ops[i].a_lo[1] >= 0;
+  const int n16max = (b->max_n + 15) & ~15;
+  a.bn = std::min(split ? 128 : 256, n16max);
+  a.b_bytes = ((a.bn + 63) / 64) * kBoxBytes;
+  a.stage_bytes = (kATileBytes + a.b_bytes) * (split ? 2 : 1);
+  a.stages = std::min(kMaxStages, (kSmemLimit - 1024) / a.stage_bytes);
+  a.mt = (b->max_n + kTileM - 1) / kTileM;
+  a.ntl = (n16max + a.bn - 1) / a.bn;
+  a.maps = b->d_maps;
+  a.n_half = b->n_half;
+  a.n_unit = b->n_unit;
+  for (int i = 0; i < b->n_half; ++i) a.hbuf[i] = b->h[i];
+  for (int i = 0; i < b->n_unit; ++i) a.ubuf[i] = b->u[i];
+  a.count = b->count;
+  a.ld = b->ld;
+  a.slab = (int64_t)b->ld * b->ld;
+  a.dims = b->d_dims;
+  a.alpha_div = alpha_div;
+  a.ready = b->d_ready;
+  a.tiles_done = b->d_tiles_done;
+  a.state = b->d_state;
+  a.iters = b->d_iters;
+  a.group_active = b->d_group_active;
+  a.tile_counter = b->d_tile_counter;
+  a.resid2 = b->d_resid2;
+  a.lastres = b->d_lastres;
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)(2 * ctx->mcast_clusters));
+  cfg.blockDim = dim3(kThreads);
+  cfg.dynamicSmemBytes = (size_t)(a.stages * a.stage_bytes + 1024);
+  cfg.stream = st;
+  cudaLaunchAttribute at[2];
+  at[0].id = cudaLaunchAttributeClusterDimension;
+  at[0].val.clusterDim.x = 2; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+  at[1].id = cudaLaunchAttributeCooperative;
+  at[1].val.cooperative = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = 2;
+  return cudaLaunchKernelEx(&cfg, k_chain_mcast, a);
+}

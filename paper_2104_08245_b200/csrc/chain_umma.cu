@@ -517,6 +517,7 @@ nolsm_status umma_init(nolsm_ctx *ctx) {
   }
   ctx->umma_ok = true;
   pair_init(ctx);   // optional: the single-CTA engine is the fallback
+  mcast_init(ctx);
   return NOLSM_OK;
 }
 
@@ -588,6 +589,7 @@ cudaError_t launch_chain(nolsm_ctx *ctx, const nolsm_batch *b, const ChainProgra
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
   if (ctx->pair_ok && (ctx->cfg.flags & NOLSM_FLAG_PAIR)) return launch_chain_pair(ctx, b, a.prog, alpha_div, st);
+  if (ctx->mcast_ok && (ctx->cfg.flags & NOLSM_FLAG_MCAST)) return launch_chain_mcast(ctx, b, a.prog, alpha_div, st);
   const int smem_bytes = a.stages * a.stage_bytes + 1024;
   void *params[] = {&a};
   return cudaLaunchCooperativeKernel(reinterpret_cast<void *>(k_chain), dim3(ctx->sm_count), dim3(kThreads), params,

@@ -121,6 +121,8 @@ struct nolsm_ctx {
   bool umma_ok = false;
   bool pair_ok = false;           // pair-CTA (cta_group::2) engine usable
   int pair_clusters = 0;          // co-resident CTA pairs
+  bool mcast_ok = false;          // cluster-multicast engine usable
+  int mcast_clusters = 0;
   // device mirrors of the caller's HOST store (nolsm_solve_mu_host), grown on demand
   int32_t *m_row_ptr = nullptr, *m_col_idx = nullptr;
   float *m_h = nullptr, *m_s = nullptr, *m_d = nullptr;
@@ -178,5 +180,8 @@ nolsm_status umma_make_maps(nolsm_ctx *ctx, nolsm_batch *b);
 nolsm_status pair_init(nolsm_ctx *ctx);
 cudaError_t launch_chain_pair(nolsm_ctx *ctx, const nolsm_batch *b, const ChainProgram &prog, const float *alpha_div,
                               cudaStream_t st);
+nolsm_status mcast_init(nolsm_ctx *ctx);
+cudaError_t launch_chain_mcast(nolsm_ctx *ctx, const nolsm_batch *b, const ChainProgram &prog, const float *alpha_div,
+                               cudaStream_t st);
 cudaError_t launch_chain(nolsm_ctx *ctx, const nolsm_batch *b, const ChainProgram &prog, const float *alpha_div,
                          bool touch_stats, cudaStream_t st);

@@ -368,3 +368,58 @@ def test_baseline_configs_sampled(nolsm, name, precision, begin, count, sample):
     assert np.abs(qs - 8.0).max() < 0.03
     assert abs(ne.item() - qs.sum()) < 1e-6 * count
     ctx.close()
+
+
+# ---------------------------------------------------------------------------------------------
+# the optional pair engines (cta_group::2 pair tiles / cluster multicast of the B operand)
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("flag", ["FLAG_PAIR", "FLAG_MCAST"])
+@pytest.mark.parametrize("precision", [0, 1])
+def test_pair_engines_density_tiny_and_mid(nolsm, tiny_system, tiny_solution, mid_system, mid_solution, flag, precision):
+    """Same parity bounds as the default engine, through nolsm_solve_mu (tiny) and a partial batch (mid:
+    n ~ 478 = 4 row tiles, so the 256-row pair tiles have a ragged second half)."""
+    import torch
+    import oracle.nolsm_oracle as orc
+    flags = getattr(nolsm, flag)
+    sols = tiny_solution["solutions"]
+    H, S = _device_system(nolsm, tiny_system)
+    ctx = nolsm.Context(nolsm.Config(precision=precision, flags=flags))
+    mu, ne, D, stats = ctx.solve_mu(H, S, tiny_system.n_electrons, -3.0, 0.0, tol_ne_per_mol=1e-3, max_steps=30)
+    d_ref = orc.density_blocks(sols, tiny_system.row_ptr, mu)
+    assert np.abs(D.val.cpu().numpy() - d_ref).max() < TOL_D[precision]
+    assert abs(ne - orc.electron_count(sols, mu)) / tiny_system.n_mol <= TOL_NE_PER_MOL
+    ctx.close()
+    # mid system, molecules 50..109
+    sols = mid_solution["solutions"]
+    d_ref = orc.density_blocks(sols, mid_system.row_ptr, MU)
+    H, S = _device_system(nolsm, mid_system)
+    D = S.like()
+    ctx = nolsm.Context(nolsm.Config(precision=precision, flags=flags))
+    batch = ctx.build_submatrices(H, S, 50, 60)
+    st = ctx.sign_batched(batch, MU)
+    assert st.n_unconverged == 0
+    ne_t = torch.zeros(1, dtype=torch.float64, device="cuda")
+    ctx.scatter_density(batch, S, D, ne_t, None, None)
+    lo, hi = mid_system.row_ptr[50], mid_system.row_ptr[110]
+    assert np.abs(D.val.cpu().numpy()[lo:hi] - d_ref[lo:hi]).max() < TOL_D[precision]
+    ctx.close()
+
+
+@pytest.mark.parametrize("flag", ["FLAG_PAIR", "FLAG_MCAST"])
+@pytest.mark.parametrize("kind,tol", [(1, 2e-2), (2, 2e-5)])
+@pytest.mark.parametrize("n,batch", [(64, 3), (146, 5), (300, 2), (863, 2)])
+def test_pair_engines_building_block(nolsm, torch_mod, flag, kind, tol, n, batch):
+    rng = np.random.default_rng(n * 7 + kind)
+    a = rng.uniform(-1, 1, (batch, n, n)).astype(np.float32)
+    b = rng.uniform(-1, 1, (batch, n, n)).astype(np.float32)
+    cin = rng.uniform(-1, 1, (batch, n, n)).astype(np.float32)
+    ref = a.astype(np.float64) @ b.astype(np.float64)
+    ctx = nolsm.Context(nolsm.Config(flags=getattr(nolsm, flag)))
+    ta, tb, tc = (torch_mod.as_tensor(x).cuda() for x in (a, b, cin))
+    c, _ = ctx.gemm_batched(kind, ta, tb, cin=tc, alpha=0.5, beta=1.0)
+    assert np.abs(c.cpu().numpy() - (0.5 * ref + cin)).max() / np.sqrt(n) < tol
+    c, r2 = ctx.gemm_batched(kind, ta, tb, ident=True)
+    want = np.eye(n)[None] - ref
+    assert np.abs(c.cpu().numpy() - want).max() / np.sqrt(n) < tol
+    assert np.allclose(r2.cpu().numpy(), (want ** 2).sum(axis=(1, 2)), rtol=5e-3 if kind == 1 else 1e-4)
+    ctx.close()
