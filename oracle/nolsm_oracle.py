@@ -12,6 +12,8 @@ What it computes (PAPER.md = /root/reference/PAPER.md):
     sign(A) and S^-1, so the oracle solves H v = lambda S v (LAPACK) and forms sign and D from the
     eigenvectors;
   * the chemical potential mu such that 2 tr(DS) = N_electrons by bisection.
+  * the electronic energy E = Tr(D H0) over the stored blocks (Eq. 7, 11) and the
+    energy-weighted density T_j(W) = T_j(D) T_j(H0) T_j(D) (Eq. 8, 13).
 The literal iterations (Eq. 9-10, Eq. 15-17) are also written out step by step
 (`newton_schulz_sign`, `newton_schulz_inverse`) for fixed-iteration comparisons and residual traces.
 
@@ -195,6 +197,15 @@ class SubmatrixSolution:
     def homo_lumo(self, n_occ):
         return float(self.lam[n_occ - 1]), float(self.lam[n_occ])
 
+    def energy_weighted(self, mu):
+        """T_j(W) = T_j(D) T_j(H0) T_j(D)  (Eq. 13), by its plain definition."""
+        d = self.density(mu)
+        return d @ self.h_sub @ d
+
+    def energy_weighted_columns(self, mu):
+        """Own columns of T_j(W): [n_j, 6], same block layout as density_columns."""
+        return self.energy_weighted(mu)[:, self.own]
+
 
 def solve_molecule(row_ptr, col_idx, h_val, s_val, j, nbrs=None):
     if nbrs is None:
@@ -222,6 +233,26 @@ def electron_count_blocks(row_ptr, col_idx, d_val, s_val):
             if p < hi and col_idx[p] == j:
                 total += float((d_val[k].astype(np.float64) * s_val[p].astype(np.float64)).sum())
     return 2.0 * total
+
+
+def electronic_energy_blocks(row_ptr, col_idx, d_val, h_val):
+    """E_elec = Tr(D H0) = sum_{i,j} D_ij H0_ji  (Eq. 7 and 11) over the stored
+    blocks: D is column-owned (block k of row j = D(col_idx[k], j)) and H0(j, col_idx[k]) is block k of
+    row j of the H store, so the pair shares one index k:  E = sum_k sum_{o,p} D_k[o,p] H_k[p,o]."""
+    d = np.asarray(d_val, dtype=np.float64)
+    h = np.asarray(h_val, dtype=np.float64)
+    return float(np.einsum("kop,kpo->", d, h))
+
+
+def energy_weighted_blocks(solutions, row_ptr, mu, dtype=np.float64):
+    """Column-owned W store, same layout as density_blocks."""
+    nnzb = int(row_ptr[-1])
+    out = np.zeros((nnzb, BS, BS), dtype=dtype)
+    for s in solutions:
+        cols = s.energy_weighted_columns(mu)
+        lo = int(row_ptr[s.j])
+        out[lo:lo + s.nbrs.shape[0]] = cols.reshape(-1, BS, BS)
+    return out
 
 
 def bisect_mu(solutions, n_electrons, mu_lo, mu_hi, tol_per_mol=1e-3, max_steps=60):

@@ -467,20 +467,23 @@ static nolsm_status prepare_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, int prec
       stats->inv_iter_max = std::max(stats->inv_iter_max, it[m]);
       if (!(res[m] <= stats->inv_worst_residual)) stats->inv_worst_residual = res[m];
       const double n = b->n_host[m];
-      const int products = 3 * it[m] + 2 + 2 * refine;
+      const int products = 3 * it[m] + 2 + 2 * refine;   // products, whatever the MMAs per product
       inv_gemm_sum += products;
       fl += 2.0 * n * n * n * products;
     }
     stats->flops_prepare = fl;
   }
   const int g1 = group_size(ctx, b, 16);
-  // S^-1 = Z^2 / s_S from the FP32 master: split Z -> (h0,h1); result -> u2 and split (h2,h3)
-  LAUNCH(ctx, launch_scale_copy(b, b->u[3], nullptr, 0, nullptr, b->h[0], b->h[1], st));
+  // S^-1 = Z^2 / s_S (Eq. 17) from the FP32 master; result -> u2 and split (h2,h3).  When a Newton
+  // refinement follows (it squares the error) plain FP16 operands are enough here; otherwise split Z.
+  const bool z_split = refine == 0;
+  LAUNCH(ctx, launch_scale_copy(b, b->u[3], nullptr, 0, nullptr, b->h[0], z_split ? b->h[1] : nullptr, st));
   {
     ChainProgram p1 = one_shot(g1);
     p1.n_ops = 1;
     ChainOp &o = p1.ops[0] = make_op(EPI_AXPBY, 1.f, 0.f);
-    set2(o.a, 0, 0); set2(o.a_lo, 1, 1); set2(o.b, 0, 0); set2(o.b_lo, 1, 1);
+    set2(o.a, 0, 0); set2(o.b, 0, 0);
+    if (z_split) { set2(o.a_lo, 1, 1); set2(o.b_lo, 1, 1); }
     o.use_div = 1; o.cout32 = 2; set2(o.out16, 2, 2); set2(o.out16_lo, 3, 3);
     CHECK(run_chain(ctx, b, p1, b->d_scale, false, st));
   }

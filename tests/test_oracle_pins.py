@@ -300,3 +300,31 @@ def test_microbench_matrix_properties():
     assert 0.05 <= np.abs(lam).min() and np.abs(lam).max() <= 1.0 and (lam > 0).any() and (lam < 0).any()
     assert np.abs(np.linalg.eigvalsh(a.astype(np.float64)) - np.sort(lam)).max() < 1e-6
     assert gi.microbench_batch(256) == 512 and gi.microbench_batch(1024) == 8 and gi.microbench_batch(4096) == 1
+
+
+def test_energy_weighted_density_and_energy_pins(tiny_system, tiny_solution):
+    """Eq. 7, 8, 11, 13.  Pins: (i) with V^T S V = I and H V = S V Lambda, D H D collapses to
+    V_occ Lambda_occ V_occ^T, a different formula from the triple product the oracle evaluates;
+    (ii) tr(W_j S_j) = tr(D_j H_j) = sum of the occupied eigenvalues of the submatrix; (iii) at full
+    cutoff every submatrix is the whole system, so the block sum of Eq. 11 equals the sum of the
+    occupied eigenvalues of the full generalized problem (textbook band energy)."""
+    mu = tiny_solution["mu"]
+    for s in tiny_solution["solutions"][:6]:
+        occ = s.lam < mu
+        w = s.energy_weighted(mu)
+        closed = (s.v[:, occ] * s.lam[occ]) @ s.v[:, occ].T
+        assert np.abs(w - closed).max() < 1e-12
+        assert abs(np.trace(w @ s.s_sub) - s.lam[occ].sum()) < 1e-11
+        assert abs(np.trace(s.density(mu) @ s.h_sub) - s.lam[occ].sum()) < 1e-11
+        assert np.abs(w - w.T).max() < 1e-12
+        assert np.array_equal(s.energy_weighted_columns(mu), w[:, s.own])
+    # full cutoff: block contraction of Eq. 11 against the full-matrix eigenvalues
+    full = gi.make_water_system(32, 9.0)
+    sol = orc.solve_system(full, mu=-0.85)
+    d = orc.density_blocks(sol["solutions"], full.row_ptr, -0.85)
+    e_blocks = orc.electronic_energy_blocks(full.row_ptr, full.col_idx, d, full.h_val)
+    lam = sla.eigh(to_dense(full, "H"), to_dense(full, "S"), eigvals_only=True)
+    assert abs(e_blocks - lam[lam < -0.85].sum()) < 1e-9
+    # and the own columns of W in the store layout give tr(W S) = E when contracted like tr(D S)
+    w_blocks = orc.energy_weighted_blocks(sol["solutions"], full.row_ptr, -0.85)
+    assert abs(0.5 * orc.electron_count_blocks(full.row_ptr, full.col_idx, w_blocks, full.s_val) - e_blocks) < 1e-9
