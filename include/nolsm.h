@@ -167,6 +167,22 @@ nolsm_status nolsm_solve_mu(nolsm_ctx *ctx, const nolsm_bsr *H, const nolsm_bsr 
                             double *ne_out /*host*/, double *q_mol, nolsm_solve_stats *stats /*host*/,
                             void *stream);
 
+/* Energy and energy-weighted density (Eq. 7, 8, 11, 13) of a batch whose sign
+ * iterate is current (after nolsm_sign_batched) and whose D columns have been written (nolsm_scatter_density):
+ *   W != NULL:        W(:, own_j) = [T_j(D) T_j(H0) T_j(D)](:, own_j) into rows [mol_begin, ...) of the column-owned
+ *                     store W (pattern of H; four n x n x 6 products per submatrix, FP32);
+ *   e_partial != NULL: sum_j sum_{i in N_j} sum_{o,p} D(i,j)[o,p] H0(j,i)[p,o] ADDED to *e_partial (device double;
+ *                     D = the density store; FP32 products, FP64 accumulation).  Asynchronous. */
+nolsm_status nolsm_scatter_energy(nolsm_ctx *ctx, nolsm_batch *batch, const nolsm_bsr *H, const nolsm_bsr *D,
+                                  nolsm_bsr *W, double *e_partial, void *stream);
+
+/* One evaluation of the whole path (a1-a7) at a GIVEN mu, plus E_elec = Tr(D H0) (Eq. 7, 11) and, if W != NULL,
+ * the energy-weighted density (Eq. 8, 13).  ne_out, e_out: host doubles (N(mu) = 2 tr(DS); E counts every
+ * occupied orbital once, as Eq. 7 does).  q_mol: device double [n_mol] or NULL.  Synchronises. */
+nolsm_status nolsm_evaluate(nolsm_ctx *ctx, const nolsm_bsr *H, const nolsm_bsr *S, double mu, int32_t precision,
+                            nolsm_bsr *D, nolsm_bsr *W, double *ne_out /*host*/, double *e_out /*host*/,
+                            double *q_mol, nolsm_solve_stats *stats /*host*/, void *stream);
+
 /* The same whole path with HOST buffers (the end-to-end call: Fig. 2 d-h of the paper include the
  * transfers).  row_ptr [n_mol+1], col_idx [nnzb], h_val, s_val, d_val [nnzb*36]
  * are HOST pointers (pinned memory makes the copies asynchronous; pageable works).  The context

@@ -18,6 +18,7 @@ EXPORTED_SYMBOLS = [
     "nolsm_build_submatrices", "nolsm_batch_capacity", "nolsm_release_batch", "nolsm_sign_batched",
     "nolsm_scatter_density", "nolsm_solve_mu", "nolsm_solve_mu_host", "nolsm_sign_dense_batched", "nolsm_batch_read",
     "nolsm_batch_size", "nolsm_batch_ld", "nolsm_gemm_batched", "nolsm_launch_count",
+    "nolsm_scatter_energy", "nolsm_evaluate",
 ]
 
 
@@ -104,6 +105,11 @@ def load_library():
     lib.nolsm_release_batch.restype = None
     lib.nolsm_sign_batched.argtypes = [vp, vp, f64, i32, f32, i32, i32, P(SignStats), vp]
     lib.nolsm_sign_batched.restype = i32
+    lib.nolsm_scatter_energy.argtypes = [vp, vp, P(_Bsr), P(_Bsr), P(_Bsr), vp, vp]
+    lib.nolsm_scatter_energy.restype = i32
+    lib.nolsm_evaluate.argtypes = [vp, P(_Bsr), P(_Bsr), f64, i32, P(_Bsr), P(_Bsr), P(f64), P(f64), vp,
+                                   P(SolveStats), vp]
+    lib.nolsm_evaluate.restype = i32
     lib.nolsm_scatter_density.argtypes = [vp, vp, P(_Bsr), P(_Bsr), vp, vp, vp, vp]
     lib.nolsm_scatter_density.restype = i32
     lib.nolsm_solve_mu.argtypes = [vp, P(_Bsr), P(_Bsr), f64, f64, f64, f64, i32, i32, P(_Bsr), P(f64), P(f64),
@@ -284,7 +290,29 @@ class Context:
                                                    _ptr(ne_partial, torch.float64), _ptr(q_mol, torch.float64),
                                                    _ptr(ne_diag, torch.float64), _stream(stream)))
 
+    def scatter_energy(self, batch, H, D, W=None, e_partial=None, stream=None):
+        """Own columns of W = D H0 D into W (optional) and Tr(D H0) of the batch's molecules added to e_partial."""
+        torch = _torch()
+        self._check(self.lib.nolsm_scatter_energy(self.handle, batch.handle, H.ref(), D.ref() if D is not None else None,
+                                                  W.ref() if W is not None else None, _ptr(e_partial, torch.float64),
+                                                  _stream(stream)))
+
     # whole path -----------------------------------------------------------------------------------
+    def evaluate(self, H, S, mu, precision=-1, D=None, W=None, want_w=True, q_mol=None, stream=None):
+        """One evaluation at a given mu. Returns (n_electrons, E_elec, D, W, stats)."""
+        torch = _torch()
+        if D is None:
+            D = S.like()
+        if W is None and want_w:
+            W = S.like()
+        ne, e = C.c_double(0.0), C.c_double(0.0)
+        stats = SolveStats()
+        st = self.lib.nolsm_evaluate(self.handle, H.ref(), S.ref(), float(mu), precision, D.ref(),
+                                     W.ref() if W is not None else None, C.byref(ne), C.byref(e),
+                                     _ptr(q_mol, torch.float64), C.byref(stats), _stream(stream))
+        self._check(st)
+        return ne.value, e.value, D, W, stats
+
     def solve_mu(self, H, S, n_electrons, mu_lo, mu_hi, tol_ne_per_mol=1e-3, max_steps=40, precision=-1, D=None,
                  q_mol=None, want_stats=True, stream=None):
         """Returns (mu, n_electrons(mu), D, stats)."""

@@ -105,6 +105,7 @@ static void free_batch(nolsm_batch *b) {
   cudaFree(b->d_tiles_done);
   cudaFree(b->d_group_active);
   cudaFree(b->d_tile_counter);
+  cudaFree(b->d_thin);
   cudaFree(b->d_maps);
   delete b;
 }
@@ -802,6 +803,46 @@ extern "C" nolsm_status nolsm_scatter_density(nolsm_ctx *ctx, const nolsm_batch 
   return NOLSM_OK;
 }
 
+// Eq. 7/11 and Eq. 8/13 for the molecules of a batch
+extern "C" nolsm_status nolsm_scatter_energy(nolsm_ctx *ctx, nolsm_batch *batch, const nolsm_bsr *H,
+                                             const nolsm_bsr *D, nolsm_bsr *W, double *e_partial, void *stream) {
+  if (!ctx || !batch) return NOLSM_EINVAL;
+  CHECK(check_bsr(ctx, H, "H"));
+  if (!batch->sparse || !batch->prepared) { ctx->err = "batch has no sign iterate (call nolsm_sign_batched first)"; return NOLSM_EINVAL; }
+  cudaStream_t st = (cudaStream_t)stream;
+  if (W) {
+    CHECK(check_bsr(ctx, W, "W"));
+    if (W->n_mol != H->n_mol || W->row_ptr != H->row_ptr || W->col_idx != H->col_idx) {
+      ctx->err = "W must share the pattern of H";
+      return NOLSM_EINVAL;
+    }
+    const size_t need = (size_t)2 * batch->count * NOLSM_BS * batch->ld;
+    if (need > batch->thin_cap) {
+      cudaStreamSynchronize(st);
+      cudaFree(batch->d_thin);
+      batch->d_thin = nullptr;
+      batch->thin_cap = 0;
+      if (need && cudaMalloc(&batch->d_thin, need * sizeof(float)) != cudaSuccess) {
+        cudaGetLastError(); ctx->err = "cudaMalloc of the thin-product scratch failed"; return NOLSM_ENOMEM;
+      }
+      batch->thin_cap = need;
+    }
+    cudaError_t e = launch_energy_weighted(batch, x_ptr(batch), sinv_ptr(batch), batch->u[1], H->row_ptr, H->col_idx,
+                                           batch->d_thin, W->val, st);
+    ctx->launches += 4;
+    if (e != cudaSuccess) { ctx->err = std::string("energy-weighted density: ") + cudaGetErrorString(e); return NOLSM_ECUDA; }
+  }
+  if (e_partial) {
+    CHECK(check_bsr(ctx, D, "D"));
+    if (D->n_mol != H->n_mol || D->row_ptr != H->row_ptr || D->col_idx != H->col_idx) {
+      ctx->err = "D must share the pattern of H";
+      return NOLSM_EINVAL;
+    }
+    LAUNCH(ctx, launch_energy(batch, H->row_ptr, D->val, H->val, e_partial, st));
+  }
+  return NOLSM_OK;
+}
+
 // ------------------------------------------------------------------------------------------------
 // Whole path with batching and bisection
 // ------------------------------------------------------------------------------------------------
@@ -898,6 +939,10 @@ extern "C" nolsm_status nolsm_solve_mu(nolsm_ctx *ctx, const nolsm_bsr *H, const
       if (timed) cudaEventRecord(tev[3], st);
       rc = nolsm_scatter_density(ctx, b, S, D, ctx->d_scalars, q_mol, ctx->d_scalars + 1, st);
       if (rc != NOLSM_OK) break;
+      if (ctx->eval_energy) {   // nolsm_evaluate: E = Tr(D H0) and the own columns of W = D H0 D
+        rc = nolsm_scatter_energy(ctx, b, H, D, ctx->eval_w, ctx->d_scalars + 2, st);
+        if (rc != NOLSM_OK) break;
+      }
       if (timed) {
         cudaEventRecord(tev[4], st);
         nolsm_sign_stats cs;
@@ -956,6 +1001,24 @@ extern "C" nolsm_status nolsm_solve_mu(nolsm_ctx *ctx, const nolsm_bsr *H, const
       rc = NOLSM_ENOCONV;
     }
   }
+  return rc;
+}
+
+// One evaluation of the whole path at a given mu, with the electronic energy and (optionally) the
+// energy-weighted density (Eq. 7, 8, 11, 13).
+extern "C" nolsm_status nolsm_evaluate(nolsm_ctx *ctx, const nolsm_bsr *H, const nolsm_bsr *S, double mu,
+                                       int32_t precision, nolsm_bsr *D, nolsm_bsr *W, double *ne_out, double *e_out,
+                                       double *q_mol, nolsm_solve_stats *stats, void *stream) {
+  if (!ctx || !ne_out || !e_out) return NOLSM_EINVAL;
+  ctx->eval_energy = true;
+  ctx->eval_w = W;
+  double mu_found = 0.0;
+  const double half = 1.0;   // bracket [mu - 1, mu + 1]: the first (and only) midpoint is mu itself
+  nolsm_status rc = nolsm_solve_mu(ctx, H, S, 0.0, mu - half, mu + half, -1.0, 1, precision, D, &mu_found, ne_out,
+                                   q_mol, stats, stream);
+  ctx->eval_energy = false;
+  ctx->eval_w = nullptr;
+  *e_out = ctx->h_scalars[2];
   return rc;
 }
 

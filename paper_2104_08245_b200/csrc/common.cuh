@@ -100,6 +100,8 @@ struct nolsm_batch {
   int32_t *d_tiles_done = nullptr;// [count] chain engine: epilogue-warp arrivals per submatrix
   int32_t *d_group_active = nullptr; // [count] chain engine: unfinished submatrices per group
   unsigned long long *d_tile_counter = nullptr;   // chain engine: next tile index to claim
+  float *d_thin = nullptr;        // [2][count][6][ld] scratch of the thin products (energy-weighted density)
+  size_t thin_cap = 0;            // floats
   CUtensorMap *d_maps = nullptr;  // device array: n_half FP16 maps {64,64,1}, then n_unit FP32 maps {32,32,1}
   bool maps_valid = false;
 };
@@ -118,6 +120,8 @@ struct nolsm_ctx {
   cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
   cudaEvent_t tev[2] = {nullptr, nullptr};   // timing of the sign-iteration chain kernel
   void *encode_tiled = nullptr;   // cuTensorMapEncodeTiled entry point
+  bool eval_energy = false;       // nolsm_evaluate in progress: also E (and W) per batch
+  nolsm_bsr *eval_w = nullptr;
   bool umma_ok = false;
   bool pair_ok = false;           // pair-CTA (cta_group::2) engine usable
   int pair_clusters = 0;          // co-resident CTA pairs
@@ -156,6 +160,11 @@ cudaError_t launch_density(const nolsm_batch *b, const float *x, const float *x_
 cudaError_t launch_trace(const nolsm_batch *b, const int32_t *row_ptr, const int32_t *col_idx,
                          const float *d_val, const float *s_val, double *ne, double *q_mol,
                          cudaStream_t st);
+cudaError_t launch_energy_weighted(const nolsm_batch *b, const float *x, const float *sinv, const float *h,
+                                   const int32_t *row_ptr, const int32_t *col_idx, float *thin, float *w_val,
+                                   cudaStream_t st);
+cudaError_t launch_energy(const nolsm_batch *b, const int32_t *row_ptr, const float *d_val, const float *h_val,
+                          double *e_out, cudaStream_t st);
 // dense helpers
 cudaError_t launch_norm_bound(const nolsm_batch *b, const float *a, float mu, float *norm2,
                               cudaStream_t st);

@@ -317,3 +317,124 @@ cudaError_t launch_trace(const nolsm_batch *b, const int32_t *row_ptr, const int
       row_ptr, col_idx, b->mol_begin, b->count, d_val, s_val, ne, q_mol);
   return cudaGetLastError();
 }
+
+// ------------------------------------------------------------------------------------------------
+// Energy-weighted density and electronic energy.
+//   T_j(W) = T_j(D) T_j(H0) T_j(D)   (Eq. 8, 13 PAPER.md:127-129,163-168); only the own columns are kept
+//   (PAPER.md:168), and with T_j(D) = 1/2 (I - X) S^-1 they need no n^3 product:
+//       y1 = D[:, own]           = 1/2 (t - X t),  t = S^-1[:, own]
+//       y2 = H0 y1,   y3 = S^-1 y2,
+//       W[:, own] = D (H0 D[:, own]) = 1/2 (y3 - X y3)
+//   four n x n x 6 products per submatrix, FP32, bound by reading the dense matrices once each.
+// k_thin: out = beta * add + alpha * A * in for one submatrix per blockIdx.y; `in` (n x 6) is staged in
+// shared memory, one thread per row, A read column by column (coalesced).  Thin operands live in a
+// scratch [submatrix][6][ld]; in_cols / out_blocks switch the first input to columns own0.. of a dense
+// matrix and the last output to the column-owned block store.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(DN_THREADS)
+k_thin(const int32_t *__restrict__ row_ptr, const int32_t *__restrict__ col_idx, int mol_begin, int ld,
+       int64_t slab, const float *__restrict__ a, const float *__restrict__ in_thin,
+       const float *__restrict__ in_cols, const float *__restrict__ add_thin, float alpha, float beta,
+       float *__restrict__ out_thin, float *__restrict__ out_blocks) {
+  extern __shared__ float s_in[];  // [6][n]
+  const int mat = blockIdx.y;
+  const int j = mol_begin + mat;
+  const int lo = row_ptr[j];
+  const int m = row_ptr[j + 1] - lo;
+  const int n = m * NOLSM_BS;
+  int l = 0, r_ = m;
+  while (l < r_) {
+    const int mid = (l + r_) >> 1;
+    if (col_idx[lo + mid] < j) l = mid + 1; else r_ = mid;
+  }
+  const int own0 = l * NOLSM_BS;
+  const float *aj = a + (int64_t)mat * slab;
+  const int64_t thin0 = (int64_t)mat * NOLSM_BS * ld;
+  for (int t = threadIdx.x; t < NOLSM_BS * n; t += blockDim.x) {
+    const int p = t / n, k = t - p * n;
+    s_in[t] = in_cols ? in_cols[(int64_t)mat * slab + (int64_t)(own0 + p) * ld + k] : in_thin[thin0 + (int64_t)p * ld + k];
+  }
+  __syncthreads();
+  const int r = blockIdx.x * DN_THREADS + threadIdx.x;
+  if (r >= n) return;
+  float acc[NOLSM_BS];
+#pragma unroll
+  for (int p = 0; p < NOLSM_BS; ++p) acc[p] = 0.f;
+  for (int k = 0; k < n; ++k) {
+    const float av = aj[(int64_t)k * ld + r];
+#pragma unroll
+    for (int p = 0; p < NOLSM_BS; ++p) acc[p] = fmaf(av, s_in[p * n + k], acc[p]);
+  }
+#pragma unroll
+  for (int p = 0; p < NOLSM_BS; ++p) {
+    float v = alpha * acc[p];
+    if (beta != 0.f) v = fmaf(beta, add_thin ? add_thin[thin0 + (int64_t)p * ld + r] : s_in[p * n + r], v);
+    if (out_blocks) out_blocks[(int64_t)lo * 36 + (int64_t)r * NOLSM_BS + p] = v;
+    else out_thin[thin0 + (int64_t)p * ld + r] = v;
+  }
+}
+
+static cudaError_t thin_launch(const nolsm_batch *b, const int32_t *row_ptr, const int32_t *col_idx, const float *a,
+                               const float *in_thin, const float *in_cols, const float *add_thin, float alpha,
+                               float beta, float *out_thin, float *out_blocks, cudaStream_t st) {
+  const size_t smem = (size_t)NOLSM_BS * b->max_n * sizeof(float);
+  static size_t smem_set = 0;
+  if (smem > 48 * 1024 && smem > smem_set) {
+    cudaError_t e = cudaFuncSetAttribute(k_thin, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    smem_set = smem;
+  }
+  dim3 grid((b->max_n + DN_THREADS - 1) / DN_THREADS, b->count);
+  k_thin<<<grid, DN_THREADS, smem, st>>>(row_ptr, col_idx, b->mol_begin, b->ld, (int64_t)b->ld * b->ld, a, in_thin,
+                                         in_cols, add_thin, alpha, beta, out_thin, out_blocks);
+  return cudaGetLastError();
+}
+
+// thin: scratch of 2 * count * 6 * ld floats.  beta with add_thin == nullptr adds beta * (the staged input).
+cudaError_t launch_energy_weighted(const nolsm_batch *b, const float *x, const float *sinv, const float *h,
+                                   const int32_t *row_ptr, const int32_t *col_idx, float *thin, float *w_val,
+                                   cudaStream_t st) {
+  if (b->count == 0) return cudaSuccess;
+  float *t0 = thin, *t1 = thin + (size_t)b->count * NOLSM_BS * b->ld;
+  cudaError_t e;
+  // y1 = 1/2 t - 1/2 X t,  t = S^-1[:, own]
+  if ((e = thin_launch(b, row_ptr, col_idx, x, nullptr, sinv, nullptr, -0.5f, 0.5f, t0, nullptr, st)) != cudaSuccess) return e;
+  // y2 = H0 y1
+  if ((e = thin_launch(b, row_ptr, col_idx, h, t0, nullptr, nullptr, 1.f, 0.f, t1, nullptr, st)) != cudaSuccess) return e;
+  // y3 = S^-1 y2
+  if ((e = thin_launch(b, row_ptr, col_idx, sinv, t1, nullptr, nullptr, 1.f, 0.f, t0, nullptr, st)) != cudaSuccess) return e;
+  // W[:, own] = 1/2 y3 - 1/2 X y3 -> block store
+  return thin_launch(b, row_ptr, col_idx, x, t0, nullptr, nullptr, -0.5f, 0.5f, nullptr, w_val, st);
+}
+
+// E = sum over the batch's molecules j and their stored blocks k of sum_{o,p} D_k[o][p] H_k[p][o]
+// (Eq. 11: D_k = D(i, j) column-owned, H_k = H0(j, i), i = col_idx[k]).  One warp per
+// molecule, FP32 products, FP64 accumulation.
+__global__ void __launch_bounds__(TR_WARPS * 32)
+k_energy(const int32_t *__restrict__ row_ptr, int mol_begin, int count, const float *__restrict__ d_val,
+         const float *__restrict__ h_val, double *__restrict__ e_out) {
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int mat = blockIdx.x * TR_WARPS + warp;
+  if (mat >= count) return;
+  const int j = mol_begin + mat;
+  double sum = 0.0;
+  for (int k = row_ptr[j] + lane; k < row_ptr[j + 1]; k += 32) {
+    const float *db = d_val + (int64_t)k * 36, *hb = h_val + (int64_t)k * 36;
+    double part = 0.0;
+#pragma unroll
+    for (int o = 0; o < NOLSM_BS; ++o)
+#pragma unroll
+      for (int p = 0; p < NOLSM_BS; ++p) part += (double)(db[o * NOLSM_BS + p] * hb[p * NOLSM_BS + o]);
+    sum += part;
+  }
+  for (int d = 16; d > 0; d >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, d);
+  if (lane == 0) atomicAdd(e_out, sum);
+}
+
+cudaError_t launch_energy(const nolsm_batch *b, const int32_t *row_ptr, const float *d_val, const float *h_val,
+                          double *e_out, cudaStream_t st) {
+  if (b->count == 0) return cudaSuccess;
+  k_energy<<<(b->count + TR_WARPS - 1) / TR_WARPS, TR_WARPS * 32, 0, st>>>(row_ptr, b->mol_begin, b->count, d_val,
+                                                                          h_val, e_out);
+  return cudaGetLastError();
+}

@@ -423,3 +423,60 @@ def test_pair_engines_building_block(nolsm, torch_mod, flag, kind, tol, n, batch
     assert np.abs(c.cpu().numpy() - want).max() / np.sqrt(n) < tol
     assert np.allclose(r2.cpu().numpy(), (want ** 2).sum(axis=(1, 2)), rtol=5e-3 if kind == 1 else 1e-4)
     ctx.close()
+
+
+# ---------------------------------------------------------------------------------------------
+# energy-weighted density and electronic energy (Eq. 7, 8, 11, 13)
+# ---------------------------------------------------------------------------------------------
+TOL_W = {0: 5e-3, 1: 2e-5}       # |W| <~ 2.5 |D| (H0 eigenvalues down to -2.5 Ha): same relative bound as D
+TOL_E_PER_MOL = {0: 2e-3, 1: 2e-5}
+
+
+@pytest.mark.parametrize("precision", [1, 0])
+def test_energy_weighted_density_tiny(nolsm, tiny_system, tiny_solution, precision):
+    import oracle.nolsm_oracle as orc
+    sols = tiny_solution["solutions"]
+    H, S = _device_system(nolsm, tiny_system)
+    ctx = nolsm.Context(nolsm.Config(precision=precision))
+    ne, e, D, W, stats = ctx.evaluate(H, S, MU)
+    d_ref = orc.density_blocks(sols, tiny_system.row_ptr, MU)
+    w_ref = orc.energy_weighted_blocks(sols, tiny_system.row_ptr, MU)
+    assert np.abs(D.val.cpu().numpy() - d_ref).max() < TOL_D[precision]
+    assert np.abs(W.val.cpu().numpy() - w_ref).max() < TOL_W[precision]
+    e_ref = orc.electronic_energy_blocks(tiny_system.row_ptr, tiny_system.col_idx, d_ref, tiny_system.h_val)
+    assert abs(e - e_ref) / tiny_system.n_mol < TOL_E_PER_MOL[precision]
+    # the GPU's own reduction agrees with the oracle's contraction of the GPU's D
+    e_own = orc.electronic_energy_blocks(tiny_system.row_ptr, tiny_system.col_idx, D.val.cpu().numpy(), tiny_system.h_val)
+    assert abs(e - e_own) < 1e-4
+    assert abs(ne - orc.electron_count(sols, MU)) / tiny_system.n_mol <= TOL_NE_PER_MOL
+    # E only (no W store)
+    ne2, e2, _, W2, _ = ctx.evaluate(H, S, MU, want_w=False)
+    assert W2 is None and abs(e2 - e) < 1e-6
+    ctx.close()
+
+
+@pytest.mark.parametrize("precision", [1, 0])
+def test_energy_weighted_density_mid_batch(nolsm, mid_system, mid_solution, precision):
+    """Batch-level entry on a partial batch (n ~ 478): W columns and the batch's share of Tr(D H0)."""
+    import torch
+    import oracle.nolsm_oracle as orc
+    sols = mid_solution["solutions"]
+    begin, count = 50, 60
+    H, S = _device_system(nolsm, mid_system)
+    D, W = S.like(), S.like()
+    ctx = nolsm.Context(nolsm.Config(precision=precision))
+    batch = ctx.build_submatrices(H, S, begin, count)
+    ctx.sign_batched(batch, MU)
+    ne = torch.zeros(1, dtype=torch.float64, device="cuda")
+    e = torch.zeros(1, dtype=torch.float64, device="cuda")
+    ctx.scatter_density(batch, S, D, ne, None, None)
+    ctx.scatter_energy(batch, H, D, W, e)
+    lo, hi = mid_system.row_ptr[begin], mid_system.row_ptr[begin + count]
+    w_ref = orc.energy_weighted_blocks(sols[begin:begin + count], mid_system.row_ptr, MU)
+    d_ref = orc.density_blocks(sols[begin:begin + count], mid_system.row_ptr, MU)
+    w = W.val.cpu().numpy()
+    assert np.abs(w[lo:hi] - w_ref[lo:hi]).max() < TOL_W[precision]
+    assert not w[:lo].any() and not w[hi:].any()
+    e_ref = float(np.einsum("kop,kpo->", d_ref[lo:hi], mid_system.h_val[lo:hi].astype(np.float64)))
+    assert abs(e.item() - e_ref) / count < TOL_E_PER_MOL[precision]
+    ctx.close()
