@@ -429,32 +429,43 @@ static nolsm_status prepare_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, int prec
   pg.max_iter = ctx->cfg.inv_max_iter;
   pg.fixed_iter = 0;
   pg.tol = inv_tol;
+  // Iteration 0 in closed form (Z0 = I): E0 = I - Y0, Z1 = 3/2 I - 1/2 Y0 element-wise, Y1 = Y0 + 1/2 Y0 E0 by
+  // one product; the chain then starts at iteration 1, i.e. on the odd-parity buffers.
+  pg.max_iter = std::max(1, ctx->cfg.inv_max_iter - 1);
+  ChainProgram p0 = one_shot(group_size(ctx, b, 16));
+  p0.n_ops = 1;
+  ChainOp &y1 = p0.ops[0] = make_op(EPI_AXPBY, 0.5f, 1.f);
+  y1.cin32 = y1.cout32 = 2;
   if (fp16) {
     // Y16: h0/h1 (ping-pong), Z16: h2/h3, E16: h4; masters Y32 = u2, Z32 = u3
-    LAUNCH(ctx, launch_init_inverse(b, S, b->d_norm, b->u[2], b->u[3], b->h[0], b->h[2], nullptr, nullptr,
-                                    b->d_scale, st));
+    LAUNCH(ctx, launch_init_inverse_first(b, S, b->d_norm, b->u[2], b->u[3], b->h[0], nullptr, b->h[3], nullptr,
+                                          b->h[4], nullptr, b->d_scale, st));
+    set2(y1.a, 0, 0); set2(y1.b, 4, 4); set2(y1.out16, 1, 1);
     pg.group = group_size(ctx, b, 18);
     ChainOp &e = pg.ops[0] = make_op(EPI_IDENT, 1.f, 0.f);
-    set2(e.a, 2, 3); set2(e.b, 0, 1); set2(e.out16, 4, 4); e.resid = 1;
+    set2(e.a, 3, 2); set2(e.b, 1, 0); set2(e.out16, 4, 4); e.resid = 1;
     ChainOp &y = pg.ops[1] = make_op(EPI_AXPBY, 0.5f, 1.f);
-    set2(y.a, 0, 1); set2(y.b, 4, 4); y.cin32 = y.cout32 = 2; set2(y.out16, 1, 0);
+    set2(y.a, 1, 0); set2(y.b, 4, 4); y.cin32 = y.cout32 = 2; set2(y.out16, 0, 1);
     ChainOp &z = pg.ops[2] = make_op(EPI_AXPBY, 0.5f, 1.f);
-    set2(z.a, 4, 4); set2(z.b, 2, 3); z.cin32 = z.cout32 = 3; set2(z.out16, 3, 2);
+    set2(z.a, 4, 4); set2(z.b, 3, 2); z.cin32 = z.cout32 = 3; set2(z.out16, 2, 3);
   } else {
     // split operands: Y (h0,h1)/(h2,h3), Z (h4,h5)/(h6,h7), E (h8,h9)
-    LAUNCH(ctx, launch_init_inverse(b, S, b->d_norm, b->u[2], b->u[3], b->h[0], b->h[4], b->h[1], b->h[5],
-                                    b->d_scale, st));
+    LAUNCH(ctx, launch_init_inverse_first(b, S, b->d_norm, b->u[2], b->u[3], b->h[0], b->h[1], b->h[6], b->h[7],
+                                          b->h[8], b->h[9], b->d_scale, st));
+    set2(y1.a, 0, 0); set2(y1.a_lo, 1, 1); set2(y1.b, 8, 8); set2(y1.b_lo, 9, 9);
+    set2(y1.out16, 2, 2); set2(y1.out16_lo, 3, 3);
     pg.group = group_size(ctx, b, 28);
     ChainOp &e = pg.ops[0] = make_op(EPI_IDENT, 1.f, 0.f);
-    set2(e.a, 4, 6); set2(e.a_lo, 5, 7); set2(e.b, 0, 2); set2(e.b_lo, 1, 3);
+    set2(e.a, 6, 4); set2(e.a_lo, 7, 5); set2(e.b, 2, 0); set2(e.b_lo, 3, 1);
     set2(e.out16, 8, 8); set2(e.out16_lo, 9, 9); e.resid = 1;
     ChainOp &y = pg.ops[1] = make_op(EPI_AXPBY, 0.5f, 1.f);
-    set2(y.a, 0, 2); set2(y.a_lo, 1, 3); set2(y.b, 8, 8); set2(y.b_lo, 9, 9);
-    y.cin32 = y.cout32 = 2; set2(y.out16, 2, 0); set2(y.out16_lo, 3, 1);
+    set2(y.a, 2, 0); set2(y.a_lo, 3, 1); set2(y.b, 8, 8); set2(y.b_lo, 9, 9);
+    y.cin32 = y.cout32 = 2; set2(y.out16, 0, 2); set2(y.out16_lo, 1, 3);
     ChainOp &z = pg.ops[2] = make_op(EPI_AXPBY, 0.5f, 1.f);
-    set2(z.a, 8, 8); set2(z.a_lo, 9, 9); set2(z.b, 4, 6); set2(z.b_lo, 5, 7);
-    z.cin32 = z.cout32 = 3; set2(z.out16, 6, 4); set2(z.out16_lo, 7, 5);
+    set2(z.a, 8, 8); set2(z.a_lo, 9, 9); set2(z.b, 6, 4); set2(z.b_lo, 7, 5);
+    z.cin32 = z.cout32 = 3; set2(z.out16, 4, 6); set2(z.out16_lo, 5, 7);
   }
+  CHECK(run_chain(ctx, b, p0, nullptr, false, st));
   CHECK(run_chain(ctx, b, pg, nullptr, true, st));
   int64_t inv_gemm_sum = 0;
   if (stats) {   // iterations and residuals of Eq. 15-17, before the sign iteration reuses the arrays
@@ -465,10 +476,11 @@ static nolsm_status prepare_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, int prec
     NOLSM_CUDA(ctx, cudaStreamSynchronize(st));
     double fl = 0.0;
     for (int m = 0; m < b->count; ++m) {
+      it[m] += 1;   // iteration 0 ran in closed form
       stats->inv_iter_max = std::max(stats->inv_iter_max, it[m]);
       if (!(res[m] <= stats->inv_worst_residual)) stats->inv_worst_residual = res[m];
       const double n = b->n_host[m];
-      const int products = 3 * it[m] + 2 + 2 * refine;   // products, whatever the MMAs per product
+      const int products = 3 * it[m] - 2 + 2 + 2 * refine;   // products, whatever the MMAs per product
       inv_gemm_sum += products;
       fl += 2.0 * n * n * n * products;
     }

@@ -171,6 +171,9 @@ cudaError_t launch_norm_bound(const nolsm_batch *b, const float *a, float mu, fl
 cudaError_t launch_init_inverse(const nolsm_batch *b, const float *s, const float *norm2, float *y32,
                                 float *z32, __half *y16, __half *z16, __half *y16_lo, __half *z16_lo,
                                 float *scale_out, cudaStream_t st);
+cudaError_t launch_init_inverse_first(const nolsm_batch *b, const float *s, const float *norm2, float *y32,
+                                      float *z32, __half *y16, __half *y16_lo, __half *z16, __half *z16_lo,
+                                      __half *e16, __half *e16_lo, float *scale_out, cudaStream_t st);
 cudaError_t launch_make_x0(const nolsm_batch *b, const float *bmat, float mu, const float *norm2,
                            const float *scale_in, float *x32, __half *x16, __half *x16_lo, float *scale_out,
                            cudaStream_t st);

@@ -141,6 +141,45 @@ cudaError_t launch_init_inverse(const nolsm_batch *b, const float *s, const floa
   return cudaGetLastError();
 }
 
+// Eq. 15-16 with the first iteration done in closed form: Z0 = I gives E0 = I - Z0 Y0 = I - Y0 and
+// Z1 = Z0 + 1/2 E0 Z0 = 3/2 I - 1/2 Y0 without any product; only Y1 = Y0 + 1/2 Y0 E0 needs one.
+// Writes Y0 (FP32 master + FP16 operand), E0 (FP16 operand) and Z1 (FP32 master + FP16 operand).
+__global__ void __launch_bounds__(256)
+k_init_inverse_first(const int32_t *__restrict__ dims, int ld, int64_t slab, int count,
+                     const float *__restrict__ s, const float *__restrict__ norm2, float *__restrict__ y32,
+                     float *__restrict__ z32, __half *__restrict__ y16, __half *__restrict__ y16_lo,
+                     __half *__restrict__ z16, __half *__restrict__ z16_lo, __half *__restrict__ e16,
+                     __half *__restrict__ e16_lo, float *__restrict__ scale_out) {
+  Elem4 e;
+  if (!elem4(dims, ld, slab, e)) return;
+  const int mat = blockIdx.y;
+  const float sc = fmaxf(1.f, sqrtf(norm2[mat] * norm2[count + mat]));
+  if (e.r == 0 && e.c == 0) scale_out[mat] = sc;
+  const float4 sv = *reinterpret_cast<const float4 *>(s + e.off);
+  const float y[4] = {sv.x / sc, sv.y / sc, sv.z / sc, sv.w / sc};
+  float ev[4], z[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const float d = (e.r + i == e.c) ? 1.f : 0.f;
+    ev[i] = d - y[i];
+    z[i] = fmaf(0.5f, ev[i], d);
+  }
+  *reinterpret_cast<float4 *>(y32 + e.off) = make_float4(y[0], y[1], y[2], y[3]);
+  *reinterpret_cast<float4 *>(z32 + e.off) = make_float4(z[0], z[1], z[2], z[3]);
+  store_split4(y16 + e.off, y16_lo ? y16_lo + e.off : nullptr, y);
+  store_split4(z16 + e.off, z16_lo ? z16_lo + e.off : nullptr, z);
+  store_split4(e16 + e.off, e16_lo ? e16_lo + e.off : nullptr, ev);
+}
+
+cudaError_t launch_init_inverse_first(const nolsm_batch *b, const float *s, const float *norm2, float *y32,
+                                      float *z32, __half *y16, __half *y16_lo, __half *z16, __half *z16_lo,
+                                      __half *e16, __half *e16_lo, float *scale_out, cudaStream_t st) {
+  if (b->count == 0) return cudaSuccess;
+  k_init_inverse_first<<<elem4_grid(b), 256, 0, st>>>(b->d_dims, b->ld, (int64_t)b->ld * b->ld, b->count, s, norm2,
+                                                      y32, z32, y16, y16_lo, z16, z16_lo, e16, e16_lo, scale_out);
+  return cudaGetLastError();
+}
+
 // X0 = (B - mu I)/s  (Eq. 9 with the rescaling of PAPER.md:138), s from the norm bound or from the
 // caller (scale_in, dense microbench).  Padded diagonal = 1: a fixed point of the iteration that adds
 // nothing to the residual (reading 19).
