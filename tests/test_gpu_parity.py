@@ -480,3 +480,99 @@ def test_energy_weighted_density_mid_batch(nolsm, mid_system, mid_solution, prec
     e_ref = float(np.einsum("kop,kpo->", d_ref[lo:hi], mid_system.h_val[lo:hi].astype(np.float64)))
     assert abs(e.item() - e_ref) / count < TOL_E_PER_MOL[precision]
     ctx.close()
+
+
+# ---------------------------------------------------------------------------------------------
+# more shapes: isolated molecules (n = 6), config-4-sized submatrices (n ~ 1489), larger microbench
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("precision", [1, 0])
+def test_isolated_molecules_n6(nolsm, precision):
+    """Cutoff 1 A: every neighbour list is the molecule itself, every submatrix is 6 x 6 (one padded tile)."""
+    import nolsm_inputs as gi
+    import oracle.nolsm_oracle as orc
+    system = gi.make_water_system(32, 1.0)
+    assert system.nnzb == 32
+    sol = orc.solve_system(system, mu=MU)
+    H, S = _device_system(nolsm, system)
+    ctx = nolsm.Context(nolsm.Config(precision=precision))
+    ne, e, D, W, stats = ctx.evaluate(H, S, MU)
+    d_ref = orc.density_blocks(sol["solutions"], system.row_ptr, MU)
+    w_ref = orc.energy_weighted_blocks(sol["solutions"], system.row_ptr, MU)
+    assert np.abs(D.val.cpu().numpy() - d_ref).max() < TOL_D[precision]
+    assert np.abs(W.val.cpu().numpy() - w_ref).max() < TOL_W[precision]
+    assert abs(ne - orc.electron_count(sol["solutions"], MU)) / 32 <= TOL_NE_PER_MOL
+    ctx.close()
+
+
+def test_config4_sized_submatrices_sampled(nolsm):
+    """4096 molecules at the 12 A cutoff of BASELINE configs[3]: n ~ 1489 (12 row tiles, 6 column tiles)."""
+    import torch
+    import nolsm_inputs as gi
+    import oracle.nolsm_oracle as orc
+    system = gi.make_water_system(4096, 12.0)
+    H, S = _device_system(nolsm, system)
+    D = S.like()
+    ctx = nolsm.Context(nolsm.Config(precision=0))
+    begin, count = 2100, 40
+    batch = ctx.build_submatrices(H, S, begin, count)
+    stats = ctx.sign_batched(batch, MU)
+    assert stats.n_unconverged == 0
+    ne = torch.zeros(1, dtype=torch.float64, device="cuda")
+    q = torch.zeros(system.n_mol, dtype=torch.float64, device="cuda")
+    ctx.scatter_density(batch, S, D, ne, q, None)
+    d = D.val.cpu().numpy()
+    for local in (0, 39):
+        j = begin + local
+        sol = orc.solve_molecule(system.row_ptr, system.col_idx, system.h_val, system.s_val, j)
+        assert sol.n > 1400
+        ref = sol.density_columns(MU).reshape(-1, 6, 6)
+        lo = system.row_ptr[j]
+        assert np.abs(d[lo:lo + ref.shape[0]] - ref).max() < TOL_D[0]
+        assert abs(q[j].item() - sol.population(MU)) < 5e-3
+        assert orc.sign_residual(batch.read(local, nolsm.MAT_X).cpu().numpy()) <= TOL_RESID
+    ctx.close()
+
+
+@pytest.mark.parametrize("precision,tol_x", [(1, 2e-5), (0, 3e-3)])
+def test_sign_dense_n1024(nolsm, torch_mod, precision, tol_x):
+    import nolsm_inputs as gi
+    import oracle.nolsm_oracle as orc
+    mats = [gi.make_gapped_symmetric(1024, seed=11, index=i) for i in range(2)]
+    a = torch_mod.as_tensor(np.stack([m[0] for m in mats])).cuda()
+    scale = torch_mod.as_tensor(np.array([np.abs(m[2]).max() for m in mats], dtype=np.float32)).cuda()
+    ctx = nolsm.Context(nolsm.Config(precision=precision))
+    x, stats = ctx.sign_dense_batched(a, scale)
+    assert stats.n_unconverged == 0
+    for i, (_, q, lam) in enumerate(mats):
+        assert np.abs(x[i].cpu().numpy() - orc.sign_by_construction(q, lam)).max() < tol_x
+    ctx.close()
+
+
+def test_w32768_whole_step_in_bench_configuration_sampled(nolsm):
+    """BASELINE configs[2] at full size through the call bench.py times (nolsm_solve_mu, 24 GiB workspace,
+    38 streamed batches, default engine): sampled molecules against the oracle, plus properties that hold
+    for every molecule (plateau populations, pattern-only writes)."""
+    import torch
+    import nolsm_inputs as gi
+    import oracle.nolsm_oracle as orc
+    n_mol, cutoff = gi.CONFIGS["w32768"]
+    system = gi.make_water_system(n_mol, cutoff)
+    H, S = _device_system(nolsm, system)
+    ctx = nolsm.Context(nolsm.Config(precision=0, workspace_bytes=24 << 30))
+    q = torch.zeros(n_mol, dtype=torch.float64, device="cuda")
+    mu, ne, D, stats = ctx.solve_mu(H, S, system.n_electrons, 2 * MU, 0.0, tol_ne_per_mol=-1.0, max_steps=1, q_mol=q)
+    assert mu == MU and stats.n_batches > 30 and stats.last.n_unconverged == 0
+    assert 8 <= stats.last.iter_min and stats.last.iter_max <= 12
+    d = D.val.cpu().numpy()
+    qh = q.cpu().numpy()
+    for j in (0, 12345, 20000, 32767):           # first / last batch and two in between
+        sol = orc.solve_molecule(system.row_ptr, system.col_idx, system.h_val, system.s_val, j)
+        ref = sol.density_columns(MU).reshape(-1, 6, 6)
+        lo = system.row_ptr[j]
+        assert np.abs(d[lo:lo + ref.shape[0]] - ref).max() < TOL_D[0], j
+        assert abs(qh[j] - sol.population(MU)) < 5e-3
+    assert np.abs(qh - 8.0).max() < 0.03          # every molecule sits on the plateau (reading 14)
+    assert abs(ne - qh.sum()) < 1e-6 * n_mol
+    assert abs(ne - system.n_electrons) / n_mol < 1e-3
+    assert np.isfinite(d).all()
+    ctx.close()
