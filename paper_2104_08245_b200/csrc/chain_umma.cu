@@ -92,6 +92,18 @@ __device__ __forceinline__ void tma_load_3d(void *dst, const CUtensorMap *map, u
       "l"(reinterpret_cast<uint64_t>(map)), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2)
       : "memory");
 }
+// one lane of the (converged) warp; the compiler keeps code guarded by it on the uniform datapath
+__device__ __forceinline__ bool elect_one() {
+  uint32_t p;
+  asm volatile(
+      "{\n\t"
+      ".reg .pred P;\n\t"
+      "elect.sync _|P, 0xffffffff;\n\t"
+      "selp.u32 %0, 1, 0, P;\n\t"
+      "}\n"
+      : "=r"(p));
+  return p != 0;
+}
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
@@ -109,6 +121,24 @@ __device__ __forceinline__ void tc_mma_f16(uint32_t tmem_d, uint64_t adesc, uint
       "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t"
       "}\n" ::"r"(tmem_d),
       "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+// Same with the descriptors given as 32-bit halves: the high half (stride offset, version, swizzle) is a
+// constant, the low half is base + k * step, so the single issuing thread spends a handful of integer
+// instructions per MMA instead of rebuilding two 64-bit descriptors (it was issue-bound at ~200 cycles
+// per MMA against the 128 the tensor pipe needs, profiles/r1_k_chain_sign_w32768.md).
+__device__ __forceinline__ void tc_mma_f16_lh(uint32_t tmem_d, uint32_t a_lo, uint32_t b_lo, uint32_t desc_hi,
+                                              uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t"
+      ".reg .pred p;\n\t"
+      ".reg .b64 da, db;\n\t"
+      "setp.ne.b32 p, %5, 0;\n\t"
+      "mov.b64 da, {%1, %3};\n\t"
+      "mov.b64 db, {%2, %3};\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], da, db, %4, p;\n\t"
+      "}\n" ::"r"(tmem_d),
+      "r"(a_lo), "r"(b_lo), "r"(desc_hi), "r"(idesc), "r"(accumulate)
       : "memory");
 }
 __device__ __forceinline__ void tc_ld32(uint32_t taddr, uint32_t (&v)[32]) {
@@ -271,6 +301,9 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
   } else if (warp == 2) {
     // ===================== TMA producer =====================
     if (lane == 0) {
+#ifdef NOLSM_NOTMA
+      int tma_issued = 0;
+#endif
 #ifdef NOLSM_TRACE
       int tti = 0;
 #endif
@@ -296,6 +329,10 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
         for (int kb = 0; kb < c.kblocks; ++kb) {
           mbar_wait(&empty_bar[stage], phase ^ 1u);
           uint8_t *st = smem + (size_t)stage * args.stage_bytes;
+#ifdef NOLSM_NOTMA   // timing experiment only: the barrier protocol without any operand traffic (results are wrong)
+          if (tma_issued >= args.stages) { mbar_arrive(&full_bar[stage]); if (++stage == args.stages) { stage = 0; phase ^= 1u; } continue; }
+          ++tma_issued;
+#endif
           mbar_expect_tx(&full_bar[stage], bytes);
           const int k0 = kb * kBK;
           tma_load_3d(st, ma, &full_bar[stage], m0, k0, m);
@@ -318,16 +355,23 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
     }
   } else if (warp == 1) {
     // ===================== MMA issuer =====================
-    if (lane == 0) {
+    // The whole warp walks the tile sequence (uniform control flow, operands in uniform registers); one
+    // elected lane issues the MMAs, commits and arrivals.
+    {
+      const bool one = elect_one();
 #ifdef NOLSM_TRACE
       int mti = 0;
 #endif
       int stage = 0, slot = 0, acc = 0;
       uint32_t phase = 0, ring_phase = 0, acc_phase = 0;
+      const uint32_t smem_base = smem_u32(smem);
+      // high half of every operand descriptor: stride offset 1024 B (8-row atoms), version 1, 128-byte swizzle
+      constexpr uint32_t kDescHi = (1024u >> 4) | (1u << 14) | (2u << 29);
       for (;;) {
         mbar_wait(&cmd_full[slot], ring_phase);
         const TileCmd c = cmds[slot];
-        mbar_arrive(&cmd_empty[slot]);
+        __syncwarp();
+        if (one) mbar_arrive(&cmd_empty[slot]);
         if (++slot == kRing) { slot = 0; ring_phase ^= 1u; }
         if (c.op < 0) break;
         const bool split = pg.ops[c.op].a_lo[c.iter & 1] >= 0;
@@ -354,25 +398,35 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
           wsum += clock64() - w0;
 #endif
           tc_fence_after();
-          const uint32_t sa = smem_u32(smem + (size_t)stage * args.stage_bytes);
+          // descriptor low halves: (address >> 4) | leading offset << 16; A (M-major): leading offset = the
+          // second 64-row chunk (8192 B), +2048 B per K=16 step; B (K-major): leading offset 16 B, +32 B per step
+          const uint32_t sa = smem_base + (uint32_t)stage * (uint32_t)args.stage_bytes;
+          const uint32_t a_lo = ((sa >> 4) & 0x3FFFu) | ((uint32_t)(kBoxBytes >> 4) << 16);
+          const uint32_t b_lo = (((sa + off_b) >> 4) & 0x3FFFu) | (1u << 16);
           const int steps = kb == c.kblocks - 1 ? c.ktail : kBK / 16;
-          for (int k4 = 0; k4 < steps; ++k4) {
-            // A (M-major): 16 K-rows of 128 B per MMA -> +2048 B; B (K-major): 16 K elements -> +32 B
-            const uint64_t ad = make_smem_desc(sa + k4 * 2048, kBoxBytes, 1024);
-            const uint64_t bd = make_smem_desc(sa + off_b + k4 * 32, 16, 1024);
-            const uint32_t accum = (kb | k4) ? 1u : 0u;
-            tc_mma_f16(d_main, ad, bd, idesc, accum);
-            if (split) {
-              const uint64_t adl = make_smem_desc(sa + off_a_lo + k4 * 2048, kBoxBytes, 1024);
-              const uint64_t bdl = make_smem_desc(sa + off_b_lo + k4 * 32, 16, 1024);
-              tc_mma_f16(d_corr, ad, bdl, idesc, accum);
-              tc_mma_f16(d_corr, adl, bd, idesc, 1u);
+          if (one) {
+          if (!split) {
+            tc_mma_f16_lh(d_main, a_lo, b_lo, kDescHi, idesc, kb ? 1u : 0u);
+            if (steps > 1) tc_mma_f16_lh(d_main, a_lo + 128u, b_lo + 2u, kDescHi, idesc, 1u);
+            if (steps > 2) tc_mma_f16_lh(d_main, a_lo + 256u, b_lo + 4u, kDescHi, idesc, 1u);
+            if (steps > 3) tc_mma_f16_lh(d_main, a_lo + 384u, b_lo + 6u, kDescHi, idesc, 1u);
+          } else {
+            const uint32_t al_lo = (((sa + off_a_lo) >> 4) & 0x3FFFu) | ((uint32_t)(kBoxBytes >> 4) << 16);
+            const uint32_t bl_lo = (((sa + off_b_lo) >> 4) & 0x3FFFu) | (1u << 16);
+            for (int k4 = 0; k4 < steps; ++k4) {
+              const uint32_t accum = (kb | k4) ? 1u : 0u;
+              tc_mma_f16_lh(d_main, a_lo + 128u * k4, b_lo + 2u * k4, kDescHi, idesc, accum);
+              tc_mma_f16_lh(d_corr, a_lo + 128u * k4, bl_lo + 2u * k4, kDescHi, idesc, accum);
+              tc_mma_f16_lh(d_corr, al_lo + 128u * k4, b_lo + 2u * k4, kDescHi, idesc, 1u);
             }
           }
           tc_commit(&empty_bar[stage]);
+          }
+          __syncwarp();
           if (++stage == args.stages) { stage = 0; phase ^= 1u; }
         }
-        tc_commit(&tfull_bar[acc]);
+        if (one) tc_commit(&tfull_bar[acc]);
+        __syncwarp();
 #ifdef NOLSM_TRACE
         if (blockIdx.x == 0 && mti - 1 < 4096) { g_wait[mti - 1][0] = wsum; g_wait[mti - 1][2] = clock64() - t_begin; }
 #endif
