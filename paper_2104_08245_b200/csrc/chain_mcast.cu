@@ -117,6 +117,33 @@ __device__ __forceinline__ void tc_mma2_f16(uint32_t tmem_d, uint64_t adesc, uin
       "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
       : "memory");
 }
+// descriptors as 32-bit halves (constant high half, low half = base + k * step): few integer instructions
+// per MMA for the issuing lane (see chain_umma.cu)
+__device__ __forceinline__ void tc_mma_lh(uint32_t tmem_d, uint32_t a_lo, uint32_t b_lo, uint32_t desc_hi,
+                                          uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t"
+      ".reg .pred p;\n\t"
+      ".reg .b64 da, db;\n\t"
+      "setp.ne.b32 p, %5, 0;\n\t"
+      "mov.b64 da, {%1, %3};\n\t"
+      "mov.b64 db, {%2, %3};\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], da, db, %4, p;\n\t"
+      "}\n" ::"r"(tmem_d),
+      "r"(a_lo), "r"(b_lo), "r"(desc_hi), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+__device__ __forceinline__ bool elect_one() {
+  uint32_t p;
+  asm volatile(
+      "{\n\t"
+      ".reg .pred P;\n\t"
+      "elect.sync _|P, 0xffffffff;\n\t"
+      "selp.u32 %0, 1, 0, P;\n\t"
+      "}\n"
+      : "=r"(p));
+  return p != 0;
+}
 __device__ __forceinline__ void tc_ld32(uint32_t taddr, uint32_t (&v)[32]) {
   asm volatile(
       "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
@@ -335,7 +362,10 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain_mcast(const PairArgs args
     }
   } else if (warp == 1) {
     // ===================== MMA issuer (each CTA for its own tile) =====================
-    if (lane == 0) {
+    {   // whole warp, uniform control flow; one elected lane issues (see chain_umma.cu)
+      const bool one = elect_one();
+      const uint32_t smem_base = smem_u32(smem);
+      constexpr uint32_t kDescHi = (1024u >> 4) | (1u << 14) | (2u << 29);
 #ifdef NOLSM_TRACE
       int mti = 0;
 #endif
@@ -344,7 +374,8 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain_mcast(const PairArgs args
       for (;;) {
         mbar_wait(&cmd_full[slot], ring_phase);
         const TileCmd c = cmds[slot];
-        mbar_arrive_cluster(mapa(smem_u32(&cmd_empty[slot]), 0));
+        __syncwarp();
+        if (one) mbar_arrive_cluster(mapa(smem_u32(&cmd_empty[slot]), 0));
         if (++slot == kRing) { slot = 0; ring_phase ^= 1u; }
         if (c.op < 0) break;
         const bool split = pg.ops[c.op].a_lo[c.iter & 1] >= 0;
@@ -373,24 +404,33 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain_mcast(const PairArgs args
           if (kb == 0) t_first = clock64() - w0;
 #endif
           tc_fence_after();
-          const uint32_t sa = smem_u32(smem + (size_t)stage * args.stage_bytes);
+          const uint32_t sa = smem_base + (uint32_t)stage * (uint32_t)args.stage_bytes;
+          const uint32_t a_lo = ((sa >> 4) & 0x3FFFu) | ((uint32_t)(kBoxBytes >> 4) << 16);
+          const uint32_t b_lo = (((sa + off_b) >> 4) & 0x3FFFu) | (1u << 16);
           const int steps = phantom ? 0 : (kb == c.kblocks - 1 ? c.ktail : kBK / 16);
-          for (int k4 = 0; k4 < steps; ++k4) {
-            const uint64_t ad = make_smem_desc(sa + k4 * 2048, kBoxBytes, 1024);
-            const uint64_t bd = make_smem_desc(sa + off_b + k4 * 32, 16, 1024);
-            const uint32_t accum = (kb | k4) ? 1u : 0u;
-            tc_mma2_f16(d_main, ad, bd, idesc, accum);
-            if (split) {
-              const uint64_t adl = make_smem_desc(sa + off_a_lo + k4 * 2048, kBoxBytes, 1024);
-              const uint64_t bdl = make_smem_desc(sa + off_b_lo + k4 * 32, 16, 1024);
-              tc_mma2_f16(d_corr, ad, bdl, idesc, accum);
-              tc_mma2_f16(d_corr, adl, bd, idesc, 1u);
+          if (one) {
+            if (!split) {
+              if (steps > 0) tc_mma_lh(d_main, a_lo, b_lo, kDescHi, idesc, kb ? 1u : 0u);
+              if (steps > 1) tc_mma_lh(d_main, a_lo + 128u, b_lo + 2u, kDescHi, idesc, 1u);
+              if (steps > 2) tc_mma_lh(d_main, a_lo + 256u, b_lo + 4u, kDescHi, idesc, 1u);
+              if (steps > 3) tc_mma_lh(d_main, a_lo + 384u, b_lo + 6u, kDescHi, idesc, 1u);
+            } else {
+              const uint32_t al_lo = (((sa + off_a_lo) >> 4) & 0x3FFFu) | ((uint32_t)(kBoxBytes >> 4) << 16);
+              const uint32_t bl_lo = (((sa + off_b_lo) >> 4) & 0x3FFFu) | (1u << 16);
+              for (int k4 = 0; k4 < steps; ++k4) {
+                const uint32_t accum = (kb | k4) ? 1u : 0u;
+                tc_mma_lh(d_main, a_lo + 128u * k4, b_lo + 2u * k4, kDescHi, idesc, accum);
+                tc_mma_lh(d_corr, a_lo + 128u * k4, bl_lo + 2u * k4, kDescHi, idesc, accum);
+                tc_mma_lh(d_corr, al_lo + 128u * k4, b_lo + 2u * k4, kDescHi, idesc, 1u);
+              }
             }
+            tc_commit_both(&empty_bar[stage]);
           }
-          tc_commit_both(&empty_bar[stage]);
+          __syncwarp();
           if (++stage == args.stages) { stage = 0; phase ^= 1u; }
         }
-        tc_commit(&tfull_bar[acc]);
+        if (one) tc_commit(&tfull_bar[acc]);
+        __syncwarp();
 #ifdef NOLSM_TRACE
         if (blockIdx.x == 0 && mti - 1 < 4096) { g_mwait[mti - 1][0] = wsum; g_mwait[mti - 1][1] = t_first; g_mwait[mti - 1][2] = clock64() - t_begin; }
 #endif
