@@ -209,7 +209,8 @@ def run_native(args, system, rank, world, local_rank):
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     precision = WORKLOADS[args.workload][0] if args.precision < 0 else args.precision
-    cfg = nolsm.Config(precision=precision, workspace_bytes=int(args.workspace_gib * (1 << 30)))
+    cfg = nolsm.Config(precision=precision, workspace_bytes=int(args.workspace_gib * (1 << 30)), group=args.group,
+                       flags=args.flags)
     ctx = nolsm.Context(cfg)
     dev = torch.device("cuda", local_rank)
     pos = torch.as_tensor(system.pos_q).to(dev)
@@ -299,6 +300,7 @@ def run_native(args, system, rank, world, local_rank):
                    "cutoff_A": system.cutoff, "mu": MU, "seed": system.seed, "nnz_blocks": system.nnzb,
                    "mean_submatrix_dim": 6.0 * system.nnzb / system.n_mol, "tol": 1e-2 if precision == 0 else 1e-5,
                    "workspace_gib": args.workspace_gib, "batches": st.n_batches, "replicas": world,
+                   "group": args.group, "engine_flags": args.flags,
                    "l2": "inputs larger than L2 (block stores 3 x %.0f MB, dense workspace %.0f GiB)" %
                          (system.nnzb * 144 / 1e6, args.workspace_gib)},
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
@@ -337,6 +339,8 @@ def main():
     ap.add_argument("--workload", default="w32768", choices=sorted(WORKLOADS))
     ap.add_argument("--precision", type=int, default=-1, help="0 = FP16/FP32, 1 = FP32 (default: the workload's)")
     ap.add_argument("--workspace-gib", type=float, default=24.0)
+    ap.add_argument("--group", type=int, default=0, help="submatrices iterated together (0: from the L2 size)")
+    ap.add_argument("--flags", type=int, default=0, help="NOLSM_FLAG_* bits (2: pair engine, 4: multicast engine)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()

@@ -367,12 +367,14 @@ static bool use_simt(const nolsm_ctx *ctx) { return (ctx->cfg.flags & NOLSM_FLAG
 
 static int group_size(const nolsm_ctx *ctx, const nolsm_batch *b, int bytes_per_elem) {
   if (ctx->cfg.group > 0) return ctx->cfg.group;
-  // iterates of one group must stay in L2 over a whole iteration, yet a
-  // group must hold a few waves of tiles so that dependent products are far apart in the schedule
+  // Two pulls: the iterates of a group should stay in L2 over an iteration,
+  // and dependent products must be far apart in the claim order, or CTAs idle on the dependency flags.
+  // Measured on w32768 (bench.py --group): 8 -> 582, 14 -> 652, 24 -> 698, 40 -> 703, 96 -> 697 TFLOP/s:
+  // the distance matters more than the residency, so a group holds at least eight waves of tiles.
   const double per = (double)bytes_per_elem * b->ld * b->ld;
   int g = (int)(0.75 * (double)ctx->l2_bytes / per);
   const int tiles = std::max(1, ((b->max_n + 127) / 128) * ((b->max_n + 255) / 256));
-  const int g_min = (3 * ctx->sm_count + tiles - 1) / tiles;
+  const int g_min = (8 * ctx->sm_count + tiles - 1) / tiles;
   g = std::max(g, g_min);
   return std::max(1, std::min(g, 1024));
 }
