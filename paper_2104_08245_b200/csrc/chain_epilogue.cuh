@@ -6,7 +6,7 @@
 // and writes the FP32 result and the FP16 operand copies (hi [, lo * 2^11]) with coalesced stores: the
 // lanes of a warp hold consecutive rows, so every store instruction writes one contiguous 128-byte
 // (FP32) or 64-byte (FP16) segment of a column.  Measured store rate of an SM into L2 with this
-// pattern: ~29 B/clk (FP32), ~20 B/clk (FP16) -- the floor of the epilogue (profiles/r1_k_chain_notes.md).
+// pattern: ~29 B/clk (FP32), ~20 B/clk (FP16) -- the floor of the epilogue (profiles/r1_k_chain_sign_w32768.md).
 //
 // Completion protocol (per submatrix and op): after the stores of a tile the epilogue warps of the
 // CTA meet at a named barrier and ONE elected thread makes them visible (__threadfence) and adds 1 to
@@ -42,8 +42,7 @@ struct TileCmd {              // scheduler -> TMA producer(s), MMA issuer and ep
 
 struct ChainArgs {
   ChainProgram prog;
-  const CUtensorMap *maps;    // [n_half] FP16 load maps {64,64} swizzle-128B, [n_unit] FP32 maps {32,32},
-                              // [n_half] FP16 store maps {32,32} no swizzle
+  const CUtensorMap *maps;    // [n_half] TMA maps of the FP16 operand buffers ({64,64} boxes, 128-byte swizzle)
   __half *hbuf[NOLSM_MAX_HALF];
   float *ubuf[NOLSM_MAX_UNIT];
   int32_t n_half, n_unit;
@@ -72,15 +71,6 @@ __device__ __forceinline__ void ld_tmem32(uint32_t taddr, uint32_t (&v)[32]) {
       : "r"(taddr));
 }
 __device__ __forceinline__ void ld_tmem_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
-__device__ __forceinline__ void tma_store_3d(const CUtensorMap *map, const void *src, int c0, int c1, int c2) {
-  asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.tile.bulk_group [%0, {%2, %3, %4}], [%1];" ::"l"(
-                   reinterpret_cast<uint64_t>(map)),
-               "r"(s32(src)), "r"(c0), "r"(c1), "r"(c2)
-               : "memory");
-}
-__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
-__device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
-__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 __device__ __forceinline__ void st_release_gpu(int32_t *p, int32_t v) {
   asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }

@@ -6,14 +6,16 @@
 // Why one kernel: the two products of a sign iteration are strictly dependent and one product of an
 // n ~ 860 submatrix is < 1 us of the whole GPU, so kernel boundaries would cost more than the work, and
 // a batch-wide launch per product streams every iterate through HBM (18 n^2 bytes per 4 n^3 FLOP,
-// DESIGN.md "Roofline").  Here the submatrices are walked in GROUPS small enough that the iterates of
-// a group stay in the 126 MB L2 for all of its iterations (the B200 analogue of the paper's "caching
-// strategy for the matrices during the iterations"), and the products inside a group
-// are ordered  iteration -> op -> submatrix -> tile  so that by the time a CTA reaches a tile of op
-// s of a submatrix, op s-1 of that submatrix finished several waves ago.  The dependency itself is
-// enforced by a per-submatrix counter in global memory (ready[m] = ops completed, acquire/release at
-// GPU scope), not by a grid barrier; every tile only ever waits for tiles that come earlier in the
-// common order, and all CTAs are co-resident (cooperative launch), so the schedule cannot deadlock.
+// DESIGN.md "Roofline").  The submatrices are walked in GROUPS, each iterated to convergence before the
+// next is touched (the B200 analogue of the paper's "caching strategy for the matrices during the
+// iterations"; DESIGN.md section 5.1 on how the group size trades L2 residency against
+// the distance between dependent products), and the products inside a group are ordered
+// iteration -> op -> submatrix -> tile  so that by the time a CTA reaches a tile of op s of a submatrix,
+// op s-1 of that submatrix finished several waves ago.  CTAs claim tile indices in that order with one
+// atomicAdd per tile.  The dependency itself is enforced by a per-submatrix counter in global memory
+// (ready[m] = ops completed, acquire/release at GPU scope), not by a grid barrier; a tile only ever
+// waits for tiles with a smaller index, all of which have been claimed by running CTAs, and all CTAs
+// are co-resident (cooperative launch), so the schedule cannot deadlock.
 //
 // Layout facts:
 //   * all matrices are column-major, so the A operand (M x K) is M-major and the B operand (K x N) is
@@ -25,8 +27,9 @@
 //   * the FP32 master iterate (reading 12) is read in the epilogue with L2-only loads
 //     (ld.global.cg: other SMs wrote it) issued one chunk ahead, and written back with coalesced stores.
 //
-// Warp roles (352 threads): warp 0 = scheduler (resolves the next tiles and their dependencies, up to
-// kRing tiles ahead), warp 1 = MMA issuer (+ TMEM allocation), warp 2 = TMA producer, warps 3..10 =
+// Warp roles (352 threads): warp 0 = scheduler (claims the next tiles and resolves their dependencies, up
+// to kRing tiles ahead), warp 1 = MMA issuer (whole warp, one elected lane issues; + TMEM allocation),
+// warp 2 = TMA producer, warps 3..10 =
 // epilogue (TMEM lane quadrant = warp_id % 4; the two warps of a quadrant take alternate 32-column
 // chunks of the tile).
 #include "common.cuh"
@@ -71,19 +74,6 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
       "r"(parity)
       : "memory");
 }
-__device__ __forceinline__ bool mbar_test(uint64_t *bar, uint32_t parity) {
-  uint32_t ok;
-  asm volatile(
-      "{\n\t"
-      ".reg .pred p;\n\t"
-      "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
-      "selp.b32 %0, 1, 0, p;\n\t"
-      "}\n"
-      : "=r"(ok)
-      : "r"(smem_u32(bar)), "r"(parity)
-      : "memory");
-  return ok != 0;
-}
 __device__ __forceinline__ void tma_load_3d(void *dst, const CUtensorMap *map, uint64_t *bar, int c0,
                                             int c1, int c2) {
   asm volatile(
@@ -112,17 +102,6 @@ __device__ __forceinline__ void tc_commit(uint64_t *bar) {
                    smem_u32(bar))
                : "memory");
 }
-__device__ __forceinline__ void tc_mma_f16(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc,
-                                           uint32_t accumulate) {
-  asm volatile(
-      "{\n\t"
-      ".reg .pred p;\n\t"
-      "setp.ne.b32 p, %4, 0;\n\t"
-      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t"
-      "}\n" ::"r"(tmem_d),
-      "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
-      : "memory");
-}
 // Same with the descriptors given as 32-bit halves: the high half (stride offset, version, swizzle) is a
 // constant, the low half is base + k * step, so the single issuing thread spends a handful of integer
 // instructions per MMA instead of rebuilding two 64-bit descriptors (it was issue-bound at ~200 cycles
@@ -141,62 +120,11 @@ __device__ __forceinline__ void tc_mma_f16_lh(uint32_t tmem_d, uint32_t a_lo, ui
       "r"(a_lo), "r"(b_lo), "r"(desc_hi), "r"(idesc), "r"(accumulate)
       : "memory");
 }
-__device__ __forceinline__ void tc_ld32(uint32_t taddr, uint32_t (&v)[32]) {
-  asm volatile(
-      "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
-      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, %17, %18, %19, %20, %21, "
-      "%22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
-      : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
-        "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]),
-        "=r"(v[15]), "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]),
-        "=r"(v[22]), "=r"(v[23]), "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]),
-        "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
-      : "r"(taddr));
-}
-__device__ __forceinline__ void tc_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ int32_t ld_acquire(const int32_t *p) {
   int32_t v;
   asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
   return v;
 }
-__device__ __forceinline__ void st_release(int32_t *p, int32_t v) {
-  asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
-}
-
-// Shared-memory matrix descriptor (tcgen05): start address, leading / stride byte offsets (all >> 4),
-// descriptor version 1, 128-byte swizzle.
-__device__ __forceinline__ uint64_t make_smem_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
-  uint64_t d = 0;
-  d |= (uint64_t)((saddr & 0x3FFFF) >> 4);
-  d |= (uint64_t)((lbo_bytes >> 4) & 0x3FFF) << 16;
-  d |= (uint64_t)((sbo_bytes >> 4) & 0x3FFF) << 32;
-  d |= (uint64_t)1 << 46;   // version
-  d |= (uint64_t)2 << 61;   // SWIZZLE_128B
-  return d;
-}
-
-// Stores `cnt` (16 or 32) consecutive tile columns of one row held in v[]: FP32 master and / or FP16
-// operand copies (hi [, lo * 2^11]).  Column stride = ld elements; lanes hold consecutive rows, so
-// every store instruction of a warp writes one contiguous 128-byte (FP32) or 64-byte (FP16) segment.
-template <bool H32, bool H16, bool HLO>
-__device__ __forceinline__ void store_cols(const uint32_t (&v)[32], float *p32, __half *p16, __half *p16l, int ld,
-                                           bool full) {
-#pragma unroll
-  for (int half = 0; half < 2; ++half) {
-    if (half == 1 && !full) break;
-#pragma unroll
-    for (int jj = 0; jj < 16; ++jj) {
-      const float val = __uint_as_float(v[half * 16 + jj]);
-      if (H32) { *p32 = val; p32 += ld; }
-      if (H16) {
-        const __half hi = __float2half_rn(val);
-        *p16 = hi; p16 += ld;
-        if (HLO) { *p16l = __float2half_rn((val - __half2float(hi)) * 2048.f); p16l += ld; }
-      }
-    }
-  }
-}
-
 #ifdef NOLSM_TRACE
 __device__ long long g_trace[4][4096][2];
 #define TRACE(role, ti, j) do { if (blockIdx.x == 0 && (ti) < 4096) g_trace[role][ti][j] = clock64(); } while (0)
@@ -516,18 +444,16 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t
                                   CUtensorMapFloatOOBfill);
 
 // stored matrix: dim0 = row index (contiguous), dim1 = column index, dim2 = submatrix
-// operand: FP16 {64,64} box with 128-byte swizzle (TMA loads of the MMA operands); otherwise a plain
-// {32,32} box (FP32 units; FP16 store maps of the epilogue)
-nolsm_status encode_map(nolsm_ctx *ctx, CUtensorMap *map, void *ptr, bool half, bool operand, int ld, int count) {
-  const size_t es = half ? sizeof(__half) : sizeof(float);
+// FP16 operand buffer: {64 storage rows, 64 storage columns} box with 128-byte swizzle, one map serving
+// both operand roles (see the header comment)
+nolsm_status encode_map(nolsm_ctx *ctx, CUtensorMap *map, void *ptr, int ld, int count) {
   cuuint64_t dims[3] = {(cuuint64_t)ld, (cuuint64_t)ld, (cuuint64_t)count};
-  cuuint64_t strides[2] = {(cuuint64_t)ld * es, (cuuint64_t)ld * ld * es};
-  cuuint32_t box[3] = {operand ? 64u : 32u, operand ? 64u : 32u, 1};
+  cuuint64_t strides[2] = {(cuuint64_t)ld * sizeof(__half), (cuuint64_t)ld * ld * sizeof(__half)};
+  cuuint32_t box[3] = {64u, 64u, 1};
   cuuint32_t estr[3] = {1, 1, 1};
   CUresult r = reinterpret_cast<EncodeTiledFn>(ctx->encode_tiled)(
-      map, half ? CU_TENSOR_MAP_DATA_TYPE_FLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, ptr, dims, strides, box,
-      estr, CU_TENSOR_MAP_INTERLEAVE_NONE, operand ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE,
-      CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+      map, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 3, ptr, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+      CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) {
     ctx->err = "cuTensorMapEncodeTiled failed with CUresult " + std::to_string((int)r);
     return NOLSM_ECUDA;
@@ -578,19 +504,13 @@ nolsm_status umma_init(nolsm_ctx *ctx) {
 nolsm_status umma_make_maps(nolsm_ctx *ctx, nolsm_batch *b) {
   b->maps_valid = false;
   if (!ctx->umma_ok || b->count == 0) return NOLSM_OK;
-  std::vector<CUtensorMap> maps(2 * b->n_half + b->n_unit);
+  std::vector<CUtensorMap> maps(b->n_half);
   for (int i = 0; i < b->n_half; ++i) {
-    nolsm_status s = encode_map(ctx, &maps[i], b->h[i], true, true, b->ld, b->count);
-    if (s != NOLSM_OK) return s;
-    s = encode_map(ctx, &maps[b->n_half + b->n_unit + i], b->h[i], true, false, b->ld, b->count);
-    if (s != NOLSM_OK) return s;
-  }
-  for (int i = 0; i < b->n_unit; ++i) {
-    nolsm_status s = encode_map(ctx, &maps[b->n_half + i], b->u[i], false, false, b->ld, b->count);
+    nolsm_status s = encode_map(ctx, &maps[i], b->h[i], b->ld, b->count);
     if (s != NOLSM_OK) return s;
   }
   if (!b->d_maps) {
-    if (cudaMalloc(&b->d_maps, sizeof(CUtensorMap) * (2 * NOLSM_MAX_HALF + NOLSM_MAX_UNIT)) != cudaSuccess) {
+    if (cudaMalloc(&b->d_maps, sizeof(CUtensorMap) * NOLSM_MAX_HALF) != cudaSuccess) {
       cudaGetLastError();
       ctx->err = "cudaMalloc of the tensor maps failed";
       return NOLSM_ENOMEM;
