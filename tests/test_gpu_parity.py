@@ -576,3 +576,23 @@ def test_w32768_whole_step_in_bench_configuration_sampled(nolsm):
     assert abs(ne - system.n_electrons) / n_mol < 1e-3
     assert np.isfinite(d).all()
     ctx.close()
+
+
+@pytest.mark.parametrize("flag", [0, "FLAG_PAIR", "FLAG_MCAST"])
+def test_run_to_run_bitwise_identical(nolsm, flag):
+    """The tile schedule is dynamic (claim order and timing differ from run to run) but every tile's arithmetic
+    is fixed, so two runs must give bit-identical D: any race in the dependency protocol (a tile reading an
+    operand before its producer finished) would show up here."""
+    import torch
+    import nolsm_inputs as gi
+    system = gi.make_water_system(*gi.CONFIGS["w4096"])
+    H, S = _device_system(nolsm, system)
+    flags = getattr(nolsm, flag) if flag else 0
+    runs = []
+    for _ in range(2):
+        ctx = nolsm.Context(nolsm.Config(precision=0, flags=flags))
+        mu, ne, D, st = ctx.solve_mu(H, S, system.n_electrons, 2 * MU, 0.0, tol_ne_per_mol=-1.0, max_steps=1)
+        runs.append((D.val.clone(), ne))
+        ctx.close()
+    assert torch.equal(runs[0][0], runs[1][0])
+    assert abs(runs[0][1] - runs[1][1]) < 1e-6
