@@ -217,6 +217,9 @@ def run_native(args, system, rank, world, local_rank):
     h_val = torch.as_tensor(system.h_val).to(dev)
     s_val = torch.as_tensor(system.s_val).to(dev)
     mu_lo, mu_hi = 2 * MU, 0.0        # one evaluation at the midpoint mu = -0.85
+    if args.elements == "generated":   # T_j(H), T_j(S) evaluated on the device from the positions
+        import nolsm_inputs as gi
+        ctx.set_model(pos, **gi.model_parameters(system))
 
     def step():
         rp, ci = ctx.build_neighbours(pos, system.box_q, system.rc_q, cap=system.nnzb)
@@ -300,7 +303,7 @@ def run_native(args, system, rank, world, local_rank):
                    "cutoff_A": system.cutoff, "mu": MU, "seed": system.seed, "nnz_blocks": system.nnzb,
                    "mean_submatrix_dim": 6.0 * system.nnzb / system.n_mol, "tol": 1e-2 if precision == 0 else 1e-5,
                    "workspace_gib": args.workspace_gib, "batches": st.n_batches, "replicas": world,
-                   "group": args.group, "engine_flags": args.flags,
+                   "group": args.group, "engine_flags": args.flags, "elements": args.elements,
                    "l2": "inputs larger than L2 (block stores 3 x %.0f MB, dense workspace %.0f GiB)" %
                          (system.nnzb * 144 / 1e6, args.workspace_gib)},
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
@@ -341,6 +344,9 @@ def main():
     ap.add_argument("--workspace-gib", type=float, default=24.0)
     ap.add_argument("--group", type=int, default=0, help="submatrices iterated together (0: from the L2 size)")
     ap.add_argument("--flags", type=int, default=0, help="NOLSM_FLAG_* bits (2: pair engine, 4: multicast engine)")
+    ap.add_argument("--elements", default="gathered", choices=["gathered", "generated"],
+                    help="submatrix elements gathered from the block stores (the north_star path) or evaluated "
+                         "on the device from the positions (nolsm_set_model)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()

@@ -3,6 +3,7 @@
  * The path (PAPER.md = the paper text; DESIGN.md lists every reading taken):
  *   a0  neighbour lists / index sets            Fig. 2 b,c  PAPER.md:172,190; merged pattern :158
  *   a1  dense submatrices T_j(H), T_j(S)        step (i)    PAPER.md:140; NOLSM :158
+ *   a1' the same from positions + a model     Fig. 2 d,e  PAPER.md:172,202 (nolsm_set_model)
  *   a2  S_j^-1 by the coupled Newton-Schulz     Eq. 15-17
  *   a3  B_j = S_j^-1 H_j, X0 = (B_j - mu I)/s   Eq. 12      PAPER.md:160; rescaling :138
  *   a4  sign iteration X <- 1/2 X (3I - X^2)    Eq. 9-10
@@ -133,6 +134,39 @@ nolsm_status nolsm_build_neighbours(nolsm_ctx *ctx, int32_t n_mol, const int32_t
 nolsm_status nolsm_build_submatrices(nolsm_ctx *ctx, const nolsm_bsr *H, const nolsm_bsr *S,
                                      int32_t mol_begin, int32_t mol_count, int32_t slot,
                                      nolsm_batch **out, void *stream);
+/* a1', SURVEY 8(f)#2 (Fig. 2 d-e: "the matrix elements of the submatrices are
+ * generated on the accelerator, only the index metadata crosses"): a two-centre model from which the
+ * elements of T_j(H), T_j(S) are evaluated on the device instead of being gathered from the block
+ * stores.  Molecule i has n_site = 3 sites at pos_i + site_offset[s]; basis function o sits on site
+ * orb_site[o].  For a stored pair (ia, ib) (centre distance <= rc_q, integer minimum image as in
+ * nolsm_build_neighbours) and functions o on ia, p on ib:
+ *   d   = ((pos_ia - pos_ib) * unit_per_grid + site_offset[orb_site[o]]) - site_offset[orb_site[p]],
+ *         then per axis d -= L * rint(d / L), L = box_q * unit_per_grid;   r2 = (dx^2 + dy^2) + dz^2
+ *   S   = s_ampl * exp(-0.5 * r2),   H = h_ampl * exp(-sqrt(r2) / h_len)
+ *   ia == ib: o == p -> S = 1, H = orb_energy[o];  o != p on the same site -> S = H = 0.
+ * Everything above is evaluated in FP64 with separately rounded operations in exactly that order and
+ * the result rounded once to FP32 (so it can differ from a host evaluation only through exp()'s last
+ * bit).  Pairs that are not stored give 0, padding is the identity, as in nolsm_build_submatrices. */
+typedef struct {
+  const int32_t *pos_q;      /* device [n_mol*3], grid units in [0, box_q) */
+  int32_t n_mol;
+  int32_t box_q[3];          /* each even */
+  int32_t rc_q;
+  double unit_per_grid;      /* length of one grid step */
+  double site_offset[3][3];  /* [site][axis] */
+  int32_t orb_site[6];       /* each in 0..2 */
+  double orb_energy[6];
+  double s_ampl, h_ampl, h_len;
+} nolsm_model;
+
+/* Attach (model != NULL; the struct is copied, pos_q stays caller-owned and must outlive its use) or
+ * detach (NULL) a model.  While one is attached, every submatrix build of this context --
+ * nolsm_build_submatrices and the builds inside nolsm_solve_mu / nolsm_evaluate -- evaluates the model
+ * instead of reading H->val and S->val (the pattern arrays are still read; the traces of a6/a7 still
+ * read the block stores).  NOLSM_EINVAL for a null pos_q, odd or non-positive box, orb_site out of
+ * range, or n_mol different from the matrices' at build time. */
+nolsm_status nolsm_set_model(nolsm_ctx *ctx, const nolsm_model *model /*host*/);
+
 /* How many molecules starting at mol_begin fit in one batch given the workspace bound (host logic;
  * needs row_ptr on the device, synchronises).  Returns the count (>= 0) or -status. */
 int32_t nolsm_batch_capacity(nolsm_ctx *ctx, const nolsm_bsr *H, int32_t mol_begin, int32_t n_slots,

@@ -7,11 +7,11 @@ The recipe is the one stated in BASELINE.json:configs and completed in DESIGN.md
 """
 from .rng import splitmix64, uniform_u53
 from .water import (GRID_PER_ANGSTROM, BS, N_OCC_PER_MOL, N_ELEC_PER_MOL, WaterSystem,
-                    make_positions, make_water_system, CONFIGS)
+                    make_positions, make_water_system, model_parameters, CONFIGS)
 from .dense import make_gapped_symmetric, microbench_batch
 
 __all__ = [
     "splitmix64", "uniform_u53", "GRID_PER_ANGSTROM", "BS", "N_OCC_PER_MOL", "N_ELEC_PER_MOL",
-    "WaterSystem", "make_positions", "make_water_system", "CONFIGS", "make_gapped_symmetric",
+    "WaterSystem", "make_positions", "make_water_system", "model_parameters", "CONFIGS", "make_gapped_symmetric",
     "microbench_batch",
 ]

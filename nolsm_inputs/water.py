@@ -173,6 +173,15 @@ def make_water_system(n_mol, cutoff, seed=DEFAULT_SEED):
                        n_electrons=float(N_ELEC_PER_MOL * n_mol))
 
 
+def model_parameters(system):
+    """The constants of the element model above (the recipe of `_blocks`), for consumers that evaluate
+    the elements themselves (nolsm.h: nolsm_model).  Values only; the positions stay in `system`."""
+    return dict(box_q=[int(x) for x in system.box_q], rc_q=int(system.rc_q),
+                unit_per_grid=1.0 / GRID_PER_ANGSTROM, site_offset=SITE_OFFSETS.tolist(),
+                orb_site=ORB_SITE.tolist(), orb_energy=ORB_ENERGY.tolist(),
+                s_ampl=S_AMPL, h_ampl=H_AMPL, h_len=H_LEN)
+
+
 def to_dense(system, which):
     """Assemble the full (6 n_mol)^2 FP64 matrix from the block store (tests only; small systems)."""
     val = system.h_val if which == "H" else system.s_val

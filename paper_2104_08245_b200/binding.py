@@ -18,7 +18,7 @@ EXPORTED_SYMBOLS = [
     "nolsm_build_submatrices", "nolsm_batch_capacity", "nolsm_release_batch", "nolsm_sign_batched",
     "nolsm_scatter_density", "nolsm_solve_mu", "nolsm_solve_mu_host", "nolsm_sign_dense_batched", "nolsm_batch_read",
     "nolsm_batch_size", "nolsm_batch_ld", "nolsm_gemm_batched", "nolsm_launch_count",
-    "nolsm_scatter_energy", "nolsm_evaluate",
+    "nolsm_scatter_energy", "nolsm_evaluate", "nolsm_set_model",
 ]
 
 
@@ -42,6 +42,13 @@ class Config(C.Structure):
 class _Bsr(C.Structure):
     _fields_ = [("n_mol", C.c_int32), ("bs", C.c_int32), ("row_ptr", C.c_void_p), ("col_idx", C.c_void_p),
                 ("val", C.c_void_p)]
+
+
+class _Model(C.Structure):
+    _fields_ = [("pos_q", C.c_void_p), ("n_mol", C.c_int32), ("box_q", C.c_int32 * 3), ("rc_q", C.c_int32),
+                ("unit_per_grid", C.c_double), ("site_offset", (C.c_double * 3) * 3), ("orb_site", C.c_int32 * 6),
+                ("orb_energy", C.c_double * 6), ("s_ampl", C.c_double), ("h_ampl", C.c_double),
+                ("h_len", C.c_double)]
 
 
 class SignStats(C.Structure):
@@ -97,6 +104,8 @@ def load_library():
     lib.nolsm_launch_count.restype = i64
     lib.nolsm_build_neighbours.argtypes = [vp, i32, vp, P(i32), i32, vp, vp, i64, P(i64), vp]
     lib.nolsm_build_neighbours.restype = i32
+    lib.nolsm_set_model.argtypes = [vp, P(_Model)]
+    lib.nolsm_set_model.restype = i32
     lib.nolsm_build_submatrices.argtypes = [vp, P(_Bsr), P(_Bsr), i32, i32, i32, P(vp), vp]
     lib.nolsm_build_submatrices.restype = i32
     lib.nolsm_batch_capacity.argtypes = [vp, P(_Bsr), i32, i32, vp]
@@ -260,6 +269,32 @@ class Context:
                                                     _ptr(row_ptr), _ptr(col_idx), cap, C.byref(nnzb),
                                                     _stream(stream)))
         return row_ptr, col_idx[: nnzb.value]
+
+    # a1' ----------------------------------------------------------------------------------------
+    def set_model(self, pos_q=None, box_q=None, rc_q=0, unit_per_grid=1.0, site_offset=None, orb_site=None,
+                  orb_energy=None, s_ampl=0.0, h_ampl=0.0, h_len=1.0):
+        """Attach the two-centre model of nolsm.h (nolsm_model): submatrix builds then evaluate the elements
+        from pos_q (int32 CUDA tensor [n_mol,3], kept alive here) instead of gathering.  pos_q=None detaches."""
+        if pos_q is None:
+            self._model_pos = None
+            self._check(self.lib.nolsm_set_model(self.handle, None))
+            return
+        torch = _torch()
+        m = _Model()
+        m.pos_q = _ptr(pos_q, torch.int32)
+        m.n_mol = int(pos_q.shape[0])
+        m.rc_q = int(rc_q)
+        m.unit_per_grid = float(unit_per_grid)
+        for i in range(3):
+            m.box_q[i] = int(box_q[i])
+            for k in range(3):
+                m.site_offset[i][k] = float(site_offset[i][k])
+        for o in range(6):
+            m.orb_site[o] = int(orb_site[o])
+            m.orb_energy[o] = float(orb_energy[o])
+        m.s_ampl, m.h_ampl, m.h_len = float(s_ampl), float(h_ampl), float(h_len)
+        self._check(self.lib.nolsm_set_model(self.handle, C.byref(m)))
+        self._model_pos = pos_q
 
     # a1 -----------------------------------------------------------------------------------------
     def build_submatrices(self, H, S, mol_begin, mol_count, slot=0, stream=None):

@@ -328,6 +328,23 @@ extern "C" int32_t nolsm_batch_capacity(nolsm_ctx *ctx, const nolsm_bsr *H, int3
   return count;
 }
 
+extern "C" nolsm_status nolsm_set_model(nolsm_ctx *ctx, const nolsm_model *model) {
+  if (!ctx) return NOLSM_EINVAL;
+  if (!model) { ctx->has_model = false; return NOLSM_OK; }
+  if (!model->pos_q || model->n_mol <= 0 || model->rc_q < 0 || !(model->unit_per_grid > 0.0) ||
+      !(model->h_len > 0.0)) {
+    ctx->err = "model: null positions, empty system, negative cutoff or non-positive length scale";
+    return NOLSM_EINVAL;
+  }
+  for (int i = 0; i < 3; ++i)
+    if (model->box_q[i] <= 0 || (model->box_q[i] & 1)) { ctx->err = "model: box_q must be positive and even"; return NOLSM_EINVAL; }
+  for (int o = 0; o < NOLSM_BS; ++o)
+    if (model->orb_site[o] < 0 || model->orb_site[o] > 2) { ctx->err = "model: orb_site must be 0, 1 or 2"; return NOLSM_EINVAL; }
+  ctx->model = *model;
+  ctx->has_model = true;
+  return NOLSM_OK;
+}
+
 static nolsm_status build_submatrices_impl(nolsm_ctx *ctx, const nolsm_bsr *H, const nolsm_bsr *S,
                                            int32_t mol_begin, int32_t mol_count, int32_t slot, int units,
                                            nolsm_batch **out, void *stream) {
@@ -347,7 +364,15 @@ static nolsm_status build_submatrices_impl(nolsm_ctx *ctx, const nolsm_bsr *H, c
   if (mol_count > 0) CHECK(read_dims(ctx, H->row_ptr, mol_begin, mol_count, dims, st));
   nolsm_batch *b = nullptr;
   CHECK(setup_batch(ctx, slot, dims, mol_begin, true, units, &b, st));
-  LAUNCH(ctx, launch_gather(b, H->row_ptr, H->col_idx, H->val, S->val, b->u[1], b->u[0], st));
+  if (ctx->has_model) {
+    if (ctx->model.n_mol != H->n_mol) {
+      ctx->err = "the attached model has a different number of molecules than the matrices";
+      return NOLSM_EINVAL;
+    }
+    LAUNCH(ctx, launch_generate(b, H->row_ptr, H->col_idx, &ctx->model, b->u[1], b->u[0], st));
+  } else {
+    LAUNCH(ctx, launch_gather(b, H->row_ptr, H->col_idx, H->val, S->val, b->u[1], b->u[0], st));
+  }
   *out = b;
   return NOLSM_OK;
 }

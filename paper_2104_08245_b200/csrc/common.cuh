@@ -131,6 +131,8 @@ struct nolsm_ctx {
   int32_t *m_row_ptr = nullptr, *m_col_idx = nullptr;
   float *m_h = nullptr, *m_s = nullptr, *m_d = nullptr;
   size_t m_cap_mol = 0, m_cap_nnzb = 0;
+  bool has_model = false;         // nolsm_set_model: builds evaluate the model instead of gathering
+  nolsm_model model;
 };
 
 #define NOLSM_CUDA(ctx, call)                                                          \
@@ -151,6 +153,8 @@ cudaError_t launch_neighbour_count(int n_mol, const int32_t *pos, const int32_t 
 cudaError_t launch_exclusive_scan(const int32_t *counts, int32_t *row_ptr, int n, cudaStream_t st);
 cudaError_t launch_neighbour_fill(int n_mol, const int32_t *pos, const int32_t *box, int32_t rc,
                                   const int32_t *row_ptr, int32_t *col_idx, cudaStream_t st);
+cudaError_t launch_generate(const nolsm_batch *b, const int32_t *row_ptr, const int32_t *col_idx,
+                            const nolsm_model *model, float *h_out, float *s_out, cudaStream_t st);
 cudaError_t launch_gather(const nolsm_batch *b, const int32_t *row_ptr, const int32_t *col_idx,
                           const float *h_val, const float *s_val, float *h_out, float *s_out,
                           cudaStream_t st);

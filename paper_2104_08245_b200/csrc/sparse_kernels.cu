@@ -1,4 +1,4 @@
-// a0 neighbour lists, a1 gather, a5/a6 density columns + write-back, a7 block trace.
+// a0 neighbour lists, a1 gather, a1' element generation from positions, a5/a6 density columns + write-back, a7 block trace.
 // All integer work is exact (int64 squared distances on the 2^-16 A grid, reading 2).
 #include "common.cuh"
 
@@ -195,6 +195,137 @@ cudaError_t launch_gather(const nolsm_batch *b, const int32_t *row_ptr, const in
   dim3 grid((cols + GA_WARPS - 1) / GA_WARPS, b->count);
   k_gather<<<grid, GA_WARPS * 32, smem, st>>>(row_ptr, col_idx, h_val, s_val, b->mol_begin, b->ld,
                                               (int64_t)b->ld * b->ld, h_out, s_out);
+  return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------
+// a1' (SURVEY 8(f)#2; Fig. 2 d-e PAPER.md:172, :202): the elements of T_j(H), T_j(S) evaluated from
+// the positions with the two-centre model of nolsm.h (nolsm_model) instead of gathered.  Same shape
+// as the gather: one warp per block-column b.  Phase 1: the lanes evaluate, for every block-row a,
+// the 3 x 3 site-pair values (two exponentials each) in FP64 -- every operation rounded on its own
+// (__dadd_rn/__dmul_rn/...: no contraction into FMAs) in the order nolsm.h states, so the FP32 result
+// differs from a host evaluation only where exp()'s last bit does -- and park them in shared memory as
+// FP32.  Phase 2 fans them out to the 6 x 6 elements and writes the six columns top to bottom, 128
+// contiguous bytes per store instruction.  Whether a pair is stored is the integer minimum-image test
+// of a0, so no CSR row of a neighbour is searched.
+// ------------------------------------------------------------------------------------------------
+struct ModelDev {
+  const int32_t *pos;
+  int32_t box[3];
+  int64_t rc2;
+  double unit, len[3], off[3][3];
+  double s_ampl, h_ampl, h_len;
+  float energy[NOLSM_BS];
+  uint32_t site_packed;  // 2 bits per basis function
+};
+
+__device__ __forceinline__ double wrap_axis(double d, double len) {
+  return __dsub_rn(d, __dmul_rn(len, rint(__ddiv_rn(d, len))));
+}
+
+__global__ void __launch_bounds__(GA_WARPS * 32)
+k_generate(const int32_t *__restrict__ row_ptr, const int32_t *__restrict__ col_idx,
+           const __grid_constant__ ModelDev md, int mol_begin, int ld, int64_t slab, int m_cap,
+           float *__restrict__ h_out, float *__restrict__ s_out) {
+  extern __shared__ float s_gen[];  // [GA_WARPS][2][9 * m_cap]
+  const int mat = blockIdx.y;
+  const int j = mol_begin + mat;
+  const int lo = row_ptr[j];
+  const int m = row_ptr[j + 1] - lo;
+  const int n = m * NOLSM_BS;
+  const int P = (n + NOLSM_TILE_M - 1) / NOLSM_TILE_M * NOLSM_TILE_M;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int m_pad_blocks = (P + NOLSM_BS - 1) / NOLSM_BS;
+  float *sv9 = s_gen + (size_t)warp * 18 * m_cap;
+  float *hv9 = sv9 + 9 * m_cap;
+  float *hj = h_out + (int64_t)mat * slab;
+  float *sj = s_out + (int64_t)mat * slab;
+  for (int b = blockIdx.x * GA_WARPS + warp; b < m_pad_blocks; b += gridDim.x * GA_WARPS) {
+    if (b < m) {
+      const int ib = col_idx[lo + b];
+      const int32_t xb = md.pos[3 * ib], yb = md.pos[3 * ib + 1], zb = md.pos[3 * ib + 2];
+      for (int t = lane; t < 9 * m; t += 32) {
+        const int a = t / 9, q = t - 9 * a;
+        const int so = q / 3, sp = q - 3 * so;  // site of the row function, of the column function
+        const int ia = col_idx[lo + a];
+        const int32_t xa = md.pos[3 * ia], ya = md.pos[3 * ia + 1], za = md.pos[3 * ia + 2];
+        float sv = 0.f, hv = 0.f;
+        const bool stored = min_image_sq(xa, ya, za, xb, yb, zb, md.box[0], md.box[1], md.box[2]) <= md.rc2;
+        if (stored && !(ia == ib && so == sp)) {
+          double dx = __dmul_rn((double)(xa - xb), md.unit);
+          double dy = __dmul_rn((double)(ya - yb), md.unit);
+          double dz = __dmul_rn((double)(za - zb), md.unit);
+          dx = wrap_axis(__dsub_rn(__dadd_rn(dx, md.off[so][0]), md.off[sp][0]), md.len[0]);
+          dy = wrap_axis(__dsub_rn(__dadd_rn(dy, md.off[so][1]), md.off[sp][1]), md.len[1]);
+          dz = wrap_axis(__dsub_rn(__dadd_rn(dz, md.off[so][2]), md.off[sp][2]), md.len[2]);
+          const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+          sv = (float)__dmul_rn(md.s_ampl, exp(__dmul_rn(-0.5, r2)));
+          hv = (float)__dmul_rn(md.h_ampl, exp(__ddiv_rn(-__dsqrt_rn(r2), md.h_len)));
+        }
+        sv9[t] = sv;
+        hv9[t] = hv;
+      }
+    }
+    __syncwarp();
+    for (int p = 0; p < NOLSM_BS; ++p) {
+      const int c = b * NOLSM_BS + p;
+      if (c >= P) break;
+      const int sp = (md.site_packed >> (2 * p)) & 3;
+      float *hc = hj + (int64_t)c * ld;
+      float *sc = sj + (int64_t)c * ld;
+      for (int r = lane; r < P; r += 32) {
+        float hv = 0.f, sv = 0.f;
+        if (c < n && r < n) {
+          const int a = r / NOLSM_BS, o = r - a * NOLSM_BS;
+          if (a == b && o == p) {
+            sv = 1.f;
+            hv = md.energy[o];
+          } else {
+            const int k = a * 9 + ((md.site_packed >> (2 * o)) & 3) * 3 + sp;
+            hv = hv9[k];
+            sv = sv9[k];
+          }
+        } else if (r == c) {
+          sv = 1.f;
+        }
+        hc[r] = hv;
+        sc[r] = sv;
+      }
+    }
+    __syncwarp();
+  }
+}
+
+cudaError_t launch_generate(const nolsm_batch *b, const int32_t *row_ptr, const int32_t *col_idx,
+                            const nolsm_model *model, float *h_out, float *s_out, cudaStream_t st) {
+  if (b->count == 0) return cudaSuccess;
+  ModelDev md;
+  md.pos = model->pos_q;
+  md.rc2 = (int64_t)model->rc_q * model->rc_q;
+  md.unit = model->unit_per_grid;
+  md.site_packed = 0;
+  for (int i = 0; i < 3; ++i) {
+    md.box[i] = model->box_q[i];
+    md.len[i] = (double)model->box_q[i] * model->unit_per_grid;
+    for (int k = 0; k < 3; ++k) md.off[i][k] = model->site_offset[i][k];
+  }
+  for (int o = 0; o < NOLSM_BS; ++o) {
+    md.energy[o] = (float)model->orb_energy[o];
+    md.site_packed |= (uint32_t)model->orb_site[o] << (2 * o);
+  }
+  md.s_ampl = model->s_ampl;
+  md.h_ampl = model->h_ampl;
+  md.h_len = model->h_len;
+  const int m_cap = (b->ld + NOLSM_BS - 1) / NOLSM_BS + 1;
+  const size_t smem = (size_t)GA_WARPS * 18 * m_cap * sizeof(float);
+  if (smem > 48 * 1024) {
+    cudaError_t e = cudaFuncSetAttribute(k_generate, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+  }
+  const int cols = (b->ld + NOLSM_BS - 1) / NOLSM_BS;
+  dim3 grid((cols + GA_WARPS - 1) / GA_WARPS, b->count);
+  k_generate<<<grid, GA_WARPS * 32, smem, st>>>(row_ptr, col_idx, md, b->mol_begin, b->ld,
+                                                (int64_t)b->ld * b->ld, m_cap, h_out, s_out);
   return cudaGetLastError();
 }
 

@@ -596,3 +596,88 @@ def test_run_to_run_bitwise_identical(nolsm, flag):
         ctx.close()
     assert torch.equal(runs[0][0], runs[1][0])
     assert abs(runs[0][1] - runs[1][1]) < 1e-6
+
+
+# ---------------------------------------------------------------------------------------------
+# a1': elements evaluated on the device from the positions instead of gathered
+# ---------------------------------------------------------------------------------------------
+def _attach_model(nolsm, ctx, system):
+    import torch
+    import nolsm_inputs as gi
+    pos = torch.as_tensor(system.pos_q).contiguous().cuda()
+    ctx.set_model(pos, **gi.model_parameters(system))
+    return pos
+
+
+@pytest.mark.parametrize("which", ["tiny", "tiny9", "mid"])
+def test_generated_submatrices_match_block_store(nolsm, tiny_system, mid_system, which):
+    """Same T_j(H), T_j(S) as the oracle's gather of the generator's blocks.  Both sides evaluate the model in
+    FP64 in the same operation order and round once to FP32, so the only admissible difference is exp()'s last
+    FP64 bit crossing an FP32 rounding boundary: at most one FP32 ulp, on at most 1e-5 of the elements.
+    tiny9 (cutoff 9 A > half the 9.86 A box) exercises the per-site minimum image."""
+    import oracle.nolsm_oracle as orc
+    import nolsm_inputs as gi
+    system = {"tiny": tiny_system, "mid": mid_system}.get(which) or gi.make_water_system(32, 9.0)
+    H, S = _device_system(nolsm, system)
+    zeros = nolsm.BlockSparse(H.row_ptr, H.col_idx, H.val * 0)   # the stores must not be read
+    ctx = nolsm.Context()
+    _attach_model(nolsm, ctx, system)
+    count = 24 if which == "mid" else system.n_mol
+    begin = 100 if which == "mid" else 0
+    batch = ctx.build_submatrices(zeros, zeros, begin, count)
+    n_elem = n_diff = 0
+    for local in ([0, 5, count - 1] if which == "mid" else range(count)):
+        j = begin + local
+        nbrs = system.col_idx[system.row_ptr[j]:system.row_ptr[j + 1]]
+        for mat, val in ((nolsm.MAT_H, system.h_val), (nolsm.MAT_S, system.s_val)):
+            ref = orc.dense_submatrix(system.row_ptr, system.col_idx, val, nbrs).astype(np.float32)
+            got = batch.read(local, mat).cpu().numpy()
+            assert got.shape == ref.shape
+            assert np.array_equal(got == 0, ref == 0)              # the pattern is integer work: exact
+            ulp = np.spacing(np.abs(ref))
+            assert (np.abs(got - ref) <= ulp).all()
+            n_elem += ref.size
+            n_diff += int((got.view(np.uint32) != ref.view(np.uint32)).sum())
+    assert n_diff <= max(1, int(1e-5 * n_elem)), (n_diff, n_elem)
+    ctx.set_model(None)                                            # detached: gathers again
+    batch = ctx.build_submatrices(H, S, begin, 1)
+    ref = orc.dense_submatrix(system.row_ptr, system.col_idx, system.h_val,
+                              system.col_idx[system.row_ptr[begin]:system.row_ptr[begin + 1]]).astype(np.float32)
+    assert np.array_equal(batch.read(0, nolsm.MAT_H).cpu().numpy(), ref)
+    ctx.close()
+
+
+@pytest.mark.parametrize("precision", [1, 0])
+def test_density_from_generated_elements(nolsm, mid_system, mid_solution, precision):
+    """The whole path (solve at fixed mu) with the model attached reproduces the oracle's D and N_e."""
+    system = mid_system
+    H, S = _device_system(nolsm, system)
+    ctx = nolsm.Context(nolsm.Config(precision=precision))
+    _attach_model(nolsm, ctx, system)
+    import oracle.nolsm_oracle as orc
+    ne, e, D, W, st = ctx.evaluate(H, S, MU, want_w=False)
+    sols = mid_solution["solutions"]
+    d_ref = orc.density_blocks(sols, system.row_ptr, MU)
+    ne_ref = orc.electron_count(sols, MU)
+    assert abs(ne - ne_ref) / system.n_mol <= TOL_NE_PER_MOL
+    assert np.abs(D.val.cpu().numpy() - d_ref).max() < TOL_D[precision]
+    e_ref = orc.electronic_energy_blocks(system.row_ptr, system.col_idx, d_ref, system.h_val)
+    assert abs(e - e_ref) / system.n_mol < TOL_E_PER_MOL[precision]
+    ctx.close()
+
+
+def test_model_argument_checks(nolsm, tiny_system):
+    import torch
+    import nolsm_inputs as gi
+    ctx = nolsm.Context()
+    pos = torch.as_tensor(tiny_system.pos_q).contiguous().cuda()
+    par = gi.model_parameters(tiny_system)
+    with pytest.raises(nolsm.NolsmError):
+        ctx.set_model(pos, **{**par, "box_q": [par["box_q"][0] + 1] * 3})       # odd box
+    with pytest.raises(nolsm.NolsmError):
+        ctx.set_model(pos, **{**par, "orb_site": [0, 0, 0, 0, 1, 3]})           # site out of range
+    ctx.set_model(pos[:16], **par)                                              # wrong n_mol: caught at build time
+    H, S = _device_system(nolsm, tiny_system)
+    with pytest.raises(nolsm.NolsmError):
+        ctx.build_submatrices(H, S, 0, 4)
+    ctx.close()
