@@ -68,9 +68,14 @@ typedef struct {
   int32_t flags;            /* NOLSM_FLAG_* */
 } nolsm_config;
 
+/* Engine of the matrix iterations.  With none of PAIR / MCAST / SINGLE set the context picks per batch:
+ * the pair engine when its 256-row tiles waste little (sum of the dimensions padded to 256 at most 4 % above
+ * the sum padded to 128) and the mean dimension is at least 1100 -- where it measured 5-11 % ahead -- else
+ * the single-CTA engine.  Each engine is bitwise reproducible run to run; different engines round differently. */
 #define NOLSM_FLAG_SIMT_ONLY 1 /* debugging: run every product on the FP32 SIMT kernel */
-#define NOLSM_FLAG_MCAST 4     /* run them on CTA pairs that share the B operand by TMA multicast (cta_group::1) */
-#define NOLSM_FLAG_PAIR 2      /* run the matrix iterations on CTA pairs (tcgen05 cta_group::2, 256-row tiles) */
+#define NOLSM_FLAG_PAIR 2      /* always the CTA-pair engine (tcgen05 cta_group::2, 256-row tiles) */
+#define NOLSM_FLAG_MCAST 4     /* always CTA pairs that share the B operand by TMA multicast (cta_group::1) */
+#define NOLSM_FLAG_SINGLE 8    /* always the single-CTA engine (128-row tiles) */
 
 typedef struct {            /* CSR of uniform bs x bs FP32 blocks; all pointers device, caller-owned */
   int32_t n_mol;            /* block rows = molecules */

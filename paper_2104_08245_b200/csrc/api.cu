@@ -238,6 +238,11 @@ static nolsm_status setup_batch(nolsm_ctx *ctx, int slot, const std::vector<int3
     b->tiles_simt_cap = tiles_simt.size();
   }
   b->n_tiles_simt = (int)tiles_simt.size();
+  {
+    double p128 = 0.0, p256 = 0.0, sum_n = 0.0;
+    for (int n : dims) { p128 += round_up(n, 128); p256 += round_up(n, 256); sum_n += n; }
+    b->prefer_pair = count > 0 && sum_n >= 1100.0 * count && p256 <= 1.04 * p128;
+  }
   // pageable host buffers: cudaMemcpyAsync stages them before returning, so the vectors may die
   NOLSM_CUDA(ctx, cudaMemcpyAsync(b->d_dims, dims.data(), sizeof(int32_t) * count, cudaMemcpyHostToDevice, st));
   if (!tiles_simt.empty())

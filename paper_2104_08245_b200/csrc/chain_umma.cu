@@ -562,7 +562,9 @@ cudaError_t launch_chain(nolsm_ctx *ctx, const nolsm_batch *b, const ChainProgra
                                     a.tile_counter, a.resid2, slots * b->count, a.iters, a.lastres, touch_stats ? 1 : 0);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
-  if (ctx->pair_ok && (ctx->cfg.flags & NOLSM_FLAG_PAIR)) return launch_chain_pair(ctx, b, a.prog, alpha_div, st);
+  const int forced = ctx->cfg.flags & (NOLSM_FLAG_PAIR | NOLSM_FLAG_MCAST | NOLSM_FLAG_SINGLE);
+  if (ctx->pair_ok && ((forced & NOLSM_FLAG_PAIR) || (forced == 0 && b->prefer_pair)))
+    return launch_chain_pair(ctx, b, a.prog, alpha_div, st);
   if (ctx->mcast_ok && (ctx->cfg.flags & NOLSM_FLAG_MCAST)) return launch_chain_mcast(ctx, b, a.prog, alpha_div, st);
   const int smem_bytes = a.stages * a.stage_bytes + 1024;
   void *params[] = {&a};

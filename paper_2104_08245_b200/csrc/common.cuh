@@ -70,6 +70,7 @@ struct ChainProgram {
 
 struct nolsm_batch {
   int32_t count = 0, ld = 0, mol_begin = 0, max_n = 0, slot = 0;
+  bool prefer_pair = false;       // batch shape favours the pair engine (nolsm.h, NOLSM_FLAG_*)
   bool engine_simt = false;       // prepared by the FP32 SIMT debugging path (different buffer roles)
   bool sparse = true;             // false: dense microbench batch (no neighbour list)
   bool prepared = false;          // S^-1 and B available

@@ -681,3 +681,25 @@ def test_model_argument_checks(nolsm, tiny_system):
     with pytest.raises(nolsm.NolsmError):
         ctx.build_submatrices(H, S, 0, 4)
     ctx.close()
+
+
+@pytest.mark.parametrize("precision,tol_x", [(1, 2e-5), (0, 3e-3)])
+def test_engine_selection_large_n(nolsm, torch_mod, precision, tol_x):
+    """n = 1280 is where the context switches to the pair engine on its own (nolsm.h, NOLSM_FLAG_*): the
+    automatic choice and both forced engines must all reproduce sign(A) of the construction, and the automatic
+    choice must be bit-identical to the forced pair engine (same kernel, same schedule-independent arithmetic)."""
+    import nolsm_inputs as gi
+    import oracle.nolsm_oracle as orc
+    mats = [gi.make_gapped_symmetric(1280, seed=13, index=i) for i in range(2)]
+    a = torch_mod.as_tensor(np.stack([m[0] for m in mats])).cuda()
+    scale = torch_mod.as_tensor(np.array([np.abs(m[2]).max() for m in mats], dtype=np.float32)).cuda()
+    got = {}
+    for flags in (0, nolsm.FLAG_PAIR, nolsm.FLAG_SINGLE):
+        ctx = nolsm.Context(nolsm.Config(precision=precision, flags=flags))
+        x, stats = ctx.sign_dense_batched(a, scale)
+        assert stats.n_unconverged == 0
+        for i, (_, q, lam) in enumerate(mats):
+            assert np.abs(x[i].cpu().numpy() - orc.sign_by_construction(q, lam)).max() < tol_x
+        got[flags] = x.clone()
+        ctx.close()
+    assert torch_mod.equal(got[0], got[nolsm.FLAG_PAIR])
