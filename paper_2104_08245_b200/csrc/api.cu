@@ -295,6 +295,10 @@ static nolsm_status check_bsr(nolsm_ctx *ctx, const nolsm_bsr *m, const char *na
     ctx->err = std::string("bad block-sparse matrix ") + name + " (bs must be 6, pointers non-null)";
     return NOLSM_EINVAL;
   }
+  if (reinterpret_cast<uintptr_t>(m->val) & 7) {   // the gather reads block rows with 8-byte loads
+    ctx->err = std::string("block-sparse matrix ") + name + ": val must be 8-byte aligned";
+    return NOLSM_EINVAL;
+  }
   return NOLSM_OK;
 }
 

@@ -160,25 +160,39 @@ k_gather(const int32_t *__restrict__ row_ptr, const int32_t *__restrict__ col_id
       }
     }
     __syncwarp();
-    for (int p = 0; p < NOLSM_BS; ++p) {
-      const int c = b * NOLSM_BS + p;
-      if (c >= P) break;
-      float *hc = hj + (int64_t)c * ld;
-      float *sc = sj + (int64_t)c * ld;
-      for (int r = lane; r < P; r += 32) {
-        float hv = 0.f, sv = 0.f;
-        if (c < n && r < n) {
-          const int a = r / NOLSM_BS, o = r - a * NOLSM_BS;
-          const int k = pos[a];
-          if (k >= 0) {
-            hv = h_val[(int64_t)k * 36 + o * NOLSM_BS + p];
-            sv = s_val[(int64_t)k * 36 + o * NOLSM_BS + p];
+    // Lane = row.  The six elements a row contributes to this block column are 24 contiguous bytes of
+    // the store (row o of block pos[a]): three 8-byte loads per matrix, then one 128-byte store
+    // instruction per column.
+    const int c0 = b * NOLSM_BS;
+    float *hc = hj + (int64_t)c0 * ld;
+    float *sc = sj + (int64_t)c0 * ld;
+    for (int r = lane; r < P; r += 32) {
+      float hv[NOLSM_BS], sv[NOLSM_BS];
+#pragma unroll
+      for (int p = 0; p < NOLSM_BS; ++p) hv[p] = sv[p] = 0.f;
+      if (c0 < n && r < n) {
+        const int a = r / NOLSM_BS, o = r - a * NOLSM_BS;
+        const int k = pos[a];
+        if (k >= 0) {
+          const float2 *hp = reinterpret_cast<const float2 *>(h_val + (int64_t)k * 36 + o * NOLSM_BS);
+          const float2 *sp = reinterpret_cast<const float2 *>(s_val + (int64_t)k * 36 + o * NOLSM_BS);
+#pragma unroll
+          for (int q = 0; q < 3; ++q) {
+            const float2 x = __ldg(hp + q), y = __ldg(sp + q);
+            hv[2 * q] = x.x; hv[2 * q + 1] = x.y;
+            sv[2 * q] = y.x; sv[2 * q + 1] = y.y;
           }
-        } else if (r == c) {
-          sv = 1.f;
         }
-        hc[r] = hv;
-        sc[r] = sv;
+      } else {
+#pragma unroll
+        for (int p = 0; p < NOLSM_BS; ++p) sv[p] = (r == c0 + p) ? 1.f : 0.f;   // identity padding of S
+      }
+#pragma unroll
+      for (int p = 0; p < NOLSM_BS; ++p) {
+        if (c0 + p < P) {
+          hc[(int64_t)p * ld + r] = hv[p];
+          sc[(int64_t)p * ld + r] = sv[p];
+        }
       }
     }
     __syncwarp();
@@ -343,7 +357,7 @@ k_density(const int32_t *__restrict__ row_ptr, const int32_t *__restrict__ col_i
           int ld, int64_t slab, const float *__restrict__ x, const float *__restrict__ x_alt,
           const int32_t *__restrict__ iters, const float *__restrict__ sinv,
           float *__restrict__ d_val, double *__restrict__ ne_diag) {
-  extern __shared__ float s_sinv[];  // [6][n]
+  extern __shared__ __align__(16) float s_sinv[];  // [n][6]: the six own columns of S^-1, row k contiguous
   const int mat = blockIdx.y;
   const int j = mol_begin + mat;
   const int lo = row_ptr[j];
@@ -360,7 +374,7 @@ k_density(const int32_t *__restrict__ row_ptr, const int32_t *__restrict__ col_i
   const float *sj = sinv + (int64_t)mat * slab;
   for (int t = threadIdx.x; t < NOLSM_BS * n; t += blockDim.x) {
     const int p = t / n, k = t - p * n;
-    s_sinv[t] = sj[(int64_t)(own0 + p) * ld + k];
+    s_sinv[k * NOLSM_BS + p] = sj[(int64_t)(own0 + p) * ld + k];
   }
   __syncthreads();
   const int r = blockIdx.x * DN_THREADS + threadIdx.x;
@@ -368,14 +382,17 @@ k_density(const int32_t *__restrict__ row_ptr, const int32_t *__restrict__ col_i
     float acc[NOLSM_BS];
 #pragma unroll
     for (int p = 0; p < NOLSM_BS; ++p) acc[p] = 0.f;
-    for (int k = 0; k < n; ++k) {
-      const float xv = xj[(int64_t)k * ld + r];
-#pragma unroll
-      for (int p = 0; p < NOLSM_BS; ++p) acc[p] = fmaf(xv, s_sinv[p * n + k], acc[p]);
+#pragma unroll 8
+    for (int k = 0; k < n; ++k) {   // X column by column (coalesced); S^-1 row k as three broadcast 8-byte loads
+      const float xv = __ldg(xj + (int64_t)k * ld + r);
+      const float2 *sk = reinterpret_cast<const float2 *>(s_sinv + k * NOLSM_BS);
+      const float2 s0 = sk[0], s1 = sk[1], s2 = sk[2];
+      acc[0] = fmaf(xv, s0.x, acc[0]); acc[1] = fmaf(xv, s0.y, acc[1]); acc[2] = fmaf(xv, s1.x, acc[2]);
+      acc[3] = fmaf(xv, s1.y, acc[3]); acc[4] = fmaf(xv, s2.x, acc[4]); acc[5] = fmaf(xv, s2.y, acc[5]);
     }
     float *out = d_val + ((int64_t)lo * 36 + (int64_t)r * NOLSM_BS);
 #pragma unroll
-    for (int p = 0; p < NOLSM_BS; ++p) out[p] = 0.5f * (s_sinv[p * n + r] - acc[p]);
+    for (int p = 0; p < NOLSM_BS; ++p) out[p] = 0.5f * (s_sinv[r * NOLSM_BS + p] - acc[p]);
     if (ne_diag != nullptr && r >= own0 && r < own0 + NOLSM_BS)
       atomicAdd(ne_diag, (double)(1.f - xj[(int64_t)r * ld + r]));
   }
