@@ -537,25 +537,31 @@ static nolsm_status prepare_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, int prec
     CHECK(run_chain(ctx, b, p1, b->d_scale, false, st));
   }
   if (refine > 0) LAUNCH(ctx, launch_scale_copy(b, S, nullptr, 0, nullptr, b->h[0], b->h[1], st));
+  int si_hi = 2, si_lo = 3;   // where the split S^-1 lives
   for (int it = 0; it < refine; ++it) {
     // Newton refinement S^-1 <- S^-1 + S^-1 (I - S S^-1): the residual on split operands, the small
-    // correction on plain FP16 operands (reading 11)
+    // correction on plain FP16 operands (reading 11).  The last refinement writes the split
+    // copy of the refined S^-1 from its own epilogue, over the split S (h0,h1) that only the residual
+    // product of the same submatrix read; earlier ones go through a scale_copy pass.
+    const bool last = it == refine - 1;
     ChainProgram p2 = one_shot(g1);
     p2.n_ops = 2;
     ChainOp &r = p2.ops[0] = make_op(EPI_IDENT, 1.f, 0.f);
     set2(r.a, 0, 0); set2(r.a_lo, 1, 1); set2(r.b, 2, 2); set2(r.b_lo, 3, 3); set2(r.out16, 4, 4);
     ChainOp &c = p2.ops[1] = make_op(EPI_AXPBY, 1.f, 1.f);
     set2(c.a, 2, 2); set2(c.b, 4, 4); c.cin32 = c.cout32 = 2;
+    if (last) { set2(c.out16, 0, 0); set2(c.out16_lo, 1, 1); si_hi = 0; si_lo = 1; }
     CHECK(run_chain(ctx, b, p2, nullptr, false, st));
-    LAUNCH(ctx, launch_scale_copy(b, b->u[2], nullptr, 0, nullptr, b->h[2], b->h[3], st));
+    if (!last) LAUNCH(ctx, launch_scale_copy(b, b->u[2], nullptr, 0, nullptr, b->h[2], b->h[3], st));
   }
-  // B = S^-1 H on split operands: H -> (h0,h1); result -> u3
-  LAUNCH(ctx, launch_scale_copy(b, H, nullptr, 0, nullptr, b->h[0], b->h[1], st));
+  // B = S^-1 H on split operands: H -> the free pair of halves; result -> u3
+  const int h_hi = si_hi == 0 ? 2 : 0, h_lo = h_hi + 1;
+  LAUNCH(ctx, launch_scale_copy(b, H, nullptr, 0, nullptr, b->h[h_hi], b->h[h_lo], st));
   {
     ChainProgram p4 = one_shot(g1);
     p4.n_ops = 1;
     ChainOp &o = p4.ops[0] = make_op(EPI_AXPBY, 1.f, 0.f);
-    set2(o.a, 2, 2); set2(o.a_lo, 3, 3); set2(o.b, 0, 0); set2(o.b_lo, 1, 1); o.cout32 = 3;
+    set2(o.a, si_hi, si_hi); set2(o.a_lo, si_lo, si_lo); set2(o.b, h_hi, h_hi); set2(o.b_lo, h_lo, h_lo); o.cout32 = 3;
     CHECK(run_chain(ctx, b, p4, nullptr, false, st));
   }
   b->engine_simt = false;
