@@ -58,7 +58,11 @@ typedef struct {
                                iteration is finished (reading 9).  <= 0: 1e-2 (FP16) / 1e-5 (FP32) */
   int32_t max_iter;         /* cap on sign iterations (default 30 if <= 0) */
   int32_t fixed_iter;       /* > 0: run exactly this many sign iterations, no residual test */
-  float inv_tol;            /* stop of Eq. 15-17 on ||I - Z_k Y_k||_F / sqrt(n); <= 0: 1e-2 (FP16) / 3e-6 (FP32) */
+  float inv_tol;            /* stop of Eq. 15-17 on r_k = ||I - Z_k Y_k||_F / sqrt(n) < inv_tol.  Without a
+                               refinement behind it iteration k is finished first (as for the sign iteration);
+                               with one (inv_refine > 0) Z_k is taken as it is and the two products that would
+                               finish iteration k are skipped.  <= 0: 3e-3 (FP16 with refinement), 1e-2 (FP16
+                               without), 1e-5 (FP32) */
   int32_t inv_max_iter;     /* cap on Eq. 15-17 iterations (default 20 if <= 0) */
   int32_t inv_refine;       /* FP16 mode: FP32-quality Newton refinements of S^-1 after Eq. 15-17
                                (reading 11); < 0: default 1;  0 = paper-literal all-FP16 S^-1 */

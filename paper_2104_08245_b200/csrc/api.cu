@@ -455,8 +455,10 @@ static ChainProgram one_shot(int group) {
 static nolsm_status prepare_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, int precision, cudaStream_t st,
                                         nolsm_sign_stats *stats, int64_t *gemms) {
   const bool fp16 = precision == NOLSM_FP16_FP32;
-  const float inv_tol = ctx->cfg.inv_tol > 0.f ? ctx->cfg.inv_tol : (fp16 ? 1e-2f : 1e-5f);
   const int refine = ctx->cfg.inv_refine >= 0 ? ctx->cfg.inv_refine : (fp16 ? 1 : 0);
+  // 3e-3 with a refinement behind: the iterate is taken with a relative error of about twice its residual,
+  // which the refinement squares (< 4e-5)
+  const float inv_tol = ctx->cfg.inv_tol > 0.f ? ctx->cfg.inv_tol : (fp16 ? (refine > 0 ? 3e-3f : 1e-2f) : 1e-5f);
   float *S = b->u[0], *H = b->u[1];
   LAUNCH(ctx, launch_norm_bound(b, S, 0.f, b->d_norm, st));
   ChainProgram pg;
@@ -468,6 +470,9 @@ static nolsm_status prepare_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, int prec
   // Iteration 0 in closed form (Z0 = I): E0 = I - Y0, Z1 = 3/2 I - 1/2 Y0 element-wise, Y1 = Y0 + 1/2 Y0 E0 by
   // one product; the chain then starts at iteration 1, i.e. on the odd-parity buffers.
   pg.max_iter = std::max(1, ctx->cfg.inv_max_iter - 1);
+  // With a Newton refinement behind it (which squares the error) the iterate whose residual passes the
+  // test is taken as it is: the two products that would finish that iteration are skipped (reading 11).
+  pg.stop_early = refine > 0 ? 1 : 0;
   ChainProgram p0 = one_shot(group_size(ctx, b, 16));
   p0.n_ops = 1;
   ChainOp &y1 = p0.ops[0] = make_op(EPI_AXPBY, 0.5f, 1.f);
@@ -512,11 +517,13 @@ static nolsm_status prepare_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, int prec
     NOLSM_CUDA(ctx, cudaStreamSynchronize(st));
     double fl = 0.0;
     for (int m = 0; m < b->count; ++m) {
+      // chain iterations carried out in full; a stop_early chain ran one residual product more
+      const int chain_products = 3 * it[m] + pg.stop_early;
       it[m] += 1;   // iteration 0 ran in closed form
       stats->inv_iter_max = std::max(stats->inv_iter_max, it[m]);
       if (!(res[m] <= stats->inv_worst_residual)) stats->inv_worst_residual = res[m];
       const double n = b->n_host[m];
-      const int products = 3 * it[m] - 2 + 2 + 2 * refine;   // products, whatever the MMAs per product
+      const int products = 1 + chain_products + 2 + 2 * refine;   // products, whatever the MMAs per product
       inv_gemm_sum += products;
       fl += 2.0 * n * n * n * products;
     }

@@ -97,13 +97,16 @@ __device__ __forceinline__ void epi_complete(const ChainArgs &args, const TileCm
         &args.resid2[(size_t)(k % NOLSM_MAX_RESID_SLOTS) * args.count + c.mat]);
     const float res = sqrtf(fmaxf(r2, 0.f) / (float)n);
     args.lastres[c.mat] = res;
-    args.iters[c.mat] = k + 1;
     bool stop = pg.fixed_iter > 0 ? (k + 1 >= pg.fixed_iter) : ((res < pg.tol) || !(res == res));
     if (k + 1 >= pg.max_iter) stop = true;
+    args.iters[c.mat] = (stop && pg.stop_early) ? k : k + 1;   // iterations carried out in full
     if (stop) *reinterpret_cast<volatile int32_t *>(&args.state[c.mat]) = k;
   }
   const int32_t stv = *reinterpret_cast<volatile int32_t *>(&args.state[c.mat]);
-  if (c.op == pg.n_ops - 1 && (stv == k || k + 1 >= limit)) {
+  // stop_early: the residual product is op 0; the schedulers waiting for ops 1.. of this iteration see
+  // kDone and skip their tiles
+  const bool early = pg.stop_early && o.resid && stv == k;
+  if (early || (c.op == pg.n_ops - 1 && (stv == k || k + 1 >= limit))) {
     st_release_gpu(&args.ready[c.mat], kDone);
     __threadfence();
     atomicSub(&args.group_active[c.mat / pg.group], 1);

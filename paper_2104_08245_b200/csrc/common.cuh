@@ -66,6 +66,8 @@ struct ChainProgram {
   int32_t max_iter, fixed_iter;   // fixed_iter > 0: exactly that many iterations, no residual test
   float tol;                      // stop rule of DESIGN.md reading 9 on the residual of the `resid` op
   int32_t group;                  // submatrices iterated together (L2 residency)
+  int32_t stop_early;             // 1: the iteration whose residual passes the test is NOT finished (its
+                                  // remaining products are skipped); 0: it is (reading 9, "+1 rule")
 };
 
 struct nolsm_batch {
