@@ -183,7 +183,7 @@ int32_t nolsm_batch_capacity(nolsm_ctx *ctx, const nolsm_bsr *H, int32_t mol_beg
 void nolsm_release_batch(nolsm_ctx *ctx, nolsm_batch *batch);
 
 /* a2-a4 (Eq. 15-17, Eq. 12, Eq. 9-10): for every submatrix of the batch, on the first call after the
- * gather: S_j^-1 and B_j = S_j^-1 H_j; on every call: X0 = (B_j - mu I)/s_j with s_j >= rho(B_j - mu I)
+ * gather: S_j^-1 and B_j = S_j^-1 H_j; on every call: X0 = (B_j - mu I)/s_j with 1.5 s_j >= rho(B_j - mu I)
  * and the sign iteration.  precision/tol/max_iter/fixed_iter < 0 or <= 0 take the context's values.
  * `stats` (host, may be NULL) makes the call synchronise at its end. */
 nolsm_status nolsm_sign_batched(nolsm_ctx *ctx, nolsm_batch *batch, double mu, int32_t precision,

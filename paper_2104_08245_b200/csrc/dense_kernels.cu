@@ -105,8 +105,14 @@ static dim3 elem4_grid(const nolsm_batch *b) {
   return dim3((unsigned)(((int64_t)(P >> 2) * P + 255) / 256), (unsigned)b->count);
 }
 
-// Eq. 15: Y0 = T_j(S)/s_S, Z0 = I with s_S = sqrt(||S||_1 ||S||_inf) >= lambda_max(S)
-// (reading 7).  The padded part of S is the identity, so Y0 there is 1/s_S.
+// Eq. 15: Y0 = T_j(S)/s_S, Z0 = I with s_S = 1/2 max(1, sqrt(||S||_1 ||S||_inf)) >=
+// lambda_max(S)/2 (reading 7): the spectrum of Y0 lies in (0, 2], inside the interval (0, 3) on
+// which v -> v (3 - v)^2 / 4 converges to 1, and roughly centred on 1, which saves one iteration over
+// scaling to (0, 1].  The padded part of S is the identity, so Y0 there is 1/s_S <= 2.
+constexpr float kInvScale = 0.5f;
+// X0 = A/s with s = sqrt(||A||_1 ||A||_inf)/1.5 >= rho(A)/1.5 (reading 5): every eigenvalue of X0 lies in
+// [-1.5, 1.5], inside the interval |x| < sqrt(3) on which Eq. 9 converges to sign(x).
+constexpr float kSignScale = 1.f / 1.5f;
 __global__ void __launch_bounds__(256)
 k_init_inverse(const int32_t *__restrict__ dims, int ld, int64_t slab, int count,
                const float *__restrict__ s, const float *__restrict__ norm2, float *__restrict__ y32,
@@ -115,7 +121,7 @@ k_init_inverse(const int32_t *__restrict__ dims, int ld, int64_t slab, int count
   Elem4 e;
   if (!elem4(dims, ld, slab, e)) return;
   const int mat = blockIdx.y;
-  const float sc = fmaxf(1.f, sqrtf(norm2[mat] * norm2[count + mat]));  // >= 1 covers the unit padding
+  const float sc = kInvScale * fmaxf(1.f, sqrtf(norm2[mat] * norm2[count + mat]));  // max(1, .) covers the unit padding
   if (e.r == 0 && e.c == 0) scale_out[mat] = sc;
   const float4 sv = *reinterpret_cast<const float4 *>(s + e.off);
   const float y[4] = {sv.x / sc, sv.y / sc, sv.z / sc, sv.w / sc};
@@ -153,7 +159,7 @@ k_init_inverse_first(const int32_t *__restrict__ dims, int ld, int64_t slab, int
   Elem4 e;
   if (!elem4(dims, ld, slab, e)) return;
   const int mat = blockIdx.y;
-  const float sc = fmaxf(1.f, sqrtf(norm2[mat] * norm2[count + mat]));
+  const float sc = kInvScale * fmaxf(1.f, sqrtf(norm2[mat] * norm2[count + mat]));
   if (e.r == 0 && e.c == 0) scale_out[mat] = sc;
   const float4 sv = *reinterpret_cast<const float4 *>(s + e.off);
   const float y[4] = {sv.x / sc, sv.y / sc, sv.z / sc, sv.w / sc};
@@ -191,7 +197,7 @@ k_make_x0(const int32_t *__restrict__ dims, int ld, int64_t slab, int count,
   Elem4 e;
   if (!elem4(dims, ld, slab, e)) return;
   const int mat = blockIdx.y;
-  float sc = scale_in ? scale_in[mat] : sqrtf(norm2[mat] * norm2[count + mat]);
+  float sc = scale_in ? scale_in[mat] : kSignScale * sqrtf(norm2[mat] * norm2[count + mat]);
   sc = fmaxf(sc, 1e-30f);
   if (e.r == 0 && e.c == 0 && scale_out) scale_out[mat] = sc;
   const float4 bv = *reinterpret_cast<const float4 *>(bmat + e.off);
