@@ -80,6 +80,9 @@ typedef struct {
 #define NOLSM_FLAG_PAIR 2      /* always the CTA-pair engine (tcgen05 cta_group::2, 256-row tiles) */
 #define NOLSM_FLAG_MCAST 4     /* always CTA pairs that share the B operand by TMA multicast (cta_group::1) */
 #define NOLSM_FLAG_SINGLE 8    /* always the single-CTA engine (128-row tiles) */
+#define NOLSM_FLAG_UNIT_SCALE 16 /* scale by the norm bound itself: Y0 = S/bound, X0 = A/bound (spectra in (0,1] and
+                                  [-1,1]) instead of bound/2 and bound/1.5 (readings 5, 7); costs one
+                                  iteration each */
 
 typedef struct {            /* CSR of uniform bs x bs FP32 blocks; all pointers device, caller-owned */
   int32_t n_mol;            /* block rows = molecules */

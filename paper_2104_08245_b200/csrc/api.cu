@@ -213,6 +213,9 @@ static nolsm_status setup_batch(nolsm_ctx *ctx, int slot, const std::vector<int3
   b->sparse = sparse;
   b->prepared = false;
   b->prepared_precision = -1;
+  const bool unit_scale = (ctx->cfg.flags & NOLSM_FLAG_UNIT_SCALE) != 0;
+  b->inv_scale = unit_scale ? 1.f : 0.5f;
+  b->sign_scale = unit_scale ? 1.f : 1.f / 1.5f;
   b->n_host = dims;
   b->n_unit = units;
   b->n_half = 2 * (units - 4);

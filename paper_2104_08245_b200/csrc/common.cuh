@@ -72,6 +72,8 @@ struct ChainProgram {
 
 struct nolsm_batch {
   int32_t count = 0, ld = 0, mol_begin = 0, max_n = 0, slot = 0;
+  float inv_scale = 0.5f;         // s_S = inv_scale * max(1, bound)   (reading 7; 1 with NOLSM_FLAG_UNIT_SCALE)
+  float sign_scale = 1.f / 1.5f;  // s_j = sign_scale * bound          (reading 5; 1 with NOLSM_FLAG_UNIT_SCALE)
   bool prefer_pair = false;       // batch shape favours the pair engine (nolsm.h, NOLSM_FLAG_*)
   bool engine_simt = false;       // prepared by the FP32 SIMT debugging path (different buffer roles)
   bool sparse = true;             // false: dense microbench batch (no neighbour list)

@@ -109,19 +109,19 @@ static dim3 elem4_grid(const nolsm_batch *b) {
 // lambda_max(S)/2 (reading 7): the spectrum of Y0 lies in (0, 2], inside the interval (0, 3) on
 // which v -> v (3 - v)^2 / 4 converges to 1, and roughly centred on 1, which saves one iteration over
 // scaling to (0, 1].  The padded part of S is the identity, so Y0 there is 1/s_S <= 2.
-constexpr float kInvScale = 0.5f;
 // X0 = A/s with s = sqrt(||A||_1 ||A||_inf)/1.5 >= rho(A)/1.5 (reading 5): every eigenvalue of X0 lies in
 // [-1.5, 1.5], inside the interval |x| < sqrt(3) on which Eq. 9 converges to sign(x).
-constexpr float kSignScale = 1.f / 1.5f;
+// Both factors come from the batch (1 under NOLSM_FLAG_UNIT_SCALE).
 __global__ void __launch_bounds__(256)
 k_init_inverse(const int32_t *__restrict__ dims, int ld, int64_t slab, int count,
                const float *__restrict__ s, const float *__restrict__ norm2, float *__restrict__ y32,
                float *__restrict__ z32, __half *__restrict__ y16, __half *__restrict__ z16,
-               __half *__restrict__ y16_lo, __half *__restrict__ z16_lo, float *__restrict__ scale_out) {
+               __half *__restrict__ y16_lo, __half *__restrict__ z16_lo, float *__restrict__ scale_out,
+               float factor) {
   Elem4 e;
   if (!elem4(dims, ld, slab, e)) return;
   const int mat = blockIdx.y;
-  const float sc = kInvScale * fmaxf(1.f, sqrtf(norm2[mat] * norm2[count + mat]));  // max(1, .) covers the unit padding
+  const float sc = factor * fmaxf(1.f, sqrtf(norm2[mat] * norm2[count + mat]));  // max(1, .) covers the unit padding
   if (e.r == 0 && e.c == 0) scale_out[mat] = sc;
   const float4 sv = *reinterpret_cast<const float4 *>(s + e.off);
   const float y[4] = {sv.x / sc, sv.y / sc, sv.z / sc, sv.w / sc};
@@ -143,7 +143,7 @@ cudaError_t launch_init_inverse(const nolsm_batch *b, const float *s, const floa
                                 float *scale_out, cudaStream_t st) {
   if (b->count == 0) return cudaSuccess;
   k_init_inverse<<<elem4_grid(b), 256, 0, st>>>(b->d_dims, b->ld, (int64_t)b->ld * b->ld, b->count, s, norm2,
-                                                y32, z32, y16, z16, y16_lo, z16_lo, scale_out);
+                                                y32, z32, y16, z16, y16_lo, z16_lo, scale_out, b->inv_scale);
   return cudaGetLastError();
 }
 
@@ -155,11 +155,11 @@ k_init_inverse_first(const int32_t *__restrict__ dims, int ld, int64_t slab, int
                      const float *__restrict__ s, const float *__restrict__ norm2, float *__restrict__ y32,
                      float *__restrict__ z32, __half *__restrict__ y16, __half *__restrict__ y16_lo,
                      __half *__restrict__ z16, __half *__restrict__ z16_lo, __half *__restrict__ e16,
-                     __half *__restrict__ e16_lo, float *__restrict__ scale_out) {
+                     __half *__restrict__ e16_lo, float *__restrict__ scale_out, float factor) {
   Elem4 e;
   if (!elem4(dims, ld, slab, e)) return;
   const int mat = blockIdx.y;
-  const float sc = kInvScale * fmaxf(1.f, sqrtf(norm2[mat] * norm2[count + mat]));
+  const float sc = factor * fmaxf(1.f, sqrtf(norm2[mat] * norm2[count + mat]));
   if (e.r == 0 && e.c == 0) scale_out[mat] = sc;
   const float4 sv = *reinterpret_cast<const float4 *>(s + e.off);
   const float y[4] = {sv.x / sc, sv.y / sc, sv.z / sc, sv.w / sc};
@@ -182,7 +182,8 @@ cudaError_t launch_init_inverse_first(const nolsm_batch *b, const float *s, cons
                                       __half *e16, __half *e16_lo, float *scale_out, cudaStream_t st) {
   if (b->count == 0) return cudaSuccess;
   k_init_inverse_first<<<elem4_grid(b), 256, 0, st>>>(b->d_dims, b->ld, (int64_t)b->ld * b->ld, b->count, s, norm2,
-                                                      y32, z32, y16, y16_lo, z16, z16_lo, e16, e16_lo, scale_out);
+                                                      y32, z32, y16, y16_lo, z16, z16_lo, e16, e16_lo, scale_out,
+                                                      b->inv_scale);
   return cudaGetLastError();
 }
 
@@ -193,11 +194,11 @@ __global__ void __launch_bounds__(256)
 k_make_x0(const int32_t *__restrict__ dims, int ld, int64_t slab, int count,
           const float *__restrict__ bmat, float mu, const float *__restrict__ norm2,
           const float *__restrict__ scale_in, float *__restrict__ x32, __half *__restrict__ x16,
-          __half *__restrict__ x16_lo, float *__restrict__ scale_out) {
+          __half *__restrict__ x16_lo, float *__restrict__ scale_out, float factor) {
   Elem4 e;
   if (!elem4(dims, ld, slab, e)) return;
   const int mat = blockIdx.y;
-  float sc = scale_in ? scale_in[mat] : kSignScale * sqrtf(norm2[mat] * norm2[count + mat]);
+  float sc = scale_in ? scale_in[mat] : factor * sqrtf(norm2[mat] * norm2[count + mat]);
   sc = fmaxf(sc, 1e-30f);
   if (e.r == 0 && e.c == 0 && scale_out) scale_out[mat] = sc;
   const float4 bv = *reinterpret_cast<const float4 *>(bmat + e.off);
@@ -218,7 +219,7 @@ cudaError_t launch_make_x0(const nolsm_batch *b, const float *bmat, float mu, co
                            cudaStream_t st) {
   if (b->count == 0) return cudaSuccess;
   k_make_x0<<<elem4_grid(b), 256, 0, st>>>(b->d_dims, b->ld, (int64_t)b->ld * b->ld, b->count, bmat, mu, norm2,
-                                           scale_in, x32, x16, x16_lo, scale_out);
+                                           scale_in, x32, x16, x16_lo, scale_out, b->sign_scale);
   return cudaGetLastError();
 }
 

@@ -703,3 +703,24 @@ def test_engine_selection_large_n(nolsm, torch_mod, precision, tol_x):
         got[flags] = x.clone()
         ctx.close()
     assert torch_mod.equal(got[0], got[nolsm.FLAG_PAIR])
+
+
+@pytest.mark.parametrize("precision", [1, 0])
+def test_unit_scale_flag_same_result_more_iterations(nolsm, tiny_system, tiny_solution, precision):
+    """Readings 5 and 7: the result does not depend on the scale, only the iteration count does.  With
+    NOLSM_FLAG_UNIT_SCALE (Y0 = S/bound, X0 = A/bound) D still matches the oracle and no submatrix needs
+    fewer iterations than with the centred scaling."""
+    import oracle.nolsm_oracle as orc
+    sols = tiny_solution["solutions"]
+    d_ref = orc.density_blocks(sols, tiny_system.row_ptr, MU)
+    H, S = _device_system(nolsm, tiny_system)
+    iters = {}
+    for flags in (0, nolsm.FLAG_UNIT_SCALE):
+        ctx = nolsm.Context(nolsm.Config(precision=precision, flags=flags))
+        ne, e, D, W, st = ctx.evaluate(H, S, MU, want_w=False)
+        assert np.abs(D.val.cpu().numpy() - d_ref).max() < TOL_D[precision]
+        assert abs(ne - orc.electron_count(sols, MU)) / tiny_system.n_mol <= TOL_NE_PER_MOL
+        iters[flags] = (st.last.iter_min, st.last.iter_max, st.last.inv_iter_max)
+        ctx.close()
+    assert iters[nolsm.FLAG_UNIT_SCALE][0] >= iters[0][0] and iters[nolsm.FLAG_UNIT_SCALE][1] >= iters[0][1]
+    assert iters[nolsm.FLAG_UNIT_SCALE][2] >= iters[0][2]
