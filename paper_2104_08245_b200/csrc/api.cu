@@ -99,6 +99,7 @@ static void free_batch(nolsm_batch *b) {
   cudaFree(b->d_lastres);
   cudaFree(b->d_scale);
   cudaFree(b->d_norm);
+  cudaFree(b->d_colpart);
   cudaFree(b->d_active);
   cudaFree(b->d_tiles_simt);
   cudaFree(b->d_ready);
@@ -204,6 +205,14 @@ static nolsm_status setup_batch(nolsm_ctx *ctx, int slot, const std::vector<int3
       return NOLSM_ENOMEM;
     }
     b->meta_cap = cap;
+  }
+  {
+    const size_t need_cp = (size_t)count * ((ld + 127) / 128) * ld;
+    if (need_cp > b->colpart_cap) {
+      cudaStreamSynchronize(st);
+      if (grow(&b->d_colpart, need_cp)) { cudaGetLastError(); ctx->err = "cudaMalloc of the norm scratch failed"; return NOLSM_ENOMEM; }
+      b->colpart_cap = need_cp;
+    }
   }
   b->count = count;
   b->ld = ld;
@@ -463,7 +472,7 @@ static nolsm_status prepare_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, int prec
   // which the refinement squares (< 4e-5)
   const float inv_tol = ctx->cfg.inv_tol > 0.f ? ctx->cfg.inv_tol : (fp16 ? (refine > 0 ? 3e-3f : 1e-2f) : 1e-5f);
   float *S = b->u[0], *H = b->u[1];
-  LAUNCH(ctx, launch_norm_bound(b, S, 0.f, b->d_norm, st));
+  LAUNCH(ctx, launch_norm_bound(b, S, 0.f, true, b->d_norm, st));
   ChainProgram pg;
   memset(&pg, 0, sizeof(pg));
   pg.n_ops = 3;
@@ -589,7 +598,7 @@ static nolsm_status sign_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, double mu, 
                                      bool timed) {
   const bool fp16 = precision == NOLSM_FP16_FP32;
   float *Bm = b->u[3], *X32 = b->u[0];
-  if (!scale_in) LAUNCH(ctx, launch_norm_bound(b, Bm, (float)mu, b->d_norm, st));
+  if (!scale_in) LAUNCH(ctx, launch_norm_bound(b, Bm, (float)mu, false, b->d_norm, st));
   ChainProgram pg;
   memset(&pg, 0, sizeof(pg));
   pg.n_ops = 2;
@@ -698,7 +707,7 @@ static nolsm_status prepare_batch_simt(nolsm_ctx *ctx, nolsm_batch *b, cudaStrea
   const float inv_tol = ctx->cfg.inv_tol > 0.f ? ctx->cfg.inv_tol : 1e-5f;
   const int max_it = ctx->cfg.inv_max_iter;
   float *S = b->u[0], *H = b->u[1];
-  LAUNCH(ctx, launch_norm_bound(b, S, 0.f, b->d_norm, st));
+  LAUNCH(ctx, launch_norm_bound(b, S, 0.f, true, b->d_norm, st));
   CHECK(E.control(0, 0, 0.f, 0, 0, false));
   int executed = 0;
   float *Y[2] = {b->u[2], b->u[5]}, *Z[2] = {b->u[3], b->u[6]}, *Em = b->u[4];
@@ -735,7 +744,7 @@ static nolsm_status sign_batch_simt(nolsm_ctx *ctx, nolsm_batch *b, double mu, f
                                     int fixed_iter, const float *scale_in, cudaStream_t st) {
   Engine E{ctx, b, st};
   float *Bm = b->u[2];
-  if (!scale_in) LAUNCH(ctx, launch_norm_bound(b, Bm, (float)mu, b->d_norm, st));
+  if (!scale_in) LAUNCH(ctx, launch_norm_bound(b, Bm, (float)mu, false, b->d_norm, st));
   CHECK(E.control(0, 0, 0.f, 0, 0, false));
   int executed = 0;
   float *X[2] = {b->u[0], b->u[3]}, *Em = b->u[5];

@@ -91,6 +91,8 @@ struct nolsm_batch {
   float *d_lastres = nullptr;     // [count]
   float *d_scale = nullptr;       // [count] s_j of the sign scaling
   float *d_norm = nullptr;        // [2][count] scratch for norm bounds
+  float *d_colpart = nullptr;     // [count][ld/128][ld] column-sum shares of the row strips (k_norm_bound)
+  size_t colpart_cap = 0;
   int32_t *d_active = nullptr;    // [NOLSM_MAX_RESID_SLOTS] active counters per iteration
   TileDesc *d_tiles_simt = nullptr; // 128x128 tiles for the SIMT kernel
   int32_t n_tiles_simt = 0;
@@ -175,7 +177,7 @@ cudaError_t launch_energy_weighted(const nolsm_batch *b, const float *x, const f
 cudaError_t launch_energy(const nolsm_batch *b, const int32_t *row_ptr, const float *d_val, const float *h_val,
                           double *e_out, cudaStream_t st);
 // dense helpers
-cudaError_t launch_norm_bound(const nolsm_batch *b, const float *a, float mu, float *norm2,
+cudaError_t launch_norm_bound(const nolsm_batch *b, const float *a, float mu, bool symmetric, float *norm2,
                               cudaStream_t st);
 cudaError_t launch_init_inverse(const nolsm_batch *b, const float *s, const float *norm2, float *y32,
                                 float *z32, __half *y16, __half *z16, __half *y16_lo, __half *z16_lo,

@@ -12,51 +12,93 @@ __device__ __forceinline__ void atomic_max_nonneg(float *addr, float v) {
 // ------------------------------------------------------------------------------------------------
 // Upper bound on the spectral radius: rho(A) <= ||A||_2 <= sqrt(||A||_1 ||A||_inf), A = M - mu I
 // (rescaling "prior to the sign iteration"; readings 5 and 7).
-// norm2[0][m] = ||A||_inf (max abs row sum), norm2[1][m] = ||A||_1 (max abs column sum).
-// Block = 128 rows (thread per row, coalesced over the column-major storage) + the same 128 columns
-// (warp per column, lanes along rows).
+// norm2[0][m] = ||A||_inf (max abs row sum), norm2[1][m] = ||A||_1 (max abs column sum), from ONE read of
+// the matrix.  A block owns a strip of 128 rows; warp w walks the columns c = w, w + 8, ... with one
+// 16-byte load per lane (four consecutive rows of the column-major storage).  Row sums accumulate in
+// registers and are combined over the eight warps in a fixed order; the strip's share of a column sum
+// is a warp reduction written to colpart[m][strip][c], and k_colmax adds the strips in order.  No
+// floating-point atomics: the bound is bitwise reproducible.  For a symmetric matrix (S) the column part
+// is skipped and ||A||_1 = ||A||_inf.
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(128)
-k_norm_bound(const int32_t *__restrict__ dims, int ld, int64_t slab, int count,
-             const float *__restrict__ a, float mu, float *__restrict__ norm2) {
+__global__ void __launch_bounds__(256)
+k_norm_bound(const int32_t *__restrict__ dims, int ld, int64_t slab, int count, int strips,
+             const float *__restrict__ a, float mu, float *__restrict__ norm2, float *__restrict__ colpart) {
+  __shared__ float s_row[8][128];
   const int mat = blockIdx.y;
   const int n = dims[mat];
   const int base = blockIdx.x * 128;
   if (base >= n) return;
   const float *aj = a + (int64_t)mat * slab;
-  const int r = base + threadIdx.x;
-  float rs = 0.f;
-  if (r < n) {
-    for (int c = 0; c < n; ++c) {
-      float v = aj[(int64_t)c * ld + r];
-      if (c == r) v -= mu;
-      rs += fabsf(v);
-    }
-  }
-  for (int d = 16; d > 0; d >>= 1) rs = fmaxf(rs, __shfl_xor_sync(0xffffffffu, rs, d));
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  if (lane == 0) atomic_max_nonneg(&norm2[mat], rs);
-  float cmax = 0.f;
-  for (int c = base + warp; c < min(n, base + 128); c += 4) {
+  const int r0 = base + 4 * lane;
+  float racc[4] = {0.f, 0.f, 0.f, 0.f};
+  float *cp = colpart ? colpart + ((int64_t)mat * strips + blockIdx.x) * ld : nullptr;
+  for (int c = warp; c < n; c += 8) {
+    const float4 v4 = *reinterpret_cast<const float4 *>(aj + (int64_t)c * ld + r0);
+    float v[4] = {v4.x, v4.y, v4.z, v4.w};
     float cs = 0.f;
-    for (int rr = lane; rr < n; rr += 32) {
-      float v = aj[(int64_t)c * ld + rr];
-      if (rr == c) v -= mu;
-      cs += fabsf(v);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const int r = r0 + i;
+      float x = r < n ? v[i] : 0.f;     // rows beyond n may hold stale data
+      if (r == c) x -= mu;
+      x = fabsf(x);
+      racc[i] += x;
+      cs += x;
     }
-    for (int d = 16; d > 0; d >>= 1) cs += __shfl_xor_sync(0xffffffffu, cs, d);
-    cmax = fmaxf(cmax, cs);
+    if (cp) {
+      for (int d = 16; d > 0; d >>= 1) cs += __shfl_xor_sync(0xffffffffu, cs, d);
+      if (lane == 0) cp[c] = cs;
+    }
   }
-  if (lane == 0) atomic_max_nonneg(&norm2[count + mat], cmax);
+#pragma unroll
+  for (int i = 0; i < 4; ++i) s_row[warp][4 * lane + i] = racc[i];
+  __syncthreads();
+  if (threadIdx.x < 128) {
+    float rs = 0.f;
+#pragma unroll
+    for (int w = 0; w < 8; ++w) rs += s_row[w][threadIdx.x];
+    for (int d = 16; d > 0; d >>= 1) rs = fmaxf(rs, __shfl_xor_sync(0xffffffffu, rs, d));
+    if (lane == 0) {
+      atomic_max_nonneg(&norm2[mat], rs);
+      if (!cp) atomic_max_nonneg(&norm2[count + mat], rs);
+    }
+  }
 }
 
-cudaError_t launch_norm_bound(const nolsm_batch *b, const float *a, float mu, float *norm2,
+__global__ void __launch_bounds__(256)
+k_colmax(const int32_t *__restrict__ dims, int ld, int count, int strips, const float *__restrict__ colpart,
+         float *__restrict__ norm2) {
+  __shared__ float s_max[8];
+  const int mat = blockIdx.x;
+  const int n = dims[mat];
+  const int ns = (n + 127) / 128;
+  const float *cp = colpart + (int64_t)mat * strips * ld;
+  float m = 0.f;
+  for (int c = threadIdx.x; c < n; c += blockDim.x) {
+    float cs = 0.f;
+    for (int s = 0; s < ns; ++s) cs += cp[(int64_t)s * ld + c];
+    m = fmaxf(m, cs);
+  }
+  for (int d = 16; d > 0; d >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, d));
+  if ((threadIdx.x & 31) == 0) s_max[threadIdx.x >> 5] = m;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int w = 1; w < 8; ++w) m = fmaxf(m, s_max[w]);
+    norm2[count + mat] = m;
+  }
+}
+
+cudaError_t launch_norm_bound(const nolsm_batch *b, const float *a, float mu, bool symmetric, float *norm2,
                               cudaStream_t st) {
   if (b->count == 0) return cudaSuccess;
   cudaError_t e = cudaMemsetAsync(norm2, 0, sizeof(float) * 2 * b->count, st);
   if (e != cudaSuccess) return e;
+  const int strips = (b->ld + 127) / 128;
   dim3 grid((b->max_n + 127) / 128, b->count);
-  k_norm_bound<<<grid, 128, 0, st>>>(b->d_dims, b->ld, (int64_t)b->ld * b->ld, b->count, a, mu, norm2);
+  k_norm_bound<<<grid, 256, 0, st>>>(b->d_dims, b->ld, (int64_t)b->ld * b->ld, b->count, strips, a, mu, norm2,
+                                     symmetric ? nullptr : b->d_colpart);
+  if (!symmetric) k_colmax<<<b->count, 256, 0, st>>>(b->d_dims, b->ld, b->count, strips, b->d_colpart, norm2);
   return cudaGetLastError();
 }
 
