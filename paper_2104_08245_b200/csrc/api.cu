@@ -542,45 +542,56 @@ static nolsm_status prepare_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, int prec
     stats->flops_prepare = fl;
   }
   const int g1 = group_size(ctx, b, 16);
-  // S^-1 = Z^2 / s_S (Eq. 17) from the FP32 master; result -> u2 and split (h2,h3).  When a Newton
-  // refinement follows (it squares the error) plain FP16 operands are enough here; otherwise split Z.
+  // S^-1 = Z^2 / s_S (Eq. 17); FP32 result -> u2, split copy -> (si_hi, si_lo).  The operands are the FP16
+  // copies of Z the chain itself wrote last (parity_from_iters), so no conversion pass is needed.  When a
+  // Newton refinement follows (it squares the error) plain FP16 operands are enough; otherwise split Z.
   const bool z_split = refine == 0;
-  LAUNCH(ctx, launch_scale_copy(b, b->u[3], nullptr, 0, nullptr, b->h[0], z_split ? b->h[1] : nullptr, st));
+  int si_hi, si_lo;           // where the split S^-1 lives
   {
     ChainProgram p1 = one_shot(g1);
     p1.n_ops = 1;
+    p1.parity_from_iters = 1;
     ChainOp &o = p1.ops[0] = make_op(EPI_AXPBY, 1.f, 0.f);
-    set2(o.a, 0, 0); set2(o.b, 0, 0);
-    if (z_split) { set2(o.a_lo, 1, 1); set2(o.b_lo, 1, 1); }
-    o.use_div = 1; o.cout32 = 2; set2(o.out16, 2, 2); set2(o.out16_lo, 3, 3);
+    if (fp16) {               // Z16 in h2 / h3 (chain op z), Y16 buffers h0, h1 are free
+      set2(o.a, 2, 3); set2(o.b, 2, 3);
+      si_hi = 0; si_lo = 1;
+    } else {                  // split Z in (h4,h5) / (h6,h7), split Y buffers h0..h3 are free
+      set2(o.a, 4, 6); set2(o.b, 4, 6);
+      if (z_split) { set2(o.a_lo, 5, 7); set2(o.b_lo, 5, 7); }
+      si_hi = 2; si_lo = 3;
+    }
+    o.use_div = 1; o.cout32 = 2; set2(o.out16, si_hi, si_hi); set2(o.out16_lo, si_lo, si_lo);
     CHECK(run_chain(ctx, b, p1, b->d_scale, false, st));
   }
-  if (refine > 0) LAUNCH(ctx, launch_scale_copy(b, S, nullptr, 0, nullptr, b->h[0], b->h[1], st));
-  int si_hi = 2, si_lo = 3;   // where the split S^-1 lives
+  // the other free pair of halves: split S for the refinements, split H for B = S^-1 H
+  int fr_hi = fp16 ? 2 : 0, fr_lo = fr_hi + 1;
+  if (refine > 0) LAUNCH(ctx, launch_scale_copy(b, S, nullptr, 0, nullptr, b->h[fr_hi], b->h[fr_lo], st));
   for (int it = 0; it < refine; ++it) {
     // Newton refinement S^-1 <- S^-1 + S^-1 (I - S S^-1): the residual on split operands, the small
     // correction on plain FP16 operands (reading 11).  The last refinement writes the split
-    // copy of the refined S^-1 from its own epilogue, over the split S (h0,h1) that only the residual
-    // product of the same submatrix read; earlier ones go through a scale_copy pass.
+    // copy of the refined S^-1 from its own epilogue, over the split S that only the residual product of
+    // the same submatrix read; earlier ones go through a scale_copy pass.
     const bool last = it == refine - 1;
     ChainProgram p2 = one_shot(g1);
     p2.n_ops = 2;
     ChainOp &r = p2.ops[0] = make_op(EPI_IDENT, 1.f, 0.f);
-    set2(r.a, 0, 0); set2(r.a_lo, 1, 1); set2(r.b, 2, 2); set2(r.b_lo, 3, 3); set2(r.out16, 4, 4);
+    set2(r.a, fr_hi, fr_hi); set2(r.a_lo, fr_lo, fr_lo); set2(r.b, si_hi, si_hi); set2(r.b_lo, si_lo, si_lo);
+    set2(r.out16, 4, 4);
     ChainOp &c = p2.ops[1] = make_op(EPI_AXPBY, 1.f, 1.f);
-    set2(c.a, 2, 2); set2(c.b, 4, 4); c.cin32 = c.cout32 = 2;
-    if (last) { set2(c.out16, 0, 0); set2(c.out16_lo, 1, 1); si_hi = 0; si_lo = 1; }
+    set2(c.a, si_hi, si_hi); set2(c.b, 4, 4); c.cin32 = c.cout32 = 2;
+    if (last) { set2(c.out16, fr_hi, fr_hi); set2(c.out16_lo, fr_lo, fr_lo); }
     CHECK(run_chain(ctx, b, p2, nullptr, false, st));
-    if (!last) LAUNCH(ctx, launch_scale_copy(b, b->u[2], nullptr, 0, nullptr, b->h[2], b->h[3], st));
+    if (last) { std::swap(si_hi, fr_hi); std::swap(si_lo, fr_lo); }
+    else LAUNCH(ctx, launch_scale_copy(b, b->u[2], nullptr, 0, nullptr, b->h[si_hi], b->h[si_lo], st));
   }
   // B = S^-1 H on split operands: H -> the free pair of halves; result -> u3
-  const int h_hi = si_hi == 0 ? 2 : 0, h_lo = h_hi + 1;
-  LAUNCH(ctx, launch_scale_copy(b, H, nullptr, 0, nullptr, b->h[h_hi], b->h[h_lo], st));
+  LAUNCH(ctx, launch_scale_copy(b, H, nullptr, 0, nullptr, b->h[fr_hi], b->h[fr_lo], st));
   {
     ChainProgram p4 = one_shot(g1);
     p4.n_ops = 1;
     ChainOp &o = p4.ops[0] = make_op(EPI_AXPBY, 1.f, 0.f);
-    set2(o.a, si_hi, si_hi); set2(o.a_lo, si_lo, si_lo); set2(o.b, h_hi, h_hi); set2(o.b_lo, h_lo, h_lo); o.cout32 = 3;
+    set2(o.a, si_hi, si_hi); set2(o.a_lo, si_lo, si_lo); set2(o.b, fr_hi, fr_hi); set2(o.b_lo, fr_lo, fr_lo);
+    o.cout32 = 3;
     CHECK(run_chain(ctx, b, p4, nullptr, false, st));
   }
   b->engine_simt = false;

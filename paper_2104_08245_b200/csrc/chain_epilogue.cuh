@@ -40,6 +40,11 @@ struct TileCmd {              // scheduler -> TMA producer(s), MMA issuer and ep
   int32_t op, iter;           // op < 0: no more tiles
 };
 
+// TileCmd::iter carries the iteration in its low bits and, in bit 30, a flip of the operand-table parity
+// (ChainProgram::parity_from_iters).
+__device__ __forceinline__ int cmd_iter(const TileCmd &c) { return c.iter & 0x3fffffff; }
+__device__ __forceinline__ int cmd_par(const TileCmd &c) { return (c.iter ^ (c.iter >> 30)) & 1; }
+
 struct ChainArgs {
   ChainProgram prog;
   const CUtensorMap *maps;    // [n_half] TMA maps of the FP16 operand buffers ({64,64} boxes, 128-byte swizzle)
@@ -85,13 +90,13 @@ __device__ __forceinline__ void epi_complete(const ChainArgs &args, const TileCm
   const int n = args.dims[c.mat];
   const int ncol = (n + kColRound - 1) / kColRound * kColRound;
   const int tiles_m = ((n + kTileM - 1) / kTileM) * ((ncol + args.bn - 1) / args.bn);
-  const int need = c.iter * pg.n_ops + c.op;
+  const int need = cmd_iter(c) * pg.n_ops + c.op;
   const int limit = pg.fixed_iter > 0 ? min(pg.fixed_iter, pg.max_iter) : pg.max_iter;
   __threadfence();      // the CTA's stores (ordered before us by the barrier) become visible GPU-wide
   const int32_t old = atomicAdd(&args.tiles_done[c.mat], 1);
   if (old + 1 != (need + 1) * tiles_m * kArrivals) return;
   __threadfence();
-  const int k = c.iter;
+  const int k = cmd_iter(c);
   if (o.resid) {
     const float r2 = *reinterpret_cast<volatile float *>(
         &args.resid2[(size_t)(k % NOLSM_MAX_RESID_SLOTS) * args.count + c.mat]);
@@ -132,7 +137,7 @@ __device__ __forceinline__ void epi_begin(const ChainArgs &args, const TileCmd &
                                           int chunk_first, EpiTile &t) {
   const ChainOp &o = args.prog.ops[c.op];
   t.o = &o;
-  t.par = c.iter & 1;
+  t.par = cmd_par(c);
   t.n = args.dims[c.mat];
   t.r = row0 + lane;
   t.rows_in = rows_in;

@@ -244,7 +244,8 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain_mcast(const PairArgs args
         }
         const int kblocks = (n16 + kBK - 1) / kBK;
         {
-          push(TileCmd{m, m0, n0, min(args.bn, n16 - n0), kblocks, (n16 - (kblocks - 1) * kBK) / 16, op, k});
+          push(TileCmd{m, m0, n0, min(args.bn, n16 - n0), kblocks, (n16 - (kblocks - 1) * kBK) / 16, op,
+                          k | (pg.parity_from_iters ? (((args.iters[m] + 1) & 1) << 30) : 0)});
         }
       }
       push(TileCmd{0, 0, 0, 0, 0, 0, -1, 0});
@@ -266,7 +267,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain_mcast(const PairArgs args
         PTRACE(2, tti, 0);
         fence_proxy_async();   // other CTAs' generic-proxy writes (ordered by the scheduler's acquire) -> TMA reads
         const ChainOp &o = pg.ops[c.op];
-        const int par = c.iter & 1;
+        const int par = chainep::cmd_par(c);
         const int m = c.mat;
         const int m0 = c.m0 + 128 * (int)rank;               // this CTA's tile of the vertical pair
         const int n0 = c.n0;
@@ -322,7 +323,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain_mcast(const PairArgs args
         if (one) mbar_arrive_cluster(mapa(smem_u32(&cmd_empty[slot]), 0));
         if (++slot == kRing) { slot = 0; ring_phase ^= 1u; }
         if (c.op < 0) break;
-        const bool split = pg.ops[c.op].a_lo[c.iter & 1] >= 0;
+        const bool split = pg.ops[c.op].a_lo[chainep::cmd_par(c)] >= 0;
         const bool phantom = c.m0 + 128 * (int)rank >= args.dims[c.mat];
         // instruction descriptor: D=F32, A=B=F16, A M-major, B K-major, N = nt, M = 128
         const uint32_t idesc = (1u << 4) | (1u << 15) | ((uint32_t)(c.nt >> 3) << 17) | ((128u >> 4) << 24);
@@ -413,7 +414,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain_mcast(const PairArgs args
       if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
       if (t.o->resid) {
         for (int d = 16; d > 0; d >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, d);
-        if (lane == 0) atomicAdd(&args.resid2[(size_t)(c.iter % NOLSM_MAX_RESID_SLOTS) * args.count + c.mat], ss);
+        if (lane == 0) atomicAdd(&args.resid2[(size_t)(chainep::cmd_iter(c) % NOLSM_MAX_RESID_SLOTS) * args.count + c.mat], ss);
       }
       // all epilogue warps of this CTA have issued their stores: one thread publishes the CTA's half
       asm volatile("bar.sync 1, %0;" ::"n"(kEpiWarps * 32) : "memory");

@@ -217,7 +217,8 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
         const int kblocks = (n16 + kBK - 1) / kBK;
         {
           mbar_wait(&cmd_empty[slot], ring_phase ^ 1u);
-          cmds[slot] = TileCmd{m, m0, n0, min(args.bn, n16 - n0), kblocks, (n16 - (kblocks - 1) * kBK) / 16, op, k};
+          cmds[slot] = TileCmd{m, m0, n0, min(args.bn, n16 - n0), kblocks, (n16 - (kblocks - 1) * kBK) / 16, op,
+                                  k | (pg.parity_from_iters ? (((args.iters[m] + 1) & 1) << 30) : 0)};
           mbar_arrive(&cmd_full[slot]);
           if (++slot == kRing) { slot = 0; ring_phase ^= 1u; }
         }
@@ -246,7 +247,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
         TRACE(2, tti, 0);
         fence_proxy_async();   // other CTAs' generic-proxy writes (ordered by the scheduler's acquire) -> TMA reads
         const ChainOp &o = pg.ops[c.op];
-        const int par = c.iter & 1;
+        const int par = chainep::cmd_par(c);
         const int m = c.mat, m0 = c.m0, n0 = c.n0;
         const bool split = o.a_lo[par] >= 0;
         const int nbox = (c.nt + 63) >> 6;
@@ -302,7 +303,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
         if (one) mbar_arrive(&cmd_empty[slot]);
         if (++slot == kRing) { slot = 0; ring_phase ^= 1u; }
         if (c.op < 0) break;
-        const bool split = pg.ops[c.op].a_lo[c.iter & 1] >= 0;
+        const bool split = pg.ops[c.op].a_lo[chainep::cmd_par(c)] >= 0;
         // instruction descriptor: D=F32, A=B=F16, A M-major, B K-major, N = nt, M = 128
         const uint32_t idesc = (1u << 4) | (1u << 15) | ((uint32_t)(c.nt >> 3) << 17) | ((128u >> 4) << 24);
         TRACE(0, mti, 0);
@@ -396,7 +397,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
       if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
       if (t.o->resid) {
         for (int d = 16; d > 0; d >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, d);
-        if (lane == 0) atomicAdd(&args.resid2[(size_t)(c.iter % NOLSM_MAX_RESID_SLOTS) * args.count + c.mat], ss);
+        if (lane == 0) atomicAdd(&args.resid2[(size_t)(chainep::cmd_iter(c) % NOLSM_MAX_RESID_SLOTS) * args.count + c.mat], ss);
       }
       TRACE2(eti, 5);
       // all epilogue warps have issued their stores and residual atomics: one thread publishes the tile

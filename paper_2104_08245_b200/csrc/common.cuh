@@ -66,6 +66,9 @@ struct ChainProgram {
   int32_t max_iter, fixed_iter;   // fixed_iter > 0: exactly that many iterations, no residual test
   float tol;                      // stop rule of DESIGN.md reading 9 on the residual of the `resid` op
   int32_t group;                  // submatrices iterated together (L2 residency)
+  int32_t parity_from_iters;      // 1: the operand tables are indexed by the parity of the LAST full iteration of
+                                  // the chain that ran before on this batch ((iters[m] + 1) & 1) instead of the
+                                  // own iteration's: lets a one-shot product read the final FP16 iterate in place
   int32_t stop_early;             // 1: the iteration whose residual passes the test is NOT finished (its
                                   // remaining products are skipped); 0: it is (reading 9, "+1 rule")
 };
