@@ -89,7 +89,7 @@ typedef struct {            /* CSR of uniform bs x bs FP32 blocks; all pointers 
   int32_t bs;               /* block size, must be 6 */
   const int32_t *row_ptr;   /* [n_mol+1] */
   const int32_t *col_idx;   /* [nnzb], ascending within a row */
-  float *val;               /* [nnzb*bs*bs], each block row-major; 8-byte aligned */
+  float *val;               /* [nnzb*bs*bs], each block row-major; 16-byte aligned */
 } nolsm_bsr;
 
 typedef struct {            /* filled by nolsm_sign_batched (host struct) */

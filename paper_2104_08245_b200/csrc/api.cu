@@ -143,8 +143,10 @@ extern "C" int32_t nolsm_batch_ld(const nolsm_batch *b) { return b ? b->ld : 0; 
 // Batch storage
 // ------------------------------------------------------------------------------------------------
 // FP32 units per submatrix: S/X, H, Y/S^-1, Z/B and the FP16 operand buffers (two per unit):
-// 6 of them in FP16 mode, 10 in FP32 mode (split hi/lo operands).
-static int units_for(int precision) { return precision == NOLSM_FP16_FP32 ? 7 : 9; }
+// 6 of them in FP16 mode, 10 in FP32 mode (split hi/lo operands); gathered
+// batches have four more, the last ones: the split copies of S and H the builder writes.
+static int units_dense(int precision) { return precision == NOLSM_FP16_FP32 ? 7 : 9; }
+static int units_for(int precision) { return units_dense(precision) + 2; }
 static size_t dense_bytes(int count, int ld, int units) {
   return (size_t)units * 4 * (size_t)ld * ld * (size_t)count;
 }
@@ -307,8 +309,8 @@ static nolsm_status check_bsr(nolsm_ctx *ctx, const nolsm_bsr *m, const char *na
     ctx->err = std::string("bad block-sparse matrix ") + name + " (bs must be 6, pointers non-null)";
     return NOLSM_EINVAL;
   }
-  if (reinterpret_cast<uintptr_t>(m->val) & 7) {   // the gather reads block rows with 8-byte loads
-    ctx->err = std::string("block-sparse matrix ") + name + ": val must be 8-byte aligned";
+  if (reinterpret_cast<uintptr_t>(m->val) & 15) {   // the gather reads pairs of block rows with 16-byte loads
+    ctx->err = std::string("block-sparse matrix ") + name + ": val must be 16-byte aligned";
     return NOLSM_EINVAL;
   }
   return NOLSM_OK;
@@ -385,15 +387,19 @@ static nolsm_status build_submatrices_impl(nolsm_ctx *ctx, const nolsm_bsr *H, c
   if (mol_count > 0) CHECK(read_dims(ctx, H->row_ptr, mol_begin, mol_count, dims, st));
   nolsm_batch *b = nullptr;
   CHECK(setup_batch(ctx, slot, dims, mol_begin, true, units, &b, st));
+  // the split copy of S is only read by the Newton refinements of S^-1 (reading 11)
+  const int prec = effective_precision(ctx, -1);
+  const bool split_s = (ctx->cfg.inv_refine >= 0 ? ctx->cfg.inv_refine : (prec == NOLSM_FP16_FP32 ? 1 : 0)) > 0;
   if (ctx->has_model) {
     if (ctx->model.n_mol != H->n_mol) {
       ctx->err = "the attached model has a different number of molecules than the matrices";
       return NOLSM_EINVAL;
     }
-    LAUNCH(ctx, launch_generate(b, H->row_ptr, H->col_idx, &ctx->model, b->u[1], b->u[0], st));
+    LAUNCH(ctx, launch_generate(b, H->row_ptr, H->col_idx, &ctx->model, b->u[1], b->u[0], split_s, st));
   } else {
-    LAUNCH(ctx, launch_gather(b, H->row_ptr, H->col_idx, H->val, S->val, b->u[1], b->u[0], st));
+    LAUNCH(ctx, launch_gather(b, H->row_ptr, H->col_idx, H->val, S->val, b->u[1], b->u[0], split_s, st));
   }
+  b->s_split_built = split_s;
   *out = b;
   return NOLSM_OK;
 }
@@ -563,34 +569,32 @@ static nolsm_status prepare_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, int prec
     o.use_div = 1; o.cout32 = 2; set2(o.out16, si_hi, si_hi); set2(o.out16_lo, si_lo, si_lo);
     CHECK(run_chain(ctx, b, p1, b->d_scale, false, st));
   }
-  // the other free pair of halves: split S for the refinements, split H for B = S^-1 H
-  int fr_hi = fp16 ? 2 : 0, fr_lo = fr_hi + 1;
-  if (refine > 0) LAUNCH(ctx, launch_scale_copy(b, S, nullptr, 0, nullptr, b->h[fr_hi], b->h[fr_lo], st));
+  // split S (refinements) and split H (B = S^-1 H) come from the builder, in the last four halves
+  const int ss_hi = b->n_half - 4, ss_lo = b->n_half - 3, hs_hi = b->n_half - 2, hs_lo = b->n_half - 1;
+  int fr_hi = fp16 ? 2 : 0, fr_lo = fr_hi + 1;   // a pair of halves the iterations no longer need
+  if (refine > 0 && !b->s_split_built)           // batch built under another configuration
+    LAUNCH(ctx, launch_scale_copy(b, S, nullptr, 0, nullptr, b->h[ss_hi], b->h[ss_lo], st));
   for (int it = 0; it < refine; ++it) {
     // Newton refinement S^-1 <- S^-1 + S^-1 (I - S S^-1): the residual on split operands, the small
-    // correction on plain FP16 operands (reading 11).  The last refinement writes the split
-    // copy of the refined S^-1 from its own epilogue, over the split S that only the residual product of
-    // the same submatrix read; earlier ones go through a scale_copy pass.
-    const bool last = it == refine - 1;
+    // correction on plain FP16 operands (reading 11); the refined S^-1 leaves the epilogue as
+    // FP32 master (u2) and as split copy in the free pair of halves.
     ChainProgram p2 = one_shot(g1);
     p2.n_ops = 2;
     ChainOp &r = p2.ops[0] = make_op(EPI_IDENT, 1.f, 0.f);
-    set2(r.a, fr_hi, fr_hi); set2(r.a_lo, fr_lo, fr_lo); set2(r.b, si_hi, si_hi); set2(r.b_lo, si_lo, si_lo);
+    set2(r.a, ss_hi, ss_hi); set2(r.a_lo, ss_lo, ss_lo); set2(r.b, si_hi, si_hi); set2(r.b_lo, si_lo, si_lo);
     set2(r.out16, 4, 4);
     ChainOp &c = p2.ops[1] = make_op(EPI_AXPBY, 1.f, 1.f);
     set2(c.a, si_hi, si_hi); set2(c.b, 4, 4); c.cin32 = c.cout32 = 2;
-    if (last) { set2(c.out16, fr_hi, fr_hi); set2(c.out16_lo, fr_lo, fr_lo); }
+    set2(c.out16, fr_hi, fr_hi); set2(c.out16_lo, fr_lo, fr_lo);
     CHECK(run_chain(ctx, b, p2, nullptr, false, st));
-    if (last) { std::swap(si_hi, fr_hi); std::swap(si_lo, fr_lo); }
-    else LAUNCH(ctx, launch_scale_copy(b, b->u[2], nullptr, 0, nullptr, b->h[si_hi], b->h[si_lo], st));
+    std::swap(si_hi, fr_hi); std::swap(si_lo, fr_lo);
   }
-  // B = S^-1 H on split operands: H -> the free pair of halves; result -> u3
-  LAUNCH(ctx, launch_scale_copy(b, H, nullptr, 0, nullptr, b->h[fr_hi], b->h[fr_lo], st));
+  // B = S^-1 H on split operands; result -> u3
   {
     ChainProgram p4 = one_shot(g1);
     p4.n_ops = 1;
     ChainOp &o = p4.ops[0] = make_op(EPI_AXPBY, 1.f, 0.f);
-    set2(o.a, si_hi, si_hi); set2(o.a_lo, si_lo, si_lo); set2(o.b, fr_hi, fr_hi); set2(o.b_lo, fr_lo, fr_lo);
+    set2(o.a, si_hi, si_hi); set2(o.a_lo, si_lo, si_lo); set2(o.b, hs_hi, hs_hi); set2(o.b_lo, hs_lo, hs_lo);
     o.cout32 = 3;
     CHECK(run_chain(ctx, b, p4, nullptr, false, st));
   }
@@ -1181,7 +1185,7 @@ extern "C" nolsm_status nolsm_sign_dense_batched(nolsm_ctx *ctx, const float *a,
   if (batch == 0) return NOLSM_OK;
   std::vector<int32_t> dims(batch, n);
   nolsm_batch *b = nullptr;
-  CHECK(setup_batch(ctx, 0, dims, 0, false, units_for(prec), &b, st));
+  CHECK(setup_batch(ctx, 0, dims, 0, false, units_dense(prec), &b, st));
   b->prepared = true;
   b->prepared_precision = prec;
   b->engine_simt = use_simt(ctx);

@@ -16,8 +16,9 @@
 #define NOLSM_TILE_M 128          // rows per output tile (UMMA M, one CTA)
 #define NOLSM_PAD 128             // leading dimensions are multiples of this
 #define NOLSM_MAX_RESID_SLOTS 64  // residual history kept per submatrix
-#define NOLSM_MAX_HALF 10         // FP16 operand buffers of a batch (6 in FP16 mode, 10 in FP32 mode)
-#define NOLSM_MAX_UNIT 9          // FP32 buffers of a batch (the FP16 buffers alias units 4..)
+#define NOLSM_MAX_HALF 14         // FP16 operand buffers of a batch (6 / 10 of the iterations in FP16 / FP32 mode
+                                  // + 4 of a gathered batch: split copies of S and H written by the builder)
+#define NOLSM_MAX_UNIT 11         // FP32 buffers of a batch (the FP16 buffers alias units 4..)
 
 struct TileDesc {                 // one output tile of one submatrix
   int32_t mat;                    // index inside the batch
@@ -77,6 +78,7 @@ struct nolsm_batch {
   int32_t count = 0, ld = 0, mol_begin = 0, max_n = 0, slot = 0;
   float inv_scale = 0.5f;         // s_S = inv_scale * max(1, bound)   (reading 7; 1 with NOLSM_FLAG_UNIT_SCALE)
   float sign_scale = 1.f / 1.5f;  // s_j = sign_scale * bound          (reading 5; 1 with NOLSM_FLAG_UNIT_SCALE)
+  bool s_split_built = false;     // the builder wrote the split copy of S into h[n_half-4], h[n_half-3]
   bool prefer_pair = false;       // batch shape favours the pair engine (nolsm.h, NOLSM_FLAG_*)
   bool engine_simt = false;       // prepared by the FP32 SIMT debugging path (different buffer roles)
   bool sparse = true;             // false: dense microbench batch (no neighbour list)
@@ -164,9 +166,10 @@ cudaError_t launch_exclusive_scan(const int32_t *counts, int32_t *row_ptr, int n
 cudaError_t launch_neighbour_fill(int n_mol, const int32_t *pos, const int32_t *box, int32_t rc,
                                   const int32_t *row_ptr, int32_t *col_idx, cudaStream_t st);
 cudaError_t launch_generate(const nolsm_batch *b, const int32_t *row_ptr, const int32_t *col_idx,
-                            const nolsm_model *model, float *h_out, float *s_out, cudaStream_t st);
+                            const nolsm_model *model, float *h_out, float *s_out, bool split_s,
+                            cudaStream_t st);
 cudaError_t launch_gather(const nolsm_batch *b, const int32_t *row_ptr, const int32_t *col_idx,
-                          const float *h_val, const float *s_val, float *h_out, float *s_out,
+                          const float *h_val, const float *s_val, float *h_out, float *s_out, bool split_s,
                           cudaStream_t st);
 cudaError_t launch_density(const nolsm_batch *b, const float *x, const float *x_alt, const float *sinv,
                            const int32_t *row_ptr, const int32_t *col_idx, float *d_val,

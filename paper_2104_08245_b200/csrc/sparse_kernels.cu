@@ -129,10 +129,49 @@ cudaError_t launch_exclusive_scan(const int32_t *counts, int32_t *row_ptr, int n
 // ------------------------------------------------------------------------------------------------
 #define GA_WARPS 4
 
+// Where a submatrix builder writes: the FP32 matrices and, when the pointers are set, their split FP16
+// copies (hi = fp16(v), lo = fp16((v - hi) 2^11): the operands of the FP32-quality products, same
+// arithmetic as k_scale_copy) so that no conversion pass has to read the matrices again.
+struct BuildOut {
+  float *h32, *s32;
+  __half *h_hi, *h_lo, *s_hi, *s_lo;
+};
+
+__device__ __forceinline__ void split_pair(float v0, float v1, __half2 &hi, __half2 &lo) {
+  const __half a = __float2half_rn(v0), b = __float2half_rn(v1);
+  hi = __halves2half2(a, b);
+  lo = __floats2half2_rn((v0 - __half2float(a)) * 2048.f, (v1 - __half2float(b)) * 2048.f);
+}
+
+// Rows r, r+1 (r even) of the six columns c0..c0+5: 8-byte FP32 stores (256 bytes per warp instruction)
+// and 4-byte FP16 stores (128 bytes per warp instruction).
+__device__ __forceinline__ void emit_rows2(const BuildOut &out, int64_t base, int ld, int c0, int r, int P,
+                                           const float (&hv)[2][NOLSM_BS], const float (&sv)[2][NOLSM_BS]) {
+#pragma unroll
+  for (int p = 0; p < NOLSM_BS; ++p) {
+    if (c0 + p < P) {
+      const int64_t off = base + (int64_t)(c0 + p) * ld + r;
+      *reinterpret_cast<float2 *>(out.h32 + off) = make_float2(hv[0][p], hv[1][p]);
+      *reinterpret_cast<float2 *>(out.s32 + off) = make_float2(sv[0][p], sv[1][p]);
+      __half2 hi, lo;
+      if (out.h_hi) {
+        split_pair(hv[0][p], hv[1][p], hi, lo);
+        *reinterpret_cast<__half2 *>(out.h_hi + off) = hi;
+        *reinterpret_cast<__half2 *>(out.h_lo + off) = lo;
+      }
+      if (out.s_hi) {
+        split_pair(sv[0][p], sv[1][p], hi, lo);
+        *reinterpret_cast<__half2 *>(out.s_hi + off) = hi;
+        *reinterpret_cast<__half2 *>(out.s_lo + off) = lo;
+      }
+    }
+  }
+}
+
 __global__ void __launch_bounds__(GA_WARPS * 32)
 k_gather(const int32_t *__restrict__ row_ptr, const int32_t *__restrict__ col_idx,
          const float *__restrict__ h_val, const float *__restrict__ s_val, int mol_begin, int ld,
-         int64_t slab, float *__restrict__ h_out, float *__restrict__ s_out) {
+         int64_t slab, BuildOut out) {
   extern __shared__ int32_t s_pos[];  // [GA_WARPS][m_max]
   const int mat = blockIdx.y;
   const int j = mol_begin + mat;
@@ -143,8 +182,7 @@ k_gather(const int32_t *__restrict__ row_ptr, const int32_t *__restrict__ col_id
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int m_pad_blocks = (P + NOLSM_BS - 1) / NOLSM_BS;  // block-columns incl. padding
   int32_t *pos = s_pos + warp * ((ld + NOLSM_BS - 1) / NOLSM_BS + 1);
-  float *hj = h_out + (int64_t)mat * slab;
-  float *sj = s_out + (int64_t)mat * slab;
+  const int64_t base = (int64_t)mat * slab;
   for (int b = blockIdx.x * GA_WARPS + warp; b < m_pad_blocks; b += gridDim.x * GA_WARPS) {
     if (b < m) {
       const int ib = col_idx[lo + b];
@@ -160,47 +198,52 @@ k_gather(const int32_t *__restrict__ row_ptr, const int32_t *__restrict__ col_id
       }
     }
     __syncwarp();
-    // Lane = row.  The six elements a row contributes to this block column are 24 contiguous bytes of
-    // the store (row o of block pos[a]): three 8-byte loads per matrix, then one 128-byte store
-    // instruction per column.
+    // Lane = two consecutive rows (always rows o, o+1 of one block, o even).  What they contribute to this
+    // block column are 48 contiguous bytes of the store: three 16-byte loads per matrix.
     const int c0 = b * NOLSM_BS;
-    float *hc = hj + (int64_t)c0 * ld;
-    float *sc = sj + (int64_t)c0 * ld;
-    for (int r = lane; r < P; r += 32) {
-      float hv[NOLSM_BS], sv[NOLSM_BS];
+    for (int r = 2 * lane; r < P; r += 64) {
+      float hv[2][NOLSM_BS], sv[2][NOLSM_BS];
 #pragma unroll
-      for (int p = 0; p < NOLSM_BS; ++p) hv[p] = sv[p] = 0.f;
+      for (int p = 0; p < NOLSM_BS; ++p) hv[0][p] = hv[1][p] = sv[0][p] = sv[1][p] = 0.f;
       if (c0 < n && r < n) {
         const int a = r / NOLSM_BS, o = r - a * NOLSM_BS;
         const int k = pos[a];
         if (k >= 0) {
-          const float2 *hp = reinterpret_cast<const float2 *>(h_val + (int64_t)k * 36 + o * NOLSM_BS);
-          const float2 *sp = reinterpret_cast<const float2 *>(s_val + (int64_t)k * 36 + o * NOLSM_BS);
-#pragma unroll
-          for (int q = 0; q < 3; ++q) {
-            const float2 x = __ldg(hp + q), y = __ldg(sp + q);
-            hv[2 * q] = x.x; hv[2 * q + 1] = x.y;
-            sv[2 * q] = y.x; sv[2 * q + 1] = y.y;
-          }
+          const float4 *hp = reinterpret_cast<const float4 *>(h_val + (int64_t)k * 36 + o * NOLSM_BS);
+          const float4 *sp = reinterpret_cast<const float4 *>(s_val + (int64_t)k * 36 + o * NOLSM_BS);
+          const float4 x0 = __ldg(hp), x1 = __ldg(hp + 1), x2 = __ldg(hp + 2);
+          const float4 y0 = __ldg(sp), y1 = __ldg(sp + 1), y2 = __ldg(sp + 2);
+          hv[0][0] = x0.x; hv[0][1] = x0.y; hv[0][2] = x0.z; hv[0][3] = x0.w; hv[0][4] = x1.x; hv[0][5] = x1.y;
+          hv[1][0] = x1.z; hv[1][1] = x1.w; hv[1][2] = x2.x; hv[1][3] = x2.y; hv[1][4] = x2.z; hv[1][5] = x2.w;
+          sv[0][0] = y0.x; sv[0][1] = y0.y; sv[0][2] = y0.z; sv[0][3] = y0.w; sv[0][4] = y1.x; sv[0][5] = y1.y;
+          sv[1][0] = y1.z; sv[1][1] = y1.w; sv[1][2] = y2.x; sv[1][3] = y2.y; sv[1][4] = y2.z; sv[1][5] = y2.w;
         }
       } else {
 #pragma unroll
-        for (int p = 0; p < NOLSM_BS; ++p) sv[p] = (r == c0 + p) ? 1.f : 0.f;   // identity padding of S
-      }
-#pragma unroll
-      for (int p = 0; p < NOLSM_BS; ++p) {
-        if (c0 + p < P) {
-          hc[(int64_t)p * ld + r] = hv[p];
-          sc[(int64_t)p * ld + r] = sv[p];
+        for (int p = 0; p < NOLSM_BS; ++p) {   // identity padding of S
+          sv[0][p] = (r == c0 + p) ? 1.f : 0.f;
+          sv[1][p] = (r + 1 == c0 + p) ? 1.f : 0.f;
         }
       }
+      emit_rows2(out, base, ld, c0, r, P, hv, sv);
     }
     __syncwarp();
   }
 }
 
+static BuildOut build_out(const nolsm_batch *b, float *h_out, float *s_out, bool split_s) {
+  BuildOut o;
+  o.h32 = h_out;
+  o.s32 = s_out;
+  o.h_hi = b->h[b->n_half - 2];
+  o.h_lo = b->h[b->n_half - 1];
+  o.s_hi = split_s ? b->h[b->n_half - 4] : nullptr;
+  o.s_lo = split_s ? b->h[b->n_half - 3] : nullptr;
+  return o;
+}
+
 cudaError_t launch_gather(const nolsm_batch *b, const int32_t *row_ptr, const int32_t *col_idx,
-                          const float *h_val, const float *s_val, float *h_out, float *s_out,
+                          const float *h_val, const float *s_val, float *h_out, float *s_out, bool split_s,
                           cudaStream_t st) {
   if (b->count == 0) return cudaSuccess;
   const int per_warp = (b->ld + NOLSM_BS - 1) / NOLSM_BS + 1;
@@ -208,7 +251,7 @@ cudaError_t launch_gather(const nolsm_batch *b, const int32_t *row_ptr, const in
   const int cols = (b->ld + NOLSM_BS - 1) / NOLSM_BS;
   dim3 grid((cols + GA_WARPS - 1) / GA_WARPS, b->count);
   k_gather<<<grid, GA_WARPS * 32, smem, st>>>(row_ptr, col_idx, h_val, s_val, b->mol_begin, b->ld,
-                                              (int64_t)b->ld * b->ld, h_out, s_out);
+                                              (int64_t)b->ld * b->ld, build_out(b, h_out, s_out, split_s));
   return cudaGetLastError();
 }
 
@@ -239,8 +282,7 @@ __device__ __forceinline__ double wrap_axis(double d, double len) {
 
 __global__ void __launch_bounds__(GA_WARPS * 32)
 k_generate(const int32_t *__restrict__ row_ptr, const int32_t *__restrict__ col_idx,
-           const __grid_constant__ ModelDev md, int mol_begin, int ld, int64_t slab, int m_cap,
-           float *__restrict__ h_out, float *__restrict__ s_out) {
+           const __grid_constant__ ModelDev md, int mol_begin, int ld, int64_t slab, int m_cap, BuildOut out) {
   extern __shared__ float s_gen[];  // [GA_WARPS][2][9 * m_cap]
   const int mat = blockIdx.y;
   const int j = mol_begin + mat;
@@ -252,8 +294,7 @@ k_generate(const int32_t *__restrict__ row_ptr, const int32_t *__restrict__ col_
   const int m_pad_blocks = (P + NOLSM_BS - 1) / NOLSM_BS;
   float *sv9 = s_gen + (size_t)warp * 18 * m_cap;
   float *hv9 = sv9 + 9 * m_cap;
-  float *hj = h_out + (int64_t)mat * slab;
-  float *sj = s_out + (int64_t)mat * slab;
+  const int64_t base = (int64_t)mat * slab;
   for (int b = blockIdx.x * GA_WARPS + warp; b < m_pad_blocks; b += gridDim.x * GA_WARPS) {
     if (b < m) {
       const int ib = col_idx[lo + b];
@@ -281,37 +322,43 @@ k_generate(const int32_t *__restrict__ row_ptr, const int32_t *__restrict__ col_
       }
     }
     __syncwarp();
-    for (int p = 0; p < NOLSM_BS; ++p) {
-      const int c = b * NOLSM_BS + p;
-      if (c >= P) break;
-      const int sp = (md.site_packed >> (2 * p)) & 3;
-      float *hc = hj + (int64_t)c * ld;
-      float *sc = sj + (int64_t)c * ld;
-      for (int r = lane; r < P; r += 32) {
-        float hv = 0.f, sv = 0.f;
-        if (c < n && r < n) {
-          const int a = r / NOLSM_BS, o = r - a * NOLSM_BS;
-          if (a == b && o == p) {
-            sv = 1.f;
-            hv = md.energy[o];
-          } else {
-            const int k = a * 9 + ((md.site_packed >> (2 * o)) & 3) * 3 + sp;
-            hv = hv9[k];
-            sv = sv9[k];
+    const int c0 = b * NOLSM_BS;
+    for (int r = 2 * lane; r < P; r += 64) {     // lane = rows o, o+1 of one block (o even), as in k_gather
+      float hv[2][NOLSM_BS], sv[2][NOLSM_BS];
+      if (c0 < n && r < n) {
+        const int a = r / NOLSM_BS, o = r - a * NOLSM_BS;
+#pragma unroll
+        for (int i = 0; i < 2; ++i) {
+          const int so3 = ((md.site_packed >> (2 * (o + i))) & 3) * 3;
+#pragma unroll
+          for (int p = 0; p < NOLSM_BS; ++p) {
+            if (a == b && o + i == p) {
+              sv[i][p] = 1.f;
+              hv[i][p] = md.energy[p];
+            } else {
+              const int k = a * 9 + so3 + ((md.site_packed >> (2 * p)) & 3);
+              hv[i][p] = hv9[k];
+              sv[i][p] = sv9[k];
+            }
           }
-        } else if (r == c) {
-          sv = 1.f;
         }
-        hc[r] = hv;
-        sc[r] = sv;
+      } else {
+#pragma unroll
+        for (int p = 0; p < NOLSM_BS; ++p) {
+          hv[0][p] = hv[1][p] = 0.f;
+          sv[0][p] = (r == c0 + p) ? 1.f : 0.f;
+          sv[1][p] = (r + 1 == c0 + p) ? 1.f : 0.f;
+        }
       }
+      emit_rows2(out, base, ld, c0, r, P, hv, sv);
     }
     __syncwarp();
   }
 }
 
 cudaError_t launch_generate(const nolsm_batch *b, const int32_t *row_ptr, const int32_t *col_idx,
-                            const nolsm_model *model, float *h_out, float *s_out, cudaStream_t st) {
+                            const nolsm_model *model, float *h_out, float *s_out, bool split_s,
+                            cudaStream_t st) {
   if (b->count == 0) return cudaSuccess;
   ModelDev md;
   md.pos = model->pos_q;
@@ -339,7 +386,7 @@ cudaError_t launch_generate(const nolsm_batch *b, const int32_t *row_ptr, const 
   const int cols = (b->ld + NOLSM_BS - 1) / NOLSM_BS;
   dim3 grid((cols + GA_WARPS - 1) / GA_WARPS, b->count);
   k_generate<<<grid, GA_WARPS * 32, smem, st>>>(row_ptr, col_idx, md, b->mol_begin, b->ld,
-                                                (int64_t)b->ld * b->ld, m_cap, h_out, s_out);
+                                                (int64_t)b->ld * b->ld, m_cap, build_out(b, h_out, s_out, split_s));
   return cudaGetLastError();
 }
 
