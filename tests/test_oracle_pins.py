@@ -161,6 +161,84 @@ def test_newton_schulz_inverse_limits(tiny_system):
     assert abs(sinv1[0, 0] - 0.25) < 1e-14
 
 
+# ------------------------------------------------------------------ readings 5, 7, 11: scalings and early stop
+def test_scaled_starts_stay_inside_the_convergence_intervals(tiny_system):
+    """DESIGN.md readings 5 and 7.  Eq. 9 acts on an eigenvalue as x -> x(3 - x^2)/2, which converges to
+    sign(x) exactly for 0 < |x| < sqrt(3); Eq. 16 acts on an eigenvalue of Z_k Y_k as v -> v(3 - v)^2/4, which
+    converges to 1 for 0 < v < 3.  So X0 = 1.5 A/bound and Y0 = 2 S/bound (bound >= spectral radius) are
+    valid starts, give the results of the unit scaling, and need no more iterations than it."""
+    xs = np.array([-1.5, -1.0, -0.3, 0.05, 0.8, 1.5, 1.7])
+    for _ in range(60):
+        xs = 0.5 * xs * (3.0 - xs * xs)
+    assert np.abs(xs - np.sign(xs)).max() < 1e-12
+    x_out = 1.75                                   # beyond sqrt(3): leaves the basin (sign flips)
+    for _ in range(60):
+        x_out = 0.5 * x_out * (3.0 - x_out * x_out)
+    assert not abs(x_out - 1.0) < 1e-6
+    vs = np.array([0.05, 0.5, 1.0, 1.5, 2.0, 2.9])
+    for _ in range(80):
+        vs = 0.25 * vs * (3.0 - vs) ** 2
+    assert np.abs(vs - 1.0).max() < 1e-12
+
+    s = tiny_system
+    nb = s.col_idx[s.row_ptr[5]:s.row_ptr[6]]
+    ssub = orc.dense_submatrix(s.row_ptr, s.col_idx, s.s_val, nb)
+    hsub = orc.dense_submatrix(s.row_ptr, s.col_idx, s.h_val, nb)
+    n = len(ssub)
+    a = np.linalg.solve(ssub, hsub) + 0.85 * np.eye(n)
+    lam, v = orc.generalized_eig(hsub, ssub)
+    ref = orc.sign_from_eig(lam, v, ssub, -0.85)
+    bound = np.sqrt(np.abs(a).sum(0).max() * np.abs(a).sum(1).max())
+    assert bound >= np.abs(lam + 0.85).max()
+    x1, r1 = orc.newton_schulz_sign(a, 40, scale=bound, history=True)
+    x2, r2 = orc.newton_schulz_sign(a, 40, scale=bound / 1.5, history=True)
+    x3 = orc.newton_schulz_sign(a, 60, scale=np.abs(lam + 0.85).max() / 1.5)      # |x|_max = 1.5 exactly
+    for x in (x1, x2, x3):
+        assert np.abs(x - ref).max() < 1e-9
+    first = lambda r: int(np.argmax(r < 1e-2))
+    assert first(r2) <= first(r1)
+
+    sb = np.sqrt(np.abs(ssub).sum(0).max() * np.abs(ssub).sum(1).max())
+    inv = np.linalg.inv(ssub)
+    i1, _, _, q1 = orc.newton_schulz_inverse(ssub, 40, scale=sb, history=True)
+    i2, _, _, q2 = orc.newton_schulz_inverse(ssub, 40, scale=sb / 2, history=True)
+    i3, _, _ = orc.newton_schulz_inverse(ssub, 60, scale=np.linalg.eigvalsh(ssub)[-1] / 2)   # v_max = 2 exactly
+    for i in (i1, i2, i3):
+        assert np.abs(i - inv).max() < 1e-10
+    first3 = lambda r: int(np.argmax(r < 3e-3))
+    assert first3(q2) <= first3(q1)
+
+
+def test_inverse_residual_recurrence_and_refined_early_stop(tiny_system):
+    """Reading 11.  With E_k = I - Z_k Y_k, Eq. 16 gives E_{k+1} = 3/4 E_k^2 + 1/4 E_k^3 exactly (V_{k+1} is a
+    polynomial in V_k).  Taking Z_k at the first r_k < 3e-3 WITHOUT finishing the iteration, S0 = Z_k^2/s has a
+    relative error of about 2 r_k, and one Newton step S0 + S0 (I - S S0) squares it."""
+    s = tiny_system
+    nb = s.col_idx[s.row_ptr[9]:s.row_ptr[10]]
+    ssub = orc.dense_submatrix(s.row_ptr, s.col_idx, s.s_val, nb)
+    n = len(ssub)
+    eye = np.eye(n)
+    c = 0.5 * max(1.0, np.sqrt(np.abs(ssub).sum(0).max() * np.abs(ssub).sum(1).max()))
+    prev = None
+    for k in range(0, 6):
+        _, zk, yk = orc.newton_schulz_inverse(ssub, k, scale=c)
+        e = eye - zk @ yk
+        if prev is not None:
+            assert np.abs(e - (0.75 * prev @ prev + 0.25 * prev @ prev @ prev)).max() < 1e-13
+        prev = e
+    _, _, _, res = orc.newton_schulz_inverse(ssub, 12, scale=c, history=True)
+    k_stop = int(np.argmax(res < 3e-3))
+    assert 0 < k_stop < 8
+    _, zk, _ = orc.newton_schulz_inverse(ssub, k_stop, scale=c)
+    s0 = zk @ zk / c
+    inv = np.linalg.inv(ssub)
+    rel0 = np.linalg.norm(s0 - inv, 2) / np.linalg.norm(inv, 2)
+    s1 = s0 + s0 @ (eye - ssub @ s0)
+    rel1 = np.linalg.norm(s1 - inv, 2) / np.linalg.norm(inv, 2)
+    assert rel0 < 4 * np.sqrt(n) * res[k_stop]          # ||E||_2 <= ||E||_F = sqrt(n) r_k
+    assert rel1 <= (np.linalg.cond(ssub) * rel0) ** 2 and rel1 < 1e-4
+
+
 # ------------------------------------------------------------------ Eq. 6 / 12 by eigenvectors
 def test_sign_and_density_identities(tiny_solution):
     sol = tiny_solution["solutions"][5]
