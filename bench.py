@@ -217,9 +217,9 @@ def run_native(args, system, rank, world, local_rank):
     h_val = torch.as_tensor(system.h_val).to(dev)
     s_val = torch.as_tensor(system.s_val).to(dev)
     mu_lo, mu_hi = 2 * MU, 0.0        # one evaluation at the midpoint mu = -0.85
-    if args.elements == "generated":   # T_j(H), T_j(S) evaluated on the device from the positions
+    if args.elements != "gathered":   # T_j(H), T_j(S) evaluated on the device from the positions
         import nolsm_inputs as gi
-        ctx.set_model(pos, **gi.model_parameters(system))
+        ctx.set_model(pos, eval_fp32=args.elements == "generated-fp32", **gi.model_parameters(system))
 
     def step():
         rp, ci = ctx.build_neighbours(pos, system.box_q, system.rc_q, cap=system.nnzb)
@@ -344,9 +344,9 @@ def main():
     ap.add_argument("--workspace-gib", type=float, default=24.0)
     ap.add_argument("--group", type=int, default=0, help="submatrices iterated together (0: from the L2 size)")
     ap.add_argument("--flags", type=int, default=0, help="NOLSM_FLAG_* bits (2: pair engine, 4: multicast engine)")
-    ap.add_argument("--elements", default="gathered", choices=["gathered", "generated"],
+    ap.add_argument("--elements", default="gathered", choices=["gathered", "generated", "generated-fp32"],
                     help="submatrix elements gathered from the block stores (the north_star path) or evaluated "
-                         "on the device from the positions (nolsm_set_model)")
+                         "on the device from the positions (nolsm_set_model; -fp32: FP32 + SFU as in PAPER.md:202)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()

@@ -156,9 +156,12 @@ nolsm_status nolsm_build_submatrices(nolsm_ctx *ctx, const nolsm_bsr *H, const n
  *         then per axis d -= L * rint(d / L), L = box_q * unit_per_grid;   r2 = (dx^2 + dy^2) + dz^2
  *   S   = s_ampl * exp(-0.5 * r2),   H = h_ampl * exp(-sqrt(r2) / h_len)
  *   ia == ib: o == p -> S = 1, H = orb_energy[o];  o != p on the same site -> S = H = 0.
- * Everything above is evaluated in FP64 with separately rounded operations in exactly that order and
- * the result rounded once to FP32 (so it can differ from a host evaluation only through exp()'s last
- * bit).  Pairs that are not stored give 0, padding is the identity, as in nolsm_build_submatrices. */
+ * eval_fp32 = 0: everything above is evaluated in FP64 with separately rounded operations in exactly that
+ * order and the result rounded once to FP32 (so it can differ from a host evaluation only through exp()'s
+ * last bit).  eval_fp32 = 1: the paper's choice ("computed in FP32 to make efficient use of
+ * the special function units"): FP32 arithmetic from the integer minimum image of the centre difference,
+ * __expf; elements then agree with the FP64 evaluation to about 1e-6 absolute.
+ * Pairs that are not stored give 0, padding is the identity, as in nolsm_build_submatrices. */
 typedef struct {
   const int32_t *pos_q;      /* device [n_mol*3], grid units in [0, box_q) */
   int32_t n_mol;
@@ -169,6 +172,7 @@ typedef struct {
   int32_t orb_site[6];       /* each in 0..2 */
   double orb_energy[6];
   double s_ampl, h_ampl, h_len;
+  int32_t eval_fp32;         /* 0: FP64 evaluation (bit-comparable), 1: FP32 + SFU */
 } nolsm_model;
 
 /* Attach (model != NULL; the struct is copied, pos_q stays caller-owned and must outlive its use) or

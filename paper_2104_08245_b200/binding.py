@@ -50,7 +50,7 @@ class _Model(C.Structure):
     _fields_ = [("pos_q", C.c_void_p), ("n_mol", C.c_int32), ("box_q", C.c_int32 * 3), ("rc_q", C.c_int32),
                 ("unit_per_grid", C.c_double), ("site_offset", (C.c_double * 3) * 3), ("orb_site", C.c_int32 * 6),
                 ("orb_energy", C.c_double * 6), ("s_ampl", C.c_double), ("h_ampl", C.c_double),
-                ("h_len", C.c_double)]
+                ("h_len", C.c_double), ("eval_fp32", C.c_int32)]
 
 
 class SignStats(C.Structure):
@@ -274,7 +274,7 @@ class Context:
 
     # a1' ----------------------------------------------------------------------------------------
     def set_model(self, pos_q=None, box_q=None, rc_q=0, unit_per_grid=1.0, site_offset=None, orb_site=None,
-                  orb_energy=None, s_ampl=0.0, h_ampl=0.0, h_len=1.0):
+                  orb_energy=None, s_ampl=0.0, h_ampl=0.0, h_len=1.0, eval_fp32=False):
         """Attach the two-centre model of nolsm.h (nolsm_model): submatrix builds then evaluate the elements
         from pos_q (int32 CUDA tensor [n_mol,3], kept alive here) instead of gathering.  pos_q=None detaches."""
         if pos_q is None:
@@ -295,6 +295,7 @@ class Context:
             m.orb_site[o] = int(orb_site[o])
             m.orb_energy[o] = float(orb_energy[o])
         m.s_ampl, m.h_ampl, m.h_len = float(s_ampl), float(h_ampl), float(h_len)
+        m.eval_fp32 = 1 if eval_fp32 else 0
         self._check(self.lib.nolsm_set_model(self.handle, C.byref(m)))
         self._model_pos = pos_q
 

@@ -274,7 +274,13 @@ struct ModelDev {
   double s_ampl, h_ampl, h_len;
   float energy[NOLSM_BS];
   uint32_t site_packed;  // 2 bits per basis function
+  int32_t fp32;          // evaluate in FP32 with the SFU exponential instead of FP64
 };
+
+__device__ __forceinline__ int32_t wrap_int(int32_t d, int32_t box) {
+  const int32_t h = box >> 1;
+  return d > h ? d - box : (d < -h ? d + box : d);
+}
 
 __device__ __forceinline__ double wrap_axis(double d, double len) {
   return __dsub_rn(d, __dmul_rn(len, rint(__ddiv_rn(d, len))));
@@ -306,7 +312,24 @@ k_generate(const int32_t *__restrict__ row_ptr, const int32_t *__restrict__ col_
         const int32_t xa = md.pos[3 * ia], ya = md.pos[3 * ia + 1], za = md.pos[3 * ia + 2];
         float sv = 0.f, hv = 0.f;
         const bool stored = min_image_sq(xa, ya, za, xb, yb, zb, md.box[0], md.box[1], md.box[2]) <= md.rc2;
-        if (stored && !(ia == ib && so == sp)) {
+        if (stored && !(ia == ib && so == sp) && md.fp32) {
+          // The paper's choice: FP32 arithmetic, transcendental functions on the special
+          // function units.  The centre difference is reduced to its minimum image in integers (exact),
+          // the site offsets can push a component past half the box, hence one more wrap.
+          const float unit = (float)md.unit;
+          float d[3] = {(float)wrap_int(xa - xb, md.box[0]) * unit, (float)wrap_int(ya - yb, md.box[1]) * unit,
+                        (float)wrap_int(za - zb, md.box[2]) * unit};
+          float r2 = 0.f;
+#pragma unroll
+          for (int ax = 0; ax < 3; ++ax) {
+            const float len = (float)md.len[ax];
+            float x = d[ax] + (float)(md.off[so][ax] - md.off[sp][ax]);
+            x -= len * rintf(x / len);
+            r2 = fmaf(x, x, r2);
+          }
+          sv = (float)md.s_ampl * __expf(-0.5f * r2);
+          hv = (float)md.h_ampl * __expf(-sqrtf(r2) / (float)md.h_len);
+        } else if (stored && !(ia == ib && so == sp)) {
           double dx = __dmul_rn((double)(xa - xb), md.unit);
           double dy = __dmul_rn((double)(ya - yb), md.unit);
           double dz = __dmul_rn((double)(za - zb), md.unit);
@@ -377,6 +400,7 @@ cudaError_t launch_generate(const nolsm_batch *b, const int32_t *row_ptr, const 
   md.s_ampl = model->s_ampl;
   md.h_ampl = model->h_ampl;
   md.h_len = model->h_len;
+  md.fp32 = model->eval_fp32;
   const int m_cap = (b->ld + NOLSM_BS - 1) / NOLSM_BS + 1;
   const size_t smem = (size_t)GA_WARPS * 18 * m_cap * sizeof(float);
   if (smem > 48 * 1024) {

@@ -601,11 +601,11 @@ def test_run_to_run_bitwise_identical(nolsm, flag):
 # ---------------------------------------------------------------------------------------------
 # a1': elements evaluated on the device from the positions instead of gathered
 # ---------------------------------------------------------------------------------------------
-def _attach_model(nolsm, ctx, system):
+def _attach_model(nolsm, ctx, system, eval_fp32=False):
     import torch
     import nolsm_inputs as gi
     pos = torch.as_tensor(system.pos_q).contiguous().cuda()
-    ctx.set_model(pos, **gi.model_parameters(system))
+    ctx.set_model(pos, eval_fp32=eval_fp32, **gi.model_parameters(system))
     return pos
 
 
@@ -644,6 +644,32 @@ def test_generated_submatrices_match_block_store(nolsm, tiny_system, mid_system,
     ref = orc.dense_submatrix(system.row_ptr, system.col_idx, system.h_val,
                               system.col_idx[system.row_ptr[begin]:system.row_ptr[begin + 1]]).astype(np.float32)
     assert np.array_equal(batch.read(0, nolsm.MAT_H).cpu().numpy(), ref)
+    ctx.close()
+
+
+@pytest.mark.parametrize("which", ["tiny9", "mid"])
+def test_generated_submatrices_fp32_sfu(nolsm, mid_system, which):
+    """The paper's own flavour (FP32 arithmetic, SFU exponentials): same zero pattern, elements
+    within 1e-6 of the FP64 evaluation (|S|, |H| <= 1; __expf is good to 2^-21 relative, r^2 to 1e-6 A^2)."""
+    import oracle.nolsm_oracle as orc
+    import nolsm_inputs as gi
+    system = mid_system if which == "mid" else gi.make_water_system(32, 9.0)
+    H, S = _device_system(nolsm, system)
+    ctx = nolsm.Context()
+    _attach_model(nolsm, ctx, system, eval_fp32=True)
+    count = 12 if which == "mid" else system.n_mol
+    begin = 60 if which == "mid" else 0
+    batch = ctx.build_submatrices(H, S, begin, count)
+    worst = 0.0
+    for local in ([0, count - 1] if which == "mid" else range(0, count, 5)):
+        j = begin + local
+        nbrs = system.col_idx[system.row_ptr[j]:system.row_ptr[j + 1]]
+        for mat, val in ((nolsm.MAT_H, system.h_val), (nolsm.MAT_S, system.s_val)):
+            ref = orc.dense_submatrix(system.row_ptr, system.col_idx, val, nbrs)
+            got = batch.read(local, mat).cpu().numpy()
+            assert np.array_equal(got == 0, ref == 0)
+            worst = max(worst, float(np.abs(got - ref).max()))
+    assert worst < 1e-6, worst
     ctx.close()
 
 
