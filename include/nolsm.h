@@ -70,6 +70,12 @@ typedef struct {
   int32_t group;            /* submatrices iterated together so their iterates stay L2-resident
                                (<= 0: chosen from the L2 size) */
   int32_t flags;            /* NOLSM_FLAG_* */
+  int64_t cache_bytes;      /* nolsm_solve_mu with several mu steps, batches streamed through the workspace:
+                               upper bound on the device memory used to keep B_j and the own columns of S_j^-1
+                               of every submatrix from the first step, so that later steps skip a1-a3 (gather,
+                               Eq. 15-17, refinement, B = S^-1 H).  0: what is free at the call, less
+                               workspace_bytes and 4 GiB;  < 0: off.  4 (n_j^2 + 6 ld) bytes per submatrix; when
+                               that does not fit, the steps recompute.  Freed before the call returns. */
 } nolsm_config;
 
 /* Engine of the matrix iterations.  With none of PAIR / MCAST / SINGLE set the context picks per batch:
@@ -111,6 +117,7 @@ typedef struct {            /* filled by nolsm_solve_mu (host struct) */
   int32_t mu_steps;         /* N(mu) evaluations performed */
   int32_t n_batches;
   int32_t resident;         /* 1 if every batch stayed in the workspace across mu steps (S^-1, B reused) */
+  int32_t cached;           /* 1 if B_j and S_j^-1[:,own] were kept in the operator cache instead (cache_bytes) */
   double mu_lo, mu_hi;      /* final bracket */
   double ne_diag;           /* cross-check: sum_j sum_{c in own_j} (1 - X_cc) of the last step (reading 15) */
   nolsm_sign_stats last;    /* statistics of the last mu step, summed over batches */

@@ -990,9 +990,40 @@ extern "C" nolsm_status nolsm_solve_mu(nolsm_ctx *ctx, const nolsm_bsr *H, const
   }
   std::vector<nolsm_batch *> live(plan.size(), nullptr);
 
+  // Operator cache (nolsm_config.cache_bytes): streamed batches lose S^-1 and B between mu steps; keeping
+  // B_j (FP32, padded slab) and the own columns of S_j^-1 lets steps 2.. start at the sign iteration.
+  float *cache = nullptr;
+  std::vector<size_t> cache_off(plan.size() + 1, 0), cache_sq(plan.size(), 0);
+  if (!resident && max_steps > 1 && ctx->cfg.cache_bytes >= 0 && !use_simt(ctx) && ctx->umma_ok) {
+    for (size_t bi = 0; bi < plan.size(); ++bi) {
+      int max_n = 0;
+      size_t sq = 0;     // B_j packed to its true n_j x n_j part
+      for (int i = 0; i < plan[bi].count; ++i) {
+        const int n = dims[plan[bi].begin + i];
+        max_n = std::max(max_n, n);
+        sq += (size_t)n * n;
+      }
+      const size_t ld = (size_t)std::max(NOLSM_PAD, round_up(max_n, NOLSM_PAD));
+      cache_sq[bi] = sq;
+      cache_off[bi + 1] = cache_off[bi] + sq + (size_t)plan[bi].count * NOLSM_BS * ld;
+    }
+    size_t free_b = 0, total_b = 0;
+    size_t cap = ctx->cfg.cache_bytes > 0 ? (size_t)ctx->cfg.cache_bytes : 0;
+    if (cap == 0 && cudaMemGetInfo(&free_b, &total_b) == cudaSuccess) {
+      // everything that is free now, less the workspace bound (it may not be allocated yet) and 4 GiB
+      const size_t reserve = ws + ((size_t)4 << 30);
+      cap = free_b > reserve ? free_b - reserve : 0;
+    }
+    const size_t need = cache_off.back() * sizeof(float);
+    if (need > 0 && need <= cap && cudaMalloc(&cache, need) != cudaSuccess) { cudaGetLastError(); cache = nullptr; }
+  }
+
   cudaEvent_t tev[5];
   for (int i = 0; i < 5; ++i) cudaEventCreate(&tev[i]);
-  auto cleanup = [&]() { for (int i = 0; i < 5; ++i) cudaEventDestroy(tev[i]); };
+  auto cleanup = [&]() {
+    for (int i = 0; i < 5; ++i) cudaEventDestroy(tev[i]);
+    if (cache) { cudaStreamSynchronize(st); cudaFree(cache); }
+  };
 
   double lo = mu_lo, hi = mu_hi, mu = 0.5 * (lo + hi), ne = 0.0;
   int step = 0;
@@ -1008,7 +1039,25 @@ extern "C" nolsm_status nolsm_solve_mu(nolsm_ctx *ctx, const nolsm_bsr *H, const
       nolsm_batch *b = live[bi];
       const bool timed = stats != nullptr;
       if (timed) cudaEventRecord(tev[0], st);
-      if (!b || !resident) {
+      float *cache_b = cache ? cache + cache_off[bi] : nullptr;
+      if (cache && step > 0) {
+        // operands of this batch from the cache: B -> u3, own columns of S^-1 -> u2
+        std::vector<int32_t> bd(dims.begin() + r.begin, dims.begin() + r.begin + r.count);
+        rc = setup_batch(ctx, 0, bd, r.begin, true, units, &b, st);
+        if (rc != NOLSM_OK) break;
+        const size_t slab_all = cache_sq[bi];
+        ctx->launches += 2;
+        // the padded part of u3 may hold anything: the sign stage only reads the true n x n part of B
+        if (launch_pack_square(b, b->u[3], cache_b, false, st) != cudaSuccess) {
+          ctx->err = "solve_mu: copy from the operator cache failed"; rc = NOLSM_ECUDA; break;
+        }
+        if (launch_own_columns(b, H->row_ptr, H->col_idx, b->u[2], cache_b + slab_all, false, st) != cudaSuccess) {
+          ctx->err = "solve_mu: restoring the own columns of S^-1 failed"; rc = NOLSM_ECUDA; break;
+        }
+        b->engine_simt = false;
+        b->prepared = true;
+        b->prepared_precision = prec;
+      } else if (!b || !resident) {
         rc = build_submatrices_impl(ctx, H, S, r.begin, r.count, resident ? (int)bi : 0, units, &b, st);
         if (rc != NOLSM_OK) break;
         live[bi] = resident ? b : nullptr;
@@ -1020,6 +1069,16 @@ extern "C" nolsm_status nolsm_solve_mu(nolsm_ctx *ctx, const nolsm_bsr *H, const
       if (!b->prepared) {
         rc = prepare_batch(ctx, b, prec, st, stats ? &bs : nullptr, &gemms);
         if (rc != NOLSM_OK) break;
+        if (cache) {
+          const size_t slab_all = cache_sq[bi];
+          ctx->launches += 2;
+          if (launch_pack_square(b, b->u[3], cache_b, true, st) != cudaSuccess) {
+            ctx->err = "solve_mu: copy to the operator cache failed"; rc = NOLSM_ECUDA; break;
+          }
+          if (launch_own_columns(b, H->row_ptr, H->col_idx, b->u[2], cache_b + slab_all, true, st) != cudaSuccess) {
+            ctx->err = "solve_mu: saving the own columns of S^-1 failed"; rc = NOLSM_ECUDA; break;
+          }
+        }
       }
       if (timed) cudaEventRecord(tev[2], st);
       rc = sign_batch(ctx, b, mu, prec, tol, max_iter, fixed_iter, nullptr, st, timed);
@@ -1082,6 +1141,7 @@ extern "C" nolsm_status nolsm_solve_mu(nolsm_ctx *ctx, const nolsm_bsr *H, const
   if (stats) {
     stats->n_batches = (int)plan.size();
     stats->resident = resident ? 1 : 0;
+    stats->cached = cache ? 1 : 0;
     stats->mu_lo = lo;
     stats->mu_hi = hi;
     if (rc == NOLSM_OK && stats->last.n_unconverged > 0 && fixed_iter <= 0) {

@@ -171,6 +171,10 @@ cudaError_t launch_generate(const nolsm_batch *b, const int32_t *row_ptr, const 
 cudaError_t launch_gather(const nolsm_batch *b, const int32_t *row_ptr, const int32_t *col_idx,
                           const float *h_val, const float *s_val, float *h_out, float *s_out, bool split_s,
                           cudaStream_t st);
+// own columns of S^-1 (u2) to / from a packed [count][6][ld] array (operator cache of nolsm_solve_mu)
+cudaError_t launch_pack_square(const nolsm_batch *b, float *dense, float *packed, bool save, cudaStream_t st);
+cudaError_t launch_own_columns(const nolsm_batch *b, const int32_t *row_ptr, const int32_t *col_idx, float *mat,
+                               float *packed, bool save, cudaStream_t st);
 cudaError_t launch_density(const nolsm_batch *b, const float *x, const float *x_alt, const float *sinv,
                            const int32_t *row_ptr, const int32_t *col_idx, float *d_val,
                            double *ne_diag, cudaStream_t st);

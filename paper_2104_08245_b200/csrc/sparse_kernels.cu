@@ -421,6 +421,73 @@ cudaError_t launch_generate(const nolsm_batch *b, const int32_t *row_ptr, const 
 // One thread per row r, the six own columns of S^-1 staged in shared memory, X read column by
 // column (coalesced).  Also accumulates the diagonal estimate sum_{c in own}(1 - X_cc) (reading 15).
 // ------------------------------------------------------------------------------------------------
+// Operator cache of nolsm_solve_mu: the true n_j x n_j part of every slab of a batch to / from a dense
+// packing (submatrix m at offset sum_{i<m} n_i^2, leading dimension n_m).  grid (count, PK_SPLIT).
+#define PK_SPLIT 8
+__global__ void __launch_bounds__(256)
+k_pack_square(const int32_t *__restrict__ dims, int ld, int64_t slab, float *__restrict__ dense,
+              float *__restrict__ packed, int save) {
+  __shared__ long long s_part[8];
+  __shared__ long long s_off;
+  const int m = blockIdx.x;
+  long long acc = 0;
+  for (int i = threadIdx.x; i < m; i += blockDim.x) acc += (long long)dims[i] * dims[i];
+  for (int d = 16; d > 0; d >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, d);
+  if ((threadIdx.x & 31) == 0) s_part[threadIdx.x >> 5] = acc;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    long long t = 0;
+    for (int w = 0; w < 8; ++w) t += s_part[w];
+    s_off = t;
+  }
+  __syncthreads();
+  const int n = dims[m];          // a multiple of 6: rows in pairs
+  const int h = n >> 1;
+  float2 *pk = reinterpret_cast<float2 *>(packed + s_off);
+  float *dj = dense + (int64_t)m * slab;
+  const int64_t total = (int64_t)h * n;
+  for (int64_t idx = (int64_t)blockIdx.y * blockDim.x + threadIdx.x; idx < total; idx += (int64_t)PK_SPLIT * blockDim.x) {
+    const int c = (int)(idx / h), r2 = (int)(idx - (int64_t)c * h);
+    float2 *dp = reinterpret_cast<float2 *>(dj + (int64_t)c * ld) + r2;
+    if (save) pk[idx] = *dp; else *dp = pk[idx];
+  }
+}
+
+cudaError_t launch_pack_square(const nolsm_batch *b, float *dense, float *packed, bool save, cudaStream_t st) {
+  if (b->count == 0) return cudaSuccess;
+  k_pack_square<<<dim3(b->count, PK_SPLIT), 256, 0, st>>>(b->d_dims, b->ld, (int64_t)b->ld * b->ld, dense, packed,
+                                                          save ? 1 : 0);
+  return cudaGetLastError();
+}
+
+// Operator cache of nolsm_solve_mu: the six own columns of S_j^-1 to / from a packed [count][6][ld] array.
+__global__ void __launch_bounds__(256)
+k_own_columns(const int32_t *__restrict__ row_ptr, const int32_t *__restrict__ col_idx, int mol_begin, int ld,
+              int64_t slab, float *__restrict__ mat, float *__restrict__ packed, int save) {
+  const int m_ = blockIdx.x;
+  const int j = mol_begin + m_;
+  const int lo = row_ptr[j];
+  const int m = row_ptr[j + 1] - lo;
+  int l = 0, r_ = m;
+  while (l < r_) {   // position of j in its own (sorted) neighbour list
+    const int mid = (l + r_) >> 1;
+    if (col_idx[lo + mid] < j) l = mid + 1; else r_ = mid;
+  }
+  float *src = mat + (int64_t)m_ * slab + (int64_t)l * NOLSM_BS * ld;   // six consecutive columns
+  float *pk = packed + (int64_t)m_ * NOLSM_BS * ld;
+  for (int t = threadIdx.x; t < NOLSM_BS * ld; t += blockDim.x) {
+    if (save) pk[t] = src[t]; else src[t] = pk[t];
+  }
+}
+
+cudaError_t launch_own_columns(const nolsm_batch *b, const int32_t *row_ptr, const int32_t *col_idx, float *mat,
+                               float *packed, bool save, cudaStream_t st) {
+  if (b->count == 0) return cudaSuccess;
+  k_own_columns<<<b->count, 256, 0, st>>>(row_ptr, col_idx, b->mol_begin, b->ld, (int64_t)b->ld * b->ld, mat,
+                                          packed, save ? 1 : 0);
+  return cudaGetLastError();
+}
+
 #define DN_THREADS 128
 
 __global__ void __launch_bounds__(DN_THREADS)

@@ -750,3 +750,24 @@ def test_unit_scale_flag_same_result_more_iterations(nolsm, tiny_system, tiny_so
         ctx.close()
     assert iters[nolsm.FLAG_UNIT_SCALE][0] >= iters[0][0] and iters[nolsm.FLAG_UNIT_SCALE][1] >= iters[0][1]
     assert iters[nolsm.FLAG_UNIT_SCALE][2] >= iters[0][2]
+
+
+@pytest.mark.parametrize("precision", [0, 1])
+def test_operator_cache_bitwise_same_as_recomputing(nolsm, mid_system, precision):
+    """Several mu steps with the batches streamed through a small workspace: keeping B_j and the own columns
+    of S_j^-1 from the first step (nolsm_config.cache_bytes) must give exactly the mu, N and D of redoing
+    a1-a3 in every step."""
+    import torch
+    system = mid_system
+    H, S = _device_system(nolsm, system)
+    out = {}
+    for cache_bytes in (0, -1):
+        ctx = nolsm.Context(nolsm.Config(precision=precision, workspace_bytes=384 << 20, cache_bytes=cache_bytes))
+        mu, ne, D, st = ctx.solve_mu(H, S, system.n_electrons, -1.2, -0.6, tol_ne_per_mol=-1.0, max_steps=3)
+        assert st.resident == 0 and st.n_batches > 1 and st.mu_steps == 3
+        assert st.cached == (1 if cache_bytes == 0 else 0)
+        out[cache_bytes] = (mu, ne, D.val.clone())
+        ctx.close()
+    assert out[0][0] == out[-1][0], (out[0][0], out[-1][0])
+    assert abs(out[0][1] - out[-1][1]) < 1e-7, (out[0][1], out[-1][1])      # N is summed with FP64 atomics
+    assert torch.equal(out[0][2], out[-1][2])
