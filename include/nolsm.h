@@ -217,7 +217,10 @@ nolsm_status nolsm_scatter_density(nolsm_ctx *ctx, const nolsm_batch *batch, con
  * |N(mu) - n_electrons| <= tol_ne_per_mol * n_mol or after max_steps evaluations (tol_ne_per_mol < 0:
  * always run exactly max_steps evaluations, the timing workload of BASELINE configs[1]);
  * N(mu) > N_e -> mu_hi = mu else mu_lo = mu.  D holds the density of the last evaluated mu.
- * mu_out, ne_out: host doubles.  q_mol: device double [n_mol] or NULL.  Synchronises once per step. */
+ * mu_out, ne_out: host doubles.  q_mol: device double [n_mol] or NULL.  Synchronises once per step.
+ * The sign iteration stops as nolsm_sign_batched does, but its finishing update X_{k+1} = X_k + 1/2 X_k E_k
+ * is applied to the own columns of S_j^-1 only (X_{k+1} V = X_k (V + 1/2 E_k V)) instead of being formed;
+ * the iteration counts in the statistics include it (reading 9). */
 nolsm_status nolsm_solve_mu(nolsm_ctx *ctx, const nolsm_bsr *H, const nolsm_bsr *S, double n_electrons,
                             double mu_lo, double mu_hi, double tol_ne_per_mol, int32_t max_steps,
                             int32_t precision, nolsm_bsr *D, double *mu_out /*host*/,

@@ -610,7 +610,7 @@ static nolsm_status prepare_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, int prec
 // (reading 9) comes out of the first product's epilogue.  One kernel launch for all iterations.
 static nolsm_status sign_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, double mu, int precision, float tol,
                                      int max_iter, int fixed_iter, const float *scale_in, cudaStream_t st,
-                                     bool timed) {
+                                     bool timed, bool fold_last) {
   const bool fp16 = precision == NOLSM_FP16_FP32;
   float *Bm = b->u[3], *X32 = b->u[0];
   if (!scale_in) LAUNCH(ctx, launch_norm_bound(b, Bm, (float)mu, false, b->d_norm, st));
@@ -620,6 +620,11 @@ static nolsm_status sign_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, double mu, 
   pg.max_iter = max_iter;
   pg.fixed_iter = fixed_iter > 0 ? fixed_iter : 0;
   pg.tol = tol;
+  // fold_last: stop right after the E_k that passes the test; the caller applies X_{k+1} = X_k + 1/2 X_k E_k
+  // only to the own columns of S^-1 (k_last_half), instead of forming it with an n^3 product
+  pg.stop_early = fold_last ? 1 : 0;
+  b->x_pending = fold_last;
+  b->x_pending_split = fold_last && !fp16;
   ChainOp &e = pg.ops[0] = make_op(EPI_IDENT, 1.f, 0.f);
   ChainOp &x = pg.ops[1] = make_op(EPI_AXPBY, 0.5f, 1.f);
   e.resid = 1;
@@ -784,9 +789,11 @@ static nolsm_status prepare_batch(nolsm_ctx *ctx, nolsm_batch *b, int precision,
 
 // timed: records ctx->tev[0..1] around the chain kernel; read with chain_ms() after a synchronise
 static nolsm_status sign_batch(nolsm_ctx *ctx, nolsm_batch *b, double mu, int precision, float tol, int max_iter,
-                               int fixed_iter, const float *scale_in, cudaStream_t st, bool timed) {
+                               int fixed_iter, const float *scale_in, cudaStream_t st, bool timed,
+                               bool fold_last = false) {
+  b->x_pending = false;
   if (b->engine_simt) return sign_batch_simt(ctx, b, mu, tol, max_iter, fixed_iter, scale_in, st);
-  return sign_batch_chain(ctx, b, mu, precision, tol, max_iter, fixed_iter, scale_in, st, timed);
+  return sign_batch_chain(ctx, b, mu, precision, tol, max_iter, fixed_iter, scale_in, st, timed, fold_last);
 }
 
 static float chain_ms(nolsm_ctx *ctx, const nolsm_batch *b) {
@@ -816,6 +823,13 @@ static nolsm_status collect_stats(nolsm_ctx *ctx, nolsm_batch *b, float tol, int
   s->worst_residual = 0.f;
   s->flops_sign = s->flops_sign_padded = 0.0;
   for (int m = 0; m < b->count; ++m) {
+    // a folded last iteration: the chain counted the iterations it carried out in full and ran one product more
+    const int extra = b->x_pending ? 1 : 0;
+    const double n3 = (double)b->n_host[m] * b->n_host[m] * b->n_host[m];
+    const double P3 = (double)round_up(b->n_host[m], NOLSM_TILE_M) * round_up(b->n_host[m], 64) * round_up(b->n_host[m], 64);
+    s->flops_sign -= extra * 2.0 * n3;          // (2 it + 1) products instead of 2 (it + 1)
+    s->flops_sign_padded -= extra * 2.0 * P3;
+    it[m] += extra;
     s->iter_min = std::min(s->iter_min, it[m]);
     s->iter_max = std::max(s->iter_max, it[m]);
     s->iter_sum += it[m];
@@ -885,8 +899,26 @@ extern "C" nolsm_status nolsm_scatter_density(nolsm_ctx *ctx, const nolsm_batch 
     return NOLSM_EINVAL;
   }
   cudaStream_t st = (cudaStream_t)stream;
+  float *u_thin = nullptr;
+  if (batch->x_pending) {
+    nolsm_batch *bm = const_cast<nolsm_batch *>(batch);
+    const size_t need = (size_t)2 * batch->count * NOLSM_BS * batch->ld;   // same scratch as the energy products
+    if (need > bm->thin_cap) {
+      cudaStreamSynchronize(st);
+      cudaFree(bm->d_thin);
+      bm->d_thin = nullptr;
+      bm->thin_cap = 0;
+      if (cudaMalloc(&bm->d_thin, need * sizeof(float)) != cudaSuccess) {
+        cudaGetLastError();
+        ctx->err = "cudaMalloc of the thin-product scratch failed";
+        return NOLSM_ENOMEM;
+      }
+      bm->thin_cap = need;
+    }
+    u_thin = bm->d_thin;
+  }
   LAUNCH(ctx, launch_density(batch, x_ptr(batch), nullptr, sinv_ptr(batch), S->row_ptr, S->col_idx, D->val,
-                             ne_diag, st));
+                             ne_diag, batch->h[4], batch->x_pending_split ? batch->h[5] : nullptr, u_thin, st));
   LAUNCH(ctx, launch_trace(batch, S->row_ptr, S->col_idx, D->val, S->val, ne_partial, q_mol, st));
   return NOLSM_OK;
 }
@@ -897,6 +929,7 @@ extern "C" nolsm_status nolsm_scatter_energy(nolsm_ctx *ctx, nolsm_batch *batch,
   if (!ctx || !batch) return NOLSM_EINVAL;
   CHECK(check_bsr(ctx, H, "H"));
   if (!batch->sparse || !batch->prepared) { ctx->err = "batch has no sign iterate (call nolsm_sign_batched first)"; return NOLSM_EINVAL; }
+  if (batch->x_pending) { ctx->err = "internal: the energy products need the finished sign iterate"; return NOLSM_EINVAL; }
   cudaStream_t st = (cudaStream_t)stream;
   if (W) {
     CHECK(check_bsr(ctx, W, "W"));
@@ -1081,7 +1114,8 @@ extern "C" nolsm_status nolsm_solve_mu(nolsm_ctx *ctx, const nolsm_bsr *H, const
         }
       }
       if (timed) cudaEventRecord(tev[2], st);
-      rc = sign_batch(ctx, b, mu, prec, tol, max_iter, fixed_iter, nullptr, st, timed);
+      // the last iteration is folded into the density columns unless W needs the iterate itself
+      rc = sign_batch(ctx, b, mu, prec, tol, max_iter, fixed_iter, nullptr, st, timed, !ctx->eval_energy);
       if (rc != NOLSM_OK) break;
       if (timed) cudaEventRecord(tev[3], st);
       rc = nolsm_scatter_density(ctx, b, S, D, ctx->d_scalars, q_mol, ctx->d_scalars + 1, st);
@@ -1111,7 +1145,7 @@ extern "C" nolsm_status nolsm_solve_mu(nolsm_ctx *ctx, const nolsm_bsr *H, const
         acc.flops_sign_padded += cs.flops_sign_padded;
         acc.flops_prepare += bs.flops_prepare;
         acc.inv_iter_max = std::max(acc.inv_iter_max, bs.inv_iter_max);
-        acc.gemms += gemms + 2 * cs.iter_sum;
+        acc.gemms += gemms + 2 * cs.iter_sum - (b->x_pending ? b->count : 0);
       }
     }
     if (rc != NOLSM_OK) break;

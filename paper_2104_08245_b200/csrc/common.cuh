@@ -78,6 +78,9 @@ struct nolsm_batch {
   int32_t count = 0, ld = 0, mol_begin = 0, max_n = 0, slot = 0;
   float inv_scale = 0.5f;         // s_S = inv_scale * max(1, bound)   (reading 7; 1 with NOLSM_FLAG_UNIT_SCALE)
   float sign_scale = 1.f / 1.5f;  // s_j = sign_scale * bound          (reading 5; 1 with NOLSM_FLAG_UNIT_SCALE)
+  bool x_pending = false;         // the sign chain stopped after E_k = I - X_k^2 passed the test: the update
+                                  // X_{k+1} = X_k + 1/2 X_k E_k is folded into the density columns (reading 9)
+  bool x_pending_split = false;   // E_k is stored as hi + lo (FP32 mode)
   bool s_split_built = false;     // the builder wrote the split copy of S into h[n_half-4], h[n_half-3]
   bool prefer_pair = false;       // batch shape favours the pair engine (nolsm.h, NOLSM_FLAG_*)
   bool engine_simt = false;       // prepared by the FP32 SIMT debugging path (different buffer roles)
@@ -177,7 +180,8 @@ cudaError_t launch_own_columns(const nolsm_batch *b, const int32_t *row_ptr, con
                                float *packed, bool save, cudaStream_t st);
 cudaError_t launch_density(const nolsm_batch *b, const float *x, const float *x_alt, const float *sinv,
                            const int32_t *row_ptr, const int32_t *col_idx, float *d_val,
-                           double *ne_diag, cudaStream_t st);
+                           double *ne_diag, const __half *e_hi, const __half *e_lo, float *u_thin,
+                           cudaStream_t st);
 cudaError_t launch_trace(const nolsm_batch *b, const int32_t *row_ptr, const int32_t *col_idx,
                          const float *d_val, const float *s_val, double *ne, double *q_mol,
                          cudaStream_t st);

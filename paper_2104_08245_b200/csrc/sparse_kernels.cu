@@ -494,8 +494,11 @@ __global__ void __launch_bounds__(DN_THREADS)
 k_density(const int32_t *__restrict__ row_ptr, const int32_t *__restrict__ col_idx, int mol_begin,
           int ld, int64_t slab, const float *__restrict__ x, const float *__restrict__ x_alt,
           const int32_t *__restrict__ iters, const float *__restrict__ sinv,
+          const float *__restrict__ u_thin, const __half *__restrict__ e_hi, const __half *__restrict__ e_lo,
           float *__restrict__ d_val, double *__restrict__ ne_diag) {
-  extern __shared__ __align__(16) float s_sinv[];  // [n][6]: the six own columns of S^-1, row k contiguous
+  // [n][6], row k contiguous: the six own columns V of S^-1, or (u_thin set: last iteration folded in,
+  // see k_last_half) U = V + 1/2 E V, so that X U = X_{k+1} V
+  extern __shared__ __align__(16) float s_sinv[];
   const int mat = blockIdx.y;
   const int j = mol_begin + mat;
   const int lo = row_ptr[j];
@@ -510,9 +513,10 @@ k_density(const int32_t *__restrict__ row_ptr, const int32_t *__restrict__ col_i
   const int own0 = l * NOLSM_BS;
   const float *xj = ((x_alt != nullptr && (iters[mat] & 1)) ? x_alt : x) + (int64_t)mat * slab;
   const float *sj = sinv + (int64_t)mat * slab;
+  const float *uj = u_thin ? u_thin + (int64_t)mat * NOLSM_BS * ld : nullptr;
   for (int t = threadIdx.x; t < NOLSM_BS * n; t += blockDim.x) {
     const int p = t / n, k = t - p * n;
-    s_sinv[k * NOLSM_BS + p] = sj[(int64_t)(own0 + p) * ld + k];
+    s_sinv[k * NOLSM_BS + p] = uj ? uj[(int64_t)p * ld + k] : sj[(int64_t)(own0 + p) * ld + k];
   }
   __syncthreads();
   const int r = blockIdx.x * DN_THREADS + threadIdx.x;
@@ -530,27 +534,96 @@ k_density(const int32_t *__restrict__ row_ptr, const int32_t *__restrict__ col_i
     }
     float *out = d_val + ((int64_t)lo * 36 + (int64_t)r * NOLSM_BS);
 #pragma unroll
-    for (int p = 0; p < NOLSM_BS; ++p) out[p] = 0.5f * (s_sinv[r * NOLSM_BS + p] - acc[p]);
-    if (ne_diag != nullptr && r >= own0 && r < own0 + NOLSM_BS)
-      atomicAdd(ne_diag, (double)(1.f - xj[(int64_t)r * ld + r]));
+    for (int p = 0; p < NOLSM_BS; ++p) {
+      const float v = uj ? sj[(int64_t)(own0 + p) * ld + r] : s_sinv[r * NOLSM_BS + p];
+      out[p] = 0.5f * (v - acc[p]);
+    }
+    if (ne_diag != nullptr && r >= own0 && r < own0 + NOLSM_BS) {
+      float xrr = xj[(int64_t)r * ld + r];
+      if (uj) {   // diagonal element of X_{k+1} = X_k + 1/2 X_k E_k
+        const int64_t eoff = (int64_t)mat * slab + (int64_t)r * ld;
+        float dot = 0.f;
+        for (int k = 0; k < n; ++k) {
+          float e = __half2float(e_hi[eoff + k]);
+          if (e_lo) e = fmaf(__half2float(e_lo[eoff + k]), 1.f / 2048.f, e);
+          dot = fmaf(xj[(int64_t)k * ld + r], e, dot);
+        }
+        xrr = fmaf(0.5f, dot, xrr);
+      }
+      atomicAdd(ne_diag, (double)(1.f - xrr));
+    }
+  }
+}
+
+// Last sign iteration folded into a5 (reading 9): with E_k = I - X_k^2 already formed and passing the
+// stop test, X_{k+1} = X_k + 1/2 X_k E_k is only ever applied to the six own columns V of S^-1, and
+// X_{k+1} V = X_k (V + 1/2 E_k V).  This kernel forms U = V + 1/2 E_k V (thread = row, E_k column by column,
+// coalesced FP16 loads, V in shared memory); k_density then multiplies X_k with U instead of V.  Two n^2 x 6
+// products replace the n^3 product that would finish the iteration.  u_out: [count][6][ld].
+__global__ void __launch_bounds__(DN_THREADS)
+k_last_half(const int32_t *__restrict__ row_ptr, const int32_t *__restrict__ col_idx, int mol_begin, int ld,
+            int64_t slab, const __half *__restrict__ e_hi, const __half *__restrict__ e_lo,
+            const float *__restrict__ sinv, float *__restrict__ u_out) {
+  extern __shared__ __align__(16) float s_v[];  // [n][6]
+  const int mat = blockIdx.y;
+  const int j = mol_begin + mat;
+  const int lo = row_ptr[j];
+  const int m = row_ptr[j + 1] - lo;
+  const int n = m * NOLSM_BS;
+  int l = 0, r_ = m;
+  while (l < r_) {
+    const int mid = (l + r_) >> 1;
+    if (col_idx[lo + mid] < j) l = mid + 1; else r_ = mid;
+  }
+  const int own0 = l * NOLSM_BS;
+  const float *sj = sinv + (int64_t)mat * slab;
+  for (int t = threadIdx.x; t < NOLSM_BS * n; t += blockDim.x) {
+    const int p = t / n, k = t - p * n;
+    s_v[k * NOLSM_BS + p] = sj[(int64_t)(own0 + p) * ld + k];
+  }
+  __syncthreads();
+  const int r = blockIdx.x * DN_THREADS + threadIdx.x;
+  if (r < n) {
+    const __half *eh = e_hi + (int64_t)mat * slab + r;
+    const __half *el = e_lo ? e_lo + (int64_t)mat * slab + r : nullptr;
+    float acc[NOLSM_BS];
+#pragma unroll
+    for (int p = 0; p < NOLSM_BS; ++p) acc[p] = 0.f;
+#pragma unroll 8
+    for (int c = 0; c < n; ++c) {
+      float e = __half2float(eh[(int64_t)c * ld]);
+      if (el) e = fmaf(__half2float(el[(int64_t)c * ld]), 1.f / 2048.f, e);
+      const float2 *vk = reinterpret_cast<const float2 *>(s_v + c * NOLSM_BS);
+      const float2 v0 = vk[0], v1 = vk[1], v2 = vk[2];
+      acc[0] = fmaf(e, v0.x, acc[0]); acc[1] = fmaf(e, v0.y, acc[1]); acc[2] = fmaf(e, v1.x, acc[2]);
+      acc[3] = fmaf(e, v1.y, acc[3]); acc[4] = fmaf(e, v2.x, acc[4]); acc[5] = fmaf(e, v2.y, acc[5]);
+    }
+    float *uj = u_out + (int64_t)mat * NOLSM_BS * ld;
+#pragma unroll
+    for (int p = 0; p < NOLSM_BS; ++p) uj[(int64_t)p * ld + r] = fmaf(0.5f, acc[p], s_v[r * NOLSM_BS + p]);
   }
 }
 
 cudaError_t launch_density(const nolsm_batch *b, const float *x, const float *x_alt, const float *sinv,
                            const int32_t *row_ptr, const int32_t *col_idx, float *d_val,
-                           double *ne_diag, cudaStream_t st) {
+                           double *ne_diag, const __half *e_hi, const __half *e_lo, float *u_thin,
+                           cudaStream_t st) {
   if (b->count == 0) return cudaSuccess;
   const size_t smem = (size_t)NOLSM_BS * b->max_n * sizeof(float);
   static size_t smem_set = 0;
   if (smem > 48 * 1024 && smem > smem_set) {
     cudaError_t e = cudaFuncSetAttribute(k_density, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_last_half, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     smem_set = smem;
   }
   dim3 grid((b->max_n + DN_THREADS - 1) / DN_THREADS, b->count);
+  if (u_thin)   // the last iteration is pending (e_hi [+ e_lo] = E_k): U = V + 1/2 E_k V first
+    k_last_half<<<grid, DN_THREADS, smem, st>>>(row_ptr, col_idx, b->mol_begin, b->ld, (int64_t)b->ld * b->ld,
+                                                e_hi, e_lo, sinv, u_thin);
   k_density<<<grid, DN_THREADS, smem, st>>>(row_ptr, col_idx, b->mol_begin, b->ld,
-                                            (int64_t)b->ld * b->ld, x, x_alt, b->d_iters, sinv, d_val,
-                                            ne_diag);
+                                            (int64_t)b->ld * b->ld, x, x_alt, b->d_iters, sinv, u_thin, e_hi, e_lo,
+                                            d_val, ne_diag);
   return cudaGetLastError();
 }
 
