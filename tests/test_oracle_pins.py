@@ -239,6 +239,29 @@ def test_inverse_residual_recurrence_and_refined_early_stop(tiny_system):
     assert rel1 <= (np.linalg.cond(ssub) * rel0) ** 2 and rel1 < 1e-4
 
 
+def test_last_sign_update_folded_into_thin_products(tiny_system, tiny_solution):
+    """Reading 9: with E_k = I - X_k^2, X_{k+1} V = X_k (V + 1/2 E_k V) for any thin V, so the own columns of
+    D = 1/2 (I - X_{k+1}) S^-1 follow from X_k and E_k without forming X_{k+1}."""
+    s = tiny_system
+    sol = tiny_solution["solutions"][7]
+    hsub, ssub = sol.h_sub, sol.s_sub
+    n = len(ssub)
+    a = np.linalg.solve(ssub, hsub) + 0.85 * np.eye(n)
+    bound = np.sqrt(np.abs(a).sum(0).max() * np.abs(a).sum(1).max())
+    k = 7
+    xk = orc.newton_schulz_sign(a, k, scale=bound / 1.5)
+    xk1 = orc.newton_schulz_sign(a, k + 1, scale=bound / 1.5)
+    ek = np.eye(n) - xk @ xk
+    own = orc.own_position(sol.nbrs, sol.j)
+    v = np.linalg.inv(ssub)[:, own * 6:own * 6 + 6]
+    folded = 0.5 * (v - xk @ (v + 0.5 * ek @ v))
+    direct = 0.5 * (v - xk1 @ v)
+    assert np.abs(folded - direct).max() < 1e-13
+    # and once converged this is the oracle's D column block
+    x30 = orc.newton_schulz_sign(a, 30, scale=bound / 1.5)
+    assert np.abs(0.5 * (v - x30 @ v) - sol.density_columns(-0.85)).max() < 1e-9
+
+
 # ------------------------------------------------------------------ Eq. 6 / 12 by eigenvectors
 def test_sign_and_density_identities(tiny_solution):
     sol = tiny_solution["solutions"][5]
