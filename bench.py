@@ -210,7 +210,7 @@ def run_native(args, system, rank, world, local_rank):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     precision = WORKLOADS[args.workload][0] if args.precision < 0 else args.precision
     cfg = nolsm.Config(precision=precision, workspace_bytes=int(args.workspace_gib * (1 << 30)), group=args.group,
-                       flags=args.flags, cache_bytes=-1 if args.no_cache else 0)
+                       flags=args.flags, cache_bytes=-1 if args.no_cache else 0, gap_hint=args.gap_hint)
     ctx = nolsm.Context(cfg)
     dev = torch.device("cuda", local_rank)
     pos = torch.as_tensor(system.pos_q).to(dev)
@@ -303,7 +303,7 @@ def run_native(args, system, rank, world, local_rank):
                    "cutoff_A": system.cutoff, "mu": MU, "seed": system.seed, "nnz_blocks": system.nnzb,
                    "mean_submatrix_dim": 6.0 * system.nnzb / system.n_mol, "tol": 1e-2 if precision == 0 else 1e-5,
                    "workspace_gib": args.workspace_gib, "batches": st.n_batches, "replicas": world,
-                   "group": args.group, "engine_flags": args.flags, "elements": args.elements, "mu_steps": args.mu_steps,
+                   "group": args.group, "engine_flags": args.flags, "elements": args.elements, "mu_steps": args.mu_steps, "gap_hint": args.gap_hint,
                    "l2": "inputs larger than L2 (block stores 3 x %.0f MB, dense workspace %.0f GiB)" %
                          (system.nnzb * 144 / 1e6, args.workspace_gib)},
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
@@ -349,6 +349,9 @@ def main():
                          "on the device from the positions (nolsm_set_model; -fp32: FP32 + SFU as in PAPER.md:202)")
     ap.add_argument("--mu-steps", type=int, default=1,
                     help="N(mu) evaluations per step (default 1 = the headline step; 5 = BASELINE configs[1]'s bisection)")
+    ap.add_argument("--gap-hint", type=float, default=0.0,
+                    help="nolsm_config.gap_hint: lower bound on |lambda - mu| (the generator's gap gives 0.15 at "
+                         "mu = -0.85); > 0 starts the sign iteration with scaled steps.  Default 0: plain Eq. 9")
     ap.add_argument("--no-cache", action="store_true", help="nolsm_config.cache_bytes = -1 (only matters for --mu-steps > 1)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")

@@ -70,6 +70,11 @@ typedef struct {
   int32_t group;            /* submatrices iterated together so their iterates stay L2-resident
                                (<= 0: chosen from the L2 size) */
   int32_t flags;            /* NOLSM_FLAG_* */
+  float gap_hint;           /* > 0: a lower bound on |lambda - mu| over the spectra of the S_j^-1 H_j (e.g. half the
+                               HOMO-LUMO gap of the previous MD step).  The sign iteration then starts with scaled
+                               steps X <- 1/2 a_k X (3I - a_k^2 X^2), a_k = sqrt(3/(1 + l_k + l_k^2)), l_0 = gap_hint/s_j
+                               (DESIGN.md section 8), which saves iterations; a bound that is wrong
+                               costs iterations, never convergence.  0: the plain iteration of Eq. 9 (default). */
   int64_t cache_bytes;      /* nolsm_solve_mu with several mu steps, batches streamed through the workspace:
                                upper bound on the device memory used to keep B_j and the own columns of S_j^-1
                                of every submatrix from the first step, so that later steps skip a1-a3 (gather,

@@ -139,6 +139,31 @@ def newton_schulz_sign(a, n_iter, scale=None, history=False):
     return (x, np.array(res)) if history else x
 
 
+def newton_schulz_sign_scaled(a, n_iter, scale, gap, history=False):
+    """Scaled start of Eq. 9 (the rescaling PAPER.md:138 allows): with l_k a lower
+    bound on the moduli of the eigenvalues of X_k (all <= 1), X_{k+1} = 1/2 a_k X_k (3I - a_k^2 X_k^2),
+    a_k = sqrt(3 / (1 + l_k + l_k^2)), l_{k+1} = 1/2 a_k l_k (3 - a_k^2 l_k^2); a_k < 1.02 is taken as 1.
+    X0 = A/scale may have moduli up to 1.5, so step 0 is the plain one; l_0 = gap/scale.
+    Returns X_{n_iter} (and the a_k used, if history)."""
+    a = np.asarray(a, dtype=np.float64)
+    n = a.shape[0]
+    eye = np.eye(n)
+    x = a / scale
+    ell = min(gap / scale, 1.0)
+    alphas = []
+    for k in range(n_iter):
+        if k == 0:
+            al = 1.0
+        else:
+            al = np.sqrt(3.0 / (1.0 + ell + ell * ell))
+            if al < 1.02:
+                al = 1.0
+        alphas.append(al)
+        x = 0.5 * al * x @ (3.0 * eye - al * al * (x @ x))
+        ell = 0.5 * al * ell * (3.0 - al * al * ell * ell)
+    return (x, np.array(alphas)) if history else x
+
+
 def newton_schulz_inverse(s, n_iter, scale=None, history=False):
     """Eq. 15-17: Y0 = S/scale, Z0 = I, V_k = Z_k Y_k,
     Y_{k+1} = 1/2 Y_k (3I - V_k), Z_{k+1} = 1/2 (3I - V_k) Z_k; Z -> Y0^{-1/2}; S^-1 = Z^2/scale.

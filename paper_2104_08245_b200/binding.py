@@ -34,12 +34,12 @@ class Config(C.Structure):
     _fields_ = [("precision", C.c_int32), ("tol", C.c_float), ("max_iter", C.c_int32), ("fixed_iter", C.c_int32),
                 ("inv_tol", C.c_float), ("inv_max_iter", C.c_int32), ("inv_refine", C.c_int32),
                 ("workspace_bytes", C.c_int64), ("group", C.c_int32), ("flags", C.c_int32),
-                ("cache_bytes", C.c_int64)]
+                ("gap_hint", C.c_float), ("cache_bytes", C.c_int64)]
 
     def __init__(self, precision=FP16_FP32, tol=0.0, max_iter=0, fixed_iter=0, inv_tol=0.0, inv_max_iter=0,
-                 inv_refine=-1, workspace_bytes=0, group=0, flags=0, cache_bytes=0):
+                 inv_refine=-1, workspace_bytes=0, group=0, flags=0, cache_bytes=0, gap_hint=0.0):
         super().__init__(precision, tol, max_iter, fixed_iter, inv_tol, inv_max_iter, inv_refine,
-                         workspace_bytes, group, flags, cache_bytes)
+                         workspace_bytes, group, flags, gap_hint, cache_bytes)
 
 
 class _Bsr(C.Structure):

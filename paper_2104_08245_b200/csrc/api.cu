@@ -99,6 +99,7 @@ static void free_batch(nolsm_batch *b) {
   cudaFree(b->d_lastres);
   cudaFree(b->d_scale);
   cudaFree(b->d_norm);
+  cudaFree(b->d_alpha);
   cudaFree(b->d_colpart);
   cudaFree(b->d_active);
   cudaFree(b->d_tiles_simt);
@@ -199,7 +200,7 @@ static nolsm_status setup_batch(nolsm_ctx *ctx, int slot, const std::vector<int3
     const size_t cap = (size_t)count;
     if (grow(&b->d_dims, cap) || grow(&b->d_state, cap) || grow(&b->d_iters, cap) ||
         grow(&b->d_resid2, cap * NOLSM_MAX_RESID_SLOTS) || grow(&b->d_lastres, cap) ||
-        grow(&b->d_scale, cap) || grow(&b->d_norm, cap * 2) || grow(&b->d_ready, cap) ||
+        grow(&b->d_scale, cap) || grow(&b->d_norm, cap * 2) || grow(&b->d_alpha, cap * 8) || grow(&b->d_ready, cap) ||
         grow(&b->d_tiles_done, cap) || grow(&b->d_group_active, cap) || grow(&b->d_tile_counter, (size_t)1) ||
         (b->d_active == nullptr && grow(&b->d_active, (size_t)NOLSM_MAX_RESID_SLOTS))) {
       cudaGetLastError();
@@ -643,6 +644,10 @@ static nolsm_status sign_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, double mu, 
     set2(e.out16, 4, 4); set2(e.out16_lo, 5, 5);
     set2(x.a, 0, 2); set2(x.a_lo, 1, 3); set2(x.b, 4, 4); set2(x.b_lo, 5, 5);
     set2(x.out16, 2, 0); set2(x.out16_lo, 3, 1);
+  }
+  if (ctx->cfg.gap_hint > 0.f && !scale_in && pg.fixed_iter <= 0) {   // scaled start
+    LAUNCH(ctx, launch_alpha_schedule(b, b->d_scale, ctx->cfg.gap_hint, b->d_alpha, st));
+    pg.use_alpha_tab = 1;
   }
   if (timed) NOLSM_CUDA(ctx, cudaEventRecord(ctx->tev[0], st));
   CHECK(run_chain(ctx, b, pg, nullptr, true, st));

@@ -60,7 +60,11 @@ struct ChainArgs {
   int32_t *ready, *tiles_done, *state, *iters, *group_active;
   unsigned long long *tile_counter;   // next tile index to claim (dynamic scheduling)
   float *resid2, *lastres;
+  // scaled Newton-Schulz start (nolsm_config.gap_hint): alpha_tab[m * kAlphaSteps + k] = alpha_k of submatrix m
+  // for iteration k < kAlphaSteps (1 afterwards); null = the plain iteration
+  const float *alpha_tab;
 };
+constexpr int kAlphaSteps = 8;
 
 __device__ __forceinline__ uint32_t s32(const void *p) { return static_cast<uint32_t>(__cvta_generic_to_shared(p)); }
 __device__ __forceinline__ void ld_tmem32(uint32_t taddr, uint32_t (&v)[32]) {
@@ -103,6 +107,10 @@ __device__ __forceinline__ void epi_complete(const ChainArgs &args, const TileCm
     const float res = sqrtf(fmaxf(r2, 0.f) / (float)n);
     args.lastres[c.mat] = res;
     bool stop = pg.fixed_iter > 0 ? (k + 1 >= pg.fixed_iter) : ((res < pg.tol) || !(res == res));
+    // a scaled step (alpha_k > 1) measures ||I - alpha^2 X^2||, not the residual of the stop rule
+    if (args.alpha_tab != nullptr && k < kAlphaSteps && pg.fixed_iter <= 0 && res == res &&
+        args.alpha_tab[c.mat * kAlphaSteps + k] > 1.f)
+      stop = false;
     if (k + 1 >= pg.max_iter) stop = true;
     args.iters[c.mat] = (stop && pg.stop_early) ? k : k + 1;   // iterations carried out in full
     if (stop) *reinterpret_cast<volatile int32_t *>(&args.state[c.mat]) = k;
@@ -126,7 +134,7 @@ struct EpiTile {
   const ChainOp *o;
   int par, n, r, nchunks, chunk_first;
   bool split, ident, has_cin, rows_in;
-  float alpha;
+  float alpha, beta;
   float *p32;                 // FP32 output, element (r, first chunk column) or null
   const float *cinp;          // FP32 master input, same position, or null
   __half *p16, *p16l;         // FP16 outputs (hi, lo), same position, or null
@@ -147,6 +155,12 @@ __device__ __forceinline__ void epi_begin(const ChainArgs &args, const TileCmd &
   t.ident = o.mode == EPI_IDENT;
   t.has_cin = !t.ident && o.cin32 >= 0 && o.beta != 0.f && rows_in;
   t.alpha = o.use_div ? o.alpha / args.alpha_div[c.mat] : o.alpha;
+  t.beta = o.beta;
+  if (args.alpha_tab != nullptr && cmd_iter(c) < kAlphaSteps) {
+    // X_{k+1} = 1/2 a X (3I - a^2 X^2):  E = I - a^2 X X,  X' = a X + (1/2 a) X E
+    const float a = args.alpha_tab[c.mat * kAlphaSteps + cmd_iter(c)];
+    if (t.ident) t.alpha *= a * a; else { t.alpha *= a; t.beta *= a; }
+  }
   const int64_t off = (int64_t)c.mat * args.slab + t.r + (int64_t)(c.n0 + 32 * chunk_first) * args.ld;
   t.p32 = (o.cout32 >= 0 && rows_in) ? args.ubuf[o.cout32] + off : nullptr;
   t.cinp = t.has_cin ? args.ubuf[o.cin32] + off : nullptr;
@@ -204,7 +218,7 @@ __device__ __forceinline__ float epi_chunks(const ChainArgs &args, const TileCmd
     if (t.has_cin) {
 #pragma unroll
       for (int j = 0; j < 32; ++j)
-        v[j] = __float_as_uint(fmaf(o.beta, t.cpre[j], t.alpha * __uint_as_float(v[j])));
+        v[j] = __float_as_uint(fmaf(t.beta, t.cpre[j], t.alpha * __uint_as_float(v[j])));
       if (ci + 2 < t.nchunks) {
         t.cinp += 2 * chunk_stride;
         const float *pc = t.cinp;
@@ -217,7 +231,7 @@ __device__ __forceinline__ float epi_chunks(const ChainArgs &args, const TileCmd
       const int dj = t.r - (c.n0 + c0);     // chunk column that holds the diagonal element of row r
 #pragma unroll
       for (int j = 0; j < 32; ++j) {
-        const float e = ((j == dj) ? 1.f : 0.f) - __uint_as_float(v[j]);
+        const float e = fmaf(-t.alpha, __uint_as_float(v[j]), (j == dj) ? 1.f : 0.f);
         if (j < nvalid) ss = fmaf(e, e, ss);
         v[j] = __float_as_uint(e);
       }

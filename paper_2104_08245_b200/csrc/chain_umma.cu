@@ -553,6 +553,7 @@ cudaError_t launch_chain(nolsm_ctx *ctx, const nolsm_batch *b, const ChainProgra
   a.tiles_done = b->d_tiles_done;
   a.state = b->d_state;
   a.iters = b->d_iters;
+  a.alpha_tab = prog.use_alpha_tab ? b->d_alpha : nullptr;
   a.group_active = b->d_group_active;
   a.tile_counter = b->d_tile_counter;
   a.resid2 = b->d_resid2;

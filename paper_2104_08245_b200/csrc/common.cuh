@@ -70,6 +70,7 @@ struct ChainProgram {
   int32_t parity_from_iters;      // 1: the operand tables are indexed by the parity of the LAST full iteration of
                                   // the chain that ran before on this batch ((iters[m] + 1) & 1) instead of the
                                   // own iteration's: lets a one-shot product read the final FP16 iterate in place
+  int32_t use_alpha_tab;          // 1: per-submatrix, per-iteration scaling alpha_k from nolsm_batch::d_alpha
   int32_t stop_early;             // 1: the iteration whose residual passes the test is NOT finished (its
                                   // remaining products are skipped); 0: it is (reading 9, "+1 rule")
 };
@@ -98,6 +99,7 @@ struct nolsm_batch {
   float *d_resid2 = nullptr;      // [NOLSM_MAX_RESID_SLOTS][count]
   float *d_lastres = nullptr;     // [count]
   float *d_scale = nullptr;       // [count] s_j of the sign scaling
+  float *d_alpha = nullptr;       // [count][8] alpha_k of the scaled Newton-Schulz start (gap_hint)
   float *d_norm = nullptr;        // [2][count] scratch for norm bounds
   float *d_colpart = nullptr;     // [count][ld/128][ld] column-sum shares of the row strips (k_norm_bound)
   size_t colpart_cap = 0;
@@ -199,6 +201,9 @@ cudaError_t launch_init_inverse(const nolsm_batch *b, const float *s, const floa
 cudaError_t launch_init_inverse_first(const nolsm_batch *b, const float *s, const float *norm2, float *y32,
                                       float *z32, __half *y16, __half *y16_lo, __half *z16, __half *z16_lo,
                                       __half *e16, __half *e16_lo, float *scale_out, cudaStream_t st);
+// alpha_k schedule of the scaled start from the scale s_j (d_scale) and a lower bound `gap` on |lambda - mu|
+cudaError_t launch_alpha_schedule(const nolsm_batch *b, const float *scale, float gap, float *alpha_tab,
+                                  cudaStream_t st);
 cudaError_t launch_make_x0(const nolsm_batch *b, const float *bmat, float mu, const float *norm2,
                            const float *scale_in, float *x32, __half *x16, __half *x16_lo, float *scale_out,
                            cudaStream_t st);

@@ -265,6 +265,32 @@ cudaError_t launch_make_x0(const nolsm_batch *b, const float *bmat, float mu, co
   return cudaGetLastError();
 }
 
+// Scaled Newton-Schulz start (Chen & Chow's scaling of Eq. 9): with a lower bound l
+// on the moduli of the eigenvalues of X (all <= 1), X <- 1/2 a X (3I - a^2 X^2) with a = sqrt(3 / (1 + l + l^2))
+// maps [l, 1] onto [l', 1] with l' = 1/2 a l (3 - a^2 l^2) = the image of both ends: the largest l' any a gives.
+// Any a in [1, sqrt 3] keeps a |x| <= sqrt 3, so a wrong bound costs iterations, never convergence.
+// X0 has |x| <= 1.5, so iteration 0 is the plain one (a = 1), which brings the spectrum into [-1, 1].
+__global__ void k_alpha_schedule(int count, const float *__restrict__ scale, float gap, float *__restrict__ tab) {
+  const int m = blockIdx.x * blockDim.x + threadIdx.x;
+  if (m >= count) return;
+  float l = fminf(gap / scale[m], 1.f);
+  tab[m * 8] = 1.f;
+  l = 0.5f * l * (3.f - l * l);
+  for (int k = 1; k < 8; ++k) {
+    float a = sqrtf(3.f / (1.f + l + l * l));
+    if (a < 1.02f) a = 1.f;
+    tab[m * 8 + k] = a;
+    l = 0.5f * a * l * (3.f - a * a * l * l);
+  }
+}
+
+cudaError_t launch_alpha_schedule(const nolsm_batch *b, const float *scale, float gap, float *alpha_tab,
+                                  cudaStream_t st) {
+  if (b->count == 0) return cudaSuccess;
+  k_alpha_schedule<<<(b->count + 127) / 128, 128, 0, st>>>(b->count, scale, gap, alpha_tab);
+  return cudaGetLastError();
+}
+
 // dst = src * f (f = scale[m], 1/scale[m] or 1), FP32 and/or FP16 (hi [+ lo*2^11]) copies over the
 // padded extent.  Hands FP32 results to the tensor-core path.
 __global__ void __launch_bounds__(256)

@@ -771,3 +771,26 @@ def test_operator_cache_bitwise_same_as_recomputing(nolsm, mid_system, precision
     assert out[0][0] == out[-1][0], (out[0][0], out[-1][0])
     assert abs(out[0][1] - out[-1][1]) < 1e-7, (out[0][1], out[-1][1])      # N is summed with FP64 atomics
     assert torch.equal(out[0][2], out[-1][2])
+
+
+@pytest.mark.parametrize("precision", [0, 1])
+def test_gap_hint_scaled_start(nolsm, mid_system, mid_solution, precision):
+    """nolsm_config.gap_hint: the scaled Newton-Schulz start gives the oracle's D and N in fewer
+    iterations; a hint that is far too large still converges to them."""
+    import oracle.nolsm_oracle as orc
+    system = mid_system
+    sols = mid_solution["solutions"]
+    d_ref = orc.density_blocks(sols, system.row_ptr, MU)
+    ne_ref = orc.electron_count(sols, MU)
+    gap = min(float(np.abs(s.lam - MU).min()) for s in sols)
+    H, S = _device_system(nolsm, system)
+    iters = {}
+    for hint in (0.0, 0.9 * gap, 5.0 * gap):
+        ctx = nolsm.Context(nolsm.Config(precision=precision, gap_hint=hint))
+        mu, ne, D, st = ctx.solve_mu(H, S, system.n_electrons, 2 * MU, 0.0, tol_ne_per_mol=-1.0, max_steps=1)
+        assert st.last.n_unconverged == 0
+        assert np.abs(D.val.cpu().numpy() - d_ref).max() < TOL_D[precision]
+        assert abs(ne - ne_ref) / system.n_mol <= TOL_NE_PER_MOL
+        iters[hint] = st.last.iter_max
+        ctx.close()
+    assert iters[0.9 * gap] <= iters[0.0] - 2, iters

@@ -262,6 +262,33 @@ def test_last_sign_update_folded_into_thin_products(tiny_system, tiny_solution):
     assert np.abs(0.5 * (v - x30 @ v) - sol.density_columns(-0.85)).max() < 1e-9
 
 
+def test_scaled_newton_schulz_start(tiny_solution):
+    """gap_hint.  Scalar facts: for l <= x <= 1 and a = sqrt(3/(1+l+l^2)) the step
+    g(x) = a x (3 - a^2 x^2)/2 maps both ends to the same value l' > plain step of l, stays in (0, 1], and a
+    wrong (too large) l still converges.  Matrix fact: same sign(A) as the plain iteration in fewer steps."""
+    for l in (0.02, 0.1, 0.4):
+        a = np.sqrt(3.0 / (1.0 + l + l * l))
+        g = lambda x: 0.5 * a * x * (3.0 - a * a * x * x)
+        assert abs(g(l) - g(1.0)) < 1e-14 and g(l) > 0.5 * l * (3.0 - l * l)
+        xs = np.linspace(l, 1.0, 2001)
+        assert g(xs).min() >= g(l) - 1e-14 and g(xs).max() <= 1.0 + 1e-14
+    x = np.array([[0.01]])                                   # hint ten times too large
+    assert abs(orc.newton_schulz_sign_scaled(x, 40, 1.0, 0.1)[0, 0] - 1.0) < 1e-12
+    sol = tiny_solution["solutions"][11]
+    n = sol.n
+    a = np.linalg.solve(sol.s_sub, sol.h_sub) + 0.85 * np.eye(n)
+    ref = sol.sign(-0.85)
+    scale = np.sqrt(np.abs(a).sum(0).max() * np.abs(a).sum(1).max()) / 1.5
+    gap = np.abs(sol.lam + 0.85).min()
+    res = lambda x: np.linalg.norm(x @ x - np.eye(n)) / np.sqrt(n)
+    k_plain = next(k for k in range(1, 40) if res(orc.newton_schulz_sign(a, k, scale=scale)) < 1e-8)
+    k_scaled = next(k for k in range(1, 40) if res(orc.newton_schulz_sign_scaled(a, k, scale, 0.9 * gap)) < 1e-8)
+    assert k_scaled <= k_plain - 2
+    xs, alphas = orc.newton_schulz_sign_scaled(a, k_scaled + 2, scale, 0.9 * gap, history=True)
+    assert np.abs(xs - ref).max() < 1e-9
+    assert alphas[0] == 1.0 and alphas[1] > 1.3 and alphas[-1] == 1.0 and np.all(alphas < np.sqrt(3.0))
+
+
 # ------------------------------------------------------------------ Eq. 6 / 12 by eigenvectors
 def test_sign_and_density_identities(tiny_solution):
     sol = tiny_solution["solutions"][5]
