@@ -437,6 +437,7 @@ static ChainOp make_op(int mode, float alpha, float beta) {
   memset(&o, 0, sizeof(o));
   for (int p = 0; p < 2; ++p) o.a[p] = o.b[p] = o.a_lo[p] = o.b_lo[p] = o.out16[p] = o.out16_lo[p] = -1;
   o.cin32 = o.cout32 = -1;
+  o.cin16[0] = o.cin16[1] = -1;
   o.mode = mode;
   o.alpha = alpha;
   o.beta = beta;
@@ -496,18 +497,27 @@ static nolsm_status prepare_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, int prec
   p0.n_ops = 1;
   ChainOp &y1 = p0.ops[0] = make_op(EPI_AXPBY, 0.5f, 1.f);
   y1.cin32 = y1.cout32 = 2;
+  // FP16 mode with a refinement behind the iteration: the iterates live in FP16 only (the add-in of the
+  // correction form is the FP16 operand copy itself); their 5e-4 rounding is far inside what the refinement
+  // squares away, and no tile reads or writes an FP32 master
+  const bool masters = !(fp16 && refine > 0);
   if (fp16) {
-    // Y16: h0/h1 (ping-pong), Z16: h2/h3, E16: h4; masters Y32 = u2, Z32 = u3
-    LAUNCH(ctx, launch_init_inverse_first(b, S, b->d_norm, b->u[2], b->u[3], b->h[0], nullptr, b->h[3], nullptr,
-                                          b->h[4], nullptr, b->d_scale, st));
+    // Y16: h0/h1 (ping-pong), Z16: h2/h3, E16: h4; masters (if kept) Y32 = u2, Z32 = u3
+    LAUNCH(ctx, launch_init_inverse_first(b, S, b->d_norm, masters ? b->u[2] : nullptr, masters ? b->u[3] : nullptr,
+                                          b->h[0], nullptr, b->h[3], nullptr, b->h[4], nullptr, b->d_scale, st));
     set2(y1.a, 0, 0); set2(y1.b, 4, 4); set2(y1.out16, 1, 1);
-    pg.group = group_size(ctx, b, 18);
+    pg.group = group_size(ctx, b, masters ? 18 : 10);
     ChainOp &e = pg.ops[0] = make_op(EPI_IDENT, 1.f, 0.f);
     set2(e.a, 3, 2); set2(e.b, 1, 0); set2(e.out16, 4, 4); e.resid = 1;
     ChainOp &y = pg.ops[1] = make_op(EPI_AXPBY, 0.5f, 1.f);
     set2(y.a, 1, 0); set2(y.b, 4, 4); y.cin32 = y.cout32 = 2; set2(y.out16, 0, 1);
     ChainOp &z = pg.ops[2] = make_op(EPI_AXPBY, 0.5f, 1.f);
     set2(z.a, 4, 4); set2(z.b, 3, 2); z.cin32 = z.cout32 = 3; set2(z.out16, 2, 3);
+    if (!masters) {
+      y1.cin32 = y1.cout32 = -1; set2(y1.cin16, 0, 0);
+      y.cin32 = y.cout32 = -1; set2(y.cin16, 1, 0);
+      z.cin32 = z.cout32 = -1; set2(z.cin16, 3, 2);
+    }
   } else {
     // split operands: Y (h0,h1)/(h2,h3), Z (h4,h5)/(h6,h7), E (h8,h9)
     LAUNCH(ctx, launch_init_inverse_first(b, S, b->d_norm, b->u[2], b->u[3], b->h[0], b->h[1], b->h[6], b->h[7],

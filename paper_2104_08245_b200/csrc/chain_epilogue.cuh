@@ -137,6 +137,7 @@ struct EpiTile {
   float alpha, beta;
   float *p32;                 // FP32 output, element (r, first chunk column) or null
   const float *cinp;          // FP32 master input, same position, or null
+  const __half *cinh;         // FP16 add-in instead (ChainOp::cin16), or null
   __half *p16, *p16l;         // FP16 outputs (hi, lo), same position, or null
   float cpre[32];
 };
@@ -153,7 +154,8 @@ __device__ __forceinline__ void epi_begin(const ChainArgs &args, const TileCmd &
   t.chunk_first = chunk_first;
   t.split = o.a_lo[t.par] >= 0;
   t.ident = o.mode == EPI_IDENT;
-  t.has_cin = !t.ident && o.cin32 >= 0 && o.beta != 0.f && rows_in;
+  const bool cin_half = o.cin16[t.par] >= 0;
+  t.has_cin = !t.ident && (o.cin32 >= 0 || cin_half) && o.beta != 0.f && rows_in;
   t.alpha = o.use_div ? o.alpha / args.alpha_div[c.mat] : o.alpha;
   t.beta = o.beta;
   if (args.alpha_tab != nullptr && cmd_iter(c) < kAlphaSteps) {
@@ -163,7 +165,8 @@ __device__ __forceinline__ void epi_begin(const ChainArgs &args, const TileCmd &
   }
   const int64_t off = (int64_t)c.mat * args.slab + t.r + (int64_t)(c.n0 + 32 * chunk_first) * args.ld;
   t.p32 = (o.cout32 >= 0 && rows_in) ? args.ubuf[o.cout32] + off : nullptr;
-  t.cinp = t.has_cin ? args.ubuf[o.cin32] + off : nullptr;
+  t.cinp = (t.has_cin && !cin_half) ? args.ubuf[o.cin32] + off : nullptr;
+  t.cinh = (t.has_cin && cin_half) ? args.hbuf[o.cin16[t.par]] + off : nullptr;
   t.p16 = (o.out16[t.par] >= 0 && rows_in) ? args.hbuf[o.out16[t.par]] + off : nullptr;
   t.p16l = (o.out16_lo[t.par] >= 0 && rows_in) ? args.hbuf[o.out16_lo[t.par]] + off : nullptr;
 #if defined(NOLSM_NOEPI) || defined(NOLSM_NOCIN)   // timing experiments only (results are wrong)
@@ -181,9 +184,15 @@ __device__ __forceinline__ void epi_begin(const ChainArgs &args, const TileCmd &
   }
 #endif
   if (t.has_cin && chunk_first < t.nchunks) {
-    const float *pc = t.cinp;
+    if (t.cinh) {
+      const __half *ph = t.cinh;
 #pragma unroll
-    for (int j = 0; j < 32; ++j) { t.cpre[j] = __ldcg(pc); pc += args.ld; }
+      for (int j = 0; j < 32; ++j) { t.cpre[j] = __half2float(__ldcg(ph)); ph += args.ld; }
+    } else {
+      const float *pc = t.cinp;
+#pragma unroll
+      for (int j = 0; j < 32; ++j) { t.cpre[j] = __ldcg(pc); pc += args.ld; }
+    }
   }
 }
 
@@ -220,10 +229,17 @@ __device__ __forceinline__ float epi_chunks(const ChainArgs &args, const TileCmd
       for (int j = 0; j < 32; ++j)
         v[j] = __float_as_uint(fmaf(t.beta, t.cpre[j], t.alpha * __uint_as_float(v[j])));
       if (ci + 2 < t.nchunks) {
-        t.cinp += 2 * chunk_stride;
-        const float *pc = t.cinp;
+        if (t.cinh) {
+          t.cinh += 2 * chunk_stride;
+          const __half *ph = t.cinh;
 #pragma unroll
-        for (int j = 0; j < 32; ++j) { t.cpre[j] = __ldcg(pc); pc += args.ld; }
+          for (int j = 0; j < 32; ++j) { t.cpre[j] = __half2float(__ldcg(ph)); ph += args.ld; }
+        } else {
+          t.cinp += 2 * chunk_stride;
+          const float *pc = t.cinp;
+#pragma unroll
+          for (int j = 0; j < 32; ++j) { t.cpre[j] = __ldcg(pc); pc += args.ld; }
+        }
       }
     } else if (t.ident) {
       // valid columns of this chunk inside the true n x n part (residual of the stop rule)

@@ -55,6 +55,8 @@ struct ChainOp {
   int32_t a_lo[2], b_lo[2];       // lo parts of split operands (FP32-quality product), -1: plain FP16
   int32_t out16[2], out16_lo[2];  // FP16 copy of the result (hi [, lo * 2^11]), -1: none
   int32_t cin32, cout32;          // FP32 units read (AXPBY, beta != 0) / written, -1: none
+  int32_t cin16[2];               // instead of cin32: the add-in is an FP16 buffer (by parity), -1: none.  For
+                                  // iterations whose result is refined afterwards: no FP32 master is kept
   int32_t mode;                   // EPI_IDENT: I - A B     EPI_AXPBY: beta * Cin + alpha * A B
   int32_t resid;                  // 1: ||result||_F^2 over the true n x n part drives the stop rule
   int32_t use_div;                // alpha /= alpha_div[submatrix]

@@ -212,8 +212,10 @@ k_init_inverse_first(const int32_t *__restrict__ dims, int ld, int64_t slab, int
     ev[i] = d - y[i];
     z[i] = fmaf(0.5f, ev[i], d);
   }
-  *reinterpret_cast<float4 *>(y32 + e.off) = make_float4(y[0], y[1], y[2], y[3]);
-  *reinterpret_cast<float4 *>(z32 + e.off) = make_float4(z[0], z[1], z[2], z[3]);
+  if (y32) {   // FP32 masters (not kept when the iterates live in FP16 only)
+    *reinterpret_cast<float4 *>(y32 + e.off) = make_float4(y[0], y[1], y[2], y[3]);
+    *reinterpret_cast<float4 *>(z32 + e.off) = make_float4(z[0], z[1], z[2], z[3]);
+  }
   store_split4(y16 + e.off, y16_lo ? y16_lo + e.off : nullptr, y);
   store_split4(z16 + e.off, z16_lo ? z16_lo + e.off : nullptr, z);
   store_split4(e16 + e.off, e16_lo ? e16_lo + e.off : nullptr, ev);
