@@ -64,11 +64,11 @@ typedef struct {
                                finish iteration k are skipped.  <= 0: 3e-3 (FP16 with refinement), 1e-2 (FP16
                                without), 1e-5 (FP32) */
   int32_t inv_max_iter;     /* cap on Eq. 15-17 iterations (default 20 if <= 0) */
-  int32_t inv_refine;       /* FP16 mode: FP32-quality Newton refinements of S^-1 after Eq. 15-17
-                               (reading 11); < 0: default 1;  0 = paper-literal all-FP16 S^-1 */
+  int32_t inv_refine;       /* FP32-quality Newton refinements of S^-1 after Eq. 15-17 (reading 11);
+                               < 0: default 1;  0 in FP16 mode = the paper-literal all-FP16 S^-1 */
   int64_t workspace_bytes;  /* upper bound on the dense workspace the context may allocate (<= 0: 24 GiB) */
-  int32_t group;            /* submatrices iterated together so their iterates stay L2-resident
-                               (<= 0: chosen from the L2 size) */
+  int32_t group;            /* submatrices iterated together before the next group is touched (<= 0: chosen by
+                               the context: at least eight waves of tiles) */
   int32_t flags;            /* NOLSM_FLAG_* */
   float gap_hint;           /* > 0: a lower bound on |lambda - mu| over the spectra of the S_j^-1 H_j (e.g. half the
                                HOMO-LUMO gap of the previous MD step).  The sign iteration then starts with scaled
