@@ -132,6 +132,10 @@ __device__ __forceinline__ void store_half4(__half *dst, const float (&v)[4]) {
 
 // hi = fp16(v), lo = fp16((v - hi) * 2^11): the split operands of the FP32-quality products
 __device__ __forceinline__ void store_split4(__half *hi, __half *lo, const float (&v)[4]) {
+  if (lo == nullptr) {   // plain FP16 copy: none of the lo arithmetic (these passes are issue-bound, not HBM-bound)
+    store_half4(hi, v);
+    return;
+  }
   float h[4], l[4];
 #pragma unroll
   for (int i = 0; i < 4; ++i) {
@@ -139,7 +143,7 @@ __device__ __forceinline__ void store_split4(__half *hi, __half *lo, const float
     l[i] = (v[i] - h[i]) * 2048.f;
   }
   store_half4(hi, h);
-  if (lo) store_half4(lo, l);
+  store_half4(lo, l);
 }
 
 static dim3 elem4_grid(const nolsm_batch *b) {
@@ -166,7 +170,8 @@ k_init_inverse(const int32_t *__restrict__ dims, int ld, int64_t slab, int count
   const float sc = factor * fmaxf(1.f, sqrtf(norm2[mat] * norm2[count + mat]));  // max(1, .) covers the unit padding
   if (e.r == 0 && e.c == 0) scale_out[mat] = sc;
   const float4 sv = *reinterpret_cast<const float4 *>(s + e.off);
-  const float y[4] = {sv.x / sc, sv.y / sc, sv.z / sc, sv.w / sc};
+  const float inv = 1.f / sc;
+  const float y[4] = {sv.x * inv, sv.y * inv, sv.z * inv, sv.w * inv};
   float z[4];
 #pragma unroll
   for (int i = 0; i < 4; ++i) z[i] = (e.r + i == e.c) ? 1.f : 0.f;
@@ -204,7 +209,8 @@ k_init_inverse_first(const int32_t *__restrict__ dims, int ld, int64_t slab, int
   const float sc = factor * fmaxf(1.f, sqrtf(norm2[mat] * norm2[count + mat]));
   if (e.r == 0 && e.c == 0) scale_out[mat] = sc;
   const float4 sv = *reinterpret_cast<const float4 *>(s + e.off);
-  const float y[4] = {sv.x / sc, sv.y / sc, sv.z / sc, sv.w / sc};
+  const float inv = 1.f / sc;   // one reciprocal instead of four IEEE divisions: the pass is issue-bound
+  const float y[4] = {sv.x * inv, sv.y * inv, sv.z * inv, sv.w * inv};
   float ev[4], z[4];
 #pragma unroll
   for (int i = 0; i < 4; ++i) {
@@ -244,6 +250,7 @@ k_make_x0(const int32_t *__restrict__ dims, int ld, int64_t slab, int count,
   const int mat = blockIdx.y;
   float sc = scale_in ? scale_in[mat] : factor * sqrtf(norm2[mat] * norm2[count + mat]);
   sc = fmaxf(sc, 1e-30f);
+  const float inv = 1.f / sc;
   if (e.r == 0 && e.c == 0 && scale_out) scale_out[mat] = sc;
   const float4 bv = *reinterpret_cast<const float4 *>(bmat + e.off);
   const float in[4] = {bv.x, bv.y, bv.z, bv.w};
@@ -251,7 +258,7 @@ k_make_x0(const int32_t *__restrict__ dims, int ld, int64_t slab, int count,
 #pragma unroll
   for (int i = 0; i < 4; ++i) {
     const int r = e.r + i;
-    if (r < e.n && e.c < e.n) v[i] = (in[i] - (r == e.c ? mu : 0.f)) / sc;
+    if (r < e.n && e.c < e.n) v[i] = (in[i] - (r == e.c ? mu : 0.f)) * inv;
     else v[i] = (r == e.c) ? 1.f : 0.f;
   }
   if (x32) *reinterpret_cast<float4 *>(x32 + e.off) = make_float4(v[0], v[1], v[2], v[3]);
