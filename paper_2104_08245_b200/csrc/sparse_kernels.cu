@@ -488,7 +488,7 @@ cudaError_t launch_own_columns(const nolsm_batch *b, const int32_t *row_ptr, con
   return cudaGetLastError();
 }
 
-#define DN_THREADS 128
+#define DN_THREADS 256
 
 __global__ void __launch_bounds__(DN_THREADS)
 k_density(const int32_t *__restrict__ row_ptr, const int32_t *__restrict__ col_idx, int mol_begin,
