@@ -371,7 +371,7 @@ extern "C" nolsm_status nolsm_set_model(nolsm_ctx *ctx, const nolsm_model *model
 
 static nolsm_status build_submatrices_impl(nolsm_ctx *ctx, const nolsm_bsr *H, const nolsm_bsr *S,
                                            int32_t mol_begin, int32_t mol_count, int32_t slot, int units,
-                                           nolsm_batch **out, void *stream) {
+                                           nolsm_batch **out, void *stream, bool need_h32 = true) {
   if (!ctx || !out) return NOLSM_EINVAL;
   CHECK(check_bsr(ctx, H, "H"));
   CHECK(check_bsr(ctx, S, "S"));
@@ -396,9 +396,11 @@ static nolsm_status build_submatrices_impl(nolsm_ctx *ctx, const nolsm_bsr *H, c
       ctx->err = "the attached model has a different number of molecules than the matrices";
       return NOLSM_EINVAL;
     }
-    LAUNCH(ctx, launch_generate(b, H->row_ptr, H->col_idx, &ctx->model, b->u[1], b->u[0], split_s, st));
+    LAUNCH(ctx, launch_generate(b, H->row_ptr, H->col_idx, &ctx->model, need_h32 ? b->u[1] : nullptr, b->u[0],
+                                split_s, st));
   } else {
-    LAUNCH(ctx, launch_gather(b, H->row_ptr, H->col_idx, H->val, S->val, b->u[1], b->u[0], split_s, st));
+    LAUNCH(ctx, launch_gather(b, H->row_ptr, H->col_idx, H->val, S->val, need_h32 ? b->u[1] : nullptr, b->u[0],
+                              split_s, st));
   }
   b->s_split_built = split_s;
   *out = b;
@@ -1106,7 +1108,9 @@ extern "C" nolsm_status nolsm_solve_mu(nolsm_ctx *ctx, const nolsm_bsr *H, const
         b->prepared = true;
         b->prepared_precision = prec;
       } else if (!b || !resident) {
-        rc = build_submatrices_impl(ctx, H, S, r.begin, r.count, resident ? (int)bi : 0, units, &b, st);
+        // the FP32 copy of T_j(H) is only read by the energy products (nolsm_evaluate) and the SIMT debug path
+        rc = build_submatrices_impl(ctx, H, S, r.begin, r.count, resident ? (int)bi : 0, units, &b, st,
+                                    ctx->eval_energy || use_simt(ctx) || !ctx->umma_ok);
         if (rc != NOLSM_OK) break;
         live[bi] = resident ? b : nullptr;
       }

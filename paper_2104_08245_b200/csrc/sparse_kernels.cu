@@ -133,7 +133,7 @@ cudaError_t launch_exclusive_scan(const int32_t *counts, int32_t *row_ptr, int n
 // copies (hi = fp16(v), lo = fp16((v - hi) 2^11): the operands of the FP32-quality products, same
 // arithmetic as k_scale_copy) so that no conversion pass has to read the matrices again.
 struct BuildOut {
-  float *h32, *s32;
+  float *h32, *s32;           // h32 may be null: inside nolsm_solve_mu only the split copy of H is read
   __half *h_hi, *h_lo, *s_hi, *s_lo;
 };
 
@@ -151,7 +151,7 @@ __device__ __forceinline__ void emit_rows2(const BuildOut &out, int64_t base, in
   for (int p = 0; p < NOLSM_BS; ++p) {
     if (c0 + p < P) {
       const int64_t off = base + (int64_t)(c0 + p) * ld + r;
-      *reinterpret_cast<float2 *>(out.h32 + off) = make_float2(hv[0][p], hv[1][p]);
+      if (out.h32) *reinterpret_cast<float2 *>(out.h32 + off) = make_float2(hv[0][p], hv[1][p]);
       *reinterpret_cast<float2 *>(out.s32 + off) = make_float2(sv[0][p], sv[1][p]);
       __half2 hi, lo;
       if (out.h_hi) {
