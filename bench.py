@@ -34,7 +34,7 @@ WORKLOADS = {          # name -> (precision, description)
 DATASHEET_FP16_TFLOPS = 2250.0
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE sign-iteration launch of k_chain, from the
 # `ncu --set full` capture named in profiles/ (None where no capture of that workload exists)
-NCU_TRAFFIC = {"w32768": 111.3e9}   # profiles/r1_k_chain_sign_w32768.md
+NCU_TRAFFIC = {"w32768": 78.8e9}   # profiles/r1_k_chain_sign_w32768.md
 METRIC = "molecules/s per NOLSM step (sign-iteration TFLOP/s in roofline.achieved)"
 
 
