@@ -18,7 +18,8 @@ The literal iterations (Eq. 9-10, Eq. 15-17) are also written out step by step
 (`newton_schulz_sign`, `newton_schulz_inverse`) for fixed-iteration comparisons and residual traces.
 
 Readings of the paper taken here are listed in DESIGN.md ("Readings").
-Pins: tests/test_oracle_*.py (-m "not gpu").  Unpinned: the paper's fixed iteration count
+Pins: tests/test_oracle_*.py (-m "not gpu"), including hand-computed element values for the two-centre
+model (`two_centre_block`) and for `sign_residual`.  Unpinned: the paper's fixed iteration count
 (PAPER.md:217 never states it) -- "parity unpinned" for that number only; the oracle does not use it.
 """
 import numpy as np
@@ -85,6 +86,66 @@ def dense_submatrix(row_ptr, col_idx, val, nbrs):
         for b in np.nonzero(ok)[0]:
             out[a * BS:(a + 1) * BS, b * BS:(b + 1) * BS] = val[lo + pos[b]]
     return out
+
+
+# --------------------------------------------------------------------------------------------
+# a1': submatrix elements evaluated from positions instead of gathered
+# (Fig. 2 d-e PAPER.md:172; "constructing the matrix elements of the submatrices directly on the
+# GPUs" PAPER.md:202).  The "electronic-structure method" of this build is the synthetic two-centre
+# model of BASELINE.json:configs[0] as completed in DESIGN.md section 3:
+#     different sites at distance r:   S = s_ampl exp(-r^2 / 2 A^2),  H = h_ampl exp(-r / h_len)
+#     same site, same orbital:         S = 1,  H = orbital energy
+#     same site, different orbitals:   S = H = 0
+#     molecule pair outside r_c:       S = H = 0   (integer min-image test of reading 2)
+# Site a of molecule i sits at centre_i + site_offset[a] and is NOT wrapped separately; a site-site
+# vector takes the per-axis minimum image d - L rint(d / L).  Plain scalar loops, FP64.
+# --------------------------------------------------------------------------------------------
+def two_centre_block(pos_q, box_q, i, j, model):
+    """(H, S) 6x6 blocks between molecules i (rows) and j (columns) from the positions.
+    `model`: dict with unit_per_grid, site_offset[3][3], orb_site[6], orb_energy[6], s_ampl, h_ampl, h_len
+    (the fields of nolsm_model in include/nolsm.h).  Element [o, p] couples orbital o of i with orbital p of j."""
+    import math
+    u = float(model["unit_per_grid"])
+    off = model["site_offset"]
+    site = model["orb_site"]
+    h = np.zeros((BS, BS))
+    s = np.zeros((BS, BS))
+    box = [float(box_q[ax]) * u for ax in range(3)]
+    for o in range(BS):
+        for p in range(BS):
+            if i == j and site[o] == site[p]:
+                if o == p:
+                    s[o, p] = 1.0
+                    h[o, p] = float(model["orb_energy"][o])
+                continue
+            r2 = 0.0
+            for ax in range(3):
+                d = (float(pos_q[i][ax]) - float(pos_q[j][ax])) * u + float(off[site[o]][ax]) - float(off[site[p]][ax])
+                d -= box[ax] * float(np.rint(d / box[ax]))
+                r2 += d * d
+            s[o, p] = float(model["s_ampl"]) * math.exp(-0.5 * r2)
+            h[o, p] = float(model["h_ampl"]) * math.exp(-math.sqrt(r2) / float(model["h_len"]))
+    return h, s
+
+
+def model_submatrix(pos_q, box_q, rc_q, nbrs, model):
+    """T_j(H), T_j(S) of the molecule whose neighbour list is `nbrs`, evaluated from the positions: block
+    (a, b) is the two-centre block of (nbrs[a], nbrs[b]) if that pair is itself inside r_c, else zero."""
+    nbrs = [int(x) for x in nbrs]
+    m = len(nbrs)
+    hs = np.zeros((m * BS, m * BS))
+    ss = np.zeros((m * BS, m * BS))
+    p = np.asarray(pos_q, dtype=np.int64)
+    rc2 = int(rc_q) * int(rc_q)
+    for a in range(m):
+        for b in range(m):
+            d = min_image(p[nbrs[a]] - p[nbrs[b]], box_q)
+            if int((d * d).sum()) > rc2:
+                continue
+            hb, sb = two_centre_block(pos_q, box_q, nbrs[a], nbrs[b], model)
+            hs[a * BS:(a + 1) * BS, b * BS:(b + 1) * BS] = hb
+            ss[a * BS:(a + 1) * BS, b * BS:(b + 1) * BS] = sb
+    return hs, ss
 
 
 # --------------------------------------------------------------------------------------------

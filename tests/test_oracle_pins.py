@@ -456,3 +456,105 @@ def test_energy_weighted_density_and_energy_pins(tiny_system, tiny_solution):
     # and the own columns of W in the store layout give tr(W S) = E when contracted like tr(D S)
     w_blocks = orc.energy_weighted_blocks(sol["solutions"], full.row_ptr, -0.85)
     assert abs(0.5 * orc.electron_count_blocks(full.row_ptr, full.col_idx, w_blocks, full.s_val) - e_blocks) < 1e-9
+
+
+# ------------------------------------------------------------------ two-centre element model (row f2)
+def _hand_model():
+    # the literal constants of BASELINE.json configs[0] / DESIGN.md section 3, typed here (not imported)
+    return dict(unit_per_grid=1.0 / 65536.0,
+                site_offset=[[0.0, 0.0, 0.0], [0.757, 0.586, 0.0], [-0.757, 0.586, 0.0]],
+                orb_site=[0, 0, 0, 0, 1, 2], orb_energy=[-1.0, -1.0, -1.0, -1.0, -0.5, -0.5],
+                s_ampl=0.3, h_ampl=-0.2, h_len=1.5)
+
+
+def test_two_centre_model_hand_values():
+    """Pins of oracle.two_centre_block on numbers worked out by hand (decimal literals below):
+    an intermolecular pair at the integer distance 3 A, the on-site block, the orbital -> site map, and
+    a pair that is only close across the periodic boundary."""
+    g = 65536
+    box = np.array([40 * g, 40 * g, 40 * g], dtype=np.int32)
+    pos = np.array([[0, 0, 0], [3 * g, 0, 0], [39 * g, 0, 0]], dtype=np.int32)   # molecule 2 is 1 A from 0 across the wall
+    m = _hand_model()
+    h, s = orc.two_centre_block(pos, box, 0, 1, m)
+    # O(0) - O(1): r = 3:  S = 0.3 exp(-4.5),  H = -0.2 exp(-2)
+    assert abs(s[0, 0] - 0.3 * 0.011108996538242306) < 1e-15
+    assert abs(h[0, 0] - (-0.2 * 0.1353352832366127)) < 1e-15
+    assert np.all(s[:4, :4] == s[0, 0]) and np.all(h[:4, :4] == h[0, 0])        # the four O-site orbitals share the site
+    # O(0) - H1(1): d = (0,0,0) - (3.757, 0.586, 0): r^2 = 14.115049 + 0.343396 = 14.458445
+    assert abs(s[0, 4] - 0.3 * np.exp(-0.5 * 14.458445)) < 1e-15
+    assert abs(h[0, 4] - (-0.2 * np.exp(-np.sqrt(14.458445) / 1.5))) < 1e-15
+    # O(0) - H2(1): d = -(3 - 0.757, 0.586, 0): r^2 = 2.243^2 + 0.586^2 = 5.031049 + 0.343396 = 5.374445
+    assert abs(s[0, 5] - 0.3 * np.exp(-0.5 * 5.374445)) < 1e-15
+    # H1(0) - O(1): d = (0.757 - 3, 0.586, 0): the same distance as O(0) - H2(1) by the mirror symmetry of the molecule
+    assert abs(s[4, 0] - s[0, 5]) < 1e-16 and abs(h[4, 0] - h[0, 5]) < 1e-16
+    # H1(0) - H1(1): both offsets cancel: r = 3;  H1(0) - H2(1): d = (0.757 + 0.757 - 3, 0, 0): r = 1.486
+    assert abs(s[4, 4] - s[0, 0]) < 1e-16
+    assert abs(s[4, 5] - 0.3 * np.exp(-0.5 * 1.486 ** 2)) < 1e-15
+    assert abs(h[4, 5] - (-0.2 * np.exp(-1.486 / 1.5))) < 1e-15
+    # block (1, 0) is the transpose of block (0, 1)
+    h10, s10 = orc.two_centre_block(pos, box, 1, 0, m)
+    assert np.array_equal(h10, h.T) and np.array_equal(s10, s.T)
+    # on-site block: identity / orbital energies on the diagonal, zero between orbitals of one site,
+    # O - H at r^2 = 0.757^2 + 0.586^2 = 0.916445, H1 - H2 at r = 1.514
+    h00, s00 = orc.two_centre_block(pos, box, 0, 0, m)
+    assert np.array_equal(np.diag(s00), np.ones(6)) and np.array_equal(np.diag(h00), [-1, -1, -1, -1, -0.5, -0.5])
+    assert np.all(s00[:4, :4] == np.eye(4)) and np.all(h00[:4, :4] == -np.eye(4))
+    assert abs(s00[0, 4] - 0.3 * np.exp(-0.5 * 0.916445)) < 1e-15 and abs(s00[3, 5] - s00[0, 4]) < 1e-16
+    assert abs(h00[0, 4] - (-0.2 * np.exp(-np.sqrt(0.916445) / 1.5))) < 1e-15
+    assert abs(s00[4, 5] - 0.3 * np.exp(-0.5 * 1.514 ** 2)) < 1e-15 and s00[4, 5] == s00[5, 4]
+    # across the periodic boundary: centres 0 and 39 in a 40 A box are 1 A apart
+    h02, s02 = orc.two_centre_block(pos, box, 0, 2, m)
+    assert abs(s02[0, 0] - 0.3 * 0.6065306597126334) < 1e-15                   # 0.3 exp(-1/2)
+    assert abs(h02[0, 0] - (-0.2 * 0.513417119032592)) < 1e-15                 # -0.2 exp(-1/1.5)
+
+
+def test_generator_blocks_match_the_oracle_element_model(tiny_system):
+    """nolsm_inputs.water._blocks (the shared input module) against the oracle's own, independently
+    written two-centre model, every stored block of the tiny system and of a cutoff > L/2 system (per-site
+    minimum image): equal to the last FP32 bit up to one ulp where exp() rounds differently."""
+    m = _hand_model()
+    assert gi.model_parameters(tiny_system)["site_offset"] == m["site_offset"]
+    for system in (tiny_system, gi.make_water_system(32, 9.0)):
+        worst = 0
+        for i in range(0, system.n_mol, 3):
+            for k in range(system.row_ptr[i], system.row_ptr[i + 1]):
+                h, s = orc.two_centre_block(system.pos_q, system.box_q, i, int(system.col_idx[k]), m)
+                for got, ref in ((system.h_val[k], h), (system.s_val[k], s)):
+                    r32 = ref.astype(np.float32)
+                    assert np.array_equal(got == 0, r32 == 0)
+                    ulps = np.abs(got.view(np.int32).astype(np.int64) - r32.view(np.int32).astype(np.int64))
+                    worst = max(worst, int(ulps.max()))
+        assert worst <= 1, worst
+
+
+def test_model_submatrix_equals_gathered_submatrix(tiny_system):
+    """T_j evaluated from positions (model_submatrix) = T_j gathered from the block store (dense_submatrix),
+    including the zero blocks of neighbour pairs that are themselves outside the cutoff."""
+    s = tiny_system
+    m = _hand_model()
+    for j in (0, 7, 31):
+        nbrs = s.col_idx[s.row_ptr[j]:s.row_ptr[j + 1]]
+        hm, sm = orc.model_submatrix(s.pos_q, s.box_q, s.rc_q, nbrs, m)
+        hg = orc.dense_submatrix(s.row_ptr, s.col_idx, s.h_val, nbrs)
+        sg = orc.dense_submatrix(s.row_ptr, s.col_idx, s.s_val, nbrs)
+        assert np.array_equal(hm == 0, hg == 0) and np.array_equal(sm == 0, sg == 0)
+        assert (hm == 0).any()                                               # the pattern test is not vacuous
+        assert np.abs(hm - hg).max() < 1e-7 and np.abs(sm - sg).max() < 1e-7  # FP32 rounding of the store
+
+
+# ------------------------------------------------------------------ the acceptance evaluator itself
+def test_sign_residual_pins():
+    """||X^2 - I||_F / sqrt(n): diag(1.1, 1) -> sqrt(0.21^2) / sqrt(2) = 0.21 / sqrt(2); an exact
+    involution -> 0; and the same quantity as newton_schulz_sign's residual history (computed there
+    separately)."""
+    assert abs(orc.sign_residual(np.diag([1.1, 1.0])) - 0.21 / np.sqrt(2.0)) < 1e-15
+    assert abs(orc.sign_residual(np.diag([1.1, 1.0, 1.0, 1.0])) - 0.21 / 2.0) < 1e-15     # / sqrt(n), not / n
+    refl = np.eye(5) - 2.0 * np.outer(np.ones(5), np.ones(5)) / 5.0
+    assert orc.sign_residual(refl) < 1e-15
+    a, q, lam = gi.make_gapped_symmetric(24, seed=3)
+    a = a.astype(np.float64)
+    x3, hist = orc.newton_schulz_sign(a, 4, scale=np.abs(lam).max(), history=True)
+    x_k = a / np.abs(lam).max()
+    for k in range(4):
+        assert abs(orc.sign_residual(x_k) - hist[k]) < 1e-13
+        x_k = orc.newton_schulz_sign(x_k, 1)
