@@ -67,8 +67,9 @@ typedef struct {
   int32_t inv_refine;       /* FP32-quality Newton refinements of S^-1 after Eq. 15-17 (reading 11);
                                < 0: default 1;  0 in FP16 mode = the paper-literal all-FP16 S^-1 */
   int64_t workspace_bytes;  /* upper bound on the dense workspace the context may allocate (<= 0: 24 GiB) */
-  int32_t group;            /* submatrices iterated together before the next group is touched (<= 0: chosen by
-                               the context: at least eight waves of tiles) */
+  int32_t group;            /* window: submatrices in flight together inside one iteration kernel; a submatrix that
+                               converges hands its place to the next one of the batch (<= 0: chosen by the context
+                               from the L2 size and the tile count) */
   int32_t flags;            /* NOLSM_FLAG_* */
   float gap_hint;           /* > 0: a lower bound on |lambda - mu| over the spectra of the S_j^-1 H_j (e.g. half the
                                HOMO-LUMO gap of the previous MD step).  The sign iteration then starts with scaled
@@ -83,13 +84,12 @@ typedef struct {
                                that does not fit, the steps recompute.  Freed before the call returns. */
 } nolsm_config;
 
-/* Engine of the matrix iterations.  With none of PAIR / MCAST / SINGLE set the context picks per batch:
+/* Engine of the matrix iterations.  With neither PAIR nor SINGLE set the context picks per batch:
  * the pair engine when its 256-row tiles waste little (sum of the dimensions padded to 256 at most 4 % above
  * the sum padded to 128) and the mean dimension is at least 1100 -- where it measured 5-11 % ahead -- else
  * the single-CTA engine.  Each engine is bitwise reproducible run to run; different engines round differently. */
 #define NOLSM_FLAG_SIMT_ONLY 1 /* debugging: run every product on the FP32 SIMT kernel */
 #define NOLSM_FLAG_PAIR 2      /* always the CTA-pair engine (tcgen05 cta_group::2, 256-row tiles) */
-#define NOLSM_FLAG_MCAST 4     /* always CTA pairs that share the B operand by TMA multicast (cta_group::1) */
 #define NOLSM_FLAG_SINGLE 8    /* always the single-CTA engine (128-row tiles) */
 #define NOLSM_FLAG_UNIT_SCALE 16 /* scale by the norm bound itself: Y0 = S/bound, X0 = A/bound (spectra in (0,1] and
                                   [-1,1]) instead of bound/2 and bound/1.5 (readings 5, 7); costs one
@@ -116,6 +116,8 @@ typedef struct {            /* filled by nolsm_sign_batched (host struct) */
   int32_t inv_iter_max;     /* Eq. 15-17 iterations executed (0 if the batch was already prepared) */
   float inv_worst_residual;
   float ms_chain;           /* CUDA-event time of the sign-iteration kernel alone (all iterations of the batch) */
+  float chain_mcycles;      /* SM cycles of that kernel (max over its CTAs), in millions: ms_chain and this give the
+                               SM clock the kernel ran at under the power cap */
 } nolsm_sign_stats;
 
 typedef struct {            /* filled by nolsm_solve_mu (host struct) */

@@ -9,7 +9,6 @@ FP16_FP32, FP32 = 0, 1
 MAT_S, MAT_H, MAT_SINV, MAT_B, MAT_X = 0, 1, 2, 3, 4
 FLAG_SIMT_ONLY = 1
 FLAG_PAIR = 2
-FLAG_MCAST = 4
 FLAG_SINGLE = 8
 FLAG_UNIT_SCALE = 16
 STATUS = {0: "NOLSM_OK", 1: "NOLSM_EINVAL", 2: "NOLSM_ENOMEM", 3: "NOLSM_ECUDA", 4: "NOLSM_ENOTSPD",
@@ -58,7 +57,8 @@ class SignStats(C.Structure):
     _fields_ = [("n_sub", C.c_int32), ("iter_min", C.c_int32), ("iter_max", C.c_int32), ("iter_sum", C.c_int64),
                 ("n_unconverged", C.c_int32), ("worst_residual", C.c_float), ("gemms", C.c_int64),
                 ("flops_sign", C.c_double), ("flops_sign_padded", C.c_double), ("flops_prepare", C.c_double),
-                ("inv_iter_max", C.c_int32), ("inv_worst_residual", C.c_float), ("ms_chain", C.c_float)]
+                ("inv_iter_max", C.c_int32), ("inv_worst_residual", C.c_float), ("ms_chain", C.c_float),
+                ("chain_mcycles", C.c_float)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
@@ -140,9 +140,6 @@ def load_library():
     lib.nolsm_batch_ld.restype = i32
     lib.nolsm_gemm_batched.argtypes = [vp, i32, i32, f32, f32, vp, vp, vp, vp, vp, i32, i32, vp]
     lib.nolsm_gemm_batched.restype = i32
-    if hasattr(lib, "nolsm_debug_set_desc"):
-        lib.nolsm_debug_set_desc.argtypes = [C.c_uint32, C.c_uint32, C.c_uint32]
-        lib.nolsm_debug_set_desc.restype = None
     _LIB = lib
     return lib
 

@@ -13,7 +13,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libnolsm.so")
-SOURCES = ["api.cu", "sparse_kernels.cu", "dense_kernels.cu", "chain_umma.cu", "chain_pair.cu", "chain_mcast.cu"]
+SOURCES = ["api.cu", "sparse_kernels.cu", "dense_kernels.cu", "chain_engine.cu"]
 HEADERS = [os.path.join(CSRC, "common.cuh"), os.path.join(HERE, "..", "include", "nolsm.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "--use_fast_math=false"]

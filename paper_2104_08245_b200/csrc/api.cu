@@ -103,9 +103,9 @@ static void free_batch(nolsm_batch *b) {
   cudaFree(b->d_colpart);
   cudaFree(b->d_active);
   cudaFree(b->d_tiles_simt);
-  cudaFree(b->d_ready);
-  cudaFree(b->d_tiles_done);
-  cudaFree(b->d_group_active);
+  cudaFree(b->d_slot_state);
+  cudaFree(b->d_slot_done);
+  cudaFree(b->d_sched);
   cudaFree(b->d_tile_counter);
   cudaFree(b->d_thin);
   cudaFree(b->d_maps);
@@ -200,8 +200,8 @@ static nolsm_status setup_batch(nolsm_ctx *ctx, int slot, const std::vector<int3
     const size_t cap = (size_t)count;
     if (grow(&b->d_dims, cap) || grow(&b->d_state, cap) || grow(&b->d_iters, cap) ||
         grow(&b->d_resid2, cap * NOLSM_MAX_RESID_SLOTS) || grow(&b->d_lastres, cap) ||
-        grow(&b->d_scale, cap) || grow(&b->d_norm, cap * 2) || grow(&b->d_alpha, cap * 8) || grow(&b->d_ready, cap) ||
-        grow(&b->d_tiles_done, cap) || grow(&b->d_group_active, cap) || grow(&b->d_tile_counter, (size_t)1) ||
+        grow(&b->d_scale, cap) || grow(&b->d_norm, cap * 2) || grow(&b->d_alpha, cap * 8) || grow(&b->d_slot_state, cap) ||
+        grow(&b->d_slot_done, cap) || grow(&b->d_sched, (size_t)4) || grow(&b->d_tile_counter, (size_t)1) ||
         (b->d_active == nullptr && grow(&b->d_active, (size_t)NOLSM_MAX_RESID_SLOTS))) {
       cudaGetLastError();
       ctx->err = "cudaMalloc of batch metadata failed";
@@ -440,6 +440,7 @@ static ChainOp make_op(int mode, float alpha, float beta) {
   for (int p = 0; p < 2; ++p) o.a[p] = o.b[p] = o.a_lo[p] = o.b_lo[p] = o.out16[p] = o.out16_lo[p] = -1;
   o.cin32 = o.cout32 = -1;
   o.cin16[0] = o.cin16[1] = -1;
+  o.cin16_lo[0] = o.cin16_lo[1] = -1;
   o.mode = mode;
   o.alpha = alpha;
   o.beta = beta;
@@ -641,17 +642,22 @@ static nolsm_status sign_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, double mu, 
   ChainOp &e = pg.ops[0] = make_op(EPI_IDENT, 1.f, 0.f);
   ChainOp &x = pg.ops[1] = make_op(EPI_AXPBY, 0.5f, 1.f);
   e.resid = 1;
-  x.cin32 = x.cout32 = 0;
+  b->x_split = fp16;
+  b->x32_valid = !fp16;
   if (fp16) {
-    // X16: h0/h1 (ping-pong), E16: h4
-    LAUNCH(ctx, launch_make_x0(b, Bm, (float)mu, b->d_norm, scale_in, X32, b->h[0], nullptr, b->d_scale, st));
-    pg.group = group_size(ctx, b, 10);
+    // Master iterate as hi + lo * 2^-11 (22 bits, reading 12): hi IS the FP16 operand X16 (h0/h1,
+    // ping-pong), lo lives in h2 and is updated in place by the thread that owns the element; E16: h4.
+    // Per element and iteration the epilogues write 6 bytes (E, hi, lo) instead of 8 (E, FP32 master, FP16 copy).
+    LAUNCH(ctx, launch_make_x0(b, Bm, (float)mu, b->d_norm, scale_in, nullptr, b->h[0], b->h[2], b->d_scale, st));
+    pg.group = group_size(ctx, b, 6);
     set2(e.a, 0, 1); set2(e.b, 0, 1); set2(e.out16, 4, 4);
-    set2(x.a, 0, 1); set2(x.b, 4, 4); set2(x.out16, 1, 0);
+    set2(x.a, 0, 1); set2(x.b, 4, 4); set2(x.cin16, 0, 1); set2(x.cin16_lo, 2, 2);
+    set2(x.out16, 1, 0); set2(x.out16_lo, 2, 2); x.lo_stream = 1;
   } else {
     // split operands: X (h0,h1)/(h2,h3), E (h4,h5)
+    x.cin32 = x.cout32 = 0;
     LAUNCH(ctx, launch_make_x0(b, Bm, (float)mu, b->d_norm, scale_in, X32, b->h[0], b->h[1], b->d_scale, st));
-    pg.group = group_size(ctx, b, 16);
+    pg.group = group_size(ctx, b, 12);
     set2(e.a, 0, 2); set2(e.a_lo, 1, 3); set2(e.b, 0, 2); set2(e.b_lo, 1, 3);
     set2(e.out16, 4, 4); set2(e.out16_lo, 5, 5);
     set2(x.a, 0, 2); set2(x.a_lo, 1, 3); set2(x.b, 4, 4); set2(x.b_lo, 5, 5);
@@ -809,8 +815,19 @@ static nolsm_status sign_batch(nolsm_ctx *ctx, nolsm_batch *b, double mu, int pr
                                int fixed_iter, const float *scale_in, cudaStream_t st, bool timed,
                                bool fold_last = false) {
   b->x_pending = false;
+  b->x_split = false;
+  b->x32_valid = true;
   if (b->engine_simt) return sign_batch_simt(ctx, b, mu, tol, max_iter, fixed_iter, scale_in, st);
   return sign_batch_chain(ctx, b, mu, precision, tol, max_iter, fixed_iter, scale_in, st, timed, fold_last);
+}
+
+// SM cycles of the last chain kernel of the batch (max over its CTAs), in millions; synchronises
+static float chain_mcycles(nolsm_ctx *ctx, const nolsm_batch *b, cudaStream_t st) {
+  int32_t kc = 0;
+  if (b->engine_simt || b->count == 0) return 0.f;
+  if (cudaMemcpyAsync(&kc, b->d_sched + 3, sizeof(int32_t), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+      cudaStreamSynchronize(st) != cudaSuccess) { cudaGetLastError(); return 0.f; }
+  return (float)kc * (1024.f / 1e6f);
 }
 
 static float chain_ms(nolsm_ctx *ctx, const nolsm_batch *b) {
@@ -823,6 +840,17 @@ static float chain_ms(nolsm_ctx *ctx, const nolsm_batch *b) {
 static float *sinv_ptr(const nolsm_batch *b) { return b->engine_simt ? b->u[4] : b->u[2]; }
 static float *bmat_ptr(const nolsm_batch *b) { return b->engine_simt ? b->u[2] : b->u[3]; }
 static float *x_ptr(const nolsm_batch *b) { return (b->engine_simt && b->x_parity) ? b->u[3] : b->u[0]; }
+static XRef x_ref(const nolsm_batch *b) {
+  if (b->x_split && !b->engine_simt) return XRef{nullptr, b->h[0], b->h[1], b->h[2]};
+  return XRef{x_ptr(b), nullptr, nullptr, nullptr};
+}
+// FP32 copy of a split sign iterate in u0, for the consumers that read X as FP32
+static nolsm_status join_x(nolsm_ctx *ctx, nolsm_batch *b, cudaStream_t st) {
+  if (!b->x_split || b->engine_simt || b->x32_valid) return NOLSM_OK;
+  LAUNCH(ctx, launch_join_split(b, x_ref(b), b->u[0], st));
+  b->x32_valid = true;
+  return NOLSM_OK;
+}
 
 // Collect per-submatrix iteration counts and residuals (synchronises).
 static nolsm_status collect_stats(nolsm_ctx *ctx, nolsm_batch *b, float tol, int fixed_iter, cudaStream_t st,
@@ -897,6 +925,7 @@ extern "C" nolsm_status nolsm_sign_batched(nolsm_ctx *ctx, nolsm_batch *batch, d
     stats->flops_prepare = fp;
     stats->gemms = gemms + 2 * stats->iter_sum;
     stats->ms_chain = chain_ms(ctx, batch);
+    stats->chain_mcycles = chain_mcycles(ctx, batch, st);
   }
   return NOLSM_OK;
 }
@@ -934,7 +963,7 @@ extern "C" nolsm_status nolsm_scatter_density(nolsm_ctx *ctx, const nolsm_batch 
     }
     u_thin = bm->d_thin;
   }
-  LAUNCH(ctx, launch_density(batch, x_ptr(batch), nullptr, sinv_ptr(batch), S->row_ptr, S->col_idx, D->val,
+  LAUNCH(ctx, launch_density(batch, x_ref(batch), sinv_ptr(batch), S->row_ptr, S->col_idx, D->val,
                              ne_diag, batch->h[4], batch->x_pending_split ? batch->h[5] : nullptr, u_thin, st));
   LAUNCH(ctx, launch_trace(batch, S->row_ptr, S->col_idx, D->val, S->val, ne_partial, q_mol, st));
   return NOLSM_OK;
@@ -965,6 +994,7 @@ extern "C" nolsm_status nolsm_scatter_energy(nolsm_ctx *ctx, nolsm_batch *batch,
       }
       batch->thin_cap = need;
     }
+    CHECK(join_x(ctx, batch, st));
     cudaError_t e = launch_energy_weighted(batch, x_ptr(batch), sinv_ptr(batch), batch->u[1], H->row_ptr, H->col_idx,
                                            batch->d_thin, W->val, st);
     ctx->launches += 4;
@@ -1304,11 +1334,13 @@ extern "C" nolsm_status nolsm_sign_dense_batched(nolsm_ctx *ctx, const float *a,
   b->engine_simt = use_simt(ctx);
   LAUNCH(ctx, launch_pack(a, n, batch, b->ld, bmat_ptr(b), 0, st));
   CHECK(sign_batch(ctx, b, 0.0, prec, tol, max_iter, fixed_iter, scale, st, stats != nullptr));
+  CHECK(join_x(ctx, b, st));
   LAUNCH(ctx, launch_unpack(x_ptr(b), b->ld, (int64_t)b->ld * b->ld, nullptr, nullptr, n, batch, x_out, st));
   if (stats) {
     CHECK(collect_stats(ctx, b, tol, fixed_iter, st, stats));
     stats->gemms = 2 * stats->iter_sum;
     stats->ms_chain = chain_ms(ctx, b);
+    stats->chain_mcycles = chain_mcycles(ctx, b, st);
   }
   return NOLSM_OK;
 }
@@ -1316,6 +1348,7 @@ extern "C" nolsm_status nolsm_sign_dense_batched(nolsm_ctx *ctx, const float *a,
 extern "C" nolsm_status nolsm_batch_read(nolsm_ctx *ctx, const nolsm_batch *b, int32_t local, int32_t which,
                                          float *dst, int64_t dst_elems, int32_t *n_out, void *stream) {
   if (!ctx || !b || !dst || local < 0 || local >= b->count) return NOLSM_EINVAL;
+  if (which == NOLSM_MAT_X && b->prepared) CHECK(join_x(ctx, const_cast<nolsm_batch *>(b), (cudaStream_t)stream));
   const int n = b->n_host[local];
   if (n_out) *n_out = n;
   if (dst_elems < (int64_t)n * n) { ctx->err = "dst too small"; return NOLSM_ENOMEM; }

@@ -1,49 +1,42 @@
-// Epilogue of the matrix-iteration engine, shared by the single-CTA kernel (chain_umma.cu) and the
-// pair-CTA kernel (chain_pair.cu): one epilogue warp drains its 32 TMEM lanes (= 32 rows) of the tile
-// in 32-column chunks, applies the fused epilogue of the op
+// Epilogue and completion protocol of the matrix-iteration engine (chain_engine.cu), shared by its
+// single-CTA and CTA-pair instantiations: one epilogue warp drains its 32 TMEM lanes (= 32 rows) of the
+// tile in 32-column chunks, applies the fused epilogue of the op
 //     EPI_IDENT :  E = I - A B,  ||E||_F^2 over the true n x n part (stop rule, reading 9)
-//     EPI_AXPBY :  C = beta * C32 + alpha * A B   (FP32 master update, reading 12)
-// and writes the FP32 result and the FP16 operand copies (hi [, lo * 2^11]) with coalesced stores: the
-// lanes of a warp hold consecutive rows, so every store instruction writes one contiguous 128-byte
-// (FP32) or 64-byte (FP16) segment of a column.  Measured store rate of an SM into L2 with this
-// pattern: ~29 B/clk (FP32), ~20 B/clk (FP16) -- the floor of the epilogue (profiles/r1_k_chain_sign_w32768.md).
+//     EPI_AXPBY :  C = beta * C_in + alpha * A B   (master update, reading 12)
+// and writes the FP32 result and/or the FP16 operand copies (hi [, lo * 2^11]).  The lanes of a warp hold
+// consecutive rows of a column-major matrix, so every store instruction writes one contiguous 128-byte
+// (FP32) or 64-byte (FP16) segment of a column.
 //
-// Completion protocol (per submatrix and op): after the stores of a tile the epilogue warps of the
-// CTA meet at a named barrier and ONE elected thread makes them visible (__threadfence) and adds 1 to
-// tiles_done[m]; the arrival that completes the op evaluates the stop rule and publishes ready[m].
-// (One fence + one atomic round trip cost ~3000 cycles; paid by one warp per tile, not by all eight.)
+// Completion protocol (rolling window, chain_engine.cu): after the stores of a tile the epilogue warps of
+// the CTA meet at a named barrier and ONE elected thread makes them visible (__threadfence) and adds 1 to
+// slot_done[s]; the arrival that completes the op evaluates the stop rule and publishes the slot's next
+// state (same submatrix, next op -- or the next submatrix of the batch) with one 64-bit release store.
 #pragma once
 #include "common.cuh"
 
-// store flavours (experiments: -DNOLSM_ST=1 streaming .cs, 2 write-through .wt, 3 .cg)
-#if NOLSM_ST == 1
-#define ST32(p, v) __stcs((p), (v))
-#define ST16(p, v) __stcs(reinterpret_cast<unsigned short *>(p), __half_as_ushort(v))
-#elif NOLSM_ST == 2
-#define ST32(p, v) __stwt((p), (v))
-#define ST16(p, v) __stwt(reinterpret_cast<unsigned short *>(p), __half_as_ushort(v))
-#elif NOLSM_ST == 3
-#define ST32(p, v) __stcg((p), (v))
-#define ST16(p, v) __stcg(reinterpret_cast<unsigned short *>(p), __half_as_ushort(v))
-#else
-#define ST32(p, v) (*(p) = (v))
-#define ST16(p, v) (*(p) = (v))
-#endif
-
 namespace chainep {
 
-constexpr int32_t kDone = 0x7fffffff;
-
-struct TileCmd {              // scheduler -> TMA producer(s), MMA issuer and epilogue warps
+struct TileCmd {              // scheduler -> TMA producer(s), MMA issuer and epilogue warps (48 bytes)
   int32_t mat, m0, n0, nt;    // submatrix, first row / column of the tile, tile columns
   int32_t kblocks, ktail;     // K blocks of 64; K=16 steps in the last one (1..4)
   int32_t op, iter;           // op < 0: no more tiles
+  int32_t slot, pad0, pad1, pad2;   // window slot the submatrix occupies
 };
 
 // TileCmd::iter carries the iteration in its low bits and, in bit 30, a flip of the operand-table parity
 // (ChainProgram::parity_from_iters).
 __device__ __forceinline__ int cmd_iter(const TileCmd &c) { return c.iter & 0x3fffffff; }
 __device__ __forceinline__ int cmd_par(const TileCmd &c) { return (c.iter ^ (c.iter >> 30)) & 1; }
+
+// Slot state word: round (24 bits) | ops of the submatrix already completed (8 bits) | submatrix (32 bits).
+// A retired slot (no submatrix left to admit) holds kSlotDead: its round compares >= every round.
+constexpr unsigned long long kSlotDead = 0xffffffffffffffffull;
+__device__ __forceinline__ unsigned long long slot_pack(uint32_t round, uint32_t q, uint32_t mat) {
+  return ((unsigned long long)round << 40) | ((unsigned long long)(q & 0xffu) << 32) | (unsigned long long)mat;
+}
+__device__ __forceinline__ uint32_t slot_round(unsigned long long s) { return (uint32_t)(s >> 40); }
+__device__ __forceinline__ uint32_t slot_q(unsigned long long s) { return (uint32_t)(s >> 32) & 0xffu; }
+__device__ __forceinline__ int32_t slot_mat(unsigned long long s) { return (int32_t)(uint32_t)s; }
 
 struct ChainArgs {
   ChainProgram prog;
@@ -57,8 +50,14 @@ struct ChainArgs {
   int32_t mt, ntl;            // uniform tile grid per submatrix: mt row tiles x ntl column tiles
   const int32_t *dims;
   const float *alpha_div;
-  int32_t *ready, *tiles_done, *state, *iters, *group_active;
-  unsigned long long *tile_counter;   // next tile index to claim (dynamic scheduling)
+  // rolling window of `window` submatrices
+  int32_t window;
+  unsigned long long *slot_state;     // [window]
+  int32_t *slot_done;                 // [window] tiles of the slot's current op completed
+  int32_t *sched;                     // [0] next submatrix to admit, [1] retired slots, [2] submatrices that hit max_iter,
+                                      // [3] SM cycles / 1024 of the launch (max over CTAs; statistics)
+  unsigned long long *tile_counter;   // next tile index to claim (dynamic, in-order scheduling)
+  int32_t *state, *iters;
   float *resid2, *lastres;
   // scaled Newton-Schulz start (nolsm_config.gap_hint): alpha_tab[m * kAlphaSteps + k] = alpha_k of submatrix m
   // for iteration k < kAlphaSteps (1 afterwards); null = the plain iteration
@@ -66,7 +65,6 @@ struct ChainArgs {
 };
 constexpr int kAlphaSteps = 8;
 
-__device__ __forceinline__ uint32_t s32(const void *p) { return static_cast<uint32_t>(__cvta_generic_to_shared(p)); }
 __device__ __forceinline__ void ld_tmem32(uint32_t taddr, uint32_t (&v)[32]) {
   asm volatile(
       "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
@@ -80,8 +78,8 @@ __device__ __forceinline__ void ld_tmem32(uint32_t taddr, uint32_t (&v)[32]) {
       : "r"(taddr));
 }
 __device__ __forceinline__ void ld_tmem_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
-__device__ __forceinline__ void st_release_gpu(int32_t *p, int32_t v) {
-  asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+__device__ __forceinline__ void st_release_gpu_u64(unsigned long long *p, unsigned long long v) {
+  asm volatile("st.release.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
 }
 
 // Called by ONE thread per CTA and tile after the CTA's epilogue warps have passed their barrier.
@@ -94,11 +92,10 @@ __device__ __forceinline__ void epi_complete(const ChainArgs &args, const TileCm
   const int n = args.dims[c.mat];
   const int ncol = (n + kColRound - 1) / kColRound * kColRound;
   const int tiles_m = ((n + kTileM - 1) / kTileM) * ((ncol + args.bn - 1) / args.bn);
-  const int need = cmd_iter(c) * pg.n_ops + c.op;
   const int limit = pg.fixed_iter > 0 ? min(pg.fixed_iter, pg.max_iter) : pg.max_iter;
   __threadfence();      // the CTA's stores (ordered before us by the barrier) become visible GPU-wide
-  const int32_t old = atomicAdd(&args.tiles_done[c.mat], 1);
-  if (old + 1 != (need + 1) * tiles_m * kArrivals) return;
+  const int32_t old = atomicAdd(&args.slot_done[c.slot], 1);
+  if (old + 1 != tiles_m * kArrivals) return;
   __threadfence();
   const int k = cmd_iter(c);
   if (o.resid) {
@@ -106,56 +103,194 @@ __device__ __forceinline__ void epi_complete(const ChainArgs &args, const TileCm
         &args.resid2[(size_t)(k % NOLSM_MAX_RESID_SLOTS) * args.count + c.mat]);
     const float res = sqrtf(fmaxf(r2, 0.f) / (float)n);
     args.lastres[c.mat] = res;
-    bool stop = pg.fixed_iter > 0 ? (k + 1 >= pg.fixed_iter) : ((res < pg.tol) || !(res == res));
+    const bool conv = res < pg.tol;   // false for a NaN residual
+    bool stop = pg.fixed_iter > 0 ? (k + 1 >= pg.fixed_iter) : (conv || !(res == res));
     // a scaled step (alpha_k > 1) measures ||I - alpha^2 X^2||, not the residual of the stop rule
     if (args.alpha_tab != nullptr && k < kAlphaSteps && pg.fixed_iter <= 0 && res == res &&
         args.alpha_tab[c.mat * kAlphaSteps + k] > 1.f)
       stop = false;
     if (k + 1 >= pg.max_iter) stop = true;
+    // ended by the cap or by a NaN, not by a passing residual: the submatrix counts as not converged
+    if (stop && pg.fixed_iter <= 0 && !conv) atomicAdd(&args.sched[2], 1);
     args.iters[c.mat] = (stop && pg.stop_early) ? k : k + 1;   // iterations carried out in full
     if (stop) *reinterpret_cast<volatile int32_t *>(&args.state[c.mat]) = k;
   }
   const int32_t stv = *reinterpret_cast<volatile int32_t *>(&args.state[c.mat]);
-  // stop_early: the residual product is op 0; the schedulers waiting for ops 1.. of this iteration see
-  // kDone and skip their tiles
+  // stop_early: the residual product is op 0 and the remaining products of a passing iteration are not run
   const bool early = pg.stop_early && o.resid && stv == k;
+  const unsigned long long cur = *reinterpret_cast<volatile unsigned long long *>(&args.slot_state[c.slot]);
+  const uint32_t round = slot_round(cur);
+  args.slot_done[c.slot] = 0;
+  unsigned long long next;
   if (early || (c.op == pg.n_ops - 1 && (stv == k || k + 1 >= limit))) {
-    st_release_gpu(&args.ready[c.mat], kDone);
-    __threadfence();
-    atomicSub(&args.group_active[c.mat / pg.group], 1);
+    // this submatrix is finished: the slot admits the next one of the batch, or retires
+    const int32_t m2 = atomicAdd(&args.sched[0], 1);
+    if (m2 < args.count) {
+      next = slot_pack(round + 1, 0, (uint32_t)m2);
+    } else {
+      next = kSlotDead;
+      atomicAdd(&args.sched[1], 1);
+    }
   } else {
-    st_release_gpu(&args.ready[c.mat], need + 1);
+    next = slot_pack(round + 1, slot_q(cur) + 1, (uint32_t)c.mat);
   }
+  __threadfence();
+  st_release_gpu_u64(&args.slot_state[c.slot], next);
 }
 
-// Cached per-tile epilogue parameters and the prefetch of the first FP32-master chunk; call before
-// waiting for the accumulator.
-struct EpiTile {
-  const ChainOp *o;
-  int par, n, r, nchunks, chunk_first;
-  bool split, ident, has_cin, rows_in;
-  float alpha, beta;
-  float *p32;                 // FP32 output, element (r, first chunk column) or null
-  const float *cinp;          // FP32 master input, same position, or null
-  const __half *cinh;         // FP16 add-in instead (ChainOp::cin16), or null
-  __half *p16, *p16l;         // FP16 outputs (hi, lo), same position, or null
-  float cpre[32];
+// ------------------------------------------------------------------------------------------------
+// Staged epilogue.  Every FP16 stream of the epilogue -- the FP16 add-in (master hi [+ lo]) and the FP16
+// outputs (operand copies hi [+ lo]) -- moves between global memory and a shared-memory staging buffer by TMA
+// (2D boxes of 128 rows x 64 columns, issued by ONE agent thread), never by per-lane loads and stores: a
+// warp's column segment of 32 FP16 values is a 64-byte request, and such requests cost the SM's L2 port as
+// much as 128-byte ones (measured: the same epilogue with 2-byte per-lane accesses ran 18 % slower than with
+// 4-byte ones).  FP32 streams (one-shot products of the prepare stage) stay on the direct path: a warp's FP32
+// column segment is a full 128-byte line.
+//
+// The eight compute warps (TMEM lane quadrant q = warp % 4, column half h) work through the tile in chunks of
+// 64 columns; two staging buffers of two planes (hi, lo), plane layout [64 columns][128 rows] FP16.
+// Protocol per chunk and buffer:
+//   agent:    buffer free (its last store has been read) -> TMA loads of the add-in, or a plain arrive -> in_full
+//   compute:  tcgen05.ld; wait in_full; add-in from smem; results into the SAME smem positions; fence; -> out_ready
+//   agent:    wait out_ready; TMA stores; commit
+// After the last chunk of a tile the agent waits for its stores to complete, waits for the compute warps
+// (tile_done: their direct stores and residual atomics are issued) and publishes the tile (epi_complete).
+// ------------------------------------------------------------------------------------------------
+constexpr int kChunkCols = 64;
+constexpr int kPlaneBytes = 128 * kChunkCols * 2;  // one FP16 plane of a chunk
+constexpr int kStageBufBytes = 2 * kPlaneBytes;    // hi + lo
+constexpr int kStagingBytes = 2 * kStageBufBytes;  // two buffers
+constexpr int kComputeWarps = 8;
+
+struct EpiBars {
+  uint64_t in_full[2], out_ready[2], tile_done;
 };
 
-__device__ __forceinline__ void epi_begin(const ChainArgs &args, const TileCmd &c, int row0, bool rows_in, int lane,
-                                          int chunk_first, EpiTile &t) {
+__device__ __forceinline__ uint32_t s32(const void *p) { return static_cast<uint32_t>(__cvta_generic_to_shared(p)); }
+__device__ __forceinline__ void ebar_wait(uint64_t *bar, uint32_t parity) {
+  asm volatile(
+      "{\n\t"
+      ".reg .pred p;\n\t"
+      "EWAIT_LOOP:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+      "@p bra EWAIT_DONE;\n\t"
+      "bra EWAIT_LOOP;\n\t"
+      "EWAIT_DONE:\n\t"
+      "}\n" ::"r"(s32(bar)),
+      "r"(parity)
+      : "memory");
+}
+__device__ __forceinline__ void ebar_arrive(uint64_t *bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(s32(bar)) : "memory");
+}
+__device__ __forceinline__ void ebar_expect_tx(uint64_t *bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(s32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void tma_load_box(void *dst, const CUtensorMap *map, uint64_t *bar, int c0, int c1, int c2) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
+      ::"r"(s32(dst)), "l"(reinterpret_cast<uint64_t>(map)), "r"(s32(bar)), "r"(c0), "r"(c1), "r"(c2)
+      : "memory");
+}
+__device__ __forceinline__ void tma_store_box(const void *src, const CUtensorMap *map, int c0, int c1, int c2) {
+  asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.bulk_group [%0, {%2, %3, %4}], [%1];" ::"l"(
+                   reinterpret_cast<uint64_t>(map)),
+               "r"(s32(src)), "r"(c0), "r"(c1), "r"(c2)
+               : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+
+// What a tile's op moves through the staging buffers (the same for the agent and the compute warps)
+struct EpiIO {
+  int in_hi, in_lo, out_hi, out_lo;   // FP16 buffer indices, -1: none
+  int nchunks;                        // chunks of 64 columns
+};
+__device__ __forceinline__ EpiIO epi_io(const ChainArgs &args, const TileCmd &c) {
+  const ChainOp &o = args.prog.ops[c.op];
+  const int par = cmd_par(c);
+  EpiIO io;
+  const bool ident = o.mode == EPI_IDENT;
+  const bool cin = !ident && o.beta != 0.f && o.cin16[par] >= 0;
+  io.in_hi = cin ? o.cin16[par] : -1;
+  io.in_lo = cin ? o.cin16_lo[par] : -1;
+  io.out_hi = o.out16[par];
+  io.out_lo = o.out16_lo[par];
+  io.nchunks = (c.nt + kChunkCols - 1) / kChunkCols;
+  return io;
+}
+
+// ---- the agent: one thread ----
+// emaps: the {128 x 64} box maps of the FP16 buffers; stage: the two staging buffers; row0: first row of this
+// CTA's part of the tile; uses[b]: completed uses of buffer b (barrier phases).
+__device__ __forceinline__ void epi_agent_tile(const ChainArgs &args, const TileCmd &c, const CUtensorMap *emaps,
+                                               uint8_t *stage, EpiBars &bars, int row0, uint32_t (&uses)[2]) {
+  const EpiIO io = epi_io(args, c);
+  const int nch = io.nchunks;
+  auto avail = [&](int j) {
+    const int b = j & 1;
+    uint8_t *buf = stage + b * kStageBufBytes;
+    const int col = c.n0 + kChunkCols * j;
+    if (io.in_hi >= 0) {
+      ebar_expect_tx(&bars.in_full[b], (uint32_t)kPlaneBytes * (io.in_lo >= 0 ? 2u : 1u));
+      tma_load_box(buf, &emaps[io.in_hi], &bars.in_full[b], row0, col, c.mat);
+      if (io.in_lo >= 0) tma_load_box(buf + kPlaneBytes, &emaps[io.in_lo], &bars.in_full[b], row0, col, c.mat);
+    } else {
+      ebar_arrive(&bars.in_full[b]);
+    }
+  };
+  if (nch > 0) avail(0);
+  if (nch > 1) avail(1);
+  for (int j = 0; j < nch; ++j) {
+    const int b = j & 1;
+    ebar_wait(&bars.out_ready[b], uses[b] & 1u);
+    ++uses[b];
+    const uint8_t *buf = stage + b * kStageBufBytes;
+    const int col = c.n0 + kChunkCols * j;
+    if (io.out_hi >= 0) tma_store_box(buf, &emaps[io.out_hi], row0, col, c.mat);
+    if (io.out_lo >= 0) tma_store_box(buf + kPlaneBytes, &emaps[io.out_lo], row0, col, c.mat);
+    bulk_commit();
+    if (j + 2 < nch) {
+      bulk_wait_read0();     // the store just issued has read the buffer: it may take the next add-in
+      avail(j + 2);
+    }
+  }
+  bulk_wait0();              // this tile's stores are complete (and both buffers free for the next tile)
+}
+
+// ---- compute warp: cached per-tile parameters ----
+struct EpiTile {
+  const ChainOp *o;
+  int par, n, r, nchunks, h;
+  bool split, ident, cin_direct;
+  float alpha, beta;
+  float *p32;                 // FP32 output, element (r, first column of this warp) or null
+  const float *cinp;          // FP32 master input (direct path), same position, or null
+  EpiIO io;
+  float cpre[32];             // direct path only: add-in of the next chunk
+};
+
+__device__ __forceinline__ void epi_prefetch32(const ChainArgs &args, EpiTile &t) {
+  const float *pc = t.cinp;
+#pragma unroll
+  for (int j = 0; j < 32; ++j) { t.cpre[j] = __ldcg(pc); pc += args.ld; }
+}
+
+// Before waiting for the accumulator.  row0: first row of this warp's quadrant; h: column half of the chunks.
+__device__ __forceinline__ void epi_begin(const ChainArgs &args, const TileCmd &c, int row0, int lane, int h,
+                                          EpiTile &t) {
   const ChainOp &o = args.prog.ops[c.op];
   t.o = &o;
   t.par = cmd_par(c);
   t.n = args.dims[c.mat];
   t.r = row0 + lane;
-  t.rows_in = rows_in;
-  t.nchunks = (c.nt + 31) >> 5;
-  t.chunk_first = chunk_first;
+  t.h = h;
+  t.io = epi_io(args, c);
+  t.nchunks = t.io.nchunks;
   t.split = o.a_lo[t.par] >= 0;
   t.ident = o.mode == EPI_IDENT;
-  const bool cin_half = o.cin16[t.par] >= 0;
-  t.has_cin = !t.ident && (o.cin32 >= 0 || cin_half) && o.beta != 0.f && rows_in;
+  t.cin_direct = !t.ident && o.cin32 >= 0 && o.beta != 0.f && t.io.in_hi < 0;
   t.alpha = o.use_div ? o.alpha / args.alpha_div[c.mat] : o.alpha;
   t.beta = o.beta;
   if (args.alpha_tab != nullptr && cmd_iter(c) < kAlphaSteps) {
@@ -163,126 +298,99 @@ __device__ __forceinline__ void epi_begin(const ChainArgs &args, const TileCmd &
     const float a = args.alpha_tab[c.mat * kAlphaSteps + cmd_iter(c)];
     if (t.ident) t.alpha *= a * a; else { t.alpha *= a; t.beta *= a; }
   }
-  const int64_t off = (int64_t)c.mat * args.slab + t.r + (int64_t)(c.n0 + 32 * chunk_first) * args.ld;
-  t.p32 = (o.cout32 >= 0 && rows_in) ? args.ubuf[o.cout32] + off : nullptr;
-  t.cinp = (t.has_cin && !cin_half) ? args.ubuf[o.cin32] + off : nullptr;
-  t.cinh = (t.has_cin && cin_half) ? args.hbuf[o.cin16[t.par]] + off : nullptr;
-  t.p16 = (o.out16[t.par] >= 0 && rows_in) ? args.hbuf[o.out16[t.par]] + off : nullptr;
-  t.p16l = (o.out16_lo[t.par] >= 0 && rows_in) ? args.hbuf[o.out16_lo[t.par]] + off : nullptr;
-#if defined(NOLSM_NOEPI) || defined(NOLSM_NOCIN)   // timing experiments only (results are wrong)
-  t.has_cin = false;
-#endif
-#ifdef NOLSM_NOSTORE
-  t.p32 = nullptr; t.p16 = nullptr; t.p16l = nullptr;
-#endif
-#ifdef NOLSM_SCRATCHSTORE   // all stores of a CTA land in one small L2-resident region (same request count, no DRAM traffic)
-  {
-    const int64_t o2 = (int64_t)(blockIdx.x & 15) * args.slab + t.r % 128 + (int64_t)(32 * chunk_first) * args.ld;
-    if (t.p32) t.p32 = args.ubuf[o.cout32] + o2;
-    if (t.p16) t.p16 = args.hbuf[o.out16[t.par]] + o2;
-    if (t.p16l) t.p16l = args.hbuf[o.out16_lo[t.par]] + o2;
-  }
-#endif
-  if (t.has_cin && chunk_first < t.nchunks) {
-    if (t.cinh) {
-      const __half *ph = t.cinh;
-#pragma unroll
-      for (int j = 0; j < 32; ++j) { t.cpre[j] = __half2float(__ldcg(ph)); ph += args.ld; }
-    } else {
-      const float *pc = t.cinp;
-#pragma unroll
-      for (int j = 0; j < 32; ++j) { t.cpre[j] = __ldcg(pc); pc += args.ld; }
-    }
-  }
+  const int64_t off = (int64_t)c.mat * args.slab + t.r + (int64_t)(c.n0 + 32 * h) * args.ld;
+  t.p32 = o.cout32 >= 0 ? args.ubuf[o.cout32] + off : nullptr;
+  t.cinp = t.cin_direct ? args.ubuf[o.cin32] + off : nullptr;
+  if (t.cin_direct && 32 * h < c.nt) epi_prefetch32(args, t);
 }
 
-// Drains this warp's chunks of the accumulator at TMEM address t_main (lane quadrant and accumulator
-// stage already applied); returns the warp's partial residual sum (lane-local; reduce before use).
+// Drains this warp's 32 columns of every chunk of the accumulator at TMEM address t_main (lane quadrant and
+// accumulator stage already applied).  stage: the staging buffers; q: lane quadrant; uses[b]: completed uses of
+// buffer b.  Returns the warp's partial residual sum (lane-local; reduce before use).
 __device__ __forceinline__ float epi_chunks(const ChainArgs &args, const TileCmd &c, EpiTile &t, uint32_t t_main,
-                                            int lane, long long *tr = nullptr) {
-#define EPI_TR(j) do { if (tr && lane == 0 && ci == t.chunk_first) tr[j] = clock64(); } while (0)
+                                            int lane, int q, uint8_t *stage, EpiBars &bars, uint32_t (&uses)[2]) {
   float ss = 0.f;
-  if (!t.rows_in) return ss;
-#ifdef NOLSM_NOEPI   // timing experiment only: main loop without any epilogue work (results are wrong)
-  return ss;
-#endif
-  const ChainOp &o = *t.o;
-  const int64_t chunk_stride = (int64_t)32 * args.ld;
-  for (int ci = t.chunk_first; ci < t.nchunks; ci += 2) {
-    const int c0 = ci * 32;
-    const int cnt = min(32, c.nt - c0);   // 16 or 32 valid columns
+  const int64_t chunk_stride = (int64_t)kChunkCols * args.ld;
+  const int soff = (32 * t.h) * 256 + 2 * (32 * q + lane);   // this thread's first element inside a staging plane
+  for (int ci = 0; ci < t.nchunks; ++ci) {
+    const int b = ci & 1;
+    const int c0 = ci * kChunkCols + 32 * t.h;
+    const int cnt = max(0, min(32, c.nt - c0));   // 0, 16 or 32 valid columns
     uint32_t v[32];
-    ld_tmem32(t_main + c0, v);
-    if (t.split) {
-      uint32_t w[32];
-      ld_tmem32(t_main + 128 + c0, w);
-      ld_tmem_wait();
+    if (cnt > 0) {
+      ld_tmem32(t_main + c0, v);
+      if (t.split) {
+        uint32_t w[32];
+        ld_tmem32(t_main + 128 + c0, w);
+        ld_tmem_wait();
 #pragma unroll
-      for (int j = 0; j < 32; ++j)
-        v[j] = __float_as_uint(fmaf(__uint_as_float(w[j]), 1.f / 2048.f, __uint_as_float(v[j])));
-    } else {
-      ld_tmem_wait();
+        for (int jj = 0; jj < 32; ++jj)
+          v[jj] = __float_as_uint(fmaf(__uint_as_float(w[jj]), 1.f / 2048.f, __uint_as_float(v[jj])));
+      } else {
+        ld_tmem_wait();
+      }
     }
-    EPI_TR(2);
-    if (t.has_cin) {
+    // the staging buffer is free (its previous store has been read) and holds this chunk's add-in, if any
+    ebar_wait(&bars.in_full[b], uses[b] & 1u);
+    ++uses[b];
+    uint8_t *hi_col = stage + b * kStageBufBytes + soff;
+    uint8_t *lo_col = hi_col + kPlaneBytes;
+    if (cnt > 0) {
+      if (t.io.in_hi >= 0) {
+        const bool has_lo = t.io.in_lo >= 0;
 #pragma unroll
-      for (int j = 0; j < 32; ++j)
-        v[j] = __float_as_uint(fmaf(t.beta, t.cpre[j], t.alpha * __uint_as_float(v[j])));
-      if (ci + 2 < t.nchunks) {
-        if (t.cinh) {
-          t.cinh += 2 * chunk_stride;
-          const __half *ph = t.cinh;
-#pragma unroll
-          for (int j = 0; j < 32; ++j) { t.cpre[j] = __half2float(__ldcg(ph)); ph += args.ld; }
-        } else {
-          t.cinp += 2 * chunk_stride;
-          const float *pc = t.cinp;
-#pragma unroll
-          for (int j = 0; j < 32; ++j) { t.cpre[j] = __ldcg(pc); pc += args.ld; }
+        for (int jj = 0; jj < 32; ++jj) {
+          float cin = __half2float(*reinterpret_cast<const __half *>(hi_col + jj * 256));
+          if (has_lo) cin = fmaf(__half2float(*reinterpret_cast<const __half *>(lo_col + jj * 256)), 1.f / 2048.f, cin);
+          v[jj] = __float_as_uint(fmaf(t.beta, cin, t.alpha * __uint_as_float(v[jj])));
         }
-      }
-    } else if (t.ident) {
-      // valid columns of this chunk inside the true n x n part (residual of the stop rule)
-      const int nvalid = (t.r < t.n) ? min(cnt, t.n - (c.n0 + c0)) : 0;
-      const int dj = t.r - (c.n0 + c0);     // chunk column that holds the diagonal element of row r
+      } else if (t.cin_direct) {
 #pragma unroll
-      for (int j = 0; j < 32; ++j) {
-        const float e = fmaf(-t.alpha, __uint_as_float(v[j]), (j == dj) ? 1.f : 0.f);
-        if (j < nvalid) ss = fmaf(e, e, ss);
-        v[j] = __float_as_uint(e);
-      }
-    } else {
+        for (int jj = 0; jj < 32; ++jj)
+          v[jj] = __float_as_uint(fmaf(t.beta, t.cpre[jj], t.alpha * __uint_as_float(v[jj])));
+        if (c0 + kChunkCols < c.nt) {
+          t.cinp += chunk_stride;
+          epi_prefetch32(args, t);
+        }
+      } else if (t.ident) {
+        // valid columns of this chunk inside the true n x n part (residual of the stop rule)
+        const int nvalid = (t.r < t.n) ? min(cnt, t.n - (c.n0 + c0)) : 0;
+        const int dj = t.r - (c.n0 + c0);     // chunk column that holds the diagonal element of row r
 #pragma unroll
-      for (int j = 0; j < 32; ++j) v[j] = __float_as_uint(t.alpha * __uint_as_float(v[j]));
+        for (int jj = 0; jj < 32; ++jj) {
+          const float e = fmaf(-t.alpha, __uint_as_float(v[jj]), (jj == dj) ? 1.f : 0.f);
+          if (jj < nvalid) ss = fmaf(e, e, ss);
+          v[jj] = __float_as_uint(e);
+        }
+      } else {
+#pragma unroll
+        for (int jj = 0; jj < 32; ++jj) v[jj] = __float_as_uint(t.alpha * __uint_as_float(v[jj]));
+      }
+      if (t.p32) {   // FP32 result (direct): one 128-byte segment per column and warp
+        float *qp = t.p32;
+#pragma unroll
+        for (int jj = 0; jj < 16; ++jj) { *qp = __uint_as_float(v[jj]); qp += args.ld; }
+        if (cnt == 32) {
+#pragma unroll
+          for (int jj = 16; jj < 32; ++jj) { *qp = __uint_as_float(v[jj]); qp += args.ld; }
+        }
+        t.p32 += chunk_stride;
+      }
     }
-    EPI_TR(3);
-    if (t.p32) {   // FP32 result: one 128-byte segment per column and warp
-      float *q = t.p32;
+    if (t.io.out_hi >= 0) {   // FP16 copies into the staging planes; columns beyond the tile are written as zero
+      const bool has_lo = t.io.out_lo >= 0;
 #pragma unroll
-      for (int j = 0; j < 16; ++j) { ST32(q, __uint_as_float(v[j])); q += args.ld; }
-      if (cnt == 32) {
-#pragma unroll
-        for (int j = 16; j < 32; ++j) { ST32(q, __uint_as_float(v[j])); q += args.ld; }
-      }
-      t.p32 += 2 * chunk_stride;
-    }
-    EPI_TR(4);
-    if (t.p16) {   // FP16 operand copies: one 64-byte segment per column and warp
-      __half *q = t.p16, *ql = t.p16l;
-#pragma unroll
-      for (int j = 0; j < 32; ++j) {
-        if (j == 16 && cnt < 32) break;
-        const float val = __uint_as_float(v[j]);
+      for (int jj = 0; jj < 32; ++jj) {
+        const float val = jj < cnt ? __uint_as_float(v[jj]) : 0.f;
         const __half hi = __float2half_rn(val);
-        ST16(q, hi); q += args.ld;
-        if (ql) { *ql = __float2half_rn((val - __half2float(hi)) * 2048.f); ql += args.ld; }
+        *reinterpret_cast<__half *>(hi_col + jj * 256) = hi;
+        if (has_lo) *reinterpret_cast<__half *>(lo_col + jj * 256) = __float2half_rn((val - __half2float(hi)) * 2048.f);
       }
-      t.p16 += 2 * chunk_stride;
-      if (t.p16l) t.p16l += 2 * chunk_stride;
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy smem writes -> TMA store
     }
-    EPI_TR(6);
+    __syncwarp();
+    if (lane == 0) ebar_arrive(&bars.out_ready[b]);
   }
-#undef EPI_TR
   return ss;
 }
 

@@ -57,6 +57,9 @@ struct ChainOp {
   int32_t cin32, cout32;          // FP32 units read (AXPBY, beta != 0) / written, -1: none
   int32_t cin16[2];               // instead of cin32: the add-in is an FP16 buffer (by parity), -1: none.  For
                                   // iterations whose result is refined afterwards: no FP32 master is kept
+  int32_t cin16_lo[2];            // lo part of a split add-in (master iterate kept as hi + lo * 2^-11), -1: none
+  int32_t lo_stream;              // 1: out16_lo / cin16_lo are touched once per iteration and never by an MMA: streaming
+                                  // (evict-first) loads and stores, so that they do not take L2 from the operands
   int32_t mode;                   // EPI_IDENT: I - A B     EPI_AXPBY: beta * Cin + alpha * A B
   int32_t resid;                  // 1: ||result||_F^2 over the true n x n part drives the stop rule
   int32_t use_div;                // alpha /= alpha_div[submatrix]
@@ -68,7 +71,7 @@ struct ChainProgram {
   int32_t n_ops;                  // products per iteration, strictly ordered per submatrix
   int32_t max_iter, fixed_iter;   // fixed_iter > 0: exactly that many iterations, no residual test
   float tol;                      // stop rule of DESIGN.md reading 9 on the residual of the `resid` op
-  int32_t group;                  // submatrices iterated together (L2 residency)
+  int32_t group;                  // window: submatrices in flight together (L2 residency)
   int32_t parity_from_iters;      // 1: the operand tables are indexed by the parity of the LAST full iteration of
                                   // the chain that ran before on this batch ((iters[m] + 1) & 1) instead of the
                                   // own iteration's: lets a one-shot product read the final FP16 iterate in place
@@ -84,6 +87,8 @@ struct nolsm_batch {
   bool x_pending = false;         // the sign chain stopped after E_k = I - X_k^2 passed the test: the update
                                   // X_{k+1} = X_k + 1/2 X_k E_k is folded into the density columns (reading 9)
   bool x_pending_split = false;   // E_k is stored as hi + lo (FP32 mode)
+  bool x_split = false;           // the sign iterate lives as hi (h[iters & 1]) + lo * 2^-11 (h[2]); u[0] holds X in
+  bool x32_valid = false;         // FP32 only after join_x (reading 12)
   bool s_split_built = false;     // the builder wrote the split copy of S into h[n_half-4], h[n_half-3]
   bool prefer_pair = false;       // batch shape favours the pair engine (nolsm.h, NOLSM_FLAG_*)
   bool engine_simt = false;       // prepared by the FP32 SIMT debugging path (different buffer roles)
@@ -115,9 +120,9 @@ struct nolsm_batch {
   float *u[NOLSM_MAX_UNIT] = {nullptr};
   __half *h[NOLSM_MAX_HALF] = {nullptr};
   int32_t n_half = 6, n_unit = 7; // buffers laid out in this batch (precision dependent)
-  int32_t *d_ready = nullptr;     // [count] chain engine: ops completed per submatrix
-  int32_t *d_tiles_done = nullptr;// [count] chain engine: epilogue-warp arrivals per submatrix
-  int32_t *d_group_active = nullptr; // [count] chain engine: unfinished submatrices per group
+  unsigned long long *d_slot_state = nullptr;      // [count] chain engine: window slots (chain_epilogue.cuh)
+  int32_t *d_slot_done = nullptr; // [count] chain engine: completed tiles of a slot's current op
+  int32_t *d_sched = nullptr;     // [4] chain engine: next submatrix to admit, retired slots, unconverged count
   unsigned long long *d_tile_counter = nullptr;   // chain engine: next tile index to claim
   float *d_thin = nullptr;        // [2][count][6][ld] scratch of the thin products (energy-weighted density)
   size_t thin_cap = 0;            // floats
@@ -144,8 +149,6 @@ struct nolsm_ctx {
   bool umma_ok = false;
   bool pair_ok = false;           // pair-CTA (cta_group::2) engine usable
   int pair_clusters = 0;          // co-resident CTA pairs
-  bool mcast_ok = false;          // cluster-multicast engine usable
-  int mcast_clusters = 0;
   // device mirrors of the caller's HOST store (nolsm_solve_mu_host), grown on demand
   int32_t *m_row_ptr = nullptr, *m_col_idx = nullptr;
   float *m_h = nullptr, *m_s = nullptr, *m_d = nullptr;
@@ -182,7 +185,13 @@ cudaError_t launch_gather(const nolsm_batch *b, const int32_t *row_ptr, const in
 cudaError_t launch_pack_square(const nolsm_batch *b, float *dense, float *packed, bool save, cudaStream_t st);
 cudaError_t launch_own_columns(const nolsm_batch *b, const int32_t *row_ptr, const int32_t *col_idx, float *mat,
                                float *packed, bool save, cudaStream_t st);
-cudaError_t launch_density(const nolsm_batch *b, const float *x, const float *x_alt, const float *sinv,
+// the sign iterate as the kernels of a5 read it: FP32, or split hi (by the parity of iters) + lo
+struct XRef {
+  const float *x32;
+  const __half *hi0, *hi1, *lo;   // hi0 != null: split
+};
+cudaError_t launch_join_split(const nolsm_batch *b, const XRef &x, float *dst32, cudaStream_t st);
+cudaError_t launch_density(const nolsm_batch *b, const XRef &x, const float *sinv,
                            const int32_t *row_ptr, const int32_t *col_idx, float *d_val,
                            double *ne_diag, const __half *e_hi, const __half *e_lo, float *u_thin,
                            cudaStream_t st);
@@ -221,11 +230,5 @@ cudaError_t launch_gemm_simt(const GemmParams &p, cudaStream_t st);
 // tcgen05 path
 nolsm_status umma_init(nolsm_ctx *ctx);
 nolsm_status umma_make_maps(nolsm_ctx *ctx, nolsm_batch *b);
-nolsm_status pair_init(nolsm_ctx *ctx);
-cudaError_t launch_chain_pair(nolsm_ctx *ctx, const nolsm_batch *b, const ChainProgram &prog, const float *alpha_div,
-                              cudaStream_t st);
-nolsm_status mcast_init(nolsm_ctx *ctx);
-cudaError_t launch_chain_mcast(nolsm_ctx *ctx, const nolsm_batch *b, const ChainProgram &prog, const float *alpha_div,
-                               cudaStream_t st);
 cudaError_t launch_chain(nolsm_ctx *ctx, const nolsm_batch *b, const ChainProgram &prog, const float *alpha_div,
                          bool touch_stats, cudaStream_t st);

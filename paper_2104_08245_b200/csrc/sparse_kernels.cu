@@ -490,9 +490,21 @@ cudaError_t launch_own_columns(const nolsm_batch *b, const int32_t *row_ptr, con
 
 #define DN_THREADS 256
 
+// element of the sign iterate: FP32, or hi + lo * 2^-11 (the split master of DESIGN.md reading 12)
+template <bool kSplit>
+struct XMat {
+  const float *x32;
+  const __half *hi, *lo;
+  __device__ __forceinline__ float at(int64_t off) const {
+    if constexpr (kSplit) return fmaf(__half2float(__ldg(lo + off)), 1.f / 2048.f, __half2float(__ldg(hi + off)));
+    else return __ldg(x32 + off);
+  }
+};
+
+template <bool kSplit>
 __global__ void __launch_bounds__(DN_THREADS)
 k_density(const int32_t *__restrict__ row_ptr, const int32_t *__restrict__ col_idx, int mol_begin,
-          int ld, int64_t slab, const float *__restrict__ x, const float *__restrict__ x_alt,
+          int ld, int64_t slab, const XRef xr,
           const int32_t *__restrict__ iters, const float *__restrict__ sinv,
           const float *__restrict__ u_thin, const __half *__restrict__ e_hi, const __half *__restrict__ e_lo,
           float *__restrict__ d_val, double *__restrict__ ne_diag) {
@@ -511,7 +523,13 @@ k_density(const int32_t *__restrict__ row_ptr, const int32_t *__restrict__ col_i
     if (col_idx[lo + mid] < j) l = mid + 1; else r_ = mid;
   }
   const int own0 = l * NOLSM_BS;
-  const float *xj = ((x_alt != nullptr && (iters[mat] & 1)) ? x_alt : x) + (int64_t)mat * slab;
+  XMat<kSplit> xj;
+  if constexpr (kSplit) {
+    xj.hi = ((iters[mat] & 1) ? xr.hi1 : xr.hi0) + (int64_t)mat * slab;
+    xj.lo = xr.lo + (int64_t)mat * slab;
+  } else {
+    xj.x32 = xr.x32 + (int64_t)mat * slab;
+  }
   const float *sj = sinv + (int64_t)mat * slab;
   const float *uj = u_thin ? u_thin + (int64_t)mat * NOLSM_BS * ld : nullptr;
   for (int t = threadIdx.x; t < NOLSM_BS * n; t += blockDim.x) {
@@ -526,7 +544,7 @@ k_density(const int32_t *__restrict__ row_ptr, const int32_t *__restrict__ col_i
     for (int p = 0; p < NOLSM_BS; ++p) acc[p] = 0.f;
 #pragma unroll 8
     for (int k = 0; k < n; ++k) {   // X column by column (coalesced); S^-1 row k as three broadcast 8-byte loads
-      const float xv = __ldg(xj + (int64_t)k * ld + r);
+      const float xv = xj.at((int64_t)k * ld + r);
       const float2 *sk = reinterpret_cast<const float2 *>(s_sinv + k * NOLSM_BS);
       const float2 s0 = sk[0], s1 = sk[1], s2 = sk[2];
       acc[0] = fmaf(xv, s0.x, acc[0]); acc[1] = fmaf(xv, s0.y, acc[1]); acc[2] = fmaf(xv, s1.x, acc[2]);
@@ -539,14 +557,14 @@ k_density(const int32_t *__restrict__ row_ptr, const int32_t *__restrict__ col_i
       out[p] = 0.5f * (v - acc[p]);
     }
     if (ne_diag != nullptr && r >= own0 && r < own0 + NOLSM_BS) {
-      float xrr = xj[(int64_t)r * ld + r];
+      float xrr = xj.at((int64_t)r * ld + r);
       if (uj) {   // diagonal element of X_{k+1} = X_k + 1/2 X_k E_k
         const int64_t eoff = (int64_t)mat * slab + (int64_t)r * ld;
         float dot = 0.f;
         for (int k = 0; k < n; ++k) {
           float e = __half2float(e_hi[eoff + k]);
           if (e_lo) e = fmaf(__half2float(e_lo[eoff + k]), 1.f / 2048.f, e);
-          dot = fmaf(xj[(int64_t)k * ld + r], e, dot);
+          dot = fmaf(xj.at((int64_t)k * ld + r), e, dot);
         }
         xrr = fmaf(0.5f, dot, xrr);
       }
@@ -604,26 +622,57 @@ k_last_half(const int32_t *__restrict__ row_ptr, const int32_t *__restrict__ col
   }
 }
 
-cudaError_t launch_density(const nolsm_batch *b, const float *x, const float *x_alt, const float *sinv,
+// FP32 copy of a split iterate (for the consumers that read X as FP32: energy products, nolsm_batch_read)
+__global__ void __launch_bounds__(256)
+k_join_split(const int32_t *__restrict__ dims, const int32_t *__restrict__ iters, int ld, int64_t slab, const XRef xr,
+             float *__restrict__ dst) {
+  const int mat = blockIdx.y;
+  const int n = dims[mat];
+  const int P = (n + 3) & ~3;
+  const int64_t per = (int64_t)(P >> 2) * n;
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= per) return;
+  const int c = (int)(i / (P >> 2)), r = (int)(i % (P >> 2)) * 4;
+  const int64_t off = (int64_t)mat * slab + (int64_t)c * ld + r;
+  const __half *hi = ((iters[mat] & 1) ? xr.hi1 : xr.hi0) + off;
+  const __half *lo = xr.lo + off;
+  float v[4];
+#pragma unroll
+  for (int k = 0; k < 4; ++k) v[k] = fmaf(__half2float(lo[k]), 1.f / 2048.f, __half2float(hi[k]));
+  *reinterpret_cast<float4 *>(dst + off) = make_float4(v[0], v[1], v[2], v[3]);
+}
+
+cudaError_t launch_join_split(const nolsm_batch *b, const XRef &x, float *dst32, cudaStream_t st) {
+  if (b->count == 0) return cudaSuccess;
+  const int P = (b->max_n + 3) & ~3;
+  dim3 grid((unsigned)(((int64_t)(P >> 2) * b->max_n + 255) / 256), (unsigned)b->count);
+  k_join_split<<<grid, 256, 0, st>>>(b->d_dims, b->d_iters, b->ld, (int64_t)b->ld * b->ld, x, dst32);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_density(const nolsm_batch *b, const XRef &x, const float *sinv,
                            const int32_t *row_ptr, const int32_t *col_idx, float *d_val,
                            double *ne_diag, const __half *e_hi, const __half *e_lo, float *u_thin,
                            cudaStream_t st) {
   if (b->count == 0) return cudaSuccess;
   const size_t smem = (size_t)NOLSM_BS * b->max_n * sizeof(float);
-  static size_t smem_set = 0;
-  if (smem > 48 * 1024 && smem > smem_set) {
-    cudaError_t e = cudaFuncSetAttribute(k_density, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (smem > 200 * 1024) return cudaErrorInvalidValue;   // six columns of one submatrix must fit in shared memory
+  if (smem > 48 * 1024) {   // per device and cheap: set on every such launch (a process may use several devices)
+    cudaError_t e = cudaFuncSetAttribute(k_density<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_density<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_last_half, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    smem_set = smem;
   }
   dim3 grid((b->max_n + DN_THREADS - 1) / DN_THREADS, b->count);
   if (u_thin)   // the last iteration is pending (e_hi [+ e_lo] = E_k): U = V + 1/2 E_k V first
     k_last_half<<<grid, DN_THREADS, smem, st>>>(row_ptr, col_idx, b->mol_begin, b->ld, (int64_t)b->ld * b->ld,
                                                 e_hi, e_lo, sinv, u_thin);
-  k_density<<<grid, DN_THREADS, smem, st>>>(row_ptr, col_idx, b->mol_begin, b->ld,
-                                            (int64_t)b->ld * b->ld, x, x_alt, b->d_iters, sinv, u_thin, e_hi, e_lo,
-                                            d_val, ne_diag);
+  if (x.hi0)
+    k_density<true><<<grid, DN_THREADS, smem, st>>>(row_ptr, col_idx, b->mol_begin, b->ld, (int64_t)b->ld * b->ld, x,
+                                                    b->d_iters, sinv, u_thin, e_hi, e_lo, d_val, ne_diag);
+  else
+    k_density<false><<<grid, DN_THREADS, smem, st>>>(row_ptr, col_idx, b->mol_begin, b->ld, (int64_t)b->ld * b->ld, x,
+                                                     b->d_iters, sinv, u_thin, e_hi, e_lo, d_val, ne_diag);
   return cudaGetLastError();
 }
 
@@ -737,11 +786,10 @@ static cudaError_t thin_launch(const nolsm_batch *b, const int32_t *row_ptr, con
                                const float *in_thin, const float *in_cols, const float *add_thin, float alpha,
                                float beta, float *out_thin, float *out_blocks, cudaStream_t st) {
   const size_t smem = (size_t)NOLSM_BS * b->max_n * sizeof(float);
-  static size_t smem_set = 0;
-  if (smem > 48 * 1024 && smem > smem_set) {
+  if (smem > 200 * 1024) return cudaErrorInvalidValue;
+  if (smem > 48 * 1024) {   // per device: set on every such launch
     cudaError_t e = cudaFuncSetAttribute(k_thin, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    smem_set = smem;
   }
   dim3 grid((b->max_n + DN_THREADS - 1) / DN_THREADS, b->count);
   k_thin<<<grid, DN_THREADS, smem, st>>>(row_ptr, col_idx, b->mol_begin, b->ld, (int64_t)b->ld * b->ld, a, in_thin,

@@ -23,6 +23,8 @@ def main():
     ap.add_argument("--distinct", type=int, default=4)
     ap.add_argument("--flags", type=int, default=0)
     ap.add_argument("--reps", type=int, default=3)
+    ap.add_argument("--group", type=int, default=0, help="nolsm_config.group: window of submatrices in flight (0: default)")
+    ap.add_argument("--precisions", default="0,1", help="0 = FP16/FP32, 1 = FP32 quality")
     args = ap.parse_args()
     import torch
     import nolsm_inputs as gi
@@ -37,8 +39,8 @@ def main():
         a = torch.as_tensor(np.stack([m[0] for m in mats]))[torch.as_tensor(idx)].contiguous().cuda()
         scale = torch.as_tensor(np.array([np.abs(mats[i][2]).max() for i in idx], dtype=np.float32)).cuda()
         signs = [(m[1] * np.sign(m[2])[None, :]) @ m[1].T for m in mats]
-        for precision in (0, 1):
-            ctx = Context(Config(precision=precision, flags=args.flags))
+        for precision in [int(x) for x in args.precisions.split(",")]:
+            ctx = Context(Config(precision=precision, flags=args.flags, group=args.group))
             best, stats, x = None, None, None
             for _ in range(args.reps):
                 x, st = ctx.sign_dense_batched(a, scale)
@@ -47,8 +49,8 @@ def main():
             err = max(float(np.abs(x[i].cpu().numpy() - signs[idx[i]]).max()) for i in range(min(batch, len(mats))))
             print(json.dumps({"n": n, "batch": batch, "precision": "fp16/fp32" if precision == 0 else "fp32 (split fp16)",
                               "iterations": [stats.iter_min, stats.iter_max], "unconverged": stats.n_unconverged,
-                              "ms_kernel": round(best, 4), "tflops": round(stats.flops_sign / best * 1e-9, 1),
-                              "max_abs_err_vs_construction": err, "engine_flags": args.flags}), flush=True)
+                              "ms_kernel": round(best, 4), "sm_ghz": round(stats.chain_mcycles / max(best, 1e-9), 3), "tflops": round(stats.flops_sign / best * 1e-9, 1),
+                              "max_abs_err_vs_construction": err, "engine_flags": args.flags, "group": args.group}), flush=True)
             ctx.close()
     return 0
 

@@ -373,7 +373,7 @@ def test_baseline_configs_sampled(nolsm, name, precision, begin, count, sample):
 # ---------------------------------------------------------------------------------------------
 # the optional pair engines (cta_group::2 pair tiles / cluster multicast of the B operand)
 # ---------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("flag", ["FLAG_PAIR", "FLAG_MCAST"])
+@pytest.mark.parametrize("flag", ["FLAG_PAIR", "FLAG_SINGLE"])
 @pytest.mark.parametrize("precision", [0, 1])
 def test_pair_engines_density_tiny_and_mid(nolsm, tiny_system, tiny_solution, mid_system, mid_solution, flag, precision):
     """Same parity bounds as the default engine, through nolsm_solve_mu (tiny) and a partial batch (mid:
@@ -405,7 +405,7 @@ def test_pair_engines_density_tiny_and_mid(nolsm, tiny_system, tiny_solution, mi
     ctx.close()
 
 
-@pytest.mark.parametrize("flag", ["FLAG_PAIR", "FLAG_MCAST"])
+@pytest.mark.parametrize("flag", ["FLAG_PAIR", "FLAG_SINGLE"])
 @pytest.mark.parametrize("kind,tol", [(1, 2e-2), (2, 2e-5)])
 @pytest.mark.parametrize("n,batch", [(64, 3), (146, 5), (300, 2), (863, 2)])
 def test_pair_engines_building_block(nolsm, torch_mod, flag, kind, tol, n, batch):
@@ -578,7 +578,7 @@ def test_w32768_whole_step_in_bench_configuration_sampled(nolsm):
     ctx.close()
 
 
-@pytest.mark.parametrize("flag", [0, "FLAG_PAIR", "FLAG_MCAST"])
+@pytest.mark.parametrize("flag", [0, "FLAG_PAIR", "FLAG_SINGLE"])
 def test_run_to_run_bitwise_identical(nolsm, flag):
     """The tile schedule is dynamic (claim order and timing differ from run to run) but every tile's arithmetic
     is fixed, so two runs must give bit-identical D: any race in the dependency protocol (a tile reading an
