@@ -2,10 +2,10 @@
 // dependent n x n x n products (every iteration of Eq. 9-10, or of Eq. 15-17
 // PAPER.md:203-215) for every submatrix of a batch on the 5th-generation tensor cores
 // (tcgen05 + TMEM + TMA), sm_100a only.  Two instantiations of one kernel template:
-//   k_chain<false>  one CTA per 128 x N tile (tcgen05.mma.cta_group::1)
-//   k_chain<true>   two CTAs of a cluster (one TPC) per 256 x N tile (cta_group::2): each CTA stages its own 128
-//                   rows of the A operand and only HALF of the B operand's columns, so the operand bytes an SM
-//                   takes in per 64-deep K block drop from 48 KB to 32 KB.
+//   k_chain<false>  one CTA per tile of N rows x 128 columns of the result (tcgen05.mma.cta_group::1)
+//   k_chain<true>   two CTAs of a cluster (one TPC) per tile of N rows x 256 columns (cta_group::2): each CTA stages
+//                   its own 128 columns of the right operand and only HALF of the rows of the left operand, so the
+//                   operand bytes an SM takes in per 64-deep K block drop from 48 KB to 32 KB.
 //
 // Why one kernel: the two products of a sign iteration are strictly dependent and one product of an
 // n ~ 860 submatrix is < 1 us of the whole GPU, so kernel boundaries would cost more than the work, and
@@ -25,14 +25,15 @@
 // (cooperative launch), so the schedule cannot deadlock.
 //
 // Layout facts:
-//   * all matrices are column-major, so the A operand (M x K) is M-major and the B operand (K x N) is
-//     K-major in shared memory; one TMA tensor map per FP16 buffer with box {64 storage rows,
-//     64 storage columns} serves both roles (A: 2 boxes per 128-row tile and K block; B: one box per
-//     64 tile columns), 128-byte swizzle.
-//   * accumulator: 128 TMEM lanes = tile rows, one 32-bit column per tile column; two accumulator
+//   * all matrices are column-major.  The tensor cores compute the TRANSPOSED product C^T = R^T L^T of every
+//     C = L R: the MMA's M side runs over 128 COLUMNS of C and takes the right operand R (for a fixed column
+//     its K elements are contiguous: K-major), the N side runs over up to 256 ROWS of C and takes the left
+//     operand L (for a fixed k its rows are contiguous: MN-major).  Nothing is transposed in memory; one TMA
+//     tensor map per FP16 buffer with box {64 storage rows, 64 storage columns}, 128-byte swizzle, serves both
+//     roles.  The point is the epilogue: TMEM lane = column of C, TMEM column = row of C, so a thread holds 32
+//     CONSECUTIVE elements of a column and moves them with 16-byte accesses (chain_epilogue.cuh).
+//   * accumulator: 128 TMEM lanes = tile columns, one 32-bit TMEM column per tile row; two accumulator
 //     stages so the epilogue of tile i overlaps the MMAs of tile i+1.
-//   * the master iterate (reading 12) is read in the epilogue with L2-only loads
-//     (ld.global.cg: other SMs wrote it) issued one chunk ahead, and written back with coalesced stores.
 //
 // Warp roles (384 threads): warp 0 = scheduler (leader CTA; claims the next tile, resolves its dependency and
 // writes the tile command into the ring of every CTA of the cluster), warp 1 = MMA issuer (leader CTA; whole warp,
@@ -315,6 +316,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
         const int k = q / pg.n_ops, op = q % pg.n_ops;
         const int n = args.dims[m];
         const int n16 = (n + 15) & ~15, ncol = (n + kColRound - 1) & ~(kColRound - 1);
+        // m0: first COLUMN of the result tile (the MMA's M side), n0: first ROW (N side)
         const int m0 = (t % args.mt) * kTileM, n0 = (t / args.mt) * args.bn;
         if (m0 >= n || n0 >= ncol) continue;            // tile outside this submatrix
         const int kblocks = (n16 + kBK - 1) / kBK;
@@ -339,15 +341,16 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
         const ChainOp &o = pg.ops[c.op];
         const int par = chainep::cmd_par(c);
         const int m = c.mat;
-        const int m0 = c.m0 + NOLSM_TILE_M * (int)rank;       // this CTA's rows of the tile
-        const int my_n = kPair ? (c.nt >> 1) : c.nt;          // this CTA's share of the B columns
+        const int m0 = c.m0 + NOLSM_TILE_M * (int)rank;       // this CTA's columns of the result tile
+        const int my_n = kPair ? (c.nt >> 1) : c.nt;          // this CTA's share of the tile's rows (N side)
         const int n0 = c.n0 + (kPair ? my_n * (int)rank : 0);
         const bool split = o.a_lo[par] >= 0;
         const int nbox = (my_n + 63) >> 6;
         const uint32_t bytes = (uint32_t)kCtas * (uint32_t)(kATileBytes + nbox * kBoxBytes) * (split ? 2u : 1u);
-        const CUtensorMap *ma = &args.maps[o.a[par]], *mb = &args.maps[o.b[par]];
-        const CUtensorMap *mal = split ? &args.maps[o.a_lo[par]] : nullptr;
-        const CUtensorMap *mbl = split ? &args.maps[o.b_lo[par]] : nullptr;
+        // M side <- right operand (K-major), N side <- left operand (MN-major)
+        const CUtensorMap *ma = &args.maps[o.b[par]], *mb = &args.maps[o.a[par]];
+        const CUtensorMap *mal = split ? &args.maps[o.b_lo[par]] : nullptr;
+        const CUtensorMap *mbl = split ? &args.maps[o.a_lo[par]] : nullptr;
         const int kb_go = max(0, c.kblocks - kClaimLead);
         for (int kb = 0; kb < c.kblocks; ++kb) {
           if (leader && kb == kb_go) mbar_arrive<false>(&claim_go);   // the scheduler may claim the next tile
@@ -355,15 +358,15 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
           uint8_t *st = smem + (size_t)stage * args.stage_bytes;
           if (leader) mbar_expect_tx(&full_bar[stage], bytes);
           const int k0 = kb * kBK;
-          tma_load_3d<kPair>(st, ma, &full_bar[stage], m0, k0, m);
-          tma_load_3d<kPair>(st + kBoxBytes, ma, &full_bar[stage], m0 + 64, k0, m);
+          tma_load_3d<kPair>(st, ma, &full_bar[stage], k0, m0, m);
+          tma_load_3d<kPair>(st + kBoxBytes, ma, &full_bar[stage], k0, m0 + 64, m);
           for (int j = 0; j < nbox; ++j)
-            tma_load_3d<kPair>(st + off_b + j * kBoxBytes, mb, &full_bar[stage], k0, n0 + 64 * j, m);
+            tma_load_3d<kPair>(st + off_b + j * kBoxBytes, mb, &full_bar[stage], n0 + 64 * j, k0, m);
           if (split) {
-            tma_load_3d<kPair>(st + off_a_lo, mal, &full_bar[stage], m0, k0, m);
-            tma_load_3d<kPair>(st + off_a_lo + kBoxBytes, mal, &full_bar[stage], m0 + 64, k0, m);
+            tma_load_3d<kPair>(st + off_a_lo, mal, &full_bar[stage], k0, m0, m);
+            tma_load_3d<kPair>(st + off_a_lo + kBoxBytes, mal, &full_bar[stage], k0, m0 + 64, m);
             for (int j = 0; j < nbox; ++j)
-              tma_load_3d<kPair>(st + off_b_lo + j * kBoxBytes, mbl, &full_bar[stage], k0, n0 + 64 * j, m);
+              tma_load_3d<kPair>(st + off_b_lo + j * kBoxBytes, mbl, &full_bar[stage], n0 + 64 * j, k0, m);
           }
           if (++stage == args.stages) { stage = 0; phase ^= 1u; }
         }
@@ -388,8 +391,8 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
         if (++slot == kRing) { slot = 0; ring_phase ^= 1u; }
         if (c.op < 0) break;
         const bool split = pg.ops[c.op].a_lo[chainep::cmd_par(c)] >= 0;
-        // instruction descriptor: D=F32, A=B=F16, A M-major, B K-major, N = nt, M = 128 per CTA
-        const uint32_t idesc = (1u << 4) | (1u << 15) | ((uint32_t)(c.nt >> 3) << 17) | ((uint32_t)(kTileM >> 4) << 24);
+        // instruction descriptor: D=F32, A=B=F16, A K-major, B MN-major, N = nt, M = 128 per CTA
+        const uint32_t idesc = (1u << 4) | (1u << 16) | ((uint32_t)(c.nt >> 3) << 17) | ((uint32_t)(kTileM >> 4) << 24);
         mbar_wait<kPair>(&tempty_bar[acc], acc_phase ^ 1u);
         tc_fence_after();
         const uint32_t d_main = tmem_base + (uint32_t)(acc * 256);
@@ -397,26 +400,26 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
         for (int kb = 0; kb < c.kblocks; ++kb) {
           mbar_wait<kPair>(&full_bar[stage], phase);
           tc_fence_after();
-          // descriptor low halves: (address >> 4) | leading offset << 16; A (M-major): leading offset = the
-          // second 64-row chunk (8192 B), +2048 B per K=16 step; B (K-major): leading offset 16 B, +32 B per step
+          // descriptor low halves: (address >> 4) | leading offset << 16; A (K-major): leading offset 16 B, +32 B
+          // per K=16 step; B (MN-major): leading offset = the next 64-row chunk (8192 B), +2048 B per step
           const uint32_t sa = smem_base + (uint32_t)stage * (uint32_t)args.stage_bytes;
-          const uint32_t a_lo = ((sa >> 4) & 0x3FFFu) | ((uint32_t)(kBoxBytes >> 4) << 16);
-          const uint32_t b_lo = (((sa + off_b) >> 4) & 0x3FFFu) | (1u << 16);
+          const uint32_t a_lo = ((sa >> 4) & 0x3FFFu) | (1u << 16);
+          const uint32_t b_lo = (((sa + off_b) >> 4) & 0x3FFFu) | ((uint32_t)(kBoxBytes >> 4) << 16);
           const int steps = kb == c.kblocks - 1 ? c.ktail : kBK / 16;
           if (one) {
             if (!split) {
               tc_mma<kPair>(d_main, a_lo, b_lo, kDescHi, idesc, kb ? 1u : 0u);
-              if (steps > 1) tc_mma<kPair>(d_main, a_lo + 128u, b_lo + 2u, kDescHi, idesc, 1u);
-              if (steps > 2) tc_mma<kPair>(d_main, a_lo + 256u, b_lo + 4u, kDescHi, idesc, 1u);
-              if (steps > 3) tc_mma<kPair>(d_main, a_lo + 384u, b_lo + 6u, kDescHi, idesc, 1u);
+              if (steps > 1) tc_mma<kPair>(d_main, a_lo + 2u, b_lo + 128u, kDescHi, idesc, 1u);
+              if (steps > 2) tc_mma<kPair>(d_main, a_lo + 4u, b_lo + 256u, kDescHi, idesc, 1u);
+              if (steps > 3) tc_mma<kPair>(d_main, a_lo + 6u, b_lo + 384u, kDescHi, idesc, 1u);
             } else {
-              const uint32_t al_lo = (((sa + off_a_lo) >> 4) & 0x3FFFu) | ((uint32_t)(kBoxBytes >> 4) << 16);
-              const uint32_t bl_lo = (((sa + off_b_lo) >> 4) & 0x3FFFu) | (1u << 16);
+              const uint32_t al_lo = (((sa + off_a_lo) >> 4) & 0x3FFFu) | (1u << 16);
+              const uint32_t bl_lo = (((sa + off_b_lo) >> 4) & 0x3FFFu) | ((uint32_t)(kBoxBytes >> 4) << 16);
               for (int k4 = 0; k4 < steps; ++k4) {
                 const uint32_t accum = (kb | k4) ? 1u : 0u;
-                tc_mma<kPair>(d_main, a_lo + 128u * k4, b_lo + 2u * k4, kDescHi, idesc, accum);
-                tc_mma<kPair>(d_corr, a_lo + 128u * k4, bl_lo + 2u * k4, kDescHi, idesc, accum);
-                tc_mma<kPair>(d_corr, al_lo + 128u * k4, b_lo + 2u * k4, kDescHi, idesc, 1u);
+                tc_mma<kPair>(d_main, a_lo + 2u * k4, b_lo + 128u * k4, kDescHi, idesc, accum);
+                tc_mma<kPair>(d_corr, a_lo + 2u * k4, bl_lo + 128u * k4, kDescHi, idesc, accum);
+                tc_mma<kPair>(d_corr, al_lo + 2u * k4, b_lo + 128u * k4, kDescHi, idesc, 1u);
               }
             }
             tc_commit<kPair>(&empty_bar[stage]);
@@ -446,12 +449,12 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
       // the peer's half of the last pair tile may lie beyond the leading dimension: nothing to load or store
       const bool rows_in = c.m0 + NOLSM_TILE_M * (int)rank < args.ld;
       chainep::EpiTile t;
-      if (rows_in) chainep::epi_begin(args, c, c.m0 + NOLSM_TILE_M * (int)rank + q * 32, lane, h, t);
+      if (rows_in) chainep::epi_begin(args, c, c.m0 + NOLSM_TILE_M * (int)rank + q * 32 + lane, h, t);
       mbar_wait<kPair>(&tfull_bar[acc], acc_phase);
       tc_fence_after();
       const uint32_t t_main = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(acc * 256);
       float ss = 0.f;
-      if (rows_in) ss = chainep::epi_chunks(args, c, t, t_main, lane, q, staging, ebars, uses);
+      if (rows_in) ss = chainep::epi_chunks(args, c, t, t_main, lane, q * 32 + lane, staging, ebars, uses);
       tc_fence_before();
       __syncwarp();
       if (lane == 0) mbar_arrive<kPair>(&tempty_bar[acc], 0);
@@ -478,8 +481,8 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
         if (++slot == kRing) { slot = 0; ring_phase ^= 1u; }
         if (c.op < 0) break;
         fence_proxy_async();   // other CTAs' writes (ordered by the scheduler's acquire) -> TMA reads of the add-in
-        const int row0 = c.m0 + NOLSM_TILE_M * (int)rank;
-        if (row0 < args.ld) chainep::epi_agent_tile(args, c, emaps, staging, ebars, row0, uses);
+        const int col0 = c.m0 + NOLSM_TILE_M * (int)rank;   // first column of this CTA's part of the tile
+        if (col0 < args.ld) chainep::epi_agent_tile(args, c, emaps, staging, ebars, col0, uses);
         // the TMA stores of this tile are complete; wait until every compute warp has issued its direct stores
         // and residual atomic, then publish
         chainep::ebar_arrive(&ebars.tile_done);
@@ -608,11 +611,11 @@ nolsm_status umma_make_maps(nolsm_ctx *ctx, nolsm_batch *b) {
   b->maps_valid = false;
   if (!ctx->umma_ok || b->count == 0) return NOLSM_OK;
   // [0, n_half): operand maps ({64 x 64} boxes, 128-byte swizzle); [n_half, 2 n_half): epilogue maps of the same
-  // buffers ({128 rows x 64 columns} boxes, no swizzle: the staging planes of chain_epilogue.cuh)
+  // buffers ({64 rows x 128 columns} boxes, 128-byte swizzle: the staging planes of chain_epilogue.cuh)
   std::vector<CUtensorMap> maps(2 * b->n_half);
   for (int i = 0; i < b->n_half; ++i) {
     nolsm_status s = encode_map(ctx, &maps[i], b->h[i], b->ld, b->count, 64, 64, true);
-    if (s == NOLSM_OK) s = encode_map(ctx, &maps[b->n_half + i], b->h[i], b->ld, b->count, 128, chainep::kChunkCols, false);
+    if (s == NOLSM_OK) s = encode_map(ctx, &maps[b->n_half + i], b->h[i], b->ld, b->count, chainep::kChunkRows, 128, true);
     if (s != NOLSM_OK) return s;
   }
   if (!b->d_maps) {

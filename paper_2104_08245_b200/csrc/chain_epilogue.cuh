@@ -139,16 +139,19 @@ __device__ __forceinline__ void epi_complete(const ChainArgs &args, const TileCm
 }
 
 // ------------------------------------------------------------------------------------------------
-// Staged epilogue.  Every FP16 stream of the epilogue -- the FP16 add-in (master hi [+ lo]) and the FP16
-// outputs (operand copies hi [+ lo]) -- moves between global memory and a shared-memory staging buffer by TMA
-// (2D boxes of 128 rows x 64 columns, issued by ONE agent thread), never by per-lane loads and stores: a
-// warp's column segment of 32 FP16 values is a 64-byte request, and such requests cost the SM's L2 port as
-// much as 128-byte ones (measured: the same epilogue with 2-byte per-lane accesses ran 18 % slower than with
-// 4-byte ones).  FP32 streams (one-shot products of the prepare stage) stay on the direct path: a warp's FP32
-// column segment is a full 128-byte line.
+// Staged epilogue.  The engine computes the transposed product (chain_engine.cu), so TMEM lane = COLUMN of the
+// result and TMEM column = ROW: after tcgen05.ld a thread holds 32 consecutive elements of one column, i.e. 64
+// contiguous bytes of the column-major FP16 buffers.  Every FP16 stream of the epilogue -- the FP16 add-in
+// (master hi [+ lo]) and the FP16 outputs (operand copies hi [+ lo]) -- moves between global memory and a
+// shared-memory staging buffer by TMA (boxes of 64 rows x 128 columns, 128-byte swizzle, issued by ONE agent
+// thread), and the compute warps touch the staging planes with 16-byte accesses only.  (Per-lane 2-byte global
+// accesses cost the SM's L2 port as much per request as 4-byte ones, and 2-byte shared-memory accesses made the
+// epilogue LSU-issue-bound: measured.)  FP32 streams (one-shot products of the prepare stage) stay on the
+// direct path: 128 contiguous bytes per thread, 16-byte accesses.
 //
-// The eight compute warps (TMEM lane quadrant q = warp % 4, column half h) work through the tile in chunks of
-// 64 columns; two staging buffers of two planes (hi, lo), plane layout [64 columns][128 rows] FP16.
+// The eight compute warps (TMEM lane quadrant q = warp % 4 -> 32 columns of the tile, row half h) work through
+// the tile in chunks of 64 rows; two staging buffers of two planes (hi, lo); plane = [128 columns][64 rows] FP16
+// = 128 bytes per column, 16-byte pieces XOR-swizzled with (column % 8) like the TMA box.
 // Protocol per chunk and buffer:
 //   agent:    buffer free (its last store has been read) -> TMA loads of the add-in, or a plain arrive -> in_full
 //   compute:  tcgen05.ld; wait in_full; add-in from smem; results into the SAME smem positions; fence; -> out_ready
@@ -156,8 +159,8 @@ __device__ __forceinline__ void epi_complete(const ChainArgs &args, const TileCm
 // After the last chunk of a tile the agent waits for its stores to complete, waits for the compute warps
 // (tile_done: their direct stores and residual atomics are issued) and publishes the tile (epi_complete).
 // ------------------------------------------------------------------------------------------------
-constexpr int kChunkCols = 64;
-constexpr int kPlaneBytes = 128 * kChunkCols * 2;  // one FP16 plane of a chunk
+constexpr int kChunkRows = 64;
+constexpr int kPlaneBytes = 128 * kChunkRows * 2;  // one FP16 plane of a chunk
 constexpr int kStageBufBytes = 2 * kPlaneBytes;    // hi + lo
 constexpr int kStagingBytes = 2 * kStageBufBytes;  // two buffers
 constexpr int kComputeWarps = 8;
@@ -205,7 +208,7 @@ __device__ __forceinline__ void bulk_wait0() { asm volatile("cp.async.bulk.wait_
 // What a tile's op moves through the staging buffers (the same for the agent and the compute warps)
 struct EpiIO {
   int in_hi, in_lo, out_hi, out_lo;   // FP16 buffer indices, -1: none
-  int nchunks;                        // chunks of 64 columns
+  int nchunks;                        // chunks of 64 rows
 };
 __device__ __forceinline__ EpiIO epi_io(const ChainArgs &args, const TileCmd &c) {
   const ChainOp &o = args.prog.ops[c.op];
@@ -217,25 +220,25 @@ __device__ __forceinline__ EpiIO epi_io(const ChainArgs &args, const TileCmd &c)
   io.in_lo = cin ? o.cin16_lo[par] : -1;
   io.out_hi = o.out16[par];
   io.out_lo = o.out16_lo[par];
-  io.nchunks = (c.nt + kChunkCols - 1) / kChunkCols;
+  io.nchunks = (c.nt + kChunkRows - 1) / kChunkRows;
   return io;
 }
 
 // ---- the agent: one thread ----
-// emaps: the {128 x 64} box maps of the FP16 buffers; stage: the two staging buffers; row0: first row of this
-// CTA's part of the tile; uses[b]: completed uses of buffer b (barrier phases).
+// emaps: the {64 rows x 128 columns} box maps of the FP16 buffers; stage: the two staging buffers; col0: first
+// column of this CTA's part of the tile; uses[b]: completed uses of buffer b (barrier phases).
 __device__ __forceinline__ void epi_agent_tile(const ChainArgs &args, const TileCmd &c, const CUtensorMap *emaps,
-                                               uint8_t *stage, EpiBars &bars, int row0, uint32_t (&uses)[2]) {
+                                               uint8_t *stage, EpiBars &bars, int col0, uint32_t (&uses)[2]) {
   const EpiIO io = epi_io(args, c);
   const int nch = io.nchunks;
   auto avail = [&](int j) {
     const int b = j & 1;
     uint8_t *buf = stage + b * kStageBufBytes;
-    const int col = c.n0 + kChunkCols * j;
+    const int row = c.n0 + kChunkRows * j;
     if (io.in_hi >= 0) {
       ebar_expect_tx(&bars.in_full[b], (uint32_t)kPlaneBytes * (io.in_lo >= 0 ? 2u : 1u));
-      tma_load_box(buf, &emaps[io.in_hi], &bars.in_full[b], row0, col, c.mat);
-      if (io.in_lo >= 0) tma_load_box(buf + kPlaneBytes, &emaps[io.in_lo], &bars.in_full[b], row0, col, c.mat);
+      tma_load_box(buf, &emaps[io.in_hi], &bars.in_full[b], row, col0, c.mat);
+      if (io.in_lo >= 0) tma_load_box(buf + kPlaneBytes, &emaps[io.in_lo], &bars.in_full[b], row, col0, c.mat);
     } else {
       ebar_arrive(&bars.in_full[b]);
     }
@@ -247,9 +250,9 @@ __device__ __forceinline__ void epi_agent_tile(const ChainArgs &args, const Tile
     ebar_wait(&bars.out_ready[b], uses[b] & 1u);
     ++uses[b];
     const uint8_t *buf = stage + b * kStageBufBytes;
-    const int col = c.n0 + kChunkCols * j;
-    if (io.out_hi >= 0) tma_store_box(buf, &emaps[io.out_hi], row0, col, c.mat);
-    if (io.out_lo >= 0) tma_store_box(buf + kPlaneBytes, &emaps[io.out_lo], row0, col, c.mat);
+    const int row = c.n0 + kChunkRows * j;
+    if (io.out_hi >= 0) tma_store_box(buf, &emaps[io.out_hi], row, col0, c.mat);
+    if (io.out_lo >= 0) tma_store_box(buf + kPlaneBytes, &emaps[io.out_lo], row, col0, c.mat);
     bulk_commit();
     if (j + 2 < nch) {
       bulk_wait_read0();     // the store just issued has read the buffer: it may take the next add-in
@@ -262,32 +265,33 @@ __device__ __forceinline__ void epi_agent_tile(const ChainArgs &args, const Tile
 // ---- compute warp: cached per-tile parameters ----
 struct EpiTile {
   const ChainOp *o;
-  int par, n, r, nchunks, h;
+  int par, n, col, h;         // col: this thread's column of the result; h: row half of every chunk
   bool split, ident, cin_direct;
   float alpha, beta;
-  float *p32;                 // FP32 output, element (r, first column of this warp) or null
+  float *p32;                 // FP32 output, element (first row of this warp's half, col) or null
   const float *cinp;          // FP32 master input (direct path), same position, or null
   EpiIO io;
   float cpre[32];             // direct path only: add-in of the next chunk
 };
 
-__device__ __forceinline__ void epi_prefetch32(const ChainArgs &args, EpiTile &t) {
-  const float *pc = t.cinp;
+__device__ __forceinline__ void epi_prefetch32(EpiTile &t) {
+  const float4 *pc = reinterpret_cast<const float4 *>(t.cinp);
 #pragma unroll
-  for (int j = 0; j < 32; ++j) { t.cpre[j] = __ldcg(pc); pc += args.ld; }
+  for (int j = 0; j < 8; ++j) {
+    const float4 x = __ldcg(pc + j);
+    t.cpre[4 * j] = x.x; t.cpre[4 * j + 1] = x.y; t.cpre[4 * j + 2] = x.z; t.cpre[4 * j + 3] = x.w;
+  }
 }
 
-// Before waiting for the accumulator.  row0: first row of this warp's quadrant; h: column half of the chunks.
-__device__ __forceinline__ void epi_begin(const ChainArgs &args, const TileCmd &c, int row0, int lane, int h,
-                                          EpiTile &t) {
+// Before waiting for the accumulator.  col: this thread's column of the result; h: row half of the chunks.
+__device__ __forceinline__ void epi_begin(const ChainArgs &args, const TileCmd &c, int col, int h, EpiTile &t) {
   const ChainOp &o = args.prog.ops[c.op];
   t.o = &o;
   t.par = cmd_par(c);
   t.n = args.dims[c.mat];
-  t.r = row0 + lane;
+  t.col = col;
   t.h = h;
   t.io = epi_io(args, c);
-  t.nchunks = t.io.nchunks;
   t.split = o.a_lo[t.par] >= 0;
   t.ident = o.mode == EPI_IDENT;
   t.cin_direct = !t.ident && o.cin32 >= 0 && o.beta != 0.f && t.io.in_hi < 0;
@@ -298,24 +302,25 @@ __device__ __forceinline__ void epi_begin(const ChainArgs &args, const TileCmd &
     const float a = args.alpha_tab[c.mat * kAlphaSteps + cmd_iter(c)];
     if (t.ident) t.alpha *= a * a; else { t.alpha *= a; t.beta *= a; }
   }
-  const int64_t off = (int64_t)c.mat * args.slab + t.r + (int64_t)(c.n0 + 32 * h) * args.ld;
+  const int64_t off = (int64_t)c.mat * args.slab + (int64_t)col * args.ld + c.n0 + 32 * h;
   t.p32 = o.cout32 >= 0 ? args.ubuf[o.cout32] + off : nullptr;
   t.cinp = t.cin_direct ? args.ubuf[o.cin32] + off : nullptr;
-  if (t.cin_direct && 32 * h < c.nt) epi_prefetch32(args, t);
+  if (t.cin_direct && 32 * h < c.nt) epi_prefetch32(t);
 }
 
-// Drains this warp's 32 columns of every chunk of the accumulator at TMEM address t_main (lane quadrant and
-// accumulator stage already applied).  stage: the staging buffers; q: lane quadrant; uses[b]: completed uses of
-// buffer b.  Returns the warp's partial residual sum (lane-local; reduce before use).
+// Drains this warp's 32 rows of every chunk of the accumulator at TMEM address t_main (lane quadrant and
+// accumulator stage already applied).  stage: the staging buffers; cl: this thread's column inside the CTA's part
+// of the tile (0..127); uses[b]: completed uses of buffer b.  Returns the warp's partial residual sum (lane-local;
+// reduce before use).
 __device__ __forceinline__ float epi_chunks(const ChainArgs &args, const TileCmd &c, EpiTile &t, uint32_t t_main,
-                                            int lane, int q, uint8_t *stage, EpiBars &bars, uint32_t (&uses)[2]) {
+                                            int lane, int cl, uint8_t *stage, EpiBars &bars, uint32_t (&uses)[2]) {
   float ss = 0.f;
-  const int64_t chunk_stride = (int64_t)kChunkCols * args.ld;
-  const int soff = (32 * t.h) * 256 + 2 * (32 * q + lane);   // this thread's first element inside a staging plane
-  for (int ci = 0; ci < t.nchunks; ++ci) {
+  const int sw = cl & 7;                          // XOR swizzle of the 16-byte pieces of this column
+  const int scol = cl * (2 * kChunkRows);         // byte offset of this column inside a staging plane
+  for (int ci = 0; ci < t.io.nchunks; ++ci) {
     const int b = ci & 1;
-    const int c0 = ci * kChunkCols + 32 * t.h;
-    const int cnt = max(0, min(32, c.nt - c0));   // 0, 16 or 32 valid columns
+    const int c0 = ci * kChunkRows + 32 * t.h;    // first row (inside the tile) of this warp's part of the chunk
+    const int cnt = max(0, min(32, c.nt - c0));   // 0, 16 or 32 valid rows
     uint32_t v[32];
     if (cnt > 0) {
       ld_tmem32(t_main + c0, v);
@@ -333,29 +338,40 @@ __device__ __forceinline__ float epi_chunks(const ChainArgs &args, const TileCmd
     // the staging buffer is free (its previous store has been read) and holds this chunk's add-in, if any
     ebar_wait(&bars.in_full[b], uses[b] & 1u);
     ++uses[b];
-    uint8_t *hi_col = stage + b * kStageBufBytes + soff;
+    uint8_t *hi_col = stage + b * kStageBufBytes + scol;
     uint8_t *lo_col = hi_col + kPlaneBytes;
     if (cnt > 0) {
       if (t.io.in_hi >= 0) {
         const bool has_lo = t.io.in_lo >= 0;
 #pragma unroll
-        for (int jj = 0; jj < 32; ++jj) {
-          float cin = __half2float(*reinterpret_cast<const __half *>(hi_col + jj * 256));
-          if (has_lo) cin = fmaf(__half2float(*reinterpret_cast<const __half *>(lo_col + jj * 256)), 1.f / 2048.f, cin);
-          v[jj] = __float_as_uint(fmaf(t.beta, cin, t.alpha * __uint_as_float(v[jj])));
+        for (int p = 0; p < 4; ++p) {
+          const int pc = ((4 * t.h + p) ^ sw) * 16;
+          const uint4 hq = *reinterpret_cast<const uint4 *>(hi_col + pc);
+          uint4 lq = make_uint4(0u, 0u, 0u, 0u);
+          if (has_lo) lq = *reinterpret_cast<const uint4 *>(lo_col + pc);
+          const uint32_t hw[4] = {hq.x, hq.y, hq.z, hq.w}, lw[4] = {lq.x, lq.y, lq.z, lq.w};
+#pragma unroll
+          for (int e = 0; e < 4; ++e) {
+            const float2 hf = __half22float2(*reinterpret_cast<const __half2 *>(&hw[e]));
+            const float2 lf = __half22float2(*reinterpret_cast<const __half2 *>(&lw[e]));
+            const float c_a = fmaf(lf.x, 1.f / 2048.f, hf.x), c_b = fmaf(lf.y, 1.f / 2048.f, hf.y);
+            const int jj = 8 * p + 2 * e;
+            v[jj] = __float_as_uint(fmaf(t.beta, c_a, t.alpha * __uint_as_float(v[jj])));
+            v[jj + 1] = __float_as_uint(fmaf(t.beta, c_b, t.alpha * __uint_as_float(v[jj + 1])));
+          }
         }
       } else if (t.cin_direct) {
 #pragma unroll
         for (int jj = 0; jj < 32; ++jj)
           v[jj] = __float_as_uint(fmaf(t.beta, t.cpre[jj], t.alpha * __uint_as_float(v[jj])));
-        if (c0 + kChunkCols < c.nt) {
-          t.cinp += chunk_stride;
-          epi_prefetch32(args, t);
+        if (c0 + kChunkRows < c.nt) {
+          t.cinp += kChunkRows;
+          epi_prefetch32(t);
         }
       } else if (t.ident) {
-        // valid columns of this chunk inside the true n x n part (residual of the stop rule)
-        const int nvalid = (t.r < t.n) ? min(cnt, t.n - (c.n0 + c0)) : 0;
-        const int dj = t.r - (c.n0 + c0);     // chunk column that holds the diagonal element of row r
+        // valid rows of this chunk inside the true n x n part (residual of the stop rule)
+        const int nvalid = (t.col < t.n) ? min(cnt, t.n - (c.n0 + c0)) : 0;
+        const int dj = t.col - (c.n0 + c0);   // chunk row that holds the diagonal element of this column
 #pragma unroll
         for (int jj = 0; jj < 32; ++jj) {
           const float e = fmaf(-t.alpha, __uint_as_float(v[jj]), (jj == dj) ? 1.f : 0.f);
@@ -366,25 +382,35 @@ __device__ __forceinline__ float epi_chunks(const ChainArgs &args, const TileCmd
 #pragma unroll
         for (int jj = 0; jj < 32; ++jj) v[jj] = __float_as_uint(t.alpha * __uint_as_float(v[jj]));
       }
-      if (t.p32) {   // FP32 result (direct): one 128-byte segment per column and warp
-        float *qp = t.p32;
+      if (t.p32) {   // FP32 result (direct): 128 contiguous bytes of this thread's column
+        float4 *qp = reinterpret_cast<float4 *>(t.p32);
 #pragma unroll
-        for (int jj = 0; jj < 16; ++jj) { *qp = __uint_as_float(v[jj]); qp += args.ld; }
-        if (cnt == 32) {
-#pragma unroll
-          for (int jj = 16; jj < 32; ++jj) { *qp = __uint_as_float(v[jj]); qp += args.ld; }
-        }
-        t.p32 += chunk_stride;
+        for (int j4 = 0; j4 < 8; ++j4)
+          if (4 * j4 < cnt)
+            qp[j4] = make_float4(__uint_as_float(v[4 * j4]), __uint_as_float(v[4 * j4 + 1]),
+                                 __uint_as_float(v[4 * j4 + 2]), __uint_as_float(v[4 * j4 + 3]));
+        t.p32 += kChunkRows;
       }
     }
-    if (t.io.out_hi >= 0) {   // FP16 copies into the staging planes; columns beyond the tile are written as zero
+    if (t.io.out_hi >= 0) {   // FP16 copies into the staging planes; rows beyond the tile are written as zero
       const bool has_lo = t.io.out_lo >= 0;
 #pragma unroll
-      for (int jj = 0; jj < 32; ++jj) {
-        const float val = jj < cnt ? __uint_as_float(v[jj]) : 0.f;
-        const __half hi = __float2half_rn(val);
-        *reinterpret_cast<__half *>(hi_col + jj * 256) = hi;
-        if (has_lo) *reinterpret_cast<__half *>(lo_col + jj * 256) = __float2half_rn((val - __half2float(hi)) * 2048.f);
+      for (int p = 0; p < 4; ++p) {
+        uint32_t hw[4], lw[4];
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+          const int jj = 8 * p + 2 * e;
+          const float va = jj < cnt ? __uint_as_float(v[jj]) : 0.f;
+          const float vb = jj + 1 < cnt ? __uint_as_float(v[jj + 1]) : 0.f;
+          const __half2 h2 = __floats2half2_rn(va, vb);
+          hw[e] = *reinterpret_cast<const uint32_t *>(&h2);
+          const float2 hf = __half22float2(h2);
+          const __half2 l2 = __floats2half2_rn((va - hf.x) * 2048.f, (vb - hf.y) * 2048.f);
+          lw[e] = *reinterpret_cast<const uint32_t *>(&l2);
+        }
+        const int pc = ((4 * t.h + p) ^ sw) * 16;
+        *reinterpret_cast<uint4 *>(hi_col + pc) = make_uint4(hw[0], hw[1], hw[2], hw[3]);
+        if (has_lo) *reinterpret_cast<uint4 *>(lo_col + pc) = make_uint4(lw[0], lw[1], lw[2], lw[3]);
       }
       asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy smem writes -> TMA store
     }
