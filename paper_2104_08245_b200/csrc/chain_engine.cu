@@ -37,18 +37,19 @@
 //
 // Warp roles (384 threads): warp 0 = scheduler (leader CTA; claims the next tile, resolves its dependency and
 // writes the tile command into the ring of every CTA of the cluster), warp 1 = MMA issuer (leader CTA; whole warp,
-// one elected lane issues; + TMEM allocation), warp 2 = TMA producer of the operands, warps 3..10 = epilogue
-// compute (TMEM lane quadrant = warp_id % 4; the two warps of a quadrant take the two 32-column halves of the
-// 64-column chunks of the tile), warp 11 = epilogue agent (one thread: TMA loads of the FP16 add-in into the staging
-// buffers, TMA stores of the FP16 results out of them, publication of the tile; chain_epilogue.cuh).
+// one elected lane issues; + TMEM allocation), warp 2 = TMA producer of the operands, warp 3 = epilogue agent (one
+// thread: TMA loads of the FP16 add-in into the staging buffers, TMA stores of the FP16 results out of them,
+// publication of the tile; chain_epilogue.cuh), warps 4..11 = epilogue compute (TMEM lane quadrant = warp_id % 4;
+// the two warps of a quadrant take the two 32-row halves of the 64-row chunks of the tile).
 #include "common.cuh"
 #include "chain_epilogue.cuh"
 
 namespace {
 
-constexpr int kThreads = 384;
 constexpr int kEpiWarps = chainep::kComputeWarps;
-constexpr int kAgentWarp = 3 + kEpiWarps;   // warp 11
+constexpr int kAgentWarp = 3;
+constexpr int kFirstEpiWarp = 4;
+constexpr int kThreads = 32 * (kFirstEpiWarp + kEpiWarps);
 constexpr int kBK = 64;                  // K elements per pipeline stage (= one 128-byte swizzle row)
 constexpr int kMaxStages = 8;
 constexpr int kTmemCols = 512;
@@ -120,6 +121,32 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
         "}\n" ::"r"(smem_u32(bar)),
         "r"(parity)
         : "memory");
+}
+// one non-blocking probe of a barrier phase
+template <bool kPair>
+__device__ __forceinline__ bool mbar_test(uint64_t *bar, uint32_t parity) {
+  uint32_t ok;
+  if constexpr (kPair)
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "mbarrier.test_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t"
+        "}\n"
+        : "=r"(ok)
+        : "r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+  else
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t"
+        "}\n"
+        : "=r"(ok)
+        : "r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+  return ok != 0;
 }
 // TMA load into THIS CTA's shared memory; kPair: the bytes are counted on the LEADER's barrier
 template <bool kPair>
@@ -245,7 +272,8 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
     for (int r = 0; r < kRing; ++r) { mbar_init(&cmd_full[r], 1); mbar_init(&cmd_empty[r], 1 + kCtas * (1 + kEpiWarps + 1)); }
     mbar_init(&claim_go, 1);
     for (int b = 0; b < 2; ++b) { mbar_init(&ebars.in_full[b], 1); mbar_init(&ebars.out_ready[b], kEpiWarps); }
-    mbar_init(&ebars.tile_done, kEpiWarps + 1);   // compute warps + the agent (so that nobody can run a phase ahead of it)
+    mbar_init(&ebars.tile_done[0], kEpiWarps);
+    mbar_init(&ebars.tile_done[1], kEpiWarps);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == 1) {
@@ -432,11 +460,11 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
         if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
       }
     }
-  } else if (warp < kAgentWarp) {
+  } else if (warp >= kFirstEpiWarp) {
     // ===================== epilogue compute (every CTA drains its own 128 TMEM lanes) =====================
     const int q = warp & 3;          // TMEM lane quadrant this warp may access
-    const int h = (warp - 3) >> 2;   // column half of every 64-column chunk
-    int slot = 0, acc = 0;
+    const int h = (warp - kFirstEpiWarp) >> 2;   // row half of every 64-row chunk
+    int slot = 0, acc = 0, tile_par = 0;
     uint32_t ring_phase = 0, acc_phase = 0;
     uint32_t uses[2] = {0u, 0u};
     for (;;) {
@@ -465,30 +493,48 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
       }
       // this warp's direct stores and residual atomic are issued: join the tile's completion
       __syncwarp();
-      if (lane == 0) chainep::ebar_arrive(&ebars.tile_done);
+      if (lane == 0) chainep::ebar_arrive(&ebars.tile_done[tile_par]);
+      tile_par ^= 1;
     }
   } else {
     // ===================== epilogue agent (one thread) =====================
     if (lane == 0) {
       const CUtensorMap *emaps = args.maps + args.n_half;
       int slot = 0;
-      uint32_t ring_phase = 0, tile_phase = 0;
+      uint32_t ring_phase = 0, tile_seq = 0;
       uint32_t uses[2] = {0u, 0u};
-      for (;;) {
-        mbar_wait<kPair>(&cmd_full[slot], ring_phase);
-        const TileCmd c = cmds[slot];
+      // take the next command and open its tile (both staging buffers must be free)
+      auto take = [&](TileCmd &c) {
+        c = cmds[slot];
         mbar_arrive<kPair>(&cmd_empty[slot], 0);
         if (++slot == kRing) { slot = 0; ring_phase ^= 1u; }
-        if (c.op < 0) break;
+        if (c.op < 0) return;
         fence_proxy_async();   // other CTAs' writes (ordered by the scheduler's acquire) -> TMA reads of the add-in
         const int col0 = c.m0 + NOLSM_TILE_M * (int)rank;   // first column of this CTA's part of the tile
-        if (col0 < args.ld) chainep::epi_agent_tile(args, c, emaps, staging, ebars, col0, uses);
-        // the TMA stores of this tile are complete; wait until every compute warp has issued its direct stores
-        // and residual atomic, then publish
-        chainep::ebar_arrive(&ebars.tile_done);
-        chainep::ebar_wait(&ebars.tile_done, tile_phase);
-        tile_phase ^= 1u;
+        if (col0 < args.ld) chainep::epi_agent_open(args, c, emaps, staging, ebars, col0);
+      };
+      TileCmd c, cn;
+      mbar_wait<kPair>(&cmd_full[slot], ring_phase);
+      take(c);
+      while (c.op >= 0) {
+        const int col0 = c.m0 + NOLSM_TILE_M * (int)rank;
+        if (col0 < args.ld) chainep::epi_agent_run(args, c, emaps, staging, ebars, col0, uses);
+        // Both staging buffers are free again.  If the next tile's command is already there, open that tile
+        // BEFORE publishing this one: the publication (store completion, fences, atomics: ~3000 cycles) then
+        // overlaps the compute warps' work on the next tile instead of delaying it.  Never wait for the next
+        // command here: it may depend on this tile's publication.
+        const bool have_next = mbar_test<kPair>(&cmd_full[slot], ring_phase);
+        if (have_next) take(cn);
+        chainep::bulk_wait0();   // this tile's TMA stores are complete
+        // wait until every compute warp has issued its direct stores and residual atomic, then publish
+        chainep::ebar_wait(&ebars.tile_done[tile_seq & 1u], (tile_seq >> 1) & 1u);
+        ++tile_seq;
         chainep::epi_complete<kTileM, kColRound, kCtas>(args, c);
+        if (!have_next) {
+          mbar_wait<kPair>(&cmd_full[slot], ring_phase);
+          take(cn);
+        }
+        c = cn;
       }
     }
   }

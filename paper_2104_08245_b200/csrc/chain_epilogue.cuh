@@ -77,6 +77,16 @@ __device__ __forceinline__ void ld_tmem32(uint32_t taddr, uint32_t (&v)[32]) {
         "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
       : "r"(taddr));
 }
+__device__ __forceinline__ void ld_tmem16(uint32_t taddr, uint32_t (&v)[16]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
+      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+      : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+        "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+      : "r"(taddr));
+}
+__device__ __forceinline__ void ld_tmem_rows(uint32_t taddr, uint32_t (&v)[32]) { ld_tmem32(taddr, v); }
+__device__ __forceinline__ void ld_tmem_rows(uint32_t taddr, uint32_t (&v)[16]) { ld_tmem16(taddr, v); }
 __device__ __forceinline__ void ld_tmem_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void st_release_gpu_u64(unsigned long long *p, unsigned long long v) {
   asm volatile("st.release.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
@@ -149,8 +159,8 @@ __device__ __forceinline__ void epi_complete(const ChainArgs &args, const TileCm
 // epilogue LSU-issue-bound: measured.)  FP32 streams (one-shot products of the prepare stage) stay on the
 // direct path: 128 contiguous bytes per thread, 16-byte accesses.
 //
-// The eight compute warps (TMEM lane quadrant q = warp % 4 -> 32 columns of the tile, row half h) work through
-// the tile in chunks of 64 rows; two staging buffers of two planes (hi, lo); plane = [128 columns][64 rows] FP16
+// The eight compute warps (TMEM lane quadrant q = warp % 4 -> 32 columns of the tile, row half h = 32 rows)
+// work through the tile in chunks of 64 rows; two staging buffers of two planes (hi, lo); plane = [128 columns][64 rows] FP16
 // = 128 bytes per column, 16-byte pieces XOR-swizzled with (column % 8) like the TMA box.
 // Protocol per chunk and buffer:
 //   agent:    buffer free (its last store has been read) -> TMA loads of the add-in, or a plain arrive -> in_full
@@ -163,10 +173,14 @@ constexpr int kChunkRows = 64;
 constexpr int kPlaneBytes = 128 * kChunkRows * 2;  // one FP16 plane of a chunk
 constexpr int kStageBufBytes = 2 * kPlaneBytes;    // hi + lo
 constexpr int kStagingBytes = 2 * kStageBufBytes;  // two buffers
-constexpr int kComputeWarps = 8;
+constexpr int kComputeWarps = 8;                   // 4 lane quadrants x 2 row halves of a chunk (16 warps with 16 rows
+                                                   // each measured 9 % slower: more barrier traffic, narrower accesses)
+constexpr int kWarpRows = kChunkRows * 4 / kComputeWarps;   // rows of a chunk one warp drains: 32
 
 struct EpiBars {
-  uint64_t in_full[2], out_ready[2], tile_done;
+  uint64_t in_full[2], out_ready[2];
+  uint64_t tile_done[2];   // by tile parity: the agent opens at most one tile ahead of the one it publishes, so the
+                           // compute warps can never be two phases ahead of it on one barrier
 };
 
 __device__ __forceinline__ uint32_t s32(const void *p) { return static_cast<uint32_t>(__cvta_generic_to_shared(p)); }
@@ -227,24 +241,32 @@ __device__ __forceinline__ EpiIO epi_io(const ChainArgs &args, const TileCmd &c)
 // ---- the agent: one thread ----
 // emaps: the {64 rows x 128 columns} box maps of the FP16 buffers; stage: the two staging buffers; col0: first
 // column of this CTA's part of the tile; uses[b]: completed uses of buffer b (barrier phases).
-__device__ __forceinline__ void epi_agent_tile(const ChainArgs &args, const TileCmd &c, const CUtensorMap *emaps,
-                                               uint8_t *stage, EpiBars &bars, int col0, uint32_t (&uses)[2]) {
+__device__ __forceinline__ void epi_agent_avail(const TileCmd &c, const EpiIO &io, const CUtensorMap *emaps,
+                                                uint8_t *stage, EpiBars &bars, int col0, int j) {
+  const int b = j & 1;
+  uint8_t *buf = stage + b * kStageBufBytes;
+  const int row = c.n0 + kChunkRows * j;
+  if (io.in_hi >= 0) {
+    ebar_expect_tx(&bars.in_full[b], (uint32_t)kPlaneBytes * (io.in_lo >= 0 ? 2u : 1u));
+    tma_load_box(buf, &emaps[io.in_hi], &bars.in_full[b], row, col0, c.mat);
+    if (io.in_lo >= 0) tma_load_box(buf + kPlaneBytes, &emaps[io.in_lo], &bars.in_full[b], row, col0, c.mat);
+  } else {
+    ebar_arrive(&bars.in_full[b]);
+  }
+}
+// Opens a tile: both staging buffers are free; the first two chunks become available to the compute warps.
+__device__ __forceinline__ void epi_agent_open(const ChainArgs &args, const TileCmd &c, const CUtensorMap *emaps,
+                                               uint8_t *stage, EpiBars &bars, int col0) {
+  const EpiIO io = epi_io(args, c);
+  if (io.nchunks > 0) epi_agent_avail(c, io, emaps, stage, bars, col0, 0);
+  if (io.nchunks > 1) epi_agent_avail(c, io, emaps, stage, bars, col0, 1);
+}
+// Stores every chunk of an opened tile; on return all stores have READ their staging buffers (both are free),
+// but may not be complete yet (bulk_wait0).
+__device__ __forceinline__ void epi_agent_run(const ChainArgs &args, const TileCmd &c, const CUtensorMap *emaps,
+                                              uint8_t *stage, EpiBars &bars, int col0, uint32_t (&uses)[2]) {
   const EpiIO io = epi_io(args, c);
   const int nch = io.nchunks;
-  auto avail = [&](int j) {
-    const int b = j & 1;
-    uint8_t *buf = stage + b * kStageBufBytes;
-    const int row = c.n0 + kChunkRows * j;
-    if (io.in_hi >= 0) {
-      ebar_expect_tx(&bars.in_full[b], (uint32_t)kPlaneBytes * (io.in_lo >= 0 ? 2u : 1u));
-      tma_load_box(buf, &emaps[io.in_hi], &bars.in_full[b], row, col0, c.mat);
-      if (io.in_lo >= 0) tma_load_box(buf + kPlaneBytes, &emaps[io.in_lo], &bars.in_full[b], row, col0, c.mat);
-    } else {
-      ebar_arrive(&bars.in_full[b]);
-    }
-  };
-  if (nch > 0) avail(0);
-  if (nch > 1) avail(1);
   for (int j = 0; j < nch; ++j) {
     const int b = j & 1;
     ebar_wait(&bars.out_ready[b], uses[b] & 1u);
@@ -256,34 +278,34 @@ __device__ __forceinline__ void epi_agent_tile(const ChainArgs &args, const Tile
     bulk_commit();
     if (j + 2 < nch) {
       bulk_wait_read0();     // the store just issued has read the buffer: it may take the next add-in
-      avail(j + 2);
+      epi_agent_avail(c, io, emaps, stage, bars, col0, j + 2);
     }
   }
-  bulk_wait0();              // this tile's stores are complete (and both buffers free for the next tile)
+  bulk_wait_read0();
 }
 
 // ---- compute warp: cached per-tile parameters ----
 struct EpiTile {
   const ChainOp *o;
-  int par, n, col, h;         // col: this thread's column of the result; h: row half of every chunk
+  int par, n, col, h;         // col: this thread's column of the result; h: row quarter of every chunk
   bool split, ident, cin_direct;
   float alpha, beta;
-  float *p32;                 // FP32 output, element (first row of this warp's half, col) or null
+  float *p32;                 // FP32 output, element (first row of this warp's quarter, col) or null
   const float *cinp;          // FP32 master input (direct path), same position, or null
   EpiIO io;
-  float cpre[32];             // direct path only: add-in of the next chunk
+  float cpre[kWarpRows];      // direct path only: add-in of the next chunk
 };
 
 __device__ __forceinline__ void epi_prefetch32(EpiTile &t) {
   const float4 *pc = reinterpret_cast<const float4 *>(t.cinp);
 #pragma unroll
-  for (int j = 0; j < 8; ++j) {
+  for (int j = 0; j < kWarpRows / 4; ++j) {
     const float4 x = __ldcg(pc + j);
     t.cpre[4 * j] = x.x; t.cpre[4 * j + 1] = x.y; t.cpre[4 * j + 2] = x.z; t.cpre[4 * j + 3] = x.w;
   }
 }
 
-// Before waiting for the accumulator.  col: this thread's column of the result; h: row half of the chunks.
+// Before waiting for the accumulator.  col: this thread's column of the result; h: row quarter of the chunks.
 __device__ __forceinline__ void epi_begin(const ChainArgs &args, const TileCmd &c, int col, int h, EpiTile &t) {
   const ChainOp &o = args.prog.ops[c.op];
   t.o = &o;
@@ -302,50 +324,138 @@ __device__ __forceinline__ void epi_begin(const ChainArgs &args, const TileCmd &
     const float a = args.alpha_tab[c.mat * kAlphaSteps + cmd_iter(c)];
     if (t.ident) t.alpha *= a * a; else { t.alpha *= a; t.beta *= a; }
   }
-  const int64_t off = (int64_t)c.mat * args.slab + (int64_t)col * args.ld + c.n0 + 32 * h;
+  const int64_t off = (int64_t)c.mat * args.slab + (int64_t)col * args.ld + c.n0 + kWarpRows * h;
   t.p32 = o.cout32 >= 0 ? args.ubuf[o.cout32] + off : nullptr;
   t.cinp = t.cin_direct ? args.ubuf[o.cin32] + off : nullptr;
-  if (t.cin_direct && 32 * h < c.nt) epi_prefetch32(t);
+  if (t.cin_direct && kWarpRows * h < c.nt) epi_prefetch32(t);
 }
 
-// Drains this warp's 32 rows of every chunk of the accumulator at TMEM address t_main (lane quadrant and
+// ------------------------------------------------------------------------------------------------
+// Straight-line versions of epi_chunks for the two products that carry > 90 % of the work, the sign iteration in
+// FP16/FP32 mode (and the residual product of Eq. 15-17):
+//   kIdent = true :  E = I - alpha A B, FP16 result (hi only), ||E||_F^2            (EPI_IDENT, plain operands)
+//   kIdent = false:  X' = beta (hi + lo/2048) + alpha A B, result as hi + lo        (EPI_AXPBY, split master)
+// Same protocol and staging layout as epi_chunks; no per-element predicates or branches: ragged chunks, rows beyond
+// the true dimension and chunks that hold diagonal elements are detected per warp and take the general code.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ bool epi_fast_kind(const EpiTile &t, bool &ident) {
+  ident = t.ident;
+  if (t.split || t.p32 != nullptr || t.cin_direct || kWarpRows != 32) return false;
+  if (t.ident) return t.io.out_hi >= 0 && t.io.out_lo < 0;
+  return t.io.in_hi >= 0 && t.io.in_lo >= 0 && t.io.out_hi >= 0 && t.io.out_lo >= 0;
+}
+
+template <bool kIdent>
+__device__ __forceinline__ void epi_chunk_fast(const TileCmd &c, const EpiTile &t, uint32_t (&v)[32], uint8_t *hi_col,
+                                               uint8_t *lo_col, int sw, float beta_lo, float &ss) {
+  if constexpr (kIdent) {
+#pragma unroll
+    for (int p = 0; p < 4; ++p) {
+      uint32_t hw[4];
+#pragma unroll
+      for (int e = 0; e < 4; ++e) {
+        const int jj = 8 * p + 2 * e;
+        const float ea = -t.alpha * __uint_as_float(v[jj]), eb = -t.alpha * __uint_as_float(v[jj + 1]);
+        ss = fmaf(ea, ea, ss);
+        ss = fmaf(eb, eb, ss);
+        const __half2 h2 = __floats2half2_rn(ea, eb);
+        hw[e] = *reinterpret_cast<const uint32_t *>(&h2);
+      }
+      *reinterpret_cast<uint4 *>(hi_col + (((4 * t.h + p) ^ sw) * 16)) = make_uint4(hw[0], hw[1], hw[2], hw[3]);
+    }
+  } else {
+#pragma unroll
+    for (int p = 0; p < 4; ++p) {
+      const int pc = ((4 * t.h + p) ^ sw) * 16;
+      const uint4 hq = *reinterpret_cast<const uint4 *>(hi_col + pc);
+      const uint4 lq = *reinterpret_cast<const uint4 *>(lo_col + pc);
+      const uint32_t hin[4] = {hq.x, hq.y, hq.z, hq.w}, lin[4] = {lq.x, lq.y, lq.z, lq.w};
+      uint32_t hw[4], lw[4];
+#pragma unroll
+      for (int e = 0; e < 4; ++e) {
+        const int jj = 8 * p + 2 * e;
+        const float2 hf = __half22float2(*reinterpret_cast<const __half2 *>(&hin[e]));
+        const float2 lf = __half22float2(*reinterpret_cast<const __half2 *>(&lin[e]));
+        const float xa = fmaf(t.alpha, __uint_as_float(v[jj]), fmaf(beta_lo, lf.x, t.beta * hf.x));
+        const float xb = fmaf(t.alpha, __uint_as_float(v[jj + 1]), fmaf(beta_lo, lf.y, t.beta * hf.y));
+        const __half2 h2 = __floats2half2_rn(xa, xb);
+        const float2 hb = __half22float2(h2);
+        const __half2 l2 = __floats2half2_rn((xa - hb.x) * 2048.f, (xb - hb.y) * 2048.f);
+        hw[e] = *reinterpret_cast<const uint32_t *>(&h2);
+        lw[e] = *reinterpret_cast<const uint32_t *>(&l2);
+      }
+      *reinterpret_cast<uint4 *>(hi_col + pc) = make_uint4(hw[0], hw[1], hw[2], hw[3]);
+      *reinterpret_cast<uint4 *>(lo_col + pc) = make_uint4(lw[0], lw[1], lw[2], lw[3]);
+    }
+  }
+}
+
+
+// Drains this warp's 16 rows of every chunk of the accumulator at TMEM address t_main (lane quadrant and
 // accumulator stage already applied).  stage: the staging buffers; cl: this thread's column inside the CTA's part
-// of the tile (0..127); uses[b]: completed uses of buffer b.  Returns the warp's partial residual sum (lane-local;
-// reduce before use).
+// of the tile (0..127); uses[b]: completed uses of buffer b.  Tile heights are multiples of 16, so a warp's part
+// of a chunk is complete, half (16 rows) or empty.  Returns the warp's partial residual sum (lane-local; reduce before use).
 __device__ __forceinline__ float epi_chunks(const ChainArgs &args, const TileCmd &c, EpiTile &t, uint32_t t_main,
                                             int lane, int cl, uint8_t *stage, EpiBars &bars, uint32_t (&uses)[2]) {
+  constexpr int R = kWarpRows;
   float ss = 0.f;
   const int sw = cl & 7;                          // XOR swizzle of the 16-byte pieces of this column
   const int scol = cl * (2 * kChunkRows);         // byte offset of this column inside a staging plane
-  for (int ci = 0; ci < t.io.nchunks; ++ci) {
+  const float beta_lo = t.beta * (1.f / 2048.f);
+  bool fast_ident = false;
+  const bool fast_kind = epi_fast_kind(t, fast_ident);
+  uint32_t va[R], vb[R];
+  // plain products: the accumulator rows of chunk i + 1 are fetched from TMEM while chunk i is processed
+  if (!t.split && R * t.h < c.nt) ld_tmem_rows(t_main + R * t.h, va);
+  auto chunk = [&](const int ci, uint32_t (&v)[R], uint32_t (&vnext)[R]) {
     const int b = ci & 1;
-    const int c0 = ci * kChunkRows + 32 * t.h;    // first row (inside the tile) of this warp's part of the chunk
-    const int cnt = max(0, min(32, c.nt - c0));   // 0, 16 or 32 valid rows
-    uint32_t v[32];
-    if (cnt > 0) {
-      ld_tmem32(t_main + c0, v);
-      if (t.split) {
-        uint32_t w[32];
-        ld_tmem32(t_main + 128 + c0, w);
+    const int c0 = ci * kChunkRows + R * t.h;     // first row (inside the tile) of this warp's part of the chunk
+    const int cnt = max(0, min(R, c.nt - c0));    // valid rows: R, 16 or 0
+    const bool live = cnt > 0;
+    if (t.split) {
+      if (live) {
+        uint32_t w[R];
+        ld_tmem_rows(t_main + c0, v);
+        ld_tmem_rows(t_main + 128 + c0, w);
         ld_tmem_wait();
 #pragma unroll
-        for (int jj = 0; jj < 32; ++jj)
+        for (int jj = 0; jj < R; ++jj)
           v[jj] = __float_as_uint(fmaf(__uint_as_float(w[jj]), 1.f / 2048.f, __uint_as_float(v[jj])));
-      } else {
-        ld_tmem_wait();
       }
+    } else {
+      ld_tmem_wait();
+      if (c0 + kChunkRows < c.nt) ld_tmem_rows(t_main + c0 + kChunkRows, vnext);
     }
     // the staging buffer is free (its previous store has been read) and holds this chunk's add-in, if any
     ebar_wait(&bars.in_full[b], uses[b] & 1u);
     ++uses[b];
     uint8_t *hi_col = stage + b * kStageBufBytes + scol;
     uint8_t *lo_col = hi_col + kPlaneBytes;
-    if (cnt > 0) {
+    if constexpr (R == 32) {
+      // straight-line code for the products of the sign iteration (epi_chunk_fast) when the warp's part of the
+      // chunk is complete, inside the true dimension and (residual product) holds no diagonal element
+      bool fast = fast_kind && cnt == R;
+      if (fast && fast_ident) {
+        const int dj = t.col - (c.n0 + c0);
+        fast = c.n0 + c0 + R <= t.n && !__any_sync(0xffffffffu, dj >= 0 && dj < R);
+      }
+      if (fast) {
+        float s_local = 0.f;
+        if (fast_ident) epi_chunk_fast<true>(c, t, v, hi_col, lo_col, sw, beta_lo, s_local);
+        else epi_chunk_fast<false>(c, t, v, hi_col, lo_col, sw, beta_lo, s_local);
+        if (t.col < t.n) ss += s_local;
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncwarp();
+        if (lane == 0) ebar_arrive(&bars.out_ready[b]);
+        return;
+      }
+    }
+    if (live) {
       if (t.io.in_hi >= 0) {
         const bool has_lo = t.io.in_lo >= 0;
 #pragma unroll
-        for (int p = 0; p < 4; ++p) {
-          const int pc = ((4 * t.h + p) ^ sw) * 16;
+        for (int p = 0; p < R / 8; ++p) {
+          const int pc = (((R / 8) * t.h + p) ^ sw) * 16;
           const uint4 hq = *reinterpret_cast<const uint4 *>(hi_col + pc);
           uint4 lq = make_uint4(0u, 0u, 0u, 0u);
           if (has_lo) lq = *reinterpret_cast<const uint4 *>(lo_col + pc);
@@ -354,15 +464,15 @@ __device__ __forceinline__ float epi_chunks(const ChainArgs &args, const TileCmd
           for (int e = 0; e < 4; ++e) {
             const float2 hf = __half22float2(*reinterpret_cast<const __half2 *>(&hw[e]));
             const float2 lf = __half22float2(*reinterpret_cast<const __half2 *>(&lw[e]));
-            const float c_a = fmaf(lf.x, 1.f / 2048.f, hf.x), c_b = fmaf(lf.y, 1.f / 2048.f, hf.y);
             const int jj = 8 * p + 2 * e;
-            v[jj] = __float_as_uint(fmaf(t.beta, c_a, t.alpha * __uint_as_float(v[jj])));
-            v[jj + 1] = __float_as_uint(fmaf(t.beta, c_b, t.alpha * __uint_as_float(v[jj + 1])));
+            // beta (hi + lo / 2048) + alpha v
+            v[jj] = __float_as_uint(fmaf(t.alpha, __uint_as_float(v[jj]), fmaf(beta_lo, lf.x, t.beta * hf.x)));
+            v[jj + 1] = __float_as_uint(fmaf(t.alpha, __uint_as_float(v[jj + 1]), fmaf(beta_lo, lf.y, t.beta * hf.y)));
           }
         }
       } else if (t.cin_direct) {
 #pragma unroll
-        for (int jj = 0; jj < 32; ++jj)
+        for (int jj = 0; jj < R; ++jj)
           v[jj] = __float_as_uint(fmaf(t.beta, t.cpre[jj], t.alpha * __uint_as_float(v[jj])));
         if (c0 + kChunkRows < c.nt) {
           t.cinp += kChunkRows;
@@ -373,42 +483,46 @@ __device__ __forceinline__ float epi_chunks(const ChainArgs &args, const TileCmd
         const int nvalid = (t.col < t.n) ? min(cnt, t.n - (c.n0 + c0)) : 0;
         const int dj = t.col - (c.n0 + c0);   // chunk row that holds the diagonal element of this column
 #pragma unroll
-        for (int jj = 0; jj < 32; ++jj) {
+        for (int jj = 0; jj < R; ++jj) {
           const float e = fmaf(-t.alpha, __uint_as_float(v[jj]), (jj == dj) ? 1.f : 0.f);
           if (jj < nvalid) ss = fmaf(e, e, ss);
           v[jj] = __float_as_uint(e);
         }
       } else {
 #pragma unroll
-        for (int jj = 0; jj < 32; ++jj) v[jj] = __float_as_uint(t.alpha * __uint_as_float(v[jj]));
+        for (int jj = 0; jj < R; ++jj) v[jj] = __float_as_uint(t.alpha * __uint_as_float(v[jj]));
       }
-      if (t.p32) {   // FP32 result (direct): 128 contiguous bytes of this thread's column
+      if (t.p32) {   // FP32 result (direct): 64 contiguous bytes of this thread's column
         float4 *qp = reinterpret_cast<float4 *>(t.p32);
 #pragma unroll
-        for (int j4 = 0; j4 < 8; ++j4)
+        for (int j4 = 0; j4 < R / 4; ++j4)
           if (4 * j4 < cnt)
             qp[j4] = make_float4(__uint_as_float(v[4 * j4]), __uint_as_float(v[4 * j4 + 1]),
-                                 __uint_as_float(v[4 * j4 + 2]), __uint_as_float(v[4 * j4 + 3]));
+                               __uint_as_float(v[4 * j4 + 2]), __uint_as_float(v[4 * j4 + 3]));
         t.p32 += kChunkRows;
       }
     }
     if (t.io.out_hi >= 0) {   // FP16 copies into the staging planes; rows beyond the tile are written as zero
       const bool has_lo = t.io.out_lo >= 0;
+      if (cnt < R) {          // ragged last chunk (warp-uniform, rare)
 #pragma unroll
-      for (int p = 0; p < 4; ++p) {
+        for (int jj = 0; jj < R; ++jj)
+          if (jj >= cnt) v[jj] = 0u;
+      }
+#pragma unroll
+      for (int p = 0; p < R / 8; ++p) {
         uint32_t hw[4], lw[4];
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
           const int jj = 8 * p + 2 * e;
-          const float va = jj < cnt ? __uint_as_float(v[jj]) : 0.f;
-          const float vb = jj + 1 < cnt ? __uint_as_float(v[jj + 1]) : 0.f;
-          const __half2 h2 = __floats2half2_rn(va, vb);
+          const float va_ = __uint_as_float(v[jj]), vb_ = __uint_as_float(v[jj + 1]);
+          const __half2 h2 = __floats2half2_rn(va_, vb_);
           hw[e] = *reinterpret_cast<const uint32_t *>(&h2);
           const float2 hf = __half22float2(h2);
-          const __half2 l2 = __floats2half2_rn((va - hf.x) * 2048.f, (vb - hf.y) * 2048.f);
+          const __half2 l2 = __floats2half2_rn((va_ - hf.x) * 2048.f, (vb_ - hf.y) * 2048.f);
           lw[e] = *reinterpret_cast<const uint32_t *>(&l2);
         }
-        const int pc = ((4 * t.h + p) ^ sw) * 16;
+        const int pc = (((R / 8) * t.h + p) ^ sw) * 16;
         *reinterpret_cast<uint4 *>(hi_col + pc) = make_uint4(hw[0], hw[1], hw[2], hw[3]);
         if (has_lo) *reinterpret_cast<uint4 *>(lo_col + pc) = make_uint4(lw[0], lw[1], lw[2], lw[3]);
       }
@@ -416,6 +530,10 @@ __device__ __forceinline__ float epi_chunks(const ChainArgs &args, const TileCmd
     }
     __syncwarp();
     if (lane == 0) ebar_arrive(&bars.out_ready[b]);
+  };
+  for (int ci = 0; ci < t.io.nchunks; ci += 2) {
+    chunk(ci, va, vb);
+    if (ci + 1 < t.io.nchunks) chunk(ci + 1, vb, va);
   }
   return ss;
 }
