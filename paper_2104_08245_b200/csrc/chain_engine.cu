@@ -482,10 +482,13 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
       tc_fence_after();
       const uint32_t t_main = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(acc * 256);
       float ss = 0.f;
-      if (rows_in) ss = chainep::epi_chunks(args, c, t, t_main, lane, q * 32 + lane, staging, ebars, uses);
-      tc_fence_before();
-      __syncwarp();
-      if (lane == 0) mbar_arrive<kPair>(&tempty_bar[acc], 0);
+      auto release = [&]() {   // this warp has read its part of the accumulator stage
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive<kPair>(&tempty_bar[acc], 0);
+      };
+      if (rows_in) ss = chainep::epi_chunks(args, c, t, t_main, lane, q * 32 + lane, staging, ebars, uses, release);
+      else release();
       if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
       if (rows_in && t.o->resid) {
         for (int d = 16; d > 0; d >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, d);

@@ -395,8 +395,12 @@ __device__ __forceinline__ void epi_chunk_fast(const TileCmd &c, const EpiTile &
 // accumulator stage already applied).  stage: the staging buffers; cl: this thread's column inside the CTA's part
 // of the tile (0..127); uses[b]: completed uses of buffer b.  Tile heights are multiples of 16, so a warp's part
 // of a chunk is complete, half (16 rows) or empty.  Returns the warp's partial residual sum (lane-local; reduce before use).
+// release(): called once, as soon as this warp's last accumulator rows of the tile are in registers (the MMA issuer
+// may then reuse the accumulator stage while the last chunk is still being processed).
+template <typename Release>
 __device__ __forceinline__ float epi_chunks(const ChainArgs &args, const TileCmd &c, EpiTile &t, uint32_t t_main,
-                                            int lane, int cl, uint8_t *stage, EpiBars &bars, uint32_t (&uses)[2]) {
+                                            int lane, int cl, uint8_t *stage, EpiBars &bars, uint32_t (&uses)[2],
+                                            Release release) {
   constexpr int R = kWarpRows;
   float ss = 0.f;
   const int sw = cl & 7;                          // XOR swizzle of the 16-byte pieces of this column
@@ -426,6 +430,7 @@ __device__ __forceinline__ float epi_chunks(const ChainArgs &args, const TileCmd
       ld_tmem_wait();
       if (c0 + kChunkRows < c.nt) ld_tmem_rows(t_main + c0 + kChunkRows, vnext);
     }
+    if (ci == t.io.nchunks - 1) release();
     // the staging buffer is free (its previous store has been read) and holds this chunk's add-in, if any
     ebar_wait(&bars.in_full[b], uses[b] & 1u);
     ++uses[b];
