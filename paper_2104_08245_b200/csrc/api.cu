@@ -403,6 +403,8 @@ static nolsm_status build_submatrices_impl(nolsm_ctx *ctx, const nolsm_bsr *H, c
                               split_s, st));
   }
   b->s_split_built = split_s;
+  b->row_ptr = H->row_ptr;
+  b->col_idx = H->col_idx;
   *out = b;
   return NOLSM_OK;
 }
@@ -460,6 +462,8 @@ static nolsm_status run_chain(nolsm_ctx *ctx, nolsm_batch *b, const ChainProgram
   }
   return NOLSM_OK;
 }
+
+static nolsm_status join_sinv(nolsm_ctx *ctx, nolsm_batch *b, cudaStream_t st);
 
 static ChainProgram one_shot(int group) {
   ChainProgram pg;
@@ -580,12 +584,15 @@ static nolsm_status prepare_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, int prec
       if (z_split) { set2(o.a_lo, 5, 7); set2(o.b_lo, 5, 7); }
       si_hi = 2; si_lo = 3;
     }
-    o.use_div = 1; o.cout32 = 2; set2(o.out16, si_hi, si_hi); set2(o.out16_lo, si_lo, si_lo);
+    // with a refinement behind it S^-1 only continues as the split pair; its FP32 form is not needed
+    o.use_div = 1; o.cout32 = refine > 0 ? -1 : 2; set2(o.out16, si_hi, si_hi); set2(o.out16_lo, si_lo, si_lo);
     CHECK(run_chain(ctx, b, p1, b->d_scale, false, st));
   }
   // split S (refinements) and split H (B = S^-1 H) come from the builder, in the last four halves
   const int ss_hi = b->n_half - 4, ss_lo = b->n_half - 3, hs_hi = b->n_half - 2, hs_lo = b->n_half - 1;
-  int fr_hi = fp16 ? 2 : 0, fr_lo = fr_hi + 1;   // a pair of halves the iterations no longer need
+  // a pair of halves the iterations no longer need; FP16 mode: h3 (a Z buffer) and h5, which the sign iteration
+  // (h0, h1, h2, h4) leaves alone, so that the split S^-1 of ONE refinement survives it (join_sinv)
+  int fr_hi = fp16 ? 3 : 0, fr_lo = fp16 ? 5 : 1;
   if (refine > 0 && !b->s_split_built)           // batch built under another configuration
     LAUNCH(ctx, launch_scale_copy(b, S, nullptr, 0, nullptr, b->h[ss_hi], b->h[ss_lo], st));
   for (int it = 0; it < refine; ++it) {
@@ -598,7 +605,7 @@ static nolsm_status prepare_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, int prec
     set2(r.a, ss_hi, ss_hi); set2(r.a_lo, ss_lo, ss_lo); set2(r.b, si_hi, si_hi); set2(r.b_lo, si_lo, si_lo);
     set2(r.out16, 4, 4);
     ChainOp &c = p2.ops[1] = make_op(EPI_AXPBY, 1.f, 1.f);
-    set2(c.a, si_hi, si_hi); set2(c.b, 4, 4); c.cin32 = c.cout32 = 2;
+    set2(c.a, si_hi, si_hi); set2(c.b, 4, 4); set2(c.cin16, si_hi, si_hi); set2(c.cin16_lo, si_lo, si_lo);
     set2(c.out16, fr_hi, fr_hi); set2(c.out16_lo, fr_lo, fr_lo);
     CHECK(run_chain(ctx, b, p2, nullptr, false, st));
     std::swap(si_hi, fr_hi); std::swap(si_lo, fr_lo);
@@ -611,6 +618,19 @@ static nolsm_status prepare_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, int prec
     set2(o.a, si_hi, si_hi); set2(o.a_lo, si_lo, si_lo); set2(o.b, hs_hi, hs_hi); set2(o.b_lo, hs_lo, hs_lo);
     o.cout32 = 3;
     CHECK(run_chain(ctx, b, p4, nullptr, false, st));
+  }
+  // a5 reads the six own columns of S^-1 only: they are joined to FP32 here, the rest on demand (join_sinv)
+  b->sinv_hi = b->sinv_lo = -1;
+  b->sinv32_full = true;
+  if (refine > 0) {
+    b->sinv_hi = si_hi; b->sinv_lo = si_lo;
+    b->sinv32_full = false;
+    if (fp16 && si_hi == 3 && b->sparse && b->row_ptr) {
+      LAUNCH(ctx, launch_own_join(b, b->row_ptr, b->col_idx, b->h[si_hi], b->h[si_lo], b->u[2], st));
+    } else {   // the pair will be overwritten by the sign iteration: join all of it now
+      CHECK(join_sinv(ctx, b, st));
+      b->sinv_hi = b->sinv_lo = -1;
+    }
   }
   b->engine_simt = false;
   b->prepared = true;
@@ -844,6 +864,13 @@ static XRef x_ref(const nolsm_batch *b) {
   if (b->x_split && !b->engine_simt) return XRef{nullptr, b->h[0], b->h[1], b->h[2]};
   return XRef{x_ptr(b), nullptr, nullptr, nullptr};
 }
+// full FP32 S^-1 in u2 (the prepare stage leaves only its own columns there), for the consumers that read all of it
+static nolsm_status join_sinv(nolsm_ctx *ctx, nolsm_batch *b, cudaStream_t st) {
+  if (b->engine_simt || b->sinv32_full || b->sinv_hi < 0) return NOLSM_OK;
+  LAUNCH(ctx, launch_join_split(b, XRef{nullptr, b->h[b->sinv_hi], b->h[b->sinv_hi], b->h[b->sinv_lo]}, b->u[2], st));
+  b->sinv32_full = true;
+  return NOLSM_OK;
+}
 // FP32 copy of a split sign iterate in u0, for the consumers that read X as FP32
 static nolsm_status join_x(nolsm_ctx *ctx, nolsm_batch *b, cudaStream_t st) {
   if (!b->x_split || b->engine_simt || b->x32_valid) return NOLSM_OK;
@@ -995,6 +1022,7 @@ extern "C" nolsm_status nolsm_scatter_energy(nolsm_ctx *ctx, nolsm_batch *batch,
       batch->thin_cap = need;
     }
     CHECK(join_x(ctx, batch, st));
+    CHECK(join_sinv(ctx, batch, st));
     cudaError_t e = launch_energy_weighted(batch, x_ptr(batch), sinv_ptr(batch), batch->u[1], H->row_ptr, H->col_idx,
                                            batch->d_thin, W->val, st);
     ctx->launches += 4;
@@ -1349,6 +1377,7 @@ extern "C" nolsm_status nolsm_batch_read(nolsm_ctx *ctx, const nolsm_batch *b, i
                                          float *dst, int64_t dst_elems, int32_t *n_out, void *stream) {
   if (!ctx || !b || !dst || local < 0 || local >= b->count) return NOLSM_EINVAL;
   if (which == NOLSM_MAT_X && b->prepared) CHECK(join_x(ctx, const_cast<nolsm_batch *>(b), (cudaStream_t)stream));
+  if (which == NOLSM_MAT_SINV && b->prepared) CHECK(join_sinv(ctx, const_cast<nolsm_batch *>(b), (cudaStream_t)stream));
   const int n = b->n_host[local];
   if (n_out) *n_out = n;
   if (dst_elems < (int64_t)n * n) { ctx->err = "dst too small"; return NOLSM_ENOMEM; }

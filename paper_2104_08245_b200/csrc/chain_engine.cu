@@ -589,13 +589,15 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t
 // FP16 operand buffer: {64 storage rows, 64 storage columns} box with 128-byte swizzle, one map serving
 // both operand roles (see the header comment)
 nolsm_status encode_map(nolsm_ctx *ctx, CUtensorMap *map, void *ptr, int ld, int count, unsigned box_rows,
-                        unsigned box_cols, bool swizzle) {
+                        unsigned box_cols, bool swizzle, bool fp32) {
+  const size_t es = fp32 ? sizeof(float) : sizeof(__half);
   cuuint64_t dims[3] = {(cuuint64_t)ld, (cuuint64_t)ld, (cuuint64_t)count};
-  cuuint64_t strides[2] = {(cuuint64_t)ld * sizeof(__half), (cuuint64_t)ld * ld * sizeof(__half)};
+  cuuint64_t strides[2] = {(cuuint64_t)ld * es, (cuuint64_t)ld * ld * es};
   cuuint32_t box[3] = {box_rows, box_cols, 1};
   cuuint32_t estr[3] = {1, 1, 1};
   CUresult r = reinterpret_cast<EncodeTiledFn>(ctx->encode_tiled)(
-      map, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 3, ptr, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+      map, fp32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 3, ptr, dims, strides, box, estr,
+      CU_TENSOR_MAP_INTERLEAVE_NONE,
       swizzle ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
       CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) {
@@ -661,14 +663,20 @@ nolsm_status umma_make_maps(nolsm_ctx *ctx, nolsm_batch *b) {
   if (!ctx->umma_ok || b->count == 0) return NOLSM_OK;
   // [0, n_half): operand maps ({64 x 64} boxes, 128-byte swizzle); [n_half, 2 n_half): epilogue maps of the same
   // buffers ({64 rows x 128 columns} boxes, 128-byte swizzle: the staging planes of chain_epilogue.cuh)
-  std::vector<CUtensorMap> maps(2 * b->n_half);
+  std::vector<CUtensorMap> maps(2 * b->n_half + b->n_unit);
   for (int i = 0; i < b->n_half; ++i) {
-    nolsm_status s = encode_map(ctx, &maps[i], b->h[i], b->ld, b->count, 64, 64, true);
-    if (s == NOLSM_OK) s = encode_map(ctx, &maps[b->n_half + i], b->h[i], b->ld, b->count, chainep::kChunkRows, 128, true);
+    nolsm_status s = encode_map(ctx, &maps[i], b->h[i], b->ld, b->count, 64, 64, true, false);
+    if (s == NOLSM_OK)
+      s = encode_map(ctx, &maps[b->n_half + i], b->h[i], b->ld, b->count, chainep::kChunkRows, 128, true, false);
+    if (s != NOLSM_OK) return s;
+  }
+  // FP32 units: {32 rows x 128 columns} boxes for results that leave through the staging buffers
+  for (int i = 0; i < b->n_unit; ++i) {
+    nolsm_status s = encode_map(ctx, &maps[2 * b->n_half + i], b->u[i], b->ld, b->count, 32, 128, true, true);
     if (s != NOLSM_OK) return s;
   }
   if (!b->d_maps) {
-    if (cudaMalloc(&b->d_maps, sizeof(CUtensorMap) * 2 * NOLSM_MAX_HALF) != cudaSuccess) {
+    if (cudaMalloc(&b->d_maps, sizeof(CUtensorMap) * (2 * NOLSM_MAX_HALF + NOLSM_MAX_UNIT)) != cudaSuccess) {
       cudaGetLastError();
       ctx->err = "cudaMalloc of the tensor maps failed";
       return NOLSM_ENOMEM;

@@ -222,6 +222,8 @@ __device__ __forceinline__ void bulk_wait0() { asm volatile("cp.async.bulk.wait_
 // What a tile's op moves through the staging buffers (the same for the agent and the compute warps)
 struct EpiIO {
   int in_hi, in_lo, out_hi, out_lo;   // FP16 buffer indices, -1: none
+  int out32;                          // FP32 unit written THROUGH the staging buffer (an op without FP16 outputs:
+                                      // plane 0 / plane 1 hold rows 0..31 / 32..63 of the chunk as FP32), -1: none
   int nchunks;                        // chunks of 64 rows
 };
 __device__ __forceinline__ EpiIO epi_io(const ChainArgs &args, const TileCmd &c) {
@@ -234,6 +236,7 @@ __device__ __forceinline__ EpiIO epi_io(const ChainArgs &args, const TileCmd &c)
   io.in_lo = cin ? o.cin16_lo[par] : -1;
   io.out_hi = o.out16[par];
   io.out_lo = o.out16_lo[par];
+  io.out32 = (o.cout32 >= 0 && io.out_hi < 0) ? o.cout32 : -1;
   io.nchunks = (c.nt + kChunkRows - 1) / kChunkRows;
   return io;
 }
@@ -275,6 +278,10 @@ __device__ __forceinline__ void epi_agent_run(const ChainArgs &args, const TileC
     const int row = c.n0 + kChunkRows * j;
     if (io.out_hi >= 0) tma_store_box(buf, &emaps[io.out_hi], row, col0, c.mat);
     if (io.out_lo >= 0) tma_store_box(buf + kPlaneBytes, &emaps[io.out_lo], row, col0, c.mat);
+    if (io.out32 >= 0) {   // FP32 maps follow the FP16 ones: {32 rows x 128 columns} boxes
+      tma_store_box(buf, &emaps[args.n_half + io.out32], row, col0, c.mat);
+      tma_store_box(buf + kPlaneBytes, &emaps[args.n_half + io.out32], row + 32, col0, c.mat);
+    }
     bulk_commit();
     if (j + 2 < nch) {
       bulk_wait_read0();     // the store just issued has read the buffer: it may take the next add-in
@@ -325,7 +332,7 @@ __device__ __forceinline__ void epi_begin(const ChainArgs &args, const TileCmd &
     if (t.ident) t.alpha *= a * a; else { t.alpha *= a; t.beta *= a; }
   }
   const int64_t off = (int64_t)c.mat * args.slab + (int64_t)col * args.ld + c.n0 + kWarpRows * h;
-  t.p32 = o.cout32 >= 0 ? args.ubuf[o.cout32] + off : nullptr;
+  t.p32 = (o.cout32 >= 0 && t.io.out32 < 0) ? args.ubuf[o.cout32] + off : nullptr;
   t.cinp = t.cin_direct ? args.ubuf[o.cin32] + off : nullptr;
   if (t.cin_direct && kWarpRows * h < c.nt) epi_prefetch32(t);
 }
@@ -506,6 +513,18 @@ __device__ __forceinline__ float epi_chunks(const ChainArgs &args, const TileCmd
                                __uint_as_float(v[4 * j4 + 2]), __uint_as_float(v[4 * j4 + 3]));
         t.p32 += kChunkRows;
       }
+    }
+    if (t.io.out32 >= 0) {    // FP32 result into the plane of this warp's row half; rows beyond the tile as zero
+      if (cnt < R) {
+#pragma unroll
+        for (int jj = 0; jj < R; ++jj)
+          if (jj >= cnt) v[jj] = 0u;
+      }
+      uint8_t *pl = hi_col + t.h * kPlaneBytes;
+#pragma unroll
+      for (int p = 0; p < R / 4; ++p)
+        *reinterpret_cast<uint4 *>(pl + ((p ^ sw) * 16)) = make_uint4(v[4 * p], v[4 * p + 1], v[4 * p + 2], v[4 * p + 3]);
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     }
     if (t.io.out_hi >= 0) {   // FP16 copies into the staging planes; rows beyond the tile are written as zero
       const bool has_lo = t.io.out_lo >= 0;

@@ -87,6 +87,9 @@ struct nolsm_batch {
   bool x_pending = false;         // the sign chain stopped after E_k = I - X_k^2 passed the test: the update
                                   // X_{k+1} = X_k + 1/2 X_k E_k is folded into the density columns (reading 9)
   bool x_pending_split = false;   // E_k is stored as hi + lo (FP32 mode)
+  const int32_t *row_ptr = nullptr, *col_idx = nullptr;   // pattern the batch was built from (caller-owned, sparse batches)
+  int32_t sinv_hi = -1, sinv_lo = -1;   // >= 0: S^-1 lives as the split pair h[sinv_hi] + h[sinv_lo] * 2^-11 and u[2] holds
+  bool sinv32_full = true;              // only its own columns in FP32 until join_sinv (false)
   bool x_split = false;           // the sign iterate lives as hi (h[iters & 1]) + lo * 2^-11 (h[2]); u[0] holds X in
   bool x32_valid = false;         // FP32 only after join_x (reading 12)
   bool s_split_built = false;     // the builder wrote the split copy of S into h[n_half-4], h[n_half-3]
@@ -191,6 +194,9 @@ struct XRef {
   const __half *hi0, *hi1, *lo;   // hi0 != null: split
 };
 cudaError_t launch_join_split(const nolsm_batch *b, const XRef &x, float *dst32, cudaStream_t st);
+// own columns of a split matrix (hi + lo * 2^-11) as FP32 into the same columns of dst32
+cudaError_t launch_own_join(const nolsm_batch *b, const int32_t *row_ptr, const int32_t *col_idx, const __half *hi,
+                            const __half *lo, float *dst32, cudaStream_t st);
 cudaError_t launch_density(const nolsm_batch *b, const XRef &x, const float *sinv,
                            const int32_t *row_ptr, const int32_t *col_idx, float *d_val,
                            double *ne_diag, const __half *e_hi, const __half *e_lo, float *u_thin,

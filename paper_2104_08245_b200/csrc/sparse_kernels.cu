@@ -642,6 +642,34 @@ k_join_split(const int32_t *__restrict__ dims, const int32_t *__restrict__ iters
   *reinterpret_cast<float4 *>(dst + off) = make_float4(v[0], v[1], v[2], v[3]);
 }
 
+__global__ void __launch_bounds__(256)
+k_own_join(const int32_t *__restrict__ row_ptr, const int32_t *__restrict__ col_idx, int mol_begin, int ld, int64_t slab,
+           const __half *__restrict__ hi, const __half *__restrict__ lo, float *__restrict__ dst) {
+  const int mat = blockIdx.x;
+  const int j = mol_begin + mat;
+  const int lo_ = row_ptr[j];
+  const int m = row_ptr[j + 1] - lo_;
+  const int n = m * NOLSM_BS;
+  int l = 0, r_ = m;
+  while (l < r_) {
+    const int mid = (l + r_) >> 1;
+    if (col_idx[lo_ + mid] < j) l = mid + 1; else r_ = mid;
+  }
+  const int own0 = l * NOLSM_BS;
+  for (int t = threadIdx.x; t < NOLSM_BS * n; t += blockDim.x) {
+    const int p = t / n, k = t - p * n;
+    const int64_t off = (int64_t)mat * slab + (int64_t)(own0 + p) * ld + k;
+    dst[off] = fmaf(__half2float(lo[off]), 1.f / 2048.f, __half2float(hi[off]));
+  }
+}
+
+cudaError_t launch_own_join(const nolsm_batch *b, const int32_t *row_ptr, const int32_t *col_idx, const __half *hi,
+                            const __half *lo, float *dst32, cudaStream_t st) {
+  if (b->count == 0) return cudaSuccess;
+  k_own_join<<<b->count, 256, 0, st>>>(row_ptr, col_idx, b->mol_begin, b->ld, (int64_t)b->ld * b->ld, hi, lo, dst32);
+  return cudaGetLastError();
+}
+
 cudaError_t launch_join_split(const nolsm_batch *b, const XRef &x, float *dst32, cudaStream_t st) {
   if (b->count == 0) return cudaSuccess;
   const int P = (b->max_n + 3) & ~3;
