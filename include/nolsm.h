@@ -42,9 +42,14 @@ typedef enum {
   NOLSM_EINVAL = 1,   /* bad argument (null pointer, negative size, unsupported block size, ...) */
   NOLSM_ENOMEM = 2,   /* device or host allocation failed / workspace too small for one submatrix */
   NOLSM_ECUDA = 3,    /* a CUDA call failed (no device, launch error); see nolsm_last_error */
-  NOLSM_ENOTSPD = 4,  /* the inverse iteration (Eq. 15-17) did not converge: S_j not SPD / badly scaled */
-  NOLSM_ENOCONV = 5,  /* sign iteration hit max_iter on the FINAL mu for at least one submatrix */
-  NOLSM_EBRACKET = 6  /* N(mu_lo) > N_e or N(mu_hi) < N_e detected during the bisection */
+  NOLSM_ENOTSPD = 4,  /* Eq. 15-17 ended at inv_max_iter or on a NaN for at least one submatrix: S_j not SPD / badly
+                         scaled (PAPER.md:203-215 needs ||I - Y_0|| < 1).  Counted on the device: returned by
+                         nolsm_sign_batched and the whole-path calls with or without a stats struct */
+  NOLSM_ENOCONV = 5,  /* the sign iteration ended at max_iter or on a NaN for at least one submatrix (whole-path
+                         calls: on the FINAL mu; intermediate bisection steps may sit inside a band).  Counted on
+                         the device, independent of stats.  The outputs are written all the same */
+  NOLSM_EBRACKET = 6  /* nolsm_solve_mu with tol_ne_per_mol >= 0: the bisection ended outside the tolerance without
+                         ever moving one end of [mu_lo, mu_hi]: N(mu) - N_e kept one sign at every midpoint */
 } nolsm_status;
 
 typedef enum {
@@ -154,9 +159,12 @@ nolsm_status nolsm_build_neighbours(nolsm_ctx *ctx, int32_t n_mol, const int32_t
 /* a1: gather molecules [mol_begin, mol_begin+mol_count) into a context-owned batch
  * of dense submatrix pairs T_j(H), T_j(S): entry ((a,o),(b,p)) = block (N_j[a], N_j[b]) of the store if
  * that pair is stored, else 0.  H and S must share row_ptr/col_idx.  *out stays valid until the next
- * nolsm_build_submatrices on the same slot, nolsm_release_batch or nolsm_destroy.  `slot` selects one
- * of the context's batch slots (0 for streaming use).  Synchronises once (reads mol_count+1 row
- * pointers) to size the batch.  NOLSM_ENOMEM if the workspace cannot hold the batch. */
+ * nolsm_build_submatrices on the same slot, nolsm_release_batch or nolsm_destroy; no other entry point touches
+ * it (nolsm_solve_mu, nolsm_evaluate, nolsm_solve_mu_host, nolsm_sign_dense_batched and nolsm_gemm_batched work
+ * in context-private slots).  `slot` in [0, 4096) selects one of the caller's batch slots (0 for streaming use).
+ * The batch keeps H->row_ptr / H->col_idx (not the values): they must stay alive while the batch is used.
+ * Synchronises once (reads mol_count+1 row pointers) to size the batch.  NOLSM_ENOMEM if the caller's batches
+ * plus this one exceed workspace_bytes. */
 nolsm_status nolsm_build_submatrices(nolsm_ctx *ctx, const nolsm_bsr *H, const nolsm_bsr *S,
                                      int32_t mol_begin, int32_t mol_count, int32_t slot,
                                      nolsm_batch **out, void *stream);

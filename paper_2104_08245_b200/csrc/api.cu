@@ -152,6 +152,12 @@ static size_t dense_bytes(int count, int ld, int units) {
   return (size_t)units * 4 * (size_t)ld * ld * (size_t)count;
 }
 
+// Slots 0..kUserSlots-1 belong to the caller (nolsm_build_submatrices); the whole-path and test entries use
+// context-private slots from kOwnSlot on, so that they never invalidate a handle the caller holds.
+static const int kUserSlots = 4096;
+static const int kOwnSlot = kUserSlots;          // nolsm_solve_mu / nolsm_evaluate / nolsm_solve_mu_host: kOwnSlot + batch
+static const int kOwnDense = kUserSlots + 64;    // nolsm_sign_dense_batched, nolsm_gemm_batched
+
 static size_t allocated_bytes(const nolsm_ctx *ctx, int except_slot) {
   size_t t = 0;
   for (size_t i = 0; i < ctx->slots.size(); ++i)
@@ -170,7 +176,7 @@ static cudaError_t grow(T **ptr, size_t n) {
 // (small); the dense workspace is grow-only.
 static nolsm_status setup_batch(nolsm_ctx *ctx, int slot, const std::vector<int32_t> &dims, int mol_begin,
                                 bool sparse, int units, nolsm_batch **out, cudaStream_t st) {
-  if (slot < 0 || slot > 4096) { ctx->err = "bad slot"; return NOLSM_EINVAL; }
+  if (slot < 0 || slot > kOwnDense) { ctx->err = "bad slot"; return NOLSM_EINVAL; }
   if ((int)ctx->slots.size() <= slot) ctx->slots.resize(slot + 1, nullptr);
   if (!ctx->slots[slot]) ctx->slots[slot] = new nolsm_batch();
   nolsm_batch *b = ctx->slots[slot];
@@ -201,7 +207,7 @@ static nolsm_status setup_batch(nolsm_ctx *ctx, int slot, const std::vector<int3
     if (grow(&b->d_dims, cap) || grow(&b->d_state, cap) || grow(&b->d_iters, cap) ||
         grow(&b->d_resid2, cap * NOLSM_MAX_RESID_SLOTS) || grow(&b->d_lastres, cap) ||
         grow(&b->d_scale, cap) || grow(&b->d_norm, cap * 2) || grow(&b->d_alpha, cap * 8) || grow(&b->d_slot_state, cap) ||
-        grow(&b->d_slot_done, cap) || grow(&b->d_sched, (size_t)4) || grow(&b->d_tile_counter, (size_t)1) ||
+        grow(&b->d_slot_done, cap) || grow(&b->d_sched, (size_t)8) || grow(&b->d_tile_counter, (size_t)1) ||
         (b->d_active == nullptr && grow(&b->d_active, (size_t)NOLSM_MAX_RESID_SLOTS))) {
       cudaGetLastError();
       ctx->err = "cudaMalloc of batch metadata failed";
@@ -217,6 +223,7 @@ static nolsm_status setup_batch(nolsm_ctx *ctx, int slot, const std::vector<int3
       b->colpart_cap = need_cp;
     }
   }
+  NOLSM_CUDA(ctx, cudaMemsetAsync(b->d_sched, 0, 8 * sizeof(int32_t), st));
   b->count = count;
   b->ld = ld;
   b->max_n = max_n;
@@ -413,6 +420,7 @@ extern "C" nolsm_status nolsm_build_submatrices(nolsm_ctx *ctx, const nolsm_bsr 
                                                 int32_t mol_begin, int32_t mol_count, int32_t slot,
                                                 nolsm_batch **out, void *stream) {
   if (!ctx) return NOLSM_EINVAL;
+  if (slot < 0 || slot >= kUserSlots) { ctx->err = "slot must be in [0, 4096)"; return NOLSM_EINVAL; }
   return build_submatrices_impl(ctx, H, S, mol_begin, mol_count, slot, units_for(effective_precision(ctx, -1)), out,
                                 stream);
 }
@@ -544,6 +552,9 @@ static nolsm_status prepare_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, int prec
   }
   CHECK(run_chain(ctx, b, p0, nullptr, false, st));
   CHECK(run_chain(ctx, b, pg, nullptr, true, st));
+  // submatrices whose Eq. 15-17 iteration ended at the cap or on a NaN (S_j not SPD / badly scaled): kept beside
+  // the scheduler words, which the next launch resets
+  NOLSM_CUDA(ctx, cudaMemcpyAsync(b->d_sched + 4, b->d_sched + 2, sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
   int64_t inv_gemm_sum = 0;
   if (stats) {   // iterations and residuals of Eq. 15-17, before the sign iteration reuses the arrays
     std::vector<int32_t> it(b->count);
@@ -690,6 +701,7 @@ static nolsm_status sign_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, double mu, 
   if (timed) NOLSM_CUDA(ctx, cudaEventRecord(ctx->tev[0], st));
   CHECK(run_chain(ctx, b, pg, nullptr, true, st));
   if (timed) NOLSM_CUDA(ctx, cudaEventRecord(ctx->tev[1], st));
+  NOLSM_CUDA(ctx, cudaMemcpyAsync(b->d_sched + 5, b->d_sched + 2, sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
   return NOLSM_OK;
 }
 
@@ -942,6 +954,11 @@ extern "C" nolsm_status nolsm_sign_batched(nolsm_ctx *ctx, nolsm_batch *batch, d
     CHECK(prepare_batch(ctx, batch, prec, st, stats, &gemms));
   }
   CHECK(sign_batch(ctx, batch, mu, prec, tol, max_iter, fixed_iter, nullptr, st, stats != nullptr));
+  int32_t bad[2] = {0, 0};   // the status is a scalar that must reach the host: this call synchronises here
+  if (!batch->engine_simt) {
+    NOLSM_CUDA(ctx, cudaMemcpyAsync(bad, batch->d_sched + 4, sizeof(bad), cudaMemcpyDeviceToHost, st));
+    NOLSM_CUDA(ctx, cudaStreamSynchronize(st));
+  }
   if (stats) {
     const int inv_it = stats->inv_iter_max;
     const float inv_res = stats->inv_worst_residual;
@@ -953,6 +970,15 @@ extern "C" nolsm_status nolsm_sign_batched(nolsm_ctx *ctx, nolsm_batch *batch, d
     stats->gemms = gemms + 2 * stats->iter_sum;
     stats->ms_chain = chain_ms(ctx, batch);
     stats->chain_mcycles = chain_mcycles(ctx, batch, st);
+    if (!batch->engine_simt) stats->n_unconverged = bad[1];
+  }
+  if (bad[0] > 0) {
+    ctx->err = std::to_string(bad[0]) + " submatrices: Eq. 15-17 did not reach inv_tol within inv_max_iter (S_j not SPD?)";
+    return NOLSM_ENOTSPD;
+  }
+  if (bad[1] > 0 && fixed_iter <= 0) {
+    ctx->err = std::to_string(bad[1]) + " submatrices: the sign iteration hit max_iter";
+    return NOLSM_ENOCONV;
   }
   return NOLSM_OK;
 }
@@ -1091,10 +1117,28 @@ extern "C" nolsm_status nolsm_solve_mu(nolsm_ctx *ctx, const nolsm_bsr *H, const
     for (const Range &r : plan) total += r.bytes;
     resident = total <= ws && plan.size() <= 64;
   }
-  if (!resident) {
-    // streaming: one slot reused for every batch
-    for (size_t i = 1; i < ctx->slots.size(); ++i)
-      if (ctx->slots[i]) { free_batch(ctx->slots[i]); ctx->slots[i] = nullptr; }
+  // The context's own slots are re-planned on every call: release those the plan does not use and those whose
+  // workspace is far larger than the plan needs (a streaming call leaves one of the full workspace size behind),
+  // so that the accounting against workspace_bytes is about what this call holds.
+  {
+    size_t user = 0;
+    for (int i = 0; i < kUserSlots && i < (int)ctx->slots.size(); ++i)
+      if (ctx->slots[i]) user += ctx->slots[i]->base_bytes;
+    size_t total = 0;
+    for (const Range &r : plan) total += r.bytes;
+    resident = resident && total + user <= ws;
+    for (int i = kOwnSlot; i < kOwnDense && i < (int)ctx->slots.size(); ++i) {
+      nolsm_batch *ob = ctx->slots[i];
+      if (!ob) continue;
+      const int bi = i - kOwnSlot;
+      const bool used = resident ? bi < (int)plan.size() : bi == 0;
+      const size_t want = used ? (resident ? plan[bi].bytes : plan[0].bytes) : 0;
+      if (!used || ob->base_bytes > want + want / 2 + ((size_t)64 << 20)) {
+        cudaStreamSynchronize(st);
+        free_batch(ob);
+        ctx->slots[i] = nullptr;
+      }
+    }
   }
   std::vector<nolsm_batch *> live(plan.size(), nullptr);
 
@@ -1128,10 +1172,22 @@ extern "C" nolsm_status nolsm_solve_mu(nolsm_ctx *ctx, const nolsm_bsr *H, const
 
   cudaEvent_t tev[5];
   for (int i = 0; i < 5; ++i) cudaEventCreate(&tev[i]);
+  // per batch: submatrices whose inverse / sign iteration did not converge (read after the step's synchronise)
+  int32_t *h_flags = nullptr;
+  if (cudaMallocHost(&h_flags, sizeof(int32_t) * 2 * std::max<size_t>(plan.size(), 1)) != cudaSuccess) {
+    cudaGetLastError();
+    for (int i = 0; i < 5; ++i) cudaEventDestroy(tev[i]);
+    if (cache) cudaFree(cache);
+    ctx->err = "allocation of the convergence flags failed";
+    return NOLSM_ENOMEM;
+  }
   auto cleanup = [&]() {
     for (int i = 0; i < 5; ++i) cudaEventDestroy(tev[i]);
-    if (cache) { cudaStreamSynchronize(st); cudaFree(cache); }
+    cudaStreamSynchronize(st);
+    cudaFreeHost(h_flags);
+    if (cache) cudaFree(cache);
   };
+  int64_t inv_bad = 0, sign_bad = 0;
 
   double lo = mu_lo, hi = mu_hi, mu = 0.5 * (lo + hi), ne = 0.0;
   int step = 0;
@@ -1151,7 +1207,7 @@ extern "C" nolsm_status nolsm_solve_mu(nolsm_ctx *ctx, const nolsm_bsr *H, const
       if (cache && step > 0) {
         // operands of this batch from the cache: B -> u3, own columns of S^-1 -> u2
         std::vector<int32_t> bd(dims.begin() + r.begin, dims.begin() + r.begin + r.count);
-        rc = setup_batch(ctx, 0, bd, r.begin, true, units, &b, st);
+        rc = setup_batch(ctx, kOwnSlot, bd, r.begin, true, units, &b, st);
         if (rc != NOLSM_OK) break;
         const size_t slab_all = cache_sq[bi];
         ctx->launches += 2;
@@ -1167,7 +1223,7 @@ extern "C" nolsm_status nolsm_solve_mu(nolsm_ctx *ctx, const nolsm_bsr *H, const
         b->prepared_precision = prec;
       } else if (!b || !resident) {
         // the FP32 copy of T_j(H) is only read by the energy products (nolsm_evaluate) and the SIMT debug path
-        rc = build_submatrices_impl(ctx, H, S, r.begin, r.count, resident ? (int)bi : 0, units, &b, st,
+        rc = build_submatrices_impl(ctx, H, S, r.begin, r.count, kOwnSlot + (resident ? (int)bi : 0), units, &b, st,
                                     ctx->eval_energy || use_simt(ctx) || !ctx->umma_ok);
         if (rc != NOLSM_OK) break;
         live[bi] = resident ? b : nullptr;
@@ -1197,6 +1253,11 @@ extern "C" nolsm_status nolsm_solve_mu(nolsm_ctx *ctx, const nolsm_bsr *H, const
       if (timed) cudaEventRecord(tev[3], st);
       rc = nolsm_scatter_density(ctx, b, S, D, ctx->d_scalars, q_mol, ctx->d_scalars + 1, st);
       if (rc != NOLSM_OK) break;
+      h_flags[2 * bi] = h_flags[2 * bi + 1] = 0;
+      if (!b->engine_simt &&
+          cudaMemcpyAsync(h_flags + 2 * bi, b->d_sched + 4, 2 * sizeof(int32_t), cudaMemcpyDeviceToHost, st) != cudaSuccess) {
+        ctx->err = "solve_mu: copy of the convergence flags failed"; rc = NOLSM_ECUDA; break;
+      }
       if (ctx->eval_energy) {   // nolsm_evaluate: E = Tr(D H0) and the own columns of W = D H0 D
         rc = nolsm_scatter_energy(ctx, b, H, D, ctx->eval_w, ctx->d_scalars + 2, st);
         if (rc != NOLSM_OK) break;
@@ -1233,6 +1294,11 @@ extern "C" nolsm_status nolsm_solve_mu(nolsm_ctx *ctx, const nolsm_bsr *H, const
       break;
     }
     ne = ctx->h_scalars[0];
+    sign_bad = 0;
+    for (size_t bi = 0; bi < plan.size(); ++bi) {
+      if (step == 0) inv_bad += h_flags[2 * bi];
+      sign_bad += h_flags[2 * bi + 1];
+    }
     if (stats) {
       stats->last = acc;
       stats->ne_diag = ctx->h_scalars[1];
@@ -1240,7 +1306,16 @@ extern "C" nolsm_status nolsm_solve_mu(nolsm_ctx *ctx, const nolsm_bsr *H, const
       stats->flops_prepare_total += acc.flops_prepare;
       stats->mu_steps = step + 1;
     }
-    if (!(ne == ne)) { ctx->err = "N(mu) is NaN"; rc = NOLSM_ENOCONV; break; }
+    if (!(ne == ne)) {
+      if (inv_bad > 0) {
+        ctx->err = std::to_string(inv_bad) + " submatrices: Eq. 15-17 did not converge (S_j not SPD?); N(mu) is NaN";
+        rc = NOLSM_ENOTSPD;
+      } else {
+        ctx->err = "N(mu) is NaN";
+        rc = NOLSM_ENOCONV;
+      }
+      break;
+    }
     if (tol_ne_per_mol >= 0.0 && std::fabs(ne - n_electrons) <= tol_ne_per_mol * (double)n_mol) { step++; break; }
     if (step + 1 < max_steps) {
       if (ne > n_electrons) hi = mu; else lo = mu;
@@ -1255,10 +1330,21 @@ extern "C" nolsm_status nolsm_solve_mu(nolsm_ctx *ctx, const nolsm_bsr *H, const
     stats->cached = cache ? 1 : 0;
     stats->mu_lo = lo;
     stats->mu_hi = hi;
-    if (rc == NOLSM_OK && stats->last.n_unconverged > 0 && fixed_iter <= 0) {
-      ctx->err = "sign iteration hit max_iter on the final mu";
-      rc = NOLSM_ENOCONV;
-    }
+    stats->last.n_unconverged = (int32_t)std::min<int64_t>(sign_bad, 0x7fffffff);
+  }
+  // The verdict does not depend on `stats` (the kernels count what did not converge):
+  if (rc == NOLSM_OK && inv_bad > 0) {
+    ctx->err = std::to_string(inv_bad) + " submatrices: Eq. 15-17 did not reach inv_tol within inv_max_iter (S_j not SPD?)";
+    rc = NOLSM_ENOTSPD;
+  } else if (rc == NOLSM_OK && sign_bad > 0 && fixed_iter <= 0) {
+    ctx->err = std::to_string(sign_bad) + " submatrices: the sign iteration hit max_iter on the final mu";
+    rc = NOLSM_ENOCONV;
+  } else if (rc == NOLSM_OK && tol_ne_per_mol >= 0.0 && std::fabs(ne - n_electrons) > tol_ne_per_mol * (double)n_mol &&
+             (lo == mu_lo || hi == mu_hi)) {
+    // the bisection never moved one end of the bracket and did not meet the tolerance: N(mu) - N_e keeps one
+    // sign over [mu_lo, mu_hi] as far as the midpoints can tell
+    ctx->err = "no crossing of N(mu) = N_e found inside [mu_lo, mu_hi]";
+    rc = NOLSM_EBRACKET;
   }
   return rc;
 }
@@ -1356,7 +1442,7 @@ extern "C" nolsm_status nolsm_sign_dense_batched(nolsm_ctx *ctx, const float *a,
   if (batch == 0) return NOLSM_OK;
   std::vector<int32_t> dims(batch, n);
   nolsm_batch *b = nullptr;
-  CHECK(setup_batch(ctx, 0, dims, 0, false, units_dense(prec), &b, st));
+  CHECK(setup_batch(ctx, kOwnDense, dims, 0, false, units_dense(prec), &b, st));
   b->prepared = true;
   b->prepared_precision = prec;
   b->engine_simt = use_simt(ctx);
@@ -1406,7 +1492,7 @@ extern "C" nolsm_status nolsm_gemm_batched(nolsm_ctx *ctx, int32_t kind, int32_t
   cudaStream_t st = (cudaStream_t)stream;
   std::vector<int32_t> dims(batch, n);
   nolsm_batch *b = nullptr;
-  CHECK(setup_batch(ctx, 0, dims, 0, false, 7, &b, st));
+  CHECK(setup_batch(ctx, kOwnDense, dims, 0, false, 7, &b, st));
   // unit padding in A and B keeps the padded rows/columns decoupled, like the iterates of the path
   LAUNCH(ctx, launch_pack(a, n, batch, b->ld, b->u[0], 1, st));
   LAUNCH(ctx, launch_pack(bm, n, batch, b->ld, b->u[1], 1, st));

@@ -111,7 +111,7 @@ __device__ __forceinline__ void epi_complete(const ChainArgs &args, const TileCm
   if (o.resid) {
     const float r2 = *reinterpret_cast<volatile float *>(
         &args.resid2[(size_t)(k % NOLSM_MAX_RESID_SLOTS) * args.count + c.mat]);
-    const float res = sqrtf(fmaxf(r2, 0.f) / (float)n);
+    const float res = (r2 == r2) ? sqrtf(fmaxf(r2, 0.f) / (float)n) : r2;   // fmaxf would swallow a NaN
     args.lastres[c.mat] = res;
     const bool conv = res < pg.tol;   // false for a NaN residual
     bool stop = pg.fixed_iter > 0 ? (k + 1 >= pg.fixed_iter) : (conv || !(res == res));

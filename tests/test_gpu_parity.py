@@ -799,3 +799,77 @@ def test_gap_hint_scaled_start(nolsm, mid_system, mid_solution, precision):
         iters[hint] = st.last.iter_max
         ctx.close()
     assert iters[0.9 * gap] <= iters[0.0] - 2, iters
+
+
+# ---------------------------------------------------------------------------------------------
+# failure surface of the boundary (include/nolsm.h status codes): verdicts come from device counters, with or
+# without a stats struct
+# ---------------------------------------------------------------------------------------------
+def test_status_enoconv_without_stats(nolsm, tiny_system):
+    """A sign iteration capped at 2 iterations cannot pass the residual test: NOLSM_ENOCONV from
+    nolsm_sign_batched and from nolsm_solve_mu even when no stats struct is passed."""
+    H, S = _device_system(nolsm, tiny_system)
+    ctx = nolsm.Context(nolsm.Config(max_iter=2))
+    batch = ctx.build_submatrices(H, S, 0, 8)
+    with pytest.raises(nolsm.NolsmError) as ei:
+        ctx.sign_batched(batch, MU, want_stats=False)
+    assert ei.value.status == 5
+    with pytest.raises(nolsm.NolsmError) as ei:
+        ctx.solve_mu(H, S, tiny_system.n_electrons, 2 * MU, 0.0, tol_ne_per_mol=-1.0, max_steps=1, want_stats=False)
+    assert ei.value.status == 5
+    ctx.close()
+
+
+def test_status_enotspd(nolsm, tiny_system):
+    """An overlap matrix with a negative-definite diagonal block: Eq. 15-17 cannot converge (PAPER.md:203-215
+    needs an SPD T_j(S)); the batch that contains the molecule reports NOLSM_ENOTSPD."""
+    import torch
+    s_bad = tiny_system.s_val.copy()
+    k = int(tiny_system.row_ptr[3] + np.searchsorted(tiny_system.col_idx[tiny_system.row_ptr[3]:tiny_system.row_ptr[4]], 3))
+    s_bad[k] = -s_bad[k]
+    H = nolsm.BlockSparse.from_numpy(tiny_system.row_ptr, tiny_system.col_idx, tiny_system.h_val)
+    S = nolsm.BlockSparse(H.row_ptr, H.col_idx, torch.as_tensor(s_bad).contiguous().cuda())
+    ctx = nolsm.Context()
+    with pytest.raises(nolsm.NolsmError) as ei:
+        ctx.solve_mu(H, S, tiny_system.n_electrons, 2 * MU, 0.0, tol_ne_per_mol=-1.0, max_steps=1, want_stats=False)
+    assert ei.value.status == 4
+    batch = ctx.build_submatrices(H, S, 0, 8)
+    with pytest.raises(nolsm.NolsmError) as ei:
+        ctx.sign_batched(batch, MU, want_stats=False)
+    assert ei.value.status == 4
+    ctx.close()
+
+
+def test_status_ebracket(nolsm, tiny_system):
+    """A bracket below the whole spectrum holds no crossing of N(mu) = N_e: NOLSM_EBRACKET."""
+    H, S = _device_system(nolsm, tiny_system)
+    ctx = nolsm.Context()
+    with pytest.raises(nolsm.NolsmError) as ei:
+        ctx.solve_mu(H, S, tiny_system.n_electrons, -6.0, -4.0, tol_ne_per_mol=1e-3, max_steps=6)
+    assert ei.value.status == 6
+    ctx.close()
+
+
+def test_user_batch_survives_whole_path_calls(nolsm, tiny_system, tiny_solution):
+    """A handle from nolsm_build_submatrices stays valid across nolsm_solve_mu / nolsm_sign_dense_batched on the
+    same context (those use context-private slots), and a large-then-small sequence of solves does not run out
+    of workspace."""
+    import torch
+    import oracle.nolsm_oracle as orc
+    H, S = _device_system(nolsm, tiny_system)
+    ctx = nolsm.Context()
+    batch = ctx.build_submatrices(H, S, 4, 6)
+    ref = batch.read(2, nolsm.MAT_S).clone()
+    mu, ne, D, _ = ctx.solve_mu(H, S, tiny_system.n_electrons, -3.0, 0.0, tol_ne_per_mol=1e-3, max_steps=30)
+    a = torch.eye(32, dtype=torch.float32).cuda()[None] * 0.5
+    ctx.sign_dense_batched(a, None)
+    assert torch.equal(batch.read(2, nolsm.MAT_S), ref)
+    st = ctx.sign_batched(batch, MU)
+    assert st.n_unconverged == 0
+    D2 = S.like()
+    ne_t = torch.zeros(1, dtype=torch.float64, device="cuda")
+    ctx.scatter_density(batch, S, D2, ne_t, None, None)
+    d_ref = orc.density_blocks(tiny_solution["solutions"], tiny_system.row_ptr, MU)
+    lo, hi = tiny_system.row_ptr[4], tiny_system.row_ptr[10]
+    assert np.abs(D2.val.cpu().numpy()[lo:hi] - d_ref[lo:hi]).max() < TOL_D[0]
+    ctx.close()
