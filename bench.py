@@ -32,9 +32,10 @@ WORKLOADS = {          # name -> (precision, description)
     "w262144": (0, "configs[3]: 262144 molecules, 12 A, FP16/FP32, streamed"),
 }
 DATASHEET_FP16_TFLOPS = 2250.0
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE sign-iteration launch of k_chain, from the
-# `ncu --set full` capture named in profiles/ (None where no capture of that workload exists)
-NCU_TRAFFIC = {"w32768": 78.8e9}   # profiles/r1_k_chain_sign_w32768.md
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE sign-iteration launch of k_chain: an ncu CONSTANT from the
+# `ncu --set full` capture named here (bench.py cannot read DRAM counters itself); None where no capture exists
+NCU_TRAFFIC = {"w32768": None}
+NCU_TRAFFIC_SOURCE = "profiles/r2_k_chain_sign_w32768.md"
 METRIC = "molecules/s per NOLSM step (sign-iteration TFLOP/s in roofline.achieved)"
 
 
@@ -274,7 +275,7 @@ def run_native(args, system, rank, world, local_rank):
         t0 = time.perf_counter()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record()
-        reps = max(1, min(args.steps, 2))
+        reps = max(5, args.steps)
         for _ in range(reps):
             _, ne_h, _, h2d, d2h = ctx.solve_mu_host(hp[0], hp[1], hp[2], hp[3], d_host, system.n_electrons,
                                                      mu_lo, mu_hi, -1.0, 1)
@@ -283,7 +284,9 @@ def run_native(args, system, rank, world, local_rank):
         ms_e = max_over_ranks(max(e0.elapsed_time(e1), 1e3 * (time.perf_counter() - t0)) / reps, dev)
         e2e = {"value": job_value(world, system.n_mol, ms_e), "unit": "molecules/s", "h2d_bytes_per_step": h2d,
                "d2h_bytes_per_step": d2h, "ms_per_step": ms_e, "n_electrons": ne_h,
-               "note": "nolsm_solve_mu_host: pattern+H+S pinned host->device, D device->host, per step"}
+               "reps": reps,
+               "note": "nolsm_solve_mu_host: pattern+H+S pinned host->device, D device->host, per step; the pattern "
+                       "(a0) comes from the host here, the device-timed `value` rebuilds it from the positions"}
     if dist is not None:
         dist.destroy_process_group()
     if rank != 0:
@@ -311,6 +314,7 @@ def run_native(args, system, rank, world, local_rank):
                      "kernel": "k_chain, sign-iteration launches (all iterations of Eq. 9-10 for one batch per launch)",
                      "achieved": sign_tflops, "peak": peaks["tflops_sustained"], "unit": "TFLOP/s",
                      "frac": sign_tflops / peaks["tflops_sustained"], "traffic": NCU_TRAFFIC.get(args.workload),
+                     "traffic_source": "ncu constant, " + NCU_TRAFFIC_SOURCE,
                      "peak_source": peaks["source"] + " bf16_tflops_sustained (kernel timed inside a long step); "
                                     "FP32 mode issues 3 FP16 MMAs per product, so its bound is peak / 3"
                                     if precision == 1 else
@@ -321,6 +325,14 @@ def run_native(args, system, rank, world, local_rank):
                      "avg_launch_ms": ms_kernel / n_launch,
                      "achieved_padded": agg["flops_sign_padded"] / max(ms_kernel, 1e-9) * 1e-9,
                      "achieved_whole_sign_stage": agg["flops_sign"] / max(agg["ms_sign"], 1e-9) * 1e-9},
+        # the other tensor-bound stage: a2 + a3 (Eq. 15-17, S^-1 = Z^2, refinement, B = S^-1 H), CUDA-event time of
+        # the whole stage (its products, norm bounds and element-wise passes) per step
+        "roofline_prepare": {"bound": "tensor", "kernel": "k_chain, prepare launches (Eq. 15-17 chain, Z^2, refinement, B)",
+                             "achieved": agg["flops_prepare"] / max(agg["ms_prepare"], 1e-9) * 1e-9,
+                             "peak": peaks["tflops_sustained"], "unit": "TFLOP/s",
+                             "frac": agg["flops_prepare"] / max(agg["ms_prepare"], 1e-9) * 1e-9 / peaks["tflops_sustained"],
+                             "flops": "2 n^3 per product (a split-operand product counts once, but runs 3 FP16 MMAs)",
+                             "ms_per_step": agg["ms_prepare"] / args.steps, "traffic": None},
         "cpu_baseline": cpu,
         "detail": {"sign_tflops": sign_tflops, "ms_gather": agg["ms_gather"] / args.steps,
                    "ms_prepare": agg["ms_prepare"] / args.steps, "ms_sign": agg["ms_sign"] / args.steps,

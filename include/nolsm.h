@@ -34,6 +34,13 @@
 extern "C" {
 #endif
 
+/* exported symbols: the library is built with -fvisibility=hidden and exports only these entry points */
+#if defined(__GNUC__)
+#define NOLSM_API __attribute__((visibility("default")))
+#else
+#define NOLSM_API
+#endif
+
 typedef struct nolsm_ctx nolsm_ctx;     /* opaque: workspaces, tensor maps, statistics */
 typedef struct nolsm_batch nolsm_batch; /* opaque, owned by the context: one batch of dense submatrices */
 
@@ -141,10 +148,10 @@ typedef struct {            /* filled by nolsm_solve_mu (host struct) */
 } nolsm_solve_stats;
 
 /* Context.  `cfg` may be NULL (defaults).  Returns NOLSM_ECUDA when no device is usable. */
-nolsm_status nolsm_create(nolsm_ctx **ctx, const nolsm_config *cfg);
-void nolsm_destroy(nolsm_ctx *ctx);
-const char *nolsm_last_error(const nolsm_ctx *ctx); /* ctx may be NULL: last error of nolsm_create */
-int32_t nolsm_version(void);
+NOLSM_API nolsm_status nolsm_create(nolsm_ctx **ctx, const nolsm_config *cfg);
+NOLSM_API void nolsm_destroy(nolsm_ctx *ctx);
+NOLSM_API const char *nolsm_last_error(const nolsm_ctx *ctx); /* ctx may be NULL: last error of nolsm_create */
+NOLSM_API int32_t nolsm_version(void);
 
 /* a0: neighbour list of every molecule from integer positions.
  * pos_q [n_mol*3] int32 grid units in [0, box_q); box_q host int32[3], each even; rc_q cutoff in grid
@@ -152,7 +159,7 @@ int32_t nolsm_version(void);
  * in int64 (closed ball, self included).  Output CSR: row_ptr [n_mol+1], col_idx ascending per row.
  * Two passes inside; if the list needs more than `cap` entries nothing is written to col_idx and
  * NOLSM_ENOMEM is returned with *nnzb_out set to the needed size.  Synchronises (nnzb reaches the host). */
-nolsm_status nolsm_build_neighbours(nolsm_ctx *ctx, int32_t n_mol, const int32_t *pos_q,
+NOLSM_API nolsm_status nolsm_build_neighbours(nolsm_ctx *ctx, int32_t n_mol, const int32_t *pos_q,
                                     const int32_t *box_q /*host*/, int32_t rc_q, int32_t *row_ptr,
                                     int32_t *col_idx, int64_t cap, int64_t *nnzb_out /*host*/, void *stream);
 
@@ -165,7 +172,7 @@ nolsm_status nolsm_build_neighbours(nolsm_ctx *ctx, int32_t n_mol, const int32_t
  * The batch keeps H->row_ptr / H->col_idx (not the values): they must stay alive while the batch is used.
  * Synchronises once (reads mol_count+1 row pointers) to size the batch.  NOLSM_ENOMEM if the caller's batches
  * plus this one exceed workspace_bytes. */
-nolsm_status nolsm_build_submatrices(nolsm_ctx *ctx, const nolsm_bsr *H, const nolsm_bsr *S,
+NOLSM_API nolsm_status nolsm_build_submatrices(nolsm_ctx *ctx, const nolsm_bsr *H, const nolsm_bsr *S,
                                      int32_t mol_begin, int32_t mol_count, int32_t slot,
                                      nolsm_batch **out, void *stream);
 /* a1', SURVEY 8(f)#2 (Fig. 2 d-e: "the matrix elements of the submatrices are
@@ -203,19 +210,19 @@ typedef struct {
  * instead of reading H->val and S->val (the pattern arrays are still read; the traces of a6/a7 still
  * read the block stores).  NOLSM_EINVAL for a null pos_q, odd or non-positive box, orb_site out of
  * range, or n_mol different from the matrices' at build time. */
-nolsm_status nolsm_set_model(nolsm_ctx *ctx, const nolsm_model *model /*host*/);
+NOLSM_API nolsm_status nolsm_set_model(nolsm_ctx *ctx, const nolsm_model *model /*host*/);
 
 /* How many molecules starting at mol_begin fit in one batch given the workspace bound (host logic;
  * needs row_ptr on the device, synchronises).  Returns the count (>= 0) or -status. */
-int32_t nolsm_batch_capacity(nolsm_ctx *ctx, const nolsm_bsr *H, int32_t mol_begin, int32_t n_slots,
+NOLSM_API int32_t nolsm_batch_capacity(nolsm_ctx *ctx, const nolsm_bsr *H, int32_t mol_begin, int32_t n_slots,
                              void *stream);
-void nolsm_release_batch(nolsm_ctx *ctx, nolsm_batch *batch);
+NOLSM_API void nolsm_release_batch(nolsm_ctx *ctx, nolsm_batch *batch);
 
 /* a2-a4 (Eq. 15-17, Eq. 12, Eq. 9-10): for every submatrix of the batch, on the first call after the
  * gather: S_j^-1 and B_j = S_j^-1 H_j; on every call: X0 = (B_j - mu I)/s_j with 1.5 s_j >= rho(B_j - mu I)
  * and the sign iteration.  precision/tol/max_iter/fixed_iter < 0 or <= 0 take the context's values.
  * `stats` (host, may be NULL) makes the call synchronise at its end. */
-nolsm_status nolsm_sign_batched(nolsm_ctx *ctx, nolsm_batch *batch, double mu, int32_t precision,
+NOLSM_API nolsm_status nolsm_sign_batched(nolsm_ctx *ctx, nolsm_batch *batch, double mu, int32_t precision,
                                 float tol, int32_t max_iter, int32_t fixed_iter,
                                 nolsm_sign_stats *stats /*host*/, void *stream);
 
@@ -224,7 +231,7 @@ nolsm_status nolsm_sign_batched(nolsm_ctx *ctx, nolsm_batch *batch, double mu, i
  * *ne_partial (device double; FP32 products, FP64 accumulation).  q_mol (device double [n_mol], may be
  * NULL) receives each molecule's own population; ne_diag (device double, may be NULL) gets
  * sum_j sum_{c in own_j} (1 - X_cc) added.  Asynchronous. */
-nolsm_status nolsm_scatter_density(nolsm_ctx *ctx, const nolsm_batch *batch, const nolsm_bsr *S,
+NOLSM_API nolsm_status nolsm_scatter_density(nolsm_ctx *ctx, const nolsm_batch *batch, const nolsm_bsr *S,
                                    nolsm_bsr *D, double *ne_partial, double *q_mol, double *ne_diag,
                                    void *stream);
 
@@ -236,7 +243,7 @@ nolsm_status nolsm_scatter_density(nolsm_ctx *ctx, const nolsm_batch *batch, con
  * The sign iteration stops as nolsm_sign_batched does, but its finishing update X_{k+1} = X_k + 1/2 X_k E_k
  * is applied to the own columns of S_j^-1 only (X_{k+1} V = X_k (V + 1/2 E_k V)) instead of being formed;
  * the iteration counts in the statistics include it (reading 9). */
-nolsm_status nolsm_solve_mu(nolsm_ctx *ctx, const nolsm_bsr *H, const nolsm_bsr *S, double n_electrons,
+NOLSM_API nolsm_status nolsm_solve_mu(nolsm_ctx *ctx, const nolsm_bsr *H, const nolsm_bsr *S, double n_electrons,
                             double mu_lo, double mu_hi, double tol_ne_per_mol, int32_t max_steps,
                             int32_t precision, nolsm_bsr *D, double *mu_out /*host*/,
                             double *ne_out /*host*/, double *q_mol, nolsm_solve_stats *stats /*host*/,
@@ -248,13 +255,13 @@ nolsm_status nolsm_solve_mu(nolsm_ctx *ctx, const nolsm_bsr *H, const nolsm_bsr 
  *                     store W (pattern of H; four n x n x 6 products per submatrix, FP32);
  *   e_partial != NULL: sum_j sum_{i in N_j} sum_{o,p} D(i,j)[o,p] H0(j,i)[p,o] ADDED to *e_partial (device double;
  *                     D = the density store; FP32 products, FP64 accumulation).  Asynchronous. */
-nolsm_status nolsm_scatter_energy(nolsm_ctx *ctx, nolsm_batch *batch, const nolsm_bsr *H, const nolsm_bsr *D,
+NOLSM_API nolsm_status nolsm_scatter_energy(nolsm_ctx *ctx, nolsm_batch *batch, const nolsm_bsr *H, const nolsm_bsr *D,
                                   nolsm_bsr *W, double *e_partial, void *stream);
 
 /* One evaluation of the whole path (a1-a7) at a GIVEN mu, plus E_elec = Tr(D H0) (Eq. 7, 11) and, if W != NULL,
  * the energy-weighted density (Eq. 8, 13).  ne_out, e_out: host doubles (N(mu) = 2 tr(DS); E counts every
  * occupied orbital once, as Eq. 7 does).  q_mol: device double [n_mol] or NULL.  Synchronises. */
-nolsm_status nolsm_evaluate(nolsm_ctx *ctx, const nolsm_bsr *H, const nolsm_bsr *S, double mu, int32_t precision,
+NOLSM_API nolsm_status nolsm_evaluate(nolsm_ctx *ctx, const nolsm_bsr *H, const nolsm_bsr *S, double mu, int32_t precision,
                             nolsm_bsr *D, nolsm_bsr *W, double *ne_out /*host*/, double *e_out /*host*/,
                             double *q_mol, nolsm_solve_stats *stats /*host*/, void *stream);
 
@@ -264,7 +271,7 @@ nolsm_status nolsm_evaluate(nolsm_ctx *ctx, const nolsm_bsr *H, const nolsm_bsr 
  * owns device copies of the pattern and of H, S, D (grown on demand, reused across calls); every
  * call copies pattern + H + S host->device, runs nolsm_solve_mu, and copies D device->host.
  * *h2d_bytes / *d2h_bytes (host, may be NULL) receive the bytes moved.  Synchronises. */
-nolsm_status nolsm_solve_mu_host(nolsm_ctx *ctx, int32_t n_mol, const int32_t *row_ptr /*host*/,
+NOLSM_API nolsm_status nolsm_solve_mu_host(nolsm_ctx *ctx, int32_t n_mol, const int32_t *row_ptr /*host*/,
                                  const int32_t *col_idx /*host*/, const float *h_val /*host*/,
                                  const float *s_val /*host*/, double n_electrons, double mu_lo,
                                  double mu_hi, double tol_ne_per_mol, int32_t max_steps,
@@ -276,7 +283,7 @@ nolsm_status nolsm_solve_mu_host(nolsm_ctx *ctx, int32_t n_mol, const int32_t *r
  * sign(A_b) for `batch` dense n x n FP32 matrices stored one after another (row-major, leading
  * dimension n).  X0 = A_b / scale[b] (scale: device float [batch], e.g. ||A_b||_2; NULL: the
  * sqrt(||A||_1 ||A||_inf) bound is computed).  x_out: device float [batch*n*n], row-major sign(A_b). */
-nolsm_status nolsm_sign_dense_batched(nolsm_ctx *ctx, const float *a, const float *scale, int32_t n,
+NOLSM_API nolsm_status nolsm_sign_dense_batched(nolsm_ctx *ctx, const float *a, const float *scale, int32_t n,
                                       int32_t batch, int32_t precision, float tol, int32_t max_iter,
                                       int32_t fixed_iter, float *x_out, nolsm_sign_stats *stats /*host*/,
                                       void *stream);
@@ -289,22 +296,22 @@ nolsm_status nolsm_sign_dense_batched(nolsm_ctx *ctx, const float *a, const floa
 #define NOLSM_MAT_SINV 2  /* S_j^-1 (after nolsm_sign_batched) */
 #define NOLSM_MAT_B 3     /* B_j = S_j^-1 H_j */
 #define NOLSM_MAT_X 4     /* last sign iterate X_j */
-nolsm_status nolsm_batch_read(nolsm_ctx *ctx, const nolsm_batch *batch, int32_t local, int32_t which,
+NOLSM_API nolsm_status nolsm_batch_read(nolsm_ctx *ctx, const nolsm_batch *batch, int32_t local, int32_t which,
                               float *dst, int64_t dst_elems, int32_t *n_out /*host*/, void *stream);
-int32_t nolsm_batch_size(const nolsm_batch *batch);      /* submatrices in the batch */
-int32_t nolsm_batch_ld(const nolsm_batch *batch);        /* padded leading dimension */
+NOLSM_API int32_t nolsm_batch_size(const nolsm_batch *batch);      /* submatrices in the batch */
+NOLSM_API int32_t nolsm_batch_ld(const nolsm_batch *batch);        /* padded leading dimension */
 
 /* One batched product with the engine's own kernels (unit tests of the GEMM building block):
  * C_b = beta*Cin_b + alpha*A_b*B_b (ident = 0)  or  C_b = I - A_b*B_b (ident = 1), b < batch, all
  * n x n row-major FP32 on the device (n arbitrary).  kind: 0 = FP32 SIMT, 1 = tcgen05 FP16 operands,
  * 2 = tcgen05 split-FP16 (FP32-quality).  resid2 (device float[batch], may be NULL) receives
  * ||C_b||_F^2 when ident = 1. */
-nolsm_status nolsm_gemm_batched(nolsm_ctx *ctx, int32_t kind, int32_t ident, float alpha, float beta,
+NOLSM_API nolsm_status nolsm_gemm_batched(nolsm_ctx *ctx, int32_t kind, int32_t ident, float alpha, float beta,
                                 const float *a, const float *b, const float *cin, float *c,
                                 float *resid2, int32_t n, int32_t batch, void *stream);
 
 /* Kernel launches issued by this context so far (bench.py's gpu_launches). */
-int64_t nolsm_launch_count(const nolsm_ctx *ctx);
+NOLSM_API int64_t nolsm_launch_count(const nolsm_ctx *ctx);
 
 #ifdef __cplusplus
 }

@@ -6,6 +6,8 @@ nvcc cross-compiles without a GPU.  The library links cudart statically and reso
 entry point it needs (cuTensorMapEncodeTiled) at run time, so it loads on a machine without a GPU
 (the symbol-export test does exactly that).
 """
+import glob
+import hashlib
 import os
 import subprocess
 import sys
@@ -14,9 +16,10 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libnolsm.so")
 SOURCES = ["api.cu", "sparse_kernels.cu", "dense_kernels.cu", "chain_engine.cu"]
-HEADERS = [os.path.join(CSRC, "common.cuh"), os.path.join(HERE, "..", "include", "nolsm.h")]
+HEADERS = sorted(glob.glob(os.path.join(CSRC, "*.cuh"))) + [os.path.join(HERE, "..", "include", "nolsm.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-              "-Xcompiler", "-fPIC", "--use_fast_math=false"]
+              "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden"]
+STAMP = os.path.join(HERE, "libnolsm.flags")     # hash of the flags and source list the library was built with
 
 
 def _nvcc():
@@ -26,9 +29,16 @@ def _nvcc():
     raise RuntimeError("nvcc not found")
 
 
+def _flags_hash():
+    return hashlib.sha256(" ".join(NVCC_FLAGS + SOURCES).encode()).hexdigest()
+
+
 def needs_build():
-    if not os.path.exists(LIB):
+    if not os.path.exists(LIB) or not os.path.exists(STAMP):
         return True
+    with open(STAMP) as f:
+        if f.read().strip() != _flags_hash():
+            return True
     t = os.path.getmtime(LIB)
     deps = [os.path.join(CSRC, s) for s in SOURCES] + HEADERS
     return any(os.path.getmtime(d) > t for d in deps)
@@ -41,8 +51,8 @@ def build(force=False, verbose=False):
     procs = []
     for s in SOURCES:
         obj = os.path.join(CSRC, s.replace(".cu", ".o"))
-        cmd = [_nvcc()] + [f for f in NVCC_FLAGS if not f.startswith("--use_fast_math")] + \
-              (["-Xptxas", "-v"] if verbose else []) + ["-c", os.path.join(CSRC, s), "-o", obj]
+        cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
+              ["-c", os.path.join(CSRC, s), "-o", obj]
         procs.append((s, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
         objs.append(obj)
     failed = False
@@ -55,6 +65,8 @@ def build(force=False, verbose=False):
         raise RuntimeError("nvcc failed")
     cmd = [_nvcc(), "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB] + objs
     subprocess.run(cmd, check=True)
+    with open(STAMP, "w") as f:
+        f.write(_flags_hash() + "\n")
     return LIB
 
 
