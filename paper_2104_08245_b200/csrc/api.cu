@@ -535,20 +535,22 @@ static nolsm_status prepare_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, int prec
     }
   } else {
     // split operands: Y (h0,h1)/(h2,h3), Z (h4,h5)/(h6,h7), E (h8,h9)
-    LAUNCH(ctx, launch_init_inverse_first(b, S, b->d_norm, b->u[2], b->u[3], b->h[0], b->h[1], b->h[6], b->h[7],
+    // the iterates live as split pairs only (22 bits): the add-in of the correction form is the operand pair itself
+    LAUNCH(ctx, launch_init_inverse_first(b, S, b->d_norm, nullptr, nullptr, b->h[0], b->h[1], b->h[6], b->h[7],
                                           b->h[8], b->h[9], b->d_scale, st));
     set2(y1.a, 0, 0); set2(y1.a_lo, 1, 1); set2(y1.b, 8, 8); set2(y1.b_lo, 9, 9);
     set2(y1.out16, 2, 2); set2(y1.out16_lo, 3, 3);
+    y1.cin32 = y1.cout32 = -1; set2(y1.cin16, 0, 0); set2(y1.cin16_lo, 1, 1);
     pg.group = group_size(ctx, b, 28);
     ChainOp &e = pg.ops[0] = make_op(EPI_IDENT, 1.f, 0.f);
     set2(e.a, 6, 4); set2(e.a_lo, 7, 5); set2(e.b, 2, 0); set2(e.b_lo, 3, 1);
     set2(e.out16, 8, 8); set2(e.out16_lo, 9, 9); e.resid = 1;
     ChainOp &y = pg.ops[1] = make_op(EPI_AXPBY, 0.5f, 1.f);
     set2(y.a, 2, 0); set2(y.a_lo, 3, 1); set2(y.b, 8, 8); set2(y.b_lo, 9, 9);
-    y.cin32 = y.cout32 = 2; set2(y.out16, 0, 2); set2(y.out16_lo, 1, 3);
+    set2(y.cin16, 2, 0); set2(y.cin16_lo, 3, 1); set2(y.out16, 0, 2); set2(y.out16_lo, 1, 3);
     ChainOp &z = pg.ops[2] = make_op(EPI_AXPBY, 0.5f, 1.f);
     set2(z.a, 8, 8); set2(z.a_lo, 9, 9); set2(z.b, 6, 4); set2(z.b_lo, 7, 5);
-    z.cin32 = z.cout32 = 3; set2(z.out16, 4, 6); set2(z.out16_lo, 5, 7);
+    set2(z.cin16, 6, 4); set2(z.cin16_lo, 7, 5); set2(z.out16, 4, 6); set2(z.out16_lo, 5, 7);
   }
   CHECK(run_chain(ctx, b, p0, nullptr, false, st));
   CHECK(run_chain(ctx, b, pg, nullptr, true, st));
@@ -673,8 +675,8 @@ static nolsm_status sign_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, double mu, 
   ChainOp &e = pg.ops[0] = make_op(EPI_IDENT, 1.f, 0.f);
   ChainOp &x = pg.ops[1] = make_op(EPI_AXPBY, 0.5f, 1.f);
   e.resid = 1;
-  b->x_split = fp16;
-  b->x32_valid = !fp16;
+  b->x_split = true;
+  b->x32_valid = false;
   if (fp16) {
     // Master iterate as hi + lo * 2^-11 (22 bits, reading 12): hi IS the FP16 operand X16 (h0/h1,
     // ping-pong), lo lives in h2 and is updated in place by the thread that owns the element; E16: h4.
@@ -686,12 +688,13 @@ static nolsm_status sign_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, double mu, 
     set2(x.out16, 1, 0); set2(x.out16_lo, 2, 2); x.lo_stream = 1;
   } else {
     // split operands: X (h0,h1)/(h2,h3), E (h4,h5)
-    x.cin32 = x.cout32 = 0;
-    LAUNCH(ctx, launch_make_x0(b, Bm, (float)mu, b->d_norm, scale_in, X32, b->h[0], b->h[1], b->d_scale, st));
+    // the master iterate is the split operand pair itself (no FP32 copy): X (h0,h1) / (h2,h3) ping-pong
+    LAUNCH(ctx, launch_make_x0(b, Bm, (float)mu, b->d_norm, scale_in, nullptr, b->h[0], b->h[1], b->d_scale, st));
     pg.group = group_size(ctx, b, 12);
     set2(e.a, 0, 2); set2(e.a_lo, 1, 3); set2(e.b, 0, 2); set2(e.b_lo, 1, 3);
     set2(e.out16, 4, 4); set2(e.out16_lo, 5, 5);
     set2(x.a, 0, 2); set2(x.a_lo, 1, 3); set2(x.b, 4, 4); set2(x.b_lo, 5, 5);
+    set2(x.cin16, 0, 2); set2(x.cin16_lo, 1, 3);
     set2(x.out16, 2, 0); set2(x.out16_lo, 3, 1);
   }
   if (ctx->cfg.gap_hint > 0.f && !scale_in && pg.fixed_iter <= 0) {   // scaled start
@@ -873,13 +876,17 @@ static float *sinv_ptr(const nolsm_batch *b) { return b->engine_simt ? b->u[4] :
 static float *bmat_ptr(const nolsm_batch *b) { return b->engine_simt ? b->u[2] : b->u[3]; }
 static float *x_ptr(const nolsm_batch *b) { return (b->engine_simt && b->x_parity) ? b->u[3] : b->u[0]; }
 static XRef x_ref(const nolsm_batch *b) {
-  if (b->x_split && !b->engine_simt) return XRef{nullptr, b->h[0], b->h[1], b->h[2]};
-  return XRef{x_ptr(b), nullptr, nullptr, nullptr};
+  if (b->x_split && !b->engine_simt) {
+    if (b->prepared_precision == NOLSM_FP16_FP32) return XRef{nullptr, b->h[0], b->h[1], b->h[2], b->h[2]};
+    return XRef{nullptr, b->h[0], b->h[2], b->h[1], b->h[3]};
+  }
+  return XRef{x_ptr(b), nullptr, nullptr, nullptr, nullptr};
 }
 // full FP32 S^-1 in u2 (the prepare stage leaves only its own columns there), for the consumers that read all of it
 static nolsm_status join_sinv(nolsm_ctx *ctx, nolsm_batch *b, cudaStream_t st) {
   if (b->engine_simt || b->sinv32_full || b->sinv_hi < 0) return NOLSM_OK;
-  LAUNCH(ctx, launch_join_split(b, XRef{nullptr, b->h[b->sinv_hi], b->h[b->sinv_hi], b->h[b->sinv_lo]}, b->u[2], st));
+  LAUNCH(ctx, launch_join_split(b, XRef{nullptr, b->h[b->sinv_hi], b->h[b->sinv_hi], b->h[b->sinv_lo], b->h[b->sinv_lo]},
+                                b->u[2], st));
   b->sinv32_full = true;
   return NOLSM_OK;
 }

@@ -191,7 +191,7 @@ cudaError_t launch_own_columns(const nolsm_batch *b, const int32_t *row_ptr, con
 // the sign iterate as the kernels of a5 read it: FP32, or split hi (by the parity of iters) + lo
 struct XRef {
   const float *x32;
-  const __half *hi0, *hi1, *lo;   // hi0 != null: split
+  const __half *hi0, *hi1, *lo0, *lo1;   // hi0 != null: split pair (hi, lo) number (iters & 1)
 };
 cudaError_t launch_join_split(const nolsm_batch *b, const XRef &x, float *dst32, cudaStream_t st);
 // own columns of a split matrix (hi + lo * 2^-11) as FP32 into the same columns of dst32

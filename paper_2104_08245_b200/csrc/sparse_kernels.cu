@@ -526,7 +526,7 @@ k_density(const int32_t *__restrict__ row_ptr, const int32_t *__restrict__ col_i
   XMat<kSplit> xj;
   if constexpr (kSplit) {
     xj.hi = ((iters[mat] & 1) ? xr.hi1 : xr.hi0) + (int64_t)mat * slab;
-    xj.lo = xr.lo + (int64_t)mat * slab;
+    xj.lo = ((iters[mat] & 1) ? xr.lo1 : xr.lo0) + (int64_t)mat * slab;
   } else {
     xj.x32 = xr.x32 + (int64_t)mat * slab;
   }
@@ -635,7 +635,7 @@ k_join_split(const int32_t *__restrict__ dims, const int32_t *__restrict__ iters
   const int c = (int)(i / (P >> 2)), r = (int)(i % (P >> 2)) * 4;
   const int64_t off = (int64_t)mat * slab + (int64_t)c * ld + r;
   const __half *hi = ((iters[mat] & 1) ? xr.hi1 : xr.hi0) + off;
-  const __half *lo = xr.lo + off;
+  const __half *lo = ((iters[mat] & 1) ? xr.lo1 : xr.lo0) + off;
   float v[4];
 #pragma unroll
   for (int k = 0; k < 4; ++k) v[k] = fmaf(__half2float(lo[k]), 1.f / 2048.f, __half2float(hi[k]));
