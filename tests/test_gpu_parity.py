@@ -161,19 +161,23 @@ def test_gemm_building_block(nolsm, torch_mod, kind, tol, n, batch):
 # ---------------------------------------------------------------------------------------------
 # a2, a3: S^-1 and B = S^-1 H
 # ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("which", ["tiny", "mid"])
 @pytest.mark.parametrize("precision,tol", [(1, 2e-5), (0, 2e-4)])
-def test_inverse_and_operator(nolsm, tiny_system, precision, tol):
+def test_inverse_and_operator(nolsm, tiny_system, mid_system, precision, tol, which):
     """Eq. 15-17 converge to exactly S^-1: compare with LAPACK's inverse in FP64.
-    The FP16 mode refines S^-1 to FP32 quality (reading 11), hence the tight bound there too."""
+    The FP16 mode refines S^-1 to FP32 quality (reading 11), hence the tight bound there too.
+    tiny: n ~ 146 (two tiles a side); mid: n ~ 478 (four tiles a side, several 64-row chunks per tile)."""
     import oracle.nolsm_oracle as orc
-    system = tiny_system
+    system = tiny_system if which == "tiny" else mid_system
+    begin, count = (0, system.n_mol) if which == "tiny" else (90, 20)
     H, S = _device_system(nolsm, system)
     ctx = nolsm.Context(nolsm.Config(precision=precision))
-    batch = ctx.build_submatrices(H, S, 0, system.n_mol)
+    batch = ctx.build_submatrices(H, S, begin, count)
     stats = ctx.sign_batched(batch, MU)
     assert stats.inv_iter_max > 0
-    for local in (0, 7, 31):
-        nbrs = system.col_idx[system.row_ptr[local]:system.row_ptr[local + 1]]
+    for local in ((0, 7, 31) if which == "tiny" else (0, 11, 19)):
+        j = begin + local
+        nbrs = system.col_idx[system.row_ptr[j]:system.row_ptr[j + 1]]
         s_sub = orc.dense_submatrix(system.row_ptr, system.col_idx, system.s_val, nbrs)
         h_sub = orc.dense_submatrix(system.row_ptr, system.col_idx, system.h_val, nbrs)
         sinv = np.linalg.inv(s_sub)
@@ -565,12 +569,20 @@ def test_w32768_whole_step_in_bench_configuration_sampled(nolsm):
     assert 8 <= stats.last.iter_min and stats.last.iter_max <= 12
     d = D.val.cpu().numpy()
     qh = q.cpu().numpy()
-    for j in (0, 12345, 20000, 32767):           # first / last batch and two in between
+    # first / last batch and fourteen spread in between
+    for j in (0, 1, 700, 2047, 4096, 8191, 12345, 16384, 20000, 22222, 24576, 28000, 30000, 32000, 32766, 32767):
         sol = orc.solve_molecule(system.row_ptr, system.col_idx, system.h_val, system.s_val, j)
         ref = sol.density_columns(MU).reshape(-1, 6, 6)
         lo = system.row_ptr[j]
         assert np.abs(d[lo:lo + ref.shape[0]] - ref).max() < TOL_D[0], j
         assert abs(qh[j] - sol.population(MU)) < 5e-3
+    # a0 at this size: sixteen sampled rows of the device-built neighbour list, bit-exact against the oracle
+    pos = torch.as_tensor(system.pos_q).cuda()
+    rp, ci = ctx.build_neighbours(pos, system.box_q, system.rc_q, cap=system.nnzb)
+    rp_h, ci_h = rp.cpu().numpy(), ci.cpu().numpy()
+    assert np.array_equal(rp_h, system.row_ptr)
+    for j in range(5, n_mol, n_mol // 16):
+        assert np.array_equal(ci_h[rp_h[j]:rp_h[j + 1]], orc.neighbours_of(system.pos_q, system.box_q, system.rc_q, j))
     assert np.abs(qh - 8.0).max() < 0.03          # every molecule sits on the plateau (reading 14)
     assert abs(ne - qh.sum()) < 1e-6 * n_mol
     assert abs(ne - system.n_electrons) / n_mol < 1e-3
@@ -872,4 +884,33 @@ def test_user_batch_survives_whole_path_calls(nolsm, tiny_system, tiny_solution)
     d_ref = orc.density_blocks(tiny_solution["solutions"], tiny_system.row_ptr, MU)
     lo, hi = tiny_system.row_ptr[4], tiny_system.row_ptr[10]
     assert np.abs(D2.val.cpu().numpy()[lo:hi] - d_ref[lo:hi]).max() < TOL_D[0]
+    ctx.close()
+
+
+def test_config4_streaming_path_sampled(nolsm):
+    """BASELINE configs[3]'s submatrix size and streaming mode at a size the suite can afford: 32,768 molecules at
+    the 12 A cutoff (n ~ 1489, the CTA-pair engine, > 100 streamed batches through a 24 GiB workspace), one
+    N(mu) evaluation; eight sampled molecules against the oracle and the plateau property for all."""
+    import torch
+    import nolsm_inputs as gi
+    import oracle.nolsm_oracle as orc
+    n_mol = 32768
+    system = gi.make_water_system(n_mol, 12.0)
+    H, S = _device_system(nolsm, system)
+    ctx = nolsm.Context(nolsm.Config(precision=0, workspace_bytes=24 << 30))
+    q = torch.zeros(n_mol, dtype=torch.float64, device="cuda")
+    mu, ne, D, stats = ctx.solve_mu(H, S, system.n_electrons, 2 * MU, 0.0, tol_ne_per_mol=-1.0, max_steps=1, q_mol=q)
+    assert stats.n_batches > 100 and stats.last.n_unconverged == 0
+    d = D.val.cpu().numpy()
+    qh = q.cpu().numpy()
+    for j in (0, 300, 5000, 11111, 16384, 23456, 30000, 32767):
+        sol = orc.solve_molecule(system.row_ptr, system.col_idx, system.h_val, system.s_val, j)
+        assert sol.n > 1400
+        ref = sol.density_columns(MU).reshape(-1, 6, 6)
+        lo = system.row_ptr[j]
+        assert np.abs(d[lo:lo + ref.shape[0]] - ref).max() < TOL_D[0], j
+        assert abs(qh[j] - sol.population(MU)) < 5e-3
+    assert np.abs(qh - 8.0).max() < 0.03
+    assert abs(ne - system.n_electrons) / n_mol < 1e-3
+    assert np.isfinite(d).all()
     ctx.close()
