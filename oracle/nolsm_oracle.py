@@ -412,3 +412,100 @@ def sign_residual(x):
     x = np.asarray(x, dtype=np.float64)
     n = x.shape[0]
     return float(np.linalg.norm(x @ x - np.eye(n), "fro") / np.sqrt(n))
+
+
+# --------------------------------------------------------------------------------------------
+# submatrix combination heuristic (section III-B3, Eq. 14)
+# --------------------------------------------------------------------------------------------
+# The paper fixes the acceptance criterion (Eq. 14), the candidate filter ("the row entries of T_i itself are
+# used as a first filter") and the order of consideration ("iteratively in a sequence that depends
+# on ... n_{j\i} = n_j - n_{i^j}", "for each iteration n_{j\i} in {0, ..., n}"), and that it "automatically stops
+# when no more improvement of the target metric is found".  It does not fix how ties are broken or
+# how the parallel prioritisation is serialised; the reading taken here (reading 22) is the sequential
+# one below, in units of molecules (n = 6 x rows, so Eq. 14 is unchanged by the factor).
+def merge_gain(n_i, n_j, n_common):
+    """Eq. 14: merging pays iff (n_i + n_j - n_common)^3 < n_i^3 + n_j^3 (exact integers)."""
+    return (n_i + n_j - n_common) ** 3 < n_i ** 3 + n_j ** 3
+
+
+def combine_submatrices(row_ptr, col_idx):
+    """Iterative combination heuristic.  Cluster i starts as molecule i with the row set R_i = its neighbour
+    list.  Sweeps d = 0, 1, 2, ... over n_{j\\i} = |R_j \\ R_i|: in a sweep every live cluster i (ascending id) looks
+    at the live clusters j != i that own a molecule inside R_i (the filter), ascending id, and merges j into
+    itself (R_i <- R_i u R_j, owners joined, j dies) when |R_j \\ R_i| == d and Eq. 14 holds; R_i is updated at
+    once, so later candidates of the same sweep see the grown set.  After the sweep d = d_max (largest row set)
+    the sweeps restart at d = 0; the procedure stops after a full round of sweeps without a merge.
+    Returns a list of (owners sorted, rows sorted) per surviving cluster, ordered by the smallest owner."""
+    n = len(row_ptr) - 1
+    rows = [set(int(x) for x in col_idx[row_ptr[i]:row_ptr[i + 1]]) for i in range(n)]
+    owners = [[i] for i in range(n)]
+    owner_of = list(range(n))          # molecule -> cluster that owns it
+    alive = [True] * n
+    while True:
+        merged_any = False
+        d_max = max(len(rows[i]) for i in range(n) if alive[i])
+        for d in range(d_max + 1):
+            for i in range(n):
+                if not alive[i]:
+                    continue
+                cand = sorted({owner_of[m] for m in rows[i]} - {i})
+                for j in cand:
+                    if not alive[j] or j == i:
+                        continue
+                    common = len(rows[i] & rows[j])
+                    if len(rows[j]) - common != d:
+                        continue
+                    if not merge_gain(len(rows[i]), len(rows[j]), common):
+                        continue
+                    rows[i] |= rows[j]
+                    owners[i] += owners[j]
+                    for m in owners[j]:
+                        owner_of[m] = i
+                    alive[j] = False
+                    rows[j] = set()
+                    owners[j] = []
+                    merged_any = True
+        if not merged_any:
+            break
+    out = [(sorted(owners[i]), sorted(rows[i])) for i in range(n) if alive[i]]
+    out.sort(key=lambda t: t[0][0])
+    return out
+
+
+def cubic_work(groups):
+    """The target metric of the heuristic: sum over submatrices of n^3 (n in molecules)."""
+    return sum(len(r) ** 3 for _, r in groups)
+
+
+def solve_group(row_ptr, col_idx, h_val, s_val, owners, rows):
+    """One combined submatrix ("common submatrices for multiple similar columns"): T(H), T(S) over
+    the merged row set, eigen-decomposition, and for every owner j the own columns of T(D) restricted to the rows
+    of j's own neighbour list (the blocks D(i, j) the store holds).  Returns {j: SubmatrixView}."""
+    rows = np.asarray(rows, dtype=np.int64)
+    h_sub = dense_submatrix(row_ptr, col_idx, h_val, rows)
+    s_sub = dense_submatrix(row_ptr, col_idx, s_val, rows)
+    lam, v = generalized_eig(h_sub, s_sub)
+    return GroupSolution(owners, rows, h_sub, s_sub, lam, v, row_ptr, col_idx)
+
+
+class GroupSolution:
+    def __init__(self, owners, rows, h_sub, s_sub, lam, v, row_ptr, col_idx):
+        self.owners, self.rows = list(owners), rows
+        self.h_sub, self.s_sub, self.lam, self.v = h_sub, s_sub, lam, v
+        self.row_ptr, self.col_idx = row_ptr, col_idx
+
+    @property
+    def n(self):
+        return self.h_sub.shape[0]
+
+    def density_columns(self, j, mu):
+        """Blocks D(i, j), i in N_j (ascending, the order of the column-owned store): [6 |N_j|, 6]."""
+        occ = self.lam < mu
+        a = int(np.searchsorted(self.rows, j))
+        own = np.arange(a * BS, (a + 1) * BS)
+        cols = self.v[:, occ] @ self.v[own][:, occ].T                      # own columns of T(D): [n, 6]
+        nbrs = self.col_idx[self.row_ptr[j]:self.row_ptr[j + 1]]
+        pos = np.searchsorted(self.rows, nbrs)                              # N_j is a subset of the merged rows
+        assert np.array_equal(self.rows[pos], nbrs)
+        idx = (pos[:, None] * BS + np.arange(BS)[None, :]).reshape(-1)
+        return cols[idx]

@@ -558,3 +558,63 @@ def test_sign_residual_pins():
     for k in range(4):
         assert abs(orc.sign_residual(x_k) - hist[k]) < 1e-13
         x_k = orc.newton_schulz_sign(x_k, 1)
+
+
+# ------------------------------------------------------------------ combination heuristic (row f3, Eq. 14)
+def _csr(lists):
+    rp = np.zeros(len(lists) + 1, dtype=np.int32)
+    rp[1:] = np.cumsum([len(l) for l in lists])
+    return rp, np.concatenate([np.asarray(l, dtype=np.int32) for l in lists])
+
+
+def test_merge_criterion_eq14_hand_cases():
+    """Eq. 14 on numbers worked by hand: identical sets always merge (n^3 < 2 n^3); disjoint sets
+    never do ((a+b)^3 > a^3 + b^3); 10 and 10 rows with 8 common: 12^3 = 1728 < 2000 merges, with 7 common:
+    13^3 = 2197 > 2000 does not; the threshold for equal sizes is n_common > (2 - 2^(1/3)) n = 0.74 n."""
+    assert orc.merge_gain(5, 5, 5)
+    assert not orc.merge_gain(4, 9, 0)
+    assert orc.merge_gain(10, 10, 8) and not orc.merge_gain(10, 10, 7)
+    assert orc.merge_gain(100, 100, 75) and not orc.merge_gain(100, 100, 74)
+    # a small set inside a large one: 30^3 = 27000 < 27027 merges; one new row: 31^3 = 29791 > 27027 does not
+    assert orc.merge_gain(30, 3, 3) and not orc.merge_gain(30, 3, 2)
+
+
+def test_combination_heuristic_hand_built_examples():
+    """Hand-built systems (lists include self, symmetric):
+    (a) a clique of 4: every row set is {0,1,2,3}: everything merges into one cluster in the sweep d = 0;
+    (b) two cliques {0,1,2} and {3,4,5} without a link: two clusters, no cross merge (disjoint sets never pay);
+    (c) a chain 0-1-2-3-4 (each molecule sees its neighbours and itself): sets of size 2,3,3,3,2.  Sweep d = 0:
+        cluster 1 absorbs 0 ({0,1} inside {0,1,2}: (3+2-2)^3 = 27 < 35), cluster 3 absorbs 4; sweep d = 1: cluster 1
+        ({0,1,2}) looks at 2 ({1,2,3}): common 2, merged 4: 64 > 54, no; so three clusters remain: {0,1}, {2}, {3,4}."""
+    rp, ci = _csr([[0, 1, 2, 3]] * 4)
+    g = orc.combine_submatrices(rp, ci)
+    assert g == [([0, 1, 2, 3], [0, 1, 2, 3])]
+    rp, ci = _csr([[0, 1, 2]] * 3 + [[3, 4, 5]] * 3)
+    assert orc.combine_submatrices(rp, ci) == [([0, 1, 2], [0, 1, 2]), ([3, 4, 5], [3, 4, 5])]
+    rp, ci = _csr([[0, 1], [0, 1, 2], [1, 2, 3], [2, 3, 4], [3, 4]])
+    assert orc.combine_submatrices(rp, ci) == [([0, 1], [0, 1, 2]), ([2], [1, 2, 3]), ([3, 4], [2, 3, 4])]
+
+
+def test_combination_heuristic_invariants_on_water(tiny_system, tiny_solution):
+    """On the generated system: the clusters partition the molecules, every owner's neighbour list lies inside its
+    cluster's row set, the cubic work never exceeds the one-per-molecule value (each accepted merge lowers it by
+    Eq. 14), and D from a combined submatrix equals the one-per-molecule D when the merged row set is the whole
+    system (cutoff 9 A: every list is full, everything merges, the result is the full-matrix projector)."""
+    s = tiny_system
+    groups = orc.combine_submatrices(s.row_ptr, s.col_idx)
+    owners = sorted(m for o, _ in groups for m in o)
+    assert owners == list(range(s.n_mol))
+    for o, r in groups:
+        for j in o:
+            assert set(s.col_idx[s.row_ptr[j]:s.row_ptr[j + 1]]) <= set(r)
+    singles = [([j], list(s.col_idx[s.row_ptr[j]:s.row_ptr[j + 1]])) for j in range(s.n_mol)]
+    assert orc.cubic_work(groups) <= orc.cubic_work(singles)
+    assert len(groups) < s.n_mol                      # water-like lists overlap by ~ 0.8: merging pays
+    full = gi.make_water_system(32, 9.0)
+    g = orc.combine_submatrices(full.row_ptr, full.col_idx)
+    assert len(g) == 1 and g[0][0] == list(range(32))
+    sol = orc.solve_group(full.row_ptr, full.col_idx, full.h_val, full.s_val, *g[0])
+    ref = orc.solve_system(full, mu=-0.85)
+    for j in (0, 13, 31):
+        cols = ref["solutions"][j].density_columns(-0.85)
+        assert np.abs(sol.density_columns(j, -0.85) - cols).max() < 1e-12
