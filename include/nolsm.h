@@ -288,6 +288,42 @@ NOLSM_API nolsm_status nolsm_sign_dense_batched(nolsm_ctx *ctx, const float *a, 
                                       int32_t fixed_iter, float *x_out, nolsm_sign_stats *stats /*host*/,
                                       void *stream);
 
+/* --- submatrix combination heuristic (section III-B3, Eq. 14) ---
+ * nolsm_combine_submatrices: HOST integer work (the paper runs it on CPU cores, off the clock).
+ * Input: the neighbour lists (host CSR, ascending, self included) = the row sets of the one-per-molecule submatrices.
+ * Clusters are merged while (n_i + n_j - n_common)^3 < n_i^3 + n_j^3 (Eq. 14); candidates j are the clusters that own
+ * a row entry of T_i; they are taken in sweeps over n_{j\i} = |R_j \ R_i| = 0, 1, 2, ...; clusters and candidates in
+ * ascending order, T_i updated at once; the sweeps restart until a whole round merges nothing (reading 22).
+ * Output (host, caller-allocated): *n_groups_out groups ordered by their smallest owner; own_ptr[n_groups+1] /
+ * own_idx[n_mol] = the owners of every group, ascending; list_ptr[n_groups+1] / list_idx = the merged row sets,
+ * ascending.  own_ptr and list_ptr need room for n_mol + 1 entries.  If the row sets need more than list_cap
+ * entries nothing is written to list_idx and NOLSM_ENOMEM is returned with *list_len_out set to the needed size
+ * (it never exceeds the input's nnz).  NOLSM_EINVAL: lists not ascending / out of range, n_mol >= 2^20. */
+NOLSM_API nolsm_status nolsm_combine_submatrices(int32_t n_mol, const int32_t *row_ptr /*host*/,
+                                                 const int32_t *col_idx /*host*/, int32_t *n_groups_out /*host*/,
+                                                 int32_t *own_ptr /*host*/, int32_t *own_idx /*host*/,
+                                                 int32_t *list_ptr /*host*/, int32_t *list_idx /*host*/,
+                                                 int64_t list_cap, int64_t *list_len_out /*host*/);
+
+typedef struct {            /* the groups on the DEVICE (caller-owned, must outlive the batches built from them) */
+  int32_t n_groups;
+  const int32_t *own_ptr;   /* [n_groups+1] */
+  const int32_t *own_idx;   /* owners (molecules) of every group, ascending */
+  const int32_t *list_ptr;  /* [n_groups+1] */
+  const int32_t *list_idx;  /* merged row set (molecules) of every group, ascending; contains N_j of every owner j */
+} nolsm_groups;
+
+/* Like nolsm_build_submatrices for groups [grp_begin, grp_begin + grp_count): submatrix m of the batch is
+ * T(H), T(S) over the merged row set of group grp_begin + m ("common submatrices for multiple similar
+ * columns").  nolsm_sign_batched works on it unchanged; nolsm_scatter_density then writes, for every owner j of
+ * every group, the blocks D(i, j), i in N_j, from the columns of j inside the combined submatrix (rows of the merged
+ * set outside N_j are not stored: the result keeps the pattern of the input) and adds 2 tr(DS) of
+ * those owners to *ne_partial.  Gathers from the block stores only (NOLSM_EINVAL while a model is attached). */
+NOLSM_API nolsm_status nolsm_build_submatrices_grouped(nolsm_ctx *ctx, const nolsm_bsr *H, const nolsm_bsr *S,
+                                                       const nolsm_groups *groups /*host struct*/, int32_t grp_begin,
+                                                       int32_t grp_count, int32_t slot, nolsm_batch **out,
+                                                       void *stream);
+
 /* Inspection of a batch (tests, parity of the intermediate steps).  which: see NOLSM_MAT_*.
  * Copies submatrix `local` (0-based inside the batch) as a row-major n_j x n_j FP32 matrix into dst
  * (device, capacity dst_elems floats).  *n_out (host) = n_j.  Synchronises. */

@@ -19,7 +19,8 @@ EXPORTED_SYMBOLS = [
     "nolsm_build_submatrices", "nolsm_batch_capacity", "nolsm_release_batch", "nolsm_sign_batched",
     "nolsm_scatter_density", "nolsm_solve_mu", "nolsm_solve_mu_host", "nolsm_sign_dense_batched", "nolsm_batch_read",
     "nolsm_batch_size", "nolsm_batch_ld", "nolsm_gemm_batched", "nolsm_launch_count",
-    "nolsm_scatter_energy", "nolsm_evaluate", "nolsm_set_model",
+    "nolsm_scatter_energy", "nolsm_evaluate", "nolsm_set_model", "nolsm_combine_submatrices",
+    "nolsm_build_submatrices_grouped",
 ]
 
 
@@ -51,6 +52,11 @@ class _Model(C.Structure):
                 ("unit_per_grid", C.c_double), ("site_offset", (C.c_double * 3) * 3), ("orb_site", C.c_int32 * 6),
                 ("orb_energy", C.c_double * 6), ("s_ampl", C.c_double), ("h_ampl", C.c_double),
                 ("h_len", C.c_double), ("eval_fp32", C.c_int32)]
+
+
+class _Groups(C.Structure):
+    _fields_ = [("n_groups", C.c_int32), ("own_ptr", C.c_void_p), ("own_idx", C.c_void_p), ("list_ptr", C.c_void_p),
+                ("list_idx", C.c_void_p)]
 
 
 class SignStats(C.Structure):
@@ -140,6 +146,10 @@ def load_library():
     lib.nolsm_batch_ld.restype = i32
     lib.nolsm_gemm_batched.argtypes = [vp, i32, i32, f32, f32, vp, vp, vp, vp, vp, i32, i32, vp]
     lib.nolsm_gemm_batched.restype = i32
+    lib.nolsm_combine_submatrices.argtypes = [i32, vp, vp, P(i32), vp, vp, vp, vp, i64, P(i64)]
+    lib.nolsm_combine_submatrices.restype = i32
+    lib.nolsm_build_submatrices_grouped.argtypes = [vp, P(_Bsr), P(_Bsr), P(_Groups), i32, i32, i32, P(vp), vp]
+    lib.nolsm_build_submatrices_grouped.restype = i32
     _LIB = lib
     return lib
 
@@ -215,6 +225,43 @@ class Batch:
         self.ctx._check(self.ctx.lib.nolsm_batch_read(self.ctx.handle, self.handle, local, which, _ptr(buf),
                                                       buf.numel(), C.byref(n), _stream(stream)))
         return buf[: n.value * n.value].view(n.value, n.value)
+
+
+def combine_submatrices(row_ptr, col_idx):
+    """nolsm_combine_submatrices on host int32 numpy arrays (the heuristic is host work: no device, no context).
+    Returns (own_ptr, own_idx, list_ptr, list_idx) as numpy int32 arrays."""
+    import numpy as np
+    lib = load_library()
+    row_ptr = np.ascontiguousarray(row_ptr, dtype=np.int32)
+    col_idx = np.ascontiguousarray(col_idx, dtype=np.int32)
+    n = int(row_ptr.shape[0]) - 1
+    own_ptr = np.zeros(n + 1, dtype=np.int32)
+    own_idx = np.zeros(max(n, 1), dtype=np.int32)
+    list_ptr = np.zeros(n + 1, dtype=np.int32)
+    list_idx = np.zeros(max(int(col_idx.shape[0]), 1), dtype=np.int32)
+    ng, ll = C.c_int32(0), C.c_int64(0)
+    st = lib.nolsm_combine_submatrices(n, row_ptr.ctypes.data, col_idx.ctypes.data, C.byref(ng), own_ptr.ctypes.data,
+                                       own_idx.ctypes.data, list_ptr.ctypes.data, list_idx.ctypes.data,
+                                       int(list_idx.shape[0]), C.byref(ll))
+    if st != 0:
+        raise NolsmError(st, "nolsm_combine_submatrices")
+    g = ng.value
+    return own_ptr[:g + 1].copy(), own_idx[:n].copy(), list_ptr[:g + 1].copy(), list_idx[:ll.value].copy()
+
+
+class Groups:
+    """Device copy of the combined submatrices (nolsm_groups)."""
+
+    def __init__(self, own_ptr, own_idx, list_ptr, list_idx):
+        torch = _torch()
+        self.n_groups = int(len(own_ptr)) - 1
+        self.own_ptr, self.own_idx, self.list_ptr, self.list_idx = (
+            torch.as_tensor(x, dtype=torch.int32).contiguous().cuda() for x in (own_ptr, own_idx, list_ptr, list_idx))
+        self._ref = _Groups(self.n_groups, self.own_ptr.data_ptr(), self.own_idx.data_ptr(), self.list_ptr.data_ptr(),
+                            self.list_idx.data_ptr())
+
+    def ref(self):
+        return C.byref(self._ref)
 
 
 class Context:
@@ -302,6 +349,13 @@ class Context:
         h = C.c_void_p()
         self._check(self.lib.nolsm_build_submatrices(self.handle, H.ref(), S.ref(), mol_begin, mol_count, slot,
                                                      C.byref(h), _stream(stream)))
+        return Batch(self, h)
+
+    def build_submatrices_grouped(self, H, S, groups, grp_begin, grp_count, slot=0, stream=None):
+        """groups: a Groups object (device arrays of the combined submatrices)."""
+        h = C.c_void_p()
+        self._check(self.lib.nolsm_build_submatrices_grouped(self.handle, H.ref(), S.ref(), groups.ref(), grp_begin,
+                                                             grp_count, slot, C.byref(h), _stream(stream)))
         return Batch(self, h)
 
     def batch_capacity(self, H, mol_begin=0, n_slots=1, stream=None):

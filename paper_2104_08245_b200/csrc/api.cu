@@ -406,12 +406,64 @@ static nolsm_status build_submatrices_impl(nolsm_ctx *ctx, const nolsm_bsr *H, c
     LAUNCH(ctx, launch_generate(b, H->row_ptr, H->col_idx, &ctx->model, need_h32 ? b->u[1] : nullptr, b->u[0],
                                 split_s, st));
   } else {
-    LAUNCH(ctx, launch_gather(b, H->row_ptr, H->col_idx, H->val, S->val, need_h32 ? b->u[1] : nullptr, b->u[0],
-                              split_s, st));
+    LAUNCH(ctx, launch_gather(b, H->row_ptr, H->col_idx, nullptr, nullptr, H->val, S->val,
+                              need_h32 ? b->u[1] : nullptr, b->u[0], split_s, st));
   }
   b->s_split_built = split_s;
   b->row_ptr = H->row_ptr;
   b->col_idx = H->col_idx;
+  b->grouped = false;
+  *out = b;
+  return NOLSM_OK;
+}
+
+// a batch of COMBINED submatrices.  Group g's dense pair is T(H), T(S) over its
+// merged row set; everything downstream of the gather (Eq. 15-17, sign iteration) is the same batch machinery.
+extern "C" nolsm_status nolsm_build_submatrices_grouped(nolsm_ctx *ctx, const nolsm_bsr *H, const nolsm_bsr *S,
+                                                        const nolsm_groups *groups, int32_t grp_begin,
+                                                        int32_t grp_count, int32_t slot, nolsm_batch **out,
+                                                        void *stream) {
+  if (!ctx || !out || !groups) return NOLSM_EINVAL;
+  CHECK(check_bsr(ctx, H, "H"));
+  CHECK(check_bsr(ctx, S, "S"));
+  if (slot < 0 || slot >= kUserSlots) { ctx->err = "slot must be in [0, 4096)"; return NOLSM_EINVAL; }
+  if (H->n_mol != S->n_mol || H->row_ptr != S->row_ptr || H->col_idx != S->col_idx) {
+    ctx->err = "H and S must share one pattern (row_ptr, col_idx)";
+    return NOLSM_EINVAL;
+  }
+  if (!groups->own_ptr || !groups->own_idx || !groups->list_ptr || !groups->list_idx || grp_begin < 0 ||
+      grp_count < 0 || grp_begin + grp_count > groups->n_groups) {
+    ctx->err = "bad group arrays or group range";
+    return NOLSM_EINVAL;
+  }
+  if (ctx->has_model) { ctx->err = "combined submatrices are gathered from the block stores (detach the model)"; return NOLSM_EINVAL; }
+  cudaStream_t st = (cudaStream_t)stream;
+  std::vector<int32_t> lp(grp_count + 1), op(grp_count + 1), dims(grp_count);
+  if (grp_count > 0) {
+    NOLSM_CUDA(ctx, cudaMemcpyAsync(lp.data(), groups->list_ptr + grp_begin, sizeof(int32_t) * (grp_count + 1),
+                                    cudaMemcpyDeviceToHost, st));
+    NOLSM_CUDA(ctx, cudaMemcpyAsync(op.data(), groups->own_ptr + grp_begin, sizeof(int32_t) * (grp_count + 1),
+                                    cudaMemcpyDeviceToHost, st));
+    NOLSM_CUDA(ctx, cudaStreamSynchronize(st));
+  }
+  for (int i = 0; i < grp_count; ++i) {
+    dims[i] = (lp[i + 1] - lp[i]) * NOLSM_BS;
+    if (dims[i] <= 0 || op[i + 1] <= op[i]) { ctx->err = "group with an empty row set or without an owner"; return NOLSM_EINVAL; }
+  }
+  nolsm_batch *b = nullptr;
+  const int prec = effective_precision(ctx, -1);
+  CHECK(setup_batch(ctx, slot, dims, grp_begin, true, units_for(prec), &b, st));
+  const bool split_s = (ctx->cfg.inv_refine >= 0 ? ctx->cfg.inv_refine : (prec == NOLSM_FP16_FP32 ? 1 : 0)) > 0;
+  LAUNCH(ctx, launch_gather(b, H->row_ptr, H->col_idx, groups->list_ptr, groups->list_idx, H->val, S->val, b->u[1],
+                            b->u[0], split_s, st));
+  b->s_split_built = split_s;
+  b->row_ptr = H->row_ptr;
+  b->col_idx = H->col_idx;
+  b->grouped = true;
+  b->g_own_ptr = groups->own_ptr; b->g_own_idx = groups->own_idx;
+  b->g_list_ptr = groups->list_ptr; b->g_list_idx = groups->list_idx;
+  b->own_first = grp_count > 0 ? op[0] : 0;
+  b->own_count = grp_count > 0 ? op[grp_count] - op[0] : 0;
   *out = b;
   return NOLSM_OK;
 }
@@ -638,7 +690,9 @@ static nolsm_status prepare_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, int prec
   if (refine > 0) {
     b->sinv_hi = si_hi; b->sinv_lo = si_lo;
     b->sinv32_full = false;
-    if (fp16 && si_hi == 3 && b->sparse && b->row_ptr) {
+    if (fp16 && si_hi == 3 && b->sparse && b->grouped) {
+      LAUNCH(ctx, launch_own_join_grouped(b, b->h[si_hi], b->h[si_lo], b->u[2], st));
+    } else if (fp16 && si_hi == 3 && b->sparse && b->row_ptr) {
       LAUNCH(ctx, launch_own_join(b, b->row_ptr, b->col_idx, b->h[si_hi], b->h[si_lo], b->u[2], st));
     } else {   // the pair will be overwritten by the sign iteration: join all of it now
       CHECK(join_sinv(ctx, b, st));
@@ -1005,6 +1059,12 @@ extern "C" nolsm_status nolsm_scatter_density(nolsm_ctx *ctx, const nolsm_batch 
     return NOLSM_EINVAL;
   }
   cudaStream_t st = (cudaStream_t)stream;
+  if (batch->grouped) {   // combined submatrices: several owners per submatrix
+    if (batch->x_pending || batch->engine_simt) { ctx->err = "combined submatrices need the finished tensor-core iterate"; return NOLSM_EINVAL; }
+    LAUNCH(ctx, launch_density_grouped(batch, x_ref(batch), sinv_ptr(batch), S->row_ptr, S->col_idx, D->val, st));
+    LAUNCH(ctx, launch_trace(batch, S->row_ptr, S->col_idx, D->val, S->val, ne_partial, q_mol, st));
+    return NOLSM_OK;
+  }
   float *u_thin = nullptr;
   if (batch->x_pending) {
     nolsm_batch *bm = const_cast<nolsm_batch *>(batch);

@@ -88,6 +88,10 @@ struct nolsm_batch {
                                   // X_{k+1} = X_k + 1/2 X_k E_k is folded into the density columns (reading 9)
   bool x_pending_split = false;   // E_k is stored as hi + lo (FP32 mode)
   const int32_t *row_ptr = nullptr, *col_idx = nullptr;   // pattern the batch was built from (caller-owned, sparse batches)
+  // combined submatrices (nolsm_build_submatrices_grouped): submatrix m of the batch is group mol_begin + m
+  bool grouped = false;
+  const int32_t *g_own_ptr = nullptr, *g_own_idx = nullptr, *g_list_ptr = nullptr, *g_list_idx = nullptr;
+  int32_t own_first = 0, own_count = 0;   // the batch's owners: g_own_idx[own_first, own_first + own_count)
   int32_t sinv_hi = -1, sinv_lo = -1;   // >= 0: S^-1 lives as the split pair h[sinv_hi] + h[sinv_lo] * 2^-11 and u[2] holds
   bool sinv32_full = true;              // only its own columns in FP32 until join_sinv (false)
   bool x_split = false;           // the sign iterate lives as hi (h[iters & 1]) + lo * 2^-11 (h[2]); u[0] holds X in
@@ -182,8 +186,10 @@ cudaError_t launch_generate(const nolsm_batch *b, const int32_t *row_ptr, const 
                             const nolsm_model *model, float *h_out, float *s_out, bool split_s,
                             cudaStream_t st);
 cudaError_t launch_gather(const nolsm_batch *b, const int32_t *row_ptr, const int32_t *col_idx,
+                          const int32_t *list_ptr, const int32_t *list_idx,
                           const float *h_val, const float *s_val, float *h_out, float *s_out, bool split_s,
                           cudaStream_t st);
+
 // own columns of S^-1 (u2) to / from a packed [count][6][ld] array (operator cache of nolsm_solve_mu)
 cudaError_t launch_pack_square(const nolsm_batch *b, float *dense, float *packed, bool save, cudaStream_t st);
 cudaError_t launch_own_columns(const nolsm_batch *b, const int32_t *row_ptr, const int32_t *col_idx, float *mat,
@@ -194,6 +200,10 @@ struct XRef {
   const __half *hi0, *hi1, *lo0, *lo1;   // hi0 != null: split pair (hi, lo) number (iters & 1)
 };
 cudaError_t launch_join_split(const nolsm_batch *b, const XRef &x, float *dst32, cudaStream_t st);
+cudaError_t launch_own_join_grouped(const nolsm_batch *b, const __half *hi, const __half *lo, float *dst32,
+                                    cudaStream_t st);
+cudaError_t launch_density_grouped(const nolsm_batch *b, const XRef &x, const float *sinv, const int32_t *row_ptr,
+                                   const int32_t *col_idx, float *d_val, cudaStream_t st);
 // own columns of a split matrix (hi + lo * 2^-11) as FP32 into the same columns of dst32
 cudaError_t launch_own_join(const nolsm_batch *b, const int32_t *row_ptr, const int32_t *col_idx, const __half *hi,
                             const __half *lo, float *dst32, cudaStream_t st);

@@ -170,13 +170,16 @@ __device__ __forceinline__ void emit_rows2(const BuildOut &out, int64_t base, in
 
 __global__ void __launch_bounds__(GA_WARPS * 32)
 k_gather(const int32_t *__restrict__ row_ptr, const int32_t *__restrict__ col_idx,
+         const int32_t *__restrict__ list_ptr, const int32_t *__restrict__ list_idx,
          const float *__restrict__ h_val, const float *__restrict__ s_val, int mol_begin, int ld,
          int64_t slab, BuildOut out) {
+  // (list_ptr, list_idx): the row set of every submatrix -- the molecule's own neighbour list (= the store's
+  // pattern arrays) or the merged row set of a combined submatrix
   extern __shared__ int32_t s_pos[];  // [GA_WARPS][m_max]
   const int mat = blockIdx.y;
   const int j = mol_begin + mat;
-  const int lo = row_ptr[j];
-  const int m = row_ptr[j + 1] - lo;
+  const int lo = list_ptr[j];
+  const int m = list_ptr[j + 1] - lo;
   const int n = m * NOLSM_BS;
   const int P = (n + NOLSM_TILE_M - 1) / NOLSM_TILE_M * NOLSM_TILE_M;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -185,9 +188,9 @@ k_gather(const int32_t *__restrict__ row_ptr, const int32_t *__restrict__ col_id
   const int64_t base = (int64_t)mat * slab;
   for (int b = blockIdx.x * GA_WARPS + warp; b < m_pad_blocks; b += gridDim.x * GA_WARPS) {
     if (b < m) {
-      const int ib = col_idx[lo + b];
+      const int ib = list_idx[lo + b];
       for (int a = lane; a < m; a += 32) {
-        const int ia = col_idx[lo + a];
+        const int ia = list_idx[lo + a];
         int l = row_ptr[ia], r = row_ptr[ia + 1];
         const int end = r;
         while (l < r) {  // lower bound of ib in the sorted CSR row of ia
@@ -243,6 +246,7 @@ static BuildOut build_out(const nolsm_batch *b, float *h_out, float *s_out, bool
 }
 
 cudaError_t launch_gather(const nolsm_batch *b, const int32_t *row_ptr, const int32_t *col_idx,
+                          const int32_t *list_ptr, const int32_t *list_idx,
                           const float *h_val, const float *s_val, float *h_out, float *s_out, bool split_s,
                           cudaStream_t st) {
   if (b->count == 0) return cudaSuccess;
@@ -250,7 +254,8 @@ cudaError_t launch_gather(const nolsm_batch *b, const int32_t *row_ptr, const in
   const size_t smem = (size_t)GA_WARPS * per_warp * sizeof(int32_t);
   const int cols = (b->ld + NOLSM_BS - 1) / NOLSM_BS;
   dim3 grid((cols + GA_WARPS - 1) / GA_WARPS, b->count);
-  k_gather<<<grid, GA_WARPS * 32, smem, st>>>(row_ptr, col_idx, h_val, s_val, b->mol_begin, b->ld,
+  k_gather<<<grid, GA_WARPS * 32, smem, st>>>(row_ptr, col_idx, list_ptr ? list_ptr : row_ptr,
+                                              list_idx ? list_idx : col_idx, h_val, s_val, b->mol_begin, b->ld,
                                               (int64_t)b->ld * b->ld, build_out(b, h_out, s_out, split_s));
   return cudaGetLastError();
 }
@@ -705,6 +710,126 @@ cudaError_t launch_density(const nolsm_batch *b, const XRef &x, const float *sin
 }
 
 // ------------------------------------------------------------------------------------------------
+// Combined submatrices: one submatrix serves several molecules (its owners).
+// Group g has the merged row set U_g = list_idx[list_ptr[g] ..) and the owners own_idx[own_ptr[g] ..).
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ int lower_bound_i32(const int32_t *a, int n, int key) {
+  int l = 0, r = n;
+  while (l < r) {
+    const int mid = (l + r) >> 1;
+    if (a[mid] < key) l = mid + 1; else r = mid;
+  }
+  return l;
+}
+
+// own columns (all owners) of a split matrix to FP32
+__global__ void __launch_bounds__(256)
+k_own_join_grouped(const int32_t *__restrict__ own_ptr, const int32_t *__restrict__ own_idx,
+                   const int32_t *__restrict__ list_ptr, const int32_t *__restrict__ list_idx, int grp_begin, int ld,
+                   int64_t slab, const __half *__restrict__ hi, const __half *__restrict__ lo, float *__restrict__ dst) {
+  const int mat = blockIdx.x;
+  const int g = grp_begin + mat;
+  const int l0 = list_ptr[g];
+  const int m = list_ptr[g + 1] - l0;
+  const int n = m * NOLSM_BS;
+  for (int o = own_ptr[g]; o < own_ptr[g + 1]; ++o) {
+    const int own0 = lower_bound_i32(list_idx + l0, m, own_idx[o]) * NOLSM_BS;
+    for (int t = threadIdx.x; t < NOLSM_BS * n; t += blockDim.x) {
+      const int p = t / n, k = t - p * n;
+      const int64_t off = (int64_t)mat * slab + (int64_t)(own0 + p) * ld + k;
+      dst[off] = fmaf(__half2float(lo[off]), 1.f / 2048.f, __half2float(hi[off]));
+    }
+  }
+}
+
+cudaError_t launch_own_join_grouped(const nolsm_batch *b, const __half *hi, const __half *lo, float *dst32,
+                                    cudaStream_t st) {
+  if (b->count == 0) return cudaSuccess;
+  k_own_join_grouped<<<b->count, 256, 0, st>>>(b->g_own_ptr, b->g_own_idx, b->g_list_ptr, b->g_list_idx, b->mol_begin,
+                                               b->ld, (int64_t)b->ld * b->ld, hi, lo, dst32);
+  return cudaGetLastError();
+}
+
+// a5 + a6 for a combined submatrix: for every owner j the columns D[:, own_j] = 1/2 (I - X) S^-1[:, own_j]; the row
+// block of molecule i = U[r / 6] goes to block D(i, j) of the column-owned store if i is in N_j (position found in
+// the store's pattern), else it is not stored (the result keeps the input pattern).
+template <bool kSplit>
+__global__ void __launch_bounds__(DN_THREADS)
+k_density_grouped(const int32_t *__restrict__ row_ptr, const int32_t *__restrict__ col_idx,
+                  const int32_t *__restrict__ own_ptr, const int32_t *__restrict__ own_idx,
+                  const int32_t *__restrict__ list_ptr, const int32_t *__restrict__ list_idx, int grp_begin, int ld,
+                  int64_t slab, const XRef xr, const int32_t *__restrict__ iters, const float *__restrict__ sinv,
+                  float *__restrict__ d_val) {
+  extern __shared__ __align__(16) float s_sinv[];   // [n][6]: own columns of S^-1 of the current owner
+  const int mat = blockIdx.y;
+  const int g = grp_begin + mat;
+  const int l0 = list_ptr[g];
+  const int m = list_ptr[g + 1] - l0;
+  const int n = m * NOLSM_BS;
+  XMat<kSplit> xj;
+  if constexpr (kSplit) {
+    xj.hi = ((iters[mat] & 1) ? xr.hi1 : xr.hi0) + (int64_t)mat * slab;
+    xj.lo = ((iters[mat] & 1) ? xr.lo1 : xr.lo0) + (int64_t)mat * slab;
+  } else {
+    xj.x32 = xr.x32 + (int64_t)mat * slab;
+  }
+  const float *sj = sinv + (int64_t)mat * slab;
+  const int r = blockIdx.x * DN_THREADS + threadIdx.x;
+  for (int o = own_ptr[g]; o < own_ptr[g + 1]; ++o) {
+    const int j = own_idx[o];
+    const int own0 = lower_bound_i32(list_idx + l0, m, j) * NOLSM_BS;
+    __syncthreads();
+    for (int t = threadIdx.x; t < NOLSM_BS * n; t += blockDim.x) {
+      const int p = t / n, k = t - p * n;
+      s_sinv[k * NOLSM_BS + p] = sj[(int64_t)(own0 + p) * ld + k];
+    }
+    __syncthreads();
+    if (r < n) {
+      float acc[NOLSM_BS];
+#pragma unroll
+      for (int p = 0; p < NOLSM_BS; ++p) acc[p] = 0.f;
+#pragma unroll 4
+      for (int k = 0; k < n; ++k) {
+        const float xv = xj.at((int64_t)k * ld + r);
+#pragma unroll
+        for (int p = 0; p < NOLSM_BS; ++p) acc[p] = fmaf(xv, s_sinv[k * NOLSM_BS + p], acc[p]);
+      }
+      const int i = list_idx[l0 + r / NOLSM_BS];
+      const int jlo = row_ptr[j], jm = row_ptr[j + 1] - jlo;
+      const int q = lower_bound_i32(col_idx + jlo, jm, i);
+      if (q < jm && col_idx[jlo + q] == i) {
+        float *out = d_val + ((int64_t)(jlo + q) * 36 + (int64_t)(r % NOLSM_BS) * NOLSM_BS);
+#pragma unroll
+        for (int p = 0; p < NOLSM_BS; ++p) out[p] = 0.5f * (s_sinv[r * NOLSM_BS + p] - acc[p]);
+      }
+    }
+  }
+}
+
+cudaError_t launch_density_grouped(const nolsm_batch *b, const XRef &x, const float *sinv, const int32_t *row_ptr,
+                                   const int32_t *col_idx, float *d_val, cudaStream_t st) {
+  if (b->count == 0) return cudaSuccess;
+  const size_t smem = (size_t)NOLSM_BS * b->max_n * sizeof(float);
+  if (smem > 200 * 1024) return cudaErrorInvalidValue;
+  if (smem > 48 * 1024) {
+    cudaError_t e = cudaFuncSetAttribute(k_density_grouped<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess)
+      e = cudaFuncSetAttribute(k_density_grouped<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+  }
+  dim3 grid((b->max_n + DN_THREADS - 1) / DN_THREADS, b->count);
+  if (x.hi0)
+    k_density_grouped<true><<<grid, DN_THREADS, smem, st>>>(row_ptr, col_idx, b->g_own_ptr, b->g_own_idx, b->g_list_ptr,
+                                                            b->g_list_idx, b->mol_begin, b->ld, (int64_t)b->ld * b->ld, x,
+                                                            b->d_iters, sinv, d_val);
+  else
+    k_density_grouped<false><<<grid, DN_THREADS, smem, st>>>(row_ptr, col_idx, b->g_own_ptr, b->g_own_idx, b->g_list_ptr,
+                                                             b->g_list_idx, b->mol_begin, b->ld, (int64_t)b->ld * b->ld, x,
+                                                             b->d_iters, sinv, d_val);
+  return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------
 // a7: N = 2 sum over stored blocks <D(i,j), S(i,j)>_F  (reading 15).
 // One warp per molecule j; lane k handles block (N_j[k], j): D block k of row j against S block
 // (i, j), found by binary search of j in row i of S.  FP32 products, FP64 accumulation.
@@ -713,12 +838,12 @@ cudaError_t launch_density(const nolsm_batch *b, const XRef &x, const float *sin
 
 __global__ void __launch_bounds__(TR_WARPS * 32)
 k_trace(const int32_t *__restrict__ row_ptr, const int32_t *__restrict__ col_idx, int mol_begin,
-        int count, const float *__restrict__ d_val, const float *__restrict__ s_val,
-        double *__restrict__ ne, double *__restrict__ q_mol) {
+        int count, const int32_t *__restrict__ mol_list, const float *__restrict__ d_val,
+        const float *__restrict__ s_val, double *__restrict__ ne, double *__restrict__ q_mol) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int mat = blockIdx.x * TR_WARPS + warp;
   if (mat >= count) return;
-  const int j = mol_begin + mat;
+  const int j = mol_list ? mol_list[mol_begin + mat] : mol_begin + mat;   // owners of combined submatrices: a list
   const int lo = row_ptr[j], hi = row_ptr[j + 1];
   double sum = 0.0;
   for (int k = lo + lane; k < hi; k += 32) {
@@ -749,8 +874,14 @@ cudaError_t launch_trace(const nolsm_batch *b, const int32_t *row_ptr, const int
                          const float *d_val, const float *s_val, double *ne, double *q_mol,
                          cudaStream_t st) {
   if (b->count == 0) return cudaSuccess;
+  if (b->grouped) {   // the owners of the batch's groups are own_idx[own_first, own_first + own_count)
+    if (b->own_count == 0) return cudaSuccess;
+    k_trace<<<(b->own_count + TR_WARPS - 1) / TR_WARPS, TR_WARPS * 32, 0, st>>>(
+        row_ptr, col_idx, b->own_first, b->own_count, b->g_own_idx, d_val, s_val, ne, q_mol);
+    return cudaGetLastError();
+  }
   k_trace<<<(b->count + TR_WARPS - 1) / TR_WARPS, TR_WARPS * 32, 0, st>>>(
-      row_ptr, col_idx, b->mol_begin, b->count, d_val, s_val, ne, q_mol);
+      row_ptr, col_idx, b->mol_begin, b->count, nullptr, d_val, s_val, ne, q_mol);
   return cudaGetLastError();
 }
 

@@ -70,3 +70,37 @@ int main(void) { printf("%zu %zu %zu %zu\n", sizeof(nolsm_config), sizeof(nolsm_
     sizes = [int(x) for x in out]
     assert sizes == [ctypes.sizeof(b.Config), ctypes.sizeof(b._Bsr), ctypes.sizeof(b.SignStats),
                      ctypes.sizeof(b.SolveStats)]
+
+
+def test_combination_heuristic_host_entry_matches_oracle():
+    """nolsm_combine_submatrices is host integer work (no device needed): bit-exact groups against the oracle's
+    plain-Python restatement of section III-B3 on the hand-built examples of test_oracle_pins.py, on the tiny system
+    and on 108- and 256-molecule systems whose lists are far from covering the box (a few pairs and triples merge)."""
+    import numpy as np
+    import nolsm_inputs as gi
+    import oracle.nolsm_oracle as orc
+    import paper_2104_08245_b200 as nolsm
+
+    def csr(lists):
+        rp = np.zeros(len(lists) + 1, dtype=np.int32)
+        rp[1:] = np.cumsum([len(l) for l in lists])
+        return rp, np.concatenate([np.asarray(l, dtype=np.int32) for l in lists])
+
+    cases = [csr([[0, 1, 2, 3]] * 4), csr([[0, 1, 2]] * 3 + [[3, 4, 5]] * 3),
+             csr([[0, 1], [0, 1, 2], [1, 2, 3], [2, 3, 4], [3, 4]])]
+    for n_mol, cutoff in ((32, 6.0), (108, 6.0), (256, 6.0)):
+        s = gi.make_water_system(n_mol, cutoff)
+        cases.append((s.row_ptr, s.col_idx))
+    for rp, ci in cases:
+        ref = orc.combine_submatrices(rp, ci)
+        own_ptr, own_idx, list_ptr, list_idx = nolsm.combine_submatrices(rp, ci)
+        got = [(list(own_idx[own_ptr[g]:own_ptr[g + 1]]), list(list_idx[list_ptr[g]:list_ptr[g + 1]]))
+               for g in range(len(own_ptr) - 1)]
+        assert got == [(list(o), list(r)) for o, r in ref]
+    # the last system has several groups of different sizes (the comparison above is not vacuous)
+    assert 1 < len(got) < 256
+    # error behaviour: a list that is not ascending
+    rp, ci = csr([[1, 0], [0, 1]])
+    import pytest
+    with pytest.raises(nolsm.NolsmError):
+        nolsm.combine_submatrices(rp, ci)

@@ -914,3 +914,54 @@ def test_config4_streaming_path_sampled(nolsm):
     assert abs(ne - system.n_electrons) / n_mol < 1e-3
     assert np.isfinite(d).all()
     ctx.close()
+
+
+# ---------------------------------------------------------------------------------------------
+# combined submatrices (section III-B3, Eq. 14)
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("precision", [1, 0])
+@pytest.mark.parametrize("which", ["tiny", "w256"])
+def test_combined_submatrices_density(nolsm, tiny_system, precision, which):
+    """Groups from nolsm_combine_submatrices (bit-exact against the oracle's heuristic), one dense submatrix per
+    group through nolsm_build_submatrices_grouped / nolsm_sign_batched / nolsm_scatter_density; every owner's
+    blocks D(i, j) and its population against the oracle's solution of the same combined submatrix.
+    tiny: the 32-molecule box, where the lists nearly cover the box and the heuristic merges everything into a few
+    groups; w256: 256 molecules at 6 A, mostly single molecules plus pairs and triples."""
+    import torch
+    import nolsm_inputs as gi
+    import oracle.nolsm_oracle as orc
+    system = tiny_system if which == "tiny" else gi.make_water_system(256, 6.0)
+    ref_groups = orc.combine_submatrices(system.row_ptr, system.col_idx)
+    own_ptr, own_idx, list_ptr, list_idx = nolsm.combine_submatrices(system.row_ptr, system.col_idx)
+    got = [(list(own_idx[own_ptr[g]:own_ptr[g + 1]]), list(list_idx[list_ptr[g]:list_ptr[g + 1]]))
+           for g in range(len(own_ptr) - 1)]
+    assert got == [(list(o), list(r)) for o, r in ref_groups]
+    assert len(got) < system.n_mol
+    H, S = _device_system(nolsm, system)
+    D = S.like()
+    D.val.fill_(float("nan"))
+    groups = nolsm.Groups(own_ptr, own_idx, list_ptr, list_idx)
+    ctx = nolsm.Context(nolsm.Config(precision=precision))
+    batch = ctx.build_submatrices_grouped(H, S, groups, 0, groups.n_groups)
+    st = ctx.sign_batched(batch, MU)
+    assert st.n_unconverged == 0 and st.n_sub == len(got)
+    ne = torch.zeros(1, dtype=torch.float64, device="cuda")
+    q = torch.zeros(system.n_mol, dtype=torch.float64, device="cuda")
+    ctx.scatter_density(batch, S, D, ne, q, None)
+    d = D.val.cpu().numpy()
+    assert np.isfinite(d).all()                    # every stored block was written by its owner's group
+    qh = q.cpu().numpy()
+    checked = 0
+    for g, (owners, rows) in enumerate(ref_groups):
+        if which == "w256" and len(owners) == 1 and g % 16:
+            continue
+        sol = orc.solve_group(system.row_ptr, system.col_idx, system.h_val, system.s_val, owners, rows)
+        for j in owners:
+            ref = sol.density_columns(j, MU).reshape(-1, 6, 6)
+            lo = system.row_ptr[j]
+            assert np.abs(d[lo:lo + ref.shape[0]] - ref).max() < TOL_D[precision], (g, j)
+            checked += 1
+    assert checked >= 20
+    assert abs(ne.item() - qh.sum()) < 1e-6 * system.n_mol
+    assert np.abs(qh - 8.0).max() < 0.05
+    ctx.close()
