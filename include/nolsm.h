@@ -103,6 +103,10 @@ typedef struct {
 #define NOLSM_FLAG_SIMT_ONLY 1 /* debugging: run every product on the FP32 SIMT kernel */
 #define NOLSM_FLAG_PAIR 2      /* always the CTA-pair engine (tcgen05 cta_group::2, 256-row tiles) */
 #define NOLSM_FLAG_SINGLE 8    /* always the single-CTA engine (128-row tiles) */
+#define NOLSM_FLAG_ORDER3 32    /* SURVEY 8(f)#4, "higher-order Pade approximants / arbitrary-order schemes": the
+                                  third-order member X <- X (I + 1/2 E + 3/8 E^2), E = I - X^2 (three products per
+                                  iteration, residual E -> 5/8 E^3) instead of Eq. 9's second-order one.  FP16/FP32 mode
+                                  only; the last iteration is then not folded into the density columns */
 #define NOLSM_FLAG_UNIT_SCALE 16 /* scale by the norm bound itself: Y0 = S/bound, X0 = A/bound (spectra in (0,1] and
                                   [-1,1]) instead of bound/2 and bound/1.5 (readings 5, 7); costs one
                                   iteration each */

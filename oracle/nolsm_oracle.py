@@ -225,6 +225,23 @@ def newton_schulz_sign_scaled(a, n_iter, scale, gap, history=False):
     return (x, np.array(alphas)) if history else x
 
 
+def sign_iteration_order3(a, n_iter, scale=None, history=False):
+    """Third-order member of the Pade family the paper points to as an alternative to Eq. 9 ("higher-order Pade
+    approximants", "arbitrary-order sign matrix iteration schemes", refs [51],[52]): with
+    E_k = I - X_k^2,  X_{k+1} = X_k (I + 1/2 E_k + 3/8 E_k^2)  -- the first three terms of (1 - e)^(-1/2), so
+    E_{k+1} = 5/8 E_k^3 + O(E_k^4).  Returns X_{n_iter} (and r_k = ||E_k||_F / sqrt(n) if history)."""
+    a = np.asarray(a, dtype=np.float64)
+    n = a.shape[0]
+    eye = np.eye(n)
+    x = a / (1.0 if scale is None else scale)
+    res = []
+    for _ in range(n_iter):
+        e = eye - x @ x
+        res.append(np.linalg.norm(e, "fro") / np.sqrt(n))
+        x = x @ (eye + 0.5 * e + 0.375 * (e @ e))
+    return (x, np.array(res)) if history else x
+
+
 def newton_schulz_inverse(s, n_iter, scale=None, history=False):
     """Eq. 15-17: Y0 = S/scale, Z0 = I, V_k = Z_k Y_k,
     Y_{k+1} = 1/2 Y_k (3I - V_k), Z_{k+1} = 1/2 (3I - V_k) Z_k; Z -> Y0^{-1/2}; S^-1 = Z^2/scale.

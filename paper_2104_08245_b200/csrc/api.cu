@@ -723,9 +723,12 @@ static nolsm_status sign_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, double mu, 
   pg.tol = tol;
   // fold_last: stop right after the E_k that passes the test; the caller applies X_{k+1} = X_k + 1/2 X_k E_k
   // only to the own columns of S^-1 (k_last_half), instead of forming it with an n^3 product
+  const bool order3 = fp16 && (ctx->cfg.flags & NOLSM_FLAG_ORDER3) != 0;
+  if (order3) fold_last = false;   // the folded update is Eq. 9's
   pg.stop_early = fold_last ? 1 : 0;
   b->x_pending = fold_last;
   b->x_pending_split = fold_last && !fp16;
+  b->sign_ops = order3 ? 3 : 2;
   ChainOp &e = pg.ops[0] = make_op(EPI_IDENT, 1.f, 0.f);
   ChainOp &x = pg.ops[1] = make_op(EPI_AXPBY, 0.5f, 1.f);
   e.resid = 1;
@@ -740,6 +743,18 @@ static nolsm_status sign_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, double mu, 
     set2(e.a, 0, 1); set2(e.b, 0, 1); set2(e.out16, 4, 4);
     set2(x.a, 0, 1); set2(x.b, 4, 4); set2(x.cin16, 0, 1); set2(x.cin16_lo, 2, 2);
     set2(x.out16, 1, 0); set2(x.out16_lo, 2, 2); x.lo_stream = 1;
+    if (order3) {
+      // X <- X (I + 1/2 E + 3/8 E^2) = X + X G,  G = 1/2 E + 3/8 E E  (refs [51],[52]); G in a half the
+      // iterations do not use: the builder's split copy of S (sparse batches, free after the prepare stage) or h5
+      const int gbuf = b->sparse ? b->n_half - 4 : 5;
+      pg.n_ops = 3;
+      pg.ops[2] = x;
+      ChainOp &g = pg.ops[1] = make_op(EPI_AXPBY, 0.375f, 0.5f);
+      set2(g.a, 4, 4); set2(g.b, 4, 4); set2(g.cin16, 4, 4); set2(g.out16, gbuf, gbuf);
+      ChainOp &x3 = pg.ops[2];
+      x3.alpha = 1.f;
+      set2(x3.b, gbuf, gbuf);
+    }
   } else {
     // split operands: X (h0,h1)/(h2,h3), E (h4,h5)
     // the master iterate is the split operand pair itself (no FP32 copy): X (h0,h1) / (h2,h3) ping-pong
@@ -981,8 +996,8 @@ static nolsm_status collect_stats(nolsm_ctx *ctx, nolsm_batch *b, float tol, int
     if (!(res[m] < tol) && fixed_iter <= 0) s->n_unconverged++;
     if (!(res[m] <= s->worst_residual)) s->worst_residual = res[m];
     const double n = b->n_host[m], P = round_up(b->n_host[m], NOLSM_TILE_M), Pn = round_up(b->n_host[m], 64);
-    s->flops_sign += 2.0 * it[m] * 2.0 * n * n * n;
-    s->flops_sign_padded += 2.0 * it[m] * 2.0 * P * Pn * Pn;
+    s->flops_sign += 2.0 * it[m] * (double)b->sign_ops * n * n * n;
+    s->flops_sign_padded += 2.0 * it[m] * (double)b->sign_ops * P * Pn * Pn;
   }
   return NOLSM_OK;
 }
@@ -1028,7 +1043,7 @@ extern "C" nolsm_status nolsm_sign_batched(nolsm_ctx *ctx, nolsm_batch *batch, d
     stats->inv_iter_max = inv_it;
     stats->inv_worst_residual = inv_res;
     stats->flops_prepare = fp;
-    stats->gemms = gemms + 2 * stats->iter_sum;
+    stats->gemms = gemms + batch->sign_ops * stats->iter_sum;
     stats->ms_chain = chain_ms(ctx, batch);
     stats->chain_mcycles = chain_mcycles(ctx, batch, st);
     if (!batch->engine_simt) stats->n_unconverged = bad[1];
@@ -1350,7 +1365,7 @@ extern "C" nolsm_status nolsm_solve_mu(nolsm_ctx *ctx, const nolsm_bsr *H, const
         acc.flops_sign_padded += cs.flops_sign_padded;
         acc.flops_prepare += bs.flops_prepare;
         acc.inv_iter_max = std::max(acc.inv_iter_max, bs.inv_iter_max);
-        acc.gemms += gemms + 2 * cs.iter_sum - (b->x_pending ? b->count : 0);
+        acc.gemms += gemms + b->sign_ops * cs.iter_sum - (b->x_pending ? b->count : 0);
       }
     }
     if (rc != NOLSM_OK) break;
@@ -1519,7 +1534,7 @@ extern "C" nolsm_status nolsm_sign_dense_batched(nolsm_ctx *ctx, const float *a,
   LAUNCH(ctx, launch_unpack(x_ptr(b), b->ld, (int64_t)b->ld * b->ld, nullptr, nullptr, n, batch, x_out, st));
   if (stats) {
     CHECK(collect_stats(ctx, b, tol, fixed_iter, st, stats));
-    stats->gemms = 2 * stats->iter_sum;
+    stats->gemms = b->sign_ops * stats->iter_sum;
     stats->ms_chain = chain_ms(ctx, b);
     stats->chain_mcycles = chain_mcycles(ctx, b, st);
   }

@@ -94,6 +94,7 @@ struct nolsm_batch {
   int32_t own_first = 0, own_count = 0;   // the batch's owners: g_own_idx[own_first, own_first + own_count)
   int32_t sinv_hi = -1, sinv_lo = -1;   // >= 0: S^-1 lives as the split pair h[sinv_hi] + h[sinv_lo] * 2^-11 and u[2] holds
   bool sinv32_full = true;              // only its own columns in FP32 until join_sinv (false)
+  int32_t sign_ops = 2;           // products per sign iteration of the last chain (3 with NOLSM_FLAG_ORDER3)
   bool x_split = false;           // the sign iterate lives as hi (h[iters & 1]) + lo * 2^-11 (h[2]); u[0] holds X in
   bool x32_valid = false;         // FP32 only after join_x (reading 12)
   bool s_split_built = false;     // the builder wrote the split copy of S into h[n_half-4], h[n_half-3]

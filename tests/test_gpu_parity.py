@@ -965,3 +965,38 @@ def test_combined_submatrices_density(nolsm, tiny_system, precision, which):
     assert abs(ne.item() - qh.sum()) < 1e-6 * system.n_mol
     assert np.abs(qh - 8.0).max() < 0.05
     ctx.close()
+
+
+@pytest.mark.parametrize("n,batch", [(200, 3), (512, 2)])
+def test_order3_iteration_variant(nolsm, torch_mod, mid_system, mid_solution, n, batch):
+    """NOLSM_FLAG_ORDER3 (the third-order Pade member): same sign matrix as the
+    construction Q sign(lam) Q^T, fewer iterations than Eq. 9 and the iteration count of the oracle's literal
+    restatement; same density matrix as the oracle on a partial batch of the 216-molecule system."""
+    import nolsm_inputs as gi
+    import oracle.nolsm_oracle as orc
+    import torch
+    mats = [gi.make_gapped_symmetric(n, seed=23, index=i) for i in range(batch)]
+    a = torch_mod.as_tensor(np.stack([m[0] for m in mats])).cuda()
+    scale = torch_mod.as_tensor(np.array([np.abs(m[2]).max() for m in mats], dtype=np.float32)).cuda()
+    ctx3 = nolsm.Context(nolsm.Config(precision=0, flags=nolsm.FLAG_ORDER3))
+    ctx2 = nolsm.Context(nolsm.Config(precision=0))
+    x3, st3 = ctx3.sign_dense_batched(a, scale)
+    x2, st2 = ctx2.sign_dense_batched(a, scale)
+    assert st3.n_unconverged == 0 and st3.iter_max < st2.iter_max
+    for i, (am, q, lam) in enumerate(mats):
+        assert np.abs(x3[i].cpu().numpy() - orc.sign_by_construction(q, lam)).max() < 3e-3
+        _, hist = orc.sign_iteration_order3(am.astype(np.float64), 12, scale=np.abs(lam).max(), history=True)
+        k_pass = int(np.argmax(hist < 1e-2))          # first iteration whose residual passes; it is finished ("+1")
+        assert st3.iter_min <= k_pass + 1 <= st3.iter_max
+    ctx2.close()
+    H, S = _device_system(nolsm, mid_system)
+    D = S.like()
+    batch_h = ctx3.build_submatrices(H, S, 30, 24)
+    st = ctx3.sign_batched(batch_h, MU)
+    assert st.n_unconverged == 0
+    ne_t = torch.zeros(1, dtype=torch.float64, device="cuda")
+    ctx3.scatter_density(batch_h, S, D, ne_t, None, None)
+    d_ref = orc.density_blocks(mid_solution["solutions"], mid_system.row_ptr, MU)
+    lo, hi = mid_system.row_ptr[30], mid_system.row_ptr[54]
+    assert np.abs(D.val.cpu().numpy()[lo:hi] - d_ref[lo:hi]).max() < TOL_D[0]
+    ctx3.close()

@@ -618,3 +618,23 @@ def test_combination_heuristic_invariants_on_water(tiny_system, tiny_solution):
     for j in (0, 13, 31):
         cols = ref["solutions"][j].density_columns(-0.85)
         assert np.abs(sol.density_columns(j, -0.85) - cols).max() < 1e-12
+
+
+def test_order3_sign_iteration_pins():
+    """Scalar closed form (worked by hand): x = 0.5 -> e = 0.75 -> x (1 + 0.375 + 0.2109375) = 0.79296875; cubic
+    convergence e' -> 5/8 e^3 (the first three terms of (1 - e)^(-1/2)); the fixed points are +-1; and the matrix
+    iteration reaches Q sign(lam) Q^T (known by construction) in fewer iterations than Eq. 9."""
+    assert orc.sign_iteration_order3(np.array([[0.5]]), 1)[0, 0] == 0.79296875
+    x = np.array([[0.99]])
+    e0 = 1 - 0.99 ** 2
+    x1 = orc.sign_iteration_order3(x, 1)[0, 0]
+    assert abs((1 - x1 * x1) / e0 ** 3 - 0.625) < 0.02
+    assert orc.sign_iteration_order3(np.diag([1.0, -1.0]), 3).tolist() == [[1.0, 0.0], [0.0, -1.0]]
+    a, q, lam = gi.make_gapped_symmetric(48, seed=7)
+    a = a.astype(np.float64)
+    sc = np.abs(lam).max()
+    x3, r3 = orc.sign_iteration_order3(a, 8, scale=sc, history=True)
+    x2, r2 = orc.newton_schulz_sign(a, 14, scale=sc, history=True)
+    assert (r2 < 1e-2).any()
+    assert np.abs(x3 - orc.sign_by_construction(q, lam)).max() < 1e-5      # FP32 input matrix
+    assert np.argmax(r3 < 1e-2) < np.argmax(r2 < 1e-2)                     # fewer iterations to the same residual
