@@ -292,6 +292,19 @@ NOLSM_API nolsm_status nolsm_sign_dense_batched(nolsm_ctx *ctx, const float *a, 
                                       int32_t fixed_iter, float *x_out, nolsm_sign_stats *stats /*host*/,
                                       void *stream);
 
+/* --- the merged pattern of H0 and S ("row i is kept if H_ij != 0 or S_ij != 0") ---
+ * The iteration entry points take H and S on ONE pattern.  When the two stores come with different patterns:
+ * nolsm_union_pattern (HOST integer work, ascending CSR rows in and out; two passes; NOLSM_ENOMEM with *nnzb_out =
+ * needed size when cap is too small) builds the merged pattern, and nolsm_expand_store (device, asynchronous) lays a
+ * store out on it: block k of row i = the source's block (i, col_idx_dst[k]) if stored, else zero.  The source
+ * pattern must be a subset of the destination's rows-wise (blocks of the source outside it are dropped). */
+NOLSM_API nolsm_status nolsm_union_pattern(int32_t n_mol, const int32_t *row_ptr_a /*host*/, const int32_t *col_idx_a /*host*/,
+                                           const int32_t *row_ptr_b /*host*/, const int32_t *col_idx_b /*host*/,
+                                           int32_t *row_ptr_u /*host [n_mol+1]*/, int32_t *col_idx_u /*host*/, int64_t cap,
+                                           int64_t *nnzb_out /*host*/);
+NOLSM_API nolsm_status nolsm_expand_store(nolsm_ctx *ctx, const nolsm_bsr *src, const int32_t *row_ptr_dst,
+                                          const int32_t *col_idx_dst, float *val_dst, void *stream);
+
 /* --- submatrix combination heuristic (section III-B3, Eq. 14) ---
  * nolsm_combine_submatrices: HOST integer work (the paper runs it on CPU cores, off the clock).
  * Input: the neighbour lists (host CSR, ascending, self included) = the row sets of the one-per-molecule submatrices.

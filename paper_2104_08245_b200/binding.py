@@ -21,7 +21,7 @@ EXPORTED_SYMBOLS = [
     "nolsm_scatter_density", "nolsm_solve_mu", "nolsm_solve_mu_host", "nolsm_sign_dense_batched", "nolsm_batch_read",
     "nolsm_batch_size", "nolsm_batch_ld", "nolsm_gemm_batched", "nolsm_launch_count",
     "nolsm_scatter_energy", "nolsm_evaluate", "nolsm_set_model", "nolsm_combine_submatrices",
-    "nolsm_build_submatrices_grouped",
+    "nolsm_build_submatrices_grouped", "nolsm_union_pattern", "nolsm_expand_store",
 ]
 
 
@@ -151,6 +151,10 @@ def load_library():
     lib.nolsm_combine_submatrices.restype = i32
     lib.nolsm_build_submatrices_grouped.argtypes = [vp, P(_Bsr), P(_Bsr), P(_Groups), i32, i32, i32, P(vp), vp]
     lib.nolsm_build_submatrices_grouped.restype = i32
+    lib.nolsm_union_pattern.argtypes = [i32, vp, vp, vp, vp, vp, vp, i64, P(i64)]
+    lib.nolsm_union_pattern.restype = i32
+    lib.nolsm_expand_store.argtypes = [vp, P(_Bsr), vp, vp, vp, vp]
+    lib.nolsm_expand_store.restype = i32
     _LIB = lib
     return lib
 
@@ -248,6 +252,23 @@ def combine_submatrices(row_ptr, col_idx):
         raise NolsmError(st, "nolsm_combine_submatrices")
     g = ng.value
     return own_ptr[:g + 1].copy(), own_idx[:n].copy(), list_ptr[:g + 1].copy(), list_idx[:ll.value].copy()
+
+
+def union_pattern(row_ptr_a, col_idx_a, row_ptr_b, col_idx_b):
+    """nolsm_union_pattern on host int32 numpy arrays. Returns (row_ptr, col_idx) of the merged pattern."""
+    import numpy as np
+    lib = load_library()
+    a_rp, a_ci, b_rp, b_ci = (np.ascontiguousarray(x, dtype=np.int32) for x in (row_ptr_a, col_idx_a, row_ptr_b, col_idx_b))
+    n = int(a_rp.shape[0]) - 1
+    rp = np.zeros(n + 1, dtype=np.int32)
+    cap = int(a_ci.shape[0] + b_ci.shape[0])
+    ci = np.zeros(max(cap, 1), dtype=np.int32)
+    nnzb = C.c_int64(0)
+    st = lib.nolsm_union_pattern(n, a_rp.ctypes.data, a_ci.ctypes.data, b_rp.ctypes.data, b_ci.ctypes.data,
+                                 rp.ctypes.data, ci.ctypes.data, cap, C.byref(nnzb))
+    if st != 0:
+        raise NolsmError(st, "nolsm_union_pattern")
+    return rp, ci[:nnzb.value].copy()
 
 
 class Groups:
@@ -358,6 +379,14 @@ class Context:
         self._check(self.lib.nolsm_build_submatrices_grouped(self.handle, H.ref(), S.ref(), groups.ref(), grp_begin,
                                                              grp_count, slot, C.byref(h), _stream(stream)))
         return Batch(self, h)
+
+    def expand_store(self, src, row_ptr, col_idx, stream=None):
+        """src (BlockSparse) laid out on the (larger) device pattern (row_ptr, col_idx): a new BlockSparse."""
+        torch = _torch()
+        val = torch.empty((int(col_idx.numel()), 6, 6), dtype=torch.float32, device="cuda")
+        self._check(self.lib.nolsm_expand_store(self.handle, src.ref(), _ptr(row_ptr, torch.int32), _ptr(col_idx, torch.int32),
+                                                _ptr(val, torch.float32), _stream(stream)))
+        return BlockSparse(row_ptr, col_idx, val)
 
     def batch_capacity(self, H, mol_begin=0, n_slots=1, stream=None):
         r = self.lib.nolsm_batch_capacity(self.handle, H.ref(), mol_begin, n_slots, _stream(stream))

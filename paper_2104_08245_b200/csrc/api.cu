@@ -417,6 +417,17 @@ static nolsm_status build_submatrices_impl(nolsm_ctx *ctx, const nolsm_bsr *H, c
   return NOLSM_OK;
 }
 
+// The merged H0 u S pattern: a store re-laid on the union pattern of nolsm_union_pattern.
+extern "C" nolsm_status nolsm_expand_store(nolsm_ctx *ctx, const nolsm_bsr *src, const int32_t *row_ptr_dst,
+                                           const int32_t *col_idx_dst, float *val_dst, void *stream) {
+  if (!ctx) return NOLSM_EINVAL;
+  CHECK(check_bsr(ctx, src, "src"));
+  if (!row_ptr_dst || (src->n_mol > 0 && (!col_idx_dst || !val_dst))) { ctx->err = "nolsm_expand_store: null destination"; return NOLSM_EINVAL; }
+  LAUNCH(ctx, launch_expand_store(src->n_mol, src->row_ptr, src->col_idx, src->val, row_ptr_dst, col_idx_dst, val_dst,
+                                  (cudaStream_t)stream));
+  return NOLSM_OK;
+}
+
 // a batch of COMBINED submatrices.  Group g's dense pair is T(H), T(S) over its
 // merged row set; everything downstream of the gather (Eq. 15-17, sign iteration) is the same batch machinery.
 extern "C" nolsm_status nolsm_build_submatrices_grouped(nolsm_ctx *ctx, const nolsm_bsr *H, const nolsm_bsr *S,

@@ -134,3 +134,36 @@ extern "C" nolsm_status nolsm_combine_submatrices(int32_t n_mol, const int32_t *
   }
   return NOLSM_OK;
 }
+
+// Merged sparsity pattern of H0 and S ("row i is kept if H_ij != 0 or S_ij != 0"): the union of two
+// block patterns given as host CSR arrays with ascending rows.  Host integer work, done once per pattern change.
+extern "C" nolsm_status nolsm_union_pattern(int32_t n_mol, const int32_t *row_ptr_a, const int32_t *col_idx_a,
+                                            const int32_t *row_ptr_b, const int32_t *col_idx_b, int32_t *row_ptr_u,
+                                            int32_t *col_idx_u, int64_t cap, int64_t *nnzb_out) {
+  if (n_mol < 0 || !row_ptr_a || !row_ptr_b || !row_ptr_u || cap < 0 || (cap > 0 && !col_idx_u)) return NOLSM_EINVAL;
+  int64_t total = 0;
+  for (int pass = 0; pass < 2; ++pass) {
+    int64_t w = 0;
+    for (int32_t i = 0; i < n_mol; ++i) {
+      int32_t a = row_ptr_a[i], ae = row_ptr_a[i + 1], b = row_ptr_b[i], be = row_ptr_b[i + 1];
+      if (ae < a || be < b) return NOLSM_EINVAL;
+      if (pass == 1) row_ptr_u[i] = (int32_t)w;
+      while (a < ae || b < be) {
+        int32_t c;
+        if (b >= be || (a < ae && col_idx_a[a] < col_idx_b[b])) c = col_idx_a[a++];
+        else if (a >= ae || col_idx_b[b] < col_idx_a[a]) c = col_idx_b[b++];
+        else { c = col_idx_a[a]; ++a; ++b; }
+        if (pass == 1) col_idx_u[w] = c;
+        ++w;
+      }
+    }
+    if (pass == 0) {
+      total = w;
+      if (nnzb_out) *nnzb_out = total;
+      if (total > cap || total > 0x7fffffff) return NOLSM_ENOMEM;
+    } else {
+      row_ptr_u[n_mol] = (int32_t)w;
+    }
+  }
+  return NOLSM_OK;
+}

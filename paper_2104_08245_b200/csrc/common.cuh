@@ -201,6 +201,8 @@ struct XRef {
   const __half *hi0, *hi1, *lo0, *lo1;   // hi0 != null: split pair (hi, lo) number (iters & 1)
 };
 cudaError_t launch_join_split(const nolsm_batch *b, const XRef &x, float *dst32, cudaStream_t st);
+cudaError_t launch_expand_store(int n_mol, const int32_t *rp_src, const int32_t *ci_src, const float *val_src,
+                                const int32_t *rp_dst, const int32_t *ci_dst, float *val_dst, cudaStream_t st);
 cudaError_t launch_own_join_grouped(const nolsm_batch *b, const __half *hi, const __half *lo, float *dst32,
                                     cudaStream_t st);
 cudaError_t launch_density_grouped(const nolsm_batch *b, const XRef &x, const float *sinv, const int32_t *row_ptr,

@@ -710,6 +710,37 @@ cudaError_t launch_density(const nolsm_batch *b, const XRef &x, const float *sin
 }
 
 // ------------------------------------------------------------------------------------------------
+// Block store on a larger pattern (the merged H0 u S pattern): block k of row i of the destination is
+// the source's block (i, col_idx_dst[k]) if the source stores that pair, else zero.  One warp per destination block.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+k_expand_store(int n_mol, const int32_t *__restrict__ rp_src, const int32_t *__restrict__ ci_src,
+               const float *__restrict__ val_src, const int32_t *__restrict__ rp_dst,
+               const int32_t *__restrict__ ci_dst, float *__restrict__ val_dst) {
+  const int lane = threadIdx.x & 31;
+  const int i = blockIdx.x;
+  if (i >= n_mol) return;
+  const int s0 = rp_src[i], sm = rp_src[i + 1] - s0;
+  for (int k = rp_dst[i] + (threadIdx.x >> 5); k < rp_dst[i + 1]; k += blockDim.x >> 5) {
+    const int c = ci_dst[k];
+    int l = 0, r = sm;
+    while (l < r) {
+      const int mid = (l + r) >> 1;
+      if (ci_src[s0 + mid] < c) l = mid + 1; else r = mid;
+    }
+    const bool hit = l < sm && ci_src[s0 + l] == c;
+    for (int e = lane; e < 36; e += 32) val_dst[(int64_t)k * 36 + e] = hit ? val_src[(int64_t)(s0 + l) * 36 + e] : 0.f;
+  }
+}
+
+cudaError_t launch_expand_store(int n_mol, const int32_t *rp_src, const int32_t *ci_src, const float *val_src,
+                                const int32_t *rp_dst, const int32_t *ci_dst, float *val_dst, cudaStream_t st) {
+  if (n_mol == 0) return cudaSuccess;
+  k_expand_store<<<n_mol, 256, 0, st>>>(n_mol, rp_src, ci_src, val_src, rp_dst, ci_dst, val_dst);
+  return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------
 // Combined submatrices: one submatrix serves several molecules (its owners).
 // Group g has the merged row set U_g = list_idx[list_ptr[g] ..) and the owners own_idx[own_ptr[g] ..).
 // ------------------------------------------------------------------------------------------------

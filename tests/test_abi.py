@@ -104,3 +104,22 @@ def test_combination_heuristic_host_entry_matches_oracle():
     import pytest
     with pytest.raises(nolsm.NolsmError):
         nolsm.combine_submatrices(rp, ci)
+
+
+def test_union_pattern_host_entry():
+    """nolsm_union_pattern against Python sets (row i kept if H_ij != 0 or S_ij != 0)."""
+    import numpy as np
+    import paper_2104_08245_b200 as nolsm
+    rng = np.random.default_rng(3)
+    n = 40
+    def rand_pattern(p):
+        lists = [sorted(set(np.nonzero(rng.random(n) < p)[0].tolist()) | {i}) for i in range(n)]
+        rp = np.zeros(n + 1, dtype=np.int32)
+        rp[1:] = np.cumsum([len(l) for l in lists])
+        return rp, np.concatenate([np.asarray(l, dtype=np.int32) for l in lists]), lists
+    rpa, cia, la = rand_pattern(0.2)
+    rpb, cib, lb = rand_pattern(0.1)
+    rp, ci = nolsm.union_pattern(rpa, cia, rpb, cib)
+    for i in range(n):
+        assert list(ci[rp[i]:rp[i + 1]]) == sorted(set(la[i]) | set(lb[i]))
+    assert rp[-1] == len(ci)

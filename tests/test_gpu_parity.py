@@ -1000,3 +1000,46 @@ def test_order3_iteration_variant(nolsm, torch_mod, mid_system, mid_solution, n,
     lo, hi = mid_system.row_ptr[30], mid_system.row_ptr[54]
     assert np.abs(D.val.cpu().numpy()[lo:hi] - d_ref[lo:hi]).max() < TOL_D[0]
     ctx3.close()
+
+
+def test_merged_pattern_of_h_and_s(nolsm, mid_system):
+    """H0 and S stored on DIFFERENT patterns: S truncated at 6 A, H at 8 A with a seventh of its
+    off-diagonal blocks dropped, so neither pattern contains the other.  nolsm_union_pattern + nolsm_expand_store
+    give the merged pattern; D on it against the oracle, which slices each matrix from its own store over the
+    merged index set."""
+    import torch
+    import nolsm_inputs as gi
+    import oracle.nolsm_oracle as orc
+    sys_h = mid_system                                   # 216 molecules, 8 A
+    sys_s = gi.make_water_system(216, 6.0)               # same seed -> same positions
+    assert np.array_equal(sys_h.pos_q, sys_s.pos_q)
+    rows = np.repeat(np.arange(216), np.diff(sys_h.row_ptr))
+    keep = (rows == sys_h.col_idx) | ((rows + sys_h.col_idx) % 7 != 0)
+    rp_h = np.zeros(217, dtype=np.int32)
+    rp_h[1:] = np.cumsum(np.bincount(rows[keep], minlength=216))
+    ci_h, h_val = sys_h.col_idx[keep], sys_h.h_val[keep]
+    rp_u, ci_u = nolsm.union_pattern(rp_h, ci_h, sys_s.row_ptr, sys_s.col_idx)
+    assert len(ci_u) > len(ci_h) and len(ci_u) > sys_s.nnzb
+    Hs = nolsm.BlockSparse.from_numpy(rp_h, ci_h, h_val)
+    Ss = nolsm.BlockSparse.from_numpy(sys_s.row_ptr, sys_s.col_idx, sys_s.s_val)
+    ctx = nolsm.Context(nolsm.Config(precision=1))
+    rp_d = torch.as_tensor(rp_u).cuda()
+    ci_d = torch.as_tensor(ci_u).cuda()
+    H = ctx.expand_store(Hs, rp_d, ci_d)
+    S = ctx.expand_store(Ss, rp_d, ci_d)
+    begin, count = 40, 16
+    batch = ctx.build_submatrices(H, S, begin, count)
+    st = ctx.sign_batched(batch, MU)
+    assert st.n_unconverged == 0
+    D = S.like()
+    ne = torch.zeros(1, dtype=torch.float64, device="cuda")
+    ctx.scatter_density(batch, S, D, ne, None, None)
+    d = D.val.cpu().numpy()
+    for j in (begin, begin + 7, begin + count - 1):
+        nbrs = ci_u[rp_u[j]:rp_u[j + 1]]
+        h_sub = orc.dense_submatrix(rp_h, ci_h, h_val, nbrs)
+        s_sub = orc.dense_submatrix(sys_s.row_ptr, sys_s.col_idx, sys_s.s_val, nbrs)
+        sol = orc.SubmatrixSolution(j, nbrs, h_sub, s_sub)
+        ref = sol.density_columns(MU).reshape(-1, 6, 6)
+        assert np.abs(d[rp_u[j]:rp_u[j + 1]] - ref).max() < TOL_D[1]
+    ctx.close()
