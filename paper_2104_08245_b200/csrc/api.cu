@@ -550,10 +550,19 @@ static ChainProgram one_shot(int group) {
 // S^-1 = Z^2 / s_S (Eq. 17), optional Newton refinements (reading 11) and B = S^-1 H
 // (Eq. 12).  FP16 mode: the iteration runs on plain FP16 operands, everything after it
 // on split (hi + lo) operands; FP32 mode: every product on split operands.
+static nolsm_status ensure_thin(nolsm_ctx *ctx, nolsm_batch *b, cudaStream_t st);
+
+// own_only (nolsm_solve_mu without energy products: nothing downstream reads S^-1 outside its six own columns):
+// the refinement is applied to B and to those columns instead of to all of S^-1, see below.
 static nolsm_status prepare_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, int precision, cudaStream_t st,
-                                        nolsm_sign_stats *stats, int64_t *gemms) {
+                                        nolsm_sign_stats *stats, int64_t *gemms, bool own_only) {
   const bool fp16 = precision == NOLSM_FP16_FP32;
   const int refine = ctx->cfg.inv_refine >= 0 ? ctx->cfg.inv_refine : (fp16 ? 1 : 0);
+  // one refinement, FP16 mode, one owner per submatrix: B1 = B0 + A0 (H - S B0) with B0 = A0 H and A0 = Z^2/s_S the
+  // FP16-quality inverse -- the same second-order error (I - A0 S)^2 S^-1 H as refining S^-1 first, in five MMAs
+  // (1 + 3 + 1) instead of seven (3 + 1 for the refinement, 3 for B on split operands); the own columns of S^-1
+  // get their refinement as two thin products (k_own_refine)
+  const bool fast_b = own_only && fp16 && refine == 1 && b->sparse && b->row_ptr != nullptr && !b->grouped;
   // 3e-3 with a refinement behind: the iterate is taken with a relative error of about twice its residual,
   // which the refinement squares (< 4e-5)
   const float inv_tol = ctx->cfg.inv_tol > 0.f ? ctx->cfg.inv_tol : (fp16 ? (refine > 0 ? 3e-3f : 1e-2f) : 1e-5f);
@@ -661,7 +670,8 @@ static nolsm_status prepare_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, int prec
       si_hi = 2; si_lo = 3;
     }
     // with a refinement behind it S^-1 only continues as the split pair; its FP32 form is not needed
-    o.use_div = 1; o.cout32 = refine > 0 ? -1 : 2; set2(o.out16, si_hi, si_hi); set2(o.out16_lo, si_lo, si_lo);
+    o.use_div = 1; o.cout32 = refine > 0 ? -1 : 2; set2(o.out16, si_hi, si_hi);
+    if (!fast_b) set2(o.out16_lo, si_lo, si_lo);
     CHECK(run_chain(ctx, b, p1, b->d_scale, false, st));
   }
   // split S (refinements) and split H (B = S^-1 H) come from the builder, in the last four halves
@@ -671,6 +681,32 @@ static nolsm_status prepare_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, int prec
   int fr_hi = fp16 ? 3 : 0, fr_lo = fp16 ? 5 : 1;
   if (refine > 0 && !b->s_split_built)           // batch built under another configuration
     LAUNCH(ctx, launch_scale_copy(b, S, nullptr, 0, nullptr, b->h[ss_hi], b->h[ss_lo], st));
+  if (fast_b) {
+    // A0: h0.  B0 = A0 H (plain FP16 operands) -> split pair (h1, h4);  R = H - S B0 on split operands -> h5;
+    // B1 = B0 + A0 R -> u3.  Z (h2 / h3) is not read any more.
+    ChainProgram p5 = one_shot(g1);
+    p5.n_ops = 3;
+    ChainOp &b0 = p5.ops[0] = make_op(EPI_AXPBY, 1.f, 0.f);
+    set2(b0.a, si_hi, si_hi); set2(b0.b, hs_hi, hs_hi); set2(b0.out16, 1, 1); set2(b0.out16_lo, 4, 4);
+    ChainOp &r = p5.ops[1] = make_op(EPI_AXPBY, -1.f, 1.f);
+    set2(r.a, ss_hi, ss_hi); set2(r.a_lo, ss_lo, ss_lo); set2(r.b, 1, 1); set2(r.b_lo, 4, 4);
+    set2(r.cin16, hs_hi, hs_hi); set2(r.cin16_lo, hs_lo, hs_lo); set2(r.out16, 5, 5);
+    ChainOp &b1 = p5.ops[2] = make_op(EPI_AXPBY, 1.f, 1.f);
+    set2(b1.a, si_hi, si_hi); set2(b1.b, 5, 5); set2(b1.cin16, 1, 1); set2(b1.cin16_lo, 4, 4);
+    b1.cout32 = 3;
+    CHECK(run_chain(ctx, b, p5, nullptr, false, st));
+    CHECK(ensure_thin(ctx, b, st));
+    LAUNCH(ctx, launch_own_refine(b, b->row_ptr, b->col_idx, b->h[ss_hi], b->h[ss_lo], b->h[si_hi], b->d_thin, b->u[2], st));
+    b->sinv_hi = b->sinv_lo = -1;
+    b->sinv32_full = false;
+    b->sinv_own_only = true;
+    b->engine_simt = false;
+    b->prepared = true;
+    b->prepared_precision = precision;
+    *gemms += inv_gemm_sum;
+    return NOLSM_OK;
+  }
+  b->sinv_own_only = false;
   for (int it = 0; it < refine; ++it) {
     // Newton refinement S^-1 <- S^-1 + S^-1 (I - S S^-1): the residual on split operands, the small
     // correction on plain FP16 operands (reading 11); the refined S^-1 leaves the epilogue as
@@ -920,9 +956,10 @@ static nolsm_status sign_batch_simt(nolsm_ctx *ctx, nolsm_batch *b, double mu, f
 }
 
 static nolsm_status prepare_batch(nolsm_ctx *ctx, nolsm_batch *b, int precision, cudaStream_t st,
-                                  nolsm_sign_stats *stats, int64_t *gemms) {
+                                  nolsm_sign_stats *stats, int64_t *gemms, bool own_only = false) {
+  b->sinv_own_only = false;
   if (use_simt(ctx)) return prepare_batch_simt(ctx, b, st, stats, gemms);
-  return prepare_batch_chain(ctx, b, precision, st, stats, gemms);
+  return prepare_batch_chain(ctx, b, precision, st, stats, gemms, own_only);
 }
 
 // timed: records ctx->tev[0..1] around the chain kernel; read with chain_ms() after a synchronise
@@ -963,7 +1000,25 @@ static XRef x_ref(const nolsm_batch *b) {
   return XRef{x_ptr(b), nullptr, nullptr, nullptr, nullptr};
 }
 // full FP32 S^-1 in u2 (the prepare stage leaves only its own columns there), for the consumers that read all of it
+// scratch of the thin (n x 6) products: 2 * count * 6 * ld floats
+static nolsm_status ensure_thin(nolsm_ctx *ctx, nolsm_batch *b, cudaStream_t st) {
+  const size_t need = (size_t)2 * b->count * NOLSM_BS * b->ld;
+  if (need <= b->thin_cap) return NOLSM_OK;
+  cudaStreamSynchronize(st);
+  cudaFree(b->d_thin);
+  b->d_thin = nullptr;
+  b->thin_cap = 0;
+  if (need && cudaMalloc(&b->d_thin, need * sizeof(float)) != cudaSuccess) {
+    cudaGetLastError();
+    ctx->err = "cudaMalloc of the thin-product scratch failed";
+    return NOLSM_ENOMEM;
+  }
+  b->thin_cap = need;
+  return NOLSM_OK;
+}
+
 static nolsm_status join_sinv(nolsm_ctx *ctx, nolsm_batch *b, cudaStream_t st) {
+  if (b->sinv_own_only) { ctx->err = "this batch holds the own columns of S^-1 only"; return NOLSM_EINVAL; }
   if (b->engine_simt || b->sinv32_full || b->sinv_hi < 0) return NOLSM_OK;
   LAUNCH(ctx, launch_join_split(b, XRef{nullptr, b->h[b->sinv_hi], b->h[b->sinv_hi], b->h[b->sinv_lo], b->h[b->sinv_lo]},
                                 b->u[2], st));
@@ -1094,19 +1149,7 @@ extern "C" nolsm_status nolsm_scatter_density(nolsm_ctx *ctx, const nolsm_batch 
   float *u_thin = nullptr;
   if (batch->x_pending) {
     nolsm_batch *bm = const_cast<nolsm_batch *>(batch);
-    const size_t need = (size_t)2 * batch->count * NOLSM_BS * batch->ld;   // same scratch as the energy products
-    if (need > bm->thin_cap) {
-      cudaStreamSynchronize(st);
-      cudaFree(bm->d_thin);
-      bm->d_thin = nullptr;
-      bm->thin_cap = 0;
-      if (cudaMalloc(&bm->d_thin, need * sizeof(float)) != cudaSuccess) {
-        cudaGetLastError();
-        ctx->err = "cudaMalloc of the thin-product scratch failed";
-        return NOLSM_ENOMEM;
-      }
-      bm->thin_cap = need;
-    }
+    CHECK(ensure_thin(ctx, bm, st));   // same scratch as the energy products
     u_thin = bm->d_thin;
   }
   LAUNCH(ctx, launch_density(batch, x_ref(batch), sinv_ptr(batch), S->row_ptr, S->col_idx, D->val,
@@ -1326,7 +1369,7 @@ extern "C" nolsm_status nolsm_solve_mu(nolsm_ctx *ctx, const nolsm_bsr *H, const
       nolsm_sign_stats bs;
       memset(&bs, 0, sizeof(bs));
       if (!b->prepared) {
-        rc = prepare_batch(ctx, b, prec, st, stats ? &bs : nullptr, &gemms);
+        rc = prepare_batch(ctx, b, prec, st, stats ? &bs : nullptr, &gemms, !ctx->eval_energy);
         if (rc != NOLSM_OK) break;
         if (cache) {
           const size_t slab_all = cache_sq[bi];

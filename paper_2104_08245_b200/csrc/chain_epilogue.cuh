@@ -514,6 +514,10 @@ __device__ __forceinline__ float epi_chunks(const ChainArgs &args, const TileCmd
         t.p32 += kChunkRows;
       }
     }
+    // an FP32 result over an FP16 add-in: the result of row half h fills all of plane h, which holds add-in pieces
+    // of the other half's warps, so every compute warp has to have read its add-in first (all of them pass here:
+    // the chunk loop and the branches above are uniform over the compute warps)
+    if (t.io.out32 >= 0 && t.io.in_hi >= 0) asm volatile("bar.sync 1, %0;" ::"n"(kComputeWarps * 32) : "memory");
     if (t.io.out32 >= 0) {    // FP32 result into the plane of this warp's row half; rows beyond the tile as zero
       if (cnt < R) {
 #pragma unroll

@@ -94,6 +94,7 @@ struct nolsm_batch {
   int32_t own_first = 0, own_count = 0;   // the batch's owners: g_own_idx[own_first, own_first + own_count)
   int32_t sinv_hi = -1, sinv_lo = -1;   // >= 0: S^-1 lives as the split pair h[sinv_hi] + h[sinv_lo] * 2^-11 and u[2] holds
   bool sinv32_full = true;              // only its own columns in FP32 until join_sinv (false)
+  bool sinv_own_only = false;           // S^-1 was refined in its own columns only (nolsm_solve_mu): no full S^-1
   int32_t sign_ops = 2;           // products per sign iteration of the last chain (3 with NOLSM_FLAG_ORDER3)
   bool x_split = false;           // the sign iterate lives as hi (h[iters & 1]) + lo * 2^-11 (h[2]); u[0] holds X in
   bool x32_valid = false;         // FP32 only after join_x (reading 12)
@@ -208,6 +209,12 @@ cudaError_t launch_own_join_grouped(const nolsm_batch *b, const __half *hi, cons
 cudaError_t launch_density_grouped(const nolsm_batch *b, const XRef &x, const float *sinv, const int32_t *row_ptr,
                                    const int32_t *col_idx, float *d_val, cudaStream_t st);
 // own columns of a split matrix (hi + lo * 2^-11) as FP32 into the same columns of dst32
+// thin_kernels.cu
+cudaError_t launch_density_split(const nolsm_batch *b, const XRef &x, const float *sinv, const int32_t *row_ptr,
+                                 const int32_t *col_idx, float *d_val, double *ne_diag, const __half *e_hi,
+                                 const __half *e_lo, float *u_thin, cudaStream_t st);
+cudaError_t launch_own_refine(const nolsm_batch *b, const int32_t *row_ptr, const int32_t *col_idx, const __half *s_hi,
+                              const __half *s_lo, const __half *a0, float *thin, float *out32, cudaStream_t st);
 cudaError_t launch_own_join(const nolsm_batch *b, const int32_t *row_ptr, const int32_t *col_idx, const __half *hi,
                             const __half *lo, float *dst32, cudaStream_t st);
 cudaError_t launch_density(const nolsm_batch *b, const XRef &x, const float *sinv,

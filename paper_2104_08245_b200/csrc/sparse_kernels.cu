@@ -495,6 +495,22 @@ cudaError_t launch_own_columns(const nolsm_batch *b, const int32_t *row_ptr, con
 
 #define DN_THREADS 256
 
+// a5: D columns of the own molecule, 1/2 (V - X V) with V the six own columns of
+// S^-1.  An n x n x 6 product bound by reading X once.  CTA = DN_ROWS rows x DN_KSPLIT slices of the k range;
+// a thread owns two consecutive rows (n = 6m is even, ld a multiple of 128: every pair is one aligned 4-byte FP16
+// or 8-byte FP32 load, so a warp request is a full 128-byte line or two) and one k slice; the slices are summed
+// through shared memory.
+#define DN_KSPLIT 4
+#define DN_ROWS 128   // rows per CTA: (DN_THREADS / DN_KSPLIT) threads x 2 rows
+#define DN_RED_FLOATS ((DN_KSPLIT - 1) * DN_ROWS * NOLSM_BS)
+
+__device__ __forceinline__ float2 split_pair(const __half *hi, const __half *lo, int64_t off) {
+  const float2 h = __half22float2(__ldg(reinterpret_cast<const __half2 *>(hi + off)));
+  if (lo == nullptr) return h;
+  const float2 l = __half22float2(__ldg(reinterpret_cast<const __half2 *>(lo + off)));
+  return make_float2(fmaf(l.x, 1.f / 2048.f, h.x), fmaf(l.y, 1.f / 2048.f, h.y));
+}
+
 // element of the sign iterate: FP32, or hi + lo * 2^-11 (the split master of DESIGN.md reading 12)
 template <bool kSplit>
 struct XMat {
@@ -504,7 +520,63 @@ struct XMat {
     if constexpr (kSplit) return fmaf(__half2float(__ldg(lo + off)), 1.f / 2048.f, __half2float(__ldg(hi + off)));
     else return __ldg(x32 + off);
   }
+  // elements off, off + 1 (off even)
+  __device__ __forceinline__ float2 at2(int64_t off) const {
+    if constexpr (kSplit) return split_pair(hi, lo, off);
+    else return __ldg(reinterpret_cast<const float2 *>(x32 + off));
+  }
 };
+
+// position of molecule j in its own (sorted) neighbour list
+__device__ __forceinline__ int own_position(const int32_t *__restrict__ col_idx, int lo, int m, int j) {
+  int l = 0, r_ = m;
+  while (l < r_) {
+    const int mid = (l + r_) >> 1;
+    if (col_idx[lo + mid] < j) l = mid + 1; else r_ = mid;
+  }
+  return l;
+}
+
+// sum of the k slices: slices 1.. park their partial sums in shared memory, slice 0 adds them up
+__device__ __forceinline__ void slice_reduce(float *red, int ks, int rp, float (&acc)[2][NOLSM_BS]) {
+  if (ks > 0) {
+    float *dst = red + ((ks - 1) * DN_ROWS + 2 * rp) * NOLSM_BS;
+#pragma unroll
+    for (int q = 0; q < 2; ++q)
+#pragma unroll
+      for (int p = 0; p < NOLSM_BS; ++p) dst[q * NOLSM_BS + p] = acc[q][p];
+  }
+  __syncthreads();
+  if (ks == 0) {
+#pragma unroll
+    for (int s = 0; s < DN_KSPLIT - 1; ++s) {
+      const float *src = red + (s * DN_ROWS + 2 * rp) * NOLSM_BS;
+#pragma unroll
+      for (int q = 0; q < 2; ++q)
+#pragma unroll
+        for (int p = 0; p < NOLSM_BS; ++p) acc[q][p] += src[q * NOLSM_BS + p];
+    }
+  }
+}
+
+// acc[q][p] += sum_k A(r + q, k) in(k, p) over k0 <= k < k1: A column by column through load(offset) (rows r, r + 1 as
+// one aligned pair, coalesced), row k of the staged thin operand as three broadcast 8-byte loads
+template <typename LoadPair>
+__device__ __forceinline__ void thin_mac(const float *s_in, int k0, int k1, int ld, int r, LoadPair load,
+                                         float (&acc)[2][NOLSM_BS]) {
+#pragma unroll 8
+  for (int k = k0; k < k1; ++k) {
+    const float2 xv = load((int64_t)k * ld + r);
+    const float2 *sk = reinterpret_cast<const float2 *>(s_in + k * NOLSM_BS);
+    const float2 s0 = sk[0], s1 = sk[1], s2 = sk[2];
+    acc[0][0] = fmaf(xv.x, s0.x, acc[0][0]); acc[0][1] = fmaf(xv.x, s0.y, acc[0][1]);
+    acc[0][2] = fmaf(xv.x, s1.x, acc[0][2]); acc[0][3] = fmaf(xv.x, s1.y, acc[0][3]);
+    acc[0][4] = fmaf(xv.x, s2.x, acc[0][4]); acc[0][5] = fmaf(xv.x, s2.y, acc[0][5]);
+    acc[1][0] = fmaf(xv.y, s0.x, acc[1][0]); acc[1][1] = fmaf(xv.y, s0.y, acc[1][1]);
+    acc[1][2] = fmaf(xv.y, s1.x, acc[1][2]); acc[1][3] = fmaf(xv.y, s1.y, acc[1][3]);
+    acc[1][4] = fmaf(xv.y, s2.x, acc[1][4]); acc[1][5] = fmaf(xv.y, s2.y, acc[1][5]);
+  }
+}
 
 template <bool kSplit>
 __global__ void __launch_bounds__(DN_THREADS)
@@ -514,20 +586,15 @@ k_density(const int32_t *__restrict__ row_ptr, const int32_t *__restrict__ col_i
           const float *__restrict__ u_thin, const __half *__restrict__ e_hi, const __half *__restrict__ e_lo,
           float *__restrict__ d_val, double *__restrict__ ne_diag) {
   // [n][6], row k contiguous: the six own columns V of S^-1, or (u_thin set: last iteration folded in,
-  // see k_last_half) U = V + 1/2 E V, so that X U = X_{k+1} V
+  // see k_last_half) U = V + 1/2 E V, so that X U = X_{k+1} V; then the slice sums
   extern __shared__ __align__(16) float s_sinv[];
   const int mat = blockIdx.y;
   const int j = mol_begin + mat;
   const int lo = row_ptr[j];
   const int m = row_ptr[j + 1] - lo;
   const int n = m * NOLSM_BS;
-  // position of j in its own (sorted) neighbour list
-  int l = 0, r_ = m;
-  while (l < r_) {
-    const int mid = (l + r_) >> 1;
-    if (col_idx[lo + mid] < j) l = mid + 1; else r_ = mid;
-  }
-  const int own0 = l * NOLSM_BS;
+  if ((int)blockIdx.x * DN_ROWS >= n) return;
+  const int own0 = own_position(col_idx, lo, m, j) * NOLSM_BS;
   XMat<kSplit> xj;
   if constexpr (kSplit) {
     xj.hi = ((iters[mat] & 1) ? xr.hi1 : xr.hi0) + (int64_t)mat * slab;
@@ -541,89 +608,55 @@ k_density(const int32_t *__restrict__ row_ptr, const int32_t *__restrict__ col_i
     const int p = t / n, k = t - p * n;
     s_sinv[k * NOLSM_BS + p] = uj ? uj[(int64_t)p * ld + k] : sj[(int64_t)(own0 + p) * ld + k];
   }
+  float *red = s_sinv + NOLSM_BS * n;
   __syncthreads();
-  const int r = blockIdx.x * DN_THREADS + threadIdx.x;
-  if (r < n) {
-    float acc[NOLSM_BS];
+  const int ks = threadIdx.x / (DN_THREADS / DN_KSPLIT);
+  const int rp = threadIdx.x % (DN_THREADS / DN_KSPLIT);
+  const int r = blockIdx.x * DN_ROWS + 2 * rp;
+  const int klen = (n + DN_KSPLIT - 1) / DN_KSPLIT;
+  const int k0 = ks * klen, k1 = min(n, k0 + klen);
+  const bool live = r < n;
+  float acc[2][NOLSM_BS];
 #pragma unroll
-    for (int p = 0; p < NOLSM_BS; ++p) acc[p] = 0.f;
-#pragma unroll 8
-    for (int k = 0; k < n; ++k) {   // X column by column (coalesced); S^-1 row k as three broadcast 8-byte loads
-      const float xv = xj.at((int64_t)k * ld + r);
-      const float2 *sk = reinterpret_cast<const float2 *>(s_sinv + k * NOLSM_BS);
-      const float2 s0 = sk[0], s1 = sk[1], s2 = sk[2];
-      acc[0] = fmaf(xv, s0.x, acc[0]); acc[1] = fmaf(xv, s0.y, acc[1]); acc[2] = fmaf(xv, s1.x, acc[2]);
-      acc[3] = fmaf(xv, s1.y, acc[3]); acc[4] = fmaf(xv, s2.x, acc[4]); acc[5] = fmaf(xv, s2.y, acc[5]);
-    }
-    float *out = d_val + ((int64_t)lo * 36 + (int64_t)r * NOLSM_BS);
-#pragma unroll
-    for (int p = 0; p < NOLSM_BS; ++p) {
-      const float v = uj ? sj[(int64_t)(own0 + p) * ld + r] : s_sinv[r * NOLSM_BS + p];
-      out[p] = 0.5f * (v - acc[p]);
-    }
-    if (ne_diag != nullptr && r >= own0 && r < own0 + NOLSM_BS) {
-      float xrr = xj.at((int64_t)r * ld + r);
-      if (uj) {   // diagonal element of X_{k+1} = X_k + 1/2 X_k E_k
-        const int64_t eoff = (int64_t)mat * slab + (int64_t)r * ld;
-        float dot = 0.f;
-        for (int k = 0; k < n; ++k) {
-          float e = __half2float(e_hi[eoff + k]);
-          if (e_lo) e = fmaf(__half2float(e_lo[eoff + k]), 1.f / 2048.f, e);
-          dot = fmaf(xj.at((int64_t)k * ld + r), e, dot);
+  for (int p = 0; p < NOLSM_BS; ++p) acc[0][p] = acc[1][p] = 0.f;
+  if (live) thin_mac(s_sinv, k0, k1, ld, r, [&](int64_t off) { return xj.at2(off); }, acc);
+  if (live && ne_diag != nullptr && r >= own0 && r < own0 + NOLSM_BS) {
+    // electron count: 1 - X_rr of the own rows; with the last iteration folded in, the diagonal of
+    // X_{k+1} = X_k + 1/2 X_k E_k, this thread's k slice of the two dot products
+    float part = 0.f;
+    if (ks == 0) part = 2.f - xj.at((int64_t)r * ld + r) - xj.at((int64_t)(r + 1) * ld + r + 1);
+    if (uj) {
+      const int64_t eoff = (int64_t)mat * slab + (int64_t)r * ld;
+      float dot = 0.f;
+      for (int k = k0; k < k1; ++k) {
+        float ea = __half2float(e_hi[eoff + k]), eb = __half2float(e_hi[eoff + ld + k]);
+        if (e_lo) {
+          ea = fmaf(__half2float(e_lo[eoff + k]), 1.f / 2048.f, ea);
+          eb = fmaf(__half2float(e_lo[eoff + ld + k]), 1.f / 2048.f, eb);
         }
-        xrr = fmaf(0.5f, dot, xrr);
+        const float2 xv = xj.at2((int64_t)k * ld + r);
+        dot = fmaf(xv.x, ea, dot);
+        dot = fmaf(xv.y, eb, dot);
       }
-      atomicAdd(ne_diag, (double)(1.f - xrr));
+      part = fmaf(-0.5f, dot, part);
     }
+    atomicAdd(ne_diag, (double)part);
   }
-}
-
-// Last sign iteration folded into a5 (reading 9): with E_k = I - X_k^2 already formed and passing the
-// stop test, X_{k+1} = X_k + 1/2 X_k E_k is only ever applied to the six own columns V of S^-1, and
-// X_{k+1} V = X_k (V + 1/2 E_k V).  This kernel forms U = V + 1/2 E_k V (thread = row, E_k column by column,
-// coalesced FP16 loads, V in shared memory); k_density then multiplies X_k with U instead of V.  Two n^2 x 6
-// products replace the n^3 product that would finish the iteration.  u_out: [count][6][ld].
-__global__ void __launch_bounds__(DN_THREADS)
-k_last_half(const int32_t *__restrict__ row_ptr, const int32_t *__restrict__ col_idx, int mol_begin, int ld,
-            int64_t slab, const __half *__restrict__ e_hi, const __half *__restrict__ e_lo,
-            const float *__restrict__ sinv, float *__restrict__ u_out) {
-  extern __shared__ __align__(16) float s_v[];  // [n][6]
-  const int mat = blockIdx.y;
-  const int j = mol_begin + mat;
-  const int lo = row_ptr[j];
-  const int m = row_ptr[j + 1] - lo;
-  const int n = m * NOLSM_BS;
-  int l = 0, r_ = m;
-  while (l < r_) {
-    const int mid = (l + r_) >> 1;
-    if (col_idx[lo + mid] < j) l = mid + 1; else r_ = mid;
-  }
-  const int own0 = l * NOLSM_BS;
-  const float *sj = sinv + (int64_t)mat * slab;
-  for (int t = threadIdx.x; t < NOLSM_BS * n; t += blockDim.x) {
-    const int p = t / n, k = t - p * n;
-    s_v[k * NOLSM_BS + p] = sj[(int64_t)(own0 + p) * ld + k];
-  }
-  __syncthreads();
-  const int r = blockIdx.x * DN_THREADS + threadIdx.x;
-  if (r < n) {
-    const __half *eh = e_hi + (int64_t)mat * slab + r;
-    const __half *el = e_lo ? e_lo + (int64_t)mat * slab + r : nullptr;
-    float acc[NOLSM_BS];
+  slice_reduce(red, ks, rp, acc);
+  if (live && ks == 0) {
+    float o[2 * NOLSM_BS];
 #pragma unroll
-    for (int p = 0; p < NOLSM_BS; ++p) acc[p] = 0.f;
-#pragma unroll 8
-    for (int c = 0; c < n; ++c) {
-      float e = __half2float(eh[(int64_t)c * ld]);
-      if (el) e = fmaf(__half2float(el[(int64_t)c * ld]), 1.f / 2048.f, e);
-      const float2 *vk = reinterpret_cast<const float2 *>(s_v + c * NOLSM_BS);
-      const float2 v0 = vk[0], v1 = vk[1], v2 = vk[2];
-      acc[0] = fmaf(e, v0.x, acc[0]); acc[1] = fmaf(e, v0.y, acc[1]); acc[2] = fmaf(e, v1.x, acc[2]);
-      acc[3] = fmaf(e, v1.y, acc[3]); acc[4] = fmaf(e, v2.x, acc[4]); acc[5] = fmaf(e, v2.y, acc[5]);
-    }
-    float *uj = u_out + (int64_t)mat * NOLSM_BS * ld;
+    for (int q = 0; q < 2; ++q)
 #pragma unroll
-    for (int p = 0; p < NOLSM_BS; ++p) uj[(int64_t)p * ld + r] = fmaf(0.5f, acc[p], s_v[r * NOLSM_BS + p]);
+      for (int p = 0; p < NOLSM_BS; ++p) {
+        const float v = uj ? sj[(int64_t)(own0 + p) * ld + r + q] : s_sinv[(r + q) * NOLSM_BS + p];
+        o[q * NOLSM_BS + p] = 0.5f * (v - acc[q][p]);
+      }
+    // rows r, r + 1 of the [n][6] block column: 12 consecutive floats, 48-byte aligned (r even)
+    float4 *out = reinterpret_cast<float4 *>(d_val + ((int64_t)lo * 36 + (int64_t)r * NOLSM_BS));
+    out[0] = make_float4(o[0], o[1], o[2], o[3]);
+    out[1] = make_float4(o[4], o[5], o[6], o[7]);
+    out[2] = make_float4(o[8], o[9], o[10], o[11]);
   }
 }
 
@@ -688,24 +721,18 @@ cudaError_t launch_density(const nolsm_batch *b, const XRef &x, const float *sin
                            double *ne_diag, const __half *e_hi, const __half *e_lo, float *u_thin,
                            cudaStream_t st) {
   if (b->count == 0) return cudaSuccess;
-  const size_t smem = (size_t)NOLSM_BS * b->max_n * sizeof(float);
+  if (x.hi0)   // split iterate of the tensor-core engine: thin_kernels.cu
+    return launch_density_split(b, x, sinv, row_ptr, col_idx, d_val, ne_diag, e_hi, e_lo, u_thin, st);
+  if (u_thin) return cudaErrorInvalidValue;   // a pending last iteration only exists on the split iterate
+  const size_t smem = ((size_t)NOLSM_BS * b->max_n + DN_RED_FLOATS) * sizeof(float);
   if (smem > 200 * 1024) return cudaErrorInvalidValue;   // six columns of one submatrix must fit in shared memory
   if (smem > 48 * 1024) {   // per device and cheap: set on every such launch (a process may use several devices)
     cudaError_t e = cudaFuncSetAttribute(k_density<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_density<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_last_half, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
   }
-  dim3 grid((b->max_n + DN_THREADS - 1) / DN_THREADS, b->count);
-  if (u_thin)   // the last iteration is pending (e_hi [+ e_lo] = E_k): U = V + 1/2 E_k V first
-    k_last_half<<<grid, DN_THREADS, smem, st>>>(row_ptr, col_idx, b->mol_begin, b->ld, (int64_t)b->ld * b->ld,
-                                                e_hi, e_lo, sinv, u_thin);
-  if (x.hi0)
-    k_density<true><<<grid, DN_THREADS, smem, st>>>(row_ptr, col_idx, b->mol_begin, b->ld, (int64_t)b->ld * b->ld, x,
-                                                    b->d_iters, sinv, u_thin, e_hi, e_lo, d_val, ne_diag);
-  else
-    k_density<false><<<grid, DN_THREADS, smem, st>>>(row_ptr, col_idx, b->mol_begin, b->ld, (int64_t)b->ld * b->ld, x,
-                                                     b->d_iters, sinv, u_thin, e_hi, e_lo, d_val, ne_diag);
+  dim3 grid((b->max_n + DN_ROWS - 1) / DN_ROWS, b->count);
+  k_density<false><<<grid, DN_THREADS, smem, st>>>(row_ptr, col_idx, b->mol_begin, b->ld, (int64_t)b->ld * b->ld, x,
+                                                   b->d_iters, sinv, nullptr, nullptr, nullptr, d_val, ne_diag);
   return cudaGetLastError();
 }
 

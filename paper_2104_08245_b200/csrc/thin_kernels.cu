@@ -1,0 +1,291 @@
+// Thin products of the hot path: C = A V with A a dense n x n submatrix held as FP16 planes (hi [+ lo * 2^-11], the
+// split form of DESIGN.md reading 12) and V its n x 6 "own" operand.  They are bound by reading A once from HBM
+// (DESIGN.md 5.2); on the FP32 pipe the 6 FMAs per element plus conversions exhaust the issue slots at about half of
+// the HBM rate, so the contraction itself runs on mma.sync (m16n8k16, FP16 operands, FP32 accumulate) -- a thin GEMM
+// where the tensor core only takes the arithmetic out of the way of the loads; tcgen05/TMEM would add nothing at 6
+// columns.
+//
+//   a5            D[:, own] = 1/2 (V - X V),  V = S^-1[:, own]            kDensity
+//   a4 last iteration folded into a5   U = V + 1/2 E V  (reading 9)                  kLastHalf
+//   a2 refinement of the own columns   T = I[:, own] - S V0,  V1 = V0 + A0 T  (reading 11)     kOwnResid, kOwnCorrect
+//
+// Orientation: C^T = V^T A^T, i.e. the MMA's M side (16) carries the six columns of V twice -- rows 0..5 its FP16 hi
+// part, rows 8..13 its lo part * 2^11 -- and the N side (8) rows of A.  A thread loads 16 contiguous bytes (8 rows) of
+// four columns k of A (a warp instruction: 4 x 128 contiguous bytes) and pairs the halves of two columns with one
+// PRMT into the B fragment of the row's tile; no shared-memory staging of A.  One accumulator tile holds
+// c0,c1 = A_hi V_hi and c2,c3 = A_hi V_lo + A_lo V_hi (the second MMA feeds V_hi into rows 8..13), so that
+// C = c01 + c23 * 2^-11 has the 22 bits of both operands.
+#include "common.cuh"
+
+namespace {
+
+constexpr int kThinThreads = 256;
+constexpr int kThinRows = 128;     // rows of A per CTA: 2 warps x 64 rows
+constexpr int kThinSlices = 4;     // k slices per CTA, summed through shared memory in a fixed order (run-to-run bitwise equal)
+
+enum ThinMode { kDensity = 0, kLastHalf = 1, kOwnResid = 2, kOwnCorrect = 3 };
+
+struct ThinArgs {
+  const int32_t *row_ptr, *col_idx;
+  int mol_begin, ld;
+  int64_t slab;
+  const __half *a_hi[2], *a_lo[2];   // planes of A by the parity of iters[mat] (iters null: [0]); a_lo null: FP16 A
+  const int32_t *iters;
+  const float *sinv;                 // FP32 S^-1 (own columns valid), [count][slab]
+  const __half *a0;                  // kOwnResid / kOwnCorrect: FP16 approximate inverse
+  float *thin;                       // [count][6][ld]: U (kLastHalf out, kDensity in when folded), T (kOwnResid out, kOwnCorrect in)
+  int folded;                        // kDensity: V is U from thin, the diagonal gets the pending half iteration
+  const __half *e_hi, *e_lo;         // kDensity, folded: E_k for the diagonal
+  float *d_val;                      // kDensity: column-owned block store
+  double *ne_diag;                   // kDensity: sum of 1 - X_rr over the own rows, or null
+  float *out32;                      // kOwnCorrect: FP32 S^-1, own columns written
+};
+
+__device__ __forceinline__ uint32_t pack_half2(float a, float b) {
+  const __half2 h = __floats2half2_rn(a, b);
+  return *reinterpret_cast<const uint32_t *>(&h);
+}
+__device__ __forceinline__ void mma16816(float (&c)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, uint32_t b0,
+                                         uint32_t b1) {
+  asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+               : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
+               : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
+}
+// eight rows (16 bytes) of column k of a plane, zero beyond column n
+__device__ __forceinline__ uint4 load_rows8(const __half *plane, int64_t off, bool ok) {
+  return ok ? __ldg(reinterpret_cast<const uint4 *>(plane + off)) : make_uint4(0u, 0u, 0u, 0u);
+}
+__device__ __forceinline__ float split_at(const __half *hi, const __half *lo, int64_t off) {
+  float v = __half2float(hi[off]);
+  if (lo) v = fmaf(__half2float(lo[off]), 1.f / 2048.f, v);
+  return v;
+}
+
+// the eight row tiles of one 16-column step: q[j] = 8 rows of columns k0 + 2t + {0, 1, 8, 9}
+template <bool kLoPlane>
+__device__ __forceinline__ void step_mma(float (&acc)[8][4], const uint4 (&q)[4], const uint4 &f) {
+  const uint32_t w0[4] = {q[0].x, q[0].y, q[0].z, q[0].w}, w1[4] = {q[1].x, q[1].y, q[1].z, q[1].w};
+  const uint32_t w2[4] = {q[2].x, q[2].y, q[2].z, q[2].w}, w3[4] = {q[3].x, q[3].y, q[3].z, q[3].w};
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
+    const uint32_t sel = (i & 1) ? 0x7632u : 0x5410u;
+    const uint32_t b0 = __byte_perm(w0[i >> 1], w1[i >> 1], sel), b1 = __byte_perm(w2[i >> 1], w3[i >> 1], sel);
+    if constexpr (kLoPlane) mma16816(acc[i], 0u, f.x, 0u, f.z, b0, b1);   // V_hi in rows 8..13: A_lo V_hi joins A_hi V_lo
+    else mma16816(acc[i], f.x, f.y, f.z, f.w, b0, b1);
+  }
+}
+
+template <int kMode>
+__global__ void __launch_bounds__(kThinThreads, 2) k_thin_mma(const ThinArgs a) {
+  extern __shared__ __align__(16) uint8_t smem_raw[];
+  const int mat = blockIdx.y;
+  const int j = a.mol_begin + mat;
+  const int lo = a.row_ptr[j];
+  const int m = a.row_ptr[j + 1] - lo;
+  const int n = m * NOLSM_BS;
+  if ((int)blockIdx.x * kThinRows >= n) return;
+  int own0;
+  {
+    int l = 0, r_ = m;
+    while (l < r_) {   // position of j in its own (sorted) neighbour list
+      const int mid = (l + r_) >> 1;
+      if (a.col_idx[lo + mid] < j) l = mid + 1; else r_ = mid;
+    }
+    own0 = l * NOLSM_BS;
+  }
+  const int ld = a.ld;
+  const int nkb = (n + 15) >> 4;                              // 16-column steps
+  uint4 *s_frag = reinterpret_cast<uint4 *>(smem_raw);        // [nkb][6][4]: A fragments of the stacked V^T
+  float *s_red = reinterpret_cast<float *>(s_frag + (size_t)nkb * 24);   // [kThinSlices][kThinRows][6]
+  const int par = a.iters ? (a.iters[mat] & 1) : 0;
+  const __half *ahi = a.a_hi[par] + (int64_t)mat * a.slab;
+  const __half *alo = a.a_lo[par] ? a.a_lo[par] + (int64_t)mat * a.slab : nullptr;
+  const float *sj = a.sinv ? a.sinv + (int64_t)mat * a.slab : nullptr;
+  const __half *a0j = a.a0 ? a.a0 + (int64_t)mat * a.slab : nullptr;
+  float *tj = a.thin ? a.thin + (int64_t)mat * NOLSM_BS * ld : nullptr;
+  // element (k, p) of the thin operand
+  auto vsrc = [&](int k, int p) -> float {
+    if (k >= n) return 0.f;
+    if constexpr (kMode == kDensity) return a.folded ? tj[(int64_t)p * ld + k] : sj[(int64_t)(own0 + p) * ld + k];
+    else if constexpr (kMode == kLastHalf) return sj[(int64_t)(own0 + p) * ld + k];
+    else if constexpr (kMode == kOwnResid) return __half2float(a0j[(int64_t)(own0 + p) * ld + k]);
+    else return tj[(int64_t)p * ld + k];
+  };
+  for (int i = threadIdx.x; i < nkb * 24; i += kThinThreads) {
+    const int t = i & 3, kb = (i >> 2) % nkb, p = (i >> 2) / nkb;
+    const int k = kb * 16 + 2 * t;
+    const float v[4] = {vsrc(k, p), vsrc(k + 1, p), vsrc(k + 8, p), vsrc(k + 9, p)};
+    float l[4];
+#pragma unroll
+    for (int e = 0; e < 4; ++e) l[e] = (v[e] - __half2float(__float2half_rn(v[e]))) * 2048.f;
+    s_frag[(kb * 6 + p) * 4 + t] = make_uint4(pack_half2(v[0], v[1]), pack_half2(l[0], l[1]), pack_half2(v[2], v[3]),
+                                               pack_half2(l[2], l[3]));
+  }
+  __syncthreads();
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int g = lane >> 2, t = lane & 3;
+  const int rw = (warp & 1) * 64;                 // this warp's rows inside the CTA
+  const int ks = warp >> 1;
+  const int per = (nkb + kThinSlices - 1) / kThinSlices;
+  const int kb0 = ks * per, kb1 = min(nkb, kb0 + per);
+  const int r0 = blockIdx.x * kThinRows + rw;
+  float acc[8][4];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) acc[i][0] = acc[i][1] = acc[i][2] = acc[i][3] = 0.f;
+  if (r0 < n && kb0 < kb1) {   // (else: this warp's part of s_red stays zero, written below)
+    const int64_t rowoff = r0 + 8 * g;
+    uint4 qh[2][4], ql[2][4];
+    auto fetch = [&](int kb, uint4 (&h)[4], uint4 (&l)[4]) {
+      const int k = kb * 16 + 2 * t;
+      const int kk[4] = {k, k + 1, k + 8, k + 9};
+#pragma unroll
+      for (int e = 0; e < 4; ++e) {
+        const int64_t off = (int64_t)kk[e] * ld + rowoff;
+        h[e] = load_rows8(ahi, off, kk[e] < n);
+        if (alo) l[e] = load_rows8(alo, off, kk[e] < n);
+      }
+    };
+    fetch(kb0, qh[0], ql[0]);
+    for (int kb = kb0; kb < kb1; kb += 2) {
+      if (kb + 1 < kb1) fetch(kb + 1, qh[1], ql[1]);
+      uint4 f = make_uint4(0u, 0u, 0u, 0u);
+      if (g < NOLSM_BS) f = s_frag[(kb * 6 + g) * 4 + t];
+      step_mma<false>(acc, qh[0], f);
+      if (alo) step_mma<true>(acc, ql[0], f);
+      if (kb + 1 < kb1) {
+        if (kb + 2 < kb1) fetch(kb + 2, qh[0], ql[0]);
+        f = make_uint4(0u, 0u, 0u, 0u);
+        if (g < NOLSM_BS) f = s_frag[((kb + 1) * 6 + g) * 4 + t];
+        step_mma<false>(acc, qh[1], f);
+        if (alo) step_mma<true>(acc, ql[1], f);
+      }
+    }
+  }
+  if (g < NOLSM_BS) {   // C^T rows 0..5 (hi) and 8..13 (lo * 2^11) of column p = g; tile i holds rows r0 + 8 n + i
+    float *red = s_red + (size_t)ks * kThinRows * NOLSM_BS;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      red[(rw + 16 * t + i) * NOLSM_BS + g] = fmaf(acc[i][2], 1.f / 2048.f, acc[i][0]);
+      red[(rw + 16 * t + 8 + i) * NOLSM_BS + g] = fmaf(acc[i][3], 1.f / 2048.f, acc[i][1]);
+    }
+  }
+  __syncthreads();
+  auto total = [&](int i) {   // i = row * 6 + p
+    float c = s_red[i];
+#pragma unroll
+    for (int sl = 1; sl < kThinSlices; ++sl) c += s_red[sl * kThinRows * NOLSM_BS + i];
+    return c;
+  };
+
+  const int rb = blockIdx.x * kThinRows;
+  if constexpr (kMode == kDensity) {
+    // [n][6] block column of D: rows contiguous, six floats each
+    for (int i = threadIdx.x; i < kThinRows * NOLSM_BS; i += kThinThreads) {
+      const int rr = i / NOLSM_BS, p = i - rr * NOLSM_BS;
+      if (rb + rr < n)
+        a.d_val[(int64_t)lo * 36 + (int64_t)(rb + rr) * NOLSM_BS + p] = 0.5f * (sj[(int64_t)(own0 + p) * ld + rb + rr] - total(i));
+    }
+    if (a.ne_diag != nullptr && blockIdx.x == 0 && warp < NOLSM_BS) {
+      // electron count: 1 - X_rr over the own rows; folded: the diagonal of X_{k+1} = X_k + 1/2 X_k E_k
+      const int r = own0 + warp;
+      float dot = 0.f;
+      if (a.folded) {
+        const int64_t eoff = (int64_t)mat * a.slab + (int64_t)r * ld;
+        for (int k = lane; k < n; k += 32)
+          dot = fmaf(split_at(ahi, alo, (int64_t)k * ld + r), split_at(a.e_hi + eoff, a.e_lo ? a.e_lo + eoff : nullptr, k), dot);
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) dot += __shfl_xor_sync(0xffffffffu, dot, d);
+      }
+      if (lane == 0) atomicAdd(a.ne_diag, (double)(1.f - fmaf(0.5f, dot, split_at(ahi, alo, (int64_t)r * ld + r))));
+    }
+  } else {
+    for (int i = threadIdx.x; i < kThinRows * NOLSM_BS; i += kThinThreads) {
+      const int p = i / kThinRows, rr = i - p * kThinRows;
+      const int r = rb + rr;
+      if (r >= n) continue;
+      const float c = total(rr * NOLSM_BS + p);
+      if constexpr (kMode == kLastHalf) tj[(int64_t)p * ld + r] = fmaf(0.5f, c, sj[(int64_t)(own0 + p) * ld + r]);
+      else if constexpr (kMode == kOwnResid) tj[(int64_t)p * ld + r] = (r == own0 + p ? 1.f : 0.f) - c;
+      else a.out32[(int64_t)mat * a.slab + (int64_t)(own0 + p) * ld + r] = __half2float(a0j[(int64_t)(own0 + p) * ld + r]) + c;
+    }
+  }
+}
+
+template <int kMode>
+cudaError_t thin_launch(const nolsm_batch *b, const ThinArgs &a, cudaStream_t st) {
+  const int nkb = (b->max_n + 15) / 16;
+  const size_t smem = (size_t)nkb * 24 * sizeof(uint4) + (size_t)kThinSlices * kThinRows * NOLSM_BS * sizeof(float);
+  if (smem > 200 * 1024) return cudaErrorInvalidValue;   // the thin operand of one submatrix must fit in shared memory
+  if (smem > 48 * 1024) {   // per device and cheap: set on every such launch (a process may use several devices)
+    cudaError_t e = cudaFuncSetAttribute(k_thin_mma<kMode>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+  }
+  dim3 grid((b->max_n + kThinRows - 1) / kThinRows, b->count);
+  k_thin_mma<kMode><<<grid, kThinThreads, smem, st>>>(a);
+  return cudaGetLastError();
+}
+
+ThinArgs base_args(const nolsm_batch *b, const int32_t *row_ptr, const int32_t *col_idx) {
+  ThinArgs a;
+  memset(&a, 0, sizeof(a));
+  a.row_ptr = row_ptr;
+  a.col_idx = col_idx;
+  a.mol_begin = b->mol_begin;
+  a.ld = b->ld;
+  a.slab = (int64_t)b->ld * b->ld;
+  return a;
+}
+
+}  // namespace
+
+// a5 on a split iterate (x.hi0 set).  u_thin set: the last iteration is pending (e_hi [+ e_lo] = E_k): U = V + 1/2 E_k V
+// first, then D[:, own] = 1/2 (V - X_k U).
+cudaError_t launch_density_split(const nolsm_batch *b, const XRef &x, const float *sinv, const int32_t *row_ptr,
+                                 const int32_t *col_idx, float *d_val, double *ne_diag, const __half *e_hi,
+                                 const __half *e_lo, float *u_thin, cudaStream_t st) {
+  if (b->count == 0) return cudaSuccess;
+  if (u_thin) {
+    ThinArgs h = base_args(b, row_ptr, col_idx);
+    h.a_hi[0] = h.a_hi[1] = e_hi;
+    h.a_lo[0] = h.a_lo[1] = e_lo;
+    h.sinv = sinv;
+    h.thin = u_thin;
+    cudaError_t e = thin_launch<kLastHalf>(b, h, st);
+    if (e != cudaSuccess) return e;
+  }
+  ThinArgs a = base_args(b, row_ptr, col_idx);
+  a.a_hi[0] = x.hi0; a.a_hi[1] = x.hi1;
+  a.a_lo[0] = x.lo0; a.a_lo[1] = x.lo1;
+  a.iters = b->d_iters;
+  a.sinv = sinv;
+  a.thin = u_thin;
+  a.folded = u_thin ? 1 : 0;
+  a.e_hi = e_hi;
+  a.e_lo = e_lo;
+  a.d_val = d_val;
+  a.ne_diag = ne_diag;
+  return thin_launch<kDensity>(b, a, st);
+}
+
+// Newton refinement of the six own columns of S^-1 alone (reading 11, own-columns form): with A0 the
+// FP16-quality inverse of the Eq. 15-17 iteration and V0 = A0[:, own],  V1 = V0 + A0 (I[:, own] - S V0); the error
+// (I - A0 S)(V - V0) is of second order whatever the rounding of A0, as long as both uses read the same A0.
+// s_hi, s_lo: split S; thin: scratch of count * 6 * ld floats; out32: FP32 S^-1, its own columns are written.
+cudaError_t launch_own_refine(const nolsm_batch *b, const int32_t *row_ptr, const int32_t *col_idx, const __half *s_hi,
+                              const __half *s_lo, const __half *a0, float *thin, float *out32, cudaStream_t st) {
+  if (b->count == 0) return cudaSuccess;
+  ThinArgs r = base_args(b, row_ptr, col_idx);
+  r.a_hi[0] = r.a_hi[1] = s_hi;
+  r.a_lo[0] = r.a_lo[1] = s_lo;
+  r.a0 = a0;
+  r.thin = thin;
+  cudaError_t e = thin_launch<kOwnResid>(b, r, st);
+  if (e != cudaSuccess) return e;
+  ThinArgs c = base_args(b, row_ptr, col_idx);
+  c.a_hi[0] = c.a_hi[1] = a0;
+  c.a0 = a0;
+  c.thin = thin;
+  c.out32 = out32;
+  return thin_launch<kOwnCorrect>(b, c, st);
+}
