@@ -559,9 +559,9 @@ static nolsm_status prepare_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, int prec
   const bool fp16 = precision == NOLSM_FP16_FP32;
   const int refine = ctx->cfg.inv_refine >= 0 ? ctx->cfg.inv_refine : (fp16 ? 1 : 0);
   // one refinement, FP16 mode, one owner per submatrix: B1 = B0 + A0 (H - S B0) with B0 = A0 H and A0 = Z^2/s_S the
-  // FP16-quality inverse -- the same second-order error (I - A0 S)^2 S^-1 H as refining S^-1 first, in five MMAs
-  // (1 + 3 + 1) instead of seven (3 + 1 for the refinement, 3 for B on split operands); the own columns of S^-1
-  // get their refinement as two thin products (k_own_refine)
+  // FP16-quality inverse -- the same second-order error (I - A0 S)^2 S^-1 H as refining S^-1 first, in four MMAs
+  // (1 + 2 + 1) instead of seven (3 + 1 for the refinement, 3 for B on split operands); the own columns of S^-1
+  // get their refinement as two thin products (launch_own_refine)
   const bool fast_b = own_only && fp16 && refine == 1 && b->sparse && b->row_ptr != nullptr && !b->grouped;
   // 3e-3 with a refinement behind: the iterate is taken with a relative error of about twice its residual,
   // which the refinement squares (< 4e-5)
@@ -682,19 +682,26 @@ static nolsm_status prepare_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, int prec
   if (refine > 0 && !b->s_split_built)           // batch built under another configuration
     LAUNCH(ctx, launch_scale_copy(b, S, nullptr, 0, nullptr, b->h[ss_hi], b->h[ss_lo], st));
   if (fast_b) {
-    // A0: h0.  B0 = A0 H (plain FP16 operands) -> split pair (h1, h4);  R = H - S B0 on split operands -> h5;
-    // B1 = B0 + A0 R -> u3.  Z (h2 / h3) is not read any more.
+    // A0: h0.  B0 = fp16(A0 H) -> h1 (whatever B0 is, the refinement only needs the SAME B0 in both places, so the
+    // FP16 result is B0 and no lo part exists);  R = H - S B0 with S split, B0 exact -> h5;  B1 = B0 + A0 R -> u3.
+    // Three launches: the plain products run on 256-row tiles, the half-split one on 128-row tiles.
     ChainProgram p5 = one_shot(g1);
-    p5.n_ops = 3;
+    p5.n_ops = 1;
     ChainOp &b0 = p5.ops[0] = make_op(EPI_AXPBY, 1.f, 0.f);
-    set2(b0.a, si_hi, si_hi); set2(b0.b, hs_hi, hs_hi); set2(b0.out16, 1, 1); set2(b0.out16_lo, 4, 4);
-    ChainOp &r = p5.ops[1] = make_op(EPI_AXPBY, -1.f, 1.f);
-    set2(r.a, ss_hi, ss_hi); set2(r.a_lo, ss_lo, ss_lo); set2(r.b, 1, 1); set2(r.b_lo, 4, 4);
-    set2(r.cin16, hs_hi, hs_hi); set2(r.cin16_lo, hs_lo, hs_lo); set2(r.out16, 5, 5);
-    ChainOp &b1 = p5.ops[2] = make_op(EPI_AXPBY, 1.f, 1.f);
-    set2(b1.a, si_hi, si_hi); set2(b1.b, 5, 5); set2(b1.cin16, 1, 1); set2(b1.cin16_lo, 4, 4);
-    b1.cout32 = 3;
+    set2(b0.a, si_hi, si_hi); set2(b0.b, hs_hi, hs_hi); set2(b0.out16, 1, 1);
     CHECK(run_chain(ctx, b, p5, nullptr, false, st));
+    ChainProgram p6 = one_shot(g1);
+    p6.n_ops = 1;
+    ChainOp &r = p6.ops[0] = make_op(EPI_AXPBY, -1.f, 1.f);
+    set2(r.a, ss_hi, ss_hi); set2(r.a_lo, ss_lo, ss_lo); set2(r.b, 1, 1);
+    set2(r.cin16, hs_hi, hs_hi); set2(r.cin16_lo, hs_lo, hs_lo); set2(r.out16, 5, 5);
+    CHECK(run_chain(ctx, b, p6, nullptr, false, st));
+    ChainProgram p7 = one_shot(g1);
+    p7.n_ops = 1;
+    ChainOp &b1 = p7.ops[0] = make_op(EPI_AXPBY, 1.f, 1.f);
+    set2(b1.a, si_hi, si_hi); set2(b1.b, 5, 5); set2(b1.cin16, 1, 1);
+    b1.cout32 = 3;
+    CHECK(run_chain(ctx, b, p7, nullptr, false, st));
     CHECK(ensure_thin(ctx, b, st));
     LAUNCH(ctx, launch_own_refine(b, b->row_ptr, b->col_idx, b->h[ss_hi], b->h[ss_lo], b->h[si_hi], b->d_thin, b->u[2], st));
     b->sinv_hi = b->sinv_lo = -1;

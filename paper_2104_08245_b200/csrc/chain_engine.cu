@@ -373,12 +373,17 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
         const int my_n = kPair ? (c.nt >> 1) : c.nt;          // this CTA's share of the tile's rows (N side)
         const int n0 = c.n0 + (kPair ? my_n * (int)rank : 0);
         const bool split = o.a_lo[par] >= 0;
+        // only the left operand split (the right one is exact in FP16): no lo part on the M side, and the lo
+        // boxes of the N side follow its hi boxes, so that one MMA can take both (see the issuer)
+        const bool half = split && o.b_lo[par] < 0;
         const int nbox = (my_n + 63) >> 6;
-        const uint32_t bytes = (uint32_t)kCtas * (uint32_t)(kATileBytes + nbox * kBoxBytes) * (split ? 2u : 1u);
+        const uint32_t bytes = (uint32_t)kCtas * (uint32_t)(kATileBytes * (split && !half ? 2 : 1) +
+                                                            nbox * kBoxBytes * (split ? 2 : 1));
         // M side <- right operand (K-major), N side <- left operand (MN-major)
         const CUtensorMap *ma = &args.maps[o.b[par]], *mb = &args.maps[o.a[par]];
-        const CUtensorMap *mal = split ? &args.maps[o.b_lo[par]] : nullptr;
+        const CUtensorMap *mal = split && !half ? &args.maps[o.b_lo[par]] : nullptr;
         const CUtensorMap *mbl = split ? &args.maps[o.a_lo[par]] : nullptr;
+        const int off_bl = half ? off_b + args.b_bytes : off_b_lo;
         const int kb_go = max(0, c.kblocks - kClaimLead);
         for (int kb = 0; kb < c.kblocks; ++kb) {
           if (leader && kb == kb_go) mbar_arrive<false>(&claim_go);   // the scheduler may claim the next tile
@@ -391,10 +396,12 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
           for (int j = 0; j < nbox; ++j)
             tma_load_3d<kPair>(st + off_b + j * kBoxBytes, mb, &full_bar[stage], n0 + 64 * j, k0, m);
           if (split) {
-            tma_load_3d<kPair>(st + off_a_lo, mal, &full_bar[stage], k0, m0, m);
-            tma_load_3d<kPair>(st + off_a_lo + kBoxBytes, mal, &full_bar[stage], k0, m0 + 64, m);
+            if (!half) {
+              tma_load_3d<kPair>(st + off_a_lo, mal, &full_bar[stage], k0, m0, m);
+              tma_load_3d<kPair>(st + off_a_lo + kBoxBytes, mal, &full_bar[stage], k0, m0 + 64, m);
+            }
             for (int j = 0; j < nbox; ++j)
-              tma_load_3d<kPair>(st + off_b_lo + j * kBoxBytes, mbl, &full_bar[stage], n0 + 64 * j, k0, m);
+              tma_load_3d<kPair>(st + off_bl + j * kBoxBytes, mbl, &full_bar[stage], n0 + 64 * j, k0, m);
           }
           if (++stage == args.stages) { stage = 0; phase ^= 1u; }
         }
@@ -419,8 +426,15 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
         if (++slot == kRing) { slot = 0; ring_phase ^= 1u; }
         if (c.op < 0) break;
         const bool split = pg.ops[c.op].a_lo[chainep::cmd_par(c)] >= 0;
+        const bool half = split && pg.ops[c.op].b_lo[chainep::cmd_par(c)] < 0;
+        // half split, one CTA, 128-row tiles: the lo boxes of the N side start exactly 128 rows behind the hi boxes,
+        // and the correction accumulator 128 columns behind the main one -- ONE MMA of N = 128 + nt forms
+        // [A_hi B_hi | A_hi B_lo] and reads the M-side tile once (columns nt..127 are never read back)
+        const bool stacked = half && !kPair && args.b_bytes == 2 * kBoxBytes;
         // instruction descriptor: D=F32, A=B=F16, A K-major, B MN-major, N = nt, M = 128 per CTA
         const uint32_t idesc = (1u << 4) | (1u << 16) | ((uint32_t)(c.nt >> 3) << 17) | ((uint32_t)(kTileM >> 4) << 24);
+        const uint32_t idesc_stacked =
+            (1u << 4) | (1u << 16) | ((uint32_t)((128 + c.nt) >> 3) << 17) | ((uint32_t)(kTileM >> 4) << 24);
         mbar_wait<kPair>(&tempty_bar[acc], acc_phase ^ 1u);
         tc_fence_after();
         const uint32_t d_main = tmem_base + (uint32_t)(acc * 256);
@@ -435,19 +449,21 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
           const uint32_t b_lo = (((sa + off_b) >> 4) & 0x3FFFu) | ((uint32_t)(kBoxBytes >> 4) << 16);
           const int steps = kb == c.kblocks - 1 ? c.ktail : kBK / 16;
           if (one) {
-            if (!split) {
-              tc_mma<kPair>(d_main, a_lo, b_lo, kDescHi, idesc, kb ? 1u : 0u);
-              if (steps > 1) tc_mma<kPair>(d_main, a_lo + 2u, b_lo + 128u, kDescHi, idesc, 1u);
-              if (steps > 2) tc_mma<kPair>(d_main, a_lo + 4u, b_lo + 256u, kDescHi, idesc, 1u);
-              if (steps > 3) tc_mma<kPair>(d_main, a_lo + 6u, b_lo + 384u, kDescHi, idesc, 1u);
+            if (!split || stacked) {
+              const uint32_t id = stacked ? idesc_stacked : idesc;
+              tc_mma<kPair>(d_main, a_lo, b_lo, kDescHi, id, kb ? 1u : 0u);
+              if (steps > 1) tc_mma<kPair>(d_main, a_lo + 2u, b_lo + 128u, kDescHi, id, 1u);
+              if (steps > 2) tc_mma<kPair>(d_main, a_lo + 4u, b_lo + 256u, kDescHi, id, 1u);
+              if (steps > 3) tc_mma<kPair>(d_main, a_lo + 6u, b_lo + 384u, kDescHi, id, 1u);
             } else {
               const uint32_t al_lo = (((sa + off_a_lo) >> 4) & 0x3FFFu) | (1u << 16);
-              const uint32_t bl_lo = (((sa + off_b_lo) >> 4) & 0x3FFFu) | ((uint32_t)(kBoxBytes >> 4) << 16);
+              const uint32_t bl_lo = (((sa + (half ? off_b + args.b_bytes : off_b_lo)) >> 4) & 0x3FFFu) |
+                                     ((uint32_t)(kBoxBytes >> 4) << 16);
               for (int k4 = 0; k4 < steps; ++k4) {
                 const uint32_t accum = (kb | k4) ? 1u : 0u;
                 tc_mma<kPair>(d_main, a_lo + 2u * k4, b_lo + 128u * k4, kDescHi, idesc, accum);
                 tc_mma<kPair>(d_corr, a_lo + 2u * k4, bl_lo + 128u * k4, kDescHi, idesc, accum);
-                tc_mma<kPair>(d_corr, al_lo + 2u * k4, b_lo + 128u * k4, kDescHi, idesc, 1u);
+                if (!half) tc_mma<kPair>(d_corr, al_lo + 2u * k4, b_lo + 128u * k4, kDescHi, idesc, 1u);
               }
             }
             tc_commit<kPair>(&empty_bar[stage]);
@@ -697,14 +713,17 @@ cudaError_t launch_chain(nolsm_ctx *ctx, const nolsm_batch *b, const ChainProgra
   ChainArgs a;
   memset(&a, 0, sizeof(a));
   a.prog = prog;
-  bool split = false;
-  for (int i = 0; i < prog.n_ops; ++i) split |= prog.ops[i].a_lo[0] >= 0 || prog.ops[i].a_lo[1] >= 0;
+  bool split = false, full_split = false;   // full: both operands split (lo tiles on both sides of a stage)
+  for (int i = 0; i < prog.n_ops; ++i) {
+    split |= prog.ops[i].a_lo[0] >= 0 || prog.ops[i].a_lo[1] >= 0;
+    full_split |= prog.ops[i].b_lo[0] >= 0 || prog.ops[i].b_lo[1] >= 0;
+  }
   const int col_round = pair ? 32 : 16;
   const int ncol_max = (b->max_n + col_round - 1) / col_round * col_round;
   const int tile_m = pair ? 2 * NOLSM_TILE_M : NOLSM_TILE_M;
   a.bn = std::min(split ? 128 : 256, ncol_max);
   a.b_bytes = (((pair ? a.bn >> 1 : a.bn) + 63) / 64) * kBoxBytes;
-  a.stage_bytes = (kATileBytes + a.b_bytes) * (split ? 2 : 1);
+  a.stage_bytes = full_split ? 2 * (kATileBytes + a.b_bytes) : kATileBytes + a.b_bytes * (split ? 2 : 1);
   a.stages = std::min(kMaxStages, (kSmemLimit - 1024 - chainep::kStagingBytes) / a.stage_bytes);
   a.mt = (b->max_n + tile_m - 1) / tile_m;
   a.ntl = (ncol_max + a.bn - 1) / a.bn;

@@ -53,6 +53,7 @@ struct GemmParams {
 struct ChainOp {
   int32_t a[2], b[2];             // FP16 operands (hi parts), by iteration parity
   int32_t a_lo[2], b_lo[2];       // lo parts of split operands (FP32-quality product), -1: plain FP16
+                                  // a_lo set, b_lo -1: only the left operand is split (the right one is exact in FP16)
   int32_t out16[2], out16_lo[2];  // FP16 copy of the result (hi [, lo * 2^11]), -1: none
   int32_t cin32, cout32;          // FP32 units read (AXPBY, beta != 0) / written, -1: none
   int32_t cin16[2];               // instead of cin32: the add-in is an FP16 buffer (by parity), -1: none.  For

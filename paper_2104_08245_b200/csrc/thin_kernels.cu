@@ -20,8 +20,10 @@
 namespace {
 
 constexpr int kThinThreads = 256;
-constexpr int kThinRows = 128;     // rows of A per CTA: 2 warps x 64 rows
-constexpr int kThinSlices = 4;     // k slices per CTA, summed through shared memory in a fixed order (run-to-run bitwise equal)
+constexpr int kThinRowWarps = 8;   // warps side by side along the rows of a row block
+constexpr int kThinRows = 64 * kThinRowWarps;   // rows of A per row block
+constexpr int kThinCtaRows = kThinRows;  // rows per CTA (row blocks one after the other: the staged thin operand serves both)
+constexpr int kThinSlices = 8 / kThinRowWarps;     // k slices per CTA, summed through shared memory in a fixed order (run-to-run bitwise equal)
 
 enum ThinMode { kDensity = 0, kLastHalf = 1, kOwnResid = 2, kOwnCorrect = 3 };
 
@@ -75,117 +77,173 @@ __device__ __forceinline__ void step_mma(float (&acc)[8][4], const uint4 (&q)[4]
   }
 }
 
-template <int kMode>
+template <int kMode, bool kLo>
 __global__ void __launch_bounds__(kThinThreads, 2) k_thin_mma(const ThinArgs a) {
+  // register stages of A in flight per thread: 16 bytes x 4 columns [x 2 planes] each
+  constexpr int kDepth = kLo ? 2 : 4;
   extern __shared__ __align__(16) uint8_t smem_raw[];
   const int mat = blockIdx.y;
   const int j = a.mol_begin + mat;
   const int lo = a.row_ptr[j];
   const int m = a.row_ptr[j + 1] - lo;
   const int n = m * NOLSM_BS;
-  if ((int)blockIdx.x * kThinRows >= n) return;
-  int own0;
-  {
-    int l = 0, r_ = m;
-    while (l < r_) {   // position of j in its own (sorted) neighbour list
-      const int mid = (l + r_) >> 1;
-      if (a.col_idx[lo + mid] < j) l = mid + 1; else r_ = mid;
-    }
-    own0 = l * NOLSM_BS;
-  }
+  if ((int)blockIdx.x * kThinCtaRows >= n) return;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int g = lane >> 2, t = lane & 3;
   const int ld = a.ld;
   const int nkb = (n + 15) >> 4;                              // 16-column steps
   uint4 *s_frag = reinterpret_cast<uint4 *>(smem_raw);        // [nkb][6][4]: A fragments of the stacked V^T
   float *s_red = reinterpret_cast<float *>(s_frag + (size_t)nkb * 24);   // [kThinSlices][kThinRows][6]
   const int par = a.iters ? (a.iters[mat] & 1) : 0;
   const __half *ahi = a.a_hi[par] + (int64_t)mat * a.slab;
-  const __half *alo = a.a_lo[par] ? a.a_lo[par] + (int64_t)mat * a.slab : nullptr;
+  const __half *alo = kLo ? a.a_lo[par] + (int64_t)mat * a.slab : nullptr;
   const float *sj = a.sinv ? a.sinv + (int64_t)mat * a.slab : nullptr;
   const __half *a0j = a.a0 ? a.a0 + (int64_t)mat * a.slab : nullptr;
   float *tj = a.thin ? a.thin + (int64_t)mat * NOLSM_BS * ld : nullptr;
-  // element (k, p) of the thin operand
-  auto vsrc = [&](int k, int p) -> float {
-    if (k >= n) return 0.f;
-    if constexpr (kMode == kDensity) return a.folded ? tj[(int64_t)p * ld + k] : sj[(int64_t)(own0 + p) * ld + k];
-    else if constexpr (kMode == kLastHalf) return sj[(int64_t)(own0 + p) * ld + k];
-    else if constexpr (kMode == kOwnResid) return __half2float(a0j[(int64_t)(own0 + p) * ld + k]);
-    else return tj[(int64_t)p * ld + k];
-  };
-  for (int i = threadIdx.x; i < nkb * 24; i += kThinThreads) {
-    const int t = i & 3, kb = (i >> 2) % nkb, p = (i >> 2) / nkb;
-    const int k = kb * 16 + 2 * t;
-    const float v[4] = {vsrc(k, p), vsrc(k + 1, p), vsrc(k + 8, p), vsrc(k + 9, p)};
-    float l[4];
-#pragma unroll
-    for (int e = 0; e < 4; ++e) l[e] = (v[e] - __half2float(__float2half_rn(v[e]))) * 2048.f;
-    s_frag[(kb * 6 + p) * 4 + t] = make_uint4(pack_half2(v[0], v[1]), pack_half2(l[0], l[1]), pack_half2(v[2], v[3]),
-                                               pack_half2(l[2], l[3]));
-  }
-  __syncthreads();
 
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int g = lane >> 2, t = lane & 3;
-  const int rw = (warp & 1) * 64;                 // this warp's rows inside the CTA
-  const int ks = warp >> 1;
+  const int rw = (warp % kThinRowWarps) * 64;                 // this warp's rows inside a row block
+  const int ks = warp / kThinRowWarps;
   const int per = (nkb + kThinSlices - 1) / kThinSlices;
   const int kb0 = ks * per, kb1 = min(nkb, kb0 + per);
-  const int r0 = blockIdx.x * kThinRows + rw;
-  float acc[8][4];
+  uint4 qh[kDepth][4], ql[kLo ? kDepth : 1][4];
+  auto fetch = [&](int kb, int r0, uint4 (&h)[4], uint4 (&l)[4]) {
+    const int k = kb * 16 + 2 * t;
+    const int kk[4] = {k, k + 1, k + 8, k + 9};
 #pragma unroll
-  for (int i = 0; i < 8; ++i) acc[i][0] = acc[i][1] = acc[i][2] = acc[i][3] = 0.f;
-  if (r0 < n && kb0 < kb1) {   // (else: this warp's part of s_red stays zero, written below)
-    const int64_t rowoff = r0 + 8 * g;
-    uint4 qh[2][4], ql[2][4];
-    auto fetch = [&](int kb, uint4 (&h)[4], uint4 (&l)[4]) {
-      const int k = kb * 16 + 2 * t;
-      const int kk[4] = {k, k + 1, k + 8, k + 9};
-#pragma unroll
-      for (int e = 0; e < 4; ++e) {
-        const int64_t off = (int64_t)kk[e] * ld + rowoff;
-        h[e] = load_rows8(ahi, off, kk[e] < n);
-        if (alo) l[e] = load_rows8(alo, off, kk[e] < n);
-      }
-    };
-    fetch(kb0, qh[0], ql[0]);
-    for (int kb = kb0; kb < kb1; kb += 2) {
-      if (kb + 1 < kb1) fetch(kb + 1, qh[1], ql[1]);
-      uint4 f = make_uint4(0u, 0u, 0u, 0u);
-      if (g < NOLSM_BS) f = s_frag[(kb * 6 + g) * 4 + t];
-      step_mma<false>(acc, qh[0], f);
-      if (alo) step_mma<true>(acc, ql[0], f);
-      if (kb + 1 < kb1) {
-        if (kb + 2 < kb1) fetch(kb + 2, qh[0], ql[0]);
-        f = make_uint4(0u, 0u, 0u, 0u);
-        if (g < NOLSM_BS) f = s_frag[((kb + 1) * 6 + g) * 4 + t];
-        step_mma<false>(acc, qh[1], f);
-        if (alo) step_mma<true>(acc, ql[1], f);
-      }
+    for (int e = 0; e < 4; ++e) {
+      const int64_t off = (int64_t)kk[e] * ld + r0 + 8 * g;
+      h[e] = load_rows8(ahi, off, kk[e] < n);
+      if constexpr (kLo) l[e] = load_rows8(alo, off, kk[e] < n);
     }
-  }
-  if (g < NOLSM_BS) {   // C^T rows 0..5 (hi) and 8..13 (lo * 2^11) of column p = g; tile i holds rows r0 + 8 n + i
-    float *red = s_red + (size_t)ks * kThinRows * NOLSM_BS;
+  };
+  auto prologue = [&](int r0) {
+    if (r0 < n) {
 #pragma unroll
-    for (int i = 0; i < 8; ++i) {
-      red[(rw + 16 * t + i) * NOLSM_BS + g] = fmaf(acc[i][2], 1.f / 2048.f, acc[i][0]);
-      red[(rw + 16 * t + 8 + i) * NOLSM_BS + g] = fmaf(acc[i][3], 1.f / 2048.f, acc[i][1]);
+      for (int sg = 0; sg < kDepth - 1; ++sg)
+        if (kb0 + sg < kb1) fetch(kb0 + sg, r0, qh[sg], ql[kLo ? sg : 0]);
+    }
+  };
+  const int rb_first = blockIdx.x * kThinCtaRows;
+  prologue(rb_first + rw);   // the first loads of A are under way while the thin operand is staged
+
+  // position of j in its own (sorted) neighbour list = entries below j.  All loads of this kernel's prologue and
+  // epilogue are issued in batches: under the streaming load of the other CTAs a dependent round trip costs
+  // microseconds, and a CTA only streams for a few tens of them.
+  int own0 = 0;
+  for (int base = 0; base < m; base += 8 * 32) {
+    int c[8];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+      const int i = base + 32 * u + lane;
+      c[u] = i < m ? a.col_idx[lo + i] : j;
+    }
+#pragma unroll
+    for (int u = 0; u < 8; ++u) own0 += c[u] < j ? 1 : 0;
+  }
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) own0 += __shfl_xor_sync(0xffffffffu, own0, d);
+  own0 *= NOLSM_BS;
+  // elements (k, p), (k + 1, p) of the thin operand, k even
+  auto vsrc2 = [&](int k, int p) -> float2 {
+    if (k >= n) return make_float2(0.f, 0.f);
+    if constexpr (kMode == kOwnResid) {
+      return __half22float2(*reinterpret_cast<const __half2 *>(a0j + (int64_t)(own0 + p) * ld + k));
+    } else {
+      const float *src = (kMode == kOwnCorrect || (kMode == kDensity && a.folded)) ? tj + (int64_t)p * ld
+                                                                                  : sj + (int64_t)(own0 + p) * ld;
+      return *reinterpret_cast<const float2 *>(src + k);
+    }
+  };
+  // item = (p, pair of columns): one half (hi, lo words) of the fragment of thread t of step kb
+  const int pairs = nkb * 8;
+  for (int base = threadIdx.x; base < NOLSM_BS * pairs; base += 4 * kThinThreads) {
+    float2 v[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int i = base + u * kThinThreads;
+      v[u] = i < NOLSM_BS * pairs ? vsrc2(2 * (i % pairs), i / pairs) : make_float2(0.f, 0.f);
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int i = base + u * kThinThreads;
+      if (i < NOLSM_BS * pairs) {
+        const int p = i / pairs, kp = i - p * pairs;
+        const int kb = kp >> 3, tt = kp & 3, upper = (kp >> 2) & 1;
+        const float l0 = (v[u].x - __half2float(__float2half_rn(v[u].x))) * 2048.f;
+        const float l1 = (v[u].y - __half2float(__float2half_rn(v[u].y))) * 2048.f;
+        reinterpret_cast<uint2 *>(s_frag + (kb * 6 + p) * 4 + tt)[upper] = make_uint2(pack_half2(v[u].x, v[u].y), pack_half2(l0, l1));
+      }
     }
   }
   __syncthreads();
-  auto total = [&](int i) {   // i = row * 6 + p
-    float c = s_red[i];
-#pragma unroll
-    for (int sl = 1; sl < kThinSlices; ++sl) c += s_red[sl * kThinRows * NOLSM_BS + i];
-    return c;
-  };
 
-  const int rb = blockIdx.x * kThinRows;
-  if constexpr (kMode == kDensity) {
-    // [n][6] block column of D: rows contiguous, six floats each
-    for (int i = threadIdx.x; i < kThinRows * NOLSM_BS; i += kThinThreads) {
-      const int rr = i / NOLSM_BS, p = i - rr * NOLSM_BS;
-      if (rb + rr < n)
-        a.d_val[(int64_t)lo * 36 + (int64_t)(rb + rr) * NOLSM_BS + p] = 0.5f * (sj[(int64_t)(own0 + p) * ld + rb + rr] - total(i));
+  for (int rb = rb_first; rb < min(n, rb_first + kThinCtaRows); rb += kThinRows) {
+    const int r0 = rb + rw;
+    if (rb != rb_first) prologue(r0);
+    float acc[8][4];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) acc[i][0] = acc[i][1] = acc[i][2] = acc[i][3] = 0.f;
+    if (r0 < n) {
+      for (int kb = kb0; kb < kb1; kb += kDepth) {
+#pragma unroll
+        for (int sg = 0; sg < kDepth; ++sg) {
+          if (kb + sg < kb1) {
+            constexpr int kAhead = kDepth - 1;
+            if (kb + sg + kAhead < kb1)
+              fetch(kb + sg + kAhead, r0, qh[(sg + kAhead) % kDepth], ql[kLo ? (sg + kAhead) % kDepth : 0]);
+            uint4 f = make_uint4(0u, 0u, 0u, 0u);
+            if (g < NOLSM_BS) f = s_frag[((kb + sg) * 6 + g) * 4 + t];
+            step_mma<false>(acc, qh[sg], f);
+            if constexpr (kLo) step_mma<true>(acc, ql[sg], f);
+          }
+        }
+      }
     }
+    if (g < NOLSM_BS) {   // C^T rows 0..5 (hi) and 8..13 (lo * 2^11) of column p = g; tile i holds rows r0 + 8 n + i
+      float *red = s_red + (size_t)ks * kThinRows * NOLSM_BS;
+#pragma unroll
+      for (int i = 0; i < 8; ++i) {
+        red[(rw + 16 * t + i) * NOLSM_BS + g] = fmaf(acc[i][2], 1.f / 2048.f, acc[i][0]);
+        red[(rw + 16 * t + 8 + i) * NOLSM_BS + g] = fmaf(acc[i][3], 1.f / 2048.f, acc[i][1]);
+      }
+    }
+    __syncthreads();
+    auto total = [&](int i) {   // i = row * 6 + p
+      float c = s_red[i];
+#pragma unroll
+      for (int sl = 1; sl < kThinSlices; ++sl) c += s_red[sl * kThinRows * NOLSM_BS + i];
+      return c;
+    };
+    static_assert(kThinRows * NOLSM_BS % (4 * kThinThreads) == 0, "finalize: four outputs per thread and pass");
+    for (int base = threadIdx.x; base < kThinRows * NOLSM_BS; base += 4 * kThinThreads) {
+      float v[4];
+      int rr[4], pp[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int i = base + u * kThinThreads;
+        if constexpr (kMode == kDensity) { rr[u] = i / NOLSM_BS; pp[u] = i - rr[u] * NOLSM_BS; }   // [n][6] block column of D
+        else { pp[u] = i / kThinRows; rr[u] = i - pp[u] * kThinRows; }                              // [6][ld] thin / dense columns
+        const int r = rb + rr[u];
+        v[u] = 0.f;
+        if (r < n) {
+          if constexpr (kMode == kDensity || kMode == kLastHalf) v[u] = sj[(int64_t)(own0 + pp[u]) * ld + r];
+          else if constexpr (kMode == kOwnCorrect) v[u] = __half2float(a0j[(int64_t)(own0 + pp[u]) * ld + r]);
+        }
+      }
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int r = rb + rr[u], p = pp[u];
+        if (r >= n) continue;
+        const float c = total(rr[u] * NOLSM_BS + p);
+        if constexpr (kMode == kDensity) a.d_val[(int64_t)lo * 36 + (int64_t)r * NOLSM_BS + p] = 0.5f * (v[u] - c);
+        else if constexpr (kMode == kLastHalf) tj[(int64_t)p * ld + r] = fmaf(0.5f, c, v[u]);
+        else if constexpr (kMode == kOwnResid) tj[(int64_t)p * ld + r] = (r == own0 + p ? 1.f : 0.f) - c;
+        else a.out32[(int64_t)mat * a.slab + (int64_t)(own0 + p) * ld + r] = v[u] + c;
+      }
+    }
+    __syncthreads();   // s_red is rewritten by the next row block
+  }
+  if constexpr (kMode == kDensity) {
     if (a.ne_diag != nullptr && blockIdx.x == 0 && warp < NOLSM_BS) {
       // electron count: 1 - X_rr over the own rows; folded: the diagonal of X_{k+1} = X_k + 1/2 X_k E_k
       const int r = own0 + warp;
@@ -199,16 +257,6 @@ __global__ void __launch_bounds__(kThinThreads, 2) k_thin_mma(const ThinArgs a) 
       }
       if (lane == 0) atomicAdd(a.ne_diag, (double)(1.f - fmaf(0.5f, dot, split_at(ahi, alo, (int64_t)r * ld + r))));
     }
-  } else {
-    for (int i = threadIdx.x; i < kThinRows * NOLSM_BS; i += kThinThreads) {
-      const int p = i / kThinRows, rr = i - p * kThinRows;
-      const int r = rb + rr;
-      if (r >= n) continue;
-      const float c = total(rr * NOLSM_BS + p);
-      if constexpr (kMode == kLastHalf) tj[(int64_t)p * ld + r] = fmaf(0.5f, c, sj[(int64_t)(own0 + p) * ld + r]);
-      else if constexpr (kMode == kOwnResid) tj[(int64_t)p * ld + r] = (r == own0 + p ? 1.f : 0.f) - c;
-      else a.out32[(int64_t)mat * a.slab + (int64_t)(own0 + p) * ld + r] = __half2float(a0j[(int64_t)(own0 + p) * ld + r]) + c;
-    }
   }
 }
 
@@ -217,12 +265,15 @@ cudaError_t thin_launch(const nolsm_batch *b, const ThinArgs &a, cudaStream_t st
   const int nkb = (b->max_n + 15) / 16;
   const size_t smem = (size_t)nkb * 24 * sizeof(uint4) + (size_t)kThinSlices * kThinRows * NOLSM_BS * sizeof(float);
   if (smem > 200 * 1024) return cudaErrorInvalidValue;   // the thin operand of one submatrix must fit in shared memory
+  const bool lo = a.a_lo[0] != nullptr;
   if (smem > 48 * 1024) {   // per device and cheap: set on every such launch (a process may use several devices)
-    cudaError_t e = cudaFuncSetAttribute(k_thin_mma<kMode>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = lo ? cudaFuncSetAttribute(k_thin_mma<kMode, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)
+                       : cudaFuncSetAttribute(k_thin_mma<kMode, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
   }
-  dim3 grid((b->max_n + kThinRows - 1) / kThinRows, b->count);
-  k_thin_mma<kMode><<<grid, kThinThreads, smem, st>>>(a);
+  dim3 grid((b->max_n + kThinCtaRows - 1) / kThinCtaRows, b->count);
+  if (lo) k_thin_mma<kMode, true><<<grid, kThinThreads, smem, st>>>(a);
+  else k_thin_mma<kMode, false><<<grid, kThinThreads, smem, st>>>(a);
   return cudaGetLastError();
 }
 
