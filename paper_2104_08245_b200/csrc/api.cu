@@ -99,6 +99,7 @@ static void free_batch(nolsm_batch *b) {
   cudaFree(b->d_lastres);
   cudaFree(b->d_scale);
   cudaFree(b->d_norm);
+  cudaFree(b->d_norm_s);
   cudaFree(b->d_alpha);
   cudaFree(b->d_colpart);
   cudaFree(b->d_active);
@@ -206,7 +207,7 @@ static nolsm_status setup_batch(nolsm_ctx *ctx, int slot, const std::vector<int3
     const size_t cap = (size_t)count;
     if (grow(&b->d_dims, cap) || grow(&b->d_state, cap) || grow(&b->d_iters, cap) ||
         grow(&b->d_resid2, cap * NOLSM_MAX_RESID_SLOTS) || grow(&b->d_lastres, cap) ||
-        grow(&b->d_scale, cap) || grow(&b->d_norm, cap * 2) || grow(&b->d_alpha, cap * 8) || grow(&b->d_slot_state, cap) ||
+        grow(&b->d_scale, cap) || grow(&b->d_norm, cap * 2) || grow(&b->d_norm_s, cap * 2) || grow(&b->d_alpha, cap * 8) || grow(&b->d_slot_state, cap) ||
         grow(&b->d_slot_done, cap) || grow(&b->d_sched, (size_t)8) || grow(&b->d_tile_counter, (size_t)1) ||
         (b->d_active == nullptr && grow(&b->d_active, (size_t)NOLSM_MAX_RESID_SLOTS))) {
       cudaGetLastError();
@@ -225,6 +226,9 @@ static nolsm_status setup_batch(nolsm_ctx *ctx, int slot, const std::vector<int3
   }
   NOLSM_CUDA(ctx, cudaMemsetAsync(b->d_sched, 0, 8 * sizeof(int32_t), st));
   b->count = count;
+  b->s32_built = true;
+  b->s_norm_built = false;
+  b->sinv_own_only = false;
   b->ld = ld;
   b->max_n = max_n;
   b->mol_begin = mol_begin;
@@ -378,7 +382,8 @@ extern "C" nolsm_status nolsm_set_model(nolsm_ctx *ctx, const nolsm_model *model
 
 static nolsm_status build_submatrices_impl(nolsm_ctx *ctx, const nolsm_bsr *H, const nolsm_bsr *S,
                                            int32_t mol_begin, int32_t mol_count, int32_t slot, int units,
-                                           nolsm_batch **out, void *stream, bool need_h32 = true) {
+                                           nolsm_batch **out, void *stream, bool need_h32 = true,
+                                           bool need_s32 = true) {
   if (!ctx || !out) return NOLSM_EINVAL;
   CHECK(check_bsr(ctx, H, "H"));
   CHECK(check_bsr(ctx, S, "S"));
@@ -398,6 +403,9 @@ static nolsm_status build_submatrices_impl(nolsm_ctx *ctx, const nolsm_bsr *H, c
   // the split copy of S is only read by the Newton refinements of S^-1 (reading 11)
   const int prec = effective_precision(ctx, -1);
   const bool split_s = (ctx->cfg.inv_refine >= 0 ? ctx->cfg.inv_refine : (prec == NOLSM_FP16_FP32 ? 1 : 0)) > 0;
+  // the FP32 copy of T_j(S) can only be left out where the lean FP16 start of Eq. 15-17 reads the split copy
+  if (!(split_s && prec == NOLSM_FP16_FP32) || ctx->has_model) need_s32 = true;
+  b->s_norm_built = false;
   if (ctx->has_model) {
     if (ctx->model.n_mol != H->n_mol) {
       ctx->err = "the attached model has a different number of molecules than the matrices";
@@ -406,10 +414,14 @@ static nolsm_status build_submatrices_impl(nolsm_ctx *ctx, const nolsm_bsr *H, c
     LAUNCH(ctx, launch_generate(b, H->row_ptr, H->col_idx, &ctx->model, need_h32 ? b->u[1] : nullptr, b->u[0],
                                 split_s, st));
   } else {
+    // the builder sees every column of T_j(S) whole: its norm bound comes out of the same pass
+    NOLSM_CUDA(ctx, cudaMemsetAsync(b->d_norm_s, 0, sizeof(float) * 2 * b->count, st));
     LAUNCH(ctx, launch_gather(b, H->row_ptr, H->col_idx, nullptr, nullptr, H->val, S->val,
-                              need_h32 ? b->u[1] : nullptr, b->u[0], split_s, st));
+                              need_h32 ? b->u[1] : nullptr, need_s32 ? b->u[0] : nullptr, split_s, b->d_norm_s, st));
+    b->s_norm_built = true;
   }
   b->s_split_built = split_s;
+  b->s32_built = need_s32;
   b->row_ptr = H->row_ptr;
   b->col_idx = H->col_idx;
   b->grouped = false;
@@ -466,7 +478,7 @@ extern "C" nolsm_status nolsm_build_submatrices_grouped(nolsm_ctx *ctx, const no
   CHECK(setup_batch(ctx, slot, dims, grp_begin, true, units_for(prec), &b, st));
   const bool split_s = (ctx->cfg.inv_refine >= 0 ? ctx->cfg.inv_refine : (prec == NOLSM_FP16_FP32 ? 1 : 0)) > 0;
   LAUNCH(ctx, launch_gather(b, H->row_ptr, H->col_idx, groups->list_ptr, groups->list_idx, H->val, S->val, b->u[1],
-                            b->u[0], split_s, st));
+                            b->u[0], split_s, nullptr, st));
   b->s_split_built = split_s;
   b->row_ptr = H->row_ptr;
   b->col_idx = H->col_idx;
@@ -567,7 +579,15 @@ static nolsm_status prepare_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, int prec
   // which the refinement squares (< 4e-5)
   const float inv_tol = ctx->cfg.inv_tol > 0.f ? ctx->cfg.inv_tol : (fp16 ? (refine > 0 ? 3e-3f : 1e-2f) : 1e-5f);
   float *S = b->u[0], *H = b->u[1];
-  LAUNCH(ctx, launch_norm_bound(b, S, 0.f, true, b->d_norm, st));
+  // FP16 mode with a refinement behind the iteration: the iterates live in FP16 only (the add-in of the
+  // correction form is the FP16 operand copy itself); their 5e-4 rounding is far inside what the refinement
+  // squares away, and no tile reads or writes an FP32 master
+  const bool masters = !(fp16 && refine > 0);
+  // lean start: the builder left the split copy of S and its norm bound; Y0 is never written (launch_init_z1)
+  const bool lean = !masters && b->s_split_built && b->s_norm_built;
+  if (!lean && !b->s32_built) { ctx->err = "this batch was built without the FP32 copy of S"; return NOLSM_EINVAL; }
+  const float *s_norm = b->s_norm_built ? b->d_norm_s : b->d_norm;
+  if (!b->s_norm_built) LAUNCH(ctx, launch_norm_bound(b, S, 0.f, true, b->d_norm, st));
   ChainProgram pg;
   memset(&pg, 0, sizeof(pg));
   pg.n_ops = 3;
@@ -584,14 +604,13 @@ static nolsm_status prepare_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, int prec
   p0.n_ops = 1;
   ChainOp &y1 = p0.ops[0] = make_op(EPI_AXPBY, 0.5f, 1.f);
   y1.cin32 = y1.cout32 = 2;
-  // FP16 mode with a refinement behind the iteration: the iterates live in FP16 only (the add-in of the
-  // correction form is the FP16 operand copy itself); their 5e-4 rounding is far inside what the refinement
-  // squares away, and no tile reads or writes an FP32 master
-  const bool masters = !(fp16 && refine > 0);
   if (fp16) {
     // Y16: h0/h1 (ping-pong), Z16: h2/h3, E16: h4; masters (if kept) Y32 = u2, Z32 = u3
-    LAUNCH(ctx, launch_init_inverse_first(b, S, b->d_norm, masters ? b->u[2] : nullptr, masters ? b->u[3] : nullptr,
-                                          b->h[0], nullptr, b->h[3], nullptr, b->h[4], nullptr, b->d_scale, st));
+    if (lean)
+      LAUNCH(ctx, launch_init_z1(b, b->h[b->n_half - 4], b->h[b->n_half - 3], s_norm, b->h[3], b->d_scale, st));
+    else
+      LAUNCH(ctx, launch_init_inverse_first(b, S, s_norm, masters ? b->u[2] : nullptr, masters ? b->u[3] : nullptr,
+                                            b->h[0], nullptr, b->h[3], nullptr, b->h[4], nullptr, b->d_scale, st));
     set2(y1.a, 0, 0); set2(y1.b, 4, 4); set2(y1.out16, 1, 1);
     pg.group = group_size(ctx, b, masters ? 18 : 10);
     ChainOp &e = pg.ops[0] = make_op(EPI_IDENT, 1.f, 0.f);
@@ -600,15 +619,20 @@ static nolsm_status prepare_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, int prec
     set2(y.a, 1, 0); set2(y.b, 4, 4); y.cin32 = y.cout32 = 2; set2(y.out16, 0, 1);
     ChainOp &z = pg.ops[2] = make_op(EPI_AXPBY, 0.5f, 1.f);
     set2(z.a, 4, 4); set2(z.b, 3, 2); z.cin32 = z.cout32 = 3; set2(z.out16, 2, 3);
+    if (lean) {   // Y1 = Y0 Z1 = (S_hi Z1)/s_S: plain product, scaled in the epilogue
+      y1 = make_op(EPI_AXPBY, 1.f, 0.f);
+      y1.use_div = 1;
+      set2(y1.a, b->n_half - 4, b->n_half - 4); set2(y1.b, 3, 3); set2(y1.out16, 1, 1);
+    }
     if (!masters) {
-      y1.cin32 = y1.cout32 = -1; set2(y1.cin16, 0, 0);
+      if (!lean) { y1.cin32 = y1.cout32 = -1; set2(y1.cin16, 0, 0); }
       y.cin32 = y.cout32 = -1; set2(y.cin16, 1, 0);
       z.cin32 = z.cout32 = -1; set2(z.cin16, 3, 2);
     }
   } else {
     // split operands: Y (h0,h1)/(h2,h3), Z (h4,h5)/(h6,h7), E (h8,h9)
     // the iterates live as split pairs only (22 bits): the add-in of the correction form is the operand pair itself
-    LAUNCH(ctx, launch_init_inverse_first(b, S, b->d_norm, nullptr, nullptr, b->h[0], b->h[1], b->h[6], b->h[7],
+    LAUNCH(ctx, launch_init_inverse_first(b, S, s_norm, nullptr, nullptr, b->h[0], b->h[1], b->h[6], b->h[7],
                                           b->h[8], b->h[9], b->d_scale, st));
     set2(y1.a, 0, 0); set2(y1.a_lo, 1, 1); set2(y1.b, 8, 8); set2(y1.b_lo, 9, 9);
     set2(y1.out16, 2, 2); set2(y1.out16_lo, 3, 3);
@@ -624,7 +648,7 @@ static nolsm_status prepare_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, int prec
     set2(z.a, 8, 8); set2(z.a_lo, 9, 9); set2(z.b, 6, 4); set2(z.b_lo, 7, 5);
     set2(z.cin16, 6, 4); set2(z.cin16_lo, 7, 5); set2(z.out16, 4, 6); set2(z.out16_lo, 5, 7);
   }
-  CHECK(run_chain(ctx, b, p0, nullptr, false, st));
+  CHECK(run_chain(ctx, b, p0, lean ? b->d_scale : nullptr, false, st));
   CHECK(run_chain(ctx, b, pg, nullptr, true, st));
   // submatrices whose Eq. 15-17 iteration ended at the cap or on a NaN (S_j not SPD / badly scaled): kept beside
   // the scheduler words, which the next launch resets
@@ -1366,8 +1390,9 @@ extern "C" nolsm_status nolsm_solve_mu(nolsm_ctx *ctx, const nolsm_bsr *H, const
         b->prepared_precision = prec;
       } else if (!b || !resident) {
         // the FP32 copy of T_j(H) is only read by the energy products (nolsm_evaluate) and the SIMT debug path
+        const bool need32 = ctx->eval_energy || use_simt(ctx) || !ctx->umma_ok;
         rc = build_submatrices_impl(ctx, H, S, r.begin, r.count, kOwnSlot + (resident ? (int)bi : 0), units, &b, st,
-                                    ctx->eval_energy || use_simt(ctx) || !ctx->umma_ok);
+                                    need32, need32);
         if (rc != NOLSM_OK) break;
         live[bi] = resident ? b : nullptr;
       }

@@ -100,6 +100,8 @@ struct nolsm_batch {
   bool x_split = false;           // the sign iterate lives as hi (h[iters & 1]) + lo * 2^-11 (h[2]); u[0] holds X in
   bool x32_valid = false;         // FP32 only after join_x (reading 12)
   bool s_split_built = false;     // the builder wrote the split copy of S into h[n_half-4], h[n_half-3]
+  bool s32_built = true;          // u0 holds the FP32 T_j(S) (false: nolsm_solve_mu built the split copy only)
+  bool s_norm_built = false;      // d_norm_s holds ||S_j||_1 = ||S_j||_inf from the builder
   bool prefer_pair = false;       // batch shape favours the pair engine (nolsm.h, NOLSM_FLAG_*)
   bool engine_simt = false;       // prepared by the FP32 SIMT debugging path (different buffer roles)
   bool sparse = true;             // false: dense microbench batch (no neighbour list)
@@ -118,6 +120,7 @@ struct nolsm_batch {
   float *d_scale = nullptr;       // [count] s_j of the sign scaling
   float *d_alpha = nullptr;       // [count][8] alpha_k of the scaled Newton-Schulz start (gap_hint)
   float *d_norm = nullptr;        // [2][count] scratch for norm bounds
+  float *d_norm_s = nullptr;      // [2][count] norm bound of S from the builder (s_norm_built)
   float *d_colpart = nullptr;     // [count][ld/128][ld] column-sum shares of the row strips (k_norm_bound)
   size_t colpart_cap = 0;
   int32_t *d_active = nullptr;    // [NOLSM_MAX_RESID_SLOTS] active counters per iteration
@@ -191,7 +194,7 @@ cudaError_t launch_generate(const nolsm_batch *b, const int32_t *row_ptr, const 
 cudaError_t launch_gather(const nolsm_batch *b, const int32_t *row_ptr, const int32_t *col_idx,
                           const int32_t *list_ptr, const int32_t *list_idx,
                           const float *h_val, const float *s_val, float *h_out, float *s_out, bool split_s,
-                          cudaStream_t st);
+                          float *s_norm, cudaStream_t st);
 
 // own columns of S^-1 (u2) to / from a packed [count][6][ld] array (operator cache of nolsm_solve_mu)
 cudaError_t launch_pack_square(const nolsm_batch *b, float *dense, float *packed, bool save, cudaStream_t st);
@@ -236,6 +239,9 @@ cudaError_t launch_norm_bound(const nolsm_batch *b, const float *a, float mu, bo
 cudaError_t launch_init_inverse(const nolsm_batch *b, const float *s, const float *norm2, float *y32,
                                 float *z32, __half *y16, __half *z16, __half *y16_lo, __half *z16_lo,
                                 float *scale_out, cudaStream_t st);
+// lean start of Eq. 15-17 in FP16 mode: only Z1 = 3/2 I - 1/2 S/s_S is formed; Y1 = (S_hi Z1)/s_S is a product
+cudaError_t launch_init_z1(const nolsm_batch *b, const __half *s_hi, const __half *s_lo, const float *norm2, __half *z16,
+                           float *scale_out, cudaStream_t st);
 cudaError_t launch_init_inverse_first(const nolsm_batch *b, const float *s, const float *norm2, float *y32,
                                       float *z32, __half *y16, __half *y16_lo, __half *z16, __half *z16_lo,
                                       __half *e16, __half *e16_lo, float *scale_out, cudaStream_t st);

@@ -237,6 +237,87 @@ cudaError_t launch_init_inverse_first(const nolsm_batch *b, const float *s, cons
   return cudaGetLastError();
 }
 
+// Lean start of Eq. 15-17 when the iterates live in FP16 only (FP16 mode with a refinement behind the iteration):
+// Y0 = S/s_S is never written -- with Z0 = I the first iteration gives Z1 = 3/2 I - 1/2 Y0 element-wise and
+// Y1 = Y0 + 1/2 Y0 (I - Y0) = Y0 Z1 = (S_hi Z1)/s_S as ONE product whose left operand is the FP16 copy of S the
+// builder wrote (scaled by 1/s_S in the product's epilogue, so Y0 = S_hi/s_S carries no second rounding).
+// Reads the split S (4 bytes per element), writes Z1 (2 bytes) instead of reading 4 and writing 6.
+// Element-wise passes, eight rows per thread: thread t of a block owns rows 8t..8t+7 (one 16-byte FP16 access, two
+// for FP32) of kElemCols consecutive columns -- no index division, 16-byte accesses, all loads of a thread issued
+// before the first use (the four-element version was bound by instruction issue, not by HBM).
+constexpr int kElemCols = 4;
+static dim3 elem8_grid(const nolsm_batch *b) {
+  const int P = round_up(b->max_n, NOLSM_TILE_M);
+  return dim3((unsigned)((P + kElemCols - 1) / kElemCols), (unsigned)b->count);
+}
+static int elem8_threads(const nolsm_batch *b) { return std::min(256, (round_up(b->max_n, NOLSM_TILE_M) / 8 + 31) / 32 * 32); }
+
+__device__ __forceinline__ void unpack8(const uint4 &q, float (&v)[8]) {
+  const uint32_t w[4] = {q.x, q.y, q.z, q.w};
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const float2 f = __half22float2(*reinterpret_cast<const __half2 *>(&w[i]));
+    v[2 * i] = f.x; v[2 * i + 1] = f.y;
+  }
+}
+__device__ __forceinline__ uint4 pack8(const float (&v)[8]) {
+  uint32_t w[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const __half2 h = __floats2half2_rn(v[2 * i], v[2 * i + 1]);
+    w[i] = *reinterpret_cast<const uint32_t *>(&h);
+  }
+  return make_uint4(w[0], w[1], w[2], w[3]);
+}
+// hi = fp16(v), lo = fp16((v - hi) * 2^11)
+__device__ __forceinline__ void split8(const float (&v)[8], uint4 &hi, uint4 &lo) {
+  hi = pack8(v);
+  float h[8], l[8];
+  unpack8(hi, h);
+#pragma unroll
+  for (int i = 0; i < 8; ++i) l[i] = (v[i] - h[i]) * 2048.f;
+  lo = pack8(l);
+}
+
+__global__ void __launch_bounds__(256)
+k_init_z1(const int32_t *__restrict__ dims, int ld, int64_t slab, int count, const __half *__restrict__ s_hi,
+          const __half *__restrict__ s_lo, const float *__restrict__ norm2, __half *__restrict__ z16,
+          float *__restrict__ scale_out, float factor) {
+  const int mat = blockIdx.y;
+  const int P = padded_dim(dims[mat]);
+  const int c0 = blockIdx.x * kElemCols;
+  if (c0 >= P) return;
+  const float sc = factor * fmaxf(1.f, sqrtf(norm2[mat] * norm2[count + mat]));
+  if (threadIdx.x == 0 && c0 == 0) scale_out[mat] = sc;
+  for (int r = 8 * threadIdx.x; r < P; r += 8 * blockDim.x) {
+  const int64_t off = (int64_t)mat * slab + (int64_t)c0 * ld + r;
+  uint4 hq[kElemCols], lq[kElemCols];
+#pragma unroll
+  for (int u = 0; u < kElemCols; ++u) {   // P is a multiple of 128: a block's columns are all inside or all outside
+    hq[u] = *reinterpret_cast<const uint4 *>(s_hi + off + (int64_t)u * ld);
+    lq[u] = *reinterpret_cast<const uint4 *>(s_lo + off + (int64_t)u * ld);
+  }
+  const float inv = -0.5f / sc;
+#pragma unroll
+  for (int u = 0; u < kElemCols; ++u) {
+    float h[8], l[8], z[8];
+    unpack8(hq[u], h);
+    unpack8(lq[u], l);
+#pragma unroll
+    for (int i = 0; i < 8; ++i) z[i] = fmaf(fmaf(l[i], 1.f / 2048.f, h[i]), inv, (r + i == c0 + u) ? 1.5f : 0.f);
+    *reinterpret_cast<uint4 *>(z16 + off + (int64_t)u * ld) = pack8(z);
+  }
+  }
+}
+
+cudaError_t launch_init_z1(const nolsm_batch *b, const __half *s_hi, const __half *s_lo, const float *norm2, __half *z16,
+                           float *scale_out, cudaStream_t st) {
+  if (b->count == 0) return cudaSuccess;
+  k_init_z1<<<elem8_grid(b), elem8_threads(b), 0, st>>>(b->d_dims, b->ld, (int64_t)b->ld * b->ld, b->count, s_hi, s_lo,
+                                                         norm2, z16, scale_out, b->inv_scale);
+  return cudaGetLastError();
+}
+
 // X0 = (B - mu I)/s  (Eq. 9 with the rescaling of PAPER.md:138), s from the norm bound or from the
 // caller (scale_in, dense microbench).  Padded diagonal = 1: a fixed point of the iteration that adds
 // nothing to the residual (reading 19).
@@ -265,10 +346,57 @@ k_make_x0(const int32_t *__restrict__ dims, int ld, int64_t slab, int count,
   if (x16) store_split4(x16 + e.off, x16_lo ? x16_lo + e.off : nullptr, v);
 }
 
+// the same for the split iterate of the tensor-core engine (no FP32 copy), eight rows per thread
+__global__ void __launch_bounds__(256)
+k_make_x0_split(const int32_t *__restrict__ dims, int ld, int64_t slab, int count, const float *__restrict__ bmat,
+                float mu, const float *__restrict__ norm2, const float *__restrict__ scale_in,
+                __half *__restrict__ x16, __half *__restrict__ x16_lo, float *__restrict__ scale_out, float factor) {
+  const int mat = blockIdx.y;
+  const int n = dims[mat];
+  const int P = padded_dim(n);
+  const int c0 = blockIdx.x * kElemCols;
+  if (c0 >= P) return;
+  float sc = scale_in ? scale_in[mat] : factor * sqrtf(norm2[mat] * norm2[count + mat]);
+  sc = fmaxf(sc, 1e-30f);
+  const float inv = 1.f / sc;
+  if (threadIdx.x == 0 && c0 == 0 && scale_out) scale_out[mat] = sc;
+  for (int r = 8 * threadIdx.x; r < P; r += 8 * blockDim.x) {
+  const int64_t off = (int64_t)mat * slab + (int64_t)c0 * ld + r;
+  float4 bq[kElemCols][2];
+#pragma unroll
+  for (int u = 0; u < kElemCols; ++u) {
+    const float4 *src = reinterpret_cast<const float4 *>(bmat + off + (int64_t)u * ld);
+    bq[u][0] = src[0];
+    bq[u][1] = src[1];
+  }
+#pragma unroll
+  for (int u = 0; u < kElemCols; ++u) {
+    const int c = c0 + u;
+    const float in[8] = {bq[u][0].x, bq[u][0].y, bq[u][0].z, bq[u][0].w, bq[u][1].x, bq[u][1].y, bq[u][1].z, bq[u][1].w};
+    float v[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      if (r + i < n && c < n) v[i] = (in[i] - (r + i == c ? mu : 0.f)) * inv;
+      else v[i] = (r + i == c) ? 1.f : 0.f;
+    }
+    uint4 hi, lo;
+    split8(v, hi, lo);
+    *reinterpret_cast<uint4 *>(x16 + off + (int64_t)u * ld) = hi;
+    *reinterpret_cast<uint4 *>(x16_lo + off + (int64_t)u * ld) = lo;
+  }
+  }
+}
+
 cudaError_t launch_make_x0(const nolsm_batch *b, const float *bmat, float mu, const float *norm2,
                            const float *scale_in, float *x32, __half *x16, __half *x16_lo, float *scale_out,
                            cudaStream_t st) {
   if (b->count == 0) return cudaSuccess;
+  if (!x32 && x16 && x16_lo) {
+    k_make_x0_split<<<elem8_grid(b), elem8_threads(b), 0, st>>>(b->d_dims, b->ld, (int64_t)b->ld * b->ld, b->count, bmat,
+                                                                 mu, norm2, scale_in, x16, x16_lo, scale_out,
+                                                                 b->sign_scale);
+    return cudaGetLastError();
+  }
   k_make_x0<<<elem4_grid(b), 256, 0, st>>>(b->d_dims, b->ld, (int64_t)b->ld * b->ld, b->count, bmat, mu, norm2,
                                            scale_in, x32, x16, x16_lo, scale_out, b->sign_scale);
   return cudaGetLastError();

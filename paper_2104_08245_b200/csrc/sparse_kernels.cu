@@ -133,7 +133,10 @@ cudaError_t launch_exclusive_scan(const int32_t *counts, int32_t *row_ptr, int n
 // copies (hi = fp16(v), lo = fp16((v - hi) 2^11): the operands of the FP32-quality products, same
 // arithmetic as k_scale_copy) so that no conversion pass has to read the matrices again.
 struct BuildOut {
-  float *h32, *s32;           // h32 may be null: inside nolsm_solve_mu only the split copy of H is read
+  float *h32, *s32;           // may be null: inside nolsm_solve_mu only the split copies are read
+  float *s_norm;              // [2 * count], zeroed by the caller: max absolute column sum of the true n x n part of
+                              // T_j(S) (= ||S||_1 = ||S||_inf, S symmetric) in [mat] and [count + mat], or null
+  int count;
   __half *h_hi, *h_lo, *s_hi, *s_lo;
 };
 
@@ -152,7 +155,7 @@ __device__ __forceinline__ void emit_rows2(const BuildOut &out, int64_t base, in
     if (c0 + p < P) {
       const int64_t off = base + (int64_t)(c0 + p) * ld + r;
       if (out.h32) *reinterpret_cast<float2 *>(out.h32 + off) = make_float2(hv[0][p], hv[1][p]);
-      *reinterpret_cast<float2 *>(out.s32 + off) = make_float2(sv[0][p], sv[1][p]);
+      if (out.s32) *reinterpret_cast<float2 *>(out.s32 + off) = make_float2(sv[0][p], sv[1][p]);
       __half2 hi, lo;
       if (out.h_hi) {
         split_pair(hv[0][p], hv[1][p], hi, lo);
@@ -204,6 +207,9 @@ k_gather(const int32_t *__restrict__ row_ptr, const int32_t *__restrict__ col_id
     // Lane = two consecutive rows (always rows o, o+1 of one block, o even).  What they contribute to this
     // block column are 48 contiguous bytes of the store: three 16-byte loads per matrix.
     const int c0 = b * NOLSM_BS;
+    float csum[NOLSM_BS];
+#pragma unroll
+    for (int p = 0; p < NOLSM_BS; ++p) csum[p] = 0.f;
     for (int r = 2 * lane; r < P; r += 64) {
       float hv[2][NOLSM_BS], sv[2][NOLSM_BS];
 #pragma unroll
@@ -220,6 +226,8 @@ k_gather(const int32_t *__restrict__ row_ptr, const int32_t *__restrict__ col_id
           hv[1][0] = x1.z; hv[1][1] = x1.w; hv[1][2] = x2.x; hv[1][3] = x2.y; hv[1][4] = x2.z; hv[1][5] = x2.w;
           sv[0][0] = y0.x; sv[0][1] = y0.y; sv[0][2] = y0.z; sv[0][3] = y0.w; sv[0][4] = y1.x; sv[0][5] = y1.y;
           sv[1][0] = y1.z; sv[1][1] = y1.w; sv[1][2] = y2.x; sv[1][3] = y2.y; sv[1][4] = y2.z; sv[1][5] = y2.w;
+#pragma unroll
+          for (int p = 0; p < NOLSM_BS; ++p) csum[p] += fabsf(sv[0][p]) + fabsf(sv[1][p]);
         }
       } else {
 #pragma unroll
@@ -230,14 +238,30 @@ k_gather(const int32_t *__restrict__ row_ptr, const int32_t *__restrict__ col_id
       }
       emit_rows2(out, base, ld, c0, r, P, hv, sv);
     }
+    if (out.s_norm != nullptr && c0 < n) {   // this warp saw all of its six columns: their absolute sums are complete
+      float cmax = 0.f;
+#pragma unroll
+      for (int p = 0; p < NOLSM_BS; ++p) {
+        float v = csum[p];
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
+        cmax = fmaxf(cmax, v);
+      }
+      if (lane == 0) {   // non-negative floats order like their bit patterns
+        atomicMax(reinterpret_cast<int *>(out.s_norm + mat), __float_as_int(cmax));
+        atomicMax(reinterpret_cast<int *>(out.s_norm + out.count + mat), __float_as_int(cmax));
+      }
+    }
     __syncwarp();
   }
 }
 
-static BuildOut build_out(const nolsm_batch *b, float *h_out, float *s_out, bool split_s) {
+static BuildOut build_out(const nolsm_batch *b, float *h_out, float *s_out, bool split_s, float *s_norm = nullptr) {
   BuildOut o;
   o.h32 = h_out;
   o.s32 = s_out;
+  o.s_norm = s_norm;
+  o.count = b->count;
   o.h_hi = b->h[b->n_half - 2];
   o.h_lo = b->h[b->n_half - 1];
   o.s_hi = split_s ? b->h[b->n_half - 4] : nullptr;
@@ -248,7 +272,7 @@ static BuildOut build_out(const nolsm_batch *b, float *h_out, float *s_out, bool
 cudaError_t launch_gather(const nolsm_batch *b, const int32_t *row_ptr, const int32_t *col_idx,
                           const int32_t *list_ptr, const int32_t *list_idx,
                           const float *h_val, const float *s_val, float *h_out, float *s_out, bool split_s,
-                          cudaStream_t st) {
+                          float *s_norm, cudaStream_t st) {
   if (b->count == 0) return cudaSuccess;
   const int per_warp = (b->ld + NOLSM_BS - 1) / NOLSM_BS + 1;
   const size_t smem = (size_t)GA_WARPS * per_warp * sizeof(int32_t);
@@ -256,7 +280,7 @@ cudaError_t launch_gather(const nolsm_batch *b, const int32_t *row_ptr, const in
   dim3 grid((cols + GA_WARPS - 1) / GA_WARPS, b->count);
   k_gather<<<grid, GA_WARPS * 32, smem, st>>>(row_ptr, col_idx, list_ptr ? list_ptr : row_ptr,
                                               list_idx ? list_idx : col_idx, h_val, s_val, b->mol_begin, b->ld,
-                                              (int64_t)b->ld * b->ld, build_out(b, h_out, s_out, split_s));
+                                              (int64_t)b->ld * b->ld, build_out(b, h_out, s_out, split_s, s_norm));
   return cudaGetLastError();
 }
 
