@@ -258,7 +258,8 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
   const bool leader = rank == 0;
   uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
   // stage layout: [A hi 16K][B hi b_bytes][A lo 16K][B lo b_bytes]
-  const int off_b = kATileBytes, off_a_lo = kATileBytes + args.b_bytes, off_b_lo = 2 * kATileBytes + args.b_bytes;
+  // a stage: [M-side hi][N-side hi][N-side lo][M-side lo] -- the lo boxes of the N side directly behind its hi boxes
+  const int off_b = kATileBytes, off_b_lo = kATileBytes + args.b_bytes, off_a_lo = kATileBytes + 2 * args.b_bytes;
   uint8_t *staging = smem + (size_t)args.stages * args.stage_bytes;   // epilogue staging buffers behind the operand ring
 
   if (threadIdx.x == 0) {
@@ -383,7 +384,6 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
         const CUtensorMap *ma = &args.maps[o.b[par]], *mb = &args.maps[o.a[par]];
         const CUtensorMap *mal = split && !half ? &args.maps[o.b_lo[par]] : nullptr;
         const CUtensorMap *mbl = split ? &args.maps[o.a_lo[par]] : nullptr;
-        const int off_bl = half ? off_b + args.b_bytes : off_b_lo;
         const int kb_go = max(0, c.kblocks - kClaimLead);
         for (int kb = 0; kb < c.kblocks; ++kb) {
           if (leader && kb == kb_go) mbar_arrive<false>(&claim_go);   // the scheduler may claim the next tile
@@ -401,7 +401,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
               tma_load_3d<kPair>(st + off_a_lo + kBoxBytes, mal, &full_bar[stage], k0, m0 + 64, m);
             }
             for (int j = 0; j < nbox; ++j)
-              tma_load_3d<kPair>(st + off_bl + j * kBoxBytes, mbl, &full_bar[stage], n0 + 64 * j, k0, m);
+              tma_load_3d<kPair>(st + off_b_lo + j * kBoxBytes, mbl, &full_bar[stage], n0 + 64 * j, k0, m);
           }
           if (++stage == args.stages) { stage = 0; phase ^= 1u; }
         }
@@ -427,10 +427,11 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
         if (c.op < 0) break;
         const bool split = pg.ops[c.op].a_lo[chainep::cmd_par(c)] >= 0;
         const bool half = split && pg.ops[c.op].b_lo[chainep::cmd_par(c)] < 0;
-        // half split, one CTA, 128-row tiles: the lo boxes of the N side start exactly 128 rows behind the hi boxes,
-        // and the correction accumulator 128 columns behind the main one -- ONE MMA of N = 128 + nt forms
-        // [A_hi B_hi | A_hi B_lo] and reads the M-side tile once (columns nt..127 are never read back)
-        const bool stacked = half && !kPair && args.b_bytes == 2 * kBoxBytes;
+        // split, one CTA, 128-row tiles: the lo boxes of the N side start exactly 128 rows behind the hi boxes, and
+        // the correction accumulator 128 columns behind the main one -- ONE MMA of N = 128 + nt forms
+        // [A_hi B_hi | A_hi B_lo] and reads the M-side tile once (columns nt..127 are never read back); a full
+        // split adds A_lo B_hi to the correction accumulator with a second MMA
+        const bool stacked = split && !kPair && args.b_bytes == 2 * kBoxBytes;
         // instruction descriptor: D=F32, A=B=F16, A K-major, B MN-major, N = nt, M = 128 per CTA
         const uint32_t idesc = (1u << 4) | (1u << 16) | ((uint32_t)(c.nt >> 3) << 17) | ((uint32_t)(kTileM >> 4) << 24);
         const uint32_t idesc_stacked =
@@ -449,16 +450,21 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
           const uint32_t b_lo = (((sa + off_b) >> 4) & 0x3FFFu) | ((uint32_t)(kBoxBytes >> 4) << 16);
           const int steps = kb == c.kblocks - 1 ? c.ktail : kBK / 16;
           if (one) {
-            if (!split || stacked) {
+            if (!split || (stacked && half)) {
               const uint32_t id = stacked ? idesc_stacked : idesc;
               tc_mma<kPair>(d_main, a_lo, b_lo, kDescHi, id, kb ? 1u : 0u);
               if (steps > 1) tc_mma<kPair>(d_main, a_lo + 2u, b_lo + 128u, kDescHi, id, 1u);
               if (steps > 2) tc_mma<kPair>(d_main, a_lo + 4u, b_lo + 256u, kDescHi, id, 1u);
               if (steps > 3) tc_mma<kPair>(d_main, a_lo + 6u, b_lo + 384u, kDescHi, id, 1u);
+            } else if (stacked) {
+              const uint32_t al_lo = (((sa + off_a_lo) >> 4) & 0x3FFFu) | (1u << 16);
+              for (int k4 = 0; k4 < steps; ++k4) {
+                tc_mma<kPair>(d_main, a_lo + 2u * k4, b_lo + 128u * k4, kDescHi, idesc_stacked, (kb | k4) ? 1u : 0u);
+                tc_mma<kPair>(d_corr, al_lo + 2u * k4, b_lo + 128u * k4, kDescHi, idesc, 1u);
+              }
             } else {
               const uint32_t al_lo = (((sa + off_a_lo) >> 4) & 0x3FFFu) | (1u << 16);
-              const uint32_t bl_lo = (((sa + (half ? off_b + args.b_bytes : off_b_lo)) >> 4) & 0x3FFFu) |
-                                     ((uint32_t)(kBoxBytes >> 4) << 16);
+              const uint32_t bl_lo = (((sa + off_b_lo) >> 4) & 0x3FFFu) | ((uint32_t)(kBoxBytes >> 4) << 16);
               for (int k4 = 0; k4 < steps; ++k4) {
                 const uint32_t accum = (kb | k4) ? 1u : 0u;
                 tc_mma<kPair>(d_main, a_lo + 2u * k4, b_lo + 128u * k4, kDescHi, idesc, accum);
