@@ -357,7 +357,8 @@ NOLSM_API int32_t nolsm_batch_ld(const nolsm_batch *batch);        /* padded lea
 /* One batched product with the engine's own kernels (unit tests of the GEMM building block):
  * C_b = beta*Cin_b + alpha*A_b*B_b (ident = 0)  or  C_b = I - A_b*B_b (ident = 1), b < batch, all
  * n x n row-major FP32 on the device (n arbitrary).  kind: 0 = FP32 SIMT, 1 = tcgen05 FP16 operands,
- * 2 = tcgen05 split-FP16 (FP32-quality).  resid2 (device float[batch], may be NULL) receives
+ * 2 = tcgen05 split-FP16 (FP32-quality), 3 = tcgen05 half-split (A split, B taken as its FP16 rounding: FP32-quality
+ * when B is exact in FP16; the add-in travels as a split FP16 pair, 22 bits).  resid2 (device float[batch], may be NULL) receives
  * ||C_b||_F^2 when ident = 1. */
 NOLSM_API nolsm_status nolsm_gemm_batched(nolsm_ctx *ctx, int32_t kind, int32_t ident, float alpha, float beta,
                                 const float *a, const float *b, const float *cin, float *c,

@@ -1655,7 +1655,7 @@ extern "C" nolsm_status nolsm_batch_read(nolsm_ctx *ctx, const nolsm_batch *b, i
 extern "C" nolsm_status nolsm_gemm_batched(nolsm_ctx *ctx, int32_t kind, int32_t ident, float alpha, float beta,
                                            const float *a, const float *bm, const float *cin, float *c,
                                            float *resid2, int32_t n, int32_t batch, void *stream) {
-  if (!ctx || !a || !bm || !c || n <= 0 || batch <= 0 || kind < 0 || kind > 2) return NOLSM_EINVAL;
+  if (!ctx || !a || !bm || !c || n <= 0 || batch <= 0 || kind < 0 || kind > 3) return NOLSM_EINVAL;
   if (!ident && beta != 0.f && !cin) return NOLSM_EINVAL;
   cudaStream_t st = (cudaStream_t)stream;
   std::vector<int32_t> dims(batch, n);
@@ -1672,14 +1672,22 @@ extern "C" nolsm_status nolsm_gemm_batched(nolsm_ctx *ctx, int32_t kind, int32_t
     CHECK(E.zero_resid(0));
     CHECK(E.simt(mode, alpha, beta, nullptr, b->u[0], b->u[1], b->u[2], b->u[3], E.resid_slot(0), nullptr, 0));
   } else {
-    LAUNCH(ctx, launch_scale_copy(b, b->u[0], nullptr, 0, nullptr, b->h[0], kind == 2 ? b->h[1] : nullptr, st));
+    LAUNCH(ctx, launch_scale_copy(b, b->u[0], nullptr, 0, nullptr, b->h[0], kind >= 2 ? b->h[1] : nullptr, st));
     LAUNCH(ctx, launch_scale_copy(b, b->u[1], nullptr, 0, nullptr, b->h[2], kind == 2 ? b->h[3] : nullptr, st));
     ChainProgram pg = one_shot(group_size(ctx, b, 16));
     pg.n_ops = 1;
     ChainOp &o = pg.ops[0] = make_op(mode, alpha, beta);
     set2(o.a, 0, 0); set2(o.b, 2, 2);
-    if (kind == 2) { set2(o.a_lo, 1, 1); set2(o.b_lo, 3, 3); }
-    if (!ident && beta != 0.f) o.cin32 = 2;
+    if (kind >= 2) set2(o.a_lo, 1, 1);
+    if (kind == 2) set2(o.b_lo, 3, 3);
+    if (!ident && beta != 0.f) {
+      if (kind == 3) {   // the add-in as a split FP16 pair through the staging buffers, like B1 = B0 + A0 R
+        LAUNCH(ctx, launch_scale_copy(b, b->u[2], nullptr, 0, nullptr, b->h[4], b->h[5], st));
+        set2(o.cin16, 4, 4); set2(o.cin16_lo, 5, 5);
+      } else {
+        o.cin32 = 2;
+      }
+    }
     o.cout32 = 3;
     o.resid = ident ? 1 : 0;
     CHECK(run_chain(ctx, b, pg, nullptr, true, st));

@@ -129,15 +129,19 @@ def test_gather_bitwise(nolsm, tiny_system, mid_system, which):
 # ---------------------------------------------------------------------------------------------
 # the GEMM building block
 # ---------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("kind,tol", [(0, 2e-5), (1, 2e-2), (2, 2e-5)])
+@pytest.mark.parametrize("kind,tol", [(0, 2e-5), (1, 2e-2), (2, 2e-5), (3, 2e-5)])
 @pytest.mark.parametrize("n,batch", [(64, 3), (146, 5), (478, 2), (863, 2)])
 def test_gemm_building_block(nolsm, torch_mod, kind, tol, n, batch):
     """C = A B and C = I - A B against FP64 numpy; kind 0 SIMT FP32, 1 tcgen05 FP16 operands,
-    2 tcgen05 split-FP16.  Tolerances relative to sqrt(n) * max|A| * max|B| (rounding of a length-n
+    2 tcgen05 split-FP16, 3 tcgen05 half-split (A split, B exact in FP16: one stacked MMA per K step; its add-in
+    goes through the staging buffers as a split FP16 pair with an FP32 result, the path of B1 = B0 + A0 R).
+    Tolerances relative to sqrt(n) * max|A| * max|B| (rounding of a length-n
     dot product: FP32 ~ 6e-8 * sqrt(n); FP16 operands ~ 5e-4 * sqrt(n))."""
     rng = np.random.default_rng(n * 10 + kind)
     a = rng.uniform(-1, 1, (batch, n, n)).astype(np.float32)
     b = rng.uniform(-1, 1, (batch, n, n)).astype(np.float32)
+    if kind == 3:
+        b = b.astype(np.float16).astype(np.float32)
     cin = rng.uniform(-1, 1, (batch, n, n)).astype(np.float32)
     ref = a.astype(np.float64) @ b.astype(np.float64)
     scale = np.sqrt(n)
@@ -410,12 +414,14 @@ def test_pair_engines_density_tiny_and_mid(nolsm, tiny_system, tiny_solution, mi
 
 
 @pytest.mark.parametrize("flag", ["FLAG_PAIR", "FLAG_SINGLE"])
-@pytest.mark.parametrize("kind,tol", [(1, 2e-2), (2, 2e-5)])
+@pytest.mark.parametrize("kind,tol", [(1, 2e-2), (2, 2e-5), (3, 2e-5)])
 @pytest.mark.parametrize("n,batch", [(64, 3), (146, 5), (300, 2), (863, 2)])
 def test_pair_engines_building_block(nolsm, torch_mod, flag, kind, tol, n, batch):
     rng = np.random.default_rng(n * 7 + kind)
     a = rng.uniform(-1, 1, (batch, n, n)).astype(np.float32)
     b = rng.uniform(-1, 1, (batch, n, n)).astype(np.float32)
+    if kind == 3:   # half-split: the pair kernel runs it as two MMAs per K step, the single-CTA one as one stacked MMA
+        b = b.astype(np.float16).astype(np.float32)
     cin = rng.uniform(-1, 1, (batch, n, n)).astype(np.float32)
     ref = a.astype(np.float64) @ b.astype(np.float64)
     ctx = nolsm.Context(nolsm.Config(flags=getattr(nolsm, flag)))
