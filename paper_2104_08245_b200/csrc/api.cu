@@ -229,6 +229,8 @@ static nolsm_status setup_batch(nolsm_ctx *ctx, int slot, const std::vector<int3
   b->s32_built = true;
   b->s_norm_built = false;
   b->sinv_own_only = false;
+  b->x0_built = false;
+  b->b32_built = true;
   b->ld = ld;
   b->max_n = max_n;
   b->mol_begin = mol_begin;
@@ -566,8 +568,11 @@ static nolsm_status ensure_thin(nolsm_ctx *ctx, nolsm_batch *b, cudaStream_t st)
 
 // own_only (nolsm_solve_mu without energy products: nothing downstream reads S^-1 outside its six own columns):
 // the refinement is applied to B and to those columns instead of to all of S^-1, see below.
+// x0_mu (with own_only): the chemical potential of the ONE sign evaluation that will follow -- B is then never
+// written; B1's epilogue emits X0 = (B1 - mu I)/s_j as the split pair the sign iteration starts from.
 static nolsm_status prepare_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, int precision, cudaStream_t st,
-                                        nolsm_sign_stats *stats, int64_t *gemms, bool own_only) {
+                                        nolsm_sign_stats *stats, int64_t *gemms, bool own_only,
+                                        const double *x0_mu) {
   const bool fp16 = precision == NOLSM_FP16_FP32;
   const int refine = ctx->cfg.inv_refine >= 0 ? ctx->cfg.inv_refine : (fp16 ? 1 : 0);
   // one refinement, FP16 mode, one owner per submatrix: B1 = B0 + A0 (H - S B0) with B0 = A0 H and A0 = Z^2/s_S the
@@ -575,6 +580,9 @@ static nolsm_status prepare_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, int prec
   // (1 + 2 + 1) instead of seven (3 + 1 for the refinement, 3 for B on split operands); the own columns of S^-1
   // get their refinement as two thin products (launch_own_refine)
   const bool fast_b = own_only && fp16 && refine == 1 && b->sparse && b->row_ptr != nullptr && !b->grouped;
+  const bool x0_direct = fast_b && x0_mu != nullptr && (ctx->cfg.flags & NOLSM_FLAG_ORDER3) == 0;
+  b->x0_built = false;
+  b->b32_built = true;
   // 3e-3 with a refinement behind: the iterate is taken with a relative error of about twice its residual,
   // which the refinement squares (< 4e-5)
   const float inv_tol = ctx->cfg.inv_tol > 0.f ? ctx->cfg.inv_tol : (fp16 ? (refine > 0 ? 3e-3f : 1e-2f) : 1e-5f);
@@ -688,6 +696,7 @@ static nolsm_status prepare_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, int prec
     if (fp16) {               // Z16 in h2 / h3 (chain op z), Y16 buffers h0, h1 are free
       set2(o.a, 2, 3); set2(o.b, 2, 3);
       si_hi = 0; si_lo = 1;
+      if (x0_direct) si_hi = 4;   // the E buffer: h0 will receive X0 while A0 is still an operand
     } else {                  // split Z in (h4,h5) / (h6,h7), split Y buffers h0..h3 are free
       set2(o.a, 4, 6); set2(o.b, 4, 6);
       if (z_split) { set2(o.a_lo, 5, 7); set2(o.b_lo, 5, 7); }
@@ -724,8 +733,23 @@ static nolsm_status prepare_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, int prec
     p7.n_ops = 1;
     ChainOp &b1 = p7.ops[0] = make_op(EPI_AXPBY, 1.f, 1.f);
     set2(b1.a, si_hi, si_hi); set2(b1.b, 5, 5); set2(b1.cin16, 1, 1);
-    b1.cout32 = 3;
-    CHECK(run_chain(ctx, b, p7, nullptr, false, st));
+    if (x0_direct) {
+      // X0 = (B0 + A0 R - mu I)/s_j straight from the epilogue (hi -> h0, lo -> h2, where the sign iteration
+      // expects its iterate), s_j from the norm bound of B0 - mu I, 1 % up for B1 - B0 (which is <= 2 r ~ 0.6 %
+      // of B; the scale leaves 15 % to the edge of the convergence interval anyway, reading 5)
+      LAUNCH(ctx, launch_norm_bound16(b, b->h[1], (float)*x0_mu, b->d_norm, st));
+      LAUNCH(ctx, launch_x0_scale(b, b->d_norm, 1.01f, b->d_scale, st));
+      b1.use_div = 2;
+      b1.diag = -(float)*x0_mu;
+      set2(b1.out16, 0, 0); set2(b1.out16_lo, 2, 2);
+      CHECK(run_chain(ctx, b, p7, b->d_scale, false, st));
+      b->x0_built = true;
+      b->x0_mu = *x0_mu;
+      b->b32_built = false;
+    } else {
+      b1.cout32 = 3;
+      CHECK(run_chain(ctx, b, p7, nullptr, false, st));
+    }
     CHECK(ensure_thin(ctx, b, st));
     LAUNCH(ctx, launch_own_refine(b, b->row_ptr, b->col_idx, b->h[ss_hi], b->h[ss_lo], b->h[si_hi], b->d_thin, b->u[2], st));
     b->sinv_hi = b->sinv_lo = -1;
@@ -792,7 +816,11 @@ static nolsm_status sign_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, double mu, 
                                      bool timed, bool fold_last) {
   const bool fp16 = precision == NOLSM_FP16_FP32;
   float *Bm = b->u[3], *X32 = b->u[0];
-  if (!scale_in) LAUNCH(ctx, launch_norm_bound(b, Bm, (float)mu, false, b->d_norm, st));
+  // the prepare stage of the whole path may have left X0 for this mu in place (prepare_batch_chain, x0_mu)
+  const bool x0_ready = fp16 && b->x0_built && b->x0_mu == mu && !scale_in;
+  b->x0_built = false;
+  if (!x0_ready && !b->b32_built) { ctx->err = "this batch holds no B (its X0 was consumed)"; return NOLSM_EINVAL; }
+  if (!scale_in && !x0_ready) LAUNCH(ctx, launch_norm_bound(b, Bm, (float)mu, false, b->d_norm, st));
   ChainProgram pg;
   memset(&pg, 0, sizeof(pg));
   pg.n_ops = 2;
@@ -816,7 +844,8 @@ static nolsm_status sign_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, double mu, 
     // Master iterate as hi + lo * 2^-11 (22 bits, reading 12): hi IS the FP16 operand X16 (h0/h1,
     // ping-pong), lo lives in h2 and is updated in place by the thread that owns the element; E16: h4.
     // Per element and iteration the epilogues write 6 bytes (E, hi, lo) instead of 8 (E, FP32 master, FP16 copy).
-    LAUNCH(ctx, launch_make_x0(b, Bm, (float)mu, b->d_norm, scale_in, nullptr, b->h[0], b->h[2], b->d_scale, st));
+    if (!x0_ready)
+      LAUNCH(ctx, launch_make_x0(b, Bm, (float)mu, b->d_norm, scale_in, nullptr, b->h[0], b->h[2], b->d_scale, st));
     pg.group = group_size(ctx, b, 6);
     set2(e.a, 0, 1); set2(e.b, 0, 1); set2(e.out16, 4, 4);
     set2(x.a, 0, 1); set2(x.b, 4, 4); set2(x.cin16, 0, 1); set2(x.cin16_lo, 2, 2);
@@ -987,10 +1016,11 @@ static nolsm_status sign_batch_simt(nolsm_ctx *ctx, nolsm_batch *b, double mu, f
 }
 
 static nolsm_status prepare_batch(nolsm_ctx *ctx, nolsm_batch *b, int precision, cudaStream_t st,
-                                  nolsm_sign_stats *stats, int64_t *gemms, bool own_only = false) {
+                                  nolsm_sign_stats *stats, int64_t *gemms, bool own_only = false,
+                                  const double *x0_mu = nullptr) {
   b->sinv_own_only = false;
   if (use_simt(ctx)) return prepare_batch_simt(ctx, b, st, stats, gemms);
-  return prepare_batch_chain(ctx, b, precision, st, stats, gemms, own_only);
+  return prepare_batch_chain(ctx, b, precision, st, stats, gemms, own_only, x0_mu);
 }
 
 // timed: records ctx->tev[0..1] around the chain kernel; read with chain_ms() after a synchronise
@@ -1401,7 +1431,9 @@ extern "C" nolsm_status nolsm_solve_mu(nolsm_ctx *ctx, const nolsm_bsr *H, const
       nolsm_sign_stats bs;
       memset(&bs, 0, sizeof(bs));
       if (!b->prepared) {
-        rc = prepare_batch(ctx, b, prec, st, stats ? &bs : nullptr, &gemms, !ctx->eval_energy);
+        // a single N(mu) evaluation (the chemical potential is fixed): B itself is never needed
+        const bool single = max_steps == 1 && !cache && !ctx->eval_energy;
+        rc = prepare_batch(ctx, b, prec, st, stats ? &bs : nullptr, &gemms, !ctx->eval_energy, single ? &mu : nullptr);
         if (rc != NOLSM_OK) break;
         if (cache) {
           const size_t slab_all = cache_sq[bi];

@@ -296,7 +296,7 @@ struct EpiTile {
   const ChainOp *o;
   int par, n, col, h;         // col: this thread's column of the result; h: row quarter of every chunk
   bool split, ident, cin_direct;
-  float alpha, beta;
+  float alpha, beta, diag;
   float *p32;                 // FP32 output, element (first row of this warp's quarter, col) or null
   const float *cinp;          // FP32 master input (direct path), same position, or null
   EpiIO io;
@@ -325,7 +325,8 @@ __device__ __forceinline__ void epi_begin(const ChainArgs &args, const TileCmd &
   t.ident = o.mode == EPI_IDENT;
   t.cin_direct = !t.ident && o.cin32 >= 0 && o.beta != 0.f && t.io.in_hi < 0;
   t.alpha = o.use_div ? o.alpha / args.alpha_div[c.mat] : o.alpha;
-  t.beta = o.beta;
+  t.beta = o.use_div == 2 ? o.beta / args.alpha_div[c.mat] : o.beta;
+  t.diag = o.use_div == 2 ? o.diag / args.alpha_div[c.mat] : o.diag;
   if (args.alpha_tab != nullptr && cmd_iter(c) < kAlphaSteps) {
     // X_{k+1} = 1/2 a X (3I - a^2 X^2):  E = I - a^2 X X,  X' = a X + (1/2 a) X E
     const float a = args.alpha_tab[c.mat * kAlphaSteps + cmd_iter(c)];
@@ -347,7 +348,7 @@ __device__ __forceinline__ void epi_begin(const ChainArgs &args, const TileCmd &
 // ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ bool epi_fast_kind(const EpiTile &t, bool &ident) {
   ident = t.ident;
-  if (t.split || t.p32 != nullptr || t.cin_direct || kWarpRows != 32) return false;
+  if (t.split || t.p32 != nullptr || t.cin_direct || kWarpRows != 32 || t.diag != 0.f) return false;
   if (t.ident) return t.io.out_hi >= 0 && t.io.out_lo < 0;
   return t.io.in_hi >= 0 && t.io.in_lo >= 0 && t.io.out_hi >= 0 && t.io.out_lo >= 0;
 }
@@ -503,6 +504,12 @@ __device__ __forceinline__ float epi_chunks(const ChainArgs &args, const TileCmd
       } else {
 #pragma unroll
         for (int jj = 0; jj < R; ++jj) v[jj] = __float_as_uint(t.alpha * __uint_as_float(v[jj]));
+      }
+      if (t.diag != 0.f && !t.ident) {   // + diag * I: the chunk row that holds the diagonal element of this column
+        const int dj = t.col - (c.n0 + c0);
+#pragma unroll
+        for (int jj = 0; jj < R; ++jj)
+          if (jj == dj) v[jj] = __float_as_uint(__uint_as_float(v[jj]) + t.diag);
       }
       if (t.p32) {   // FP32 result (direct): 64 contiguous bytes of this thread's column
         float4 *qp = reinterpret_cast<float4 *>(t.p32);

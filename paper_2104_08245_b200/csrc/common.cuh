@@ -63,8 +63,9 @@ struct ChainOp {
                                   // (evict-first) loads and stores, so that they do not take L2 from the operands
   int32_t mode;                   // EPI_IDENT: I - A B     EPI_AXPBY: beta * Cin + alpha * A B
   int32_t resid;                  // 1: ||result||_F^2 over the true n x n part drives the stop rule
-  int32_t use_div;                // alpha /= alpha_div[submatrix]
+  int32_t use_div;                // 1: alpha /= alpha_div[submatrix]; 2: alpha, beta and diag
   float alpha, beta;
+  float diag;                     // AXPBY: + diag * I (after the division)
 };
 
 struct ChainProgram {
@@ -95,6 +96,9 @@ struct nolsm_batch {
   int32_t own_first = 0, own_count = 0;   // the batch's owners: g_own_idx[own_first, own_first + own_count)
   int32_t sinv_hi = -1, sinv_lo = -1;   // >= 0: S^-1 lives as the split pair h[sinv_hi] + h[sinv_lo] * 2^-11 and u[2] holds
   bool sinv32_full = true;              // only its own columns in FP32 until join_sinv (false)
+  bool x0_built = false;                // X0 for mu = x0_mu is in place (written by the prepare stage), d_scale set
+  double x0_mu = 0.0;
+  bool b32_built = true;                // u3 holds B (false: the whole path went from B0 straight to X0)
   bool sinv_own_only = false;           // S^-1 was refined in its own columns only (nolsm_solve_mu): no full S^-1
   int32_t sign_ops = 2;           // products per sign iteration of the last chain (3 with NOLSM_FLAG_ORDER3)
   bool x_split = false;           // the sign iterate lives as hi (h[iters & 1]) + lo * 2^-11 (h[2]); u[0] holds X in
@@ -236,6 +240,8 @@ cudaError_t launch_energy(const nolsm_batch *b, const int32_t *row_ptr, const fl
 // dense helpers
 cudaError_t launch_norm_bound(const nolsm_batch *b, const float *a, float mu, bool symmetric, float *norm2,
                               cudaStream_t st);
+cudaError_t launch_norm_bound16(const nolsm_batch *b, const __half *a, float mu, float *norm2, cudaStream_t st);
+cudaError_t launch_x0_scale(const nolsm_batch *b, const float *norm2, float slack, float *scale_out, cudaStream_t st);
 cudaError_t launch_init_inverse(const nolsm_batch *b, const float *s, const float *norm2, float *y32,
                                 float *z32, __half *y16, __half *z16, __half *y16_lo, __half *z16_lo,
                                 float *scale_out, cudaStream_t st);

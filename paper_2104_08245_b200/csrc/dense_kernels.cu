@@ -20,22 +20,34 @@ __device__ __forceinline__ void atomic_max_nonneg(float *addr, float v) {
 // floating-point atomics: the bound is bitwise reproducible.  For a symmetric matrix (S) the column part
 // is skipped and ||A||_1 = ||A||_inf.
 // ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void load4(const float *p, float (&v)[4]) {
+  const float4 q = *reinterpret_cast<const float4 *>(p);
+  v[0] = q.x; v[1] = q.y; v[2] = q.z; v[3] = q.w;
+}
+__device__ __forceinline__ void load4(const __half *p, float (&v)[4]) {
+  const uint2 q = *reinterpret_cast<const uint2 *>(p);
+  const float2 a = __half22float2(*reinterpret_cast<const __half2 *>(&q.x));
+  const float2 b = __half22float2(*reinterpret_cast<const __half2 *>(&q.y));
+  v[0] = a.x; v[1] = a.y; v[2] = b.x; v[3] = b.y;
+}
+
+template <typename T>
 __global__ void __launch_bounds__(256)
 k_norm_bound(const int32_t *__restrict__ dims, int ld, int64_t slab, int count, int strips,
-             const float *__restrict__ a, float mu, float *__restrict__ norm2, float *__restrict__ colpart) {
+             const T *__restrict__ a, float mu, float *__restrict__ norm2, float *__restrict__ colpart) {
   __shared__ float s_row[8][128];
   const int mat = blockIdx.y;
   const int n = dims[mat];
   const int base = blockIdx.x * 128;
   if (base >= n) return;
-  const float *aj = a + (int64_t)mat * slab;
+  const T *aj = a + (int64_t)mat * slab;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int r0 = base + 4 * lane;
   float racc[4] = {0.f, 0.f, 0.f, 0.f};
   float *cp = colpart ? colpart + ((int64_t)mat * strips + blockIdx.x) * ld : nullptr;
   for (int c = warp; c < n; c += 8) {
-    const float4 v4 = *reinterpret_cast<const float4 *>(aj + (int64_t)c * ld + r0);
-    float v[4] = {v4.x, v4.y, v4.z, v4.w};
+    float v[4];
+    load4(aj + (int64_t)c * ld + r0, v);
     float cs = 0.f;
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
@@ -89,16 +101,38 @@ k_colmax(const int32_t *__restrict__ dims, int ld, int count, int strips, const 
   }
 }
 
-cudaError_t launch_norm_bound(const nolsm_batch *b, const float *a, float mu, bool symmetric, float *norm2,
-                              cudaStream_t st) {
+template <typename T>
+static cudaError_t norm_bound_impl(const nolsm_batch *b, const T *a, float mu, bool symmetric, float *norm2,
+                                   cudaStream_t st) {
   if (b->count == 0) return cudaSuccess;
   cudaError_t e = cudaMemsetAsync(norm2, 0, sizeof(float) * 2 * b->count, st);
   if (e != cudaSuccess) return e;
   const int strips = (b->ld + 127) / 128;
   dim3 grid((b->max_n + 127) / 128, b->count);
-  k_norm_bound<<<grid, 256, 0, st>>>(b->d_dims, b->ld, (int64_t)b->ld * b->ld, b->count, strips, a, mu, norm2,
-                                     symmetric ? nullptr : b->d_colpart);
+  k_norm_bound<T><<<grid, 256, 0, st>>>(b->d_dims, b->ld, (int64_t)b->ld * b->ld, b->count, strips, a, mu, norm2,
+                                        symmetric ? nullptr : b->d_colpart);
   if (!symmetric) k_colmax<<<b->count, 256, 0, st>>>(b->d_dims, b->ld, b->count, strips, b->d_colpart, norm2);
+  return cudaGetLastError();
+}
+cudaError_t launch_norm_bound(const nolsm_batch *b, const float *a, float mu, bool symmetric, float *norm2,
+                              cudaStream_t st) {
+  return norm_bound_impl(b, a, mu, symmetric, norm2, st);
+}
+// the same bound from an FP16 matrix
+cudaError_t launch_norm_bound16(const nolsm_batch *b, const __half *a, float mu, float *norm2, cudaStream_t st) {
+  return norm_bound_impl(b, a, mu, false, norm2, st);
+}
+
+// s_j of X0 = (B - mu I)/s_j (reading 5) from the norm bound, inflated by `slack` where the bound was taken on an
+// approximation of the matrix
+__global__ void k_x0_scale(int count, const float *__restrict__ norm2, float factor, float slack,
+                           float *__restrict__ scale_out) {
+  const int m = blockIdx.x * blockDim.x + threadIdx.x;
+  if (m < count) scale_out[m] = fmaxf(slack * factor * sqrtf(norm2[m] * norm2[count + m]), 1e-30f);
+}
+cudaError_t launch_x0_scale(const nolsm_batch *b, const float *norm2, float slack, float *scale_out, cudaStream_t st) {
+  if (b->count == 0) return cudaSuccess;
+  k_x0_scale<<<(b->count + 255) / 256, 256, 0, st>>>(b->count, norm2, b->sign_scale, slack, scale_out);
   return cudaGetLastError();
 }
 

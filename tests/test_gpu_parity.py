@@ -337,6 +337,32 @@ def test_solve_mu_tiny(nolsm, tiny_system, tiny_solution, precision):
     ctx2.close()
 
 
+def test_single_evaluation_path_mid(nolsm, mid_system, mid_solution):
+    """A single N(mu) evaluation (fixed chemical potential; max_steps = 1) takes the shortest form of
+    the prepare stage in FP16 mode (reading 11): B is never written, X0 = (B0 + A0 R - mu I)/s_j comes out
+    of the last product's epilogue.  Same D, N and populations as the oracle, the same iteration counts as the
+    path that forms B (max_steps = 2 evaluates the same mu first), and D within rounding of that path."""
+    import oracle.nolsm_oracle as orc
+    sols = mid_solution["solutions"]
+    H, S = _device_system(nolsm, mid_system)
+    ctx = nolsm.Context(nolsm.Config(precision=0))
+    lo, hi = MU - 0.1, MU + 0.1
+    mu1, ne1, D1, st1 = ctx.solve_mu(H, S, mid_system.n_electrons, lo, hi, tol_ne_per_mol=-1.0, max_steps=1)
+    assert mu1 == MU
+    d_ref = orc.density_blocks(sols, mid_system.row_ptr, MU)
+    assert np.abs(D1.val.cpu().numpy() - d_ref).max() < TOL_D[0]
+    ne_ref = orc.electron_count(sols, MU)
+    assert abs(ne1 - ne_ref) / mid_system.n_mol <= TOL_NE_PER_MOL
+    # the general path: tolerance met at the first midpoint, but a second step was allowed, so B was formed
+    mu2, ne2, D2, st2 = ctx.solve_mu(H, S, mid_system.n_electrons, lo, hi, tol_ne_per_mol=1.0, max_steps=2)
+    assert mu2 == MU and st2.mu_steps == 1
+    assert (st1.last.iter_min, st1.last.iter_max) == (st2.last.iter_min, st2.last.iter_max)
+    # two FP16-mode evaluations with different scales s_j: each is ~2e-4 from the oracle (bound 5e-3)
+    assert np.abs(D1.val.cpu().numpy() - D2.val.cpu().numpy()).max() < 6e-4
+    assert abs(ne1 - ne2) / mid_system.n_mol < 2e-4
+    ctx.close()
+
+
 # ---------------------------------------------------------------------------------------------
 # BASELINE sizes, sampled (the oracle solves the sampled molecules one by one)
 # ---------------------------------------------------------------------------------------------
