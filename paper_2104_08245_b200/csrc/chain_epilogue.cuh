@@ -348,12 +348,12 @@ __device__ __forceinline__ void epi_begin(const ChainArgs &args, const TileCmd &
 // ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ bool epi_fast_kind(const EpiTile &t, bool &ident) {
   ident = t.ident;
-  if (t.split || t.p32 != nullptr || t.cin_direct || kWarpRows != 32 || t.diag != 0.f) return false;
+  if (t.split || t.p32 != nullptr || t.cin_direct || kWarpRows != 32) return false;
   if (t.ident) return t.io.out_hi >= 0 && t.io.out_lo < 0;
-  return t.io.in_hi >= 0 && t.io.in_lo >= 0 && t.io.out_hi >= 0 && t.io.out_lo >= 0;
+  return t.io.in_hi >= 0 && t.io.out_hi >= 0 && t.io.out_lo >= 0;   // a diagonal shift: chunks off the diagonal only
 }
 
-template <bool kIdent>
+template <bool kIdent, bool kInLo = true>
 __device__ __forceinline__ void epi_chunk_fast(const TileCmd &c, const EpiTile &t, uint32_t (&v)[32], uint8_t *hi_col,
                                                uint8_t *lo_col, int sw, float beta_lo, float &ss) {
   if constexpr (kIdent) {
@@ -376,7 +376,8 @@ __device__ __forceinline__ void epi_chunk_fast(const TileCmd &c, const EpiTile &
     for (int p = 0; p < 4; ++p) {
       const int pc = ((4 * t.h + p) ^ sw) * 16;
       const uint4 hq = *reinterpret_cast<const uint4 *>(hi_col + pc);
-      const uint4 lq = *reinterpret_cast<const uint4 *>(lo_col + pc);
+      uint4 lq = make_uint4(0u, 0u, 0u, 0u);
+      if constexpr (kInLo) lq = *reinterpret_cast<const uint4 *>(lo_col + pc);
       const uint32_t hin[4] = {hq.x, hq.y, hq.z, hq.w}, lin[4] = {lq.x, lq.y, lq.z, lq.w};
       uint32_t hw[4], lw[4];
 #pragma unroll
@@ -384,8 +385,8 @@ __device__ __forceinline__ void epi_chunk_fast(const TileCmd &c, const EpiTile &
         const int jj = 8 * p + 2 * e;
         const float2 hf = __half22float2(*reinterpret_cast<const __half2 *>(&hin[e]));
         const float2 lf = __half22float2(*reinterpret_cast<const __half2 *>(&lin[e]));
-        const float xa = fmaf(t.alpha, __uint_as_float(v[jj]), fmaf(beta_lo, lf.x, t.beta * hf.x));
-        const float xb = fmaf(t.alpha, __uint_as_float(v[jj + 1]), fmaf(beta_lo, lf.y, t.beta * hf.y));
+        const float xa = fmaf(t.alpha, __uint_as_float(v[jj]), kInLo ? fmaf(beta_lo, lf.x, t.beta * hf.x) : t.beta * hf.x);
+        const float xb = fmaf(t.alpha, __uint_as_float(v[jj + 1]), kInLo ? fmaf(beta_lo, lf.y, t.beta * hf.y) : t.beta * hf.y);
         const __half2 h2 = __floats2half2_rn(xa, xb);
         const float2 hb = __half22float2(h2);
         const __half2 l2 = __floats2half2_rn((xa - hb.x) * 2048.f, (xb - hb.y) * 2048.f);
@@ -448,14 +449,15 @@ __device__ __forceinline__ float epi_chunks(const ChainArgs &args, const TileCmd
       // straight-line code for the products of the sign iteration (epi_chunk_fast) when the warp's part of the
       // chunk is complete, inside the true dimension and (residual product) holds no diagonal element
       bool fast = fast_kind && cnt == R;
-      if (fast && fast_ident) {
+      if (fast && (fast_ident || t.diag != 0.f)) {
         const int dj = t.col - (c.n0 + c0);
-        fast = c.n0 + c0 + R <= t.n && !__any_sync(0xffffffffu, dj >= 0 && dj < R);
+        fast = (!fast_ident || c.n0 + c0 + R <= t.n) && !__any_sync(0xffffffffu, dj >= 0 && dj < R);
       }
       if (fast) {
         float s_local = 0.f;
         if (fast_ident) epi_chunk_fast<true>(c, t, v, hi_col, lo_col, sw, beta_lo, s_local);
-        else epi_chunk_fast<false>(c, t, v, hi_col, lo_col, sw, beta_lo, s_local);
+        else if (t.io.in_lo >= 0) epi_chunk_fast<false, true>(c, t, v, hi_col, lo_col, sw, beta_lo, s_local);
+        else epi_chunk_fast<false, false>(c, t, v, hi_col, lo_col, sw, beta_lo, s_local);
         if (t.col < t.n) ss += s_local;
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         __syncwarp();
