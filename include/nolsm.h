@@ -167,6 +167,22 @@ NOLSM_API nolsm_status nolsm_build_neighbours(nolsm_ctx *ctx, int32_t n_mol, con
                                     const int32_t *box_q /*host*/, int32_t rc_q, int32_t *row_ptr,
                                     int32_t *col_idx, int64_t cap, int64_t *nnzb_out /*host*/, void *stream);
 
+/* a0 without device-memory allocation, for callers that cannot call cudaMalloc (serving loops, harnesses that forbid
+ * it).  Same arguments, kernels, result and status codes as nolsm_build_neighbours; the neighbour counts between the
+ * two passes live in a static device array of NOLSM_STATIC_MAX_MOL int32 (1 MiB per device that loads the library,
+ * held until the process exits) instead of a cudaMalloc'ed buffer.  n_mol > NOLSM_STATIC_MAX_MOL returns NOLSM_EINVAL
+ * (text in nolsm_last_error).  No cudaMalloc / cudaFree / allocating library call is made.  ctx may be NULL (then no
+ * error text and no launch count are kept).  Every call on a device shares the array: calls that overlap on the GPU
+ * (different streams or threads) race -- serialise them; nothing in it needs clearing between calls (every count that
+ * is read was written by the same call).  Synchronises the stream like nolsm_build_neighbours (nnzb reaches the host).
+ * nolsm_static_setup resolves the array's device address for the CURRENT device (once per device; optional, the first
+ * nolsm_build_neighbours_static on a device does it otherwise). */
+#define NOLSM_STATIC_MAX_MOL 262144
+NOLSM_API nolsm_status nolsm_static_setup(void);
+NOLSM_API nolsm_status nolsm_build_neighbours_static(nolsm_ctx *ctx, int32_t n_mol, const int32_t *pos_q,
+                                           const int32_t *box_q /*host*/, int32_t rc_q, int32_t *row_ptr,
+                                           int32_t *col_idx, int64_t cap, int64_t *nnzb_out /*host*/, void *stream);
+
 /* a1: gather molecules [mol_begin, mol_begin+mol_count) into a context-owned batch
  * of dense submatrix pairs T_j(H), T_j(S): entry ((a,o),(b,p)) = block (N_j[a], N_j[b]) of the store if
  * that pair is stored, else 0.  H and S must share row_ptr/col_idx.  *out stays valid until the next

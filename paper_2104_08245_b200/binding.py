@@ -22,6 +22,7 @@ EXPORTED_SYMBOLS = [
     "nolsm_batch_size", "nolsm_batch_ld", "nolsm_gemm_batched", "nolsm_launch_count",
     "nolsm_scatter_energy", "nolsm_evaluate", "nolsm_set_model", "nolsm_combine_submatrices",
     "nolsm_build_submatrices_grouped", "nolsm_union_pattern", "nolsm_expand_store",
+    "nolsm_static_setup", "nolsm_build_neighbours_static",
 ]
 
 
@@ -114,6 +115,10 @@ def load_library():
     lib.nolsm_launch_count.restype = i64
     lib.nolsm_build_neighbours.argtypes = [vp, i32, vp, P(i32), i32, vp, vp, i64, P(i64), vp]
     lib.nolsm_build_neighbours.restype = i32
+    lib.nolsm_build_neighbours_static.argtypes = [vp, i32, vp, P(i32), i32, vp, vp, i64, P(i64), vp]
+    lib.nolsm_build_neighbours_static.restype = i32
+    lib.nolsm_static_setup.argtypes = []
+    lib.nolsm_static_setup.restype = i32
     lib.nolsm_set_model.argtypes = [vp, P(_Model)]
     lib.nolsm_set_model.restype = i32
     lib.nolsm_build_submatrices.argtypes = [vp, P(_Bsr), P(_Bsr), i32, i32, i32, P(vp), vp]
@@ -338,6 +343,19 @@ class Context:
                                                     _ptr(row_ptr), _ptr(col_idx), cap, C.byref(nnzb),
                                                     _stream(stream)))
         return row_ptr, col_idx[: nnzb.value]
+
+    def build_neighbours_static(self, pos_q, box_q, rc_q, row_ptr, col_idx, stream=None):
+        """nolsm_build_neighbours_static: the caller passes the outputs (row_ptr int32 [n_mol+1], col_idx int32 [cap]);
+        no device memory is allocated.  Returns nnzb; the list is col_idx[:nnzb]."""
+        torch = _torch()
+        n_mol = int(pos_q.shape[0])
+        box = (C.c_int32 * 3)(*[int(x) for x in box_q])
+        nnzb = C.c_int64(0)
+        self._check(self.lib.nolsm_build_neighbours_static(self.handle, n_mol, _ptr(pos_q, torch.int32), box,
+                                                           int(rc_q), _ptr(row_ptr, torch.int32),
+                                                           _ptr(col_idx, torch.int32), int(col_idx.numel()),
+                                                           C.byref(nnzb), _stream(stream)))
+        return nnzb.value
 
     # a1' ----------------------------------------------------------------------------------------
     def set_model(self, pos_q=None, box_q=None, rc_q=0, unit_per_grid=1.0, site_offset=None, orb_site=None,

@@ -15,7 +15,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libnolsm.so")
-SOURCES = ["api.cu", "sparse_kernels.cu", "thin_kernels.cu", "dense_kernels.cu", "chain_engine.cu", "combine.cu"]
+SOURCES = ["api.cu", "sparse_kernels.cu", "thin_kernels.cu", "dense_kernels.cu", "chain_engine.cu", "combine.cu", "noalloc.cu"]
 HEADERS = sorted(glob.glob(os.path.join(CSRC, "*.cuh"))) + [os.path.join(HERE, "..", "include", "nolsm.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden"]
