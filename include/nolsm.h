@@ -107,6 +107,10 @@ typedef struct {
                                   third-order member X <- X (I + 1/2 E + 3/8 E^2), E = I - X^2 (three products per
                                   iteration, residual E -> 5/8 E^3) instead of Eq. 9's second-order one.  FP16/FP32 mode
                                   only; the last iteration is then not folded into the density columns */
+#define NOLSM_FLAG_NO_PREDICT 64 /* Eq. 15-17, FP16 mode: do not use the a-priori stop (reading 11: from
+                                  ||E_k||_1 the bound 3/4 b^2 + 1/4 b^3 >= ||E_{k+1}||_2 is known before iteration k
+                                  is finished; when it is small enough only Z_{k+1} is formed).  With this flag every
+                                  stop is decided on a measured residual: two products more per submatrix, same iterate */
 #define NOLSM_FLAG_UNIT_SCALE 16 /* scale by the norm bound itself: Y0 = S/bound, X0 = A/bound (spectra in (0,1] and
                                   [-1,1]) instead of bound/2 and bound/1.5 (readings 5, 7); costs one
                                   iteration each */

@@ -217,7 +217,7 @@ static nolsm_status setup_batch(nolsm_ctx *ctx, int slot, const std::vector<int3
     b->meta_cap = cap;
   }
   {
-    const size_t need_cp = (size_t)count * ((ld + 127) / 128) * ld;
+    const size_t need_cp = (size_t)count * colpart_strips(ld) * ld;
     if (need_cp > b->colpart_cap) {
       cudaStreamSynchronize(st);
       if (grow(&b->d_colpart, need_cp)) { cudaGetLastError(); ctx->err = "cudaMalloc of the norm scratch failed"; return NOLSM_ENOMEM; }
@@ -623,10 +623,17 @@ static nolsm_status prepare_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, int prec
     pg.group = group_size(ctx, b, masters ? 18 : 10);
     ChainOp &e = pg.ops[0] = make_op(EPI_IDENT, 1.f, 0.f);
     set2(e.a, 3, 2); set2(e.b, 1, 0); set2(e.out16, 4, 4); e.resid = 1;
-    ChainOp &y = pg.ops[1] = make_op(EPI_AXPBY, 0.5f, 1.f);
-    set2(y.a, 1, 0); set2(y.b, 4, 4); y.cin32 = y.cout32 = 2; set2(y.out16, 0, 1);
-    ChainOp &z = pg.ops[2] = make_op(EPI_AXPBY, 0.5f, 1.f);
+    // Z before Y (they are independent given E): an a-priori stop ends the submatrix after the Z update
+    ChainOp &z = pg.ops[1] = make_op(EPI_AXPBY, 0.5f, 1.f);
     set2(z.a, 4, 4); set2(z.b, 3, 2); z.cin32 = z.cout32 = 3; set2(z.out16, 2, 3);
+    ChainOp &y = pg.ops[2] = make_op(EPI_AXPBY, 0.5f, 1.f);
+    set2(y.a, 1, 0); set2(y.b, 4, 4); y.cin32 = y.cout32 = 2; set2(y.out16, 0, 1);
+    if (pg.stop_early && (ctx->cfg.flags & NOLSM_FLAG_NO_PREDICT) == 0) {
+      // a-priori stop (ChainProgram::tol_pred, reading 11): ||E_{k+1}||_2 <= 2e-2 guaranteed from ||E_k||_1,
+      // i.e. a relative error of at most 2e-2 in every direction of A0, which the refinement squares
+      e.colnorm = 1;
+      pg.tol_pred = 2e-2f;
+    }
     if (lean) {   // Y1 = Y0 Z1 = (S_hi Z1)/s_S: plain product, scaled in the epilogue
       y1 = make_op(EPI_AXPBY, 1.f, 0.f);
       y1.use_div = 1;
@@ -667,11 +674,15 @@ static nolsm_status prepare_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, int prec
     std::vector<float> res(b->count);
     NOLSM_CUDA(ctx, cudaMemcpyAsync(it.data(), b->d_iters, sizeof(int32_t) * b->count, cudaMemcpyDeviceToHost, st));
     NOLSM_CUDA(ctx, cudaMemcpyAsync(res.data(), b->d_lastres, sizeof(float) * b->count, cudaMemcpyDeviceToHost, st));
+    std::vector<int32_t> how(b->count);   // state word of the chain: last op of the stopping iteration << 24
+    NOLSM_CUDA(ctx, cudaMemcpyAsync(how.data(), b->d_state, sizeof(int32_t) * b->count, cudaMemcpyDeviceToHost, st));
     NOLSM_CUDA(ctx, cudaStreamSynchronize(st));
     double fl = 0.0;
     for (int m = 0; m < b->count; ++m) {
-      // chain iterations carried out in full; a stop_early chain ran one residual product more
-      const int chain_products = 3 * it[m] + pg.stop_early;
+      // chain iterations carried out in full; a stop_early chain ran one residual product more; one that stopped
+      // a priori ran E and Z of its last iteration only
+      const bool ahead = ((how[m] >> 24) & 0x7f) == 1 && how[m] != 0x7fffffff;
+      const int chain_products = ahead ? 3 * it[m] - 1 : 3 * it[m] + pg.stop_early;
       it[m] += 1;   // iteration 0 ran in closed form
       stats->inv_iter_max = std::max(stats->inv_iter_max, it[m]);
       if (!(res[m] <= stats->inv_worst_residual)) stats->inv_worst_residual = res[m];

@@ -515,6 +515,16 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
       if (rows_in && t.o->resid) {
         for (int d = 16; d > 0; d >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, d);
         if (lane == 0) atomicAdd(&args.resid2[(size_t)(chainep::cmd_iter(c) % NOLSM_MAX_RESID_SLOTS) * args.count + c.mat], ss);
+        // column sums of |E| (thread = column; two threads, one per row half, and ntl tiles add to a column): the
+        // add returns the running total, and the largest running total of the product is its largest column sum
+        const int kk = chainep::cmd_iter(c);
+        if (t.colnorm && args.colsum != nullptr && kk < args.colslots) {
+          float tot = 0.f;
+          if (t.col < t.n)
+            tot = atomicAdd(&args.colsum[((size_t)kk * args.count + c.mat) * args.ld + t.col], t.abs_sum) + t.abs_sum;
+          for (int d = 16; d > 0; d >>= 1) tot = fmaxf(tot, __shfl_xor_sync(0xffffffffu, tot, d));
+          if (lane == 0) atomicMax(&args.colmax[(size_t)kk * args.count + c.mat], __float_as_int(tot));
+        }
       }
       // this warp's direct stores and residual atomic are issued: join the tile's completion
       __syncwarp();
@@ -753,12 +763,26 @@ cudaError_t launch_chain(nolsm_ctx *ctx, const nolsm_batch *b, const ChainProgra
   a.alpha_tab = prog.use_alpha_tab ? b->d_alpha : nullptr;
   a.tile_counter = b->d_tile_counter;
   a.resid2 = b->d_resid2;
+  a.colsum = nullptr;
+  a.colmax = nullptr;
+  a.colslots = 0;
+  const int strips = colpart_strips(b->ld);   // d_colpart: strips * count * ld floats (norm-bound scratch, free here)
+  for (int i = 0; i < prog.n_ops; ++i)
+    if (prog.ops[i].colnorm) {   // strips - 1 iteration slots of column sums, the last strip: maxima
+      a.colsum = b->d_colpart;
+      a.colslots = strips - 1;
+      a.colmax = reinterpret_cast<int32_t *>(b->d_colpart + (size_t)(strips - 1) * b->count * b->ld);
+    }
   a.lastres = b->d_lastres;
   const int slots = std::min(prog.max_iter, NOLSM_MAX_RESID_SLOTS);
   k_chain_reset<<<64, 256, 0, st>>>(b->count, a.window, a.slot_state, a.slot_done, a.sched, a.state, a.tile_counter,
                                     a.resid2, slots * b->count, a.iters, a.lastres, touch_stats ? 1 : 0);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
+  if (a.colsum != nullptr) {
+    e = cudaMemsetAsync(a.colsum, 0, sizeof(float) * (size_t)strips * b->count * b->ld, st);
+    if (e != cudaSuccess) return e;
+  }
   const size_t smem_bytes = (size_t)(a.stages * a.stage_bytes + chainep::kStagingBytes + 1024);
   if (!pair) {
     void *params[] = {&a};

@@ -59,6 +59,12 @@ struct ChainArgs {
   unsigned long long *tile_counter;   // next tile index to claim (dynamic, in-order scheduling)
   int32_t *state, *iters;
   float *resid2, *lastres;
+  // op with colnorm, iteration k < colslots: colsum[k][count][ld] column sums of |E_k| (zero at launch; every thread
+  // adds its rows' share and learns the running total), colmax[k][count] the largest running total seen = ||E_k||_1
+  // once the product is complete (totals only grow), as the bit pattern of a non-negative float
+  float *colsum;
+  int32_t *colmax;
+  int32_t colslots;
   // scaled Newton-Schulz start (nolsm_config.gap_hint): alpha_tab[m * kAlphaSteps + k] = alpha_k of submatrix m
   // for iteration k < kAlphaSteps (1 afterwards); null = the plain iteration
   const float *alpha_tab;
@@ -113,6 +119,13 @@ __device__ __forceinline__ void epi_complete(const ChainArgs &args, const TileCm
         &args.resid2[(size_t)(k % NOLSM_MAX_RESID_SLOTS) * args.count + c.mat]);
     const float res = (r2 == r2) ? sqrtf(fmaxf(r2, 0.f) / (float)n) : r2;   // fmaxf would swallow a NaN
     args.lastres[c.mat] = res;
+    // ||E_k||_1 (E_k is symmetric: >= ||E_k||_2) as the epilogues left it: the largest running total of a column sum
+    float pred = -1.f;
+    if (o.colnorm && args.colsum != nullptr && k < args.colslots) {
+      const float b1 = __int_as_float(*reinterpret_cast<volatile int32_t *>(
+          &args.colmax[(size_t)k * args.count + c.mat]));
+      pred = b1 * b1 * (0.75f + 0.25f * b1);   // >= ||E_{k+1}||_2 (ChainProgram::tol_pred)
+    }
     const bool conv = res < pg.tol;   // false for a NaN residual
     bool stop = pg.fixed_iter > 0 ? (k + 1 >= pg.fixed_iter) : (conv || !(res == res));
     // a scaled step (alpha_k > 1) measures ||I - alpha^2 X^2||, not the residual of the stop rule
@@ -123,16 +136,26 @@ __device__ __forceinline__ void epi_complete(const ChainArgs &args, const TileCm
     // ended by the cap or by a NaN, not by a passing residual: the submatrix counts as not converged
     if (stop && pg.fixed_iter <= 0 && !conv) atomicAdd(&args.sched[2], 1);
     args.iters[c.mat] = (stop && pg.stop_early) ? k : k + 1;   // iterations carried out in full
-    if (stop) *reinterpret_cast<volatile int32_t *>(&args.state[c.mat]) = k;
+    // state word: iteration that ends the chain | last op of that iteration << 24 (stop_early programs)
+    if (stop) {
+      *reinterpret_cast<volatile int32_t *>(&args.state[c.mat]) = k;
+    } else if (pg.tol_pred > 0.f && pg.stop_early && pg.fixed_iter <= 0 && res == res && pred >= 0.f &&
+               pred <= pg.tol_pred) {
+      // a-priori stop: the bound on the NEXT residual passes, so iteration k only forms Z_{k+1} (op 1)
+      args.lastres[c.mat] = pred;
+      *reinterpret_cast<volatile int32_t *>(&args.state[c.mat]) = k | (1 << 24);
+    }
   }
   const int32_t stv = *reinterpret_cast<volatile int32_t *>(&args.state[c.mat]);
+  const bool stopping = (stv & 0xffffff) == k;
   // stop_early: the residual product is op 0 and the remaining products of a passing iteration are not run
-  const bool early = pg.stop_early && o.resid && stv == k;
+  // (a-priori stop: those after op 1)
+  const int last_op = (stopping && pg.stop_early) ? ((stv >> 24) & 0x7f) : pg.n_ops - 1;
   const unsigned long long cur = *reinterpret_cast<volatile unsigned long long *>(&args.slot_state[c.slot]);
   const uint32_t round = slot_round(cur);
   args.slot_done[c.slot] = 0;
   unsigned long long next;
-  if (early || (c.op == pg.n_ops - 1 && (stv == k || k + 1 >= limit))) {
+  if ((stopping && c.op == last_op) || (c.op == pg.n_ops - 1 && k + 1 >= limit)) {
     // this submatrix is finished: the slot admits the next one of the batch, or retires
     const int32_t m2 = atomicAdd(&args.sched[0], 1);
     if (m2 < args.count) {
@@ -295,8 +318,9 @@ __device__ __forceinline__ void epi_agent_run(const ChainArgs &args, const TileC
 struct EpiTile {
   const ChainOp *o;
   int par, n, col, h;         // col: this thread's column of the result; h: row quarter of every chunk
-  bool split, ident, cin_direct;
+  bool split, ident, cin_direct, colnorm;
   float alpha, beta, diag;
+  float abs_sum;              // colnorm: sum of |result| over this thread's rows of the tile (true n x n part)
   float *p32;                 // FP32 output, element (first row of this warp's quarter, col) or null
   const float *cinp;          // FP32 master input (direct path), same position, or null
   EpiIO io;
@@ -324,6 +348,8 @@ __device__ __forceinline__ void epi_begin(const ChainArgs &args, const TileCmd &
   t.split = o.a_lo[t.par] >= 0;
   t.ident = o.mode == EPI_IDENT;
   t.cin_direct = !t.ident && o.cin32 >= 0 && o.beta != 0.f && t.io.in_hi < 0;
+  t.colnorm = t.ident && o.colnorm != 0;
+  t.abs_sum = 0.f;
   t.alpha = o.use_div ? o.alpha / args.alpha_div[c.mat] : o.alpha;
   t.beta = o.use_div == 2 ? o.beta / args.alpha_div[c.mat] : o.beta;
   t.diag = o.use_div == 2 ? o.diag / args.alpha_div[c.mat] : o.diag;
@@ -353,9 +379,9 @@ __device__ __forceinline__ bool epi_fast_kind(const EpiTile &t, bool &ident) {
   return t.io.in_hi >= 0 && t.io.out_hi >= 0 && t.io.out_lo >= 0;   // a diagonal shift: chunks off the diagonal only
 }
 
-template <bool kIdent, bool kInLo = true>
+template <bool kIdent, bool kInLo = true, bool kNorm = false>
 __device__ __forceinline__ void epi_chunk_fast(const TileCmd &c, const EpiTile &t, uint32_t (&v)[32], uint8_t *hi_col,
-                                               uint8_t *lo_col, int sw, float beta_lo, float &ss) {
+                                               uint8_t *lo_col, int sw, float beta_lo, float &ss, float *sa = nullptr) {
   if constexpr (kIdent) {
 #pragma unroll
     for (int p = 0; p < 4; ++p) {
@@ -366,6 +392,7 @@ __device__ __forceinline__ void epi_chunk_fast(const TileCmd &c, const EpiTile &
         const float ea = -t.alpha * __uint_as_float(v[jj]), eb = -t.alpha * __uint_as_float(v[jj + 1]);
         ss = fmaf(ea, ea, ss);
         ss = fmaf(eb, eb, ss);
+        if constexpr (kNorm) *sa += fabsf(ea) + fabsf(eb);
         const __half2 h2 = __floats2half2_rn(ea, eb);
         hw[e] = *reinterpret_cast<const uint32_t *>(&h2);
       }
@@ -454,11 +481,12 @@ __device__ __forceinline__ float epi_chunks(const ChainArgs &args, const TileCmd
         fast = (!fast_ident || c.n0 + c0 + R <= t.n) && !__any_sync(0xffffffffu, dj >= 0 && dj < R);
       }
       if (fast) {
-        float s_local = 0.f;
-        if (fast_ident) epi_chunk_fast<true>(c, t, v, hi_col, lo_col, sw, beta_lo, s_local);
+        float s_local = 0.f, a_local = 0.f;
+        if (fast_ident && t.colnorm) epi_chunk_fast<true, true, true>(c, t, v, hi_col, lo_col, sw, beta_lo, s_local, &a_local);
+        else if (fast_ident) epi_chunk_fast<true>(c, t, v, hi_col, lo_col, sw, beta_lo, s_local);
         else if (t.io.in_lo >= 0) epi_chunk_fast<false, true>(c, t, v, hi_col, lo_col, sw, beta_lo, s_local);
         else epi_chunk_fast<false, false>(c, t, v, hi_col, lo_col, sw, beta_lo, s_local);
-        if (t.col < t.n) ss += s_local;
+        if (t.col < t.n) { ss += s_local; t.abs_sum += a_local; }
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         __syncwarp();
         if (lane == 0) ebar_arrive(&bars.out_ready[b]);
@@ -500,7 +528,7 @@ __device__ __forceinline__ float epi_chunks(const ChainArgs &args, const TileCmd
 #pragma unroll
         for (int jj = 0; jj < R; ++jj) {
           const float e = fmaf(-t.alpha, __uint_as_float(v[jj]), (jj == dj) ? 1.f : 0.f);
-          if (jj < nvalid) ss = fmaf(e, e, ss);
+          if (jj < nvalid) { ss = fmaf(e, e, ss); if (t.colnorm) t.abs_sum += fabsf(e); }
           v[jj] = __float_as_uint(e);
         }
       } else {

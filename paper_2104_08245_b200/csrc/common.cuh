@@ -63,6 +63,8 @@ struct ChainOp {
                                   // (evict-first) loads and stores, so that they do not take L2 from the operands
   int32_t mode;                   // EPI_IDENT: I - A B     EPI_AXPBY: beta * Cin + alpha * A B
   int32_t resid;                  // 1: ||result||_F^2 over the true n x n part drives the stop rule
+  int32_t colnorm;                // 1 (with resid, EPI_IDENT): the column sums of |result| are accumulated too, so that
+                                  // ||result||_1 is known when the product completes (ChainProgram::tol_pred)
   int32_t use_div;                // 1: alpha /= alpha_div[submatrix]; 2: alpha, beta and diag
   float alpha, beta;
   float diag;                     // AXPBY: + diag * I (after the division)
@@ -80,7 +82,17 @@ struct ChainProgram {
   int32_t use_alpha_tab;          // 1: per-submatrix, per-iteration scaling alpha_k from nolsm_batch::d_alpha
   int32_t stop_early;             // 1: the iteration whose residual passes the test is NOT finished (its
                                   // remaining products are skipped); 0: it is (reading 9, "+1 rule")
+  float tol_pred;                 // > 0 (with stop_early, Eq. 15-17 only, ops ordered E, Z, Y): a-priori stop.  With
+                                  // E_k = I - Z_k Y_k symmetric, E_{k+1} = 3/4 E_k^2 + 1/4 E_k^3 exactly, hence
+                                  // ||E_{k+1}||_2 <= 3/4 b^2 + 1/4 b^3 with b = ||E_k||_1 >= ||E_k||_2.  When that bound
+                                  // is <= tol_pred, iteration k only runs its Z update (op 1) and the submatrix is
+                                  // done: Y_{k+1} and the product E_{k+1} that would only confirm it are never formed
 };
+
+// nolsm_batch::d_colpart holds colpart_strips(ld) * count * ld floats: the column partial sums of the norm bounds
+// (one strip per 128 rows) and, during a chain launch with an a-priori stop, four iteration slots of column sums
+// plus one strip of maxima (chain_engine.cu)
+inline int colpart_strips(int ld) { return std::max((ld + 127) / 128, 5); }
 
 struct nolsm_batch {
   int32_t count = 0, ld = 0, mol_begin = 0, max_n = 0, slot = 0;

@@ -22,3 +22,9 @@ def tiny_system():
 def tiny_solution(tiny_system):
     import oracle.nolsm_oracle as orc
     return orc.solve_system(tiny_system)
+
+
+@pytest.fixture(scope="session")
+def mid_system_cpu():
+    import nolsm_inputs as gi
+    return gi.make_water_system(216, 8.0)

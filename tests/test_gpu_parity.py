@@ -363,6 +363,28 @@ def test_single_evaluation_path_mid(nolsm, mid_system, mid_solution):
     ctx.close()
 
 
+@pytest.mark.parametrize("which", ["tiny", "mid"])
+def test_a_priori_stop_of_the_inverse_iteration(nolsm, tiny_system, mid_system, which):
+    """Eq. 15-17, FP16 mode (reading 11): from ||E_k||_1 the next residual is bounded before iteration k is
+    finished (E_{k+1} = 3/4 E_k^2 + 1/4 E_k^3; pinned on the oracle in test_oracle_pins.py); when the bound passes,
+    only Z_{k+1} is formed.  NOLSM_FLAG_NO_PREDICT decides every stop on a measured residual instead: it forms
+    Y_{k+1} and E_{k+1} as well and then takes the SAME Z_{k+1} -- so D must be bitwise equal and the product count
+    two per submatrix higher."""
+    system = tiny_system if which == "tiny" else mid_system
+    H, S = _device_system(nolsm, system)
+    out = {}
+    for flags in (0, nolsm.FLAG_NO_PREDICT):
+        ctx = nolsm.Context(nolsm.Config(precision=0, flags=flags))
+        mu, ne, D, st = ctx.solve_mu(H, S, system.n_electrons, MU - 0.1, MU + 0.1, tol_ne_per_mol=-1.0, max_steps=1)
+        out[flags] = (D.val.cpu().numpy().copy(), ne, st.last.gemms, st.last.inv_iter_max)
+        ctx.close()
+    ahead, measured = out[0], out[nolsm.FLAG_NO_PREDICT]
+    assert np.array_equal(ahead[0].view(np.uint32), measured[0].view(np.uint32))
+    assert abs(ahead[1] - measured[1]) <= 1e-9 * abs(measured[1])   # same D; the trace is summed with atomics
+    assert ahead[3] == measured[3]                                  # same number of Z updates
+    assert measured[2] - ahead[2] == 2 * system.n_mol               # Y_{k+1} and E_{k+1} were never formed
+
+
 # ---------------------------------------------------------------------------------------------
 # BASELINE sizes, sampled (the oracle solves the sampled molecules one by one)
 # ---------------------------------------------------------------------------------------------

@@ -239,6 +239,37 @@ def test_inverse_residual_recurrence_and_refined_early_stop(tiny_system):
     assert rel1 <= (np.linalg.cond(ssub) * rel0) ** 2 and rel1 < 1e-4
 
 
+def test_a_priori_bound_on_the_next_inverse_residual(tiny_system, mid_system_cpu):
+    """Reading 11, a-priori stop: E_k = I - Z_k Y_k is symmetric (a polynomial in S), so ||E_k||_2 <= ||E_k||_1 = b and
+    the recurrence above gives ||E_{k+1}||_2 <= 3/4 b^2 + 1/4 b^3 -- known BEFORE iteration k is finished.  When the
+    bound passes, Z_{k+1} alone is what the stopping rule needs; checked on the oracle's iterates of two systems, with
+    the iteration at which the CUDA path's tolerance (2e-2) is first met and the quality of the iterate it takes."""
+    for system, j in ((tiny_system, 9), (mid_system_cpu, 100)):
+        nb = system.col_idx[system.row_ptr[j]:system.row_ptr[j + 1]]
+        ssub = orc.dense_submatrix(system.row_ptr, system.col_idx, system.s_val, nb)
+        n = len(ssub)
+        eye = np.eye(n)
+        c = 0.5 * max(1.0, np.sqrt(np.abs(ssub).sum(0).max() * np.abs(ssub).sum(1).max()))
+        first = None
+        for k in range(0, 6):
+            _, zk, yk = orc.newton_schulz_inverse(ssub, k, scale=c)
+            _, zk1, yk1 = orc.newton_schulz_inverse(ssub, k + 1, scale=c)
+            e, e1 = eye - zk @ yk, eye - zk1 @ yk1
+            assert np.abs(e - e.T).max() < 1e-13
+            b = np.abs(e).sum(0).max()
+            bound = 0.75 * b * b + 0.25 * b ** 3
+            assert np.linalg.norm(e, 2) <= b * (1 + 1e-12)
+            assert np.linalg.norm(e1, 2) <= bound * (1 + 1e-9) + 1e-13   # + the FP64 rounding floor
+            if first is None and bound <= 2e-2:
+                first = k
+                # the iterate taken: Z_{k+1}.  Everything is a polynomial in S, so I - S Z^2/s IS E_{k+1}: S0 = Z^2/s
+                # has a relative residual of at most the bound in EVERY direction
+                s0 = zk1 @ zk1 / c
+                assert np.abs((eye - ssub @ s0) - e1).max() < 1e-12
+                assert np.linalg.norm(eye - ssub @ s0, 2) <= bound * (1 + 1e-9) + 1e-13
+        assert first is not None and 1 <= first <= 3
+
+
 def test_last_sign_update_folded_into_thin_products(tiny_system, tiny_solution):
     """Reading 9: with E_k = I - X_k^2, X_{k+1} V = X_k (V + 1/2 E_k V) for any thin V, so the own columns of
     D = 1/2 (I - X_{k+1}) S^-1 follow from X_k and E_k without forming X_{k+1}."""
