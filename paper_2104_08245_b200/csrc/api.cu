@@ -628,6 +628,7 @@ static nolsm_status prepare_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, int prec
     set2(z.a, 4, 4); set2(z.b, 3, 2); z.cin32 = z.cout32 = 3; set2(z.out16, 2, 3);
     ChainOp &y = pg.ops[2] = make_op(EPI_AXPBY, 0.5f, 1.f);
     set2(y.a, 1, 0); set2(y.b, 4, 4); y.cin32 = y.cout32 = 2; set2(y.out16, 0, 1);
+    pg.skip_tail = 1;   // without stop_early: the iteration that ends the chain does not form Y_{k+1}
     if (pg.stop_early && (ctx->cfg.flags & NOLSM_FLAG_NO_PREDICT) == 0) {
       // a-priori stop (ChainProgram::tol_pred, reading 11): ||E_{k+1}||_2 <= 2e-2 guaranteed from ||E_k||_1,
       // i.e. a relative error of at most 2e-2 in every direction of A0, which the refinement squares
@@ -656,12 +657,14 @@ static nolsm_status prepare_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, int prec
     ChainOp &e = pg.ops[0] = make_op(EPI_IDENT, 1.f, 0.f);
     set2(e.a, 6, 4); set2(e.a_lo, 7, 5); set2(e.b, 2, 0); set2(e.b_lo, 3, 1);
     set2(e.out16, 8, 8); set2(e.out16_lo, 9, 9); e.resid = 1;
-    ChainOp &y = pg.ops[1] = make_op(EPI_AXPBY, 0.5f, 1.f);
-    set2(y.a, 2, 0); set2(y.a_lo, 3, 1); set2(y.b, 8, 8); set2(y.b_lo, 9, 9);
-    set2(y.cin16, 2, 0); set2(y.cin16_lo, 3, 1); set2(y.out16, 0, 2); set2(y.out16_lo, 1, 3);
-    ChainOp &z = pg.ops[2] = make_op(EPI_AXPBY, 0.5f, 1.f);
+    // Z before Y: the iteration that ends the chain does not form Y_{k+1} (nothing reads it)
+    ChainOp &z = pg.ops[1] = make_op(EPI_AXPBY, 0.5f, 1.f);
     set2(z.a, 8, 8); set2(z.a_lo, 9, 9); set2(z.b, 6, 4); set2(z.b_lo, 7, 5);
     set2(z.cin16, 6, 4); set2(z.cin16_lo, 7, 5); set2(z.out16, 4, 6); set2(z.out16_lo, 5, 7);
+    ChainOp &y = pg.ops[2] = make_op(EPI_AXPBY, 0.5f, 1.f);
+    set2(y.a, 2, 0); set2(y.a_lo, 3, 1); set2(y.b, 8, 8); set2(y.b_lo, 9, 9);
+    set2(y.cin16, 2, 0); set2(y.cin16_lo, 3, 1); set2(y.out16, 0, 2); set2(y.out16_lo, 1, 3);
+    pg.skip_tail = 1;
   }
   CHECK(run_chain(ctx, b, p0, lean ? b->d_scale : nullptr, false, st));
   CHECK(run_chain(ctx, b, pg, nullptr, true, st));
@@ -682,7 +685,7 @@ static nolsm_status prepare_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, int prec
       // chain iterations carried out in full; a stop_early chain ran one residual product more; one that stopped
       // a priori ran E and Z of its last iteration only
       const bool ahead = ((how[m] >> 24) & 0x7f) == 1 && how[m] != 0x7fffffff;
-      const int chain_products = ahead ? 3 * it[m] - 1 : 3 * it[m] + pg.stop_early;
+      const int chain_products = ahead ? 3 * it[m] - 1 : 3 * it[m] + pg.stop_early - (pg.stop_early ? 0 : pg.skip_tail);
       it[m] += 1;   // iteration 0 ran in closed form
       stats->inv_iter_max = std::max(stats->inv_iter_max, it[m]);
       if (!(res[m] <= stats->inv_worst_residual)) stats->inv_worst_residual = res[m];

@@ -150,7 +150,7 @@ __device__ __forceinline__ void epi_complete(const ChainArgs &args, const TileCm
   const bool stopping = (stv & 0xffffff) == k;
   // stop_early: the residual product is op 0 and the remaining products of a passing iteration are not run
   // (a-priori stop: those after op 1)
-  const int last_op = (stopping && pg.stop_early) ? ((stv >> 24) & 0x7f) : pg.n_ops - 1;
+  const int last_op = !stopping ? pg.n_ops - 1 : (pg.stop_early ? ((stv >> 24) & 0x7f) : pg.n_ops - 1 - pg.skip_tail);
   const unsigned long long cur = *reinterpret_cast<volatile unsigned long long *>(&args.slot_state[c.slot]);
   const uint32_t round = slot_round(cur);
   args.slot_done[c.slot] = 0;
