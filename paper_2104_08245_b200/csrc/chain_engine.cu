@@ -2,8 +2,8 @@
 // dependent n x n x n products (every iteration of Eq. 9-10, or of Eq. 15-17
 // PAPER.md:203-215) for every submatrix of a batch on the 5th-generation tensor cores
 // (tcgen05 + TMEM + TMA), sm_100a only.  Two instantiations of one kernel template:
-//   k_chain<false>  one CTA per tile of N rows x 128 columns of the result (tcgen05.mma.cta_group::1)
-//   k_chain<true>   two CTAs of a cluster (one TPC) per tile of N rows x 256 columns (cta_group::2): each CTA stages
+//   k_chain<false, *>  one CTA per tile of N rows x 128 columns of the result (tcgen05.mma.cta_group::1)
+//   k_chain<true, *>   two CTAs of a cluster (one TPC) per tile of N rows x 256 columns (cta_group::2): each CTA stages
 //                   its own 128 columns of the right operand and only HALF of the rows of the left operand, so the
 //                   operand bytes an SM takes in per 64-deep K block drop from 48 KB to 32 KB.
 //
@@ -239,7 +239,8 @@ __device__ __forceinline__ int32_t ld_acquire(const int32_t *p) {
 using chainep::TileCmd;
 using chainep::ChainArgs;
 
-template <bool kPair>
+// kLean: program_is_lean(args.prog) -- only plain FP16 products with FP16 staging input / output (see epi_begin)
+template <bool kPair, bool kLean>
 __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
   constexpr int kCtas = kPair ? 2 : 1;
   constexpr int kTileM = NOLSM_TILE_M * kCtas;      // rows of a tile
@@ -373,7 +374,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
         const int m0 = c.m0 + NOLSM_TILE_M * (int)rank;       // this CTA's columns of the result tile
         const int my_n = kPair ? (c.nt >> 1) : c.nt;          // this CTA's share of the tile's rows (N side)
         const int n0 = c.n0 + (kPair ? my_n * (int)rank : 0);
-        const bool split = o.a_lo[par] >= 0;
+        const bool split = !kLean && o.a_lo[par] >= 0;
         // only the left operand split (the right one is exact in FP16): no lo part on the M side, and the lo
         // boxes of the N side follow its hi boxes, so that one MMA can take both (see the issuer)
         const bool half = split && o.b_lo[par] < 0;
@@ -425,7 +426,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
         if (one) mbar_arrive<kPair>(&cmd_empty[slot], 0);
         if (++slot == kRing) { slot = 0; ring_phase ^= 1u; }
         if (c.op < 0) break;
-        const bool split = pg.ops[c.op].a_lo[chainep::cmd_par(c)] >= 0;
+        const bool split = !kLean && pg.ops[c.op].a_lo[chainep::cmd_par(c)] >= 0;
         const bool half = split && pg.ops[c.op].b_lo[chainep::cmd_par(c)] < 0;
         // split, one CTA, 128-row tiles: the lo boxes of the N side start exactly 128 rows behind the hi boxes, and
         // the correction accumulator 128 columns behind the main one -- ONE MMA of N = 128 + nt forms
@@ -499,7 +500,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
       // the peer's half of the last pair tile may lie beyond the leading dimension: nothing to load or store
       const bool rows_in = c.m0 + NOLSM_TILE_M * (int)rank < args.ld;
       chainep::EpiTile t;
-      if (rows_in) chainep::epi_begin(args, c, c.m0 + NOLSM_TILE_M * (int)rank + q * 32 + lane, h, t);
+      if (rows_in) chainep::epi_begin<kLean>(args, c, c.m0 + NOLSM_TILE_M * (int)rank + q * 32 + lane, h, t);
       mbar_wait<kPair>(&tfull_bar[acc], acc_phase);
       tc_fence_after();
       const uint32_t t_main = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(acc * 256);
@@ -642,7 +643,8 @@ nolsm_status encode_map(nolsm_ctx *ctx, CUtensorMap *map, void *ptr, int ld, int
 // all pairs must be co-resident: the CTAs wait on one another through global flags
 void pair_init(nolsm_ctx *ctx) {
   ctx->pair_ok = false;
-  cudaError_t e = cudaFuncSetAttribute(k_chain<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit);
+  cudaError_t e = cudaFuncSetAttribute(k_chain<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_chain<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit);
   if (e != cudaSuccess) { cudaGetLastError(); return; }
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3((unsigned)(ctx->sm_count & ~1));
@@ -654,7 +656,7 @@ void pair_init(nolsm_ctx *ctx) {
   cfg.attrs = at;
   cfg.numAttrs = 1;
   int max_clusters = 0;
-  e = cudaOccupancyMaxActiveClusters(&max_clusters, k_chain<true>, &cfg);
+  e = cudaOccupancyMaxActiveClusters(&max_clusters, k_chain<true, false>, &cfg);
   if (e != cudaSuccess || max_clusters < 1) { cudaGetLastError(); return; }
   ctx->pair_clusters = std::min(max_clusters, ctx->sm_count / 2);
   ctx->pair_ok = true;
@@ -673,7 +675,8 @@ nolsm_status umma_init(nolsm_ctx *ctx) {
     return NOLSM_ECUDA;
   }
   ctx->encode_tiled = fn;
-  e = cudaFuncSetAttribute(k_chain<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit);
+  e = cudaFuncSetAttribute(k_chain<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_chain<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit);
   if (e != cudaSuccess) {
     ctx->err = std::string("cudaFuncSetAttribute(k_chain): ") + cudaGetErrorString(e);
     cudaGetLastError();
@@ -717,6 +720,17 @@ nolsm_status umma_make_maps(nolsm_ctx *ctx, nolsm_batch *b) {
   NOLSM_CUDA(ctx, cudaMemcpy(b->d_maps, maps.data(), sizeof(CUtensorMap) * maps.size(), cudaMemcpyHostToDevice));
   b->maps_valid = true;
   return NOLSM_OK;
+}
+
+// Programs the lean kernel instantiation can run (chain_epilogue.cuh: epi_begin<kLean>)
+static bool program_is_lean(const ChainProgram &prog) {
+  if (prog.use_alpha_tab) return false;
+  for (int i = 0; i < prog.n_ops; ++i) {
+    const ChainOp &o = prog.ops[i];
+    if (o.a_lo[0] >= 0 || o.a_lo[1] >= 0 || o.cin32 >= 0 || o.cout32 >= 0 || o.colnorm || o.diag != 0.f || o.use_div == 2)
+      return false;
+  }
+  return true;
 }
 
 // Runs `prog` over every submatrix of the batch.  touch_stats: reset and fill iters / lastres.
@@ -784,10 +798,12 @@ cudaError_t launch_chain(nolsm_ctx *ctx, const nolsm_batch *b, const ChainProgra
     if (e != cudaSuccess) return e;
   }
   const size_t smem_bytes = (size_t)(a.stages * a.stage_bytes + chainep::kStagingBytes + 1024);
+  const bool lean = program_is_lean(prog);
   if (!pair) {
     void *params[] = {&a};
-    return cudaLaunchCooperativeKernel(reinterpret_cast<void *>(k_chain<false>), dim3(ctx->sm_count), dim3(kThreads),
-                                       params, smem_bytes, st);
+    return cudaLaunchCooperativeKernel(lean ? reinterpret_cast<void *>(k_chain<false, true>)
+                                            : reinterpret_cast<void *>(k_chain<false, false>),
+                                       dim3(ctx->sm_count), dim3(kThreads), params, smem_bytes, st);
   }
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3((unsigned)(2 * ctx->pair_clusters));
@@ -801,5 +817,5 @@ cudaError_t launch_chain(nolsm_ctx *ctx, const nolsm_batch *b, const ChainProgra
   at[1].val.cooperative = 1;
   cfg.attrs = at;
   cfg.numAttrs = 2;
-  return cudaLaunchKernelEx(&cfg, k_chain<true>, a);
+  return lean ? cudaLaunchKernelEx(&cfg, k_chain<true, true>, a) : cudaLaunchKernelEx(&cfg, k_chain<true, false>, a);
 }

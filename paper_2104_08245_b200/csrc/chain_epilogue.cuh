@@ -337,6 +337,11 @@ __device__ __forceinline__ void epi_prefetch32(EpiTile &t) {
 }
 
 // Before waiting for the accumulator.  col: this thread's column of the result; h: row quarter of the chunks.
+// kLean: the program was checked on the host (chain_engine.cu: program_is_lean) to use plain FP16 operands, FP16 staging
+// input and output only, no diagonal shift, no column norms and no scaling table -- the flags below become compile-time
+// constants and the code for everything else drops out of the kernel (the sign iteration's two products are such a
+// program, and the compute warps' code decides the kernel's register budget).
+template <bool kLean>
 __device__ __forceinline__ void epi_begin(const ChainArgs &args, const TileCmd &c, int col, int h, EpiTile &t) {
   const ChainOp &o = args.prog.ops[c.op];
   t.o = &o;
@@ -345,12 +350,21 @@ __device__ __forceinline__ void epi_begin(const ChainArgs &args, const TileCmd &
   t.col = col;
   t.h = h;
   t.io = epi_io(args, c);
-  t.split = o.a_lo[t.par] >= 0;
   t.ident = o.mode == EPI_IDENT;
-  t.cin_direct = !t.ident && o.cin32 >= 0 && o.beta != 0.f && t.io.in_hi < 0;
-  t.colnorm = t.ident && o.colnorm != 0;
   t.abs_sum = 0.f;
   t.alpha = o.use_div ? o.alpha / args.alpha_div[c.mat] : o.alpha;
+  if constexpr (kLean) {
+    t.io.out32 = -1;
+    t.split = t.cin_direct = t.colnorm = false;
+    t.beta = o.beta;
+    t.diag = 0.f;
+    t.p32 = nullptr;
+    t.cinp = nullptr;
+    return;
+  }
+  t.split = o.a_lo[t.par] >= 0;
+  t.cin_direct = !t.ident && o.cin32 >= 0 && o.beta != 0.f && t.io.in_hi < 0;
+  t.colnorm = t.ident && o.colnorm != 0;
   t.beta = o.use_div == 2 ? o.beta / args.alpha_div[c.mat] : o.beta;
   t.diag = o.use_div == 2 ? o.diag / args.alpha_div[c.mat] : o.diag;
   if (args.alpha_tab != nullptr && cmd_iter(c) < kAlphaSteps) {
