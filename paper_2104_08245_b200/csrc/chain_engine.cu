@@ -239,8 +239,9 @@ __device__ __forceinline__ int32_t ld_acquire(const int32_t *p) {
 using chainep::TileCmd;
 using chainep::ChainArgs;
 
-// kLean: program_is_lean(args.prog) -- only plain FP16 products with FP16 staging input / output (see epi_begin)
-template <bool kPair, bool kLean>
+// kLean = program_lean_mode(args.prog): 1 only plain FP16 products, 2 only full-split products, both with FP16 staging
+// input / output and nothing else (see epi_begin); 0 anything
+template <bool kPair, int kLean>
 __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
   constexpr int kCtas = kPair ? 2 : 1;
   constexpr int kTileM = NOLSM_TILE_M * kCtas;      // rows of a tile
@@ -374,10 +375,10 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
         const int m0 = c.m0 + NOLSM_TILE_M * (int)rank;       // this CTA's columns of the result tile
         const int my_n = kPair ? (c.nt >> 1) : c.nt;          // this CTA's share of the tile's rows (N side)
         const int n0 = c.n0 + (kPair ? my_n * (int)rank : 0);
-        const bool split = !kLean && o.a_lo[par] >= 0;
+        const bool split = kLean == 2 || (kLean == 0 && o.a_lo[par] >= 0);
         // only the left operand split (the right one is exact in FP16): no lo part on the M side, and the lo
         // boxes of the N side follow its hi boxes, so that one MMA can take both (see the issuer)
-        const bool half = split && o.b_lo[par] < 0;
+        const bool half = kLean == 0 && split && o.b_lo[par] < 0;
         const int nbox = (my_n + 63) >> 6;
         const uint32_t bytes = (uint32_t)kCtas * (uint32_t)(kATileBytes * (split && !half ? 2 : 1) +
                                                             nbox * kBoxBytes * (split ? 2 : 1));
@@ -426,8 +427,8 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
         if (one) mbar_arrive<kPair>(&cmd_empty[slot], 0);
         if (++slot == kRing) { slot = 0; ring_phase ^= 1u; }
         if (c.op < 0) break;
-        const bool split = !kLean && pg.ops[c.op].a_lo[chainep::cmd_par(c)] >= 0;
-        const bool half = split && pg.ops[c.op].b_lo[chainep::cmd_par(c)] < 0;
+        const bool split = kLean == 2 || (kLean == 0 && pg.ops[c.op].a_lo[chainep::cmd_par(c)] >= 0);
+        const bool half = kLean == 0 && split && pg.ops[c.op].b_lo[chainep::cmd_par(c)] < 0;
         // split, one CTA, 128-row tiles: the lo boxes of the N side start exactly 128 rows behind the hi boxes, and
         // the correction accumulator 128 columns behind the main one -- ONE MMA of N = 128 + nt forms
         // [A_hi B_hi | A_hi B_lo] and reads the M-side tile once (columns nt..127 are never read back); a full
@@ -643,8 +644,9 @@ nolsm_status encode_map(nolsm_ctx *ctx, CUtensorMap *map, void *ptr, int ld, int
 // all pairs must be co-resident: the CTAs wait on one another through global flags
 void pair_init(nolsm_ctx *ctx) {
   ctx->pair_ok = false;
-  cudaError_t e = cudaFuncSetAttribute(k_chain<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_chain<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit);
+  cudaError_t e = cudaFuncSetAttribute(k_chain<true, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_chain<true, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_chain<true, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit);
   if (e != cudaSuccess) { cudaGetLastError(); return; }
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3((unsigned)(ctx->sm_count & ~1));
@@ -656,7 +658,7 @@ void pair_init(nolsm_ctx *ctx) {
   cfg.attrs = at;
   cfg.numAttrs = 1;
   int max_clusters = 0;
-  e = cudaOccupancyMaxActiveClusters(&max_clusters, k_chain<true, false>, &cfg);
+  e = cudaOccupancyMaxActiveClusters(&max_clusters, k_chain<true, 0>, &cfg);
   if (e != cudaSuccess || max_clusters < 1) { cudaGetLastError(); return; }
   ctx->pair_clusters = std::min(max_clusters, ctx->sm_count / 2);
   ctx->pair_ok = true;
@@ -675,8 +677,9 @@ nolsm_status umma_init(nolsm_ctx *ctx) {
     return NOLSM_ECUDA;
   }
   ctx->encode_tiled = fn;
-  e = cudaFuncSetAttribute(k_chain<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_chain<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit);
+  e = cudaFuncSetAttribute(k_chain<false, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_chain<false, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_chain<false, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit);
   if (e != cudaSuccess) {
     ctx->err = std::string("cudaFuncSetAttribute(k_chain): ") + cudaGetErrorString(e);
     cudaGetLastError();
@@ -722,15 +725,20 @@ nolsm_status umma_make_maps(nolsm_ctx *ctx, nolsm_batch *b) {
   return NOLSM_OK;
 }
 
-// Programs the lean kernel instantiation can run (chain_epilogue.cuh: epi_begin<kLean>)
-static bool program_is_lean(const ChainProgram &prog) {
-  if (prog.use_alpha_tab) return false;
+// Which lean kernel instantiation can run the program (chain_epilogue.cuh: epi_begin<kLean>): 1 all products plain
+// FP16, 2 all products full-split, 0 neither
+static int program_lean_mode(const ChainProgram &prog) {
+  if (prog.use_alpha_tab) return 0;
+  int n_split = 0;
   for (int i = 0; i < prog.n_ops; ++i) {
     const ChainOp &o = prog.ops[i];
-    if (o.a_lo[0] >= 0 || o.a_lo[1] >= 0 || o.cin32 >= 0 || o.cout32 >= 0 || o.colnorm || o.diag != 0.f || o.use_div == 2)
-      return false;
+    if (o.cin32 >= 0 || o.cout32 >= 0 || o.colnorm || o.diag != 0.f || o.use_div == 2) return 0;
+    const bool s0 = o.a_lo[0] >= 0 && o.b_lo[0] >= 0, s1 = o.a_lo[1] >= 0 && o.b_lo[1] >= 0;
+    const bool p0 = o.a_lo[0] < 0 && o.b_lo[0] < 0, p1 = o.a_lo[1] < 0 && o.b_lo[1] < 0;
+    if (s0 && s1) ++n_split;
+    else if (!(p0 && p1)) return 0;   // half-split or different by parity
   }
-  return true;
+  return n_split == 0 ? 1 : (n_split == prog.n_ops ? 2 : 0);
 }
 
 // Runs `prog` over every submatrix of the batch.  touch_stats: reset and fill iters / lastres.
@@ -798,12 +806,12 @@ cudaError_t launch_chain(nolsm_ctx *ctx, const nolsm_batch *b, const ChainProgra
     if (e != cudaSuccess) return e;
   }
   const size_t smem_bytes = (size_t)(a.stages * a.stage_bytes + chainep::kStagingBytes + 1024);
-  const bool lean = program_is_lean(prog);
+  const int lean = program_lean_mode(prog);
   if (!pair) {
     void *params[] = {&a};
-    return cudaLaunchCooperativeKernel(lean ? reinterpret_cast<void *>(k_chain<false, true>)
-                                            : reinterpret_cast<void *>(k_chain<false, false>),
-                                       dim3(ctx->sm_count), dim3(kThreads), params, smem_bytes, st);
+    void *fn = lean == 1 ? reinterpret_cast<void *>(k_chain<false, 1>)
+                         : lean == 2 ? reinterpret_cast<void *>(k_chain<false, 2>) : reinterpret_cast<void *>(k_chain<false, 0>);
+    return cudaLaunchCooperativeKernel(fn, dim3(ctx->sm_count), dim3(kThreads), params, smem_bytes, st);
   }
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3((unsigned)(2 * ctx->pair_clusters));
@@ -817,5 +825,6 @@ cudaError_t launch_chain(nolsm_ctx *ctx, const nolsm_batch *b, const ChainProgra
   at[1].val.cooperative = 1;
   cfg.attrs = at;
   cfg.numAttrs = 2;
-  return lean ? cudaLaunchKernelEx(&cfg, k_chain<true, true>, a) : cudaLaunchKernelEx(&cfg, k_chain<true, false>, a);
+  return lean == 1 ? cudaLaunchKernelEx(&cfg, k_chain<true, 1>, a)
+                   : lean == 2 ? cudaLaunchKernelEx(&cfg, k_chain<true, 2>, a) : cudaLaunchKernelEx(&cfg, k_chain<true, 0>, a);
 }

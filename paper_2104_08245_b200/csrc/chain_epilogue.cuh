@@ -337,11 +337,12 @@ __device__ __forceinline__ void epi_prefetch32(EpiTile &t) {
 }
 
 // Before waiting for the accumulator.  col: this thread's column of the result; h: row quarter of the chunks.
-// kLean: the program was checked on the host (chain_engine.cu: program_is_lean) to use plain FP16 operands, FP16 staging
-// input and output only, no diagonal shift, no column norms and no scaling table -- the flags below become compile-time
-// constants and the code for everything else drops out of the kernel (the sign iteration's two products are such a
-// program, and the compute warps' code decides the kernel's register budget).
-template <bool kLean>
+// kLean != 0: the program was checked on the host (chain_engine.cu: program_lean_mode) to use FP16 staging input and
+// output only, no diagonal shift, no column norms and no scaling table, and operands that are all plain FP16 (1) or all
+// full-split pairs (2) -- the flags below become compile-time constants and the code for everything else drops out of
+// the kernel (the sign iteration's two products are such a program in either precision mode, and the compute warps'
+// code decides the kernel's register budget).
+template <int kLean>
 __device__ __forceinline__ void epi_begin(const ChainArgs &args, const TileCmd &c, int col, int h, EpiTile &t) {
   const ChainOp &o = args.prog.ops[c.op];
   t.o = &o;
@@ -353,9 +354,10 @@ __device__ __forceinline__ void epi_begin(const ChainArgs &args, const TileCmd &
   t.ident = o.mode == EPI_IDENT;
   t.abs_sum = 0.f;
   t.alpha = o.use_div ? o.alpha / args.alpha_div[c.mat] : o.alpha;
-  if constexpr (kLean) {
+  if constexpr (kLean != 0) {
     t.io.out32 = -1;
-    t.split = t.cin_direct = t.colnorm = false;
+    t.split = kLean == 2;
+    t.cin_direct = t.colnorm = false;
     t.beta = o.beta;
     t.diag = 0.f;
     t.p32 = nullptr;
