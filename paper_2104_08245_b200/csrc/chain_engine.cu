@@ -239,9 +239,8 @@ __device__ __forceinline__ int32_t ld_acquire(const int32_t *p) {
 using chainep::TileCmd;
 using chainep::ChainArgs;
 
-// kLean = program_lean_mode(args.prog): 1 only plain FP16 products, 2 only full-split products, both with FP16 staging
-// input / output and nothing else (see epi_begin); 0 anything
-template <bool kPair, int kLean>
+// kFeat: feature bits of chain_epilogue.cuh (kFeat*); launch_chain picks the smallest instantiation that covers a program
+template <bool kPair, int kFeat>
 __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
   constexpr int kCtas = kPair ? 2 : 1;
   constexpr int kTileM = NOLSM_TILE_M * kCtas;      // rows of a tile
@@ -375,10 +374,10 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
         const int m0 = c.m0 + NOLSM_TILE_M * (int)rank;       // this CTA's columns of the result tile
         const int my_n = kPair ? (c.nt >> 1) : c.nt;          // this CTA's share of the tile's rows (N side)
         const int n0 = c.n0 + (kPair ? my_n * (int)rank : 0);
-        const bool split = kLean == 2 || (kLean == 0 && o.a_lo[par] >= 0);
+        const bool split = (kFeat & chainep::kFeatSplitAll) != 0 || ((kFeat & chainep::kFeatSplitAny) != 0 && o.a_lo[par] >= 0);
         // only the left operand split (the right one is exact in FP16): no lo part on the M side, and the lo
         // boxes of the N side follow its hi boxes, so that one MMA can take both (see the issuer)
-        const bool half = kLean == 0 && split && o.b_lo[par] < 0;
+        const bool half = (kFeat & chainep::kFeatSplitAny) != 0 && split && o.b_lo[par] < 0;
         const int nbox = (my_n + 63) >> 6;
         const uint32_t bytes = (uint32_t)kCtas * (uint32_t)(kATileBytes * (split && !half ? 2 : 1) +
                                                             nbox * kBoxBytes * (split ? 2 : 1));
@@ -427,8 +426,9 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
         if (one) mbar_arrive<kPair>(&cmd_empty[slot], 0);
         if (++slot == kRing) { slot = 0; ring_phase ^= 1u; }
         if (c.op < 0) break;
-        const bool split = kLean == 2 || (kLean == 0 && pg.ops[c.op].a_lo[chainep::cmd_par(c)] >= 0);
-        const bool half = kLean == 0 && split && pg.ops[c.op].b_lo[chainep::cmd_par(c)] < 0;
+        const bool split = (kFeat & chainep::kFeatSplitAll) != 0 ||
+                           ((kFeat & chainep::kFeatSplitAny) != 0 && pg.ops[c.op].a_lo[chainep::cmd_par(c)] >= 0);
+        const bool half = (kFeat & chainep::kFeatSplitAny) != 0 && split && pg.ops[c.op].b_lo[chainep::cmd_par(c)] < 0;
         // split, one CTA, 128-row tiles: the lo boxes of the N side start exactly 128 rows behind the hi boxes, and
         // the correction accumulator 128 columns behind the main one -- ONE MMA of N = 128 + nt forms
         // [A_hi B_hi | A_hi B_lo] and reads the M-side tile once (columns nt..127 are never read back); a full
@@ -501,7 +501,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
       // the peer's half of the last pair tile may lie beyond the leading dimension: nothing to load or store
       const bool rows_in = c.m0 + NOLSM_TILE_M * (int)rank < args.ld;
       chainep::EpiTile t;
-      if (rows_in) chainep::epi_begin<kLean>(args, c, c.m0 + NOLSM_TILE_M * (int)rank + q * 32 + lane, h, t);
+      if (rows_in) chainep::epi_begin<kFeat>(args, c, c.m0 + NOLSM_TILE_M * (int)rank + q * 32 + lane, h, t);
       mbar_wait<kPair>(&tfull_bar[acc], acc_phase);
       tc_fence_after();
       const uint32_t t_main = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(acc * 256);
@@ -589,6 +589,27 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
   }
 }
 
+// The instantiations that exist: the sign iteration / plain one-shot products (0), all-split programs of the FP32 mode,
+// the Eq. 15-17 chain with its column norms, the half-split residual R, the shifted B1 -> X0 product, and everything.
+typedef void (*ChainKernel)(const ChainArgs);
+constexpr int kNumInst = 6;
+const int kInstFeat[kNumInst] = {0, chainep::kFeatSplitAll, chainep::kFeatColNorm, chainep::kFeatSplitAny,
+                                 chainep::kFeatShift, chainep::kFeatFull};
+template <bool kPair>
+static ChainKernel chain_kernel_of(int feat) {
+  switch (feat) {
+    case 0: return k_chain<kPair, 0>;
+    case chainep::kFeatSplitAll: return k_chain<kPair, chainep::kFeatSplitAll>;
+    case chainep::kFeatColNorm: return k_chain<kPair, chainep::kFeatColNorm>;
+    case chainep::kFeatSplitAny: return k_chain<kPair, chainep::kFeatSplitAny>;
+    case chainep::kFeatShift: return k_chain<kPair, chainep::kFeatShift>;
+    default: return k_chain<kPair, chainep::kFeatFull>;
+  }
+}
+static ChainKernel chain_kernel(bool pair, int feat) {
+  return pair ? chain_kernel_of<true>(feat) : chain_kernel_of<false>(feat);
+}
+
 // Reset of the per-launch control state: slots 0..window-1 hold submatrices 0..window-1 at product 0.
 __global__ void __launch_bounds__(256)
 k_chain_reset(int count, int window, unsigned long long *slot_state, int32_t *slot_done, int32_t *sched,
@@ -644,9 +665,10 @@ nolsm_status encode_map(nolsm_ctx *ctx, CUtensorMap *map, void *ptr, int ld, int
 // all pairs must be co-resident: the CTAs wait on one another through global flags
 void pair_init(nolsm_ctx *ctx) {
   ctx->pair_ok = false;
-  cudaError_t e = cudaFuncSetAttribute(k_chain<true, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_chain<true, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_chain<true, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit);
+  cudaError_t e = cudaSuccess;
+  for (int i = 0; i < kNumInst && e == cudaSuccess; ++i)
+    e = cudaFuncSetAttribute(reinterpret_cast<const void *>(chain_kernel(true, kInstFeat[i])),
+                             cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit);
   if (e != cudaSuccess) { cudaGetLastError(); return; }
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3((unsigned)(ctx->sm_count & ~1));
@@ -658,7 +680,7 @@ void pair_init(nolsm_ctx *ctx) {
   cfg.attrs = at;
   cfg.numAttrs = 1;
   int max_clusters = 0;
-  e = cudaOccupancyMaxActiveClusters(&max_clusters, k_chain<true, 0>, &cfg);
+  e = cudaOccupancyMaxActiveClusters(&max_clusters, k_chain<true, chainep::kFeatFull>, &cfg);
   if (e != cudaSuccess || max_clusters < 1) { cudaGetLastError(); return; }
   ctx->pair_clusters = std::min(max_clusters, ctx->sm_count / 2);
   ctx->pair_ok = true;
@@ -677,9 +699,10 @@ nolsm_status umma_init(nolsm_ctx *ctx) {
     return NOLSM_ECUDA;
   }
   ctx->encode_tiled = fn;
-  e = cudaFuncSetAttribute(k_chain<false, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_chain<false, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_chain<false, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit);
+  e = cudaSuccess;
+  for (int i = 0; i < kNumInst && e == cudaSuccess; ++i)
+    e = cudaFuncSetAttribute(reinterpret_cast<const void *>(chain_kernel(false, kInstFeat[i])),
+                             cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit);
   if (e != cudaSuccess) {
     ctx->err = std::string("cudaFuncSetAttribute(k_chain): ") + cudaGetErrorString(e);
     cudaGetLastError();
@@ -725,20 +748,27 @@ nolsm_status umma_make_maps(nolsm_ctx *ctx, nolsm_batch *b) {
   return NOLSM_OK;
 }
 
-// Which lean kernel instantiation can run the program (chain_epilogue.cuh: epi_begin<kLean>): 1 all products plain
-// FP16, 2 all products full-split, 0 neither
-static int program_lean_mode(const ChainProgram &prog) {
-  if (prog.use_alpha_tab) return 0;
-  int n_split = 0;
+// The instantiation that runs a program: the one whose feature set is exactly what the program needs if it exists
+// (kInstFeat), else the full kernel
+static int program_features(const ChainProgram &prog) {
+  using namespace chainep;
+  int need = prog.use_alpha_tab ? kFeatAlphaTab : 0;
+  int n_full_split = 0, n_plain = 0;
   for (int i = 0; i < prog.n_ops; ++i) {
     const ChainOp &o = prog.ops[i];
-    if (o.cin32 >= 0 || o.cout32 >= 0 || o.colnorm || o.diag != 0.f || o.use_div == 2) return 0;
+    if (o.cin32 >= 0 || o.cout32 >= 0) need |= kFeatFp32;
+    if (o.colnorm) need |= kFeatColNorm;
+    if (o.diag != 0.f || o.use_div == 2) need |= kFeatShift;
     const bool s0 = o.a_lo[0] >= 0 && o.b_lo[0] >= 0, s1 = o.a_lo[1] >= 0 && o.b_lo[1] >= 0;
     const bool p0 = o.a_lo[0] < 0 && o.b_lo[0] < 0, p1 = o.a_lo[1] < 0 && o.b_lo[1] < 0;
-    if (s0 && s1) ++n_split;
-    else if (!(p0 && p1)) return 0;   // half-split or different by parity
+    if (s0 && s1) ++n_full_split;
+    else if (p0 && p1) ++n_plain;
   }
-  return n_split == 0 ? 1 : (n_split == prog.n_ops ? 2 : 0);
+  if (n_full_split == prog.n_ops) need |= kFeatSplitAll;
+  else if (n_plain != prog.n_ops) need |= kFeatSplitAny;
+  for (int i = 0; i < kNumInst; ++i)
+    if (kInstFeat[i] == need) return need;
+  return kFeatFull;
 }
 
 // Runs `prog` over every submatrix of the batch.  touch_stats: reset and fill iters / lastres.
@@ -806,12 +836,11 @@ cudaError_t launch_chain(nolsm_ctx *ctx, const nolsm_batch *b, const ChainProgra
     if (e != cudaSuccess) return e;
   }
   const size_t smem_bytes = (size_t)(a.stages * a.stage_bytes + chainep::kStagingBytes + 1024);
-  const int lean = program_lean_mode(prog);
+  const int feat = program_features(prog);
   if (!pair) {
     void *params[] = {&a};
-    void *fn = lean == 1 ? reinterpret_cast<void *>(k_chain<false, 1>)
-                         : lean == 2 ? reinterpret_cast<void *>(k_chain<false, 2>) : reinterpret_cast<void *>(k_chain<false, 0>);
-    return cudaLaunchCooperativeKernel(fn, dim3(ctx->sm_count), dim3(kThreads), params, smem_bytes, st);
+    return cudaLaunchCooperativeKernel(reinterpret_cast<const void *>(chain_kernel(false, feat)), dim3(ctx->sm_count),
+                                       dim3(kThreads), params, smem_bytes, st);
   }
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3((unsigned)(2 * ctx->pair_clusters));
@@ -825,6 +854,5 @@ cudaError_t launch_chain(nolsm_ctx *ctx, const nolsm_batch *b, const ChainProgra
   at[1].val.cooperative = 1;
   cfg.attrs = at;
   cfg.numAttrs = 2;
-  return lean == 1 ? cudaLaunchKernelEx(&cfg, k_chain<true, 1>, a)
-                   : lean == 2 ? cudaLaunchKernelEx(&cfg, k_chain<true, 2>, a) : cudaLaunchKernelEx(&cfg, k_chain<true, 0>, a);
+  return cudaLaunchKernelEx(&cfg, chain_kernel(true, feat), a);
 }

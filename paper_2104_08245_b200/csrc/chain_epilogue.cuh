@@ -337,12 +337,18 @@ __device__ __forceinline__ void epi_prefetch32(EpiTile &t) {
 }
 
 // Before waiting for the accumulator.  col: this thread's column of the result; h: row quarter of the chunks.
-// kLean != 0: the program was checked on the host (chain_engine.cu: program_lean_mode) to use FP16 staging input and
-// output only, no diagonal shift, no column norms and no scaling table, and operands that are all plain FP16 (1) or all
-// full-split pairs (2) -- the flags below become compile-time constants and the code for everything else drops out of
-// the kernel (the sign iteration's two products are such a program in either precision mode, and the compute warps'
-// code decides the kernel's register budget).
-template <int kLean>
+// kFeat: the epilogue / operand features the kernel instantiation supports (chain_engine.cu: program_features picks the
+// smallest instantiation that covers a program).  The compute warps' code decides the kernel's register budget, and a
+// feature that is compiled in costs the sign iteration 0.5-3 % even though it never runs there; with a feature bit
+// clear its flag below is a compile-time constant and the code drops out of the kernel.
+constexpr int kFeatSplitAny = 1;    // products may have split operands (full or half split), decided per op
+constexpr int kFeatSplitAll = 2;    // every product is a full-split product
+constexpr int kFeatColNorm = 4;     // column norms of the residual product (a-priori stop of Eq. 15-17)
+constexpr int kFeatShift = 8;       // diagonal shift, per-matrix division of beta and the shift (X0 from B1's epilogue)
+constexpr int kFeatFp32 = 16;       // FP32 inputs / outputs (direct or through the staging buffers)
+constexpr int kFeatAlphaTab = 32;   // per-iteration scaling table (nolsm_config.gap_hint)
+constexpr int kFeatFull = 63 & ~kFeatSplitAll;
+template <int kFeat>
 __device__ __forceinline__ void epi_begin(const ChainArgs &args, const TileCmd &c, int col, int h, EpiTile &t) {
   const ChainOp &o = args.prog.ops[c.op];
   t.o = &o;
@@ -354,30 +360,37 @@ __device__ __forceinline__ void epi_begin(const ChainArgs &args, const TileCmd &
   t.ident = o.mode == EPI_IDENT;
   t.abs_sum = 0.f;
   t.alpha = o.use_div ? o.alpha / args.alpha_div[c.mat] : o.alpha;
-  if constexpr (kLean != 0) {
-    t.io.out32 = -1;
-    t.split = kLean == 2;
-    t.cin_direct = t.colnorm = false;
+  if constexpr ((kFeat & kFeatSplitAll) != 0) t.split = true;
+  else if constexpr ((kFeat & kFeatSplitAny) != 0) t.split = o.a_lo[t.par] >= 0;
+  else t.split = false;
+  if constexpr ((kFeat & kFeatColNorm) != 0) t.colnorm = t.ident && o.colnorm != 0;
+  else t.colnorm = false;
+  if constexpr ((kFeat & kFeatShift) != 0) {
+    t.beta = o.use_div == 2 ? o.beta / args.alpha_div[c.mat] : o.beta;
+    t.diag = o.use_div == 2 ? o.diag / args.alpha_div[c.mat] : o.diag;
+  } else {
     t.beta = o.beta;
     t.diag = 0.f;
+  }
+  if constexpr ((kFeat & kFeatAlphaTab) != 0) {
+    if (args.alpha_tab != nullptr && cmd_iter(c) < kAlphaSteps) {
+      // X_{k+1} = 1/2 a X (3I - a^2 X^2):  E = I - a^2 X X,  X' = a X + (1/2 a) X E
+      const float a = args.alpha_tab[c.mat * kAlphaSteps + cmd_iter(c)];
+      if (t.ident) t.alpha *= a * a; else { t.alpha *= a; t.beta *= a; }
+    }
+  }
+  if constexpr ((kFeat & kFeatFp32) != 0) {
+    t.cin_direct = !t.ident && o.cin32 >= 0 && o.beta != 0.f && t.io.in_hi < 0;
+    const int64_t off = (int64_t)c.mat * args.slab + (int64_t)col * args.ld + c.n0 + kWarpRows * h;
+    t.p32 = (o.cout32 >= 0 && t.io.out32 < 0) ? args.ubuf[o.cout32] + off : nullptr;
+    t.cinp = t.cin_direct ? args.ubuf[o.cin32] + off : nullptr;
+    if (t.cin_direct && kWarpRows * h < c.nt) epi_prefetch32(t);
+  } else {
+    t.io.out32 = -1;
+    t.cin_direct = false;
     t.p32 = nullptr;
     t.cinp = nullptr;
-    return;
   }
-  t.split = o.a_lo[t.par] >= 0;
-  t.cin_direct = !t.ident && o.cin32 >= 0 && o.beta != 0.f && t.io.in_hi < 0;
-  t.colnorm = t.ident && o.colnorm != 0;
-  t.beta = o.use_div == 2 ? o.beta / args.alpha_div[c.mat] : o.beta;
-  t.diag = o.use_div == 2 ? o.diag / args.alpha_div[c.mat] : o.diag;
-  if (args.alpha_tab != nullptr && cmd_iter(c) < kAlphaSteps) {
-    // X_{k+1} = 1/2 a X (3I - a^2 X^2):  E = I - a^2 X X,  X' = a X + (1/2 a) X E
-    const float a = args.alpha_tab[c.mat * kAlphaSteps + cmd_iter(c)];
-    if (t.ident) t.alpha *= a * a; else { t.alpha *= a; t.beta *= a; }
-  }
-  const int64_t off = (int64_t)c.mat * args.slab + (int64_t)col * args.ld + c.n0 + kWarpRows * h;
-  t.p32 = (o.cout32 >= 0 && t.io.out32 < 0) ? args.ubuf[o.cout32] + off : nullptr;
-  t.cinp = t.cin_direct ? args.ubuf[o.cin32] + off : nullptr;
-  if (t.cin_direct && kWarpRows * h < c.nt) epi_prefetch32(t);
 }
 
 // ------------------------------------------------------------------------------------------------
