@@ -59,6 +59,7 @@ extern "C" nolsm_status nolsm_create(nolsm_ctx **out, const nolsm_config *cfg) {
   if (c.max_iter > NOLSM_MAX_RESID_SLOTS) c.max_iter = NOLSM_MAX_RESID_SLOTS;
   if (c.inv_max_iter <= 0) c.inv_max_iter = 20;
   if (c.inv_max_iter > NOLSM_MAX_RESID_SLOTS) c.inv_max_iter = NOLSM_MAX_RESID_SLOTS;
+  ctx->inv_refine_default = c.inv_refine < 0;
   if (c.inv_refine < 0) c.inv_refine = 1;
   if (c.workspace_bytes <= 0) c.workspace_bytes = (int64_t)24 << 30;
   ctx->cfg = c;
@@ -385,7 +386,7 @@ extern "C" nolsm_status nolsm_set_model(nolsm_ctx *ctx, const nolsm_model *model
 static nolsm_status build_submatrices_impl(nolsm_ctx *ctx, const nolsm_bsr *H, const nolsm_bsr *S,
                                            int32_t mol_begin, int32_t mol_count, int32_t slot, int units,
                                            nolsm_batch **out, void *stream, bool need_h32 = true,
-                                           bool need_s32 = true) {
+                                           bool need_s32 = true, bool fast32 = false) {
   if (!ctx || !out) return NOLSM_EINVAL;
   CHECK(check_bsr(ctx, H, "H"));
   CHECK(check_bsr(ctx, S, "S"));
@@ -404,9 +405,10 @@ static nolsm_status build_submatrices_impl(nolsm_ctx *ctx, const nolsm_bsr *H, c
   CHECK(setup_batch(ctx, slot, dims, mol_begin, true, units, &b, st));
   // the split copy of S is only read by the Newton refinements of S^-1 (reading 11)
   const int prec = effective_precision(ctx, -1);
-  const bool split_s = (ctx->cfg.inv_refine >= 0 ? ctx->cfg.inv_refine : (prec == NOLSM_FP16_FP32 ? 1 : 0)) > 0;
+  // (fast32: the whole path's FP32 mode runs the FP16 chain and refines twice, prepare_batch_chain)
+  const bool split_s = fast32 || (ctx->cfg.inv_refine >= 0 ? ctx->cfg.inv_refine : (prec == NOLSM_FP16_FP32 ? 1 : 0)) > 0;
   // the FP32 copy of T_j(S) can only be left out where the lean FP16 start of Eq. 15-17 reads the split copy
-  if (!(split_s && prec == NOLSM_FP16_FP32) || ctx->has_model) need_s32 = true;
+  if (!(split_s && (prec == NOLSM_FP16_FP32 || fast32)) || ctx->has_model) need_s32 = true;
   b->s_norm_built = false;
   if (ctx->has_model) {
     if (ctx->model.n_mol != H->n_mol) {
@@ -573,14 +575,21 @@ static nolsm_status ensure_thin(nolsm_ctx *ctx, nolsm_batch *b, cudaStream_t st)
 static nolsm_status prepare_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, int precision, cudaStream_t st,
                                         nolsm_sign_stats *stats, int64_t *gemms, bool own_only,
                                         const double *x0_mu) {
-  const bool fp16 = precision == NOLSM_FP16_FP32;
-  const int refine = ctx->cfg.inv_refine >= 0 ? ctx->cfg.inv_refine : (fp16 ? 1 : 0);
+  // FP32 mode of the whole path (defaults only): the same FP16 chain and A0, then TWO refinements of B and of the own
+  // columns of S^-1 -- with F = I - A0 S the errors are F^3 B and F^3 V, ||F||_2 <= 1e-2 by the a-priori stop, and the
+  // residuals are formed on split operands -- instead of running Eq. 15-17 itself on split operands to 1e-5:
+  // 14 MMA-equivalents instead of about 30.  Below, `fp16` then selects the FP16 chain and buffer layout.
+  const bool fp32_fast = precision != NOLSM_FP16_FP32 && own_only && ctx->inv_refine_default && ctx->cfg.inv_tol <= 0.f &&
+                         (ctx->cfg.flags & NOLSM_FLAG_NO_PREDICT) == 0 && b->sparse && b->row_ptr != nullptr &&
+                         !b->grouped && b->s_split_built && b->s_norm_built;
+  const bool fp16 = precision == NOLSM_FP16_FP32 || fp32_fast;
+  const int refine = fp32_fast ? 1 : (ctx->cfg.inv_refine >= 0 ? ctx->cfg.inv_refine : (fp16 ? 1 : 0));
   // one refinement, FP16 mode, one owner per submatrix: B1 = B0 + A0 (H - S B0) with B0 = A0 H and A0 = Z^2/s_S the
   // FP16-quality inverse -- the same second-order error (I - A0 S)^2 S^-1 H as refining S^-1 first, in four MMAs
   // (1 + 2 + 1) instead of seven (3 + 1 for the refinement, 3 for B on split operands); the own columns of S^-1
   // get their refinement as two thin products (launch_own_refine)
   const bool fast_b = own_only && fp16 && refine == 1 && b->sparse && b->row_ptr != nullptr && !b->grouped;
-  const bool x0_direct = fast_b && x0_mu != nullptr && (ctx->cfg.flags & NOLSM_FLAG_ORDER3) == 0;
+  const bool x0_direct = fast_b && !fp32_fast && x0_mu != nullptr && (ctx->cfg.flags & NOLSM_FLAG_ORDER3) == 0;
   b->x0_built = false;
   b->b32_built = true;
   // 3e-3 with a refinement behind: the iterate is taken with a relative error of about twice its residual,
@@ -633,7 +642,7 @@ static nolsm_status prepare_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, int prec
       // a-priori stop (ChainProgram::tol_pred, reading 11): ||E_{k+1}||_2 <= 2e-2 guaranteed from ||E_k||_1,
       // i.e. a relative error of at most 2e-2 in every direction of A0, which the refinement squares
       e.colnorm = 1;
-      pg.tol_pred = 2e-2f;
+      pg.tol_pred = fp32_fast ? 1e-2f : 2e-2f;
     }
     if (lean) {   // Y1 = Y0 Z1 = (S_hi Z1)/s_S: plain product, scaled in the epilogue
       y1 = make_op(EPI_AXPBY, 1.f, 0.f);
@@ -690,7 +699,7 @@ static nolsm_status prepare_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, int prec
       stats->inv_iter_max = std::max(stats->inv_iter_max, it[m]);
       if (!(res[m] <= stats->inv_worst_residual)) stats->inv_worst_residual = res[m];
       const double n = b->n_host[m];
-      const int products = 1 + chain_products + 2 + 2 * refine;   // products, whatever the MMAs per product
+      const int products = 1 + chain_products + 2 + 2 * refine + (fp32_fast ? 2 : 0);   // products, whatever the MMAs per product
       inv_gemm_sum += products;
       fl += 2.0 * n * n * n * products;
     }
@@ -760,12 +769,30 @@ static nolsm_status prepare_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, int prec
       b->x0_built = true;
       b->x0_mu = *x0_mu;
       b->b32_built = false;
+    } else if (fp32_fast) {
+      // B1 -> split pair (h6, h7); R2 = H - S B1 on full-split operands -> h5 (it is ~1e-4 |H|: FP16 holds it to
+      // 5e-8); B2 = B1 + A0 R2 -> u3
+      set2(b1.out16, 6, 6); set2(b1.out16_lo, 7, 7);
+      CHECK(run_chain(ctx, b, p7, nullptr, false, st));
+      ChainProgram p8 = one_shot(g1);
+      p8.n_ops = 1;
+      ChainOp &r2 = p8.ops[0] = make_op(EPI_AXPBY, -1.f, 1.f);
+      set2(r2.a, ss_hi, ss_hi); set2(r2.a_lo, ss_lo, ss_lo); set2(r2.b, 6, 6); set2(r2.b_lo, 7, 7);
+      set2(r2.cin16, hs_hi, hs_hi); set2(r2.cin16_lo, hs_lo, hs_lo); set2(r2.out16, 5, 5);
+      CHECK(run_chain(ctx, b, p8, nullptr, false, st));
+      ChainProgram p9 = one_shot(g1);
+      p9.n_ops = 1;
+      ChainOp &b2 = p9.ops[0] = make_op(EPI_AXPBY, 1.f, 1.f);
+      set2(b2.a, si_hi, si_hi); set2(b2.b, 5, 5); set2(b2.cin16, 6, 6); set2(b2.cin16_lo, 7, 7);
+      b2.cout32 = 3;
+      CHECK(run_chain(ctx, b, p9, nullptr, false, st));
     } else {
       b1.cout32 = 3;
       CHECK(run_chain(ctx, b, p7, nullptr, false, st));
     }
     CHECK(ensure_thin(ctx, b, st));
-    LAUNCH(ctx, launch_own_refine(b, b->row_ptr, b->col_idx, b->h[ss_hi], b->h[ss_lo], b->h[si_hi], b->d_thin, b->u[2], st));
+    LAUNCH(ctx, launch_own_refine(b, b->row_ptr, b->col_idx, b->h[ss_hi], b->h[ss_lo], b->h[si_hi], b->d_thin, b->u[2],
+                                  fp32_fast ? 2 : 1, st));
     b->sinv_hi = b->sinv_lo = -1;
     b->sinv32_full = false;
     b->sinv_own_only = true;
@@ -1435,8 +1462,10 @@ extern "C" nolsm_status nolsm_solve_mu(nolsm_ctx *ctx, const nolsm_bsr *H, const
       } else if (!b || !resident) {
         // the FP32 copy of T_j(H) is only read by the energy products (nolsm_evaluate) and the SIMT debug path
         const bool need32 = ctx->eval_energy || use_simt(ctx) || !ctx->umma_ok;
+        const bool fast32 = prec != NOLSM_FP16_FP32 && !ctx->eval_energy && ctx->inv_refine_default &&
+                            ctx->cfg.inv_tol <= 0.f && (ctx->cfg.flags & NOLSM_FLAG_NO_PREDICT) == 0;
         rc = build_submatrices_impl(ctx, H, S, r.begin, r.count, kOwnSlot + (resident ? (int)bi : 0), units, &b, st,
-                                    need32, need32);
+                                    need32, need32, fast32);
         if (rc != NOLSM_OK) break;
         live[bi] = resident ? b : nullptr;
       }

@@ -163,6 +163,7 @@ struct nolsm_batch {
 
 struct nolsm_ctx {
   nolsm_config cfg;
+  bool inv_refine_default = true;   // the caller left nolsm_config.inv_refine < 0
   int device = 0;
   int sm_count = 148;
   size_t l2_bytes = 0;
@@ -236,7 +237,8 @@ cudaError_t launch_density_split(const nolsm_batch *b, const XRef &x, const floa
                                  const int32_t *col_idx, float *d_val, double *ne_diag, const __half *e_hi,
                                  const __half *e_lo, float *u_thin, cudaStream_t st);
 cudaError_t launch_own_refine(const nolsm_batch *b, const int32_t *row_ptr, const int32_t *col_idx, const __half *s_hi,
-                              const __half *s_lo, const __half *a0, float *thin, float *out32, cudaStream_t st);
+                              const __half *s_lo, const __half *a0, float *thin, float *out32, int rounds,
+                              cudaStream_t st);
 cudaError_t launch_own_join(const nolsm_batch *b, const int32_t *row_ptr, const int32_t *col_idx, const __half *hi,
                             const __half *lo, float *dst32, cudaStream_t st);
 cudaError_t launch_density(const nolsm_batch *b, const XRef &x, const float *sinv,

@@ -41,6 +41,8 @@ struct ThinArgs {
   float *d_val;                      // kDensity: column-owned block store
   double *ne_diag;                   // kDensity: sum of 1 - X_rr over the own rows, or null
   float *out32;                      // kOwnCorrect: FP32 S^-1, own columns written
+  int v32;                           // kOwnResid / kOwnCorrect: the current V is in the own columns of sinv (a later
+                                     // refinement round) instead of being A0's own columns
 };
 
 __device__ __forceinline__ uint32_t pack_half2(float a, float b) {
@@ -147,6 +149,7 @@ __global__ void __launch_bounds__(kThinThreads, 2) k_thin_mma(const ThinArgs a) 
   auto vsrc2 = [&](int k, int p) -> float2 {
     if (k >= n) return make_float2(0.f, 0.f);
     if constexpr (kMode == kOwnResid) {
+      if (a.v32) return *reinterpret_cast<const float2 *>(sj + (int64_t)(own0 + p) * ld + k);
       return __half22float2(*reinterpret_cast<const __half2 *>(a0j + (int64_t)(own0 + p) * ld + k));
     } else {
       const float *src = (kMode == kOwnCorrect || (kMode == kDensity && a.folded)) ? tj + (int64_t)p * ld
@@ -227,7 +230,8 @@ __global__ void __launch_bounds__(kThinThreads, 2) k_thin_mma(const ThinArgs a) 
         v[u] = 0.f;
         if (r < n) {
           if constexpr (kMode == kDensity || kMode == kLastHalf) v[u] = sj[(int64_t)(own0 + pp[u]) * ld + r];
-          else if constexpr (kMode == kOwnCorrect) v[u] = __half2float(a0j[(int64_t)(own0 + pp[u]) * ld + r]);
+          else if constexpr (kMode == kOwnCorrect)
+            v[u] = a.v32 ? sj[(int64_t)(own0 + pp[u]) * ld + r] : __half2float(a0j[(int64_t)(own0 + pp[u]) * ld + r]);
         }
       }
 #pragma unroll
@@ -324,19 +328,28 @@ cudaError_t launch_density_split(const nolsm_batch *b, const XRef &x, const floa
 // (I - A0 S)(V - V0) is of second order whatever the rounding of A0, as long as both uses read the same A0.
 // s_hi, s_lo: split S; thin: scratch of count * 6 * ld floats; out32: FP32 S^-1, its own columns are written.
 cudaError_t launch_own_refine(const nolsm_batch *b, const int32_t *row_ptr, const int32_t *col_idx, const __half *s_hi,
-                              const __half *s_lo, const __half *a0, float *thin, float *out32, cudaStream_t st) {
+                              const __half *s_lo, const __half *a0, float *thin, float *out32, int rounds,
+                              cudaStream_t st) {
   if (b->count == 0) return cudaSuccess;
-  ThinArgs r = base_args(b, row_ptr, col_idx);
-  r.a_hi[0] = r.a_hi[1] = s_hi;
-  r.a_lo[0] = r.a_lo[1] = s_lo;
-  r.a0 = a0;
-  r.thin = thin;
-  cudaError_t e = thin_launch<kOwnResid>(b, r, st);
-  if (e != cudaSuccess) return e;
-  ThinArgs c = base_args(b, row_ptr, col_idx);
-  c.a_hi[0] = c.a_hi[1] = a0;
-  c.a0 = a0;
-  c.thin = thin;
-  c.out32 = out32;
-  return thin_launch<kOwnCorrect>(b, c, st);
+  for (int round = 0; round < rounds; ++round) {   // round r: V_{r+1} = V_r + A0 (I[:, own] - S V_r), error F^(r+2) V
+    ThinArgs r = base_args(b, row_ptr, col_idx);
+    r.a_hi[0] = r.a_hi[1] = s_hi;
+    r.a_lo[0] = r.a_lo[1] = s_lo;
+    r.a0 = a0;
+    r.thin = thin;
+    r.v32 = round > 0 ? 1 : 0;
+    r.sinv = round > 0 ? out32 : nullptr;
+    cudaError_t e = thin_launch<kOwnResid>(b, r, st);
+    if (e != cudaSuccess) return e;
+    ThinArgs c = base_args(b, row_ptr, col_idx);
+    c.a_hi[0] = c.a_hi[1] = a0;
+    c.a0 = a0;
+    c.thin = thin;
+    c.out32 = out32;
+    c.v32 = r.v32;
+    c.sinv = r.sinv;
+    e = thin_launch<kOwnCorrect>(b, c, st);
+    if (e != cudaSuccess) return e;
+  }
+  return cudaSuccess;
 }

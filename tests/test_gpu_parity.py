@@ -385,6 +385,35 @@ def test_a_priori_stop_of_the_inverse_iteration(nolsm, tiny_system, mid_system, 
     assert measured[2] - ahead[2] == 2 * system.n_mol               # Y_{k+1} and E_{k+1} were never formed
 
 
+def test_fp32_whole_path_two_refinements(nolsm, mid_system, mid_solution):
+    """FP32 mode of nolsm_solve_mu (reading 11): Eq. 15-17 runs on FP16 operands to the a-priori stop, then
+    B and the own columns of S^-1 are refined twice with their residuals on split operands (errors F^3 B, F^3 V with
+    ||F||_2 <= 1e-2; pinned on the oracle in test_oracle_pins.py).  D, N and the populations against the oracle at the
+    FP32 tolerances, and against the path that iterates Eq. 15-17 itself on split operands (NOLSM_FLAG_NO_PREDICT)."""
+    import oracle.nolsm_oracle as orc
+    import torch
+    sols = mid_solution["solutions"]
+    H, S = _device_system(nolsm, mid_system)
+    d_ref = orc.density_blocks(sols, mid_system.row_ptr, MU)
+    ne_ref = orc.electron_count(sols, MU)
+    out = {}
+    for flags in (0, nolsm.FLAG_NO_PREDICT):
+        ctx = nolsm.Context(nolsm.Config(precision=1, flags=flags))
+        q = torch.zeros(mid_system.n_mol, dtype=torch.float64, device="cuda")
+        mu, ne, D, st = ctx.solve_mu(H, S, mid_system.n_electrons, MU - 0.1, MU + 0.1, tol_ne_per_mol=-1.0,
+                                     max_steps=1, q_mol=q)
+        d = D.val.cpu().numpy().copy()
+        assert np.abs(d - d_ref).max() < TOL_D[1]
+        assert abs(ne - ne_ref) / mid_system.n_mol <= TOL_NE_PER_MOL
+        pop = np.array([s.population(MU) for s in sols])
+        assert np.abs(q.cpu().numpy() - pop).max() < 2e-5
+        out[flags] = (d, st.last.gemms, st.last.inv_iter_max)
+        ctx.close()
+    fast, slow = out[0], out[nolsm.FLAG_NO_PREDICT]
+    assert np.abs(fast[0] - slow[0]).max() < 5e-6
+    assert fast[1] < slow[1] and fast[2] < slow[2]      # fewer products, fewer iterations of Eq. 15-17
+
+
 # ---------------------------------------------------------------------------------------------
 # BASELINE sizes, sampled (the oracle solves the sampled molecules one by one)
 # ---------------------------------------------------------------------------------------------

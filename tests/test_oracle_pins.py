@@ -270,6 +270,45 @@ def test_a_priori_bound_on_the_next_inverse_residual(tiny_system, mid_system_cpu
         assert first is not None and 1 <= first <= 3
 
 
+def test_refinements_of_the_operator_cube_the_inverse_error(mid_system_cpu):
+    """Reading 11, FP32 mode of the whole path: with A0 any approximate inverse of S and F = I - A0 S, the iteration
+    B_{r+1} = B_r + A0 (H - S B_r) from B_0 = A0 H has B - B_r = F^(r+1) B exactly (B = S^-1 H), and the same for the
+    own columns V of S^-1.  With the iterate the a-priori stop takes at 1e-2, two refinements leave < 1e-6 |B|."""
+    system, j = mid_system_cpu, 100
+    nb = system.col_idx[system.row_ptr[j]:system.row_ptr[j + 1]]
+    ssub = orc.dense_submatrix(system.row_ptr, system.col_idx, system.s_val, nb)
+    hsub = orc.dense_submatrix(system.row_ptr, system.col_idx, system.h_val, nb)
+    n = len(ssub)
+    eye = np.eye(n)
+    c = 0.5 * max(1.0, np.sqrt(np.abs(ssub).sum(0).max() * np.abs(ssub).sum(1).max()))
+    k_stop = None
+    for k in range(6):
+        _, zk, yk = orc.newton_schulz_inverse(ssub, k, scale=c)
+        b1 = np.abs(eye - zk @ yk).sum(0).max()
+        if 0.75 * b1 * b1 + 0.25 * b1 ** 3 <= 1e-2:
+            k_stop = k
+            break
+    assert k_stop is not None
+    _, z, _ = orc.newton_schulz_inverse(ssub, k_stop + 1, scale=c)
+    a0 = (z @ z / c).astype(np.float16).astype(np.float64)          # the CUDA path keeps A0 in FP16
+    f = eye - a0 @ ssub
+    assert np.linalg.norm(f, 2) <= 1e-2 + 2e-3                        # the bound + the FP16 rounding of A0
+    b_exact = np.linalg.solve(ssub, hsub)
+    v_exact = np.linalg.inv(ssub)[:, :6]
+    br, vr = a0 @ hsub, a0[:, :6].copy()
+    fp = f.copy()
+    for r in range(3):
+        assert np.abs((b_exact - br) - fp @ b_exact).max() < 1e-12
+        assert np.abs((v_exact - vr) - fp @ v_exact).max() < 1e-12
+        br = br + a0 @ (hsub - ssub @ br)
+        vr = vr + a0 @ (eye[:, :6] - ssub @ vr)
+        fp = fp @ f
+    b2 = a0 @ hsub
+    for _ in range(2):
+        b2 = b2 + a0 @ (hsub - ssub @ b2)
+    assert np.abs(b2 - b_exact).max() < 1e-6 * np.abs(b_exact).max()
+
+
 def test_last_sign_update_folded_into_thin_products(tiny_system, tiny_solution):
     """Reading 9: with E_k = I - X_k^2, X_{k+1} V = X_k (V + 1/2 E_k V) for any thin V, so the own columns of
     D = 1/2 (I - X_{k+1}) S^-1 follow from X_k and E_k without forming X_{k+1}."""
