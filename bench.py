@@ -34,7 +34,7 @@ WORKLOADS = {          # name -> (precision, description)
 DATASHEET_FP16_TFLOPS = 2250.0
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE sign-iteration launch of k_chain: an ncu CONSTANT from the
 # `ncu --set full` capture named here (bench.py cannot read DRAM counters itself); None where no capture exists
-NCU_TRAFFIC = {"w32768": 62.9e9}
+NCU_TRAFFIC = {"w32768": 62.7e9}   # dram read 35.39 + write 27.33 GB, end-of-round capture
 NCU_TRAFFIC_SOURCE = "profiles/r2_k_chain_sign_w32768.md"
 METRIC = "molecules/s per NOLSM step (sign-iteration TFLOP/s in roofline.achieved)"
 
