@@ -110,7 +110,9 @@ typedef struct {
 #define NOLSM_FLAG_NO_PREDICT 64 /* Eq. 15-17, FP16 mode: do not use the a-priori stop (reading 11: from
                                   ||E_k||_1 the bound 3/4 b^2 + 1/4 b^3 >= ||E_{k+1}||_2 is known before iteration k
                                   is finished; when it is small enough only Z_{k+1} is formed).  With this flag every
-                                  stop is decided on a measured residual: two products more per submatrix, same iterate */
+                                  stop is decided on a measured residual: two products more per submatrix, same iterate.
+                                  In FP32 mode nolsm_solve_mu then iterates Eq. 15-17 on split operands to inv_tol
+                                  instead of refining twice */
 #define NOLSM_FLAG_UNIT_SCALE 16 /* scale by the norm bound itself: Y0 = S/bound, X0 = A/bound (spectra in (0,1] and
                                   [-1,1]) instead of bound/2 and bound/1.5 (readings 5, 7); costs one
                                   iteration each */
@@ -266,7 +268,12 @@ NOLSM_API nolsm_status nolsm_scatter_density(nolsm_ctx *ctx, const nolsm_batch *
  * mu_out, ne_out: host doubles.  q_mol: device double [n_mol] or NULL.  Synchronises once per step.
  * The sign iteration stops as nolsm_sign_batched does, but its finishing update X_{k+1} = X_k + 1/2 X_k E_k
  * is applied to the own columns of S_j^-1 only (X_{k+1} V = X_k (V + 1/2 E_k V)) instead of being formed;
- * the iteration counts in the statistics include it (reading 9). */
+ * the iteration counts in the statistics include it (reading 9).
+ * The prepare stage (a2, a3) of this call refines what it uses instead of all of S^-1 (reading 11): Eq. 15-17
+ * runs on FP16 operands up to its a-priori stop, then B_j and the six own columns of S_j^-1 are refined against S_j
+ * once (FP16 mode) or twice (FP32 mode) with the residuals at FP32 quality; the full S_j^-1 does not exist on this
+ * path.  nolsm_config.inv_refine >= 0, inv_tol > 0 or NOLSM_FLAG_NO_PREDICT select the forms nolsm_sign_batched
+ * uses (FP32 mode: Eq. 15-17 itself on split operands). */
 NOLSM_API nolsm_status nolsm_solve_mu(nolsm_ctx *ctx, const nolsm_bsr *H, const nolsm_bsr *S, double n_electrons,
                             double mu_lo, double mu_hi, double tol_ne_per_mol, int32_t max_steps,
                             int32_t precision, nolsm_bsr *D, double *mu_out /*host*/,
