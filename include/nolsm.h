@@ -272,8 +272,9 @@ NOLSM_API nolsm_status nolsm_scatter_density(nolsm_ctx *ctx, const nolsm_batch *
  * The prepare stage (a2, a3) of this call refines what it uses instead of all of S^-1 (reading 11): Eq. 15-17
  * runs on FP16 operands up to its a-priori stop, then B_j and the six own columns of S_j^-1 are refined against S_j
  * once (FP16 mode) or twice (FP32 mode) with the residuals at FP32 quality; the full S_j^-1 does not exist on this
- * path.  nolsm_config.inv_refine >= 0, inv_tol > 0 or NOLSM_FLAG_NO_PREDICT select the forms nolsm_sign_batched
- * uses (FP32 mode: Eq. 15-17 itself on split operands). */
+ * path.  The forms nolsm_sign_batched uses are selected by nolsm_config.inv_refine other than 1 (FP16 mode: the
+ * refinements then apply to S^-1) and, in FP32 mode, by an explicit inv_refine or inv_tol or by NOLSM_FLAG_NO_PREDICT
+ * (Eq. 15-17 itself on split operands to inv_tol). */
 NOLSM_API nolsm_status nolsm_solve_mu(nolsm_ctx *ctx, const nolsm_bsr *H, const nolsm_bsr *S, double n_electrons,
                             double mu_lo, double mu_hi, double tol_ne_per_mol, int32_t max_steps,
                             int32_t precision, nolsm_bsr *D, double *mu_out /*host*/,
