@@ -113,6 +113,11 @@ typedef struct {
                                   stop is decided on a measured residual: two products more per submatrix, same iterate.
                                   In FP32 mode nolsm_solve_mu then iterates Eq. 15-17 on split operands to inv_tol
                                   instead of refining twice */
+#define NOLSM_FLAG_LOWDIN 128    /* SURVEY 8(f)#4, symmetric Loewdin form (nolsm_solve_mu, FP32 mode only): with Z = (S_j/s)^-1/2
+                                  from Eq. 15-17 run to its end on split operands, the sign function is taken of the
+                                  SYMMETRIC A~ = Z H_j Z / s - mu I = S^-1/2 H S^-1/2 - mu I, and
+                                  D_j[:, own] = Z (1/2 (I - sign A~)) Z[:, own] / s.  Same D as the non-orthogonal
+                                  form of Eq. 12 up to rounding; no S^-1, no B */
 #define NOLSM_FLAG_UNIT_SCALE 16 /* scale by the norm bound itself: Y0 = S/bound, X0 = A/bound (spectra in (0,1] and
                                   [-1,1]) instead of bound/2 and bound/1.5 (readings 5, 7); costs one
                                   iteration each */

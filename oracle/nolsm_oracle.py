@@ -310,6 +310,22 @@ class SubmatrixSolution:
         return self.energy_weighted(mu)[:, self.own]
 
 
+def density_columns_lowdin(h_sub, s_sub, own, mu):
+    """SURVEY 8(f)#4, the symmetric Loewdin form (PAPER.md:121 uses the non-orthogonal one): with S^-1/2 from the
+    eigendecomposition of S, A~ = S^-1/2 H S^-1/2 - mu I is symmetric, P~ = 1/2 (I - sign A~) is the projector of the
+    ORTHOGONAL problem and T_j(D) = S^-1/2 P~ S^-1/2.  Returns its own columns [n, 6] (the same matrix as
+    MoleculeSolution.density_columns in exact arithmetic: S^-1/2 maps the eigenvectors of A~ onto the generalized
+    eigenvectors of (H, S))."""
+    sl, sv = np.linalg.eigh(s_sub)
+    s_mhalf = (sv / np.sqrt(sl)) @ sv.T
+    at = s_mhalf @ h_sub @ s_mhalf
+    at = 0.5 * (at + at.T)
+    lam, u = np.linalg.eigh(at)
+    sign = (u * np.where(lam < mu, -1.0, 1.0)) @ u.T
+    p = 0.5 * (np.eye(len(s_sub)) - sign)
+    return (s_mhalf @ p @ s_mhalf)[:, own]
+
+
 def solve_molecule(row_ptr, col_idx, h_val, s_val, j, nbrs=None):
     if nbrs is None:
         nbrs = col_idx[row_ptr[j]:row_ptr[j + 1]]

@@ -101,6 +101,7 @@ static void free_batch(nolsm_batch *b) {
   cudaFree(b->d_scale);
   cudaFree(b->d_norm);
   cudaFree(b->d_norm_s);
+  cudaFree(b->d_scale_s);
   cudaFree(b->d_alpha);
   cudaFree(b->d_colpart);
   cudaFree(b->d_active);
@@ -208,7 +209,7 @@ static nolsm_status setup_batch(nolsm_ctx *ctx, int slot, const std::vector<int3
     const size_t cap = (size_t)count;
     if (grow(&b->d_dims, cap) || grow(&b->d_state, cap) || grow(&b->d_iters, cap) ||
         grow(&b->d_resid2, cap * NOLSM_MAX_RESID_SLOTS) || grow(&b->d_lastres, cap) ||
-        grow(&b->d_scale, cap) || grow(&b->d_norm, cap * 2) || grow(&b->d_norm_s, cap * 2) || grow(&b->d_alpha, cap * 8) || grow(&b->d_slot_state, cap) ||
+        grow(&b->d_scale, cap) || grow(&b->d_norm, cap * 2) || grow(&b->d_norm_s, cap * 2) || grow(&b->d_scale_s, cap) || grow(&b->d_alpha, cap * 8) || grow(&b->d_slot_state, cap) ||
         grow(&b->d_slot_done, cap) || grow(&b->d_sched, (size_t)8) || grow(&b->d_tile_counter, (size_t)1) ||
         (b->d_active == nullptr && grow(&b->d_active, (size_t)NOLSM_MAX_RESID_SLOTS))) {
       cudaGetLastError();
@@ -232,6 +233,7 @@ static nolsm_status setup_batch(nolsm_ctx *ctx, int slot, const std::vector<int3
   b->sinv_own_only = false;
   b->x0_built = false;
   b->b32_built = true;
+  b->lowdin = false;
   b->ld = ld;
   b->max_n = max_n;
   b->mol_begin = mol_begin;
@@ -579,11 +581,15 @@ static nolsm_status prepare_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, int prec
   // columns of S^-1 -- with F = I - A0 S the errors are F^3 B and F^3 V, ||F||_2 <= 1e-2 by the a-priori stop, and the
   // residuals are formed on split operands -- instead of running Eq. 15-17 itself on split operands to 1e-5:
   // 14 MMA-equivalents instead of about 30.  Below, `fp16` then selects the FP16 chain and buffer layout.
-  const bool fp32_fast = precision != NOLSM_FP16_FP32 && own_only && ctx->inv_refine_default && ctx->cfg.inv_tol <= 0.f &&
+  // Loewdin form (NOLSM_FLAG_LOWDIN; nolsm_solve_mu checked the precision): Eq. 15-17 on split operands to its end
+  const bool lowdin = own_only && (ctx->cfg.flags & NOLSM_FLAG_LOWDIN) != 0 && precision != NOLSM_FP16_FP32 &&
+                      b->sparse && b->row_ptr != nullptr && !b->grouped;
+  b->lowdin = false;
+  const bool fp32_fast = !lowdin && precision != NOLSM_FP16_FP32 && own_only && ctx->inv_refine_default && ctx->cfg.inv_tol <= 0.f &&
                          (ctx->cfg.flags & NOLSM_FLAG_NO_PREDICT) == 0 && b->sparse && b->row_ptr != nullptr &&
                          !b->grouped && b->s_split_built && b->s_norm_built;
   const bool fp16 = precision == NOLSM_FP16_FP32 || fp32_fast;
-  const int refine = fp32_fast ? 1 : (ctx->cfg.inv_refine >= 0 ? ctx->cfg.inv_refine : (fp16 ? 1 : 0));
+  const int refine = lowdin ? 0 : (fp32_fast ? 1 : (ctx->cfg.inv_refine >= 0 ? ctx->cfg.inv_refine : (fp16 ? 1 : 0)));
   // one refinement, FP16 mode, one owner per submatrix: B1 = B0 + A0 (H - S B0) with B0 = A0 H and A0 = Z^2/s_S the
   // FP16-quality inverse -- the same second-order error (I - A0 S)^2 S^-1 H as refining S^-1 first, in four MMAs
   // (1 + 2 + 1) instead of seven (3 + 1 for the refinement, 3 for B on split operands); the own columns of S^-1
@@ -706,6 +712,36 @@ static nolsm_status prepare_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, int prec
     stats->flops_prepare = fl;
   }
   const int g1 = group_size(ctx, b, 16);
+  if (lowdin) {
+    // Z = (S / s_S)^-1/2 is the chain's last Z iterate, in (h4,h5) or (h6,h7) by parity: make it (h6,h7) for all, which
+    // the sign iteration (h0..h5) leaves alone.  T = H Z -> (h8,h9);  A~ = Z T / s_S -> u3 (symmetric);
+    // Z[:, own] -> FP32 own columns of u2 (where a5 looks for its thin operand); s_S kept for a5.
+    LAUNCH(ctx, launch_canon_pair(b, b->d_iters, b->h[4], b->h[5], b->h[6], b->h[7], st));
+    NOLSM_CUDA(ctx, cudaMemcpyAsync(b->d_scale_s, b->d_scale, sizeof(float) * b->count, cudaMemcpyDeviceToDevice, st));
+    const int hh = b->n_half - 2, hl = b->n_half - 1;
+    ChainProgram pt = one_shot(g1);
+    pt.n_ops = 1;
+    ChainOp &t = pt.ops[0] = make_op(EPI_AXPBY, 1.f, 0.f);
+    set2(t.a, hh, hh); set2(t.a_lo, hl, hl); set2(t.b, 6, 6); set2(t.b_lo, 7, 7);
+    set2(t.out16, 8, 8); set2(t.out16_lo, 9, 9);
+    CHECK(run_chain(ctx, b, pt, nullptr, false, st));
+    ChainProgram pa = one_shot(g1);
+    pa.n_ops = 1;
+    ChainOp &at = pa.ops[0] = make_op(EPI_AXPBY, 1.f, 0.f);
+    set2(at.a, 6, 6); set2(at.a_lo, 7, 7); set2(at.b, 8, 8); set2(at.b_lo, 9, 9);
+    at.use_div = 1; at.cout32 = 3;
+    CHECK(run_chain(ctx, b, pa, b->d_scale, false, st));
+    LAUNCH(ctx, launch_own_join(b, b->row_ptr, b->col_idx, b->h[6], b->h[7], b->u[2], st));
+    b->lowdin = true;
+    b->sinv_hi = b->sinv_lo = -1;
+    b->sinv32_full = false;
+    b->sinv_own_only = true;
+    b->engine_simt = false;
+    b->prepared = true;
+    b->prepared_precision = precision;
+    *gemms += inv_gemm_sum + 2 * b->count;
+    return NOLSM_OK;
+  }
   // S^-1 = Z^2 / s_S (Eq. 17); FP32 result -> u2, split copy -> (si_hi, si_lo).  The operands are the FP16
   // copies of Z the chain itself wrote last (parity_from_iters), so no conversion pass is needed.  When a
   // Newton refinement follows (it squares the error) plain FP16 operands are enough; otherwise split Z.
@@ -1254,6 +1290,21 @@ extern "C" nolsm_status nolsm_scatter_density(nolsm_ctx *ctx, const nolsm_batch 
     CHECK(ensure_thin(ctx, bm, st));   // same scratch as the energy products
     u_thin = bm->d_thin;
   }
+  if (batch->lowdin) {
+    // Loewdin form: U = 1/2 (W - X~ W) with W = Z[:, own] (u2), then D[:, own] = Z U / s_S
+    nolsm_batch *bm = const_cast<nolsm_batch *>(batch);
+    CHECK(ensure_thin(ctx, bm, st));
+    float *u_out = bm->d_thin + (size_t)batch->count * NOLSM_BS * batch->ld;   // second half of the scratch
+    ctx->launches += 1;
+    if (launch_density_split(batch, x_ref(batch), sinv_ptr(batch), S->row_ptr, S->col_idx, nullptr, nullptr, batch->h[4],
+                             batch->x_pending_split ? batch->h[5] : nullptr, u_thin, st, u_out) != cudaSuccess) {
+      cudaGetLastError(); ctx->err = "density columns (Loewdin form): launch failed"; return NOLSM_ECUDA;
+    }
+    LAUNCH(ctx, launch_scaled_out(batch, S->row_ptr, S->col_idx, batch->h[6], batch->h[7], u_out, batch->d_scale_s,
+                                  D->val, st));
+    LAUNCH(ctx, launch_trace(batch, S->row_ptr, S->col_idx, D->val, S->val, ne_partial, q_mol, st));
+    return NOLSM_OK;
+  }
   LAUNCH(ctx, launch_density(batch, x_ref(batch), sinv_ptr(batch), S->row_ptr, S->col_idx, D->val,
                              ne_diag, batch->h[4], batch->x_pending_split ? batch->h[5] : nullptr, u_thin, st));
   LAUNCH(ctx, launch_trace(batch, S->row_ptr, S->col_idx, D->val, S->val, ne_partial, q_mol, st));
@@ -1317,6 +1368,12 @@ extern "C" nolsm_status nolsm_solve_mu(nolsm_ctx *ctx, const nolsm_bsr *H, const
   if (!(mu_lo < mu_hi) || max_steps <= 0) { ctx->err = "need mu_lo < mu_hi and max_steps > 0"; return NOLSM_EINVAL; }
   cudaStream_t st = (cudaStream_t)stream;
   const int prec = effective_precision(ctx, precision);
+  if ((ctx->cfg.flags & NOLSM_FLAG_LOWDIN) != 0 &&
+      (prec == NOLSM_FP16_FP32 || ctx->eval_energy || use_simt(ctx) || !ctx->umma_ok || ctx->has_model)) {
+    ctx->err = "NOLSM_FLAG_LOWDIN: FP32 mode of nolsm_solve_mu only (it needs S^-1/2 at FP32 quality; no energy "
+               "products, no generated elements)";
+    return NOLSM_EINVAL;
+  }
   float tol = 0.f;
   int max_iter = 0, fixed_iter = -1;
   resolve_sign_args(ctx, prec, &tol, &max_iter, &fixed_iter);
@@ -1384,7 +1441,8 @@ extern "C" nolsm_status nolsm_solve_mu(nolsm_ctx *ctx, const nolsm_bsr *H, const
   // B_j (FP32, padded slab) and the own columns of S_j^-1 lets steps 2.. start at the sign iteration.
   float *cache = nullptr;
   std::vector<size_t> cache_off(plan.size() + 1, 0), cache_sq(plan.size(), 0);
-  if (!resident && max_steps > 1 && ctx->cfg.cache_bytes >= 0 && !use_simt(ctx) && ctx->umma_ok) {
+  if (!resident && max_steps > 1 && ctx->cfg.cache_bytes >= 0 && !use_simt(ctx) && ctx->umma_ok &&
+      (ctx->cfg.flags & NOLSM_FLAG_LOWDIN) == 0) {   // (the Loewdin form keeps Z in the workspace: no cache)
     for (size_t bi = 0; bi < plan.size(); ++bi) {
       int max_n = 0;
       size_t sq = 0;     // B_j packed to its true n_j x n_j part
@@ -1463,6 +1521,7 @@ extern "C" nolsm_status nolsm_solve_mu(nolsm_ctx *ctx, const nolsm_bsr *H, const
         // the FP32 copy of T_j(H) is only read by the energy products (nolsm_evaluate) and the SIMT debug path
         const bool need32 = ctx->eval_energy || use_simt(ctx) || !ctx->umma_ok;
         const bool fast32 = prec != NOLSM_FP16_FP32 && !ctx->eval_energy && ctx->inv_refine_default &&
+                            (ctx->cfg.flags & NOLSM_FLAG_LOWDIN) == 0 &&
                             ctx->cfg.inv_tol <= 0.f && (ctx->cfg.flags & NOLSM_FLAG_NO_PREDICT) == 0;
         rc = build_submatrices_impl(ctx, H, S, r.begin, r.count, kOwnSlot + (resident ? (int)bi : 0), units, &b, st,
                                     need32, need32, fast32);

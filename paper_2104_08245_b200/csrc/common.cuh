@@ -113,6 +113,8 @@ struct nolsm_batch {
   bool x0_built = false;                // X0 for mu = x0_mu is in place (written by the prepare stage), d_scale set
   double x0_mu = 0.0;
   bool b32_built = true;                // u3 holds B (false: the whole path went from B0 straight to X0)
+  bool lowdin = false;                  // prepared in the symmetric Loewdin form (NOLSM_FLAG_LOWDIN): u3 = S^-1/2 H S^-1/2,
+                                        // own columns of u2 = (s_S S^-1)^1/2 = Z, Z as split pair in (h6, h7), s_S in d_scale_s
   bool sinv_own_only = false;           // S^-1 was refined in its own columns only (nolsm_solve_mu): no full S^-1
   int32_t sign_ops = 2;           // products per sign iteration of the last chain (3 with NOLSM_FLAG_ORDER3)
   bool x_split = false;           // the sign iterate lives as hi (h[iters & 1]) + lo * 2^-11 (h[2]); u[0] holds X in
@@ -138,6 +140,7 @@ struct nolsm_batch {
   float *d_scale = nullptr;       // [count] s_j of the sign scaling
   float *d_alpha = nullptr;       // [count][8] alpha_k of the scaled Newton-Schulz start (gap_hint)
   float *d_norm = nullptr;        // [2][count] scratch for norm bounds
+  float *d_scale_s = nullptr;     // [count] s_S of the Loewdin form (d_scale is reused by the sign iteration)
   float *d_norm_s = nullptr;      // [2][count] norm bound of S from the builder (s_norm_built)
   float *d_colpart = nullptr;     // [count][ld/128][ld] column-sum shares of the row strips (k_norm_bound)
   size_t colpart_cap = 0;
@@ -235,7 +238,9 @@ cudaError_t launch_density_grouped(const nolsm_batch *b, const XRef &x, const fl
 // thin_kernels.cu
 cudaError_t launch_density_split(const nolsm_batch *b, const XRef &x, const float *sinv, const int32_t *row_ptr,
                                  const int32_t *col_idx, float *d_val, double *ne_diag, const __half *e_hi,
-                                 const __half *e_lo, float *u_thin, cudaStream_t st);
+                                 const __half *e_lo, float *u_thin, cudaStream_t st, float *thin_out = nullptr);
+cudaError_t launch_scaled_out(const nolsm_batch *b, const int32_t *row_ptr, const int32_t *col_idx, const __half *a_hi,
+                              const __half *a_lo, float *thin_in, const float *scale, float *d_val, cudaStream_t st);
 cudaError_t launch_own_refine(const nolsm_batch *b, const int32_t *row_ptr, const int32_t *col_idx, const __half *s_hi,
                               const __half *s_lo, const __half *a0, float *thin, float *out32, int rounds,
                               cudaStream_t st);
@@ -256,6 +261,8 @@ cudaError_t launch_energy(const nolsm_batch *b, const int32_t *row_ptr, const fl
 // dense helpers
 cudaError_t launch_norm_bound(const nolsm_batch *b, const float *a, float mu, bool symmetric, float *norm2,
                               cudaStream_t st);
+cudaError_t launch_canon_pair(const nolsm_batch *b, const int32_t *iters, const __half *hi0, const __half *lo0,
+                              __half *hi1, __half *lo1, cudaStream_t st);
 cudaError_t launch_norm_bound16(const nolsm_batch *b, const __half *a, float mu, float *norm2, cudaStream_t st);
 cudaError_t launch_x0_scale(const nolsm_batch *b, const float *norm2, float slack, float *scale_out, cudaStream_t st);
 cudaError_t launch_init_inverse(const nolsm_batch *b, const float *s, const float *norm2, float *y32,

@@ -352,6 +352,42 @@ cudaError_t launch_init_z1(const nolsm_batch *b, const __half *s_hi, const __hal
   return cudaGetLastError();
 }
 
+// The final iterate of a ping-pong chain lives in one of two split pairs, by the parity of the submatrix's iteration
+// count ((iters[m] + 1) & 1, ChainProgram::parity_from_iters).  This copies pair 0 onto pair 1 where the parity is 0,
+// so that afterwards every submatrix has it in pair 1 (for consumers that run after iters has been reused).
+__global__ void __launch_bounds__(256)
+k_canon_pair(const int32_t *__restrict__ dims, const int32_t *__restrict__ iters, int ld, int64_t slab,
+             const __half *__restrict__ hi0, const __half *__restrict__ lo0, __half *__restrict__ hi1,
+             __half *__restrict__ lo1) {
+  const int mat = blockIdx.y;
+  if (((iters[mat] + 1) & 1) != 0) return;
+  const int P = padded_dim(dims[mat]);
+  const int c0 = blockIdx.x * kElemCols;
+  if (c0 >= P) return;
+  for (int r = 8 * threadIdx.x; r < P; r += 8 * blockDim.x) {
+    const int64_t off = (int64_t)mat * slab + (int64_t)c0 * ld + r;
+    uint4 h[kElemCols], l[kElemCols];
+#pragma unroll
+    for (int u = 0; u < kElemCols; ++u) {
+      h[u] = *reinterpret_cast<const uint4 *>(hi0 + off + (int64_t)u * ld);
+      l[u] = *reinterpret_cast<const uint4 *>(lo0 + off + (int64_t)u * ld);
+    }
+#pragma unroll
+    for (int u = 0; u < kElemCols; ++u) {
+      *reinterpret_cast<uint4 *>(hi1 + off + (int64_t)u * ld) = h[u];
+      *reinterpret_cast<uint4 *>(lo1 + off + (int64_t)u * ld) = l[u];
+    }
+  }
+}
+
+cudaError_t launch_canon_pair(const nolsm_batch *b, const int32_t *iters, const __half *hi0, const __half *lo0,
+                              __half *hi1, __half *lo1, cudaStream_t st) {
+  if (b->count == 0) return cudaSuccess;
+  k_canon_pair<<<elem8_grid(b), elem8_threads(b), 0, st>>>(b->d_dims, iters, b->ld, (int64_t)b->ld * b->ld, hi0, lo0,
+                                                            hi1, lo1);
+  return cudaGetLastError();
+}
+
 // X0 = (B - mu I)/s  (Eq. 9 with the rescaling of PAPER.md:138), s from the norm bound or from the
 // caller (scale_in, dense microbench).  Padded diagonal = 1: a fixed point of the iteration that adds
 // nothing to the residual (reading 19).

@@ -25,7 +25,7 @@ constexpr int kThinRows = 64 * kThinRowWarps;   // rows of A per row block
 constexpr int kThinCtaRows = kThinRows;  // rows per CTA (row blocks one after the other: the staged thin operand serves both)
 constexpr int kThinSlices = 8 / kThinRowWarps;     // k slices per CTA, summed through shared memory in a fixed order (run-to-run bitwise equal)
 
-enum ThinMode { kDensity = 0, kLastHalf = 1, kOwnResid = 2, kOwnCorrect = 3 };
+enum ThinMode { kDensity = 0, kLastHalf = 1, kOwnResid = 2, kOwnCorrect = 3, kScaledOut = 4 };
 
 struct ThinArgs {
   const int32_t *row_ptr, *col_idx;
@@ -41,6 +41,8 @@ struct ThinArgs {
   float *d_val;                      // kDensity: column-owned block store
   double *ne_diag;                   // kDensity: sum of 1 - X_rr over the own rows, or null
   float *out32;                      // kOwnCorrect: FP32 S^-1, own columns written
+  float *thin_out;                   // kDensity: when set, 1/2 (V - X V) goes to this [count][6][ld] scratch instead of d_val
+  const float *scale;                // kScaledOut: d_val = (A thin) / scale[mat]  (Loewdin form: D[:, own] = Z U / s_S)
   int v32;                           // kOwnResid / kOwnCorrect: the current V is in the own columns of sinv (a later
                                      // refinement round) instead of being A0's own columns
 };
@@ -152,7 +154,7 @@ __global__ void __launch_bounds__(kThinThreads, 2) k_thin_mma(const ThinArgs a) 
       if (a.v32) return *reinterpret_cast<const float2 *>(sj + (int64_t)(own0 + p) * ld + k);
       return __half22float2(*reinterpret_cast<const __half2 *>(a0j + (int64_t)(own0 + p) * ld + k));
     } else {
-      const float *src = (kMode == kOwnCorrect || (kMode == kDensity && a.folded)) ? tj + (int64_t)p * ld
+      const float *src = (kMode == kOwnCorrect || kMode == kScaledOut || (kMode == kDensity && a.folded)) ? tj + (int64_t)p * ld
                                                                                   : sj + (int64_t)(own0 + p) * ld;
       return *reinterpret_cast<const float2 *>(src + k);
     }
@@ -224,7 +226,7 @@ __global__ void __launch_bounds__(kThinThreads, 2) k_thin_mma(const ThinArgs a) 
 #pragma unroll
       for (int u = 0; u < 4; ++u) {
         const int i = base + u * kThinThreads;
-        if constexpr (kMode == kDensity) { rr[u] = i / NOLSM_BS; pp[u] = i - rr[u] * NOLSM_BS; }   // [n][6] block column of D
+        if constexpr (kMode == kDensity || kMode == kScaledOut) { rr[u] = i / NOLSM_BS; pp[u] = i - rr[u] * NOLSM_BS; }   // [n][6] block column of D
         else { pp[u] = i / kThinRows; rr[u] = i - pp[u] * kThinRows; }                              // [6][ld] thin / dense columns
         const int r = rb + rr[u];
         v[u] = 0.f;
@@ -239,7 +241,12 @@ __global__ void __launch_bounds__(kThinThreads, 2) k_thin_mma(const ThinArgs a) 
         const int r = rb + rr[u], p = pp[u];
         if (r >= n) continue;
         const float c = total(rr[u] * NOLSM_BS + p);
-        if constexpr (kMode == kDensity) a.d_val[(int64_t)lo * 36 + (int64_t)r * NOLSM_BS + p] = 0.5f * (v[u] - c);
+        if constexpr (kMode == kDensity) {
+          if (a.thin_out) a.thin_out[((int64_t)mat * NOLSM_BS + p) * ld + r] = 0.5f * (v[u] - c);
+          else a.d_val[(int64_t)lo * 36 + (int64_t)r * NOLSM_BS + p] = 0.5f * (v[u] - c);
+        } else if constexpr (kMode == kScaledOut) {
+          a.d_val[(int64_t)lo * 36 + (int64_t)r * NOLSM_BS + p] = c / a.scale[mat];
+        }
         else if constexpr (kMode == kLastHalf) tj[(int64_t)p * ld + r] = fmaf(0.5f, c, v[u]);
         else if constexpr (kMode == kOwnResid) tj[(int64_t)p * ld + r] = (r == own0 + p ? 1.f : 0.f) - c;
         else a.out32[(int64_t)mat * a.slab + (int64_t)(own0 + p) * ld + r] = v[u] + c;
@@ -298,7 +305,7 @@ ThinArgs base_args(const nolsm_batch *b, const int32_t *row_ptr, const int32_t *
 // first, then D[:, own] = 1/2 (V - X_k U).
 cudaError_t launch_density_split(const nolsm_batch *b, const XRef &x, const float *sinv, const int32_t *row_ptr,
                                  const int32_t *col_idx, float *d_val, double *ne_diag, const __half *e_hi,
-                                 const __half *e_lo, float *u_thin, cudaStream_t st) {
+                                 const __half *e_lo, float *u_thin, cudaStream_t st, float *thin_out) {
   if (b->count == 0) return cudaSuccess;
   if (u_thin) {
     ThinArgs h = base_args(b, row_ptr, col_idx);
@@ -319,6 +326,7 @@ cudaError_t launch_density_split(const nolsm_batch *b, const XRef &x, const floa
   a.e_hi = e_hi;
   a.e_lo = e_lo;
   a.d_val = d_val;
+  a.thin_out = thin_out;
   a.ne_diag = ne_diag;
   return thin_launch<kDensity>(b, a, st);
 }
@@ -352,4 +360,18 @@ cudaError_t launch_own_refine(const nolsm_batch *b, const int32_t *row_ptr, cons
     if (e != cudaSuccess) return e;
   }
   return cudaSuccess;
+}
+
+// Loewdin form: D[:, own] = S^-1/2 P S^-1/2[:, own] = Z U / s_S with U = P Z[:, own] in thin_in
+// ([count][6][ld]) and Z = (S / s_S)^-1/2 as a split pair; written to the column-owned block store.
+cudaError_t launch_scaled_out(const nolsm_batch *b, const int32_t *row_ptr, const int32_t *col_idx, const __half *a_hi,
+                              const __half *a_lo, float *thin_in, const float *scale, float *d_val, cudaStream_t st) {
+  if (b->count == 0) return cudaSuccess;
+  ThinArgs a = base_args(b, row_ptr, col_idx);
+  a.a_hi[0] = a.a_hi[1] = a_hi;
+  a.a_lo[0] = a.a_lo[1] = a_lo;
+  a.thin = thin_in;
+  a.scale = scale;
+  a.d_val = d_val;
+  return thin_launch<kScaledOut>(b, a, st);
 }

@@ -414,6 +414,39 @@ def test_fp32_whole_path_two_refinements(nolsm, mid_system, mid_solution):
     assert fast[1] < slow[1] and fast[2] < slow[2]      # fewer products, fewer iterations of Eq. 15-17
 
 
+@pytest.mark.parametrize("which", ["tiny", "mid"])
+def test_lowdin_form(nolsm, tiny_system, tiny_solution, mid_system, mid_solution, which):
+    """SURVEY 8(f)#4, NOLSM_FLAG_LOWDIN: sign of the SYMMETRIC S^-1/2 H S^-1/2 - mu I with S^-1/2 from Eq. 15-17, and
+    D[:, own] = Z (1/2 (I - X~)) Z[:, own] / s as thin products.  Same D, N and populations as the oracle (whose Loewdin
+    restatement is pinned against the generalized eigenproblem in test_oracle_pins.py) at the FP32 tolerances; the
+    flag is refused in FP16 mode."""
+    import oracle.nolsm_oracle as orc
+    import torch
+    system, solution = (tiny_system, tiny_solution) if which == "tiny" else (mid_system, mid_solution)
+    sols = solution["solutions"]
+    H, S = _device_system(nolsm, system)
+    ctx = nolsm.Context(nolsm.Config(precision=1, flags=nolsm.FLAG_LOWDIN))
+    q = torch.zeros(system.n_mol, dtype=torch.float64, device="cuda")
+    mu, ne, D, st = ctx.solve_mu(H, S, system.n_electrons, MU - 0.1, MU + 0.1, tol_ne_per_mol=-1.0, max_steps=1,
+                                 q_mol=q)
+    assert mu == MU
+    d_ref = orc.density_blocks(sols, system.row_ptr, MU)
+    assert np.abs(D.val.cpu().numpy() - d_ref).max() < TOL_D[1]
+    assert abs(ne - orc.electron_count(sols, MU)) / system.n_mol <= TOL_NE_PER_MOL
+    pop = np.array([s.population(MU) for s in sols])
+    assert np.abs(q.cpu().numpy() - pop).max() < 2e-5
+    assert st.last.n_unconverged == 0
+    # a second evaluation on the same context (bisection step with resident batches) and the streaming path
+    mu2, ne2, D2, st2 = ctx.solve_mu(H, S, system.n_electrons, MU - 0.3, MU + 0.1, tol_ne_per_mol=-1.0, max_steps=2)
+    d_ref2 = orc.density_blocks(sols, system.row_ptr, mu2)
+    assert np.abs(D2.val.cpu().numpy() - d_ref2).max() < TOL_D[1]
+    ctx.close()
+    ctx16 = nolsm.Context(nolsm.Config(precision=0, flags=nolsm.FLAG_LOWDIN))
+    with pytest.raises(nolsm.NolsmError, match="LOWDIN"):
+        ctx16.solve_mu(H, S, system.n_electrons, MU - 0.1, MU + 0.1, max_steps=1)
+    ctx16.close()
+
+
 # ---------------------------------------------------------------------------------------------
 # BASELINE sizes, sampled (the oracle solves the sampled molecules one by one)
 # ---------------------------------------------------------------------------------------------

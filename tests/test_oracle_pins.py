@@ -309,6 +309,29 @@ def test_refinements_of_the_operator_cube_the_inverse_error(mid_system_cpu):
     assert np.abs(b2 - b_exact).max() < 1e-6 * np.abs(b_exact).max()
 
 
+def test_lowdin_form_gives_the_same_density(tiny_solution, mid_system_cpu):
+    """the symmetric Loewdin form S^-1/2 (1/2 (I - sign(S^-1/2 H S^-1/2 - mu I))) S^-1/2 is the density of
+    the generalized problem (Eq. 12), and the thin-product route the CUDA path takes -- U = P~ Z[:, own],
+    D[:, own] = Z U / s with Z = (S/s)^-1/2 -- reproduces its own columns."""
+    sols = [tiny_solution["solutions"][7]]
+    sols.append(orc.solve_molecule(mid_system_cpu.row_ptr, mid_system_cpu.col_idx, mid_system_cpu.h_val,
+                                   mid_system_cpu.s_val, 100))
+    for sol in sols:
+        own = orc.own_position(sol.nbrs, sol.j)
+        cols = np.arange(own * 6, own * 6 + 6)
+        d_low = orc.density_columns_lowdin(sol.h_sub, sol.s_sub, cols, -0.85)
+        assert np.abs(d_low - sol.density_columns(-0.85)).max() < 1e-10
+        # the factored route, with an arbitrary scale s
+        s_scale = 0.5 * np.abs(sol.s_sub).sum(0).max()
+        sl, sv = np.linalg.eigh(sol.s_sub / s_scale)
+        z = (sv / np.sqrt(sl)) @ sv.T
+        at = z @ sol.h_sub @ z / s_scale
+        x = orc.newton_schulz_sign(at + 0.85 * np.eye(len(z)), 40,
+                                   scale=np.sqrt(np.abs(at + 0.85 * np.eye(len(z))).sum(0).max() ** 2) / 1.5)
+        u = 0.5 * (z[:, cols] - x @ z[:, cols])
+        assert np.abs(z @ u / s_scale - sol.density_columns(-0.85)).max() < 1e-9
+
+
 def test_last_sign_update_folded_into_thin_products(tiny_system, tiny_solution):
     """Reading 9: with E_k = I - X_k^2, X_{k+1} V = X_k (V + 1/2 E_k V) for any thin V, so the own columns of
     D = 1/2 (I - X_{k+1}) S^-1 follow from X_k and E_k without forming X_{k+1}."""
