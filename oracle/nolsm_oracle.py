@@ -200,6 +200,35 @@ def newton_schulz_sign(a, n_iter, scale=None, history=False):
     return (x, np.array(res)) if history else x
 
 
+def rescaled_first_step_factor(x0):
+    """DESIGN.md reading 5, rescaled first iteration: rho(X0)^2 = rho(X0^2) <= ||X0^2||_1 (a spectral radius is bounded by
+    any induced norm), so a X0 with a = 1.6 / sqrt(||X0^2||_1) has its spectrum inside [-1.6, 1.6], inside the interval
+    (-sqrt 3, sqrt 3) on which Eq. 9 converges to the sign.  Clamped to [1, 1.6]: never scale down (X0 already lies in
+    [-1.5, 1.5]), and not up by more than 1.6 (the update below multiplies the rounding of E_0 by a^3)."""
+    b2 = min(float(np.abs(x0 @ x0).sum(0).max()), 2.25)
+    a = 1.6 / np.sqrt(b2) if b2 > 0.0 else 1.0
+    return float(min(max(a, 1.0), 1.6))
+
+
+def newton_schulz_sign_rescaled(a, n_iter, scale=None, history=False):
+    """Eq. 9-10 with the first iteration applied to a X0 (rescaled_first_step_factor), in the form the CUDA path uses:
+    with E_0 = I - X0^2 (formed for the stop rule anyway), a X0 (I + 1/2 (I - a^2 X0^2)) =
+    a (3/2 - 1/2 a^2) X0 + 1/2 a^3 X0 E_0.  The other iterations are Eq. 9 in the correction form.  n_iter counts all."""
+    n = a.shape[0]
+    eye = np.eye(n)
+    x = a / (1.0 if scale is None else scale)
+    res = []
+    for k in range(n_iter):
+        e = eye - x @ x
+        res.append(np.linalg.norm(e, "fro") / np.sqrt(n))
+        if k == 0:
+            al = rescaled_first_step_factor(x)
+            x = al * (1.5 - 0.5 * al * al) * x + 0.5 * al ** 3 * (x @ e)
+        else:
+            x = x + 0.5 * x @ e
+    return (x, np.array(res)) if history else x
+
+
 def newton_schulz_sign_scaled(a, n_iter, scale, gap, history=False):
     """Scaled start of Eq. 9 (the rescaling PAPER.md:138 allows): with l_k a lower
     bound on the moduli of the eigenvalues of X_k (all <= 1), X_{k+1} = 1/2 a_k X_k (3I - a_k^2 X_k^2),

@@ -14,6 +14,7 @@ FLAG_UNIT_SCALE = 16
 FLAG_ORDER3 = 32
 FLAG_NO_PREDICT = 64
 FLAG_LOWDIN = 128
+FLAG_NO_RESCALE = 256
 STATUS = {0: "NOLSM_OK", 1: "NOLSM_EINVAL", 2: "NOLSM_ENOMEM", 3: "NOLSM_ECUDA", 4: "NOLSM_ENOTSPD",
           5: "NOLSM_ENOCONV", 6: "NOLSM_EBRACKET"}
 

@@ -907,6 +907,8 @@ static nolsm_status sign_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, double mu, 
   // fold_last: stop right after the E_k that passes the test; the caller applies X_{k+1} = X_k + 1/2 X_k E_k
   // only to the own columns of S^-1 (k_last_half), instead of forming it with an n^3 product
   const bool order3 = fp16 && (ctx->cfg.flags & NOLSM_FLAG_ORDER3) != 0;
+  bool rescale = false;
+  b->sign_iter0 = 0;
   if (order3) fold_last = false;   // the folded update is Eq. 9's
   pg.stop_early = fold_last ? 1 : 0;
   b->x_pending = fold_last;
@@ -927,6 +929,10 @@ static nolsm_status sign_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, double mu, 
     set2(e.a, 0, 1); set2(e.b, 0, 1); set2(e.out16, 4, 4);
     set2(x.a, 0, 1); set2(x.b, 4, 4); set2(x.cin16, 0, 1); set2(x.cin16_lo, 2, 2);
     set2(x.out16, 1, 0); set2(x.out16_lo, 2, 2); x.lo_stream = 1;
+    // rescaled first iteration (reading 5): ||X0^2||_1 from E_0's epilogue bounds rho(X0) tighter than the O(n^2)
+    // norm bound X0 was scaled with; iteration 0 is applied to a X0 with a = 1.6 / sqrt(||X0^2||_1) >= 1
+    rescale = !order3 && !scale_in && ctx->cfg.gap_hint <= 0.f && pg.fixed_iter <= 0 && max_iter > 1 &&
+              (ctx->cfg.flags & NOLSM_FLAG_NO_RESCALE) == 0;
     if (order3) {
       // X <- X (I + 1/2 E + 3/8 E^2) = X + X G,  G = 1/2 E + 3/8 E E  (refs [51],[52]); G in a half the
       // iterations do not use: the builder's split copy of S (sparse batches, free after the prepare stage) or h5
@@ -955,6 +961,25 @@ static nolsm_status sign_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, double mu, 
     pg.use_alpha_tab = 1;
   }
   if (timed) NOLSM_CUDA(ctx, cudaEventRecord(ctx->tev[0], st));
+  if (rescale) {
+    // Iteration 0 in a launch of its own (the kernel instantiation with the column norms and the per-matrix scale;
+    // the other iterations keep the plain one): E_0 gathers ||X0^2||_1, the X update applies a (ChainOp::colnorm 2)
+    ChainProgram p0 = one_shot(pg.group);
+    p0.n_ops = 2;
+    p0.tol = tol;
+    p0.ops[0] = e;
+    p0.ops[1] = x;
+    p0.ops[0].colnorm = p0.ops[1].colnorm = 2;
+    CHECK(run_chain(ctx, b, p0, nullptr, false, st));
+    // the adaptive launch starts at iteration 1: its tables are indexed by the parity of ITS iteration count
+    auto flip = [](int32_t (&d)[2]) { std::swap(d[0], d[1]); };
+    for (ChainOp *o : {&e, &x}) {
+      flip(o->a); flip(o->b); flip(o->a_lo); flip(o->b_lo); flip(o->out16); flip(o->out16_lo);
+      flip(o->cin16); flip(o->cin16_lo);
+    }
+    pg.max_iter = max_iter - 1;
+    b->sign_iter0 = 1;
+  }
   CHECK(run_chain(ctx, b, pg, nullptr, true, st));
   if (timed) NOLSM_CUDA(ctx, cudaEventRecord(ctx->tev[1], st));
   NOLSM_CUDA(ctx, cudaMemcpyAsync(b->d_sched + 5, b->d_sched + 2, sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
@@ -1132,7 +1157,9 @@ static float *bmat_ptr(const nolsm_batch *b) { return b->engine_simt ? b->u[2] :
 static float *x_ptr(const nolsm_batch *b) { return (b->engine_simt && b->x_parity) ? b->u[3] : b->u[0]; }
 static XRef x_ref(const nolsm_batch *b) {
   if (b->x_split && !b->engine_simt) {
-    if (b->prepared_precision == NOLSM_FP16_FP32) return XRef{nullptr, b->h[0], b->h[1], b->h[2], b->h[2]};
+    if (b->prepared_precision == NOLSM_FP16_FP32)   // (buffer by the parity of d_iters, which may count from iteration 1)
+      return (b->sign_iter0 & 1) ? XRef{nullptr, b->h[1], b->h[0], b->h[2], b->h[2]}
+                                 : XRef{nullptr, b->h[0], b->h[1], b->h[2], b->h[2]};
     return XRef{nullptr, b->h[0], b->h[2], b->h[1], b->h[3]};
   }
   return XRef{x_ptr(b), nullptr, nullptr, nullptr, nullptr};
@@ -1193,7 +1220,7 @@ static nolsm_status collect_stats(nolsm_ctx *ctx, nolsm_batch *b, float tol, int
     const double P3 = (double)round_up(b->n_host[m], NOLSM_TILE_M) * round_up(b->n_host[m], 64) * round_up(b->n_host[m], 64);
     s->flops_sign -= extra * 2.0 * n3;          // (2 it + 1) products instead of 2 (it + 1)
     s->flops_sign_padded -= extra * 2.0 * P3;
-    it[m] += extra;
+    it[m] += extra + b->sign_iter0;
     s->iter_min = std::min(s->iter_min, it[m]);
     s->iter_max = std::max(s->iter_max, it[m]);
     s->iter_sum += it[m];

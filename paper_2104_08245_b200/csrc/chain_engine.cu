@@ -520,12 +520,16 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
         // column sums of |E| (thread = column; two threads, one per row half, and ntl tiles add to a column): the
         // add returns the running total, and the largest running total of the product is its largest column sum
         const int kk = chainep::cmd_iter(c);
+        // (in fixed point, 2^-20: integer sums do not depend on the order of the atomics, so that what is derived from
+        // the norm is bitwise reproducible)
         if (t.colnorm && args.colsum != nullptr && kk < args.colslots) {
-          float tot = 0.f;
-          if (t.col < t.n)
-            tot = atomicAdd(&args.colsum[((size_t)kk * args.count + c.mat) * args.ld + t.col], t.abs_sum) + t.abs_sum;
-          for (int d = 16; d > 0; d >>= 1) tot = fmaxf(tot, __shfl_xor_sync(0xffffffffu, tot, d));
-          if (lane == 0) atomicMax(&args.colmax[(size_t)kk * args.count + c.mat], __float_as_int(tot));
+          unsigned int tot = 0u;
+          if (t.col < t.n) {
+            const unsigned int mine = (unsigned int)fminf(t.abs_sum * chainep::kColFix, 4.0e9f);
+            tot = atomicAdd(&args.colsum[((size_t)kk * args.count + c.mat) * args.ld + t.col], mine) + mine;
+          }
+          for (int d = 16; d > 0; d >>= 1) tot = max(tot, __shfl_xor_sync(0xffffffffu, tot, d));
+          if (lane == 0) atomicMax(&args.colmax[(size_t)kk * args.count + c.mat], tot);
         }
       }
       // this warp's direct stores and residual atomic are issued: join the tile's completion
@@ -592,9 +596,9 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
 // The instantiations that exist: the sign iteration / plain one-shot products (0), all-split programs of the FP32 mode,
 // the Eq. 15-17 chain with its column norms, the half-split residual R, the shifted B1 -> X0 product, and everything.
 typedef void (*ChainKernel)(const ChainArgs);
-constexpr int kNumInst = 6;
+constexpr int kNumInst = 7;
 const int kInstFeat[kNumInst] = {0, chainep::kFeatSplitAll, chainep::kFeatColNorm, chainep::kFeatSplitAny,
-                                 chainep::kFeatShift, chainep::kFeatFull};
+                                 chainep::kFeatShift, chainep::kFeatRescale, chainep::kFeatFull};
 template <bool kPair>
 static ChainKernel chain_kernel_of(int feat) {
   switch (feat) {
@@ -603,6 +607,7 @@ static ChainKernel chain_kernel_of(int feat) {
     case chainep::kFeatColNorm: return k_chain<kPair, chainep::kFeatColNorm>;
     case chainep::kFeatSplitAny: return k_chain<kPair, chainep::kFeatSplitAny>;
     case chainep::kFeatShift: return k_chain<kPair, chainep::kFeatShift>;
+    case chainep::kFeatRescale: return k_chain<kPair, chainep::kFeatRescale>;
     default: return k_chain<kPair, chainep::kFeatFull>;
   }
 }
@@ -757,7 +762,8 @@ static int program_features(const ChainProgram &prog) {
   for (int i = 0; i < prog.n_ops; ++i) {
     const ChainOp &o = prog.ops[i];
     if (o.cin32 >= 0 || o.cout32 >= 0) need |= kFeatFp32;
-    if (o.colnorm) need |= kFeatColNorm;
+    if (o.colnorm == 1) need |= kFeatColNorm;
+    if (o.colnorm == 2) need |= kFeatRescale;
     if (o.diag != 0.f || o.use_div == 2) need |= kFeatShift;
     const bool s0 = o.a_lo[0] >= 0 && o.b_lo[0] >= 0, s1 = o.a_lo[1] >= 0 && o.b_lo[1] >= 0;
     const bool p0 = o.a_lo[0] < 0 && o.b_lo[0] < 0, p1 = o.a_lo[1] < 0 && o.b_lo[1] < 0;
@@ -813,6 +819,7 @@ cudaError_t launch_chain(nolsm_ctx *ctx, const nolsm_batch *b, const ChainProgra
   a.state = b->d_state;
   a.iters = b->d_iters;
   a.alpha_tab = prog.use_alpha_tab ? b->d_alpha : nullptr;
+  a.alpha_rt = prog.use_alpha_tab ? nullptr : b->d_alpha;   // (the two scalings exclude one another)
   a.tile_counter = b->d_tile_counter;
   a.resid2 = b->d_resid2;
   a.colsum = nullptr;
@@ -821,9 +828,9 @@ cudaError_t launch_chain(nolsm_ctx *ctx, const nolsm_batch *b, const ChainProgra
   const int strips = colpart_strips(b->ld);   // d_colpart: strips * count * ld floats (norm-bound scratch, free here)
   for (int i = 0; i < prog.n_ops; ++i)
     if (prog.ops[i].colnorm) {   // strips - 1 iteration slots of column sums, the last strip: maxima
-      a.colsum = b->d_colpart;
+      a.colsum = reinterpret_cast<unsigned int *>(b->d_colpart);
       a.colslots = strips - 1;
-      a.colmax = reinterpret_cast<int32_t *>(b->d_colpart + (size_t)(strips - 1) * b->count * b->ld);
+      a.colmax = reinterpret_cast<unsigned int *>(b->d_colpart + (size_t)(strips - 1) * b->count * b->ld);
     }
   a.lastres = b->d_lastres;
   const int slots = std::min(prog.max_iter, NOLSM_MAX_RESID_SLOTS);

@@ -61,15 +61,18 @@ struct ChainArgs {
   float *resid2, *lastres;
   // op with colnorm, iteration k < colslots: colsum[k][count][ld] column sums of |E_k| (zero at launch; every thread
   // adds its rows' share and learns the running total), colmax[k][count] the largest running total seen = ||E_k||_1
-  // once the product is complete (totals only grow), as the bit pattern of a non-negative float
-  float *colsum;
-  int32_t *colmax;
+  // once the product is complete (totals only grow)
+  unsigned int *colsum;       // (fixed point, kColFix)
+  unsigned int *colmax;
   int32_t colslots;
   // scaled Newton-Schulz start (nolsm_config.gap_hint): alpha_tab[m * kAlphaSteps + k] = alpha_k of submatrix m
   // for iteration k < kAlphaSteps (1 afterwards); null = the plain iteration
   const float *alpha_tab;
+  // rescaled first sign iteration (ChainOp::colnorm == 2): alpha_rt[m], written when E_0 of submatrix m completes
+  float *alpha_rt;
 };
 constexpr int kAlphaSteps = 8;
+constexpr float kColFix = 1048576.f;   // column sums are accumulated as integers in units of 2^-20
 
 __device__ __forceinline__ void ld_tmem32(uint32_t taddr, uint32_t (&v)[32]) {
   asm volatile(
@@ -121,10 +124,22 @@ __device__ __forceinline__ void epi_complete(const ChainArgs &args, const TileCm
     args.lastres[c.mat] = res;
     // ||E_k||_1 (E_k is symmetric: >= ||E_k||_2) as the epilogues left it: the largest running total of a column sum
     float pred = -1.f;
-    if (o.colnorm && args.colsum != nullptr && k < args.colslots) {
-      const float b1 = __int_as_float(*reinterpret_cast<volatile int32_t *>(
-          &args.colmax[(size_t)k * args.count + c.mat]));
+    if (o.colnorm == 1 && args.colsum != nullptr && k < args.colslots) {
+      const float b1 = (float)*reinterpret_cast<volatile unsigned int *>(&args.colmax[(size_t)k * args.count + c.mat]) *
+                       (1.f / kColFix);
       pred = b1 * b1 * (0.75f + 0.25f * b1);   // >= ||E_{k+1}||_2 (ChainProgram::tol_pred)
+    }
+    if (o.colnorm == 2 && k == 0 && args.colsum != nullptr && args.alpha_rt != nullptr) {
+      // Rescaled first sign iteration (reading 5): rho(X0)^2 = rho(X0^2) <= ||X0^2||_1, known now.  X0 was
+      // scaled so that the O(n^2) norm bound on rho maps to 1.5, which on these matrices is 1.8 x too careful; the
+      // tighter bound is mapped to 1.6 (< sqrt 3, the edge of the convergence interval of Eq. 9; an eigenvalue that
+      // really sits at 1.6 goes to 0.35 and is back at 1 before the gap eigenvalues are) by applying the step to a X0.
+      const float b2 = (float)*reinterpret_cast<volatile unsigned int *>(&args.colmax[c.mat]) * (1.f / kColFix);
+      float a = 1.f;
+      if (b2 == b2 && b2 > 0.f) a = 1.6f * rsqrtf(fminf(b2, 2.25f));   // rho <= 1.5 holds in any case
+      // a <= 1.6: the update a (3/2 - 1/2 a^2) X0 + 1/2 a^3 X0 E_0 multiplies the FP16 rounding of E_0 by a^3, and
+      // with a much larger a (a norm bound that was far off) it cancels catastrophically
+      args.alpha_rt[c.mat] = fminf(fmaxf(a, 1.f), 1.6f);
     }
     const bool conv = res < pg.tol;   // false for a NaN residual
     bool stop = pg.fixed_iter > 0 ? (k + 1 >= pg.fixed_iter) : (conv || !(res == res));
@@ -319,6 +334,7 @@ struct EpiTile {
   const ChainOp *o;
   int par, n, col, h;         // col: this thread's column of the result; h: row quarter of every chunk
   bool split, ident, cin_direct, colnorm;
+  bool norm_product;          // colnorm sums |alpha * accumulator| (the product itself) instead of |result|
   float alpha, beta, diag;
   float abs_sum;              // colnorm: sum of |result| over this thread's rows of the tile (true n x n part)
   float *p32;                 // FP32 output, element (first row of this warp's quarter, col) or null
@@ -347,7 +363,8 @@ constexpr int kFeatColNorm = 4;     // column norms of the residual product (a-p
 constexpr int kFeatShift = 8;       // diagonal shift, per-matrix division of beta and the shift (X0 from B1's epilogue)
 constexpr int kFeatFp32 = 16;       // FP32 inputs / outputs (direct or through the staging buffers)
 constexpr int kFeatAlphaTab = 32;   // per-iteration scaling table (nolsm_config.gap_hint)
-constexpr int kFeatFull = 63 & ~kFeatSplitAll;
+constexpr int kFeatRescale = 64;    // first sign iteration rescaled from ||X0^2||_1 (ChainOp::colnorm == 2)
+constexpr int kFeatFull = 127 & ~kFeatSplitAll;
 template <int kFeat>
 __device__ __forceinline__ void epi_begin(const ChainArgs &args, const TileCmd &c, int col, int h, EpiTile &t) {
   const ChainOp &o = args.prog.ops[c.op];
@@ -360,11 +377,25 @@ __device__ __forceinline__ void epi_begin(const ChainArgs &args, const TileCmd &
   t.ident = o.mode == EPI_IDENT;
   t.abs_sum = 0.f;
   t.alpha = o.use_div ? o.alpha / args.alpha_div[c.mat] : o.alpha;
+  float rescale_beta = 1.f;
   if constexpr ((kFeat & kFeatSplitAll) != 0) t.split = true;
   else if constexpr ((kFeat & kFeatSplitAny) != 0) t.split = o.a_lo[t.par] >= 0;
   else t.split = false;
-  if constexpr ((kFeat & kFeatColNorm) != 0) t.colnorm = t.ident && o.colnorm != 0;
+  t.norm_product = false;
+  if constexpr ((kFeat & kFeatColNorm) != 0) t.colnorm = t.ident && o.colnorm == 1;
   else t.colnorm = false;
+  if constexpr ((kFeat & kFeatRescale) != 0) {
+    if (o.colnorm == 2 && cmd_iter(c) == 0) {
+      if (t.ident) {
+        t.colnorm = t.norm_product = true;         // E_0 = I - X0^2: column sums of |X0^2|
+      } else {
+        // X_1 = a X0 (I + 1/2 (I - a^2 X0^2)) = a (3/2 - 1/2 a^2) X0 + 1/2 a^3 X0 E_0, a from E_0's completion
+        const float a = *reinterpret_cast<volatile float *>(&args.alpha_rt[c.mat]);
+        t.alpha *= a * a * a;
+        rescale_beta = a * (1.5f - 0.5f * a * a);
+      }
+    }
+  }
   if constexpr ((kFeat & kFeatShift) != 0) {
     t.beta = o.use_div == 2 ? o.beta / args.alpha_div[c.mat] : o.beta;
     t.diag = o.use_div == 2 ? o.diag / args.alpha_div[c.mat] : o.diag;
@@ -372,6 +403,7 @@ __device__ __forceinline__ void epi_begin(const ChainArgs &args, const TileCmd &
     t.beta = o.beta;
     t.diag = 0.f;
   }
+  t.beta *= rescale_beta;
   if constexpr ((kFeat & kFeatAlphaTab) != 0) {
     if (args.alpha_tab != nullptr && cmd_iter(c) < kAlphaSteps) {
       // X_{k+1} = 1/2 a X (3I - a^2 X^2):  E = I - a^2 X X,  X' = a X + (1/2 a) X E
@@ -557,7 +589,10 @@ __device__ __forceinline__ float epi_chunks(const ChainArgs &args, const TileCmd
 #pragma unroll
         for (int jj = 0; jj < R; ++jj) {
           const float e = fmaf(-t.alpha, __uint_as_float(v[jj]), (jj == dj) ? 1.f : 0.f);
-          if (jj < nvalid) { ss = fmaf(e, e, ss); if (t.colnorm) t.abs_sum += fabsf(e); }
+          if (jj < nvalid) {
+            ss = fmaf(e, e, ss);
+            if (t.colnorm) t.abs_sum += t.norm_product ? fabsf(t.alpha * __uint_as_float(v[jj])) : fabsf(e);
+          }
           v[jj] = __float_as_uint(e);
         }
       } else {

@@ -116,6 +116,8 @@ struct nolsm_batch {
   bool lowdin = false;                  // prepared in the symmetric Loewdin form (NOLSM_FLAG_LOWDIN): u3 = S^-1/2 H S^-1/2,
                                         // own columns of u2 = (s_S S^-1)^1/2 = Z, Z as split pair in (h6, h7), s_S in d_scale_s
   bool sinv_own_only = false;           // S^-1 was refined in its own columns only (nolsm_solve_mu): no full S^-1
+  int32_t sign_iter0 = 0;         // iterations of the last sign chain that ran before its adaptive launch (0 or 1: the rescaled
+                                  // first iteration has a launch of its own); d_iters counts from there
   int32_t sign_ops = 2;           // products per sign iteration of the last chain (3 with NOLSM_FLAG_ORDER3)
   bool x_split = false;           // the sign iterate lives as hi (h[iters & 1]) + lo * 2^-11 (h[2]); u[0] holds X in
   bool x32_valid = false;         // FP32 only after join_x (reading 12)

@@ -447,6 +447,42 @@ def test_lowdin_form(nolsm, tiny_system, tiny_solution, mid_system, mid_solution
     ctx16.close()
 
 
+def test_rescaled_first_sign_iteration(nolsm, mid_system, mid_solution):
+    """DESIGN.md reading 5: the first product of the sign iteration (X0^2) also gives ||X0^2||_1 >= rho(X0)^2, and
+    iteration 0 is applied to a X0, a = 1.6 / sqrt(||X0^2||_1) in [1, 1.6] (oracle: newton_schulz_sign_rescaled, pinned in
+    test_oracle_pins.py).  Same D and N as the oracle with and without it (NOLSM_FLAG_NO_RESCALE), never more iterations,
+    and the result is bitwise reproducible although the norm is gathered with atomics (integer sums)."""
+    import oracle.nolsm_oracle as orc
+    sols = mid_solution["solutions"]
+    H, S = _device_system(nolsm, mid_system)
+    d_ref = orc.density_blocks(sols, mid_system.row_ptr, MU)
+    ne_ref = orc.electron_count(sols, MU)
+    out = {}
+    for flags in (0, nolsm.FLAG_NO_RESCALE):
+        ctx = nolsm.Context(nolsm.Config(precision=0, flags=flags))
+        runs = []
+        for rep in range(2):
+            mu, ne, D, st = ctx.solve_mu(H, S, mid_system.n_electrons, MU - 0.1, MU + 0.1, tol_ne_per_mol=-1.0,
+                                         max_steps=1)
+            runs.append(D.val.cpu().numpy().copy())
+        assert np.array_equal(runs[0].view(np.uint32), runs[1].view(np.uint32))
+        assert np.abs(runs[0] - d_ref).max() < TOL_D[0]
+        assert abs(ne - ne_ref) / mid_system.n_mol <= TOL_NE_PER_MOL
+        assert st.last.n_unconverged == 0 and st.last.worst_residual <= TOL_RESID
+        out[flags] = (st.last.iter_min, st.last.iter_max, st.last.iter_sum)
+        ctx.close()
+    assert out[0][1] <= out[nolsm.FLAG_NO_RESCALE][1] and out[0][2] < out[nolsm.FLAG_NO_RESCALE][2]
+    # the user-level entry point takes the same path: X against the oracle's sign function of the submatrix
+    ctx = nolsm.Context(nolsm.Config(precision=0))
+    batch = ctx.build_submatrices(H, S, 100, 4)
+    st = ctx.sign_batched(batch, MU)
+    x = batch.read(1, nolsm.MAT_X).cpu().numpy().astype(np.float64)
+    sol = sols[101]
+    sign_ref = np.eye(len(sol.s_sub)) - 2.0 * sol.density(MU) @ sol.s_sub
+    assert np.abs(x - sign_ref).max() < 2e-3 and orc.sign_residual(x) <= TOL_RESID
+    ctx.close()
+
+
 # ---------------------------------------------------------------------------------------------
 # BASELINE sizes, sampled (the oracle solves the sampled molecules one by one)
 # ---------------------------------------------------------------------------------------------

@@ -332,6 +332,41 @@ def test_lowdin_form_gives_the_same_density(tiny_solution, mid_system_cpu):
         assert np.abs(z @ u / s_scale - sol.density_columns(-0.85)).max() < 1e-9
 
 
+def test_rescaled_first_sign_iteration(tiny_solution, mid_system_cpu):
+    """Reading 5, rescaled first iteration: (1) the factor keeps the spectrum of a X0 inside [-1.6, 1.6]; (2) the update
+    a (3/2 - 1/2 a^2) X0 + 1/2 a^3 X0 E_0 IS Eq. 9 applied to a X0; (3) the iteration converges to the same sign
+    function (the eigenvector construction); (4) it never needs more iterations than the plain one, and on a
+    water-like submatrix scaled by the O(n^2) norm bound it needs one fewer."""
+    sols = [tiny_solution["solutions"][7]]
+    sols.append(orc.solve_molecule(mid_system_cpu.row_ptr, mid_system_cpu.col_idx, mid_system_cpu.h_val,
+                                   mid_system_cpu.s_val, 100))
+    fewer = 0
+    for sol in sols:
+        n = len(sol.s_sub)
+        eye = np.eye(n)
+        a = np.linalg.solve(sol.s_sub, sol.h_sub) + 0.85 * eye
+        scale = np.sqrt(np.abs(a).sum(0).max() * np.abs(a).sum(1).max()) / 1.5
+        x0 = a / scale
+        al = orc.rescaled_first_step_factor(x0)
+        rho = np.abs(np.linalg.eigvals(x0)).max()
+        assert 1.0 <= al <= 1.6 and al * rho <= 1.6 * (1 + 1e-12) and rho ** 2 <= np.abs(x0 @ x0).sum(0).max() * (1 + 1e-12)
+        e0 = eye - x0 @ x0
+        x1 = al * (1.5 - 0.5 * al * al) * x0 + 0.5 * al ** 3 * (x0 @ e0)
+        assert np.abs(x1 - 0.5 * (al * x0) @ (3 * eye - (al * x0) @ (al * x0))).max() < 1e-13
+        assert np.abs(orc.newton_schulz_sign_rescaled(a, 1, scale=scale) - x1).max() < 1e-14
+        # same limit as the plain iteration and as the construction from the generalized eigenvectors
+        x_res = orc.newton_schulz_sign_rescaled(a, 40, scale=scale)
+        x_plain = orc.newton_schulz_sign(a, 40, scale=scale)
+        sign_ref = eye - 2.0 * sol.density(-0.85) @ sol.s_sub          # sign(A) = I - 2 D S  (Eq. 12 solved for the sign)
+        assert np.abs(x_res - x_plain).max() < 1e-9 and np.abs(x_res - sign_ref).max() < 1e-8
+        _, r_res = orc.newton_schulz_sign_rescaled(a, 20, scale=scale, history=True)
+        _, r_plain = orc.newton_schulz_sign(a, 20, scale=scale, history=True)
+        k_res, k_plain = int(np.argmax(r_res < 1e-2)), int(np.argmax(r_plain < 1e-2))
+        assert 0 < k_res <= k_plain
+        fewer += k_plain - k_res
+    assert fewer >= 1
+
+
 def test_last_sign_update_folded_into_thin_products(tiny_system, tiny_solution):
     """Reading 9: with E_k = I - X_k^2, X_{k+1} V = X_k (V + 1/2 E_k V) for any thin V, so the own columns of
     D = 1/2 (I - X_{k+1}) S^-1 follow from X_k and E_k without forming X_{k+1}."""
