@@ -118,7 +118,7 @@ typedef struct {
                                   SYMMETRIC A~ = Z H_j Z / s - mu I = S^-1/2 H S^-1/2 - mu I, and
                                   D_j[:, own] = Z (1/2 (I - sign A~)) Z[:, own] / s.  Same D as the non-orthogonal
                                   form of Eq. 12 up to rounding; no S^-1, no B */
-#define NOLSM_FLAG_NO_RESCALE 256 /* FP16 mode: do not rescale the first sign iteration.  By default the first product of
+#define NOLSM_FLAG_NO_RESCALE 256 /* do not rescale the first sign iteration.  By default the first product of
                                   the iteration (X0^2) also yields ||X0^2||_1 >= rho(X0)^2, a tighter bound on the
                                   spectrum than the O(n^2) norm bound X0 was scaled with, and iteration 0 is applied to
                                   a X0, a = 1.6 / sqrt(||X0^2||_1) >= 1 ("rescaled so that its spectrum

@@ -955,6 +955,8 @@ static nolsm_status sign_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, double mu, 
     set2(x.a, 0, 2); set2(x.a_lo, 1, 3); set2(x.b, 4, 4); set2(x.b_lo, 5, 5);
     set2(x.cin16, 0, 2); set2(x.cin16_lo, 1, 3);
     set2(x.out16, 2, 0); set2(x.out16_lo, 3, 1);
+    rescale = !scale_in && ctx->cfg.gap_hint <= 0.f && pg.fixed_iter <= 0 && max_iter > 1 &&
+              (ctx->cfg.flags & NOLSM_FLAG_NO_RESCALE) == 0;
   }
   if (ctx->cfg.gap_hint > 0.f && !scale_in && pg.fixed_iter <= 0) {   // scaled start
     LAUNCH(ctx, launch_alpha_schedule(b, b->d_scale, ctx->cfg.gap_hint, b->d_alpha, st));
@@ -1160,7 +1162,8 @@ static XRef x_ref(const nolsm_batch *b) {
     if (b->prepared_precision == NOLSM_FP16_FP32)   // (buffer by the parity of d_iters, which may count from iteration 1)
       return (b->sign_iter0 & 1) ? XRef{nullptr, b->h[1], b->h[0], b->h[2], b->h[2]}
                                  : XRef{nullptr, b->h[0], b->h[1], b->h[2], b->h[2]};
-    return XRef{nullptr, b->h[0], b->h[2], b->h[1], b->h[3]};
+    return (b->sign_iter0 & 1) ? XRef{nullptr, b->h[2], b->h[0], b->h[3], b->h[1]}
+                               : XRef{nullptr, b->h[0], b->h[2], b->h[1], b->h[3]};
   }
   return XRef{x_ptr(b), nullptr, nullptr, nullptr, nullptr};
 }

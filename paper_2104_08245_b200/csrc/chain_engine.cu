@@ -596,9 +596,10 @@ __global__ void __launch_bounds__(kThreads, 1) k_chain(const ChainArgs args) {
 // The instantiations that exist: the sign iteration / plain one-shot products (0), all-split programs of the FP32 mode,
 // the Eq. 15-17 chain with its column norms, the half-split residual R, the shifted B1 -> X0 product, and everything.
 typedef void (*ChainKernel)(const ChainArgs);
-constexpr int kNumInst = 7;
+constexpr int kNumInst = 8;
 const int kInstFeat[kNumInst] = {0, chainep::kFeatSplitAll, chainep::kFeatColNorm, chainep::kFeatSplitAny,
-                                 chainep::kFeatShift, chainep::kFeatRescale, chainep::kFeatFull};
+                                 chainep::kFeatShift, chainep::kFeatRescale,
+                                 chainep::kFeatSplitAll | chainep::kFeatRescale, chainep::kFeatFull};
 template <bool kPair>
 static ChainKernel chain_kernel_of(int feat) {
   switch (feat) {
@@ -608,6 +609,8 @@ static ChainKernel chain_kernel_of(int feat) {
     case chainep::kFeatSplitAny: return k_chain<kPair, chainep::kFeatSplitAny>;
     case chainep::kFeatShift: return k_chain<kPair, chainep::kFeatShift>;
     case chainep::kFeatRescale: return k_chain<kPair, chainep::kFeatRescale>;
+    case chainep::kFeatSplitAll | chainep::kFeatRescale:
+      return k_chain<kPair, chainep::kFeatSplitAll | chainep::kFeatRescale>;
     default: return k_chain<kPair, chainep::kFeatFull>;
   }
 }
