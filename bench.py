@@ -361,7 +361,8 @@ def main():
     ap.add_argument("--workspace-gib", type=float, default=24.0)
     ap.add_argument("--group", type=int, default=0, help="window: submatrices in flight together (0: from the L2 size)")
     ap.add_argument("--flags", type=int, default=0, help="NOLSM_FLAG_* bits (2: pair engine, 8: single-CTA engine, 16: unit scaling, 32: third-order iteration, "
-                         "64: no a-priori stop of Eq. 15-17, 128: symmetric Loewdin form, FP32 workloads only)")
+                         "64: no a-priori stop of Eq. 15-17, 128: symmetric Loewdin form, FP32 workloads only, "
+                         "256: no rescaled first sign iteration)")
     ap.add_argument("--elements", default="gathered", choices=["gathered", "generated", "generated-fp32"],
                     help="submatrix elements gathered from the block stores (the north_star path) or evaluated "
                          "on the device from the positions (nolsm_set_model; -fp32: FP32 + SFU as in PAPER.md:202)")
