@@ -121,7 +121,7 @@ typedef struct {
 #define NOLSM_FLAG_NO_RESCALE 256 /* do not rescale the first sign iteration.  By default the first product of
                                   the iteration (X0^2) also yields ||X0^2||_1 >= rho(X0)^2, a tighter bound on the
                                   spectrum than the O(n^2) norm bound X0 was scaled with, and iteration 0 is applied to
-                                  a X0, a = 1.6 / sqrt(||X0^2||_1) >= 1 ("rescaled so that its spectrum
+                                  a X0, a = 1.7 / sqrt(||X0^2||_1) >= 1 ("rescaled so that its spectrum
                                   lies in the convergence region"; reading 5): one iteration fewer on the
                                   water systems, same sign function */
 #define NOLSM_FLAG_UNIT_SCALE 16 /* scale by the norm bound itself: Y0 = S/bound, X0 = A/bound (spectra in (0,1] and

@@ -200,14 +200,17 @@ def newton_schulz_sign(a, n_iter, scale=None, history=False):
     return (x, np.array(res)) if history else x
 
 
+RESCALE_TARGET = 1.7       # < sqrt(3): |eigenvalue| the bound on rho(X0) is mapped to
+
+
 def rescaled_first_step_factor(x0):
     """DESIGN.md reading 5, rescaled first iteration: rho(X0)^2 = rho(X0^2) <= ||X0^2||_1 (a spectral radius is bounded by
-    any induced norm), so a X0 with a = 1.6 / sqrt(||X0^2||_1) has its spectrum inside [-1.6, 1.6], inside the interval
-    (-sqrt 3, sqrt 3) on which Eq. 9 converges to the sign.  Clamped to [1, 1.6]: never scale down (X0 already lies in
-    [-1.5, 1.5]), and not up by more than 1.6 (the update below multiplies the rounding of E_0 by a^3)."""
+    any induced norm), so a X0 with a = 1.7 / sqrt(||X0^2||_1) has its spectrum inside [-1.7, 1.7], inside the interval
+    (-sqrt 3, sqrt 3) on which Eq. 9 converges to the sign.  Clamped to [1, 1.7]: never scale down (X0 already lies in
+    [-1.5, 1.5]), and not up by more than the target (the update below multiplies the rounding of E_0 by a^3)."""
     b2 = min(float(np.abs(x0 @ x0).sum(0).max()), 2.25)
-    a = 1.6 / np.sqrt(b2) if b2 > 0.0 else 1.0
-    return float(min(max(a, 1.0), 1.6))
+    a = RESCALE_TARGET / np.sqrt(b2) if b2 > 0.0 else 1.0
+    return float(min(max(a, 1.0), RESCALE_TARGET))
 
 
 def newton_schulz_sign_rescaled(a, n_iter, scale=None, history=False):

@@ -930,7 +930,7 @@ static nolsm_status sign_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, double mu, 
     set2(x.a, 0, 1); set2(x.b, 4, 4); set2(x.cin16, 0, 1); set2(x.cin16_lo, 2, 2);
     set2(x.out16, 1, 0); set2(x.out16_lo, 2, 2); x.lo_stream = 1;
     // rescaled first iteration (reading 5): ||X0^2||_1 from E_0's epilogue bounds rho(X0) tighter than the O(n^2)
-    // norm bound X0 was scaled with; iteration 0 is applied to a X0 with a = 1.6 / sqrt(||X0^2||_1) >= 1
+    // norm bound X0 was scaled with; iteration 0 is applied to a X0 with a = 1.7 / sqrt(||X0^2||_1) >= 1
     rescale = !order3 && !scale_in && ctx->cfg.gap_hint <= 0.f && pg.fixed_iter <= 0 && max_iter > 1 &&
               (ctx->cfg.flags & NOLSM_FLAG_NO_RESCALE) == 0;
     if (order3) {
@@ -972,6 +972,7 @@ static nolsm_status sign_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, double mu, 
     p0.ops[0] = e;
     p0.ops[1] = x;
     p0.ops[0].colnorm = p0.ops[1].colnorm = 2;
+    p0.rescale_target = 1.7f;   // < sqrt 3 = 1.732; measured: 1.6 leaves half of the n ~ 1489 submatrices one iteration short
     CHECK(run_chain(ctx, b, p0, nullptr, false, st));
     // the adaptive launch starts at iteration 1: its tables are indexed by the parity of ITS iteration count
     auto flip = [](int32_t (&d)[2]) { std::swap(d[0], d[1]); };

@@ -82,6 +82,7 @@ struct ChainProgram {
   int32_t use_alpha_tab;          // 1: per-submatrix, per-iteration scaling alpha_k from nolsm_batch::d_alpha
   int32_t stop_early;             // 1: the iteration whose residual passes the test is NOT finished (its
                                   // remaining products are skipped); 0: it is (reading 9, "+1 rule")
+  float rescale_target;           // ops with colnorm == 2: |eigenvalue| the bound on rho(X0) is mapped to (and cap of the factor)
   int32_t skip_tail;              // ops at the end of an iteration that the LAST iteration of a chain without stop_early
                                   // does not need (Eq. 15-17 with ops E, Z, Y: 1 -- nothing reads the final Y)
   float tol_pred;                 // > 0 (with stop_early, Eq. 15-17 only, ops ordered E, Z, Y): a-priori stop.  With

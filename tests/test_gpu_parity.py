@@ -449,7 +449,7 @@ def test_lowdin_form(nolsm, tiny_system, tiny_solution, mid_system, mid_solution
 
 def test_rescaled_first_sign_iteration(nolsm, mid_system, mid_solution):
     """DESIGN.md reading 5: the first product of the sign iteration (X0^2) also gives ||X0^2||_1 >= rho(X0)^2, and
-    iteration 0 is applied to a X0, a = 1.6 / sqrt(||X0^2||_1) in [1, 1.6] (oracle: newton_schulz_sign_rescaled, pinned in
+    iteration 0 is applied to a X0, a = 1.7 / sqrt(||X0^2||_1) in [1, 1.7] (oracle: newton_schulz_sign_rescaled, pinned in
     test_oracle_pins.py).  Same D and N as the oracle with and without it (NOLSM_FLAG_NO_RESCALE), never more iterations,
     and the result is bitwise reproducible although the norm is gathered with atomics (integer sums)."""
     import oracle.nolsm_oracle as orc

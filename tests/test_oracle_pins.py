@@ -333,7 +333,7 @@ def test_lowdin_form_gives_the_same_density(tiny_solution, mid_system_cpu):
 
 
 def test_rescaled_first_sign_iteration(tiny_solution, mid_system_cpu):
-    """Reading 5, rescaled first iteration: (1) the factor keeps the spectrum of a X0 inside [-1.6, 1.6]; (2) the update
+    """Reading 5, rescaled first iteration: (1) the factor keeps the spectrum of a X0 inside [-1.7, 1.7] (1.7 < sqrt 3); (2) the update
     a (3/2 - 1/2 a^2) X0 + 1/2 a^3 X0 E_0 IS Eq. 9 applied to a X0; (3) the iteration converges to the same sign
     function (the eigenvector construction); (4) it never needs more iterations than the plain one, and on a
     water-like submatrix scaled by the O(n^2) norm bound it needs one fewer."""
@@ -349,7 +349,8 @@ def test_rescaled_first_sign_iteration(tiny_solution, mid_system_cpu):
         x0 = a / scale
         al = orc.rescaled_first_step_factor(x0)
         rho = np.abs(np.linalg.eigvals(x0)).max()
-        assert 1.0 <= al <= 1.6 and al * rho <= 1.6 * (1 + 1e-12) and rho ** 2 <= np.abs(x0 @ x0).sum(0).max() * (1 + 1e-12)
+        assert orc.RESCALE_TARGET < np.sqrt(3.0)
+        assert 1.0 <= al <= 1.7 and al * rho <= 1.7 * (1 + 1e-12) and rho ** 2 <= np.abs(x0 @ x0).sum(0).max() * (1 + 1e-12)
         e0 = eye - x0 @ x0
         x1 = al * (1.5 - 0.5 * al * al) * x0 + 0.5 * al ** 3 * (x0 @ e0)
         assert np.abs(x1 - 0.5 * (al * x0) @ (3 * eye - (al * x0) @ (al * x0))).max() < 1e-13
