@@ -905,7 +905,7 @@ static nolsm_status sign_batch_chain(nolsm_ctx *ctx, nolsm_batch *b, double mu, 
   pg.fixed_iter = fixed_iter > 0 ? fixed_iter : 0;
   pg.tol = tol;
   // fold_last: stop right after the E_k that passes the test; the caller applies X_{k+1} = X_k + 1/2 X_k E_k
-  // only to the own columns of S^-1 (k_last_half), instead of forming it with an n^3 product
+  // only to the own columns of S^-1 (k_thin_mma<kLastHalf>), instead of forming it with an n^3 product
   const bool order3 = fp16 && (ctx->cfg.flags & NOLSM_FLAG_ORDER3) != 0;
   bool rescale = false;
   b->sign_iter0 = 0;

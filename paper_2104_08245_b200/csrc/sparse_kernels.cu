@@ -610,7 +610,7 @@ k_density(const int32_t *__restrict__ row_ptr, const int32_t *__restrict__ col_i
           const float *__restrict__ u_thin, const __half *__restrict__ e_hi, const __half *__restrict__ e_lo,
           float *__restrict__ d_val, double *__restrict__ ne_diag) {
   // [n][6], row k contiguous: the six own columns V of S^-1, or (u_thin set: last iteration folded in,
-  // see k_last_half) U = V + 1/2 E V, so that X U = X_{k+1} V; then the slice sums
+  // thin_kernels.cu kLastHalf) U = V + 1/2 E V, so that X U = X_{k+1} V; then the slice sums
   extern __shared__ __align__(16) float s_sinv[];
   const int mat = blockIdx.y;
   const int j = mol_begin + mat;
