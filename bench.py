@@ -34,7 +34,7 @@ WORKLOADS = {          # name -> (precision, description)
 DATASHEET_FP16_TFLOPS = 2250.0
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE sign-iteration launch of k_chain: an ncu CONSTANT from the
 # `ncu --set full` capture named here (bench.py cannot read DRAM counters itself); None where no capture exists
-NCU_TRAFFIC = {"w32768": 62.7e9}   # dram read 35.39 + write 27.33 GB, end-of-round capture
+NCU_TRAFFIC = {"w32768": 55.2e9}   # per batch: iteration 0 (4.35 + 3.24 GB) + the other iterations (26.83 + 20.76 GB), end-of-round capture
 NCU_TRAFFIC_SOURCE = "profiles/r2_k_chain_sign_w32768.md"
 METRIC = "molecules/s per NOLSM step (sign-iteration TFLOP/s in roofline.achieved)"
 
@@ -316,7 +316,7 @@ def run_native(args, system, rank, world, local_rank):
                          (system.nnzb * 144 / 1e6, args.workspace_gib)},
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
         "roofline": {"bound": "tensor",
-                     "kernel": "k_chain, sign-iteration launches (all iterations of Eq. 9-10 for one batch per launch)",
+                     "kernel": "k_chain, sign iteration of one batch (Eq. 9-10: iteration 0 with the rescale in one launch, all others in a second one; per launch = per batch)",
                      "achieved": sign_tflops, "peak": peaks["tflops_sustained"], "unit": "TFLOP/s",
                      "frac": sign_tflops / peaks["tflops_sustained"], "traffic": NCU_TRAFFIC.get(args.workload),
                      "traffic_source": "ncu constant, " + NCU_TRAFFIC_SOURCE,
